@@ -1,0 +1,442 @@
+"""Pins for the fp64 oracle: closed forms, the value the paper prints for eq. (23), invariants and
+brute force through independent scipy routines.  CPU only."""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate, optimize, special
+
+import oracle as O
+from workloads import lambda_vector, make_workload
+
+C = 299792.458
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def lam(**kw):
+    return lambda_vector(**kw)
+
+
+# ------------------------------------------------------------------ P1: GR limits of eq. (2)
+@pytest.mark.parametrize("kw", [dict(Xi0=1.0, n=0.7), dict(Xi0=1.0, n=4.2), dict(Xi0=0.4, n=0.0),
+                                dict(Xi0=3.0, n=0.0)])
+def test_p1_xi0_one_or_n_zero_is_gr(kw):
+    z = np.linspace(0.0, 6.0, 41)
+    d = O.distances(lam(**kw), z)
+    assert np.allclose(d["dl_gw"], d["dl_em"], rtol=1e-15, atol=0)
+
+
+def test_p1_xi_limits():
+    # Xi(0) = 1 and Xi(z->inf) = Xi0  (eq. 2): d_L^gw/d_L^em at small and huge z
+    la = lam(Xi0=1.8, n=2.5)
+    d = O.distances(la, np.array([1e-9, 9.9]))
+    r = d["dl_gw"] / d["dl_em"]
+    assert abs(r[0] - 1.0) < 1e-8
+    assert abs(r[1] - (1.8 + (1 - 1.8) / 10.9 ** 2.5)) < 1e-14
+
+
+# ------------------------------------------------------------------ P2: closed-form cosmologies
+def test_p2_einstein_de_sitter():
+    z = np.array([0.01, 0.3, 1.0, 2.5, 8.0])
+    d = O.distances(lam(Om=1.0, H0=67.0), z)
+    ref = (1 + z) * (2 * C / 67.0) * (1 - 1 / np.sqrt(1 + z))
+    assert np.allclose(d["dl_em"], ref, rtol=1e-13)
+
+
+def test_p2_empty_limit_and_inverse():
+    la = lam(Om=1e-15, H0=70.0, Xi0=1.0)
+    z = np.array([0.05, 0.7, 3.0])
+    d = O.distances(la, z)
+    assert np.allclose(d["dc"], C * z / 70.0, rtol=1e-12)
+    dl = np.array([300.0, 5000.0, 40000.0])
+    zi = O.z_of_dl(la, dl, z_table_max=20.0)
+    ref = 0.5 * (-1 + np.sqrt(1 + 4 * dl * 70.0 / C))
+    assert np.allclose(zi, ref, rtol=1e-11)
+
+
+def test_p2_eq23_value_printed_by_paper():
+    row = [l for l in open(os.path.join(GOLD, "eq23_rate.txt")) if not l.startswith("#")][0].split()
+    R0, zmax, H0, Om, g, k, zp, printed = map(float, row)
+    la = lam(H0=H0, Om=Om, gamma=g, kappa=k, z_p=zp)
+
+    def integrand(z):
+        dv, _ = O.volume(la, [z])
+        return O.psi(la, [z])[0] / (1 + z) * dv[0] / 1e9          # Mpc^3 -> Gpc^3
+    val, _ = integrate.quad(integrand, 0.0, zmax, epsabs=0, epsrel=1e-10)
+    rate = R0 * val
+    assert float(f"{rate:.1e}") == printed, rate                  # rounds to 1.4e4
+    assert abs(rate - 1.366e4) < 0.01e4                           # SURVEY probe value (full sky)
+
+
+def test_p2_volume_consistency():
+    # dVc/dz is the derivative of Vc, and Vc = 4pi/3 dC^3
+    la = lam()
+    z = np.array([0.2, 0.9, 1.5])
+    dv, vc = O.volume(la, z)
+    e = 1e-5
+    _, vp = O.volume(la, z + e)
+    _, vm = O.volume(la, z - e)
+    assert np.allclose(dv, (vp - vm) / (2 * e), rtol=1e-8)
+    assert np.allclose(vc, 4 * np.pi / 3 * O.distances(la, z)["dc"] ** 3, rtol=1e-14)
+
+
+# ------------------------------------------------------------------ P3: derivative, round trip
+@pytest.mark.parametrize("kw", [dict(), dict(Xi0=0.5, n=3.0, H0=80, Om=0.4), dict(Xi0=2.0, n=0.5, H0=60, Om=0.2)])
+def test_p3_derivative_and_round_trip(kw):
+    la = lam(**kw)
+    z = np.array([0.02, 0.4, 1.3, 4.0])
+    e = 1e-5
+    f = lambda x: O.distances(la, x)["dl_gw"]
+    fd = (f(z + e) - f(z - e)) / (2 * e)
+    assert np.allclose(O.distances(la, z)["ddl_gw_dz"], fd, rtol=1e-8)
+    assert np.allclose(O.z_of_dl(la, f(z)), z, rtol=0, atol=2e-13)
+    assert O.dl_monotone(la)
+
+
+def test_p3_dc_against_adaptive_quadrature():
+    la = lam(H0=73.0, Om=0.31)
+    for z in (0.1, 1.0, 3.3, 9.0):
+        ref, _ = integrate.quad(lambda x: C / 73.0 / math.sqrt(0.31 * (1 + x) ** 3 + 0.69), 0, z, epsabs=0, epsrel=1e-13)
+        assert abs(O.distances(la, [z])["dc"][0] / ref - 1) < 1e-12
+
+
+def test_table_range_rule():
+    la = lam()
+    dmax = O.distances(la, [2.0])["dl_gw"][0]
+    z = O.z_of_dl(la, [dmax * 0.999, dmax * 1.001], z_table_max=2.0)
+    assert np.isfinite(z[0]) and np.isnan(z[1])
+
+
+def test_nonmonotone_detected():
+    # Xi0 << 1 with large n makes d_L^gw(z) turn over (R16)
+    assert not O.dl_monotone(lam(Xi0=0.01, n=8.0))
+
+
+# ------------------------------------------------------------------ P4: one-sample KDE
+def test_p4_single_sample_is_gaussian():
+    zg = np.linspace(0.1, 0.5, 57)
+    K = O.kde([0.31], [2.5], 0.02, zg)
+    ref = 2.5 * np.exp(-0.5 * ((zg - 0.31) / 0.02) ** 2) / (0.02 * math.sqrt(2 * math.pi))
+    assert np.allclose(K, ref, rtol=1e-14)
+
+
+def test_kde_normalisation_is_by_Ns_not_sum_w():
+    # R2: int K dz = mean weight
+    rng = np.random.default_rng(1)
+    z, w = 0.3 + 0.02 * rng.standard_normal(50), rng.random(50) * 3
+    zg = np.linspace(0.0, 0.6, 6001)
+    K = O.kde(z, w, 0.004, zg)
+    assert abs(np.trapezoid(K, zg) - w.mean()) < 1e-10 * w.mean()
+
+
+# ------------------------------------------------------------------ P5: closed form of the event integral
+def test_p5_event_integral_closed_form():
+    rng = np.random.default_rng(2)
+    ns, ngal = 40, 7
+    z = 0.4 + 0.03 * rng.standard_normal(ns)
+    w = rng.random(ns) + 0.1
+    h = 0.006
+    zgal = 0.4 + 0.04 * rng.standard_normal(ngal)
+    sg = 0.0015 * (1 + zgal)
+    zg = np.linspace(0.1, 0.7, 1201)                              # dz = 5e-4 <~ sigma_g
+    pgal = np.mean(np.exp(-0.5 * ((zg[:, None] - zgal) / sg) ** 2) / (sg * math.sqrt(2 * math.pi)), axis=1)
+    K = O.kde(z, w, h, zg)
+    I = O.event_integral(lam(), zg, K, pgal)
+    s2 = h * h + sg ** 2
+    ref = np.mean(w[:, None] * np.mean(np.exp(-0.5 * (z[:, None] - zgal) ** 2 / s2) / np.sqrt(2 * math.pi * s2), axis=1, keepdims=True))
+    ref = np.mean(w * np.mean(np.exp(-0.5 * (z[:, None] - zgal[None, :]) ** 2 / s2) / np.sqrt(2 * math.pi * s2), axis=1))
+    assert abs(I / ref - 1) < 1e-10
+
+
+def test_p5_flat_pgal_gives_mean_weight():
+    rng = np.random.default_rng(3)
+    z, w = 0.5 + 0.01 * rng.standard_normal(30), rng.random(30)
+    zg = np.linspace(0.3, 0.7, 2001)
+    K = O.kde(z, w, 0.003, zg)
+    assert abs(O.event_integral(lam(), zg, K, np.ones_like(zg)) / w.mean() - 1) < 1e-11
+
+
+def test_trapezoid_on_nonuniform_grid():
+    zg = np.array([0.0, 0.1, 0.25, 0.27, 0.6])
+    K = np.array([1.0, 2.0, 0.5, 4.0, 1.0])
+    p = np.array([2.0, 1.0, 3.0, 0.5, 1.0])
+    y = K * p
+    ref = sum(0.5 * (y[i] + y[i + 1]) * (zg[i + 1] - zg[i]) for i in range(4))
+    assert abs(O.event_integral(lam(), zg, K, p) - ref) < 1e-15
+
+
+# ------------------------------------------------------------------ P6: mass function
+MASS_LAMS = [dict(), dict(alpha=1.0), dict(beta=-1.0), dict(alpha=2.2, beta=0.0, delta_m=9.0, m_low=3.0, m_high=60.0, mu_g=30.0, sigma_g=1.0, lambda_g=0.3),
+             dict(delta_m=0.05), dict(m_high=8.0, delta_m=6.0, lambda_g=0.5)]
+
+
+@pytest.mark.parametrize("kw", MASS_LAMS)
+def test_p6_primary_integrates_to_one(kw):
+    la = lam(**kw)
+    p = dict(zip(("m_low", "delta_m", "m_high", "mu_g", "sigma_g"), (la[7], la[6], la[8], la[9], la[10])))
+    pts = sorted({p["m_low"], p["m_low"] + p["delta_m"], p["m_high"], p["mu_g"]})
+    top = max(p["m_high"], p["mu_g"] + 30 * p["sigma_g"]) + 1
+    tot = 0.0
+    edges = [e for e in pts if e < top] + [top]
+    for a, b in zip(edges[:-1], edges[1:]):
+        v, _ = integrate.quad(lambda m: O.p_m1(la, [m])[0], a, b, epsabs=0, epsrel=1e-11, limit=400)
+        tot += v
+    assert abs(tot - 1) < 1e-9
+
+
+@pytest.mark.parametrize("kw", MASS_LAMS)
+@pytest.mark.parametrize("frac", [0.3, 0.95, 1.0, 4.0])
+def test_p6_secondary_integrates_to_one(kw, frac):
+    la = lam(**kw)
+    m_low, dm = la[7], la[6]
+    m1 = m_low + frac * dm
+    pts = [m_low] + ([m_low + dm] if m1 > m_low + dm else []) + [m1]
+    tot = sum(integrate.quad(lambda m: O.p_m2_given_m1(la, [m1], [m])[0], a, b, epsabs=0, epsrel=1e-11, limit=400)[0]
+              for a, b in zip(pts[:-1], pts[1:]))
+    assert abs(tot - 1) < 1e-9
+
+
+def test_p6_sharp_limit_is_truncated_power_laws():
+    # delta_m -> 0, lambda_g = 0: p(m1) = PL on [m_low, m_high], p(m2|m1) = (b+1) m2^b/(m1^(b+1) - m_low^(b+1))
+    a, b, ml, mh = 2.3, 1.4, 5.0, 80.0
+    la = lam(alpha=a, beta=b, m_low=ml, m_high=mh, delta_m=1e-9, lambda_g=0.0)
+    m1 = np.array([6.0, 20.0, 79.0])
+    m2 = np.array([5.5, 11.0, 40.0])
+    p1 = (1 - a) * m1 ** (-a) / (mh ** (1 - a) - ml ** (1 - a))
+    p2 = (b + 1) * m2 ** b / (m1 ** (b + 1) - ml ** (b + 1))
+    assert np.allclose(O.p_m1(la, m1), p1, rtol=1e-8)
+    assert np.allclose(O.p_m2_given_m1(la, m1, m2), p2, rtol=1e-8)
+    assert np.allclose(O.mass_pdf(la, m1, m2), p1 * p2, rtol=1e-8)
+
+
+def test_p6_support_and_smoothing_shape():
+    la = lam()
+    ml, dm, mh = la[7], la[6], la[8]
+    m = np.linspace(ml - 1, ml + dm + 1, 400)
+    S = O.smoothing(la, m)
+    assert np.all(np.diff(S) >= 0) and S[0] == 0 and S[-1] == 1
+    assert O.smoothing(la, [ml])[0] == 0 and O.smoothing(la, [ml + dm])[0] == 1
+    assert abs(O.smoothing(la, [ml + dm / 2])[0] - 0.5) < 1e-15          # f(dm/2) = 2 - 2 = 0
+    # R15 support: m2 < m_low, m2 > m1 -> 0 ; power law is 0 above m_high but the Gaussian is not
+    assert O.mass_pdf(la, [30.0], [ml - 0.1])[0] == 0
+    assert O.mass_pdf(la, [30.0], [30.1])[0] == 0
+    g_only = la[11] * math.exp(-0.5 * ((mh + 1 - la[9]) / la[10]) ** 2) / (la[10] * math.sqrt(2 * math.pi))
+    z1 = O.p_m1(la, [40.0])[0] / ((1 - la[11]) * (1 - la[4]) * 40.0 ** -la[4] / (mh ** (1 - la[4]) - ml ** (1 - la[4]))
+                                  + la[11] * math.exp(-0.5 * ((40 - la[9]) / la[10]) ** 2) / (la[10] * math.sqrt(2 * math.pi)))
+    assert abs(O.p_m1(la, [mh + 1])[0] / (g_only * z1) - 1) < 1e-12
+
+
+def test_p6_gaussian_component_weight():
+    # with S ~ 1 (tiny delta_m) and mu_g well inside, the Gaussian carries exactly lambda_g
+    la = lam(delta_m=1e-9, lambda_g=0.25, mu_g=40.0, sigma_g=2.0)
+    v, _ = integrate.quad(lambda m: O.p_m1(la, [m])[0], 30.0, 50.0, points=[40.0], epsabs=0, epsrel=1e-12)
+    a, ml, mh = la[4], la[7], la[8]
+    pl = 0.75 * (50.0 ** (1 - a) - 30.0 ** (1 - a)) / (mh ** (1 - a) - ml ** (1 - a))
+    assert abs(v - (pl + 0.25 * special.erf(10 / 2 / math.sqrt(2)))) < 1e-10
+
+
+# ------------------------------------------------------------------ P7: rate
+def test_p7_madau_dickinson():
+    la = lam(gamma=2.7, kappa=3.0, z_p=2.0)
+    assert abs(O.psi(la, [2.0])[0] - 3.0 ** 2.7 / 2) < 1e-13
+    assert abs(O.psi(la, [0.0])[0] - 1 / (1 + 3.0 ** -5.7)) < 1e-15
+    lb = lam(gamma=1.9, kappa=2.0, z_p=1e6)
+    z = np.array([0.1, 1.0, 3.0])
+    assert np.allclose(O.psi(lb, z), (1 + z) ** 1.9, rtol=1e-12)
+    # high-z slope is -kappa
+    zz = np.array([2000.0, 4000.0])
+    p = O.psi(la, zz)
+    assert abs(math.log(p[1] / p[0]) / math.log((1 + zz[1]) / (1 + zz[0])) + 3.0) < 1e-6
+
+
+# ------------------------------------------------------------------ P8: self-consistent injections
+def test_p8_unit_weights_give_detected_count():
+    w = make_workload("tiny")
+    la = w.lam[0]
+    n = 500
+    dl, m1, m2 = w.inj_dL[:n], w.inj_m1d[:n], w.inj_m2d[:n]
+    # p_pop^d(theta_j | lambda*) from the oracle's own pieces -> p_draw := p_pop => s_j = 1
+    _, _, s = O.selection_sums(la, dl, m1, m2, np.zeros(n), return_s=True)
+    keep = s > 0
+    assert keep.sum() > 100
+    s1, s2 = O.selection_sums(la, dl[keep], m1[keep], m2[keep], np.log(s[keep]))
+    nd, ninj = keep.sum(), 10 * keep.sum()
+    assert abs(s1 - nd) < 1e-9 * nd and abs(s2 - nd) < 1e-9 * nd
+    assert abs(O.neff(s1, s2, ninj) - nd / (1 - nd / ninj)) < 1e-6
+
+
+# ------------------------------------------------------------------ P9: xi by quadrature (statistical)
+def test_p9_selection_fraction_matches_quadrature():
+    la = lam(Xi0=1.3, n=1.5)
+    D, zcat = 6000.0, 1.5
+    rng = np.random.default_rng(9)
+    N = 120_000
+    # draw pdf covering the whole support: p(dL) ~ dL^2 on [0, D], m1d ~ 1/m on [4, 400], m2d uniform [4, m1d]
+    dl = D * rng.random(N) ** (1.0 / 3.0)
+    m1 = 4.0 * (100.0) ** rng.random(N)
+    m2 = 4.0 + (m1 - 4.0) * rng.random(N)
+    lnp = np.log(3 * dl ** 2 / D ** 3) - np.log(m1 * math.log(100.0)) - np.log(m1 - 4.0)
+    s1, s2 = O.selection_sums(la, dl, m1, m2, lnp, z_cat_max=zcat)
+    xi_mc = s1 / N
+    ne = O.neff(s1, s2, N)
+    zD = min(O.z_of_dl(la, [D])[0], zcat)
+    _, vmax = O.volume(la, [zcat])
+
+    def f(z):
+        dv, _ = O.volume(la, [z])
+        return O.psi(la, [z])[0] * dv[0] / vmax[0] / (1 + z)
+    xi_q, _ = integrate.quad(f, 0, zD, epsabs=0, epsrel=1e-10)
+    assert ne > 2000
+    assert abs(xi_mc - xi_q) < 4 * xi_q / math.sqrt(ne), (xi_mc, xi_q, ne)
+    assert 4 / math.sqrt(ne) < 0.05                                 # the check resolves 5% (a dropped (1+z) is >20%)
+
+
+# ------------------------------------------------------------------ P10: invariances
+def _one_event(w, i):
+    s = slice(w.sample_off[i], w.sample_off[i + 1])
+    g = slice(w.grid_off[i], w.grid_off[i + 1])
+    return w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s], w.z_grid[g], w.p_gal[g]
+
+
+def test_p10_weight_scaling_and_h0_rescaling():
+    w = make_workload("tiny", n_samples=300)
+    la = w.lam[0]
+    dl, m1, m2, lp, zg, pg = _one_event(w, 0)
+    a, h, _ = O.event_logI(la, dl, m1, m2, lp, zg, pg)
+    b, h2, _ = O.event_logI(la, dl, m1, m2, lp - math.log(7.0), zg, pg)
+    assert abs(b - a - math.log(7.0)) < 1e-12 and abs(h2 / h - 1) < 1e-13
+    # (H0, dL) -> (a H0, dL/a): same z_j
+    lb = la.copy()
+    lb[0] *= 1.3
+    z1, _, _ = O.sample_weights(la, dl, m1, m2, lp)
+    z2, _, _ = O.sample_weights(lb, dl / 1.3, m1, m2, lp)
+    assert np.allclose(z1, z2, rtol=0, atol=1e-12)
+
+
+def test_p10_placements_converge_for_small_h():
+    w = make_workload("tiny", n_samples=300)
+    la = w.lam[0]
+    dl, m1, m2, lp, zg, _ = _one_event(w, 1)
+    zf = np.linspace(zg[0], zg[-1], 4001)
+    pg = np.exp(-0.5 * ((zf - zf.mean()) / 0.05) ** 2)                 # smooth p_gal
+    diffs = []
+    for h in (4e-3, 1e-3):
+        a, _, _ = O.event_logI(la, dl, m1, m2, lp, zf, pg, placement=O.PLACE_SAMPLES, bw_rule=O.BW_FIXED, fixed_bw=h)
+        b, _, _ = O.event_logI(la, dl, m1, m2, lp, zf, pg, placement=O.PLACE_GRID, bw_rule=O.BW_FIXED, fixed_bw=h)
+        diffs.append(abs(a - b))
+    assert diffs[1] < diffs[0] / 8 and diffs[1] < 1e-4                  # O(h^2) convergence
+
+
+def test_scott_bandwidth_reduces_to_textbook_for_equal_weights():
+    rng = np.random.default_rng(5)
+    z = rng.standard_normal(200) * 0.1 + 1.0
+    h = O.scott_bw(z, np.full(200, 3.3))
+    assert abs(h - np.std(z, ddof=1) * 200 ** -0.2) < 1e-14
+    # duplicating a point == doubling its weight (Kish n_eff / reliability weights are not frequency
+    # weights, so only check scale invariance and finiteness here)
+    assert abs(O.scott_bw(z, np.full(200, 1e-20)) - h) < 1e-14
+    assert math.isnan(O.scott_bw([0.3], [1.0])) and math.isnan(O.scott_bw(z, np.zeros(200)))
+
+
+# ------------------------------------------------------------------ P11: brute force, independent route
+def _brute_loglike(la, events, inj, n_inj_total, z_cat_max, fixed_h=None):
+    """Independent re-computation with scipy (quad / brentq) on tiny inputs; placement N."""
+    H0, Om, Xi0, n, al, be, dm, ml, mh, mu, sg, lg, ga, ka, zp = la
+    E = lambda z: math.sqrt(Om * (1 + z) ** 3 + 1 - Om)
+    dC = lambda z: integrate.quad(lambda x: C / H0 / E(x), 0, z, epsabs=0, epsrel=1e-13)[0]
+    Xi = lambda z: Xi0 + (1 - Xi0) * (1 + z) ** (-n)
+    dL = lambda z: Xi(z) * (1 + z) * dC(z)
+    ddL = lambda z: (dL(z + 1e-5) - dL(z - 1e-5)) / 2e-5              # numerical derivative on purpose
+    S = lambda m: 0.0 if m <= ml else (1.0 if m >= ml + dm else 1 / (1 + math.exp(min(700.0, dm / (m - ml) + dm / (m - ml - dm)))))
+    PL = lambda m: (1 - al) * m ** (-al) / (mh ** (1 - al) - ml ** (1 - al)) if ml <= m <= mh else 0.0
+    G = lambda m: math.exp(-0.5 * ((m - mu) / sg) ** 2) / (sg * math.sqrt(2 * math.pi))
+    p1u = lambda m: ((1 - lg) * PL(m) + lg * G(m)) * S(m)
+    Z1 = sum(integrate.quad(p1u, a, b, epsabs=0, epsrel=1e-12, limit=500)[0] for a, b in ((ml, ml + dm), (ml + dm, mu), (mu, mh), (mh, mh + 300)))
+    Cn = lambda m1: sum(integrate.quad(lambda m: m ** be * S(m), a, b, epsabs=0, epsrel=1e-12, limit=500)[0]
+                        for a, b in ((ml, min(m1, ml + dm)), (min(m1, ml + dm), m1)) if b > a)
+    psi = lambda z: (1 + z) ** ga / (1 + ((1 + z) / (1 + zp)) ** (ga + ka))
+    pm = lambda m1, m2: p1u(m1) / Z1 * m2 ** be * S(m2) / Cn(m1) if (ml <= m2 <= m1) else 0.0
+
+    def weight(dl, m1d, m2d):
+        z = optimize.brentq(lambda x: dL(x) - dl, 0, 10, xtol=1e-14, rtol=1e-15)
+        return z, pm(m1d / (1 + z), m2d / (1 + z)) * psi(z) / ((1 + z) ** 3 * abs(ddL(z)))
+    total = 0.0
+    logI = []
+    for (dls, m1s, m2s, lps, zg, pg) in events:
+        zw = [weight(*t) for t in zip(dls, m1s, m2s)]
+        z = np.array([t[0] for t in zw])
+        w = np.array([t[1] for t in zw]) / np.exp(lps)
+        if fixed_h is None:
+            wh = w / w.sum()
+            neff = 1 / np.sum(wh ** 2)
+            zb = np.sum(wh * z)
+            h = math.sqrt(np.sum(wh * (z - zb) ** 2) / (1 - np.sum(wh ** 2))) * neff ** -0.2
+        else:
+            h = fixed_h
+        K = np.array([np.sum(w * np.exp(-0.5 * ((x - z) / h) ** 2)) for x in zg]) / (len(z) * h * math.sqrt(2 * math.pi))
+        I = np.trapezoid(K * pg, zg)
+        logI.append(math.log(I))
+    total = sum(logI)
+    Vmax = 4 * math.pi / 3 * dC(z_cat_max) ** 3
+    ssum = 0.0
+    for dl, m1d, m2d, lnp in zip(*inj):
+        z, wgt = weight(dl, m1d, m2d)
+        if z <= z_cat_max:
+            ssum += wgt * (4 * math.pi * dC(z) ** 2 * C / H0 / E(z)) / Vmax / math.exp(lnp)
+    xi = ssum / n_inj_total
+    return total - len(events) * math.log(xi), np.array(logI), math.log(xi)
+
+
+@pytest.mark.parametrize("fixed_h", [None, 0.01])
+def test_p11_brute_force_two_events_three_samples(fixed_h):
+    w = make_workload("tiny", n_events=2, n_samples=3, n_grid=40, n_inj_draw=60)
+    la = w.lam[0].copy()
+    la[2], la[3] = 1.4, 2.2                                        # exercise Xi(z)
+    events = [_one_event(w, i) for i in range(2)]
+    inj = (w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw)
+    ref_total, ref_logI, ref_logxi = _brute_loglike(la, events, inj, w.n_inj_total, w.z_cat_max, fixed_h)
+    kw = {} if fixed_h is None else dict(bw_rule=O.BW_FIXED, fixed_bw=np.full(2, fixed_h))
+    r = O.loglike_workload(w, lam=la, **kw)
+    assert np.allclose(r["event_logI"][0], ref_logI, rtol=0, atol=2e-8)
+    assert abs(r["logxi"][0] - ref_logxi) < 2e-8
+    assert abs(r["loglike"][0] - ref_total) < 1e-7
+
+
+def test_p11_trapezoid_against_simpson_on_refined_grid():
+    # analytic p_gal, 20x finer grid + Simpson: the grid trapezoid is converged to ~1e-9 on Gaussians
+    rng = np.random.default_rng(11)
+    z, w = 0.5 + 0.02 * rng.standard_normal(25), rng.random(25)
+    h = 0.008
+    pg = lambda x: np.exp(-0.5 * ((x - 0.51) / 0.004) ** 2)
+    zg = np.linspace(0.35, 0.65, 301)
+    I = O.event_integral(lam(), zg, O.kde(z, w, h, zg), pg(zg))
+    zf = np.linspace(0.35, 0.65, 6001)
+    Is = integrate.simpson(O.kde(z, w, h, zf) * pg(zf), x=zf)
+    assert abs(I / Is - 1) < 1e-9
+
+
+# ------------------------------------------------------------------ flags / degenerate cases
+def test_flags_and_degenerate_cases():
+    w = make_workload("tiny", n_events=2, n_samples=50, n_grid=60, n_inj_draw=200)
+    bad = w.lam[0].copy()
+    bad[1] = 1.5                                                    # Om outside (0, 1]
+    r = O.loglike_workload(w, lam=np.stack([w.lam[0], bad]))
+    assert r["flags"][1] & O.F_LAMBDA_DOMAIN and np.isnan(r["loglike"][1]) and np.isfinite(r["loglike"][0])
+    # an event whose secondary masses are all below m_low has zero weight -> log I = -inf
+    w.m2d[:50] = 1.0
+    r = O.loglike_workload(w, lam=w.lam[0])
+    assert r["flags"][0] & O.F_EVENT_ZERO and r["event_logI"][0, 0] == -np.inf and r["loglike"][0] == -np.inf
+    # no injections: log xi := 0
+    w2 = make_workload("tiny", n_events=2, n_samples=50, n_grid=60, n_inj_draw=200)
+    r2 = O.loglike_batch(w2.lam[0], w2.sample_off, w2.dL, w2.m1d, w2.m2d, w2.ln_prior, w2.grid_off, w2.z_grid, w2.p_gal)
+    assert r2["logxi"][0] == 0 and abs(r2["loglike"][0] - r2["event_logI"][0].sum()) < 1e-12
+
+
+def test_log_likelihood_assembly_eq3():
+    w = make_workload("tiny", n_events=3, n_samples=80, n_grid=60, n_inj_draw=400)
+    r = O.loglike_workload(w)
+    s1, s2 = O.selection_sums(w.lam[0], w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw)
+    assert abs(r["logxi"][0] - math.log(s1 / w.n_inj_total)) < 1e-13
+    assert abs(r["loglike"][0] - (r["event_logI"][0].sum() - 3 * r["logxi"][0])) < 1e-11
+    assert abs(r["neff"][0] - s1 * s1 / (s2 - s1 * s1 / w.n_inj_total)) < 1e-9
