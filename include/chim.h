@@ -1,0 +1,175 @@
+/*
+ * chim.h -- C ABI of libchim: the B200-native hot path of the CHIMERA-2.0 hierarchical likelihood
+ * (arXiv:2504.02034; citations are /root/reference PAPER.md:<line>, readings R1.., M1.. are in DESIGN.md).
+ *
+ * What one chim_loglike_batch call computes, for every hyper-parameter point lambda in the batch:
+ *
+ *   log L(lambda) = sum_i log I_i(lambda) - N_events * log xi(lambda)             (eq. 3)
+ *
+ *   I_i  = int dz  K_gw,i(z | lambda) * p_gal,i(z) [* psi/J on the grid if placement = ON_GRID]
+ *          (eq. 14, N_pix = 1), evaluated as a composite trapezoid on event i's own
+ *          redshift grid, with K_gw,i the weighted Gaussian KDE of the event's posterior samples in
+ *          redshift ("single-1d" kernel, eq. 19):
+ *              K_i(z) = 1/(N_s h sqrt(2 pi)) sum_j w_j exp(-(z - z_j)^2 / (2 h^2))
+ *          z_j solves d_L^gw(z_j; lambda) = d_L,j with d_L^gw = Xi(z) d_L^em(z), Xi = Xi0 + (1-Xi0)/(1+z)^n
+ *          (PAPER.md:17 eq. 1, :23 eq. 2, :52); m_{1,2} = m^d_{1,2}/(1+z_j);
+ *              w_j = p(m1,m2 | lambda_m) * [psi(z_j)/((1+z_j)^3 |d d_L^gw/dz|)]^{ON_SAMPLES} / pi_j
+ *          (PAPER.md:112 eq. 16 weights, :75 eq. 11 Jacobian, :195 eq. 20 mass model, :226 eq. 21 rate).
+ *   xi   = (1/N_inj) sum_{j in detected} s_j,   s_j = p_pop^d(theta_j | lambda) / p_draw,j
+ *          (eq. 12) with N_eff from PAPER.md:91 eq. 13.
+ *
+ * lambda is 15 doubles: H0 [km/s/Mpc], Om, Xi0, n, alpha, beta, delta_m, m_low, m_high, mu_g, sigma_g,
+ * lambda_g, gamma, kappa, z_p  (Table 1).
+ *
+ * Ownership: the caller owns every pointer it passes.  chim_init_* copy and re-pack their inputs before
+ * returning (inputs may be freed at once).  Outputs are caller-allocated.  The context owns its device
+ * memory until chim_destroy.  Calling an init again replaces the previous set.
+ *
+ * Threads/streams: one context per stream; calls on one context are not re-entrant.
+ *
+ * Errors: every int-returning call returns CHIM_OK (0) or a negative chim_status; the message is
+ * available from chim_last_error(ctx).  Nothing aborts or throws across the boundary.  Numerical
+ * conditions are per-lambda and do not fail the call: they set bits in out_flags (CHIM_FLAG_*).
+ *
+ * There is no CPU fallback: every entry point that computes needs a CUDA device of compute
+ * capability 10.0 (sm_100a).
+ */
+#ifndef CHIM_H
+#define CHIM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CHIM_VERSION 100 /* 0.1.0 */
+#define CHIM_N_LAMBDA_PARAMS 15
+
+typedef enum chim_status {
+    CHIM_OK = 0,
+    CHIM_EINVAL = -1, /* null pointer, bad size, non-increasing grid, m1d < m2d, non-finite input      */
+    CHIM_ESTATE = -2, /* chim_loglike_batch before chim_init_events, debug call on a missing set        */
+    CHIM_ECUDA = -3,  /* a CUDA runtime call failed (message holds the CUDA error string)               */
+    CHIM_ENOMEM = -4  /* host or device allocation failed                                               */
+} chim_status;
+
+enum { CHIM_MEM_HOST = 0, CHIM_MEM_DEVICE = 1 };   /* where the pointers given to chim_init_* live     */
+enum { CHIM_ON_SAMPLES = 0, CHIM_ON_GRID = 1 };    /* placement of psi/J (R1): N = per-sample weights  */
+enum { CHIM_BW_SCOTT = 0, CHIM_BW_FIXED = 1 };     /* KDE bandwidth rule (R3)                          */
+
+/* per-lambda flag bits written to out_flags */
+#define CHIM_FLAG_LAMBDA_DOMAIN 1u   /* H0<=0, Om not in (0,1], Xi0<=0, delta_m<=0, sigma_g<=0, lambda_g not in
+                                        [0,1], m_low<=0, m_high<=m_low, z_p<=-1, non-finite -> loglike = NaN    */
+#define CHIM_FLAG_DL_NONMONOTONE 2u  /* d d_L^gw/dz <= 0 at a table node (R16) -> loglike = NaN                  */
+#define CHIM_FLAG_EVENT_ZERO 4u      /* some I_i = 0 (all weights zero) -> loglike = -inf                        */
+#define CHIM_FLAG_XI_ZERO 8u         /* xi = 0 -> loglike = NaN                                                  */
+#define CHIM_FLAG_NEFF_LOW 16u       /* N_eff < neff_factor * N_events (R8); loglike is left untouched           */
+#define CHIM_FLAG_TABLE_RANGE 32u    /* a sample's d_L exceeds d_L^gw(z_table_max): that sample gets weight 0    */
+#define CHIM_FLAG_BW_DEGENERATE 64u  /* Scott bandwidth undefined (one effective sample) -> that log I_i = NaN   */
+
+typedef struct chim_ctx chim_ctx; /* opaque; owns all device copies */
+
+typedef struct chim_config {
+    int32_t device;      /* CUDA ordinal                                                                      */
+    int32_t mem;         /* CHIM_MEM_HOST | CHIM_MEM_DEVICE: where the chim_init_* input pointers live        */
+    void *stream;        /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream */
+    int32_t placement;   /* CHIM_ON_SAMPLES (default, benchmarked) | CHIM_ON_GRID (paper eq. 14 literally)    */
+    int32_t bw_rule;     /* CHIM_BW_SCOTT (default) | CHIM_BW_FIXED (uses fixed_bw[] of chim_init_events)      */
+    double kde_cutoff;   /* t: sample-grid pairs with |z_g - z_j| > t*h may be skipped (R9); 0 = never skip    */
+    double z_cat_max;    /* z_max of PAPER.md:65 eq. 9: support of the selection-term redshift density (R6)    */
+    double z_table_max;  /* extent of the d_C(z) table; samples with z > z_table_max get weight 0 (+ flag)     */
+    int32_t n_table;     /* panels of the d_C(z) table on [0, z_table_max] (also the monotonicity check nodes) */
+    int32_t n_dl_table;  /* intervals of the per-lambda z(ln d_L) interpolation tables                         */
+    int32_t n_win_table; /* panels of the per-lambda window table of int m^beta S(m) dm (M4)                   */
+    int32_t lambda_chunk;/* lambdas processed per internal pass (bounds the per-lambda table memory)           */
+    double neff_factor;  /* NEFF_LOW is raised if N_eff < neff_factor * N_events (R8)                          */
+} chim_config;
+
+/* Fills *cfg with the defaults: device 0, HOST, NULL stream, ON_SAMPLES, SCOTT, kde_cutoff 6.0,
+ * z_cat_max 1.5, z_table_max 10, n_table 2048, n_dl_table 2048, n_win_table 512, lambda_chunk 256,
+ * neff_factor 5. */
+void chim_default_config(chim_config *cfg);
+
+/* Creates a context on cfg->device.  cfg == NULL means chim_default_config.  *out is set to NULL on error
+ * (the status is then the only report).  Fails with CHIM_ECUDA if no sm_100 device is present. */
+int chim_create(const chim_config *cfg, chim_ctx **out);
+void chim_destroy(chim_ctx *ctx);
+const char *chim_last_error(const chim_ctx *ctx); /* never NULL; "" if no error yet */
+int chim_version(void);
+
+/*
+ * Events (PE samples, the fixed per-event redshift grid, p_gal on it).
+ *   sample_off [n_events+1] : CSR offsets into dL/m1d/m2d/ln_prior (ragged N_s allowed, N_s >= 1)
+ *   dL [Mpc] > 0, m1d >= m2d > 0 [Msun, detector frame], ln_prior = ln pi(theta^d_j) (any prior, R10)
+ *   grid_off [n_events+1]   : CSR offsets into z_grid/p_gal (N_z >= 2 per event)
+ *   z_grid strictly increasing and >= 0 per event (uniform or not, R14); p_gal >= 0
+ *   fixed_bw [n_events] or NULL: bandwidth h_i > 0 when cfg.bw_rule == CHIM_BW_FIXED
+ * All arrays live where cfg.mem says.  Samples are re-ordered internally (sorted by d_L); every
+ * per-sample output of the debug calls is returned in the caller's original order.
+ */
+int chim_init_events(chim_ctx *ctx, int32_t n_events, const int64_t *sample_off, const double *dL,
+                     const double *m1d, const double *m2d, const double *ln_prior,
+                     const int64_t *grid_off, const double *z_grid, const double *p_gal,
+                     const double *fixed_bw);
+
+/*
+ * Detected injections for the selection term: n_det stored injections out of
+ * n_inj_total drawn; ln_pdraw = ln of the draw density in (d_L, m1d, m2d) (R7).  Optional: without
+ * injections log xi := 0 and loglike = sum_i log I_i.  n_det == 0 removes a previous set.
+ */
+int chim_init_injections(chim_ctx *ctx, int64_t n_det, int64_t n_inj_total, const double *dL,
+                         const double *m1d, const double *m2d, const double *ln_pdraw);
+
+/*
+ * The hot path.  lambda [n_lambda x 15] row-major and all outputs are DEVICE pointers; the call only
+ * enqueues work on cfg.stream (no host synchronisation) -- the caller synchronises.
+ *   out_loglike    [n_lambda]            required
+ *   out_event_logI [n_lambda x n_events] or NULL   (log I_i; -inf if I_i = 0, NaN if lambda invalid)
+ *   out_logxi      [n_lambda] or NULL    (0 without injections)
+ *   out_neff       [n_lambda] or NULL    (N_eff of eq. 13; NaN without injections)
+ *   out_flags      [n_lambda] or NULL    (CHIM_FLAG_* bits)
+ */
+int chim_loglike_batch(chim_ctx *ctx, int32_t n_lambda, const double *lambda, double *out_loglike,
+                       double *out_event_logI, double *out_logxi, double *out_neff, uint32_t *out_flags);
+
+/* Same computation with HOST pointers: copies lambda to the device, runs the path, copies the
+ * requested outputs back and synchronises cfg.stream before returning (the end-to-end call). */
+int chim_loglike_batch_host(chim_ctx *ctx, int32_t n_lambda, const double *lambda, double *out_loglike,
+                            double *out_event_logI, double *out_logxi, double *out_neff,
+                            uint32_t *out_flags);
+
+/* Work counters of the last chim_loglike_batch on this context (valid after the stream is synchronised;
+ * the call itself synchronises).  kde_pairs_evaluated = sample x grid-point exponentials actually issued
+ * (after the cut-off skip); kde_pairs_dense = sum_i N_s,i N_z,i x n_lambda. */
+typedef struct chim_stats {
+    uint64_t kde_pairs_evaluated;
+    uint64_t kde_pairs_dense;
+    uint64_t sample_evals;    /* (sample, lambda) weight evaluations  */
+    uint64_t injection_evals; /* (injection, lambda) weight evaluations */
+    uint64_t kernel_launches; /* kernels launched by the last batch call */
+} chim_stats;
+int chim_get_stats(chim_ctx *ctx, chim_stats *out);
+
+/* ---- diagnostics: intermediates of the path for ONE lambda (DEVICE pointer to 15 doubles) -------------
+ * They run the same device code as the hot path and exist so that each step can be compared with the
+ * oracle (tests tier T2).  Outputs are DEVICE pointers; any of them may be NULL.  Synchronous. */
+
+/* Step S1: the per-lambda event table.  For n query distances dL[] (inside the d_L range of the event
+ * set) returns z(dL) and the smooth redshift factor of the weights, psi(z)/J(z) (1 if ON_GRID). */
+int chim_debug_table_lookup(chim_ctx *ctx, const double *lambda, int64_t n, const double *dL,
+                            double *z_out, double *ratio_out);
+/* Step S2: per-sample redshift and weight of event `event`, in the caller's sample order [N_s]. */
+int chim_debug_event_samples(chim_ctx *ctx, const double *lambda, int32_t event, double *z_out,
+                             double *w_out);
+/* Steps S2-S4: bandwidth h (1 double), KDE on the event grid K_out [N_z] (no cut-off applied to the
+ * returned K if kde_cutoff == 0; otherwise the skipped pairs are missing from it), and log I. */
+int chim_debug_event_kde(chim_ctx *ctx, const double *lambda, int32_t event, double *h_out, double *K_out,
+                         double *logI_out);
+/* Step S5: per-injection s_j in the caller's order [n_det]. */
+int chim_debug_injection_weights(chim_ctx *ctx, const double *lambda, double *s_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHIM_H */

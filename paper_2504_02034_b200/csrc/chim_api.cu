@@ -1,0 +1,575 @@
+// chim_api.cu -- the C ABI of libchim (include/chim.h): context, init-time packing, batch driver.
+//
+// Init (one-off, not on the hot path; SURVEY call stack (iii)): validate -> sort each event's samples by d_L
+// (lambda-independent order: d_L^gw(z) is monotone, so sorted d_L means sorted z_j for every lambda) ->
+// per-sample table coordinate in ln d_L, logs and mass ratio (all lambda-independent) -> centred grid and
+// q_g = p_gal x trapezoid weight -> upload.  The batch call only enqueues kernels on the caller's stream.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "chim_internal.cuh"
+
+using namespace chim;
+
+namespace {
+constexpr size_t kMaxSmemOptin = 232448;   // 227 KB per CTA on sm_100
+constexpr int kInjChunk = 1024;            // injections per CTA of k_inject
+}
+
+struct chim_ctx {
+    chim_config cfg;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    std::vector<void*> owned_ev, owned_inj, owned_work, owned_host;
+    // events
+    bool have_events = false;
+    EventSetDev ev{};
+    DlGrid ev_grid{0, 1, 0};
+    const double* ev_ln_shift = nullptr;   // [n_events] added back to log I (prior scale factored out)
+    std::vector<int64_t> h_sample_off, h_grid_off;
+    // injections
+    bool have_inj = false;
+    InjSetDev inj{};
+    DlGrid inj_grid{0, 1, 0};
+    double inj_ln_shift = 0.0;
+    int inj_blocks = 0;
+    // work buffers for one lambda chunk
+    int work_nl = 0;
+    bool work_has_dc = false;
+    LamConst* Lc = nullptr; Row* tab_ev = nullptr; Row* tab_inj = nullptr; double* wtab = nullptr;
+    double* dc_tab = nullptr; double* logI = nullptr; double2* partial = nullptr; uint32_t* flags = nullptr;
+    unsigned long long* stats = nullptr;
+    // staging for the host-pointer entry point
+    int host_nl = 0;
+    double* st_lam = nullptr; double* st_ll = nullptr; double* st_ev = nullptr; double* st_xi = nullptr;
+    double* st_neff = nullptr; uint32_t* st_fl = nullptr;
+    chim_stats last{};
+    uint64_t launches = 0;
+};
+
+namespace {
+
+int fail(chim_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg;
+    return code;
+}
+int cuda_fail(chim_ctx* c, cudaError_t e, const char* where) {
+    return fail(c, e == cudaErrorMemoryAllocation ? CHIM_ENOMEM : CHIM_ECUDA,
+                std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                  \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call); \
+    } while (0)
+
+template <class T>
+cudaError_t dev_alloc(std::vector<void*>& pool, T** p, size_t n) {
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, std::max<size_t>(n, 1) * sizeof(T));
+    if (e == cudaSuccess) { pool.push_back(q); *p = static_cast<T*>(q); }
+    return e;
+}
+void free_pool(std::vector<void*>& pool) {
+    for (void* p : pool) cudaFree(p);
+    pool.clear();
+}
+template <class T>
+cudaError_t upload(std::vector<void*>& pool, const T** dst, const std::vector<T>& src) {
+    T* d = nullptr;
+    cudaError_t e = dev_alloc(pool, &d, src.size());
+    if (e != cudaSuccess) return e;
+    if (!src.empty()) e = cudaMemcpy(d, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice);
+    *dst = d;
+    return e;
+}
+// bring an init input to the host (inputs live where cfg.mem says)
+template <class T>
+cudaError_t fetch(const chim_ctx* c, const T* src, size_t n, std::vector<T>& dst) {
+    dst.resize(n);
+    if (n == 0) return cudaSuccess;
+    if (c->cfg.mem == CHIM_MEM_DEVICE) return cudaMemcpy(dst.data(), src, n * sizeof(T), cudaMemcpyDeviceToHost);
+    std::memcpy(dst.data(), src, n * sizeof(T));
+    return cudaSuccess;
+}
+
+DlGrid make_dl_grid(double xmin, double xmax, int K) {
+    DlGrid g;
+    g.x0 = xmin;
+    g.K = K;
+    double span = xmax - xmin;
+    g.dx = (span > 0.0) ? span * (1.0 + 1e-12) / K + 1e-300 : 1e-6;
+    return g;
+}
+
+int ensure_work(chim_ctx* ctx, int nl) {
+    bool need_dc = ctx->cfg.placement == CHIM_ON_GRID;
+    if (nl <= ctx->work_nl && (!need_dc || ctx->work_has_dc)) return CHIM_OK;
+    free_pool(ctx->owned_work);
+    ctx->work_nl = 0;
+    CK(dev_alloc(ctx->owned_work, &ctx->Lc, nl));
+    CK(dev_alloc(ctx->owned_work, &ctx->tab_ev, (size_t)nl * ctx->ev_grid.rows()));
+    CK(dev_alloc(ctx->owned_work, &ctx->tab_inj, (size_t)nl * (ctx->have_inj ? ctx->inj_grid.rows() : 1)));
+    CK(dev_alloc(ctx->owned_work, &ctx->wtab, (size_t)nl * (ctx->cfg.n_win_table + 1)));
+    ctx->dc_tab = nullptr;
+    if (need_dc) CK(dev_alloc(ctx->owned_work, &ctx->dc_tab, (size_t)nl * (ctx->cfg.n_table + 1 + kZPad)));
+    CK(dev_alloc(ctx->owned_work, &ctx->logI, (size_t)nl * ctx->ev.n_events));
+    CK(dev_alloc(ctx->owned_work, &ctx->partial, (size_t)nl * std::max(ctx->inj_blocks, 1)));
+    CK(dev_alloc(ctx->owned_work, &ctx->flags, nl));
+    CK(dev_alloc(ctx->owned_work, &ctx->stats, 4));
+    ctx->work_nl = nl;
+    ctx->work_has_dc = need_dc;
+    return CHIM_OK;
+}
+
+TableParams table_params(const chim_ctx* ctx) {
+    TableParams P;
+    P.z_table_max = ctx->cfg.z_table_max;
+    P.z_cat_max = ctx->cfg.z_cat_max;
+    P.n_table = ctx->cfg.n_table;
+    P.n_win = ctx->cfg.n_win_table;
+    P.placement = ctx->cfg.placement;
+    P.ev = ctx->ev_grid;
+    P.inj = ctx->have_inj ? ctx->inj_grid : DlGrid{0, 1, 0};
+    return P;
+}
+
+EventKernelParams event_params(const chim_ctx* ctx, int nl) {
+    EventKernelParams P{};
+    P.ev = ctx->ev;
+    P.Lc = ctx->Lc; P.tab = ctx->tab_ev; P.wtab = ctx->wtab; P.dc_tab = ctx->dc_tab;
+    P.n_lambda = nl; P.tab_rows = ctx->ev_grid.rows(); P.n_win = ctx->cfg.n_win_table; P.n_table = ctx->cfg.n_table;
+    P.placement = ctx->cfg.placement; P.bw_rule = ctx->cfg.bw_rule;
+    P.z_table_max = ctx->cfg.z_table_max; P.cutoff = ctx->cfg.kde_cutoff;
+    P.logI = ctx->logI; P.flags = ctx->flags; P.stats = ctx->stats;
+    P.ln_shift = ctx->ev_ln_shift;
+    P.dbg_event = -1;
+    return P;
+}
+
+// one pass over a chunk of lambdas: S1 -> S2-S4 -> S5 -> S6
+int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* out_ev, double* out_xi, double* out_neff,
+              uint32_t* out_fl) {
+    cudaStream_t st = ctx->stream;
+    TableParams TP = table_params(ctx);
+    CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t) * nl, st));
+    CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->wtab, st));
+    EventKernelParams EP = event_params(ctx, nl);
+    CK(launch_events(EP, st));
+    ctx->launches += 2;
+    if (ctx->have_inj) {
+        InjKernelParams IP{};
+        IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.wtab = ctx->wtab;
+        IP.n_lambda = nl; IP.tab_rows = ctx->inj_grid.rows(); IP.n_win = ctx->cfg.n_win_table; IP.chunk = kInjChunk;
+        IP.z_table_max = ctx->cfg.z_table_max; IP.z_cat_max = ctx->cfg.z_cat_max;
+        IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = nullptr;
+        CK(launch_inject(IP, ctx->inj_blocks, st));
+        ctx->launches += 1;
+    }
+    CombineParams CP{};
+    CP.Lc = ctx->Lc; CP.logI = ctx->logI; CP.partial = ctx->partial;
+    CP.n_lambda = nl; CP.n_events = ctx->ev.n_events; CP.n_inj_blocks = ctx->inj_blocks;
+    CP.n_det = ctx->have_inj ? ctx->inj.n_det : 0;
+    CP.n_inj_total = ctx->have_inj ? ctx->inj.n_inj_total : 1.0;
+    CP.inj_ln_shift = ctx->inj_ln_shift;
+    CP.neff_factor = ctx->cfg.neff_factor; CP.flags_in = ctx->flags;
+    CP.out_loglike = out_ll; CP.out_event_logI = out_ev; CP.out_logxi = out_xi; CP.out_neff = out_neff; CP.out_flags = out_fl;
+    CK(launch_combine(CP, st));
+    ctx->launches += 1;
+    return CHIM_OK;
+}
+
+bool all_finite(const std::vector<double>& v) {
+    for (double x : v) if (!std::isfinite(x)) return false;
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+void chim_default_config(chim_config* cfg) {
+    if (!cfg) return;
+    std::memset(cfg, 0, sizeof(*cfg));
+    cfg->device = 0;
+    cfg->mem = CHIM_MEM_HOST;
+    cfg->stream = nullptr;
+    cfg->placement = CHIM_ON_SAMPLES;
+    cfg->bw_rule = CHIM_BW_SCOTT;
+    cfg->kde_cutoff = 6.0;
+    cfg->z_cat_max = 1.5;
+    cfg->z_table_max = 10.0;
+    cfg->n_table = 2048;
+    cfg->n_dl_table = 2048;
+    cfg->n_win_table = 512;
+    cfg->lambda_chunk = 256;
+    cfg->neff_factor = 5.0;
+}
+
+int chim_version(void) { return CHIM_VERSION; }
+
+const char* chim_last_error(const chim_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int chim_create(const chim_config* cfg, chim_ctx** out) {
+    if (!out) return CHIM_EINVAL;
+    *out = nullptr;
+    chim_config c;
+    if (cfg) c = *cfg; else chim_default_config(&c);
+    chim_config d;
+    chim_default_config(&d);
+    if (c.n_table <= 0) c.n_table = d.n_table;
+    if (c.n_dl_table <= 0) c.n_dl_table = d.n_dl_table;
+    if (c.n_win_table <= 0) c.n_win_table = d.n_win_table;
+    if (c.lambda_chunk <= 0) c.lambda_chunk = d.lambda_chunk;
+    if (!(c.z_table_max > 0.0)) c.z_table_max = d.z_table_max;
+    if (!(c.z_cat_max > 0.0)) c.z_cat_max = d.z_cat_max;
+    if (!(c.neff_factor >= 0.0)) c.neff_factor = d.neff_factor;
+    if (c.kde_cutoff < 0.0 || !std::isfinite(c.kde_cutoff)) return CHIM_EINVAL;
+    if (c.n_table < 16 || c.n_dl_table < 16 || c.n_win_table < 8 || c.z_cat_max > c.z_table_max) return CHIM_EINVAL;
+    if (c.placement != CHIM_ON_SAMPLES && c.placement != CHIM_ON_GRID) return CHIM_EINVAL;
+    if (c.bw_rule != CHIM_BW_SCOTT && c.bw_rule != CHIM_BW_FIXED) return CHIM_EINVAL;
+    if (c.mem != CHIM_MEM_HOST && c.mem != CHIM_MEM_DEVICE) return CHIM_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device < 0 || c.device >= ndev) return CHIM_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, c.device) != cudaSuccess) return CHIM_ECUDA;
+    if (prop.major != 10) return CHIM_ECUDA;   // sm_100a only: no other code path exists
+    if (cudaSetDevice(c.device) != cudaSuccess) return CHIM_ECUDA;
+    chim_ctx* ctx = new (std::nothrow) chim_ctx();
+    if (!ctx) return CHIM_ENOMEM;
+    ctx->cfg = c;
+    ctx->stream = static_cast<cudaStream_t>(c.stream);
+    TableParams TP = table_params(ctx);
+    TP.ev.K = TP.inj.K = c.n_dl_table;
+    if (tables_smem_bytes(TP) > kMaxSmemOptin) { delete ctx; return CHIM_EINVAL; }
+    if (upload_gauss_legendre() != cudaSuccess) { delete ctx; return CHIM_ECUDA; }
+    *out = ctx;
+    return CHIM_OK;
+}
+
+void chim_destroy(chim_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->cfg.device);
+    cudaStreamSynchronize(ctx->stream);
+    free_pool(ctx->owned_ev);
+    free_pool(ctx->owned_inj);
+    free_pool(ctx->owned_work);
+    free_pool(ctx->owned_host);
+    delete ctx;
+}
+
+int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off, const double* dL, const double* m1d,
+                     const double* m2d, const double* ln_prior, const int64_t* grid_off, const double* z_grid,
+                     const double* p_gal, const double* fixed_bw) {
+    if (!ctx) return CHIM_EINVAL;
+    if (n_events < 1 || !sample_off || !dL || !m1d || !m2d || !ln_prior || !grid_off || !z_grid || !p_gal)
+        return fail(ctx, CHIM_EINVAL, "chim_init_events: null pointer or n_events < 1");
+    if (ctx->cfg.bw_rule == CHIM_BW_FIXED && !fixed_bw)
+        return fail(ctx, CHIM_EINVAL, "chim_init_events: bw_rule is CHIM_BW_FIXED but fixed_bw is NULL");
+    CK(cudaSetDevice(ctx->cfg.device));
+    std::vector<int64_t> so, go;
+    CK(fetch(ctx, sample_off, (size_t)n_events + 1, so));
+    CK(fetch(ctx, grid_off, (size_t)n_events + 1, go));
+    if (so[0] != 0 || go[0] != 0) return fail(ctx, CHIM_EINVAL, "chim_init_events: offsets must start at 0");
+    int max_ns = 0, max_nz = 0;
+    for (int i = 0; i < n_events; ++i) {
+        int64_t ns = so[i + 1] - so[i], nz = go[i + 1] - go[i];
+        if (ns < 1 || nz < 2 || ns > (1 << 30) || nz > (1 << 30))
+            return fail(ctx, CHIM_EINVAL, "chim_init_events: every event needs N_s >= 1 samples and N_z >= 2 grid points");
+        max_ns = std::max<int>(max_ns, (int)ns);
+        max_nz = std::max<int>(max_nz, (int)nz);
+    }
+    if (events_smem_bytes(max_ns) > kMaxSmemOptin) {
+        char b[160];
+        std::snprintf(b, sizeof b, "chim_init_events: N_s = %d exceeds the shared-memory staging limit (%d samples per event)",
+                      max_ns, (int)((kMaxSmemOptin - 1024) / 16));
+        return fail(ctx, CHIM_EINVAL, b);
+    }
+    const size_t NS = (size_t)so[n_events], NG = (size_t)go[n_events];
+    std::vector<double> h_dl, h_m1, h_m2, h_lp, h_z, h_p, h_bw;
+    CK(fetch(ctx, dL, NS, h_dl)); CK(fetch(ctx, m1d, NS, h_m1)); CK(fetch(ctx, m2d, NS, h_m2));
+    CK(fetch(ctx, ln_prior, NS, h_lp)); CK(fetch(ctx, z_grid, NG, h_z)); CK(fetch(ctx, p_gal, NG, h_p));
+    if (fixed_bw) CK(fetch(ctx, fixed_bw, (size_t)n_events, h_bw));
+    if (!all_finite(h_dl) || !all_finite(h_m1) || !all_finite(h_m2) || !all_finite(h_lp) || !all_finite(h_z) ||
+        !all_finite(h_p) || !all_finite(h_bw))
+        return fail(ctx, CHIM_EINVAL, "chim_init_events: non-finite input");
+    double xmin = INFINITY, xmax = -INFINITY;
+    for (size_t j = 0; j < NS; ++j) {
+        if (!(h_dl[j] > 0.0) || !(h_m2[j] > 0.0) || !(h_m1[j] >= h_m2[j]))
+            return fail(ctx, CHIM_EINVAL, "chim_init_events: need dL > 0 and m1d >= m2d > 0");
+        double x = std::log(h_dl[j]);
+        xmin = std::min(xmin, x);
+        xmax = std::max(xmax, x);
+    }
+    for (int i = 0; i < n_events; ++i) {
+        for (int64_t g = go[i]; g < go[i + 1]; ++g) {
+            if (h_z[g] < 0.0 || h_p[g] < 0.0 || (g > go[i] && !(h_z[g] > h_z[g - 1])))
+                return fail(ctx, CHIM_EINVAL, "chim_init_events: z_grid must be >= 0 and strictly increasing, p_gal >= 0");
+        }
+        if (ctx->cfg.bw_rule == CHIM_BW_FIXED && !(h_bw[i] > 0.0))
+            return fail(ctx, CHIM_EINVAL, "chim_init_events: fixed_bw must be > 0");
+    }
+    DlGrid grid = make_dl_grid(xmin, xmax, ctx->cfg.n_dl_table);
+
+    std::vector<double2> rA(NS), rB(NS), rC(NS);
+    std::vector<int32_t> perm(NS);
+    std::vector<double> zc(NG), qg(NG), z0(n_events), shift(n_events);
+    std::vector<int32_t> idx;
+    for (int i = 0; i < n_events; ++i) {
+        const int64_t s0 = so[i];
+        const int ns = (int)(so[i + 1] - s0);
+        idx.resize(ns);
+        std::iota(idx.begin(), idx.end(), 0);
+        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return h_dl[s0 + a] < h_dl[s0 + b]; });
+        double sh = -INFINITY;   // factor the prior scale out of the weights: 1/pi_j = exp(sh) * ipr_j
+        for (int j = 0; j < ns; ++j) sh = std::max(sh, -h_lp[s0 + j]);
+        shift[i] = sh;
+        for (int j = 0; j < ns; ++j) {
+            const int64_t o = s0 + idx[j];
+            double q = h_m2[o] / h_m1[o];
+            rA[s0 + j] = make_double2((std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0, h_m1[o]);
+            rB[s0 + j] = make_double2(q, std::log(h_m1[o]));
+            rC[s0 + j] = make_double2(std::log(q), std::exp(-h_lp[o] - sh));
+            perm[s0 + j] = idx[j];
+        }
+        const int64_t g0 = go[i];
+        const int nz = (int)(go[i + 1] - g0);
+        z0[i] = 0.5 * (h_z[g0] + h_z[g0 + nz - 1]);
+        for (int g = 0; g < nz; ++g) {
+            double wl = (g > 0) ? h_z[g0 + g] - h_z[g0 + g - 1] : 0.0;
+            double wr = (g + 1 < nz) ? h_z[g0 + g + 1] - h_z[g0 + g] : 0.0;
+            zc[g0 + g] = h_z[g0 + g] - z0[i];
+            qg[g0 + g] = h_p[g0 + g] * 0.5 * (wl + wr);   // composite trapezoid weight (O9)
+        }
+    }
+    // replace the previous set
+    cudaStreamSynchronize(ctx->stream);
+    free_pool(ctx->owned_ev);
+    free_pool(ctx->owned_work);
+    ctx->work_nl = 0;
+    ctx->have_events = false;
+    EventSetDev E{};
+    E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz;
+    CK(upload(ctx->owned_ev, &E.sample_off, so)); CK(upload(ctx->owned_ev, &E.grid_off, go));
+    CK(upload(ctx->owned_ev, &E.recA, rA)); CK(upload(ctx->owned_ev, &E.recB, rB)); CK(upload(ctx->owned_ev, &E.recC, rC));
+    CK(upload(ctx->owned_ev, &E.perm, perm)); CK(upload(ctx->owned_ev, &E.zc, zc)); CK(upload(ctx->owned_ev, &E.qg, qg));
+    CK(upload(ctx->owned_ev, &E.z0, z0));
+    if (fixed_bw) CK(upload(ctx->owned_ev, &E.fixed_bw, h_bw));
+    CK(upload(ctx->owned_ev, &ctx->ev_ln_shift, shift));
+    ctx->ev = E;
+    ctx->ev_grid = grid;
+    ctx->h_sample_off = so;
+    ctx->h_grid_off = go;
+    ctx->have_events = true;
+    return CHIM_OK;
+}
+
+int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, const double* dL, const double* m1d,
+                         const double* m2d, const double* ln_pdraw) {
+    if (!ctx) return CHIM_EINVAL;
+    CK(cudaSetDevice(ctx->cfg.device));
+    if (n_det == 0) {
+        cudaStreamSynchronize(ctx->stream);
+        free_pool(ctx->owned_inj);
+        free_pool(ctx->owned_work);
+        ctx->work_nl = 0;
+        ctx->have_inj = false;
+        ctx->inj_blocks = 0;
+        return CHIM_OK;
+    }
+    if (n_det < 0 || n_inj_total < n_det || !dL || !m1d || !m2d || !ln_pdraw)
+        return fail(ctx, CHIM_EINVAL, "chim_init_injections: null pointer, n_det < 0 or n_inj_total < n_det");
+    const size_t N = (size_t)n_det;
+    std::vector<double> h_dl, h_m1, h_m2, h_lp;
+    CK(fetch(ctx, dL, N, h_dl)); CK(fetch(ctx, m1d, N, h_m1)); CK(fetch(ctx, m2d, N, h_m2)); CK(fetch(ctx, ln_pdraw, N, h_lp));
+    if (!all_finite(h_dl) || !all_finite(h_m1) || !all_finite(h_m2) || !all_finite(h_lp))
+        return fail(ctx, CHIM_EINVAL, "chim_init_injections: non-finite input");
+    double xmin = INFINITY, xmax = -INFINITY, sh = -INFINITY;
+    for (size_t j = 0; j < N; ++j) {
+        if (!(h_dl[j] > 0.0) || !(h_m2[j] > 0.0) || !(h_m1[j] >= h_m2[j]))
+            return fail(ctx, CHIM_EINVAL, "chim_init_injections: need dL > 0 and m1d >= m2d > 0");
+        double x = std::log(h_dl[j]);
+        xmin = std::min(xmin, x);
+        xmax = std::max(xmax, x);
+        sh = std::max(sh, -h_lp[j]);
+    }
+    DlGrid grid = make_dl_grid(xmin, xmax, ctx->cfg.n_dl_table);
+    std::vector<int64_t> idx(N);
+    std::iota(idx.begin(), idx.end(), (int64_t)0);
+    std::stable_sort(idx.begin(), idx.end(), [&](int64_t a, int64_t b) { return h_dl[a] < h_dl[b]; });
+    std::vector<double2> rA(N), rB(N), rC(N);
+    for (size_t j = 0; j < N; ++j) {
+        const size_t o = (size_t)idx[j];
+        double q = h_m2[o] / h_m1[o];
+        rA[j] = make_double2((std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0, h_m1[o]);
+        rB[j] = make_double2(q, std::log(h_m1[o]));
+        rC[j] = make_double2(std::log(q), std::exp(-h_lp[o] - sh));
+    }
+    cudaStreamSynchronize(ctx->stream);
+    free_pool(ctx->owned_inj);
+    free_pool(ctx->owned_work);
+    ctx->work_nl = 0;
+    ctx->have_inj = false;
+    InjSetDev I{};
+    I.n_det = n_det;
+    I.n_inj_total = (double)n_inj_total;
+    CK(upload(ctx->owned_inj, &I.recA, rA)); CK(upload(ctx->owned_inj, &I.recB, rB)); CK(upload(ctx->owned_inj, &I.recC, rC));
+    CK(upload(ctx->owned_inj, &I.perm, idx));
+    ctx->inj = I;
+    ctx->inj_grid = grid;
+    ctx->inj_ln_shift = sh;
+    ctx->inj_blocks = (int)((n_det + kInjChunk - 1) / kInjChunk);
+    ctx->have_inj = true;
+    return CHIM_OK;
+}
+
+int chim_loglike_batch(chim_ctx* ctx, int32_t n_lambda, const double* lambda, double* out_loglike, double* out_event_logI,
+                       double* out_logxi, double* out_neff, uint32_t* out_flags) {
+    if (!ctx) return CHIM_EINVAL;
+    if (!ctx->have_events) return fail(ctx, CHIM_ESTATE, "chim_loglike_batch: call chim_init_events first");
+    if (n_lambda < 0 || (n_lambda > 0 && (!lambda || !out_loglike)))
+        return fail(ctx, CHIM_EINVAL, "chim_loglike_batch: null lambda/out_loglike or n_lambda < 0");
+    if (n_lambda == 0) return CHIM_OK;
+    CK(cudaSetDevice(ctx->cfg.device));
+    const int chunk = std::min<int>(ctx->cfg.lambda_chunk, n_lambda);
+    int rc = ensure_work(ctx, chunk);
+    if (rc != CHIM_OK) return rc;
+    ctx->launches = 0;
+    CK(cudaMemsetAsync(ctx->stats, 0, 4 * sizeof(unsigned long long), ctx->stream));
+    for (int c0 = 0; c0 < n_lambda; c0 += chunk) {
+        const int nl = std::min(chunk, n_lambda - c0);
+        rc = run_chunk(ctx, nl, lambda + (size_t)c0 * CHIM_N_LAMBDA_PARAMS, out_loglike + c0,
+                       out_event_logI ? out_event_logI + (size_t)c0 * ctx->ev.n_events : nullptr,
+                       out_logxi ? out_logxi + c0 : nullptr, out_neff ? out_neff + c0 : nullptr,
+                       out_flags ? out_flags + c0 : nullptr);
+        if (rc != CHIM_OK) return rc;
+    }
+    ctx->last.kde_pairs_dense = 0;
+    for (int i = 0; i < ctx->ev.n_events; ++i)
+        ctx->last.kde_pairs_dense += (uint64_t)(ctx->h_sample_off[i + 1] - ctx->h_sample_off[i]) *
+                                     (uint64_t)(ctx->h_grid_off[i + 1] - ctx->h_grid_off[i]);
+    ctx->last.kde_pairs_dense *= (uint64_t)n_lambda;
+    ctx->last.sample_evals = (uint64_t)ctx->h_sample_off[ctx->ev.n_events] * (uint64_t)n_lambda;
+    ctx->last.injection_evals = ctx->have_inj ? (uint64_t)ctx->inj.n_det * (uint64_t)n_lambda : 0;
+    ctx->last.kernel_launches = ctx->launches;
+    return CHIM_OK;
+}
+
+int chim_loglike_batch_host(chim_ctx* ctx, int32_t n_lambda, const double* lambda, double* out_loglike,
+                            double* out_event_logI, double* out_logxi, double* out_neff, uint32_t* out_flags) {
+    if (!ctx) return CHIM_EINVAL;
+    if (!ctx->have_events) return fail(ctx, CHIM_ESTATE, "chim_loglike_batch_host: call chim_init_events first");
+    if (n_lambda < 0 || (n_lambda > 0 && (!lambda || !out_loglike)))
+        return fail(ctx, CHIM_EINVAL, "chim_loglike_batch_host: null lambda/out_loglike or n_lambda < 0");
+    if (n_lambda == 0) return CHIM_OK;
+    CK(cudaSetDevice(ctx->cfg.device));
+    if (n_lambda > ctx->host_nl) {
+        cudaStreamSynchronize(ctx->stream);
+        free_pool(ctx->owned_host);
+        ctx->host_nl = 0;
+        CK(dev_alloc(ctx->owned_host, &ctx->st_lam, (size_t)n_lambda * CHIM_N_LAMBDA_PARAMS));
+        CK(dev_alloc(ctx->owned_host, &ctx->st_ll, n_lambda));
+        CK(dev_alloc(ctx->owned_host, &ctx->st_ev, (size_t)n_lambda * ctx->ev.n_events));
+        CK(dev_alloc(ctx->owned_host, &ctx->st_xi, n_lambda));
+        CK(dev_alloc(ctx->owned_host, &ctx->st_neff, n_lambda));
+        CK(dev_alloc(ctx->owned_host, &ctx->st_fl, n_lambda));
+        ctx->host_nl = n_lambda;
+    }
+    cudaStream_t st = ctx->stream;
+    CK(cudaMemcpyAsync(ctx->st_lam, lambda, sizeof(double) * n_lambda * CHIM_N_LAMBDA_PARAMS, cudaMemcpyHostToDevice, st));
+    int rc = chim_loglike_batch(ctx, n_lambda, ctx->st_lam, ctx->st_ll, out_event_logI ? ctx->st_ev : nullptr,
+                                out_logxi ? ctx->st_xi : nullptr, out_neff ? ctx->st_neff : nullptr,
+                                out_flags ? ctx->st_fl : nullptr);
+    if (rc != CHIM_OK) return rc;
+    CK(cudaMemcpyAsync(out_loglike, ctx->st_ll, sizeof(double) * n_lambda, cudaMemcpyDeviceToHost, st));
+    if (out_event_logI)
+        CK(cudaMemcpyAsync(out_event_logI, ctx->st_ev, sizeof(double) * n_lambda * ctx->ev.n_events, cudaMemcpyDeviceToHost, st));
+    if (out_logxi) CK(cudaMemcpyAsync(out_logxi, ctx->st_xi, sizeof(double) * n_lambda, cudaMemcpyDeviceToHost, st));
+    if (out_neff) CK(cudaMemcpyAsync(out_neff, ctx->st_neff, sizeof(double) * n_lambda, cudaMemcpyDeviceToHost, st));
+    if (out_flags) CK(cudaMemcpyAsync(out_flags, ctx->st_fl, sizeof(uint32_t) * n_lambda, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return CHIM_OK;
+}
+
+int chim_get_stats(chim_ctx* ctx, chim_stats* out) {
+    if (!ctx || !out) return CHIM_EINVAL;
+    if (!ctx->stats) return fail(ctx, CHIM_ESTATE, "chim_get_stats: no batch has run");
+    CK(cudaSetDevice(ctx->cfg.device));
+    CK(cudaStreamSynchronize(ctx->stream));
+    unsigned long long s[4];
+    CK(cudaMemcpy(s, ctx->stats, sizeof s, cudaMemcpyDeviceToHost));
+    ctx->last.kde_pairs_evaluated = s[0];
+    *out = ctx->last;
+    return CHIM_OK;
+}
+
+// ---- diagnostics --------------------------------------------------------------------------------------
+static int debug_prepare(chim_ctx* ctx, const double* lambda, const char* who) {
+    if (!ctx) return CHIM_EINVAL;
+    if (!ctx->have_events) return fail(ctx, CHIM_ESTATE, std::string(who) + ": call chim_init_events first");
+    if (!lambda) return fail(ctx, CHIM_EINVAL, std::string(who) + ": null lambda");
+    CK(cudaSetDevice(ctx->cfg.device));
+    int rc = ensure_work(ctx, 1);
+    if (rc != CHIM_OK) return rc;
+    TableParams TP = table_params(ctx);
+    CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t), ctx->stream));
+    CK(launch_tables(lambda, 1, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->wtab, ctx->stream));
+    return CHIM_OK;
+}
+
+int chim_debug_table_lookup(chim_ctx* ctx, const double* lambda, int64_t n, const double* dL, double* z_out, double* ratio_out) {
+    int rc = debug_prepare(ctx, lambda, "chim_debug_table_lookup");
+    if (rc != CHIM_OK) return rc;
+    if (n < 0 || (n > 0 && !dL)) return fail(ctx, CHIM_EINVAL, "chim_debug_table_lookup: bad arguments");
+    CK(launch_table_lookup(ctx->Lc, ctx->tab_ev, ctx->ev_grid, n, dL, ctx->cfg.z_table_max, z_out, ratio_out, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return CHIM_OK;
+}
+
+static int debug_event(chim_ctx* ctx, const double* lambda, int32_t event, double* z_out, double* w_out, double* h_out,
+                       double* K_out, double* logI_out, const char* who) {
+    int rc = debug_prepare(ctx, lambda, who);
+    if (rc != CHIM_OK) return rc;
+    if (event < 0 || event >= ctx->ev.n_events) return fail(ctx, CHIM_EINVAL, std::string(who) + ": event out of range");
+    if ((z_out == nullptr) != (w_out == nullptr)) return fail(ctx, CHIM_EINVAL, std::string(who) + ": z_out and w_out go together");
+    EventKernelParams EP = event_params(ctx, 1);
+    EP.dbg_event = event;
+    EP.dbg_z = z_out; EP.dbg_w = w_out; EP.dbg_h = h_out; EP.dbg_K = K_out;
+    CK(launch_events(EP, ctx->stream));
+    if (logI_out) CK(cudaMemcpyAsync(logI_out, ctx->logI, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return CHIM_OK;
+}
+
+int chim_debug_event_samples(chim_ctx* ctx, const double* lambda, int32_t event, double* z_out, double* w_out) {
+    if (!z_out || !w_out) return fail(ctx, CHIM_EINVAL, "chim_debug_event_samples: null output");
+    return debug_event(ctx, lambda, event, z_out, w_out, nullptr, nullptr, nullptr, "chim_debug_event_samples");
+}
+
+int chim_debug_event_kde(chim_ctx* ctx, const double* lambda, int32_t event, double* h_out, double* K_out, double* logI_out) {
+    return debug_event(ctx, lambda, event, nullptr, nullptr, h_out, K_out, logI_out, "chim_debug_event_kde");
+}
+
+int chim_debug_injection_weights(chim_ctx* ctx, const double* lambda, double* s_out) {
+    int rc = debug_prepare(ctx, lambda, "chim_debug_injection_weights");
+    if (rc != CHIM_OK) return rc;
+    if (!ctx->have_inj) return fail(ctx, CHIM_ESTATE, "chim_debug_injection_weights: no injections loaded");
+    if (!s_out) return fail(ctx, CHIM_EINVAL, "chim_debug_injection_weights: null output");
+    InjKernelParams IP{};
+    IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.wtab = ctx->wtab;
+    IP.n_lambda = 1; IP.tab_rows = ctx->inj_grid.rows(); IP.n_win = ctx->cfg.n_win_table; IP.chunk = kInjChunk;
+    IP.z_table_max = ctx->cfg.z_table_max; IP.z_cat_max = ctx->cfg.z_cat_max;
+    IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = s_out;
+    IP.dbg_scale = std::exp(ctx->inj_ln_shift);
+    CK(launch_inject(IP, ctx->inj_blocks, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return CHIM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,407 @@
+// k_tables.cu -- step S1: per-lambda table builder (one CTA per lambda).
+//
+//   d_C(z) = (c/H0) int_0^z dz'/E(z'),  E = sqrt(Om (1+z)^3 + 1 - Om)      (eq. 1, R4)
+//       cumulative trapezoid of 1/E on a uniform z grid + the Euler-Maclaurin end term
+//       (f'_k - f'_{k+1}) dz^2/12 per panel (f' analytic), block-wide prefix sum in fp64;
+//   d_L^gw(z) = Xi(z) (1+z) d_C(z),  Xi = Xi0 + (1-Xi0)/(1+z)^n               (eq. 2)
+//       with the monotonicity check of R16 at the table nodes;
+//   z(ln d_L) tables: for each node of a uniform grid in x = ln d_L the redshift is found by bisection
+//       over the d_L^gw nodes and Newton on the cubic-Hermite d_C (node slopes c/H exact); the nodes of
+//       z, ln(1+z), 1/(1+z) and the smooth weight factor psi/J (PAPER.md:226 eq. 21, :75 eq. 11) are turned
+//       into per-interval cubic coefficients so that the sample kernels do one Horner evaluation per
+//       column (the sample's table coordinate is lambda-independent and precomputed at init);
+//   mass-function constants: N_pl, Z1 (32-node Gauss-Legendre on the smoothing window + closed-form
+//       tails), and the window table rho = W/(S m'^2), W(m) = int_{m_low}^m m'^beta S(m') dm' (M1-M4).
+#include "chim_internal.cuh"
+
+namespace chim {
+
+__constant__ double c_glw_x[kGLWin], c_glw_w[kGLWin];      // GL nodes/weights on [-1,1]
+__constant__ double c_glp_x[kGLPanel], c_glp_w[kGLPanel];
+
+// Host: Gauss-Legendre rule by Newton iteration on the three-term recurrence, symmetric fill.
+static void gauss_legendre_host(int n, double* x, double* w) {
+    const double pi = 3.14159265358979323846;
+    for (int i = 0; i < (n + 1) / 2; ++i) {
+        double t = cos(pi * (4 * i + 3) / (4.0 * n + 2.0));
+        double pn = 0.0, dpn = 1.0;
+        for (int it = 0; it < 64; ++it) {
+            double pkm1 = 1.0, pk = t;
+            for (int k = 1; k < n; ++k) {
+                double pkp1 = ((2 * k + 1) * t * pk - k * pkm1) / (k + 1);
+                pkm1 = pk;
+                pk = pkp1;
+            }
+            pn = pk;
+            dpn = n * (pkm1 - t * pk) / (1.0 - t * t);
+            double dt = pn / dpn;
+            t -= dt;
+            if (fabs(dt) < 1e-16) break;
+        }
+        // re-evaluate the derivative at the converged root
+        double pkm1 = 1.0, pk = t;
+        for (int k = 1; k < n; ++k) {
+            double pkp1 = ((2 * k + 1) * t * pk - k * pkm1) / (k + 1);
+            pkm1 = pk;
+            pk = pkp1;
+        }
+        dpn = n * (pkm1 - t * pk) / (1.0 - t * t);
+        x[i] = -t;
+        x[n - 1 - i] = t;
+        w[i] = w[n - 1 - i] = 2.0 / ((1.0 - t * t) * dpn * dpn);
+    }
+}
+
+cudaError_t upload_gauss_legendre() {
+    double x[kGLWin], w[kGLWin];
+    gauss_legendre_host(kGLWin, x, w);
+    cudaError_t e = cudaMemcpyToSymbol(c_glw_x, x, sizeof(double) * kGLWin);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyToSymbol(c_glw_w, w, sizeof(double) * kGLWin);
+    if (e != cudaSuccess) return e;
+    gauss_legendre_host(kGLPanel, x, w);
+    e = cudaMemcpyToSymbol(c_glp_x, x, sizeof(double) * kGLPanel);
+    if (e != cudaSuccess) return e;
+    return cudaMemcpyToSymbol(c_glp_w, w, sizeof(double) * kGLPanel);
+}
+
+constexpr int kTabThreads = 256;
+
+struct TabSmem {
+    LamConst L;
+    double red[4 * (kTabThreads / 32)];
+    double scan[kTabThreads];
+    int ibad;
+};
+
+__device__ __forceinline__ double invE(double z, double Om) {
+    double a = 1.0 + z;
+    return rsqrt(Om * a * a * a + 1.0 - Om);
+}
+// d(1/E)/dz = -3 Om (1+z)^2 / (2 E^3)
+__device__ __forceinline__ double dinvE(double z, double Om) {
+    double a = 1.0 + z;
+    double ie = rsqrt(Om * a * a * a + 1.0 - Om);
+    return -1.5 * Om * a * a * ie * ie * ie;
+}
+__device__ __forceinline__ double Xi_of(double z, const LamConst& L) { return L.Xi0 + (1.0 - L.Xi0) * exp(-L.n * log1p(z)); }
+__device__ __forceinline__ double dXi_of(double z, const LamConst& L) {
+    return -L.n * (1.0 - L.Xi0) * exp(-(L.n + 1.0) * log1p(z));
+}
+// Madau-Dickinson rate, eq. (21) with constant 1 (R5), from u = ln(1+z)
+__device__ __forceinline__ double psi_of_u(double u, const LamConst& L) {
+    return exp(L.gamma * u) / (1.0 + exp(L.gk * (u - L.ln1pzp)));
+}
+__device__ __forceinline__ double smooth_S_dev(double m, const LamConst& L) {
+    if (m <= L.m_low) return 0.0;
+    if (m >= L.m_c) return 1.0;
+    double mp = m - L.m_low;
+    double f = L.delta / mp + L.delta / (mp - L.delta);
+    return 1.0 / (1.0 + exp(f));
+}
+__device__ __forceinline__ double powerlaw_unnorm(double m, const LamConst& L) {
+    return (m >= L.m_low && m <= L.m_high) ? exp(-L.alpha * log(m)) : 0.0;
+}
+__device__ __forceinline__ double gauss_dev(double m, const LamConst& L) {
+    double d = (m - L.mu) / L.sigma;
+    return exp(-0.5 * d * d) / (L.sigma * 2.50662827463100050242);
+}
+
+// Inclusive block scan over `n` values in `a` (shared), in place; P = ceil(n / NT) consecutive values per thread.
+__device__ void block_inclusive_scan(double* a, int n, double* scan_scratch) {
+    int tid = threadIdx.x;
+    int P = (n + kTabThreads - 1) / kTabThreads;
+    int lo = tid * P, hi = min(lo + P, n);
+    double run = 0.0;
+    for (int i = lo; i < hi; ++i) {
+        run += a[i];
+        a[i] = run;
+    }
+    scan_scratch[tid] = run;
+    __syncthreads();
+    // serial exclusive scan of the 256 thread totals by one warp-friendly loop (fp64, tiny)
+    if (tid == 0) {
+        double acc = 0.0;
+        for (int t = 0; t < kTabThreads; ++t) {
+            double v = scan_scratch[t];
+            scan_scratch[t] = acc;
+            acc += v;
+        }
+    }
+    __syncthreads();
+    double off = scan_scratch[tid];
+    for (int i = lo; i < hi; ++i) a[i] += off;
+    __syncthreads();
+}
+
+// d_C at arbitrary z from the shared table (cubic Hermite, node slopes (c/H0)/E exact)
+__device__ __forceinline__ double dc_hermite(const double* s_dc, double dz, int nz_nodes, double z, const LamConst& L) {
+    double x = z / dz;
+    int i = (int)x;
+    i = max(0, min(i, nz_nodes - 2));
+    double t = x - (double)i;
+    double f0 = L.c_H0 * invE(i * dz, L.Om) * dz, f1 = L.c_H0 * invE((i + 1) * dz, L.Om) * dz;
+    double t2 = t * t, omt = 1.0 - t;
+    return (1.0 + 2.0 * t) * omt * omt * s_dc[i] + t2 * (3.0 - 2.0 * t) * s_dc[i + 1] + t * omt * omt * f0 - t2 * omt * f1;
+}
+
+// Build one ln d_L table (nodes in s_nodes[4][K+3], rows to global).
+__device__ void build_dl_table(const DlGrid g, bool is_inj, int placement, const TabSmem& S, const double* s_dc,
+                               const double* s_dl, double dz, int nz_nodes, double* s_nodes, Row* __restrict__ rows) {
+    const LamConst& L = S.L;
+    int NN = g.K + 3;
+    for (int idx = threadIdx.x; idx < NN; idx += kTabThreads) {
+        double target = exp(g.x0 + (idx - 1) * g.dx);
+        // bisection over the monotone node values s_dl[0..nz_nodes-1]
+        int lo = 0, hi = nz_nodes - 1;
+        double z;
+        if (target >= s_dl[hi]) {
+            // beyond the (padded) table: linear continuation with the end slope; only ever touched by the
+            // stencil of samples within 2 nodes of the table limit
+            double zend = hi * dz, dce = s_dc[hi];
+            double slope = dXi_of(zend, L) * (1.0 + zend) * dce + Xi_of(zend, L) * (dce + (1.0 + zend) * L.c_H0 * invE(zend, L.Om));
+            z = zend + (target - s_dl[hi]) / slope;
+        } else {
+            while (hi - lo > 1) {
+                int mid = (lo + hi) >> 1;
+                if (s_dl[mid] <= target) lo = mid; else hi = mid;
+            }
+            double zl = lo * dz, zh = zl + dz;
+            z = zl + dz * (target - s_dl[lo]) / (s_dl[lo + 1] - s_dl[lo]);
+            for (int it = 0; it < 8; ++it) {
+                double dc = dc_hermite(s_dc, dz, nz_nodes, z, L);
+                double xi = Xi_of(z, L);
+                double gval = xi * (1.0 + z) * dc - target;
+                double gder = dXi_of(z, L) * (1.0 + z) * dc + xi * (dc + (1.0 + z) * L.c_H0 * invE(z, L.Om));
+                double step = gval / gder;
+                z -= step;
+                z = fmin(fmax(z, zl), zh);
+                if (fabs(step) < 1e-15 * (1.0 + z)) break;
+            }
+        }
+        double u = log1p(z), a1 = 1.0 + z;
+        double R = 1.0;
+        if (is_inj || placement == CHIM_ON_SAMPLES) {
+            double dc = (z <= (nz_nodes - 1) * dz) ? dc_hermite(s_dc, dz, nz_nodes, z, L)
+                                                  : s_dc[nz_nodes - 1] + (z - (nz_nodes - 1) * dz) * L.c_H0 * invE(z, L.Om);
+            double fE = L.c_H0 * invE(z, L.Om);
+            double ddl = dXi_of(z, L) * a1 * dc + Xi_of(z, L) * (dc + a1 * fE);
+            double J = a1 * a1 * a1 * fabs(ddl);                      // eq. (11)
+            R = psi_of_u(u, L) / J;
+            if (is_inj) R *= dc * dc * fE * L.vol_norm;               // u(z) of R6
+        }
+        s_nodes[0 * NN + idx] = z;
+        s_nodes[1 * NN + idx] = u;
+        s_nodes[2 * NN + idx] = 1.0 / a1;
+        s_nodes[3 * NN + idx] = R;
+    }
+    __syncthreads();
+    // cubic through nodes k-1..k+2 expanded in t = tk - k
+    for (int k = threadIdx.x; k < g.K + 2; k += kTabThreads) {
+        Row r;
+        int i0 = max(k - 1, 0), i3 = min(k + 2, NN - 1), i2 = min(k + 1, NN - 1);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            double f0 = s_nodes[c * NN + i0], f1 = s_nodes[c * NN + k], f2 = s_nodes[c * NN + i2], f3 = s_nodes[c * NN + i3];
+            r.c[c][0] = f1;
+            r.c[c][1] = -f0 / 3.0 - 0.5 * f1 + f2 - f3 / 6.0;
+            r.c[c][2] = 0.5 * f0 - f1 + 0.5 * f2;
+            r.c[c][3] = (f3 - f0) / 6.0 + 0.5 * (f1 - f2);
+        }
+        rows[k] = r;
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict__ lam, int n_lambda, TableParams P,
+                                                       LamConst* __restrict__ Lc, double* __restrict__ dc_tab,
+                                                       Row* __restrict__ tab_ev, Row* __restrict__ tab_inj,
+                                                       double* __restrict__ wtab) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TabSmem& S = *reinterpret_cast<TabSmem*>(smem_raw);
+    const int nz_nodes = P.n_table + 1 + kZPad;
+    double* s_dc = reinterpret_cast<double*>(smem_raw + ((sizeof(TabSmem) + 15) / 16) * 16);
+    double* s_dl = s_dc + nz_nodes;
+    double* s_w = s_dl + nz_nodes;                // [n_win + 1]
+    double* s_nodes = s_w + (P.n_win + 1);        // [4][maxK + 3]
+    const int l = blockIdx.x, tid = threadIdx.x;
+    LamConst& L = S.L;
+    const double dz = P.z_table_max / P.n_table;
+
+    if (tid == 0) {
+        const double* p = lam + (size_t)l * CHIM_N_LAMBDA_PARAMS;
+        L.H0 = p[0]; L.Om = p[1]; L.Xi0 = p[2]; L.n = p[3]; L.alpha = p[4]; L.beta = p[5]; L.delta = p[6];
+        L.m_low = p[7]; L.m_high = p[8]; L.mu = p[9]; L.sigma = p[10]; L.lg = p[11]; L.gamma = p[12];
+        L.kappa = p[13]; L.zp = p[14];
+        bool ok = (L.H0 > 0.0) && (L.Om > 0.0 && L.Om <= 1.0) && (L.Xi0 > 0.0) && (L.delta > 0.0) && (L.sigma > 0.0) &&
+                  (L.lg >= 0.0 && L.lg <= 1.0) && (L.m_low > 0.0) && (L.m_high > L.m_low) && (L.zp > -1.0);
+        for (int k = 0; k < CHIM_N_LAMBDA_PARAMS; ++k) ok = ok && isfinite(p[k]);
+        L.flags = ok ? 0u : CHIM_FLAG_LAMBDA_DOMAIN;
+        L.c_H0 = kCkms / L.H0;
+        L.m_c = L.m_low + L.delta;
+        L.inv2s2 = 0.5 / (L.sigma * L.sigma);
+        L.bp1 = L.beta + 1.0;
+        L.beta_is_m1 = fabs(L.bp1) < 1e-12;
+        L.ln_mc = log(L.m_c);
+        L.pow_mc_bp1 = exp(L.bp1 * L.ln_mc);
+        L.gk = L.gamma + L.kappa;
+        L.ln1pzp = log1p(L.zp);
+        L.win_scale = P.n_win / L.delta;
+        S.ibad = 0;
+    }
+    __syncthreads();
+    if (L.flags) {
+        if (tid == 0) Lc[l] = L;
+        return;
+    }
+
+    // ---- d_C table: panel integrals (trapezoid + Euler-Maclaurin end term), prefix sum ----------------
+    for (int i = tid; i < nz_nodes; i += kTabThreads) {
+        if (i == 0) { s_dc[0] = 0.0; continue; }
+        double za = (i - 1) * dz, zb = i * dz;
+        double fa = invE(za, L.Om), fb = invE(zb, L.Om);
+        s_dc[i] = 0.5 * dz * (fa + fb) + dz * dz / 12.0 * (dinvE(za, L.Om) - dinvE(zb, L.Om));
+    }
+    __syncthreads();
+    block_inclusive_scan(s_dc, nz_nodes, S.scan);
+    for (int i = tid; i < nz_nodes; i += kTabThreads) s_dc[i] *= L.c_H0;
+    __syncthreads();
+    // ---- d_L^gw nodes + monotonicity (analytic derivative > 0 at nodes 0..n_table, R16) ---------------
+    int bad = 0;
+    for (int i = tid; i < nz_nodes; i += kTabThreads) {
+        double z = i * dz, dc = s_dc[i], xi = Xi_of(z, L);
+        s_dl[i] = xi * (1.0 + z) * dc;
+        double ddl = dXi_of(z, L) * (1.0 + z) * dc + xi * (dc + (1.0 + z) * L.c_H0 * invE(z, L.Om));
+        if (!(ddl > 0.0) && i <= P.n_table) bad = 1;   // the rule covers nodes 0..n_table only
+    }
+    bad = __syncthreads_or(bad);
+    if (bad) {
+        if (tid == 0) { L.flags |= CHIM_FLAG_DL_NONMONOTONE; Lc[l] = L; }
+        return;
+    }
+    if (dc_tab)
+        for (int i = tid; i < nz_nodes; i += kTabThreads) dc_tab[(size_t)l * nz_nodes + i] = s_dc[i];
+
+    // ---- mass-function normalisation Z1 (M2): 8 panels x 32 GL nodes on the window + closed-form tails -
+    {
+        double npl = (fabs(L.alpha - 1.0) < 1e-12)
+                         ? log(L.m_high / L.m_low)
+                         : (exp((1.0 - L.alpha) * log(L.m_high)) - exp((1.0 - L.alpha) * log(L.m_low))) / (1.0 - L.alpha);
+        bool split = L.m_high < L.m_c;   // power law ends inside the window: integrate the two pieces apart
+        int panel = tid >> 5, node = tid & 31;
+        double a, b;
+        if (split) {
+            double lo = (panel < 4) ? L.m_low : L.m_high, hi = (panel < 4) ? L.m_high : L.m_c;
+            int pp = panel & 3;
+            a = lo + (hi - lo) * pp / 4.0; b = lo + (hi - lo) * (pp + 1) / 4.0;
+        } else {
+            a = L.m_low + L.delta * panel / 8.0; b = L.m_low + L.delta * (panel + 1) / 8.0;
+        }
+        double hw = 0.5 * (b - a), m = 0.5 * (a + b) + hw * c_glw_x[node];
+        double plv = powerlaw_unnorm(m, L);
+        if (split && panel >= 4) plv = 0.0;  // open at m_high from above
+        double v[1] = {hw * c_glw_w[node] * ((1.0 - L.lg) * plv / npl + L.lg * gauss_dev(m, L)) * smooth_S_dev(m, L)};
+        block_sum<kTabThreads, 1>(v, S.red);
+        if (tid == 0) {
+            double z1 = v[0];
+            if (!split) {
+                double tail = (fabs(L.alpha - 1.0) < 1e-12)
+                                  ? log(L.m_high / L.m_c)
+                                  : (exp((1.0 - L.alpha) * log(L.m_high)) - exp((1.0 - L.alpha) * log(L.m_c))) / (1.0 - L.alpha);
+                z1 += (1.0 - L.lg) * tail / npl;
+            }
+            z1 += L.lg * 0.5 * erfc((L.m_c - L.mu) / (L.sigma * 1.41421356237309504880));
+            L.Z1 = z1;
+            L.a_pl = log((1.0 - L.lg) / (npl * z1));
+            L.a_g = log(L.lg / (L.sigma * 2.50662827463100050242 * z1));
+        }
+    }
+    // ---- window table (M4): W(m) = int m'^beta S by GL-8 per panel (the lowest 32 panels, where S varies
+    //      super-exponentially, are split 8x), prefix sum, then rho = W / (S m'^2) at the nodes --------------
+    for (int p = tid; p <= P.n_win; p += kTabThreads) {
+        if (p == 0) { s_w[0] = 0.0; continue; }
+        const int nsub = (p <= 32) ? 8 : 1;
+        double a0 = L.m_low + L.delta * (p - 1) / P.n_win, wdt = L.delta / P.n_win / nsub, acc = 0.0;
+        for (int sub = 0; sub < nsub; ++sub) {
+            double mid = a0 + (sub + 0.5) * wdt;
+#pragma unroll
+            for (int q = 0; q < kGLPanel; ++q) {
+                double m = mid + 0.5 * wdt * c_glp_x[q];
+                acc += c_glp_w[q] * exp(L.beta * log(m)) * smooth_S_dev(m, L);
+            }
+        }
+        s_w[p] = acc * 0.5 * wdt;
+    }
+    __syncthreads();
+    block_inclusive_scan(s_w, P.n_win + 1, S.scan);
+    for (int p = tid; p <= P.n_win; p += kTabThreads) {
+        double mp = L.delta * p / P.n_win, m = L.m_low + mp;
+        double S_m = (p == P.n_win) ? 1.0 : smooth_S_dev(m, L);
+        double rho = (p > 0 && S_m > 1e-280 && s_w[p] > 0.0) ? s_w[p] / (S_m * mp * mp)
+                                                             : exp(L.beta * log(m)) / L.delta;   // m' -> 0 limit
+        wtab[(size_t)l * (P.n_win + 1) + p] = rho;
+    }
+    if (tid == 0) {
+        L.W_c = s_w[P.n_win];
+        double dcc = dc_hermite(s_dc, dz, nz_nodes, P.z_cat_max, L);
+        L.vol_norm = 3.0 / (dcc * dcc * dcc);
+        L.dl_tabmax = s_dl[P.n_table];
+        double lt = log(L.dl_tabmax);
+        L.tkmax_ev = P.ev.K > 0 ? (lt - P.ev.x0) / P.ev.dx + 1.0 : 0.0;
+        L.tkmax_inj = P.inj.K > 0 ? (lt - P.inj.x0) / P.inj.dx + 1.0 : 0.0;
+    }
+    __syncthreads();
+    if (P.ev.K > 0)
+        build_dl_table(P.ev, false, P.placement, S, s_dc, s_dl, dz, nz_nodes, s_nodes, tab_ev + (size_t)l * P.ev.rows());
+    if (P.inj.K > 0)
+        build_dl_table(P.inj, true, P.placement, S, s_dc, s_dl, dz, nz_nodes, s_nodes, tab_inj + (size_t)l * P.inj.rows());
+    if (tid == 0) Lc[l] = L;
+}
+
+size_t tables_smem_bytes(const TableParams& P) {
+    int nz_nodes = P.n_table + 1 + kZPad;
+    int maxK = P.ev.K > P.inj.K ? P.ev.K : P.inj.K;
+    size_t b = ((sizeof(TabSmem) + 15) / 16) * 16;
+    b += sizeof(double) * (2 * (size_t)nz_nodes + (P.n_win + 1) + 4 * (size_t)(maxK + 3));
+    return b;
+}
+
+cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P, LamConst* Lc, double* dc_tab,
+                          Row* tab_ev, Row* tab_inj, double* wtab, cudaStream_t st) {
+    size_t smem = tables_smem_bytes(P);
+    cudaError_t e = cudaFuncSetAttribute(k_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_tables<<<n_lambda, kTabThreads, smem, st>>>(lam, n_lambda, P, Lc, dc_tab, tab_ev, tab_inj, wtab);
+    return cudaGetLastError();
+}
+
+// Diagnostics: evaluate the event table at arbitrary d_L (single lambda).
+__global__ void k_table_lookup(const LamConst* __restrict__ Lc, const Row* __restrict__ tab, DlGrid g, int64_t n,
+                               const double* __restrict__ dL, double z_table_max, double* __restrict__ z_out,
+                               double* __restrict__ r_out) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const LamConst& L = Lc[0];
+    double z = NAN, r = NAN;
+    if (L.flags == 0) {
+        double tk = (log(dL[i]) - g.x0) / g.dx + 1.0;
+        if (tk > L.tkmax_ev) { z = z_table_max; r = 0.0; }
+        else if (tk >= 1.0 && tk < g.K + 1.0) {
+            int k = (int)tk;
+            double t = tk - k;
+            z = horner3(tab[k].c[0], t);
+            r = horner3(tab[k].c[3], t);
+        }
+    }
+    if (z_out) z_out[i] = z;
+    if (r_out) r_out[i] = r;
+}
+
+cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, int64_t n, const double* dL,
+                                double z_table_max, double* z_out, double* r_out, cudaStream_t st) {
+    if (n <= 0) return cudaSuccess;
+    k_table_lookup<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(Lc, tab, g, n, dL, z_table_max, z_out, r_out);
+    return cudaGetLastError();
+}
+
+}  // namespace chim

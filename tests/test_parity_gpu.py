@@ -1,0 +1,318 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on the same
+seeded inputs.  Tolerances are north_star's: per-event log I relative 1e-4, total log L absolute 1e-3."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle as O
+from workloads import lambda_vector, make_workload
+
+pytestmark = pytest.mark.gpu
+
+REL_EVENT = 1e-4     # north_star: per-event log-likelihoods to a relative 1e-4
+ABS_TOTAL = 1e-3     # north_star: total log-likelihood to an absolute 1e-3
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2504_02034_b200 as pkg
+    pkg.lib()                      # fails loudly if libchim.so is missing
+    return pkg
+
+
+def _ctx(P, w, **kw):
+    kw.setdefault("z_cat_max", w.z_cat_max)
+    c = P.Context(**kw)
+    c.init_workload(w, fixed_bw=kw.get("_fixed"))
+    return c
+
+
+def _gpu(P, w, lam=None, fixed_bw=None, **kw):
+    import torch
+    kw.setdefault("z_cat_max", w.z_cat_max)
+    c = P.Context(**kw)
+    c.init_workload(w, fixed_bw=fixed_bw)
+    lam = w.lam if lam is None else np.atleast_2d(lam)
+    out = c.loglike_batch(torch.as_tensor(lam, device=c.device).contiguous())
+    torch.cuda.synchronize()
+    r = {k: v.cpu().numpy() for k, v in out.items()}
+    r["flags"] = r["flags"].astype(np.uint32)
+    r["stats"] = c.stats()
+    c.close()
+    return r
+
+
+def _compare(r, ref, n_events):
+    a, b = r["event_logI"], ref["event_logI"]
+    fin = np.isfinite(b)
+    assert np.array_equal(np.isfinite(a), fin)
+    assert np.array_equal(np.isnan(a), np.isnan(b))
+    rel = np.max(np.abs(a[fin] - b[fin]) / np.abs(b[fin])) if fin.any() else 0.0
+    ok = np.isfinite(ref["loglike"])
+    dtot = np.max(np.abs(r["loglike"][ok] - ref["loglike"][ok])) if ok.any() else 0.0
+    dxi = np.nanmax(np.abs(r["logxi"] - ref["logxi"])) if np.isfinite(ref["logxi"]).any() else 0.0
+    return rel, dtot, dxi
+
+
+# ---------------------------------------------------------------- T2: intermediates, step by step
+def test_s1_table_inversion_and_ratio(P):
+    w = make_workload("tiny")
+    c = _ctx(P, w)
+    rng = np.random.default_rng(0)
+    for la in (w.lam[0], lambda_vector(H0=80, Om=0.4, Xi0=0.5, n=3.0), lambda_vector(H0=60, Om=0.2, Xi0=2.0, n=0.5)):
+        dl = np.exp(rng.uniform(np.log(w.dL.min()), np.log(w.dL.max()), 4000))
+        z, r = c.debug_table_lookup(la, dl)
+        zr = O.z_of_dl(la, dl)
+        assert np.max(np.abs(z - zr)) < 1e-10          # budget: systematic dz must stay < 1e-7
+        d = O.distances(la, zr)
+        ratio = O.psi(la, zr) / ((1 + zr) ** 3 * np.abs(d["ddl_gw_dz"]))
+        assert np.max(np.abs(r / ratio - 1)) < 1e-9
+    c.close()
+
+
+@pytest.mark.parametrize("lam_kw", [dict(), dict(H0=78, Om=0.22, Xi0=1.7, n=2.6, alpha=3.1, beta=1.2, delta_m=5.2, m_low=4.7,
+                                               m_high=80, mu_g=31, sigma_g=3.9, lambda_g=0.042, gamma=2.5, kappa=3.2, z_p=2.1)])
+def test_s2_sample_redshifts_and_weights(P, lam_kw):
+    w = make_workload("tiny")
+    la = lambda_vector(**lam_kw)
+    c = _ctx(P, w)
+    for ev in (0, 3, 7):
+        s = slice(w.sample_off[ev], w.sample_off[ev + 1])
+        z, wt = c.debug_event_samples(la, ev)
+        zr, wr, _ = O.sample_weights(la, w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s])
+        assert np.max(np.abs(z - zr)) < 1e-10
+        mism = (wt == 0) != (wr == 0)
+        assert np.all(np.maximum(wt, wr)[mism] < 1e-12 * wr.max())
+        # relative to the largest weight (tiny weights deep in the smoothing window carry no mass)
+        assert np.max(np.abs(wt - wr)) < 1e-9 * wr.max()
+        big = wr > 1e-6 * wr.max()
+        assert np.max(np.abs(wt[big] / wr[big] - 1)) < 1e-7
+    c.close()
+
+
+def test_s3_bandwidth_and_kde_on_grid(P):
+    w = make_workload("tiny")
+    la = w.lam[0]
+    c = _ctx(P, w, kde_cutoff=0.0)                      # no cut-off: K must match the full sum everywhere
+    for ev in (1, 4):
+        s = slice(w.sample_off[ev], w.sample_off[ev + 1])
+        g = slice(w.grid_off[ev], w.grid_off[ev + 1])
+        h, K, logI = c.debug_event_kde(la, ev)
+        zr, wr, _ = O.sample_weights(la, w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s])
+        hr = O.scott_bw(zr, wr)
+        assert abs(h / hr - 1) < 1e-9
+        Kr = O.kde(zr, wr, hr, w.z_grid[g])
+        assert np.max(np.abs(K - Kr)) < 2e-6 * Kr.max()    # fp32 pair loop
+        Ir = O.event_integral(la, w.z_grid[g], Kr, w.p_gal[g])
+        assert abs(logI - math.log(Ir)) < 1e-6
+    c.close()
+
+
+def test_s5_injection_weights(P):
+    w = make_workload("tiny")
+    c = _ctx(P, w)
+    for la in (w.lam[0], lambda_vector(H0=64, Om=0.35, Xi0=0.7, n=1.2, m_low=5.5, delta_m=4.4)):
+        s = c.debug_injection_weights(la)
+        s1, s2, sr = O.selection_sums(la, w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw, z_cat_max=w.z_cat_max, return_s=True)
+        mism = (s == 0) != (sr == 0)      # underflow deep in the smoothing window may differ: must carry no mass
+        assert np.all(np.maximum(s, sr)[mism] < 1e-12 * sr.max())
+        assert np.max(np.abs(s - sr)) < 1e-9 * sr.max()
+        assert abs(s.sum() / s1 - 1) < 1e-9
+    c.close()
+
+
+# ---------------------------------------------------------------- T3: end to end
+def test_tiny_end_to_end(P):
+    w = make_workload("tiny")
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w)
+    rel, dtot, dxi = _compare(r, ref, w.n_events)
+    print(f"tiny: rel(logI)={rel:.2e} |dlogL|={dtot:.2e} |dlogxi|={dxi:.2e}")
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    assert abs(r["neff"][0] / ref["neff"][0] - 1) < 1e-8
+    assert np.array_equal(r["flags"], ref["flags"])
+
+
+@pytest.mark.parametrize("placement", [0, 1])
+@pytest.mark.parametrize("fixed", [False, True])
+def test_tiny_modes(P, placement, fixed):
+    w = make_workload("tiny", n_lambda=4)
+    fb = np.full(w.n_events, 0.012) if fixed else None
+    bw = O.BW_FIXED if fixed else O.BW_SCOTT
+    ref = O.loglike_workload(w, placement=placement, bw_rule=bw, fixed_bw=fb)
+    r = _gpu(P, w, fixed_bw=fb, placement=placement, bw_rule=bw)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+
+
+def test_o5_shaped_ragged_multi_tile(P):
+    # O5-spectroscopic shape scaled to what the oracle finishes in seconds; ragged N_s and N_z (tails that are
+    # not multiples of 32 / 256), several lambda chunks, lambdas spread over the whole box
+    w = make_workload("o5_spec", n_events=12, n_lambda=40, n_det=20_000)
+    rng = np.random.default_rng(3)
+    ns = rng.integers(900, 5000, w.n_events)
+    ns[0], ns[1] = 5000, 257
+    nz = rng.integers(300, 1000, w.n_events)
+    nz[0], nz[1] = 1000, 33
+    so = np.concatenate(([0], np.cumsum(ns)))
+    go = np.concatenate(([0], np.cumsum(nz)))
+    sel = np.concatenate([np.arange(w.sample_off[i], w.sample_off[i] + ns[i]) for i in range(w.n_events)])
+    # thin each grid but keep its full extent
+    gsel = np.concatenate([w.grid_off[i] + np.round(np.linspace(0, 999, nz[i])).astype(int) for i in range(w.n_events)])
+    w.dL, w.m1d, w.m2d, w.ln_prior = w.dL[sel], w.m1d[sel], w.m2d[sel], w.ln_prior[sel]
+    w.z_grid, w.p_gal = w.z_grid[gsel], w.p_gal[gsel]
+    w.sample_off, w.grid_off = so, go
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w, lambda_chunk=16)
+    rel, dtot, dxi = _compare(r, ref, w.n_events)
+    print(f"o5-shaped: rel(logI)={rel:.2e} |dlogL|={dtot:.2e} |dlogxi|={dxi:.2e} pairs={r['stats']}")
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    assert np.max(np.abs(r["neff"] / ref["neff"] - 1)) < 1e-7
+    assert r["stats"]["kde_pairs_evaluated"] < r["stats"]["kde_pairs_dense"]
+
+
+def test_three_catalogs_small(P):
+    for cat in (0, 1, 2):
+        w = make_workload("o5_spec", catalog=cat, n_events=6, n_samples=2000, n_lambda=8, n_det=5000)
+        ref = O.loglike_workload(w)
+        r = _gpu(P, w)
+        rel, dtot, _ = _compare(r, ref, w.n_events)
+        assert rel < REL_EVENT and dtot < ABS_TOTAL
+
+
+def test_events_deep_in_the_smoothing_window(P):
+    # every sample of the event sits in the lower part of [m_low, m_low + delta_m], where S and C(m1) both vanish
+    # faster than any power: the weights are tiny but their ratios decide log I (n_eff can drop to ~1)
+    w = make_workload("tiny", n_events=4, n_samples=600, n_grid=120, n_inj_draw=2000)
+    la = w.lam[0]
+    zt = w.z_true
+    for i, frac in enumerate((0.04, 0.08, 0.15, 0.3)):
+        s = slice(w.sample_off[i], w.sample_off[i + 1])
+        m1 = (la[7] + frac * la[6]) * (1 + zt[i])
+        rng = np.random.default_rng(i)
+        a = m1 * (1 + 0.02 * rng.standard_normal(600))
+        b = a * (1 - 0.03 * rng.random(600))
+        w.m1d[s], w.m2d[s] = a, b
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w)
+    assert np.all(np.isfinite(ref["event_logI"]))
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    print(f"deep window: logI={ref['event_logI'][0]} rel={rel:.2e} dtot={dtot:.2e}")
+    assert rel < 1e-6 and dtot < ABS_TOTAL
+
+
+def test_host_entry_point_matches_device_entry_point(P):
+    w = make_workload("tiny", n_lambda=5)
+    c = _ctx(P, w)
+    import torch
+    out = c.loglike_batch(torch.as_tensor(w.lam, device=c.device).contiguous())
+    torch.cuda.synchronize()
+    h = c.loglike_batch_host(np.ascontiguousarray(w.lam), event_logI=True)
+    assert np.array_equal(out["loglike"].cpu().numpy(), h["loglike"])
+    assert np.array_equal(out["event_logI"].cpu().numpy(), h["event_logI"])
+    c.close()
+
+
+# ---------------------------------------------------------------- degenerate cases and flags
+def test_flags_and_degenerate(P):
+    w = make_workload("tiny", n_events=3, n_samples=64, n_grid=70, n_inj_draw=500)
+    lam = np.stack([w.lam[0]] * 4)
+    lam[1, 1] = 1.5                     # Om out of domain
+    lam[2, 2], lam[2, 3] = 0.01, 8.0    # non-monotone d_L^gw
+    lam[3, 7] = 1e3                     # m_low above every mass... m_high <= m_low -> domain
+    w.m2d[:64] = 1.0                    # event 0 all below m_low -> I = 0
+    ref = O.loglike_workload(w, lam=lam)
+    r = _gpu(P, w, lam=lam)
+    assert np.array_equal(r["flags"], ref["flags"]), (r["flags"], ref["flags"])
+    assert r["flags"][0] & P.CHIM_FLAG_EVENT_ZERO and r["loglike"][0] == -np.inf and r["event_logI"][0, 0] == -np.inf
+    assert r["flags"][1] & P.CHIM_FLAG_LAMBDA_DOMAIN and np.isnan(r["loglike"][1])
+    assert r["flags"][2] & P.CHIM_FLAG_DL_NONMONOTONE and np.isnan(r["loglike"][2])
+    assert np.isnan(r["loglike"][3])
+    fin = np.isfinite(ref["event_logI"])
+    assert np.allclose(r["event_logI"][fin], ref["event_logI"][fin], rtol=REL_EVENT)
+
+
+def test_single_sample_event_fixed_bw_and_scott_degenerate(P):
+    w = make_workload("tiny", n_events=2, n_samples=1, n_grid=64, n_inj_draw=300)
+    fb = np.array([0.02, 0.03])
+    ref = O.loglike_workload(w, bw_rule=O.BW_FIXED, fixed_bw=fb)
+    r = _gpu(P, w, fixed_bw=fb, bw_rule=O.BW_FIXED)
+    rel, dtot, _ = _compare(r, ref, 2)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    ref = O.loglike_workload(w)         # Scott with one sample: undefined -> NaN + flag
+    r = _gpu(P, w)
+    assert r["flags"][0] & P.CHIM_FLAG_BW_DEGENERATE and np.isnan(r["loglike"][0]) and np.isnan(ref["loglike"][0])
+
+
+def test_table_range_flag(P):
+    w = make_workload("tiny", n_events=2, n_samples=100, n_grid=64, n_inj_draw=300)
+    w.dL[:5] = 3.0e5                    # beyond d_L^gw(z_table_max = 10) ~ 1e5 Mpc
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w)
+    assert r["flags"][0] & P.CHIM_FLAG_TABLE_RANGE and ref["flags"][0] & O.F_TABLE_RANGE
+    rel, dtot, _ = _compare(r, ref, 2)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+
+
+def test_no_injections_and_prior_scale(P):
+    w = make_workload("tiny", n_events=3, n_samples=200, n_grid=80, n_inj_draw=300)
+    w.ln_prior = w.ln_prior + 700.0     # absurd prior scale: weights ~ e^-700 must not underflow the path
+    ref = O.loglike_batch(w.lam, w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior - 700.0, w.grid_off, w.z_grid, w.p_gal)
+    c = P.Context()
+    c.init_events(w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal)
+    h = c.loglike_batch_host(np.ascontiguousarray(w.lam), event_logI=True)
+    assert np.all(h["logxi"] == 0) and np.all(np.isnan(h["neff"]))
+    assert np.allclose(h["event_logI"] + 700.0, ref["event_logI"], rtol=REL_EVENT)
+    assert abs(h["loglike"][0] + 3 * 700.0 - ref["loglike"][0]) < ABS_TOTAL
+    c.close()
+
+
+# ---------------------------------------------------------------- T4: ABI misuse
+def test_abi_error_paths(P):
+    import ctypes as C
+    w = make_workload("tiny", n_events=2, n_samples=50, n_grid=30, n_inj_draw=200)
+    h = P.chim_create(None)
+    lam = np.ascontiguousarray(w.lam)
+    out = np.empty(1)
+    with pytest.raises(P.ChimError) as e:
+        P.chim_loglike_batch_host(h, 1, lam, out)
+    assert e.value.status == -2                                  # CHIM_ESTATE: batch before init
+    so, go = w.sample_off.copy(), w.grid_off.copy()
+    bad = w.m1d.copy()
+    bad[3] = w.m2d[3] * 0.5                                      # m1d < m2d
+    with pytest.raises(P.ChimError) as e:
+        P.chim_init_events(h, 2, so, w.dL, bad, w.m2d, w.ln_prior, go, w.z_grid, w.p_gal)
+    assert e.value.status == -1 and "m1d" in str(e.value)
+    zg = w.z_grid.copy()
+    zg[5] = zg[4]                                                # non-increasing grid
+    with pytest.raises(P.ChimError):
+        P.chim_init_events(h, 2, so, w.dL, w.m1d, w.m2d, w.ln_prior, go, zg, w.p_gal)
+    nanl = w.dL.copy()
+    nanl[0] = np.nan
+    with pytest.raises(P.ChimError):
+        P.chim_init_events(h, 2, so, nanl, w.m1d, w.m2d, w.ln_prior, go, w.z_grid, w.p_gal)
+    with pytest.raises(P.ChimError):
+        P.chim_init_events(h, 2, None, w.dL, w.m1d, w.m2d, w.ln_prior, go, w.z_grid, w.p_gal)
+    P.chim_init_events(h, 2, so, w.dL, w.m1d, w.m2d, w.ln_prior, go, w.z_grid, w.p_gal)
+    with pytest.raises(P.ChimError):
+        P.chim_init_injections(h, 10, 5, w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw)   # n_inj_total < n_det
+    P.chim_loglike_batch_host(h, 1, lam, out)
+    assert np.isfinite(out[0])
+    cfg = P.chim_default_config()
+    cfg.kde_cutoff = -1.0
+    with pytest.raises(P.ChimError):
+        P.chim_create(cfg)
+    P.chim_destroy(h)
+
+
+def test_replacing_sets_and_reuse(P):
+    w1 = make_workload("tiny", n_events=3, n_samples=120, n_grid=50, n_inj_draw=400)
+    w2 = make_workload("tiny", n_events=5, n_samples=90, n_grid=70, n_inj_draw=300, seed_offset=7)
+    c = P.Context(z_cat_max=1.5)
+    for w in (w1, w2, w1):
+        c.init_workload(w)
+        h = c.loglike_batch_host(np.ascontiguousarray(w.lam))
+        ref = O.loglike_workload(w)
+        assert abs(h["loglike"][0] - ref["loglike"][0]) < ABS_TOTAL
+    c.close()
