@@ -1,0 +1,329 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path (S1-S6) on BASELINE.json's O5-spectroscopic workload.
+
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--config o5_spec]
+
+A "step" is one chim_loglike_batch call over one batch of n_lambda hyper-parameter points: per-lambda tables,
+per-sample weights, KDE + integral for every event, the injection reduction, and the combine.  Inputs (events,
+injections) are resident in HBM before the timed region.  Metric: event-likelihoods/s = N_events x N_lambda / t.
+N > 1 (torchrun): the path shards by lambda with no data-path collective; every rank holds a replica of the
+inputs and its own lambda batch (weak scaling), value = all ranks' units / max-over-ranks time.
+
+`--impl reference` times the fp64 CPU oracle (oracle/, test infrastructure) on the host cores on a bounded
+sample of the same workload (one lambda per step over the full event and injection sets).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "event-likelihoods/sec (events x lambda) on the O5-spectroscopic workload"
+UNIT = "event-likelihoods/s"
+SM_COUNT = 148
+MUFU_PER_CLK_PER_SM = 16      # MUFU.EX2 lanes per SM per clock on sm_100
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        # under load = samples in the upper half of the power range seen
+        if sm:
+            thr = 0.5 * (min(pw) + max(pw))
+            load = [s for s, p in zip(sm, pw) if p >= thr] or sm
+            return {"sm_mhz": float(np.median(load)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                    "samples": len(sm), "reasons": sorted(reasons)}
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+
+
+def build_workload(name, args, rank):
+    from workloads import draw_lambda_batch, make_workload, FIDUCIAL
+    kw = {}
+    if args.n_events:
+        kw["n_events"] = args.n_events
+    if args.n_det:
+        kw["n_det"] = args.n_det
+    if args.n_lambda:
+        kw["n_lambda"] = args.n_lambda
+    w = make_workload(name, catalog=args.catalog, **kw)
+    return w
+
+
+def lambda_batches(w, n_batches, rank):
+    """A fresh lambda batch per step (an MCMC never re-evaluates the same points); batch 0 is the workload's own."""
+    from workloads import draw_lambda_batch
+    from workloads.synth import LAMBDA_NAMES
+    fid = dict(zip(LAMBDA_NAMES, w.fiducial))
+    out = [w.lam] if rank == 0 else []
+    rng = np.random.default_rng(1_000_003 * (rank + 1) + w.seed)
+    while len(out) < n_batches:
+        out.append(draw_lambda_batch(rng, w.n_lambda, fid))
+    return out
+
+
+def oracle_step(O, w, lam):
+    inj = (w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw)
+    return O.loglike_batch(lam, w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal, inj=inj,
+                           n_inj_total=w.n_inj_total, z_cat_max=w.z_cat_max)
+
+
+def run_reference(args):
+    """The oracle as it stands, on the host cores: each step = 1 lambda over the full event + injection sets."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as O
+    w = build_workload(args.config, args, 0)
+    lams = lambda_batches(w, args.steps + args.warmup, 0)
+    cores = O.num_threads()
+    for i in range(args.warmup):
+        oracle_step(O, w, lams[i][:1])
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        oracle_step(O, w, lams[args.warmup + i][:1])
+    dt = (time.perf_counter() - t0) / max(args.steps, 1)
+    val = w.n_events * 1 / dt
+    sample = f"per step: 1 of {w.n_lambda} lambda over all {w.n_events} events and {w.n_det} injections"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(w, args),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def workload_config(w, args):
+    ns = int(np.diff(w.sample_off).max())
+    nz = int(np.diff(w.grid_off).max())
+    return {"workload": f"{w.name} (BASELINE.json configs[{w.meta['index']}]), catalog {w.meta['catalog']}",
+            "n_events": int(w.n_events), "n_samples": ns, "n_grid": nz, "n_lambda_per_gpu": int(w.n_lambda),
+            "n_injections_detected": int(w.n_det), "n_injections_drawn": int(w.n_inj_total),
+            "l2": "flushed between timed steps (256 MiB write)", "fresh_lambda_batch_per_step": True,
+            "parallelism": f"lambda-sharded replicas x{args.gpus}, no data-path collective"}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2504_02034_b200 as pkg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    pkg.lib()                                   # fails loudly without libchim.so: no fallback
+
+    w = build_workload(args.config, args, rank)
+    K, W = args.steps, max(args.warmup, 3)
+    lams = lambda_batches(w, K + W, rank)
+    stream = torch.cuda.current_stream(dev)
+    ctx = pkg.Context(device=local, stream=stream, z_cat_max=w.z_cat_max, kde_cutoff=args.cutoff,
+                      lambda_chunk=args.lambda_chunk)
+    ctx.init_workload(w)                        # inputs resident in HBM from here on
+    lam_dev = [torch.as_tensor(l, device=dev).contiguous() for l in lams]
+    out = ctx.alloc_outputs(w.n_lambda, event_logI=False)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident arm ---------------------------------------------------------------------------
+    for i in range(W):
+        ctx.loglike_batch(lam_dev[i], out=out)
+    barrier()
+    ctx.set_profiling(True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    ktimes = dict(tables_ms=0.0, events_ms=0.0, inject_ms=0.0, combine_ms=0.0, events_launches=0)
+    pairs_eval = 0
+    barrier()
+    t_wall0 = time.perf_counter()
+    for i in range(K):
+        flush.fill_(i & 0xFF)                   # evict L2 between timed steps
+        evs[i][0].record(stream)
+        ctx.loglike_batch(lam_dev[W + i], out=out)
+        evs[i][1].record(stream)
+        kt = ctx.kernel_times()                 # synchronises; outside the event bracket
+        for k in ktimes:
+            ktimes[k] += kt[k]
+        st = ctx.stats()
+        pairs_eval += st["kde_pairs_evaluated"]
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop() if rank == 0 else None
+    ctx.set_profiling(False)
+    ms = [a.elapsed_time(b) for a, b in evs]
+    t_dev = float(np.sum(ms)) / 1e3
+    ll_last = out["loglike"].cpu().numpy()
+
+    # ---- end-to-end arm: host buffers through chim_loglike_batch_host -----------------------------------
+    lam_pin = [torch.as_tensor(l).contiguous().pin_memory() for l in lams[W:W + K]]
+    o_pin = {k: torch.empty(w.n_lambda, dtype=torch.float64).pin_memory() for k in ("loglike", "logxi", "neff")}
+    o_pin["flags"] = torch.empty(w.n_lambda, dtype=torch.int32).pin_memory()
+    ctx.loglike_batch_host(lam_pin[0], out=o_pin)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(K):
+        flush.fill_(i & 0xFF)
+        ctx.loglike_batch_host(lam_pin[i], out=o_pin)
+    barrier()
+    t_e2e = time.perf_counter() - t0
+    # the flush is not part of the step: subtract its measured cost
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for i in range(K):
+        flush.fill_(i & 0xFF)
+    b.record(stream)
+    torch.cuda.synchronize(dev)
+    t_e2e -= a.elapsed_time(b) / 1e3
+    h2d = w.n_lambda * 15 * 8
+    d2h = w.n_lambda * (8 * 3 + 4)
+    assert np.allclose(o_pin["loglike"].numpy(), ll_last, rtol=0, atol=1e-9, equal_nan=True)
+
+    # ---- max over ranks ---------------------------------------------------------------------------------
+    t_all = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
+    t_dev_max, t_e2e_max = [float(x) for x in t_all.cpu()]
+    units = w.n_events * w.n_lambda * K * world
+    st = ctx.stats()
+
+    if rank == 0:
+        peaks, peak_src = load_peaks()
+        value = units / t_dev_max
+        n_launch = max(ktimes["events_launches"], 1)
+        ev_s = ktimes["events_ms"] / 1e3
+        clk_max = float(peaks.get("sm_max_mhz", 1965.0))
+        peak_gexp = SM_COUNT * MUFU_PER_CLK_PER_SM * clk_max * 1e6 / 1e9
+        achieved = pairs_eval / ev_s / 1e9 if ev_s > 0 else 0.0
+        clk_run = (clocks or {}).get("sm_mhz") or clk_max
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": t_dev_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64 (weights, moments, sums) + f32 (KDE pair loop)", "data": "synthetic",
+            "config": workload_config(w, args),
+            "kde_pairs_per_s_dense_equivalent": st["kde_pairs_dense"] * K * world / t_dev_max,
+            "kde_pairs_per_s_evaluated": pairs_eval * world / t_dev_max,
+            "kde_cutoff_t": args.cutoff,
+            "kernel_ms_per_step": {k: ktimes[k] / K for k in ("tables_ms", "events_ms", "inject_ms", "combine_ms")},
+            "wall_ms_per_step_incl_flush_and_sync": t_wall / K * 1e3,
+            "e2e": {"value": units / t_e2e_max, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(st["kernel_launches"]) * K,
+            "clocks": clocks,
+            "roofline": {"bound": "alu", "kernel": "k_events (S2-S4: weights + KDE + integral)",
+                         "achieved": achieved, "peak": peak_gexp, "unit": "Gexp/s (MUFU.EX2)", "frac": achieved / peak_gexp,
+                         "frac_at_sampled_clock": achieved / (peak_gexp * clk_run / clk_max),
+                         "traffic": None, "algorithmic_ops_per_launch": pairs_eval / n_launch,
+                         "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
+                         "peak_source": f"148 SM x 16 MUFU/clk x {clk_max:.0f} MHz ({peak_src} sm_max_mhz); see DESIGN.md"},
+            "loglike_sample": [float(x) for x in ll_last[:3]],
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w, lams[0], args)
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def cpu_baseline(w, lam, args):
+    """The oracle as it stands on the host cores, on a bounded sample: `n` lambdas over the full sets."""
+    import oracle as O
+    n = args.cpu_lambdas
+    t0 = time.perf_counter()
+    oracle_step(O, w, lam[:n])
+    dt = time.perf_counter() - t0
+    return {"value": w.n_events * n / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "seconds": dt,
+            "sample": f"{n} of {w.n_lambda} lambda over all {w.n_events} events and {w.n_det} injections (work is linear in lambda)"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="o5_spec")
+    ap.add_argument("--catalog", type=int, default=0)
+    ap.add_argument("--cutoff", type=float, default=6.0)
+    ap.add_argument("--lambda-chunk", type=int, default=256)
+    ap.add_argument("--n-events", type=int, default=0, help="override (debug only; invalidates the number)")
+    ap.add_argument("--n-det", type=int, default=0, help="override (debug only)")
+    ap.add_argument("--n-lambda", type=int, default=0, help="override (debug only)")
+    ap.add_argument("--cpu-lambdas", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -34,6 +34,12 @@ class ChimStats(C.Structure):
                 ("injection_evals", C.c_uint64), ("kernel_launches", C.c_uint64)]
 
 
+class ChimKernelTimes(C.Structure):
+    _fields_ = [("tables_ms", C.c_double), ("events_ms", C.c_double), ("inject_ms", C.c_double),
+                ("combine_ms", C.c_double), ("tables_launches", C.c_uint32), ("events_launches", C.c_uint32),
+                ("inject_launches", C.c_uint32), ("combine_launches", C.c_uint32)]
+
+
 _lib = None
 _vp, _dp, _ip, _up = C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p   # raw addresses (host or device)
 
@@ -65,6 +71,8 @@ def lib():
     L.chim_loglike_batch.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_loglike_batch_host.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_get_stats.argtypes = [C.c_void_p, C.POINTER(ChimStats)]
+    L.chim_set_profiling.argtypes = [C.c_void_p, C.c_int32]
+    L.chim_get_kernel_times.argtypes = [C.c_void_p, C.POINTER(ChimKernelTimes)]
     L.chim_debug_table_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
     L.chim_debug_event_samples.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.chim_debug_event_kde.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -244,6 +252,14 @@ class Context:
     def stats(self):
         s = chim_get_stats(self.h)
         return {k: int(getattr(s, k)) for k, _ in ChimStats._fields_}
+
+    def set_profiling(self, on=True):
+        _check(self.h, lib().chim_set_profiling(self.h, 1 if on else 0))
+
+    def kernel_times(self):
+        k = ChimKernelTimes()
+        _check(self.h, lib().chim_get_kernel_times(self.h, C.byref(k)))
+        return {n: getattr(k, n) for n, _ in ChimKernelTimes._fields_}
 
     # -- diagnostics -----------------------------------------------------------------------------------
     def _lam1(self, lam):

@@ -51,6 +51,10 @@ struct chim_ctx {
     double* st_neff = nullptr; uint32_t* st_fl = nullptr;
     chim_stats last{};
     uint64_t launches = 0;
+    // optional per-kernel timing (CUDA events around each launch of the last batch)
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev_pool;          // reused across batches
+    std::vector<int> ev_kind;                  // kind of the launch bracketed by events [2i, 2i+1]
 };
 
 namespace {
@@ -153,15 +157,32 @@ EventKernelParams event_params(const chim_ctx* ctx, int nl) {
     return P;
 }
 
+// profiling brackets: record an event pair around a launch of kind k (0 tables, 1 events, 2 inject, 3 combine)
+struct Bracket {
+    chim_ctx* ctx; bool on; size_t slot;
+    Bracket(chim_ctx* c, int kind) : ctx(c), on(c->profiling), slot(0) {
+        if (!on) return;
+        slot = ctx->ev_kind.size();
+        while (ctx->ev_pool.size() < 2 * (slot + 1)) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; }
+            ctx->ev_pool.push_back(e);
+        }
+        ctx->ev_kind.push_back(kind);
+        cudaEventRecord(ctx->ev_pool[2 * slot], ctx->stream);
+    }
+    ~Bracket() { if (on) cudaEventRecord(ctx->ev_pool[2 * slot + 1], ctx->stream); }
+};
+
 // one pass over a chunk of lambdas: S1 -> S2-S4 -> S5 -> S6
 int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* out_ev, double* out_xi, double* out_neff,
               uint32_t* out_fl) {
     cudaStream_t st = ctx->stream;
     TableParams TP = table_params(ctx);
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t) * nl, st));
-    CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->wtab, st));
+    { Bracket b(ctx, 0); CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->wtab, st)); }
     EventKernelParams EP = event_params(ctx, nl);
-    CK(launch_events(EP, st));
+    { Bracket b(ctx, 1); CK(launch_events(EP, st)); }
     ctx->launches += 2;
     if (ctx->have_inj) {
         InjKernelParams IP{};
@@ -169,7 +190,7 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
         IP.n_lambda = nl; IP.tab_rows = ctx->inj_grid.rows(); IP.n_win = ctx->cfg.n_win_table; IP.chunk = kInjChunk;
         IP.z_table_max = ctx->cfg.z_table_max; IP.z_cat_max = ctx->cfg.z_cat_max;
         IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = nullptr;
-        CK(launch_inject(IP, ctx->inj_blocks, st));
+        { Bracket b(ctx, 2); CK(launch_inject(IP, ctx->inj_blocks, st)); }
         ctx->launches += 1;
     }
     CombineParams CP{};
@@ -180,7 +201,7 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
     CP.inj_ln_shift = ctx->inj_ln_shift;
     CP.neff_factor = ctx->cfg.neff_factor; CP.flags_in = ctx->flags;
     CP.out_loglike = out_ll; CP.out_event_logI = out_ev; CP.out_logxi = out_xi; CP.out_neff = out_neff; CP.out_flags = out_fl;
-    CK(launch_combine(CP, st));
+    { Bracket b(ctx, 3); CK(launch_combine(CP, st)); }
     ctx->launches += 1;
     return CHIM_OK;
 }
@@ -257,6 +278,7 @@ void chim_destroy(chim_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->cfg.device);
     cudaStreamSynchronize(ctx->stream);
+    for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     free_pool(ctx->owned_ev);
     free_pool(ctx->owned_inj);
     free_pool(ctx->owned_work);
@@ -441,6 +463,7 @@ int chim_loglike_batch(chim_ctx* ctx, int32_t n_lambda, const double* lambda, do
     int rc = ensure_work(ctx, chunk);
     if (rc != CHIM_OK) return rc;
     ctx->launches = 0;
+    ctx->ev_kind.clear();
     CK(cudaMemsetAsync(ctx->stats, 0, 4 * sizeof(unsigned long long), ctx->stream));
     for (int c0 = 0; c0 < n_lambda; c0 += chunk) {
         const int nl = std::min(chunk, n_lambda - c0);
@@ -506,6 +529,29 @@ int chim_get_stats(chim_ctx* ctx, chim_stats* out) {
     CK(cudaMemcpy(s, ctx->stats, sizeof s, cudaMemcpyDeviceToHost));
     ctx->last.kde_pairs_evaluated = s[0];
     *out = ctx->last;
+    return CHIM_OK;
+}
+
+int chim_set_profiling(chim_ctx* ctx, int32_t enable) {
+    if (!ctx) return CHIM_EINVAL;
+    ctx->profiling = enable != 0;
+    ctx->ev_kind.clear();
+    return CHIM_OK;
+}
+
+int chim_get_kernel_times(chim_ctx* ctx, chim_kernel_times* out) {
+    if (!ctx || !out) return CHIM_EINVAL;
+    CK(cudaSetDevice(ctx->cfg.device));
+    CK(cudaStreamSynchronize(ctx->stream));
+    std::memset(out, 0, sizeof(*out));
+    double* ms[4] = {&out->tables_ms, &out->events_ms, &out->inject_ms, &out->combine_ms};
+    uint32_t* nl[4] = {&out->tables_launches, &out->events_launches, &out->inject_launches, &out->combine_launches};
+    for (size_t i = 0; i < ctx->ev_kind.size(); ++i) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, ctx->ev_pool[2 * i], ctx->ev_pool[2 * i + 1]));
+        *ms[ctx->ev_kind[i]] += t;
+        *nl[ctx->ev_kind[i]] += 1;
+    }
     return CHIM_OK;
 }
 
