@@ -307,10 +307,10 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
         max_ns = std::max<int>(max_ns, (int)ns);
         max_nz = std::max<int>(max_nz, (int)nz);
     }
-    if (events_smem_bytes(max_ns) > kMaxSmemOptin) {
+    if (events_smem_bytes(max_ns, max_nz) > kMaxSmemOptin) {
         char b[160];
         std::snprintf(b, sizeof b, "chim_init_events: N_s = %d exceeds the shared-memory staging limit (%d samples per event)",
-                      max_ns, (int)((kMaxSmemOptin - 1024) / 16));
+                      max_ns, (int)((kMaxSmemOptin - 4096) / 12));
         return fail(ctx, CHIM_EINVAL, b);
     }
     const size_t NS = (size_t)so[n_events], NG = (size_t)go[n_events];
@@ -587,6 +587,7 @@ static int debug_event(chim_ctx* ctx, const double* lambda, int32_t event, doubl
     EventKernelParams EP = event_params(ctx, 1);
     EP.dbg_event = event;
     EP.dbg_z = z_out; EP.dbg_w = w_out; EP.dbg_h = h_out; EP.dbg_K = K_out;
+    if (K_out) CK(cudaMemsetAsync(K_out, 0, sizeof(double) * (size_t)(ctx->h_grid_off[event + 1] - ctx->h_grid_off[event]), ctx->stream));
     CK(launch_events(EP, ctx->stream));
     if (logI_out) CK(cudaMemcpyAsync(logI_out, ctx->logI, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));

@@ -25,6 +25,7 @@ struct LamConst {
     double inv2s2;      // 1 / (2 sigma_g^2)
     double W_c;         // int_{m_low}^{m_c} m^beta S(m) dm
     double bp1;         // beta + 1
+    double inv_bp1;     // 1 / (beta + 1)
     double pow_mc_bp1;  // m_c^(beta+1)
     double ln_mc;       // ln m_c
     double gk;          // gamma + kappa
@@ -62,26 +63,60 @@ struct TableParams {
     DlGrid ev, inj;
 };
 
+// exp(x) in fp64 for the sample kernels: argument clamped to [-700, 700] (e^-700 ~ 1e-304 stands in for 0,
+// nothing on this path needs more), Cody-Waite reduction x = n ln2 + r with |r| <= ln2/2, degree-11 Taylor
+// polynomial in Horner form (relative error < 1e-14), scaling by 2^n through the exponent field.  Branch-free;
+// the coefficients live in constant memory so that DFMA takes them as direct operands.
+static __constant__ double c_exp_coef[12] = {
+    2.50521083854417187751e-08, 2.75573192239858906526e-07, 2.75573192239858906526e-06, 2.48015873015873015873e-05,
+    1.98412698412698412698e-04, 1.38888888888888888889e-03, 8.33333333333333333333e-03, 4.16666666666666666667e-02,
+    1.66666666666666666667e-01, 0.5, 1.0, 1.0};
+static __constant__ double c_exp_red[5] = {1.4426950408889634074, 6755399441055744.0 /* 1.5 * 2^52 */,
+                                           -6.93147180369123816490e-01, -1.90821492927058770002e-10, 700.0};
+
+__device__ __forceinline__ double fast_exp(double x) {
+    x = (x > -c_exp_red[4]) ? x : -c_exp_red[4];       // cheap clamps (no NaN canonicalisation): inputs are finite
+    x = (x < c_exp_red[4]) ? x : c_exp_red[4];
+    double t = fma(x, c_exp_red[0], c_exp_red[1]);     // round-to-nearest integer by the magic-number addition
+    int n = __double2loint(t);
+    double fn = t - c_exp_red[1];
+    double r = fma(fn, c_exp_red[2], x);
+    r = fma(fn, c_exp_red[3], r);
+    double p = c_exp_coef[0];
+#pragma unroll
+    for (int i = 1; i < 12; ++i) p = fma(p, r, c_exp_coef[i]);
+    return p * __hiloint2double((n + 1023) << 20, 0);  // |n| <= 1010: 2^n is a normal double
+}
+
+// 1/x for finite non-zero normal x: MUFU.RCP64H seed + two Newton steps (error ~1e-16), no special cases.
+__device__ __forceinline__ double fast_rcp(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+
 __device__ __forceinline__ double horner3(const double* c, double t) {
     return fma(fma(fma(c[3], t, c[2]), t, c[1]), t, c[0]);
 }
 
-// Smoothing denominator 1 + exp(f(m')), f = delta/m' + delta/(m'-delta) (M1), for m inside the window.
-__device__ __forceinline__ double smooth_den(double m, const LamConst& L) {
-    double mp = m - L.m_low;
-    double f = L.delta * (2.0 * mp - L.delta) / (mp * (mp - L.delta));
-    return 1.0 + exp(f);
+// Smoothing denominator 1/S(m) = 1 + exp(f(m')), f = delta/m' + delta/(m'-delta) = delta (2m'-delta)/(m'(m'-delta))
+// (M1), for m' = m - m_low clamped strictly inside the window so that the expression is finite for every lane
+// (lanes outside the window discard the value).
+__device__ __forceinline__ double smooth_den(double mp, const LamConst& L) {
+    const double lo = L.delta * 1e-6, hi = L.delta * (1.0 - 1e-12);
+    double mpc = (mp > lo) ? mp : lo;
+    mpc = (mpc < hi) ? mpc : hi;
+    double f = L.delta * (2.0 * mpc - L.delta) * fast_rcp(mpc * (mpc - L.delta));
+    return 1.0 + fast_exp(f);
 }
 
-// C(m1) = int_{m_low}^{m1} m^beta S(m) dm (M3/M4) above the window: window integral + closed-form power.
-__device__ __forceinline__ double c_norm_above(double lm1, const LamConst& L) {
-    if (L.beta_is_m1) return L.W_c + (lm1 - L.ln_mc);
-    return L.W_c + (exp(L.bp1 * lm1) - L.pow_mc_bp1) / L.bp1;
-}
-
-// Inside the window both S(m1) and C(m1) vanish faster than any power at m_low, so the table holds the smooth
-// ratio rho(m') = C / (S m'^2), m' = m - m_low (rho -> m_low^beta/delta_m as m' -> 0, rho(delta_m) = W_c/delta_m^2):
-// S(m1)/C(m1) = 1/(rho m'^2) and S(m1) cancels analytically in the weight.  Cubic Lagrange on uniform nodes.
+// Inside the window both S(m1) and C(m1) = int_{m_low}^{m1} m^beta S(m) dm (M3/M4) vanish faster than any power
+// at m_low, so the table holds the smooth ratio rho(m') = C / (S m'^2) (rho -> m_low^beta/delta_m as m' -> 0,
+// rho(delta_m) = W_c/delta_m^2): S(m1)/C(m1) = 1/(rho m'^2) and S(m1) cancels analytically in the weight.
+// Cubic Lagrange on uniform nodes.
 __device__ __forceinline__ double rho_window(double mp, const LamConst& L, const double* __restrict__ rtab, int n_win) {
     double x = mp * L.win_scale;
     int b = (int)x - 1;
@@ -95,42 +130,42 @@ __device__ __forceinline__ double rho_window(double mp, const LamConst& L, const
 // Steps S2 / S5 for one sample (or injection): redshift from the table, source-frame masses, population
 // weight.  `ipr` = 1/pi_j (events) or 1/p_draw,j (injections); R carries psi/J (and u_vol for injections).
 //   PAPER.md:52 (d_L -> z, m = m^d/(1+z)), :195-198 eq. 20 + M1-M4 (mass model), :226 eq. 21, :75 eq. 11.
+// Written without data-dependent branches (selects only): the lanes of a warp hold samples on both sides of
+// every mass-function edge, so branches would serialise the exponentials.
 __device__ __forceinline__ void sample_weight(const LamConst& L, const Row* __restrict__ tab, int n_rows,
                                               const double* __restrict__ wtab, int n_win, double tkmax,
                                               double z_table_max, double tk, double m1d, double q, double lnm1d,
                                               double lnq, double ipr, double& z, double& w, bool& out_of_range) {
     out_of_range = !(tk <= tkmax);
-    if (out_of_range) {
-        z = z_table_max;
-        w = 0.0;
-        return;
-    }
-    int k = (int)tk;
-    k = max(1, min(k, n_rows - 2));
+    int k = (int)((tk < (double)(n_rows - 2)) ? tk : (double)(n_rows - 2));
+    k = max(1, k);
     double t = tk - (double)k;
-    const Row& r = tab[k];
-    z = horner3(r.c[0], t);
-    double u = horner3(r.c[1], t);
-    double a = horner3(r.c[2], t);
-    double R = horner3(r.c[3], t);
+    const double2* rp = reinterpret_cast<const double2*>(tab + k);   // 8 x 128-bit loads of one 128-byte row
+    double2 c0 = rp[0], c1 = rp[1], c2 = rp[2], c3 = rp[3], c4 = rp[4], c5 = rp[5], c6 = rp[6], c7 = rp[7];
+    double zt = fma(fma(fma(c1.y, t, c1.x), t, c0.y), t, c0.x);
+    double u = fma(fma(fma(c3.y, t, c3.x), t, c2.y), t, c2.x);
+    double a = fma(fma(fma(c5.y, t, c5.x), t, c4.y), t, c4.x);
+    double R = fma(fma(fma(c7.y, t, c7.x), t, c6.y), t, c6.x);
+    z = out_of_range ? z_table_max : zt;
     double m1 = m1d * a, m2 = q * m1;
-    w = 0.0;
-    if (!(m2 >= L.m_low)) return;                      // R15: p(m2|m1) = 0 below m_low (m1 >= m2)
     double lm1 = lnm1d - u, lm2 = lm1 + lnq;
-    double bl2 = L.beta * lm2;                         // ln m2^beta
+    double bl2 = L.beta * lm2;                                      // ln m2^beta
     double dm = m1 - L.mu;
-    double e = exp(L.a_g - dm * dm * L.inv2s2 + bl2);  // lambda_g N(m1) m2^beta / Z1
-    if (m1 <= L.m_high) e += exp(L.a_pl - L.alpha * lm1 + bl2);
-    double den = 1.0, C;
-    if (m2 < L.m_c) den = smooth_den(m2, L);           // 1/S(m2)
-    if (m1 < L.m_c) {                                   // S(m1)/C(m1) = 1/(rho m'^2)
-        double mp = m1 - L.m_low;
-        C = rho_window(mp, L, wtab, n_win) * mp * mp;
-    } else {
-        C = c_norm_above(lm1, L);
-    }
-    if (!(C > 0.0) || !(den < INFINITY)) return;
-    w = e * R * ipr / (den * C);
+    double e = fast_exp(L.a_g - dm * dm * L.inv2s2 + bl2);          // lambda_g N(m1) m2^beta / Z1
+    double epl = fast_exp(L.a_pl - L.alpha * lm1 + bl2);            // (1-lambda_g) PL(m1) m2^beta / Z1
+    e += (m1 <= L.m_high) ? epl : 0.0;
+    double mp1 = m1 - L.m_low, mp2 = m2 - L.m_low;
+    double den2 = smooth_den(mp2, L);
+    double den = (mp2 < L.delta) ? den2 : 1.0;                      // 1/S(m2)
+    // C(m1): above the window W_c + closed-form power integral; inside, rho m'^2 (S(m1) cancelled)
+    double pw = L.beta_is_m1 ? (lm1 - L.ln_mc) : (fast_exp(L.bp1 * lm1) - L.pow_mc_bp1) * L.inv_bp1;
+    double mp1c = (mp1 > 0.0) ? mp1 : 0.0;
+    mp1c = (mp1c < L.delta) ? mp1c : L.delta;
+    double cw = rho_window(mp1c, L, wtab, n_win) * mp1c * mp1c;
+    double C = (mp1 < L.delta) ? cw : L.W_c + pw;
+    double dc = den * C;
+    bool ok = !out_of_range && (m2 >= L.m_low) && (dc > 1e-300) && (dc < 1e300);   // R15 support; underflowed S or C
+    w = ok ? e * R * ipr * fast_rcp(ok ? dc : 1.0) : 0.0;
 }
 
 // ---- small reductions ---------------------------------------------------------------------------------
@@ -231,7 +266,7 @@ cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);
 cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, int64_t n, const double* dL,
                                 double z_table_max, double* z_out, double* r_out, cudaStream_t st);
 cudaError_t upload_gauss_legendre();   // fills the __constant__ node tables used by S1
-size_t events_smem_bytes(int max_ns);
+size_t events_smem_bytes(int max_ns, int max_nz);
 size_t tables_smem_bytes(const TableParams& P);
 
 }  // namespace chim

@@ -13,6 +13,8 @@ namespace chim {
 
 constexpr int kInjThreads = 256;
 
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 struct InjSmem {
     LamConst L[2];
     double red[2 * (kInjThreads / 32)];
@@ -36,17 +38,24 @@ __global__ void __launch_bounds__(kInjThreads) k_inject(InjKernelParams P) {
     for (int i = tid; i < nw; i += kInjThreads)
         reinterpret_cast<uint32_t*>(&S.L[0])[i] = reinterpret_cast<const uint32_t*>(P.Lc)[i];
     __syncthreads();
+    // the chunk is sorted in d_L, so it addresses the table rows [k_first, k_last] of every lambda's table
+    const int k_first = max(1, (int)rA[0].x), k_span = min(P.tab_rows - 2, (int)rA[nj - 1].x) - k_first + 1;
+    const int rho_lines = (P.n_win + 1 + 15) / 16;
 
     for (int l = 0; l < P.n_lambda; ++l) {
         const LamConst& L = S.L[l & 1];
-        if (l + 1 < P.n_lambda)   // prefetch the next lambda's constants into the other buffer
+        if (l + 1 < P.n_lambda) {   // prefetch the next lambda's constants (shared memory) and table lines (L1)
             for (int i = tid; i < nw; i += kInjThreads)
                 reinterpret_cast<uint32_t*>(&S.L[(l + 1) & 1])[i] = reinterpret_cast<const uint32_t*>(P.Lc + l + 1)[i];
+            if (tid < k_span) prefetch_l1(P.tab + (size_t)(l + 1) * P.tab_rows + k_first + tid);
+            else if (tid - k_span < rho_lines) prefetch_l1(P.wtab + (size_t)(l + 1) * (P.n_win + 1) + 16 * (tid - k_span));
+        }
         double acc[2] = {0.0, 0.0};
         int oor = 0;
         if (L.flags == 0) {
             const Row* tab = P.tab + (size_t)l * P.tab_rows;
             const double* wtab = P.wtab + (size_t)l * (P.n_win + 1);
+#pragma unroll 1
             for (int j = tid; j < nj; j += kInjThreads) {
                 double2 A = rA[j], B = rB[j], C = rC[j];
                 double z, s;

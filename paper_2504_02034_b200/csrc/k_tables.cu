@@ -242,6 +242,7 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         L.inv2s2 = 0.5 / (L.sigma * L.sigma);
         L.bp1 = L.beta + 1.0;
         L.beta_is_m1 = fabs(L.bp1) < 1e-12;
+        L.inv_bp1 = L.beta_is_m1 ? 0.0 : 1.0 / L.bp1;
         L.ln_mc = log(L.m_c);
         L.pow_mc_bp1 = exp(L.bp1 * L.ln_mc);
         L.gk = L.gamma + L.kappa;

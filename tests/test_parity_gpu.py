@@ -209,8 +209,9 @@ def test_host_entry_point_matches_device_entry_point(P):
     out = c.loglike_batch(torch.as_tensor(w.lam, device=c.device).contiguous())
     torch.cuda.synchronize()
     h = c.loglike_batch_host(np.ascontiguousarray(w.lam), event_logI=True)
-    assert np.array_equal(out["loglike"].cpu().numpy(), h["loglike"])
-    assert np.array_equal(out["event_logI"].cpu().numpy(), h["event_logI"])
+    # same kernels, same inputs; work items are handed to warps dynamically, so fp64 sums may differ in order
+    assert np.allclose(out["loglike"].cpu().numpy(), h["loglike"], rtol=1e-12, atol=0)
+    assert np.allclose(out["event_logI"].cpu().numpy(), h["event_logI"], rtol=1e-12, atol=0)
     c.close()
 
 
