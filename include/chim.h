@@ -162,6 +162,16 @@ typedef struct chim_kernel_times {
 int chim_set_profiling(chim_ctx *ctx, int32_t enable);
 int chim_get_kernel_times(chim_ctx *ctx, chim_kernel_times *out);
 
+/* Plain-ALU peak rates of the device the context lives on, measured by micro-benchmarks (independent dependency
+ * chains, 8 CTAs per SM) on cfg.stream; synchronous.  These are the roofline denominators of the path, which is
+ * bound by the SMs' arithmetic pipes rather than by HBM or the tensor cores.  All four are in
+ * 1e9 lane-instructions per second: MUFU.EX2, FFMA, DFMA, and FFMA2 (packed fp32x2, counted as two). */
+typedef struct chim_alu_peaks {
+    double ex2_gops, ffma_gops, dfma_gops, ffma2_gops;
+    int32_t sm_count, reserved;
+} chim_alu_peaks;
+int chim_measure_alu_peaks(chim_ctx *ctx, chim_alu_peaks *out);
+
 /* ---- diagnostics: intermediates of the path for ONE lambda (DEVICE pointer to 15 doubles) -------------
  * They run the same device code as the hot path and exist so that each step can be compared with the
  * oracle (tests tier T2).  Outputs are DEVICE pointers; any of them may be NULL.  Synchronous. */

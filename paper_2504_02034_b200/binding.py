@@ -40,6 +40,11 @@ class ChimKernelTimes(C.Structure):
                 ("inject_launches", C.c_uint32), ("combine_launches", C.c_uint32)]
 
 
+class ChimAluPeaks(C.Structure):
+    _fields_ = [("ex2_gops", C.c_double), ("ffma_gops", C.c_double), ("dfma_gops", C.c_double),
+                ("ffma2_gops", C.c_double), ("sm_count", C.c_int32), ("reserved", C.c_int32)]
+
+
 _lib = None
 _vp, _dp, _ip, _up = C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p   # raw addresses (host or device)
 
@@ -73,6 +78,7 @@ def lib():
     L.chim_get_stats.argtypes = [C.c_void_p, C.POINTER(ChimStats)]
     L.chim_set_profiling.argtypes = [C.c_void_p, C.c_int32]
     L.chim_get_kernel_times.argtypes = [C.c_void_p, C.POINTER(ChimKernelTimes)]
+    L.chim_measure_alu_peaks.argtypes = [C.c_void_p, C.POINTER(ChimAluPeaks)]
     L.chim_debug_table_lookup.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
     L.chim_debug_event_samples.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.chim_debug_event_kde.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -149,6 +155,12 @@ def chim_get_stats(ctx) -> ChimStats:
     s = ChimStats()
     _check(ctx, lib().chim_get_stats(ctx, C.byref(s)))
     return s
+
+
+def chim_measure_alu_peaks(ctx) -> ChimAluPeaks:
+    p = ChimAluPeaks()
+    _check(ctx, lib().chim_measure_alu_peaks(ctx, C.byref(p)))
+    return p
 
 
 # ---- convenience ------------------------------------------------------------------------------------
@@ -260,6 +272,10 @@ class Context:
         k = ChimKernelTimes()
         _check(self.h, lib().chim_get_kernel_times(self.h, C.byref(k)))
         return {n: getattr(k, n) for n, _ in ChimKernelTimes._fields_}
+
+    def alu_peaks(self):
+        p = chim_measure_alu_peaks(self.h)
+        return {n: getattr(p, n) for n, _ in ChimAluPeaks._fields_ if n != "reserved"}
 
     # -- diagnostics -----------------------------------------------------------------------------------
     def _lam1(self, lam):

@@ -555,6 +555,19 @@ int chim_get_kernel_times(chim_ctx* ctx, chim_kernel_times* out) {
     return CHIM_OK;
 }
 
+int chim_measure_alu_peaks(chim_ctx* ctx, chim_alu_peaks* out) {
+    if (!ctx || !out) return CHIM_EINVAL;
+    CK(cudaSetDevice(ctx->cfg.device));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, ctx->cfg.device));
+    double g[4];
+    CK(measure_alu_peaks(prop.multiProcessorCount, 3, ctx->stream, g));
+    out->ex2_gops = g[0]; out->ffma_gops = g[1]; out->dfma_gops = g[2]; out->ffma2_gops = g[3];
+    out->sm_count = prop.multiProcessorCount;
+    out->reserved = 0;
+    return CHIM_OK;
+}
+
 // ---- diagnostics --------------------------------------------------------------------------------------
 static int debug_prepare(chim_ctx* ctx, const double* lambda, const char* who) {
     if (!ctx) return CHIM_EINVAL;

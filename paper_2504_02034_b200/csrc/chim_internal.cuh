@@ -266,6 +266,7 @@ cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);
 cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, int64_t n, const double* dL,
                                 double z_table_max, double* z_out, double* r_out, cudaStream_t st);
 cudaError_t upload_gauss_legendre();   // fills the __constant__ node tables used by S1
+cudaError_t measure_alu_peaks(int n_sm, int reps, cudaStream_t st, double out_g[4]);
 size_t events_smem_bytes(int max_ns, int max_nz);
 size_t tables_smem_bytes(const TableParams& P);
 
