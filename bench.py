@@ -200,7 +200,7 @@ def run_ours(args):
         sampler.start()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     ktimes = dict(tables_ms=0.0, events_ms=0.0, inject_ms=0.0, combine_ms=0.0, events_launches=0)
-    pairs_eval = 0
+    pairs_eval = pairs_cut = 0
     barrier()
     t_wall0 = time.perf_counter()
     for i in range(K):
@@ -213,6 +213,7 @@ def run_ours(args):
             ktimes[k] += kt[k]
         st = ctx.stats()
         pairs_eval += st["kde_pairs_evaluated"]
+        pairs_cut += st["kde_pairs_in_cutoff"]
     barrier()
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop() if rank == 0 else None

@@ -57,6 +57,8 @@ typedef enum chim_status {
 enum { CHIM_MEM_HOST = 0, CHIM_MEM_DEVICE = 1 };   /* where the pointers given to chim_init_* live     */
 enum { CHIM_ON_SAMPLES = 0, CHIM_ON_GRID = 1 };    /* placement of psi/J (R1): N = per-sample weights  */
 enum { CHIM_BW_SCOTT = 0, CHIM_BW_FIXED = 1 };     /* KDE bandwidth rule (R3)                          */
+enum { CHIM_KDE_AUTO = 0, CHIM_KDE_DIRECT = 1 };   /* pair-loop formulation: AUTO = power
+                                                      form on equally spaced grids, direct form otherwise  */
 
 /* per-lambda flag bits written to out_flags */
 #define CHIM_FLAG_LAMBDA_DOMAIN 1u   /* H0<=0, Om not in (0,1], Xi0<=0, delta_m<=0, sigma_g<=0, lambda_g not in
@@ -84,11 +86,13 @@ typedef struct chim_config {
     int32_t n_win_table; /* panels of the per-lambda window table of int m^beta S(m) dm (M4)                   */
     int32_t lambda_chunk;/* lambdas processed per internal pass (bounds the per-lambda table memory)           */
     double neff_factor;  /* NEFF_LOW is raised if N_eff < neff_factor * N_events (R8)                          */
+    int32_t kde_method;  /* CHIM_KDE_AUTO (default) | CHIM_KDE_DIRECT (one MUFU.EX2 per pair on every grid)            */
+    int32_t n_mass_table;/* intervals of the per-lambda mass table in ln m1                           */
 } chim_config;
 
 /* Fills *cfg with the defaults: device 0, HOST, NULL stream, ON_SAMPLES, SCOTT, kde_cutoff 6.0,
  * z_cat_max 1.5, z_table_max 10, n_table 2048, n_dl_table 2048, n_win_table 512, lambda_chunk 256,
- * neff_factor 5. */
+ * neff_factor 5, kde_method AUTO, n_mass_table 2048. */
 void chim_default_config(chim_config *cfg);
 
 /* Creates a context on cfg->device.  cfg == NULL means chim_default_config.  *out is set to NULL on error
@@ -140,10 +144,12 @@ int chim_loglike_batch_host(chim_ctx *ctx, int32_t n_lambda, const double *lambd
                             uint32_t *out_flags);
 
 /* Work counters of the last chim_loglike_batch on this context (valid after the stream is synchronised;
- * the call itself synchronises).  kde_pairs_evaluated = sample x grid-point exponentials actually issued
- * (after the cut-off skip); kde_pairs_dense = sum_i N_s,i N_z,i x n_lambda. */
+ * the call itself synchronises).  kde_pairs_in_cutoff = (sample, grid point) pairs with |z_g - z_j| <= t*h, the
+ * algorithmic work of S3; kde_pairs_evaluated = pairs the kernel executed (the bands are padded to whole
+ * blocks and to the widest sample of a warp pass); kde_pairs_dense = sum_i N_s,i N_z,i x n_lambda. */
 typedef struct chim_stats {
     uint64_t kde_pairs_evaluated;
+    uint64_t kde_pairs_in_cutoff;
     uint64_t kde_pairs_dense;
     uint64_t sample_evals;    /* (sample, lambda) weight evaluations  */
     uint64_t injection_evals; /* (injection, lambda) weight evaluations */

@@ -19,7 +19,7 @@ using namespace chim;
 
 namespace {
 constexpr size_t kMaxSmemOptin = 232448;   // 227 KB per CTA on sm_100
-constexpr int kInjChunk = 1024;            // injections per CTA of k_inject
+constexpr int kInjChunk = 8192;            // injections per CTA of k_inject
 }
 
 struct chim_ctx {
@@ -32,6 +32,7 @@ struct chim_ctx {
     EventSetDev ev{};
     DlGrid ev_grid{0, 1, 0};
     const double* ev_ln_shift = nullptr;   // [n_events] added back to log I (prior scale factored out)
+    const double* ev_ln_qscale = nullptr;  // [n_events] added back to log I (q_g scale factored out)
     std::vector<int64_t> h_sample_off, h_grid_off;
     // injections
     bool have_inj = false;
@@ -42,7 +43,8 @@ struct chim_ctx {
     // work buffers for one lambda chunk
     int work_nl = 0;
     bool work_has_dc = false;
-    LamConst* Lc = nullptr; Row* tab_ev = nullptr; Row* tab_inj = nullptr; double* wtab = nullptr;
+    LamConst* Lc = nullptr; Row* tab_ev = nullptr; Row* tab_inj = nullptr; MassRow* mtab = nullptr;
+    double ev_m_top = 0.0, inj_m_top = 0.0;   // largest detector-frame m1 of each loaded set
     double* dc_tab = nullptr; double* logI = nullptr; double2* partial = nullptr; uint32_t* flags = nullptr;
     unsigned long long* stats = nullptr;
     // staging for the host-pointer entry point
@@ -120,7 +122,7 @@ int ensure_work(chim_ctx* ctx, int nl) {
     CK(dev_alloc(ctx->owned_work, &ctx->Lc, nl));
     CK(dev_alloc(ctx->owned_work, &ctx->tab_ev, (size_t)nl * ctx->ev_grid.rows()));
     CK(dev_alloc(ctx->owned_work, &ctx->tab_inj, (size_t)nl * (ctx->have_inj ? ctx->inj_grid.rows() : 1)));
-    CK(dev_alloc(ctx->owned_work, &ctx->wtab, (size_t)nl * (ctx->cfg.n_win_table + 1)));
+    CK(dev_alloc(ctx->owned_work, &ctx->mtab, (size_t)nl * (ctx->cfg.n_mass_table + 2)));
     ctx->dc_tab = nullptr;
     if (need_dc) CK(dev_alloc(ctx->owned_work, &ctx->dc_tab, (size_t)nl * (ctx->cfg.n_table + 1 + kZPad)));
     CK(dev_alloc(ctx->owned_work, &ctx->logI, (size_t)nl * ctx->ev.n_events));
@@ -138,6 +140,8 @@ TableParams table_params(const chim_ctx* ctx) {
     P.z_cat_max = ctx->cfg.z_cat_max;
     P.n_table = ctx->cfg.n_table;
     P.n_win = ctx->cfg.n_win_table;
+    P.n_mass = ctx->cfg.n_mass_table;
+    P.ln_m_top = std::log(std::max(std::max(ctx->ev_m_top, ctx->have_inj ? ctx->inj_m_top : 0.0), 1e-3));
     P.placement = ctx->cfg.placement;
     P.ev = ctx->ev_grid;
     P.inj = ctx->have_inj ? ctx->inj_grid : DlGrid{0, 1, 0};
@@ -147,12 +151,13 @@ TableParams table_params(const chim_ctx* ctx) {
 EventKernelParams event_params(const chim_ctx* ctx, int nl) {
     EventKernelParams P{};
     P.ev = ctx->ev;
-    P.Lc = ctx->Lc; P.tab = ctx->tab_ev; P.wtab = ctx->wtab; P.dc_tab = ctx->dc_tab;
-    P.n_lambda = nl; P.tab_rows = ctx->ev_grid.rows(); P.n_win = ctx->cfg.n_win_table; P.n_table = ctx->cfg.n_table;
-    P.placement = ctx->cfg.placement; P.bw_rule = ctx->cfg.bw_rule;
+    P.Lc = ctx->Lc; P.tab = ctx->tab_ev; P.mtab = ctx->mtab; P.dc_tab = ctx->dc_tab;
+    P.n_lambda = nl; P.tab_rows = ctx->ev_grid.rows(); P.n_mass = ctx->cfg.n_mass_table; P.n_table = ctx->cfg.n_table;
+    P.placement = ctx->cfg.placement; P.bw_rule = ctx->cfg.bw_rule; P.kde_method = ctx->cfg.kde_method;
     P.z_table_max = ctx->cfg.z_table_max; P.cutoff = ctx->cfg.kde_cutoff;
     P.logI = ctx->logI; P.flags = ctx->flags; P.stats = ctx->stats;
     P.ln_shift = ctx->ev_ln_shift;
+    P.ln_qscale = ctx->ev_ln_qscale;
     P.dbg_event = -1;
     return P;
 }
@@ -180,14 +185,14 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
     cudaStream_t st = ctx->stream;
     TableParams TP = table_params(ctx);
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t) * nl, st));
-    { Bracket b(ctx, 0); CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->wtab, st)); }
+    { Bracket b(ctx, 0); CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, st)); }
     EventKernelParams EP = event_params(ctx, nl);
     { Bracket b(ctx, 1); CK(launch_events(EP, st)); }
     ctx->launches += 2;
     if (ctx->have_inj) {
         InjKernelParams IP{};
-        IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.wtab = ctx->wtab;
-        IP.n_lambda = nl; IP.tab_rows = ctx->inj_grid.rows(); IP.n_win = ctx->cfg.n_win_table; IP.chunk = kInjChunk;
+        IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.mtab = ctx->mtab;
+        IP.n_lambda = nl; IP.tab_rows = ctx->inj_grid.rows(); IP.n_mass = ctx->cfg.n_mass_table; IP.chunk = kInjChunk;
         IP.z_table_max = ctx->cfg.z_table_max; IP.z_cat_max = ctx->cfg.z_cat_max;
         IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = nullptr;
         { Bracket b(ctx, 2); CK(launch_inject(IP, ctx->inj_blocks, st)); }
@@ -231,6 +236,8 @@ void chim_default_config(chim_config* cfg) {
     cfg->n_win_table = 512;
     cfg->lambda_chunk = 256;
     cfg->neff_factor = 5.0;
+    cfg->kde_method = CHIM_KDE_AUTO;
+    cfg->n_mass_table = 2048;
 }
 
 int chim_version(void) { return CHIM_VERSION; }
@@ -248,13 +255,15 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     if (c.n_dl_table <= 0) c.n_dl_table = d.n_dl_table;
     if (c.n_win_table <= 0) c.n_win_table = d.n_win_table;
     if (c.lambda_chunk <= 0) c.lambda_chunk = d.lambda_chunk;
+    if (c.n_mass_table <= 0) c.n_mass_table = d.n_mass_table;
     if (!(c.z_table_max > 0.0)) c.z_table_max = d.z_table_max;
     if (!(c.z_cat_max > 0.0)) c.z_cat_max = d.z_cat_max;
     if (!(c.neff_factor >= 0.0)) c.neff_factor = d.neff_factor;
     if (c.kde_cutoff < 0.0 || !std::isfinite(c.kde_cutoff)) return CHIM_EINVAL;
-    if (c.n_table < 16 || c.n_dl_table < 16 || c.n_win_table < 8 || c.z_cat_max > c.z_table_max) return CHIM_EINVAL;
+    if (c.n_table < 16 || c.n_dl_table < 16 || c.n_win_table < 8 || c.n_mass_table < 64 || c.z_cat_max > c.z_table_max) return CHIM_EINVAL;
     if (c.placement != CHIM_ON_SAMPLES && c.placement != CHIM_ON_GRID) return CHIM_EINVAL;
     if (c.bw_rule != CHIM_BW_SCOTT && c.bw_rule != CHIM_BW_FIXED) return CHIM_EINVAL;
+    if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT) return CHIM_EINVAL;
     if (c.mem != CHIM_MEM_HOST && c.mem != CHIM_MEM_DEVICE) return CHIM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device < 0 || c.device >= ndev) return CHIM_ECUDA;
@@ -268,7 +277,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     ctx->stream = static_cast<cudaStream_t>(c.stream);
     TableParams TP = table_params(ctx);
     TP.ev.K = TP.inj.K = c.n_dl_table;
-    if (tables_smem_bytes(TP) > kMaxSmemOptin) { delete ctx; return CHIM_EINVAL; }
+    if (tables_smem_bytes(TP) > kMaxSmemOptin || inject_smem_bytes(c.n_mass_table) > kMaxSmemOptin) { delete ctx; return CHIM_EINVAL; }
     if (upload_gauss_legendre() != cudaSuccess) { delete ctx; return CHIM_ECUDA; }
     *out = ctx;
     return CHIM_OK;
@@ -310,7 +319,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     if (events_smem_bytes(max_ns, max_nz) > kMaxSmemOptin) {
         char b[160];
         std::snprintf(b, sizeof b, "chim_init_events: N_s = %d exceeds the shared-memory staging limit (%d samples per event)",
-                      max_ns, (int)((kMaxSmemOptin - 4096) / 12));
+                      max_ns, (int)((kMaxSmemOptin - 4096 - 8 * (size_t)max_nz) / 12));
         return fail(ctx, CHIM_EINVAL, b);
     }
     const size_t NS = (size_t)so[n_events], NG = (size_t)go[n_events];
@@ -321,10 +330,11 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     if (!all_finite(h_dl) || !all_finite(h_m1) || !all_finite(h_m2) || !all_finite(h_lp) || !all_finite(h_z) ||
         !all_finite(h_p) || !all_finite(h_bw))
         return fail(ctx, CHIM_EINVAL, "chim_init_events: non-finite input");
-    double xmin = INFINITY, xmax = -INFINITY;
+    double xmin = INFINITY, xmax = -INFINITY, m_top = 0.0;
     for (size_t j = 0; j < NS; ++j) {
         if (!(h_dl[j] > 0.0) || !(h_m2[j] > 0.0) || !(h_m1[j] >= h_m2[j]))
             return fail(ctx, CHIM_EINVAL, "chim_init_events: need dL > 0 and m1d >= m2d > 0");
+        m_top = std::max(m_top, h_m1[j]);
         double x = std::log(h_dl[j]);
         xmin = std::min(xmin, x);
         xmax = std::max(xmax, x);
@@ -341,7 +351,9 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
 
     std::vector<double2> rA(NS), rB(NS), rC(NS);
     std::vector<int32_t> perm(NS);
-    std::vector<double> zc(NG), qg(NG), z0(n_events), shift(n_events);
+    std::vector<double> zc(NG), qg(NG), z0(n_events), shift(n_events), qshift(n_events), udz(n_events);
+    std::vector<float> qn(NG);
+    std::vector<double> lm_lo(n_events), lm_hi(n_events);
     std::vector<int32_t> idx;
     for (int i = 0; i < n_events; ++i) {
         const int64_t s0 = so[i];
@@ -352,12 +364,16 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
         double sh = -INFINITY;   // factor the prior scale out of the weights: 1/pi_j = exp(sh) * ipr_j
         for (int j = 0; j < ns; ++j) sh = std::max(sh, -h_lp[s0 + j]);
         shift[i] = sh;
+        lm_lo[i] = INFINITY;
+        lm_hi[i] = -INFINITY;
         for (int j = 0; j < ns; ++j) {
             const int64_t o = s0 + idx[j];
+            lm_lo[i] = std::min(lm_lo[i], std::log(h_m1[o]));
+            lm_hi[i] = std::max(lm_hi[i], std::log(h_m1[o]));
             double q = h_m2[o] / h_m1[o];
             rA[s0 + j] = make_double2((std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0, h_m1[o]);
             rB[s0 + j] = make_double2(q, std::log(h_m1[o]));
-            rC[s0 + j] = make_double2(std::log(q), std::exp(-h_lp[o] - sh));
+            rC[s0 + j] = make_double2(std::log(q), -h_lp[o] - sh);   // ln(1/pi_j) with the event's scale removed
             perm[s0 + j] = idx[j];
         }
         const int64_t g0 = go[i];
@@ -369,6 +385,17 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
             zc[g0 + g] = h_z[g0 + g] - z0[i];
             qg[g0 + g] = h_p[g0 + g] * 0.5 * (wl + wr);   // composite trapezoid weight (O9)
         }
+        // q_g normalised by the event's largest value (kept in fp32; the scale returns in log I)
+        double qmax = 0.0;
+        for (int g = 0; g < nz; ++g) qmax = std::max(qmax, qg[g0 + g]);
+        if (!(qmax > 0.0)) qmax = 1.0;
+        qshift[i] = std::log(qmax);
+        for (int g = 0; g < nz; ++g) qn[g0 + g] = (float)(qg[g0 + g] / qmax);
+        // equally spaced grid?  then the KDE pair loop may take the power form
+        const double dz = (h_z[g0 + nz - 1] - h_z[g0]) / (nz - 1);
+        bool uniform = true;
+        for (int g = 0; g < nz && uniform; ++g) uniform = std::fabs(h_z[g0 + g] - (h_z[g0] + g * dz)) <= 1e-7 * dz;
+        udz[i] = uniform ? dz : 0.0;
     }
     // replace the previous set
     cudaStreamSynchronize(ctx->stream);
@@ -380,11 +407,15 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz;
     CK(upload(ctx->owned_ev, &E.sample_off, so)); CK(upload(ctx->owned_ev, &E.grid_off, go));
     CK(upload(ctx->owned_ev, &E.recA, rA)); CK(upload(ctx->owned_ev, &E.recB, rB)); CK(upload(ctx->owned_ev, &E.recC, rC));
-    CK(upload(ctx->owned_ev, &E.perm, perm)); CK(upload(ctx->owned_ev, &E.zc, zc)); CK(upload(ctx->owned_ev, &E.qg, qg));
+    CK(upload(ctx->owned_ev, &E.perm, perm)); CK(upload(ctx->owned_ev, &E.zc, zc)); CK(upload(ctx->owned_ev, &E.qn, qn));
+    CK(upload(ctx->owned_ev, &E.uni_dz, udz));
+    CK(upload(ctx->owned_ev, &E.lnm1_lo, lm_lo)); CK(upload(ctx->owned_ev, &E.lnm1_hi, lm_hi));
     CK(upload(ctx->owned_ev, &E.z0, z0));
     if (fixed_bw) CK(upload(ctx->owned_ev, &E.fixed_bw, h_bw));
     CK(upload(ctx->owned_ev, &ctx->ev_ln_shift, shift));
+    CK(upload(ctx->owned_ev, &ctx->ev_ln_qscale, qshift));
     ctx->ev = E;
+    ctx->ev_m_top = m_top;
     ctx->ev_grid = grid;
     ctx->h_sample_off = so;
     ctx->h_grid_off = go;
@@ -412,10 +443,11 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     CK(fetch(ctx, dL, N, h_dl)); CK(fetch(ctx, m1d, N, h_m1)); CK(fetch(ctx, m2d, N, h_m2)); CK(fetch(ctx, ln_pdraw, N, h_lp));
     if (!all_finite(h_dl) || !all_finite(h_m1) || !all_finite(h_m2) || !all_finite(h_lp))
         return fail(ctx, CHIM_EINVAL, "chim_init_injections: non-finite input");
-    double xmin = INFINITY, xmax = -INFINITY, sh = -INFINITY;
+    double xmin = INFINITY, xmax = -INFINITY, sh = -INFINITY, m_top = 0.0;
     for (size_t j = 0; j < N; ++j) {
         if (!(h_dl[j] > 0.0) || !(h_m2[j] > 0.0) || !(h_m1[j] >= h_m2[j]))
             return fail(ctx, CHIM_EINVAL, "chim_init_injections: need dL > 0 and m1d >= m2d > 0");
+        m_top = std::max(m_top, h_m1[j]);
         double x = std::log(h_dl[j]);
         xmin = std::min(xmin, x);
         xmax = std::max(xmax, x);
@@ -431,7 +463,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
         double q = h_m2[o] / h_m1[o];
         rA[j] = make_double2((std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0, h_m1[o]);
         rB[j] = make_double2(q, std::log(h_m1[o]));
-        rC[j] = make_double2(std::log(q), std::exp(-h_lp[o] - sh));
+        rC[j] = make_double2(std::log(q), -h_lp[o] - sh);
     }
     cudaStreamSynchronize(ctx->stream);
     free_pool(ctx->owned_inj);
@@ -444,6 +476,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     CK(upload(ctx->owned_inj, &I.recA, rA)); CK(upload(ctx->owned_inj, &I.recB, rB)); CK(upload(ctx->owned_inj, &I.recC, rC));
     CK(upload(ctx->owned_inj, &I.perm, idx));
     ctx->inj = I;
+    ctx->inj_m_top = m_top;
     ctx->inj_grid = grid;
     ctx->inj_ln_shift = sh;
     ctx->inj_blocks = (int)((n_det + kInjChunk - 1) / kInjChunk);
@@ -528,6 +561,7 @@ int chim_get_stats(chim_ctx* ctx, chim_stats* out) {
     unsigned long long s[4];
     CK(cudaMemcpy(s, ctx->stats, sizeof s, cudaMemcpyDeviceToHost));
     ctx->last.kde_pairs_evaluated = s[0];
+    ctx->last.kde_pairs_in_cutoff = s[1];
     *out = ctx->last;
     return CHIM_OK;
 }
@@ -578,7 +612,7 @@ static int debug_prepare(chim_ctx* ctx, const double* lambda, const char* who) {
     if (rc != CHIM_OK) return rc;
     TableParams TP = table_params(ctx);
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t), ctx->stream));
-    CK(launch_tables(lambda, 1, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->wtab, ctx->stream));
+    CK(launch_tables(lambda, 1, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, ctx->stream));
     return CHIM_OK;
 }
 
@@ -622,8 +656,8 @@ int chim_debug_injection_weights(chim_ctx* ctx, const double* lambda, double* s_
     if (!ctx->have_inj) return fail(ctx, CHIM_ESTATE, "chim_debug_injection_weights: no injections loaded");
     if (!s_out) return fail(ctx, CHIM_EINVAL, "chim_debug_injection_weights: null output");
     InjKernelParams IP{};
-    IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.wtab = ctx->wtab;
-    IP.n_lambda = 1; IP.tab_rows = ctx->inj_grid.rows(); IP.n_win = ctx->cfg.n_win_table; IP.chunk = kInjChunk;
+    IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.mtab = ctx->mtab;
+    IP.n_lambda = 1; IP.tab_rows = ctx->inj_grid.rows(); IP.n_mass = ctx->cfg.n_mass_table; IP.chunk = kInjChunk;
     IP.z_table_max = ctx->cfg.z_table_max; IP.z_cat_max = ctx->cfg.z_cat_max;
     IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = s_out;
     IP.dbg_scale = std::exp(ctx->inj_ln_shift);

@@ -13,6 +13,7 @@ constexpr double kCkms = 299792.458;       // speed of light [km/s]
 constexpr int kGLWin = 32;                 // Gauss-Legendre nodes for the normalisation integrals (S1)
 constexpr int kGLPanel = 8;                // Gauss-Legendre nodes per panel of the window table (S1)
 constexpr int kZPad = 32;                  // d_C table panels kept beyond z_table_max (stencil safety)
+constexpr double kLnFloor = -1.0e4;        // ln of "zero" in the log-space tables (exp underflows to the 1e-307 floor)
 constexpr double kHalfLog2e = 0.72134752044448170368;  // log2(e)/2 : exp(-d^2/2h^2) = 2^(-(d s)^2), s^2 = kHalfLog2e/h^2
 
 // Per-lambda constants written by the table kernel (S1), read by every other kernel.
@@ -36,6 +37,9 @@ struct LamConst {
     double dl_tabmax;   // d_L^gw(z_table_max)
     double Z1;          // normalisation of p(m1)
     double win_scale;   // n_win / delta_m
+    double inv_delta;   // 1 / delta_m
+    double lm0;         // mass table: node coordinate tm = (ln m1 - lm0) * inv_dlm + 1
+    double inv_dlm;
     uint32_t flags;     // CHIM_FLAG_LAMBDA_DOMAIN | CHIM_FLAG_DL_NONMONOTONE
     int32_t beta_is_m1; // |beta + 1| < 1e-12 : log form of the power integral
 };
@@ -60,32 +64,34 @@ struct DlGrid {
 struct TableParams {
     double z_table_max, z_cat_max;
     int32_t n_table, n_win, placement;
+    int32_t n_mass;      // intervals of the per-lambda mass table (in ln m1)
+    double ln_m_top;     // ln of the largest detector-frame m1 of the loaded sets (upper end of the mass table)
     DlGrid ev, inj;
 };
 
-// exp(x) in fp64 for the sample kernels: argument clamped to [-700, 700] (e^-700 ~ 1e-304 stands in for 0,
-// nothing on this path needs more), Cody-Waite reduction x = n ln2 + r with |r| <= ln2/2, degree-11 Taylor
-// polynomial in Horner form (relative error < 1e-14), scaling by 2^n through the exponent field.  Branch-free;
-// the coefficients live in constant memory so that DFMA takes them as direct operands.
-static __constant__ double c_exp_coef[12] = {
-    2.50521083854417187751e-08, 2.75573192239858906526e-07, 2.75573192239858906526e-06, 2.48015873015873015873e-05,
-    1.98412698412698412698e-04, 1.38888888888888888889e-03, 8.33333333333333333333e-03, 4.16666666666666666667e-02,
-    1.66666666666666666667e-01, 0.5, 1.0, 1.0};
-static __constant__ double c_exp_red[5] = {1.4426950408889634074, 6755399441055744.0 /* 1.5 * 2^52 */,
-                                           -6.93147180369123816490e-01, -1.90821492927058770002e-10, 700.0};
+// One interval of the per-lambda mass table in y = ln m1: cubics (local coordinate t in [0,1)) of
+//   a: ln[ p(m1)/S(m1) * m1'^2 S(m1)/C(m1) ]  with the power law present (m1 <= m_high),  m1' = m1 - m_low
+//   b: the same with the Gaussian component only (m1 > m_high)
+// i.e. ln of  p(m1) / C(m1) * m1'^2  -- smooth and finite on [m_low, inf) because C/S ~ rho m1'^2 (M3/M4).
+struct __align__(16) MassRow {
+    double a[4], b[4];
+};
 
-__device__ __forceinline__ double fast_exp(double x) {
-    x = (x > -c_exp_red[4]) ? x : -c_exp_red[4];       // cheap clamps (no NaN canonicalisation): inputs are finite
-    x = (x < c_exp_red[4]) ? x : c_exp_red[4];
-    double t = fma(x, c_exp_red[0], c_exp_red[1]);     // round-to-nearest integer by the magic-number addition
+// exp(x) for the sample kernels: fp64 range reduction x log2(e) = n + f, |f| <= 1/2 (exact in fp64), MUFU.EX2 on
+// the fp32 remainder (relative error <= 2.4e-7), 2^n through the exponent field.  |x| must stay
+// below ~1e9 (the magic-number rounding) -- every caller bounds its argument; n is clamped so that the result never
+// leaves the normal range: e^-707 ~ 1e-307 stands in for 0.
+__device__ __forceinline__ double exp_mufu(double x) {
+    const double y = x * 1.4426950408889634074;
+    const double t = y + 6755399441055744.0;            // 1.5 * 2^52: round to nearest integer
     int n = __double2loint(t);
-    double fn = t - c_exp_red[1];
-    double r = fma(fn, c_exp_red[2], x);
-    r = fma(fn, c_exp_red[3], r);
-    double p = c_exp_coef[0];
-#pragma unroll
-    for (int i = 1; i < 12; ++i) p = fma(p, r, c_exp_coef[i]);
-    return p * __hiloint2double((n + 1023) << 20, 0);  // |n| <= 1010: 2^n is a normal double
+    const double fn = t - 6755399441055744.0;
+    const float f = (float)(y - fn);
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(f));
+    n = max(-1020, min(n, 1020));
+    const double ed = (double)e;                        // in [0.70, 1.42]
+    return __hiloint2double(__double2hiint(ed) + (n << 20), __double2loint(ed));
 }
 
 // 1/x for finite non-zero normal x: MUFU.RCP64H seed + two Newton steps (error ~1e-16), no special cases.
@@ -102,70 +108,79 @@ __device__ __forceinline__ double horner3(const double* c, double t) {
     return fma(fma(fma(c[3], t, c[2]), t, c[1]), t, c[0]);
 }
 
-// Smoothing denominator 1/S(m) = 1 + exp(f(m')), f = delta/m' + delta/(m'-delta) = delta (2m'-delta)/(m'(m'-delta))
-// (M1), for m' = m - m_low clamped strictly inside the window so that the expression is finite for every lane
-// (lanes outside the window discard the value).
-__device__ __forceinline__ double smooth_den(double mp, const LamConst& L) {
-    const double lo = L.delta * 1e-6, hi = L.delta * (1.0 - 1e-12);
-    double mpc = (mp > lo) ? mp : lo;
-    mpc = (mpc < hi) ? mpc : hi;
-    double f = L.delta * (2.0 * mpc - L.delta) * fast_rcp(mpc * (mpc - L.delta));
-    return 1.0 + fast_exp(f);
+// Where a thread finds the per-lambda mass table: rows [lo, lo + cap) of the "a" variant staged in shared memory as
+// two split arrays (16-byte halves: the layout with the fewest bank conflicts for scattered rows), everything else
+// (rows outside the staged range, the Gaussian-only "b" variant beyond m_high) in global memory.
+struct MassLookup {
+    const MassRow* g;          // [n_mass + 2] rows of this lambda
+    const double2* sA;         // staged {a[0], a[1]} or null
+    const double2* sB;         // staged {a[2], a[3]}
+    int lo, cap, n_mass;
+};
+
+__device__ __forceinline__ double2 ldg256_lo(const double* p, double2& hi) {   // one 256-bit read-only load
+    double2 lo;
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(lo.x), "=d"(lo.y), "=d"(hi.x), "=d"(hi.y) : "l"(p));
+    return lo;
 }
 
-// Inside the window both S(m1) and C(m1) = int_{m_low}^{m1} m^beta S(m) dm (M3/M4) vanish faster than any power
-// at m_low, so the table holds the smooth ratio rho(m') = C / (S m'^2) (rho -> m_low^beta/delta_m as m' -> 0,
-// rho(delta_m) = W_c/delta_m^2): S(m1)/C(m1) = 1/(rho m'^2) and S(m1) cancels analytically in the weight.
-// Cubic Lagrange on uniform nodes.
-__device__ __forceinline__ double rho_window(double mp, const LamConst& L, const double* __restrict__ rtab, int n_win) {
-    double x = mp * L.win_scale;
-    int b = (int)x - 1;
-    b = max(0, min(b, n_win - 3));
-    double s = x - (double)b;   // in [0, 3]
-    double s1 = s - 1.0, s2 = s - 2.0, s3 = s - 3.0;
-    double l0 = -s1 * s2 * s3 * (1.0 / 6.0), l1 = s * s2 * s3 * 0.5, l2 = -s * s1 * s3 * 0.5, l3 = s * s1 * s2 * (1.0 / 6.0);
-    return l0 * rtab[b] + l1 * rtab[b + 1] + l2 * rtab[b + 2] + l3 * rtab[b + 3];
-}
-
-// Steps S2 / S5 for one sample (or injection): redshift from the table, source-frame masses, population
-// weight.  `ipr` = 1/pi_j (events) or 1/p_draw,j (injections); R carries psi/J (and u_vol for injections).
-//   PAPER.md:52 (d_L -> z, m = m^d/(1+z)), :195-198 eq. 20 + M1-M4 (mass model), :226 eq. 21, :75 eq. 11.
-// Written without data-dependent branches (selects only): the lanes of a warp hold samples on both sides of
-// every mass-function edge, so branches would serialise the exponentials.
+// Steps S2 / S5 for one sample (or injection): redshift from the table, source-frame masses, population weight
+//   w = p(m1, m2 | lambda_m) * R(z) / prior,   p(m1,m2) = p(m1) m2^beta S(m2) / C(m1)     (M1-M4)
+// assembled in log space from two table look-ups:
+//   ln w' = LQ(ln m1) + beta ln m2 + ln R + ln(1/prior),   w = exp(ln w') S(m2) / m1'^2
+//   LQ   per-lambda mass table (MassRow): ln[p(m1)/C(m1) m1'^2], smooth on [m_low, inf)
+//   S(m2) = 1/(1 + exp(delta/m2' + delta/(m2' - delta))) inside the window, 1 above (M1)
+//   ln R, z, ln(1+z), 1/(1+z): the four cubics of the sample's row of the z(ln d_L) table
+//   PAPER.md:52 (d_L -> z, m = m^d/(1+z)), :195-198 eq. 20 (mass model), :226 eq. 21, :75 eq. 11.
+// Two exponentials (MUFU.EX2 on fp64-reduced arguments) and two reciprocals per sample; selects instead of
+// data-dependent branches, except the (rare) fall-back of the mass row to global memory.
 __device__ __forceinline__ void sample_weight(const LamConst& L, const Row* __restrict__ tab, int n_rows,
-                                              const double* __restrict__ wtab, int n_win, double tkmax,
-                                              double z_table_max, double tk, double m1d, double q, double lnm1d,
-                                              double lnq, double ipr, double& z, double& w, bool& out_of_range) {
+                                              const MassLookup& M, double tkmax, double z_table_max,
+                                              double tk, double m1d, double q, double lnm1d, double lnq, double lnipr,
+                                              double& z, double& w, bool& out_of_range) {
     out_of_range = !(tk <= tkmax);
     int k = (int)((tk < (double)(n_rows - 2)) ? tk : (double)(n_rows - 2));
     k = max(1, k);
     double t = tk - (double)k;
-    const double2* rp = reinterpret_cast<const double2*>(tab + k);   // 8 x 128-bit loads of one 128-byte row
-    double2 c0 = rp[0], c1 = rp[1], c2 = rp[2], c3 = rp[3], c4 = rp[4], c5 = rp[5], c6 = rp[6], c7 = rp[7];
+    const double* rp = reinterpret_cast<const double*>(tab + k);     // 4 x 256-bit loads of one 128-byte row
+    double2 c0, c1, c2, c3, c4, c5, c6, c7;
+    c0 = ldg256_lo(rp, c1);
+    c2 = ldg256_lo(rp + 4, c3);
+    c4 = ldg256_lo(rp + 8, c5);
+    c6 = ldg256_lo(rp + 12, c7);
     double zt = fma(fma(fma(c1.y, t, c1.x), t, c0.y), t, c0.x);
     double u = fma(fma(fma(c3.y, t, c3.x), t, c2.y), t, c2.x);
     double a = fma(fma(fma(c5.y, t, c5.x), t, c4.y), t, c4.x);
-    double R = fma(fma(fma(c7.y, t, c7.x), t, c6.y), t, c6.x);
+    double lnR = fma(fma(fma(c7.y, t, c7.x), t, c6.y), t, c6.x);
     z = out_of_range ? z_table_max : zt;
-    double m1 = m1d * a, m2 = q * m1;
-    double lm1 = lnm1d - u, lm2 = lm1 + lnq;
-    double bl2 = L.beta * lm2;                                      // ln m2^beta
-    double dm = m1 - L.mu;
-    double e = fast_exp(L.a_g - dm * dm * L.inv2s2 + bl2);          // lambda_g N(m1) m2^beta / Z1
-    double epl = fast_exp(L.a_pl - L.alpha * lm1 + bl2);            // (1-lambda_g) PL(m1) m2^beta / Z1
-    e += (m1 <= L.m_high) ? epl : 0.0;
-    double mp1 = m1 - L.m_low, mp2 = m2 - L.m_low;
-    double den2 = smooth_den(mp2, L);
-    double den = (mp2 < L.delta) ? den2 : 1.0;                      // 1/S(m2)
-    // C(m1): above the window W_c + closed-form power integral; inside, rho m'^2 (S(m1) cancelled)
-    double pw = L.beta_is_m1 ? (lm1 - L.ln_mc) : (fast_exp(L.bp1 * lm1) - L.pow_mc_bp1) * L.inv_bp1;
-    double mp1c = (mp1 > 0.0) ? mp1 : 0.0;
-    mp1c = (mp1c < L.delta) ? mp1c : L.delta;
-    double cw = rho_window(mp1c, L, wtab, n_win) * mp1c * mp1c;
-    double C = (mp1 < L.delta) ? cw : L.W_c + pw;
-    double dc = den * C;
-    bool ok = !out_of_range && (m2 >= L.m_low) && (dc > 1e-300) && (dc < 1e300);   // R15 support; underflowed S or C
-    w = ok ? e * R * ipr * fast_rcp(ok ? dc : 1.0) : 0.0;
+    const double m1 = m1d * a, m2 = q * m1;
+    const double lm1 = lnm1d - u, lm2 = lm1 + lnq;
+    const double mp1 = m1 - L.m_low, mp2 = m2 - L.m_low;
+    // mass table
+    double tm = fma(lm1 - L.lm0, L.inv_dlm, 1.0);
+    int km = max(1, min((int)tm, M.n_mass));
+    tm -= (double)km;
+    double2 d0, d1;
+    const int ks = km - M.lo;
+    if ((unsigned)ks < (unsigned)M.cap && m1 <= L.m_high) {
+        d0 = M.sA[ks];
+        d1 = M.sB[ks];
+    } else {
+        d0 = ldg256_lo(reinterpret_cast<const double*>(M.g + km) + ((m1 <= L.m_high) ? 0 : 4), d1);
+    }
+    double lnw = fma(fma(fma(d1.y, tm, d1.x), tm, d0.y), tm, d0.x);
+    lnw += fma(L.beta, lm2, lnR + lnipr);
+    // smoothing of m2 (M1): f = delta (2 m' - delta) / (m' (m' - delta)), m' clamped strictly inside the window
+    const double lo = L.delta * 1e-3, hi = L.delta * (1.0 - 1e-12);   // S(m' < 1e-3 delta) < e^-998: "0" either way
+    double mc = (mp2 > lo) ? mp2 : lo;
+    mc = (mc < hi) ? mc : hi;
+    const double f = L.delta * (2.0 * mc - L.delta) * fast_rcp(mc * (mc - L.delta));
+    const double S2 = fast_rcp(1.0 + exp_mufu(f));
+    const double r1 = fast_rcp((mp1 > 0.0) ? mp1 : 1.0);
+    double v = exp_mufu(lnw) * (r1 * r1);
+    v = (mp2 < L.delta) ? v * S2 : v;
+    const bool ok = !out_of_range && (mp2 > 0.0);      // R15 support: m_low < m2 (<= m1)
+    w = ok ? v : 0.0;
 }
 
 // ---- small reductions ---------------------------------------------------------------------------------
@@ -207,8 +222,11 @@ struct EventSetDev {
     const double2* recC;        // {ln q, 1/pi}
     const int32_t* perm;        // sorted position -> caller's index within the event
     const double* zc;           // z_g - z0_i  (centred grid)
-    const double* qg;           // p_gal(z_g) * trapezoid weight
+    const float* qn;            // p_gal(z_g) * trapezoid weight / (the event's largest such product)
+    const double* uni_dz;       // [n_events] grid spacing if the event's grid is equally spaced, else 0
     const double* z0;           // [n_events] centre of each event's grid
+    const double* lnm1_lo;      // [n_events] smallest / largest ln m1d of the event's samples
+    const double* lnm1_hi;
     const double* fixed_bw;     // [n_events] or null
 };
 
@@ -216,15 +234,16 @@ struct EventKernelParams {
     EventSetDev ev;
     const LamConst* Lc;      // [n_lambda]
     const Row* tab;          // [n_lambda][rows]
-    const double* wtab;      // [n_lambda][n_win+1]  rho(m') nodes
+    const MassRow* mtab;     // [n_lambda][n_mass+2]
     const double* dc_tab;    // [n_lambda][n_table+1+kZPad] (placement ON_GRID only) or null
-    int32_t n_lambda, tab_rows, n_win, n_table;
-    int32_t placement, bw_rule;
+    int32_t n_lambda, tab_rows, n_mass, n_table;
+    int32_t placement, bw_rule, kde_method;
     double z_table_max, cutoff;
     double* logI;            // [n_lambda][n_events]
     uint32_t* flags;         // [n_lambda]
-    unsigned long long* stats;  // [0] evaluated pairs
+    unsigned long long* stats;  // [0] executed pairs (incl. band padding), [1] pairs inside the cut-off
     const double* ln_shift;  // [n_events] prior scale factored out of the weights, added back to log I
+    const double* ln_qscale; // [n_events] ln of the event's largest q_g (qn = q / that), added back to log I
     // diagnostics (single event, single lambda) -- null in the hot path
     int32_t dbg_event;       // >= 0: blockIdx.x addresses lambda only, event = dbg_event
     double* dbg_z; double* dbg_w; double* dbg_h; double* dbg_K;
@@ -239,8 +258,8 @@ struct InjSetDev {
 
 struct InjKernelParams {
     InjSetDev inj;
-    const LamConst* Lc; const Row* tab; const double* wtab;
-    int32_t n_lambda, tab_rows, n_win, chunk;  // chunk = injections per block
+    const LamConst* Lc; const Row* tab; const MassRow* mtab;
+    int32_t n_lambda, tab_rows, n_mass, chunk;  // chunk = injections per block
     double z_table_max, z_cat_max;
     double2* partial;        // [n_blocks][n_lambda] {sum s, sum s^2}
     uint32_t* flags;
@@ -259,7 +278,8 @@ struct CombineParams {
 
 // host-callable launchers (defined in the .cu files)
 cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P, LamConst* Lc, double* dc_tab,
-                          Row* tab_ev, Row* tab_inj, double* wtab, cudaStream_t st);
+                          Row* tab_ev, Row* tab_inj, MassRow* mtab, cudaStream_t st);
+
 cudaError_t launch_events(const EventKernelParams& P, cudaStream_t st);
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st);
 cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);
@@ -269,5 +289,6 @@ cudaError_t upload_gauss_legendre();   // fills the __constant__ node tables use
 cudaError_t measure_alu_peaks(int n_sm, int reps, cudaStream_t st, double out_g[4]);
 size_t events_smem_bytes(int max_ns, int max_nz);
 size_t tables_smem_bytes(const TableParams& P);
+size_t inject_smem_bytes(int n_mass);
 
 }  // namespace chim

@@ -3,32 +3,51 @@
 //   S2  per posterior sample: z_j from the per-lambda table, source masses, population weight w_j
 //       (sample_weight, chim_internal.cuh), weighted moments -> Scott bandwidth h (R3), all in fp64.
 //       z_j and w_j never leave shared memory.
-//   S3  Gaussian KDE on the event's redshift grid (eq. 19, R2): grid points in registers (one per
-//       lane, 32-point tiles), samples broadcast from shared memory two per 128-bit load, fp32 FFMA +
-//       MUFU.EX2 + FADD per pair (expanded square around the tile centre, log2 w_j folded into the per-sample
-//       constant), fp32 partial sums over <= 256 samples flushed into fp64.  Samples are sorted
-//       in z (they are sorted in d_L at init and d_L^gw is monotone), so each tile only visits the samples within
-//       t*h of it (R9).  Work items are (tile, 256-sample chunk), handed to warps through a shared counter so
-//       that the CTA's tail stays short.
-//   S4  I_i = sum_g K(z_g) q_g, q_g = p_gal(z_g) x trapezoid weight (eq. 14): warp shuffles +
-//       block reduction in fp64, log I_i written per (lambda, event).
+//   S3+S4  I_i = sum_g q_g K(z_g) = (1/(N_s h sqrt(2 pi))) sum_j w_j A_j,  A_j = sum_g q_g exp(-(z_g - z_j)^2 / 2h^2),
+//       q_g = p_gal(z_g) x trapezoid weight (eq. 19 evaluated on the grid, eq. 14).
+//       Samples in lanes (4 per lane, 128 per warp pass, sorted in z), grid points streamed from shared memory;
+//       a pass visits the grid band within t*h of its samples (R9).  Two formulations of the Gaussian:
+//
+//       power form (equally spaced grid): with x = z sqrt(log2(e)/2)/h, delta the grid spacing in
+//       x, block start x_a, u = x_a - x_j and g = aB + b:
+//           2^-(x_g - x_j)^2 = 2^(-u^2) * (2^(-2 delta u))^b * 2^(-b^2 delta^2)
+//       so per block of B grid points  sum_b q_g E_gj = e0 * sum_b q'_b s^b  with q'_b = q_g 2^(-b^2 delta^2)
+//       precomputed per CTA: a Horner polynomial in s -- ONE fp32 FMA per pair, issued as packed FFMA2 (two
+//       samples per instruction), and two MUFU.EX2 (e0, s) per sample and block.  Exact up to fp32 rounding
+//       (no recurrence across blocks: every block restarts from fresh exponentials).
+//
+//       direct form (any grid; also bandwidths below ~3 grid spacings, no cut-off, diagnostics):
+//           A_j += q_g * ex2(-(x_g - x_j)^2)   FADD, FMUL, MUFU.EX2, FFMA per pair.
+//
+//   log I_i written per (lambda, event); block reductions in fp64.
 #include "chim_internal.cuh"
 
 namespace chim {
 
 constexpr int kEvThreads = 256;
-constexpr int kFlush = 256;   // samples per work item = length of one fp32 partial sum before it goes to fp64
-constexpr float kMaxHalfWidth = 2.5f;   // widest tile (half width, scaled units) handled by the expanded-square loop
+constexpr int kPass = 128;               // samples per warp pass (4 per lane)
+constexpr float kMaxBlockSpan = 4.8f;    // B * delta limit of the power form
+constexpr float kMaxPowExp = 100.f;      // bound on log2 of the largest s^b inside a block (fp32 overflow guard)
+constexpr int kMassStage = 384;          // mass-table rows staged per CTA during S2 (aliases the grid array of S3)
 
-__device__ __forceinline__ float lg2_approx(float x) {
-    float y;
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
+}
+typedef unsigned long long f32x2;        // two packed floats (lo, hi) for the FFMA2 pipe
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
 }
 
 // psi(z)/J(z) at a grid point for placement ON_GRID (paper eq. 14 literally); d_C from the global table.
@@ -50,31 +69,64 @@ __device__ double grid_factor(const LamConst& L, const double* __restrict__ dc, 
     return psi / (a * a * a * fabs(ddl));
 }
 
-// the float region after wbuf holds zf[ns_pad] during S2 and the per-warp scratch (kFlush float2 per warp) afterwards
-__host__ __device__ inline size_t ev_float_region(size_t ns_pad) {
-    size_t scratch = (size_t)(kEvThreads / 32) * kFlush * 2;
-    return ns_pad > scratch ? ns_pad : scratch;
-}
 struct EvSmem {
     LamConst L;
     double red[4 * (kEvThreads / 32)];
-    int item_counter;
-    int n_items;
+    int pass_counter;
+    int pad_;
 };
 
-// shared-memory layout after EvSmem: wbuf double[max_ns] (re-used in place as float2 pk[max_ns]) | zf float[max_ns] |
-// tile_jlo int[max_tiles] | tile_jhi int[max_tiles] | tile_cum int[max_tiles + 1]
+__host__ __device__ inline size_t ev_ns_pad(size_t ns) { return (ns + kPass - 1) / kPass * kPass; }
+__host__ __device__ inline size_t ev_nz_pad(size_t nz) { return (nz + 31) / 32 * 32; }
+__host__ __device__ inline size_t ev_aux_bytes(size_t nz) {   // S2: staged mass rows; S3: (q', q') or (x_g, q_g) per grid point
+    size_t a = sizeof(float2) * ev_nz_pad(nz), b = (size_t)kMassStage * 32;
+    return a > b ? a : b;
+}
+
+// One block of B grid points for the 4 samples of a lane: tot_k += 2^(-u_k^2) * sum_b q'_b s_k^b (Horner, FFMA2).
+template <int B>
+__device__ __forceinline__ void power_block(const ulonglong2* __restrict__ qp, float xs, float cs, const float (&x)[4],
+                                            f32x2& tot01, f32x2& tot23) {
+    const float u0 = xs - x[0], u1 = xs - x[1], u2 = xs - x[2], u3 = xs - x[3];
+    const f32x2 s01 = pack2(ex2_approx(cs * u0), ex2_approx(cs * u1));
+    const f32x2 s23 = pack2(ex2_approx(cs * u2), ex2_approx(cs * u3));
+    const f32x2 e01 = pack2(ex2_approx(-u0 * u0), ex2_approx(-u1 * u1));
+    const f32x2 e23 = pack2(ex2_approx(-u2 * u2), ex2_approx(-u3 * u3));
+    f32x2 a01 = 0ull, a23 = 0ull;     // (+0.f, +0.f)
+#pragma unroll
+    for (int i = B / 2 - 1; i >= 0; --i) {
+        const ulonglong2 v = qp[i];   // {(q'_2i, q'_2i), (q'_2i+1, q'_2i+1)}
+        a01 = fma2(a01, s01, v.y);
+        a23 = fma2(a23, s23, v.y);
+        a01 = fma2(a01, s01, v.x);
+        a23 = fma2(a23, s23, v.x);
+    }
+    tot01 = fma2(e01, a01, tot01);
+    tot23 = fma2(e23, a23, tot23);
+}
+
+template <int B>
+__device__ __forceinline__ void power_pass(const float2* __restrict__ gq, int a_lo, int a_hi, float xfirst, float delta,
+                                           const float (&x)[4], float (&A)[4]) {
+    f32x2 tot01 = 0ull, tot23 = 0ull;
+    const float cs = -2.f * delta;
+#pragma unroll 1
+    for (int a = a_lo; a <= a_hi; ++a) {
+        const float xs = fmaf((float)(a * B), delta, xfirst);
+        power_block<B>(reinterpret_cast<const ulonglong2*>(gq + a * B), xs, cs, x, tot01, tot23);
+    }
+    unpack2(tot01, A[0], A[1]);
+    unpack2(tot23, A[2], A[3]);
+}
+
+// shared-memory layout after EvSmem: wbuf double[ns_pad] | zf float[ns_pad] | aux = gq float2[nz_pad] / staged mass rows
 __global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     EvSmem& S = *reinterpret_cast<EvSmem*>(smem_raw);
     double* wbuf = reinterpret_cast<double*>(smem_raw + ((sizeof(EvSmem) + 15) / 16) * 16);
-    const int ns_pad = (P.ev.max_ns + 3) & ~3;
+    const size_t ns_pad = ev_ns_pad(P.ev.max_ns);
     float* zf = reinterpret_cast<float*>(wbuf + ns_pad);
-    const int max_tiles = (P.ev.max_nz + 31) / 32;
-    int* tile_jlo = reinterpret_cast<int*>(zf + ev_float_region(ns_pad));
-    int* tile_jhi = tile_jlo + max_tiles;
-    int* tile_cum = tile_jhi + max_tiles;
-    float2* pk = reinterpret_cast<float2*>(wbuf);   // aliases wbuf slot j (same thread reads then writes slot j)
+    float2* gq = reinterpret_cast<float2*>(zf + ns_pad);
     const int tid = threadIdx.x, lane = tid & 31;
 
     int l, ev;
@@ -89,7 +141,7 @@ __global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
         const uint32_t* src = reinterpret_cast<const uint32_t*>(P.Lc + l);
         uint32_t* dst = reinterpret_cast<uint32_t*>(&S.L);
         for (int i = tid; i < nw; i += kEvThreads) dst[i] = src[i];
-        if (tid == 0) S.item_counter = 0;
+        if (tid == 0) S.pass_counter = 0;
     }
     __syncthreads();
     const LamConst& L = S.L;
@@ -98,8 +150,33 @@ __global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
         return;
     }
     const Row* tab = P.tab + (size_t)l * P.tab_rows;
-    const double* wtab = P.wtab + (size_t)l * (P.n_win + 1);
     const double z0 = P.ev.z0[ev];
+
+    // ---- stage the mass-table rows this event can address: ln m1 = ln m1d - ln(1+z), z between the event's first and
+    //      last (sorted) sample; rows outside the staged range fall back to global memory inside sample_weight ----------
+    MassLookup M;
+    M.g = P.mtab + (size_t)l * (P.n_mass + 2);
+    M.n_mass = P.n_mass;
+    M.cap = kMassStage;
+    {
+        double2* sA = reinterpret_cast<double2*>(gq);
+        double2* sB = sA + kMassStage;
+        const int ka = max(1, min((int)P.ev.recA[s0].x, P.tab_rows - 2)), kb = max(1, min((int)P.ev.recA[s0 + ns - 1].x, P.tab_rows - 2));
+        const double u_lo = tab[ka].c[1][0], u_hi = tab[kb + 1].c[1][0];      // ln(1+z) at the bracketing nodes
+        const int ma = max(1, min((int)fma(P.ev.lnm1_lo[ev] - u_hi - L.lm0, L.inv_dlm, 1.0), P.n_mass));
+        const int mb = max(1, min((int)fma(P.ev.lnm1_hi[ev] - u_lo - L.lm0, L.inv_dlm, 1.0), P.n_mass));
+        M.lo = ma + max(0, (mb - ma + 1 - kMassStage) / 2);                   // wider than the stage: keep the centre
+        for (int i = tid; i < kMassStage; i += kEvThreads) {
+            const int r = min(M.lo + i, P.n_mass + 1);
+            double2 hi;
+            const double2 lo = ldg256_lo(reinterpret_cast<const double*>(M.g + r), hi);
+            sA[i] = lo;
+            sB[i] = hi;
+        }
+        M.sA = sA;
+        M.sB = sB;
+    }
+    __syncthreads();
 
     // ---- S2: weights + centred moments -----------------------------------------------------------------
     double mom[4] = {0.0, 0.0, 0.0, 0.0};   // sum w, sum w^2, sum w z', sum w z'^2
@@ -109,7 +186,7 @@ __global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
         double2 A = P.ev.recA[s0 + j], B = P.ev.recB[s0 + j], C = P.ev.recC[s0 + j];
         double z, w;
         bool o;
-        sample_weight(L, tab, P.tab_rows, wtab, P.n_win, L.tkmax_ev, P.z_table_max, A.x, A.y, B.x, B.y, C.x, C.y, z, w, o);
+        sample_weight(L, tab, P.tab_rows, M, L.tkmax_ev, P.z_table_max, A.x, A.y, B.x, B.y, C.x, C.y, z, w, o);
         oor |= (int)o;
         double zc = z - z0;
         zf[j] = (float)zc;
@@ -155,141 +232,159 @@ __global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
         if (P.dbg_K) for (int g = tid; g < nz; g += kEvThreads) P.dbg_K[g] = NAN;
         return;
     }
-    const double sc = sqrt(kHalfLog2e) / h;   // x = z' * sc  =>  exp(-d^2/2h^2) = 2^(-(dx)^2)
-    const double wscale = (double)ns / sw;    // weights normalised to mean 1 before rounding to fp32
+
+    // ---- scaled coordinates x = z' sqrt(log2(e)/2)/h: exp(-d^2/2h^2) = 2^(-dx^2) --------------------------------
+    const double sc = sqrt(kHalfLog2e) / h;
     const float scf = (float)sc;
-    for (int j = tid; j < ns; j += kEvThreads) {   // pk[j] = {x_j, log2 of the normalised weight}; log2(0) = -inf
-        float x = zf[j] * scf;
-        double w = wbuf[j];
-        pk[j] = make_float2(x, lg2_approx((float)(w * wscale)));
-    }
-    __syncthreads();   // zf is dead from here on: its storage becomes the per-warp scratch of the pair loop
-
-    // ---- tile windows, in parallel: tile t = grid points [32t, 32t+32), samples with x_j in [x_lo - T, x_hi + T] --
+    const double scd = (double)scf;             // samples and grid are scaled by the SAME rounded factor
+    const double wscale = (double)ns / sw;      // weights normalised to mean 1
     const float T = (P.cutoff > 0.0) ? (float)(P.cutoff * sqrt(kHalfLog2e)) : INFINITY;
-    const int n_tiles = (nz + 31) / 32;
     const double* zc_g = P.ev.zc + g0;
-    const double* q_g = P.ev.qg + g0;
-    unsigned long long pairs = 0;
-    for (int t = tid; t < n_tiles; t += kEvThreads) {
-        int j_lo = 0, j_hi = ns;
-        if (T < INFINITY) {
-            const float lo_key = (float)zc_g[t * 32] * scf - T, hi_key = (float)zc_g[min(t * 32 + 31, nz - 1)] * scf + T;
-            int a = 0, b = ns;
-            while (a < b) { int m = (a + b) >> 1; if (pk[m].x < lo_key) a = m + 1; else b = m; }
-            j_lo = a;
-            b = ns;
-            while (a < b) { int m = (a + b) >> 1; if (pk[m].x <= hi_key) a = m + 1; else b = m; }
-            j_hi = max(a, j_lo);
-        }
-        tile_jlo[t] = j_lo;
-        tile_jhi[t] = j_hi;
-        pairs += (unsigned long long)(j_hi - j_lo) * 32ull;
+    const float* qn_g = P.ev.qn + g0;
+    const double udz = P.ev.uni_dz[ev];
+    const float delta = (float)(udz * scd), xfirst = (float)(zc_g[0] * scd);
+    int Bsel = 0;                                // 0 = direct form
+    if (udz > 0.0 && T < INFINITY && P.kde_method == CHIM_KDE_AUTO && !P.dbg_K) {
+        if (delta * 32.f <= 3.3f) Bsel = 32;
+        else if (delta * 16.f <= kMaxBlockSpan) Bsel = 16;
     }
-    __syncthreads();
-    if (tid < 32) {   // exclusive scan of the chunk counts (warp 0)
-        int run = 0;
-        for (int base = 0; base < n_tiles; base += 32) {
-            int t = base + lane;
-            int c = (t < n_tiles) ? (tile_jhi[t] - tile_jlo[t] + kFlush - 1) / kFlush : 0;
-            int inc = c;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-            if (t < n_tiles) tile_cum[t] = run + inc - c;
-            run += __shfl_sync(0xffffffffu, inc, 31);
+    const int nzp = (int)ev_nz_pad(nz);
+    const bool on_grid = P.placement == CHIM_ON_GRID;
+    for (int g = tid; g < nzp; g += kEvThreads) {
+        float q = 0.f, xg = 0.f;
+        if (g < nz) {
+            q = qn_g[g];
+            if (on_grid)
+                q = (float)((double)q * grid_factor(L, P.dc_tab + (size_t)l * (P.n_table + 1 + kZPad), P.n_table + 1 + kZPad,
+                                                    P.z_table_max / P.n_table, zc_g[g] + z0));
+            xg = (float)(zc_g[g] * scd);
         }
-        if (lane == 0) { tile_cum[n_tiles] = run; S.n_items = run; }
+        if (Bsel) {
+            const float bd = (float)(g & (Bsel - 1)) * delta;
+            q *= ex2_approx(-bd * bd);
+            gq[g] = make_float2(q, q);
+        } else {
+            gq[g] = make_float2(xg, q);
+        }
     }
     __syncthreads();
 
-    // ---- S3 + S4: work items = (tile, chunk of <= kFlush samples), one grid point per lane ----------------
-    // With c the tile centre, x' = x - c:  -(xg - xj)^2 + log2 w_j = -xg'^2 + [ xg' (2 xj') + (log2 w_j - xj'^2) ].
-    // The warp first writes {2 xj', log2 w_j - xj'^2} for its chunk into its scratch, so that the pair loop is
-    // FFMA (argument) -> MUFU.EX2 -> FADD per pair; the lane factor 2^(-xg'^2) is applied once per item.  Tiles
-    // wider than kMaxHalfWidth (in units of h sqrt(2 ln 2)) -- a bandwidth far below the grid spacing -- take the
-    // direct path, where the products would lose fp32 precision.
-    const int n_items = S.n_items;
-    float2* scratch = reinterpret_cast<float2*>(zf) + (tid >> 5) * kFlush;
-    const float4* scratch4 = reinterpret_cast<const float4*>(scratch);
-    double lsum = 0.0;                 // this lane's sum over its (g, j) pairs of w_j e_gj q_g
+    // ---- S3 + S4: warp passes over 128 consecutive (sorted) samples ----------------------------------------
+    const int n_pass = (ns + kPass - 1) / kPass;
+    const float inv_delta = (udz > 0.0) ? 1.f / delta : 0.f;
+    double lsum = 0.0;                          // this lane's sum_j w_j A_j
+    unsigned long long pairs_exec = 0, pairs_cut = 0;
     for (;;) {
-        int item = 0;
-        if (lane == 0) item = atomicAdd(&S.item_counter, 1);
-        item = __shfl_sync(0xffffffffu, item, 0);
-        if (item >= n_items) break;
-        int a = 0, b = n_tiles;        // largest tile with tile_cum[tile] <= item
-        while (b - a > 1) { int m = (a + b) >> 1; if (tile_cum[m] <= item) a = m; else b = m; }
-        const int tile = a;
-        const int jb = tile_jlo[tile] + (item - tile_cum[tile]) * kFlush;
-        const int je = min(jb + kFlush, tile_jhi[tile]);
-        const int g = tile * 32 + lane;
-        const bool valid = g < nz;
-        const float xg = (float)zc_g[valid ? g : nz - 1] * scf;
-        const float x_lo = __shfl_sync(0xffffffffu, xg, 0), x_hi = __shfl_sync(0xffffffffu, xg, 31);
-        const float c = 0.5f * (x_lo + x_hi);
-        float acc;
-        if (0.5f * (x_hi - x_lo) <= kMaxHalfWidth) {
-            const int cnt = je - jb;
+        int pass = 0;
+        if (lane == 0) pass = atomicAdd(&S.pass_counter, 1);
+        pass = __shfl_sync(0xffffffffu, pass, 0);
+        if (pass >= n_pass) break;
+        const int j0 = pass * kPass + lane * 4;
+        const float4 zz = *reinterpret_cast<const float4*>(zf + j0);
+        const double2 w01 = *reinterpret_cast<const double2*>(wbuf + j0), w23 = *reinterpret_cast<const double2*>(wbuf + j0 + 2);
+        double w[4] = {w01.x, w01.y, w23.x, w23.y};
+        float x[4] = {zz.x * scf, zz.y * scf, zz.z * scf, zz.w * scf};
+        float xmn = INFINITY, xmx = -INFINITY;
 #pragma unroll
-            for (int i = 0; i < kFlush / 32; ++i) {
-                const int jj = lane + 32 * i;
-                if (jj < ((cnt + 7) & ~7)) {
-                    float2 sj = (jj < cnt) ? pk[jb + jj] : make_float2(c, -INFINITY);
-                    const float xp = sj.x - c;
-                    scratch[jj] = make_float2(xp + xp, fmaf(-xp, xp, sj.y));
+        for (int k = 0; k < 4; ++k) {
+            const bool valid = (j0 + k < ns) && (w[k] > 0.0);   // zero-weight samples (R15) take no part
+            w[k] = valid ? w[k] * wscale : 0.0;
+            x[k] = valid ? x[k] : NAN;
+            xmn = valid ? fminf(xmn, x[k]) : xmn;
+            xmx = valid ? fmaxf(xmx, x[k]) : xmx;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            xmn = fminf(xmn, __shfl_xor_sync(0xffffffffu, xmn, o));
+            xmx = fmaxf(xmx, __shfl_xor_sync(0xffffffffu, xmx, o));
+        }
+        if (!(xmn <= xmx)) continue;             // no sample of this pass carries weight
+#pragma unroll
+        for (int k = 0; k < 4; ++k) x[k] = (x[k] == x[k]) ? x[k] : xmn;   // idle slots sit inside the band
+        float A[4] = {0.f, 0.f, 0.f, 0.f};
+        bool done = false;
+        if (Bsel) {
+            const float bd = (float)Bsel * delta;
+            const int a_lo = max(0, (int)floorf((xmn - T - xfirst) / bd));
+            const int a_hi = min(nzp / Bsel - 1, (int)floorf((xmx + T - xfirst) / bd));
+            // largest exponent of s^b inside a block: 2 |u| delta (B-1) with |u| <= span + T + B delta
+            if (2.f * (xmx - xmn + T + bd) * bd <= kMaxPowExp) {
+                if (a_hi >= a_lo) {
+                    if (Bsel == 32) power_pass<32>(gq, a_lo, a_hi, xfirst, delta, x, A);
+                    else power_pass<16>(gq, a_lo, a_hi, xfirst, delta, x, A);
+                    if (lane == 0) pairs_exec += (unsigned long long)(a_hi - a_lo + 1) * Bsel * kPass;
+                }
+                done = true;
+            }
+        }
+        if (!done) {   // direct form over the band [g_lo, g_hi]
+            int g_lo = 0, g_hi = nz - 1;
+            if (T < INFINITY) {
+                if (udz > 0.0) {
+                    g_lo = max(0, (int)floorf((xmn - T - xfirst) * inv_delta));
+                    g_hi = min(nz - 1, (int)ceilf((xmx + T - xfirst) * inv_delta));
+                } else {
+                    const float lo_key = xmn - T, hi_key = xmx + T;
+                    int a = 0, b = nz;
+                    while (a < b) { int m = (a + b) >> 1; if (gq[m].x < lo_key) a = m + 1; else b = m; }
+                    g_lo = a;
+                    b = nz;
+                    while (a < b) { int m = (a + b) >> 1; if (gq[m].x <= hi_key) a = m + 1; else b = m; }
+                    g_hi = a - 1;
                 }
             }
-            __syncwarp();
-            const float xgp = xg - c;
-            float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
-            const int n8 = (cnt + 7) >> 3;
+            if (Bsel) {   // the q' of this CTA carry the block factor: undo it (rare path: a pass spanning a wide gap)
 #pragma unroll 1
-            for (int it = 0; it < n8; ++it) {
-                const float4 p0 = scratch4[4 * it], p1 = scratch4[4 * it + 1], p2 = scratch4[4 * it + 2], p3 = scratch4[4 * it + 3];
-                acc0 += ex2_approx(fmaf(xgp, p0.x, p0.y));
-                acc1 += ex2_approx(fmaf(xgp, p0.z, p0.w));
-                acc2 += ex2_approx(fmaf(xgp, p1.x, p1.y));
-                acc3 += ex2_approx(fmaf(xgp, p1.z, p1.w));
-                acc0 += ex2_approx(fmaf(xgp, p2.x, p2.y));
-                acc1 += ex2_approx(fmaf(xgp, p2.z, p2.w));
-                acc2 += ex2_approx(fmaf(xgp, p3.x, p3.y));
-                acc3 += ex2_approx(fmaf(xgp, p3.z, p3.w));
+                for (int g = g_lo; g <= g_hi; ++g) {
+                    const float bdg = (float)(g & (Bsel - 1)) * delta;
+                    const float xg = fmaf((float)g, delta, xfirst), q = gq[g].x * ex2_approx(bdg * bdg);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { const float d = xg - x[k]; A[k] = fmaf(q, ex2_approx(-d * d), A[k]); }
+                }
+            } else if (P.dbg_K) {
+#pragma unroll 1
+                for (int g = g_lo; g <= g_hi; ++g) {
+                    const float2 v = gq[g];
+                    float kv = 0.f;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const float d = v.x - x[k], e = ex2_approx(-d * d);
+                        A[k] = fmaf(v.y, e, A[k]);
+                        kv = fmaf((float)w[k], e, kv);
+                    }
+                    double kd = warp_sum((double)kv);
+                    if (lane == 0) atomicAdd(P.dbg_K + g, kd);
+                }
+            } else {
+#pragma unroll 2
+                for (int g = g_lo; g <= g_hi; ++g) {
+                    const float2 v = gq[g];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { const float d = v.x - x[k]; A[k] = fmaf(v.y, ex2_approx(-d * d), A[k]); }
+                }
             }
-            acc = ((acc0 + acc1) + (acc2 + acc3)) * ex2_approx(-xgp * xgp);
-            __syncwarp();              // the scratch is rewritten by the next item
-        } else {
-            float acc0 = 0.f, acc1 = 0.f;
-            int j = jb;
-            for (; j + 2 <= je; j += 2) {
-                const float2 s0_ = pk[j], s1_ = pk[j + 1];
-                const float d0 = xg - s0_.x, d1 = xg - s1_.x;
-                acc0 += ex2_approx(fmaf(-d0, d0, s0_.y));
-                acc1 += ex2_approx(fmaf(-d1, d1, s1_.y));
-            }
-            if (j < je) {
-                const float2 s0_ = pk[j];
-                const float d0 = xg - s0_.x;
-                acc0 += ex2_approx(fmaf(-d0, d0, s0_.y));
-            }
-            acc = acc0 + acc1;
+            if (lane == 0 && g_hi >= g_lo) pairs_exec += (unsigned long long)(g_hi - g_lo + 1) * kPass;
         }
-        if (valid) {
-            double accd = (double)acc;
-            double q = q_g[g];
-            if (P.placement == CHIM_ON_GRID)
-                q *= grid_factor(L, P.dc_tab + (size_t)l * (P.n_table + 1 + kZPad), P.n_table + 1 + kZPad,
-                                 P.z_table_max / P.n_table, zc_g[g] + z0);
-            lsum = fma(accd, q, lsum);
-            if (P.dbg_K) atomicAdd(P.dbg_K + g, accd);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) lsum = fma(w[k], (double)A[k], lsum);
+        if (udz > 0.0 && T < INFINITY) {   // algorithmic pair count: grid points within the cut-off of each weighted sample
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (w[k] > 0.0) {
+                    const int a = max(0, (int)ceilf((x[k] - T - xfirst) * inv_delta)), b = min(nz - 1, (int)floorf((x[k] + T - xfirst) * inv_delta));
+                    pairs_cut += (unsigned long long)max(0, b - a + 1);
+                }
+        } else if (lane == 0) {
+            pairs_cut += (unsigned long long)nz * min(kPass, ns - pass * kPass);
         }
     }
+    // K(z) = 1/(N_s h sqrt(2 pi)) sum_j w_j exp(..): undo the weight normalisation (sw/ns)
     const double knorm = (sw / ns) / ((double)ns * h * 2.50662827463100050242);
-    double tot[1] = {lsum};
-    block_sum<kEvThreads, 1>(tot, S.red);
-    {
-        double pr[1] = {(double)pairs};
-        block_sum<kEvThreads, 1>(pr, S.red);
-        if (tid == 0 && pr[0] > 0.0) atomicAdd(P.stats, (unsigned long long)pr[0]);
+    double tot[3] = {lsum, (double)pairs_exec, (double)pairs_cut};
+    block_sum<kEvThreads, 3>(tot, S.red);
+    if (tid == 0 && P.stats) {
+        if (tot[1] > 0.0) atomicAdd(P.stats, (unsigned long long)tot[1]);
+        if (tot[2] > 0.0) atomicAdd(P.stats + 1, (unsigned long long)tot[2]);
     }
     if (P.dbg_K) {   // diagnostics: turn the accumulated sums into K(z_g)
         __syncthreads();
@@ -298,16 +393,15 @@ __global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
     }
     if (tid == 0) {
         double I = tot[0] * knorm;
-        if (I > 0.0) *out = log(I) + P.ln_shift[ev];
+        if (I > 0.0) *out = log(I) + P.ln_shift[ev] + P.ln_qscale[ev];
         else if (I == 0.0) { *out = -INFINITY; atomicOr(P.flags + l, CHIM_FLAG_EVENT_ZERO); }
         else *out = NAN;
     }
 }
 
 size_t events_smem_bytes(int max_ns, int max_nz) {
-    size_t ns_pad = ((size_t)max_ns + 3) & ~(size_t)3, max_tiles = ((size_t)max_nz + 31) / 32;
-    return ((sizeof(EvSmem) + 15) / 16) * 16 + sizeof(double) * ns_pad + sizeof(float) * ev_float_region(ns_pad) +
-           sizeof(int) * (3 * max_tiles + 1);
+    return ((sizeof(EvSmem) + 15) / 16) * 16 + (sizeof(double) + sizeof(float)) * ev_ns_pad((size_t)max_ns) +
+           ev_aux_bytes((size_t)max_nz);
 }
 
 cudaError_t launch_events(const EventKernelParams& P, cudaStream_t st) {

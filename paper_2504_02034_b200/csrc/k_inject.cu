@@ -1,11 +1,13 @@
 // k_inject.cu -- step S5 (selection term, eq. 12-13) and step S6 (combine, eq. 3).
 //
-//   S5  one CTA per chunk of detected injections; the chunk's packed records are staged once in shared
-//       memory and re-used for every lambda of the pass (so the injection set is streamed from HBM once per
-//       pass, not once per lambda).  Per (injection, lambda): s_j = p_m psi u / J / p_draw via the same
-//       sample_weight() as the events (the injection table's R column carries psi u / J); z_j > z_cat_max
-//       gives s_j = 0 (R6).  Per-CTA fp64 partial sums {sum s, sum s^2} per lambda, combined in a fixed
-//       order by S6 (deterministic; no atomics on the sums).
+//   S5  one CTA per (lambda, chunk of detected injections).  The lambda's mass table ("a" variant, 64 KB) is staged
+//       once in shared memory -- the injections' source masses are scattered over the whole table, and scattered
+//       16-byte reads cost an L1 wavefront each from global memory but ~1/3 of that from shared memory -- and the
+//       chunk's packed records are streamed through it with coalesced 128-bit loads (the set is sorted in d_L, so a
+//       warp's rows of the z(ln d_L) table are one or two cache lines).  CTAs in flight share a chunk (lambda is the
+//       fast grid index), so the records come from L2.  Per (injection, lambda): s_j = p_m psi u / J / p_draw via the
+//       same sample_weight() as the events (the injection table's R column carries psi u / J); z_j > z_cat_max gives
+//       s_j = 0 (R6).  Per-CTA fp64 partial sums {sum s, sum s^2}, combined in a fixed order by S6 (deterministic).
 //   S6  log L = sum_i log I_i - N_e log xi, N_eff (eq. 13), flags.
 #include "chim_internal.cuh"
 
@@ -13,83 +15,73 @@ namespace chim {
 
 constexpr int kInjThreads = 256;
 
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-
 struct InjSmem {
-    LamConst L[2];
+    LamConst L;
     double red[2 * (kInjThreads / 32)];
 };
 
-__global__ void __launch_bounds__(kInjThreads) k_inject(InjKernelParams P) {
+__global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     InjSmem& S = *reinterpret_cast<InjSmem*>(smem_raw);
-    double2* rA = reinterpret_cast<double2*>(smem_raw + ((sizeof(InjSmem) + 15) / 16) * 16);
-    double2* rB = rA + P.chunk;
-    double2* rC = rB + P.chunk;
+    double2* sA = reinterpret_cast<double2*>(smem_raw + ((sizeof(InjSmem) + 15) / 16) * 16);
+    double2* sB = sA + (P.n_mass + 2);
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int64_t j0 = (int64_t)blockIdx.x * P.chunk;
-    const int nj = (int)min((int64_t)P.chunk, P.inj.n_det - j0);
-    for (int j = tid; j < nj; j += kInjThreads) {
-        rA[j] = P.inj.recA[j0 + j];
-        rB[j] = P.inj.recB[j0 + j];
-        rC[j] = P.inj.recC[j0 + j];
-    }
+    const int l = blockIdx.x % P.n_lambda, chunk = blockIdx.x / P.n_lambda;
+    const int64_t j0 = (int64_t)chunk * P.chunk, j1 = min(j0 + (int64_t)P.chunk, P.inj.n_det);
     const int nw = sizeof(LamConst) / 4;
     for (int i = tid; i < nw; i += kInjThreads)
-        reinterpret_cast<uint32_t*>(&S.L[0])[i] = reinterpret_cast<const uint32_t*>(P.Lc)[i];
-    __syncthreads();
-    // the chunk is sorted in d_L, so it addresses the table rows [k_first, k_last] of every lambda's table
-    const int k_first = max(1, (int)rA[0].x), k_span = min(P.tab_rows - 2, (int)rA[nj - 1].x) - k_first + 1;
-    const int rho_lines = (P.n_win + 1 + 15) / 16;
-
-    for (int l = 0; l < P.n_lambda; ++l) {
-        const LamConst& L = S.L[l & 1];
-        if (l + 1 < P.n_lambda) {   // prefetch the next lambda's constants (shared memory) and table lines (L1)
-            for (int i = tid; i < nw; i += kInjThreads)
-                reinterpret_cast<uint32_t*>(&S.L[(l + 1) & 1])[i] = reinterpret_cast<const uint32_t*>(P.Lc + l + 1)[i];
-            if (tid < k_span) prefetch_l1(P.tab + (size_t)(l + 1) * P.tab_rows + k_first + tid);
-            else if (tid - k_span < rho_lines) prefetch_l1(P.wtab + (size_t)(l + 1) * (P.n_win + 1) + 16 * (tid - k_span));
-        }
-        double acc[2] = {0.0, 0.0};
-        int oor = 0;
-        if (L.flags == 0) {
-            const Row* tab = P.tab + (size_t)l * P.tab_rows;
-            const double* wtab = P.wtab + (size_t)l * (P.n_win + 1);
-#pragma unroll 1
-            for (int j = tid; j < nj; j += kInjThreads) {
-                double2 A = rA[j], B = rB[j], C = rC[j];
-                double z, s;
-                bool o;
-                sample_weight(L, tab, P.tab_rows, wtab, P.n_win, L.tkmax_inj, P.z_table_max, A.x, A.y, B.x, B.y, C.x,
-                              C.y, z, s, o);
-                oor |= (int)o;
-                if (!(z <= P.z_cat_max)) s = 0.0;   // support of the selection-term z density (R6)
-                acc[0] += s;
-                acc[1] += s * s;
-                if (P.dbg_s) P.dbg_s[P.inj.perm[j0 + j]] = s * P.dbg_scale;
-            }
-        }
-        acc[0] = warp_sum(acc[0]);
-        acc[1] = warp_sum(acc[1]);
-        if (lane == 0) { S.red[wid] = acc[0]; S.red[kInjThreads / 32 + wid] = acc[1]; }
-        oor = __syncthreads_or(oor);   // also publishes S.red and the prefetched constants
-        if (tid == 0) {
-            double a = 0.0, b = 0.0;
-#pragma unroll
-            for (int k = 0; k < kInjThreads / 32; ++k) { a += S.red[k]; b += S.red[kInjThreads / 32 + k]; }
-            P.partial[(size_t)blockIdx.x * P.n_lambda + l] = make_double2(a, b);
-            if (oor) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
-        }
-        __syncthreads();   // S.red is re-used by the next lambda
+        reinterpret_cast<uint32_t*>(&S.L)[i] = reinterpret_cast<const uint32_t*>(P.Lc + l)[i];
+    MassLookup M;
+    M.g = P.mtab + (size_t)l * (P.n_mass + 2);
+    M.sA = sA; M.sB = sB; M.lo = 0; M.cap = P.n_mass + 2; M.n_mass = P.n_mass;
+    for (int r = tid; r < P.n_mass + 2; r += kInjThreads) {
+        double2 hi;
+        const double2 lo = ldg256_lo(reinterpret_cast<const double*>(M.g + r), hi);
+        sA[r] = lo;
+        sB[r] = hi;
     }
+    __syncthreads();
+    const LamConst& L = S.L;
+    double acc[2] = {0.0, 0.0};
+    int oor = 0;
+    if (L.flags == 0) {
+        const Row* tab = P.tab + (size_t)l * P.tab_rows;
+#pragma unroll 1
+        for (int64_t j = j0 + tid; j < j1; j += kInjThreads) {
+            const double2 A = P.inj.recA[j], B = P.inj.recB[j], C = P.inj.recC[j];
+            double z, s;
+            bool o;
+            sample_weight(L, tab, P.tab_rows, M, L.tkmax_inj, P.z_table_max, A.x, A.y, B.x, B.y, C.x, C.y, z, s, o);
+            oor |= (int)o;
+            if (!(z <= P.z_cat_max)) s = 0.0;   // support of the selection-term z density (R6)
+            acc[0] += s;
+            acc[1] = fma(s, s, acc[1]);
+            if (P.dbg_s) P.dbg_s[P.inj.perm[j]] = s * P.dbg_scale;
+        }
+    }
+    acc[0] = warp_sum(acc[0]);
+    acc[1] = warp_sum(acc[1]);
+    if (lane == 0) { S.red[wid] = acc[0]; S.red[kInjThreads / 32 + wid] = acc[1]; }
+    oor = __syncthreads_or(oor);   // also publishes S.red
+    if (tid == 0) {
+        double a = 0.0, b = 0.0;
+#pragma unroll
+        for (int k = 0; k < kInjThreads / 32; ++k) { a += S.red[k]; b += S.red[kInjThreads / 32 + k]; }
+        P.partial[(size_t)chunk * P.n_lambda + l] = make_double2(a, b);
+        if (oor) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
+    }
+}
+
+size_t inject_smem_bytes(int n_mass) {
+    return ((sizeof(InjSmem) + 15) / 16) * 16 + 2 * sizeof(double2) * (size_t)(n_mass + 2);
 }
 
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st) {
     if (n_blocks <= 0) return cudaSuccess;
-    size_t smem = ((sizeof(InjSmem) + 15) / 16) * 16 + 3 * sizeof(double2) * (size_t)P.chunk;
+    size_t smem = inject_smem_bytes(P.n_mass);
     cudaError_t e = cudaFuncSetAttribute(k_inject, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_inject<<<n_blocks, kInjThreads, smem, st>>>(P);
+    k_inject<<<(unsigned)((long long)n_blocks * P.n_lambda), kInjThreads, smem, st>>>(P);
     return cudaGetLastError();
 }
 

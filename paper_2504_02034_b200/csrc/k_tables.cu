@@ -10,8 +10,10 @@
 //       z, ln(1+z), 1/(1+z) and the smooth weight factor psi/J (PAPER.md:226 eq. 21, :75 eq. 11) are turned
 //       into per-interval cubic coefficients so that the sample kernels do one Horner evaluation per
 //       column (the sample's table coordinate is lambda-independent and precomputed at init);
-//   mass-function constants: N_pl, Z1 (32-node Gauss-Legendre on the smoothing window + closed-form
-//       tails), and the window table rho = W/(S m'^2), W(m) = int_{m_low}^m m'^beta S(m') dm' (M1-M4).
+//   mass function (M1-M4): N_pl, Z1 (32-node Gauss-Legendre on the smoothing window + closed-form tails), the
+//       cumulative window integral W(m) = int_{m_low}^m m'^beta S(m') dm', and from them the per-lambda mass table
+//       LQ(ln m1) = ln[ p(m1)/C(m1) * (m1 - m_low)^2 ] (two variants: with / without the power law, for m1 on
+//       either side of m_high) as per-interval cubics -- the sample kernels then need one exponential per sample.
 #include "chim_internal.cuh"
 
 namespace chim {
@@ -193,7 +195,7 @@ __device__ void build_dl_table(const DlGrid g, bool is_inj, int placement, const
         s_nodes[0 * NN + idx] = z;
         s_nodes[1 * NN + idx] = u;
         s_nodes[2 * NN + idx] = 1.0 / a1;
-        s_nodes[3 * NN + idx] = R;
+        s_nodes[3 * NN + idx] = log(R);     // R > 0: psi, J and the volume factor are positive for z > 0
     }
     __syncthreads();
     // cubic through nodes k-1..k+2 expanded in t = tk - k
@@ -213,10 +215,88 @@ __device__ void build_dl_table(const DlGrid g, bool is_inj, int placement, const
     __syncthreads();
 }
 
+// W(m_low + mp) = int_{m_low}^{m_low+mp} m^beta S(m) dm from the cumulative panel table s_w + GL-8 on the partial panel.
+__device__ double window_integral(const LamConst& L, const double* s_w, int n_win, double mp) {
+    double x = mp * L.win_scale;
+    int p = max(0, min((int)x, n_win - 1));
+    double a0 = L.m_low + L.delta * p / n_win, b0 = L.m_low + mp;
+    const int nsub = (p < 32) ? 8 : 1;
+    double wdt = (b0 - a0) / nsub, acc = 0.0;
+    for (int sub = 0; sub < nsub; ++sub) {
+        double mid = a0 + (sub + 0.5) * wdt;
+#pragma unroll
+        for (int q = 0; q < kGLPanel; ++q) {
+            double m = mid + 0.5 * wdt * c_glp_x[q];
+            acc += c_glp_w[q] * exp(L.beta * log(m)) * smooth_S_dev(m, L);
+        }
+    }
+    return s_w[p] + acc * 0.5 * wdt;
+}
+
+// Mass table (MassRow): nodes idx = 0..K+2 at y = lm0 + (idx-1)/inv_dlm, rows k = 0..K+1; node 1 is m1 = m_low
+// exactly, node 0 lies below the support and is never used (the first interval takes a one-sided stencil).
+__device__ void build_mass_table(const TableParams& P, const TabSmem& S, const double* s_w, double* s_nodes,
+                                 MassRow* __restrict__ rows) {
+    const LamConst& L = S.L;
+    const int K = P.n_mass, NN = K + 3;
+    const double dlm = 1.0 / L.inv_dlm;
+    for (int idx = threadIdx.x; idx < NN; idx += kTabThreads) {
+        const double lm = L.lm0 + (idx - 1) * dlm;
+        const double m = (idx <= 1) ? L.m_low : exp(lm);
+        const double mp = m - L.m_low;
+        // ln of the un-smoothed primary density / Z1: power law (no cut) + Gaussian, and the Gaussian alone
+        const double dm = m - L.mu;
+        const double lpl = L.a_pl - L.alpha * lm, lg = L.a_g - dm * dm * L.inv2s2;     // -inf if the component is absent
+        const double hi = fmax(lpl, lg);
+        double lna = (hi > -INFINITY) ? hi + log(exp(lpl - hi) + exp(lg - hi)) : -INFINITY, lnb = lg;
+        // ln[ m'^2 S / C ]: above the window S = 1 and C continues in closed form; inside, C/S = rho m'^2
+        double lnd;
+        if (mp >= L.delta) {
+            double pw = L.beta_is_m1 ? (lm - L.ln_mc) : (exp(L.bp1 * lm) - L.pow_mc_bp1) * L.inv_bp1;
+            lnd = 2.0 * log(mp) - log(L.W_c + pw);
+        } else {
+            double x = mp * L.inv_delta, rho;
+            if (x < 2e-3) rho = exp(L.beta * log(m)) * L.inv_delta * (1.0 - 2.0 * x);   // S underflows: asymptotic form
+            else rho = window_integral(L, s_w, P.n_win, mp) / (smooth_S_dev(m, L) * mp * mp);
+            lnd = -log(rho);
+        }
+        lna += lnd;
+        lnb += lnd;
+        s_nodes[idx] = (lna > kLnFloor) ? lna : kLnFloor;
+        s_nodes[NN + idx] = (lnb > kLnFloor) ? lnb : kLnFloor;
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < K + 2; k += kTabThreads) {
+        MassRow r;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const double* f = s_nodes + c * NN;
+            double* o = c ? r.b : r.a;
+            if (k <= 1) {   // forward stencil through nodes k..k+3 (k = 0 is never addressed; keep it finite)
+                int b = max(k, 1);
+                double g0 = f[b], g1 = f[b + 1], g2 = f[b + 2], g3 = f[b + 3];
+                o[0] = g0;
+                o[1] = -11.0 / 6.0 * g0 + 3.0 * g1 - 1.5 * g2 + g3 / 3.0;
+                o[2] = g0 - 2.5 * g1 + 2.0 * g2 - 0.5 * g3;
+                o[3] = (g3 - g0) / 6.0 + 0.5 * (g1 - g2);
+            } else {
+                int i3 = min(k + 2, NN - 1);
+                double f0 = f[k - 1], f1 = f[k], f2 = f[k + 1], f3 = f[i3];
+                o[0] = f1;
+                o[1] = -f0 / 3.0 - 0.5 * f1 + f2 - f3 / 6.0;
+                o[2] = 0.5 * f0 - f1 + 0.5 * f2;
+                o[3] = (f3 - f0) / 6.0 + 0.5 * (f1 - f2);
+            }
+        }
+        rows[k] = r;
+    }
+    __syncthreads();
+}
+
 __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict__ lam, int n_lambda, TableParams P,
                                                        LamConst* __restrict__ Lc, double* __restrict__ dc_tab,
                                                        Row* __restrict__ tab_ev, Row* __restrict__ tab_inj,
-                                                       double* __restrict__ wtab) {
+                                                       MassRow* __restrict__ mtab) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TabSmem& S = *reinterpret_cast<TabSmem*>(smem_raw);
     const int nz_nodes = P.n_table + 1 + kZPad;
@@ -248,6 +328,12 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         L.gk = L.gamma + L.kappa;
         L.ln1pzp = log1p(L.zp);
         L.win_scale = P.n_win / L.delta;
+        L.inv_delta = 1.0 / L.delta;
+        L.lm0 = log(L.m_low);
+        {   // the mass table spans [ln m_low, max(ln m_top, ln m_low + 1)]
+            double top = fmax(P.ln_m_top, L.lm0 + 1.0);
+            L.inv_dlm = (double)P.n_mass / ((top - L.lm0) * (1.0 + 1e-12));
+        }
         S.ibad = 0;
     }
     __syncthreads();
@@ -335,13 +421,6 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
     }
     __syncthreads();
     block_inclusive_scan(s_w, P.n_win + 1, S.scan);
-    for (int p = tid; p <= P.n_win; p += kTabThreads) {
-        double mp = L.delta * p / P.n_win, m = L.m_low + mp;
-        double S_m = (p == P.n_win) ? 1.0 : smooth_S_dev(m, L);
-        double rho = (p > 0 && S_m > 1e-280 && s_w[p] > 0.0) ? s_w[p] / (S_m * mp * mp)
-                                                             : exp(L.beta * log(m)) / L.delta;   // m' -> 0 limit
-        wtab[(size_t)l * (P.n_win + 1) + p] = rho;
-    }
     if (tid == 0) {
         L.W_c = s_w[P.n_win];
         double dcc = dc_hermite(s_dc, dz, nz_nodes, P.z_cat_max, L);
@@ -352,6 +431,7 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         L.tkmax_inj = P.inj.K > 0 ? (lt - P.inj.x0) / P.inj.dx + 1.0 : 0.0;
     }
     __syncthreads();
+    build_mass_table(P, S, s_w, s_nodes, mtab + (size_t)l * (P.n_mass + 2));
     if (P.ev.K > 0)
         build_dl_table(P.ev, false, P.placement, S, s_dc, s_dl, dz, nz_nodes, s_nodes, tab_ev + (size_t)l * P.ev.rows());
     if (P.inj.K > 0)
@@ -363,16 +443,17 @@ size_t tables_smem_bytes(const TableParams& P) {
     int nz_nodes = P.n_table + 1 + kZPad;
     int maxK = P.ev.K > P.inj.K ? P.ev.K : P.inj.K;
     size_t b = ((sizeof(TabSmem) + 15) / 16) * 16;
-    b += sizeof(double) * (2 * (size_t)nz_nodes + (P.n_win + 1) + 4 * (size_t)(maxK + 3));
+    size_t nodes = 4 * (size_t)(maxK + 3), mnodes = 2 * (size_t)(P.n_mass + 3);
+    b += sizeof(double) * (2 * (size_t)nz_nodes + (P.n_win + 1) + (nodes > mnodes ? nodes : mnodes));
     return b;
 }
 
 cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P, LamConst* Lc, double* dc_tab,
-                          Row* tab_ev, Row* tab_inj, double* wtab, cudaStream_t st) {
+                          Row* tab_ev, Row* tab_inj, MassRow* mtab, cudaStream_t st) {
     size_t smem = tables_smem_bytes(P);
     cudaError_t e = cudaFuncSetAttribute(k_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_tables<<<n_lambda, kTabThreads, smem, st>>>(lam, n_lambda, P, Lc, dc_tab, tab_ev, tab_inj, wtab);
+    k_tables<<<n_lambda, kTabThreads, smem, st>>>(lam, n_lambda, P, Lc, dc_tab, tab_ev, tab_inj, mtab);
     return cudaGetLastError();
 }
 
@@ -391,7 +472,7 @@ __global__ void k_table_lookup(const LamConst* __restrict__ Lc, const Row* __res
             int k = (int)tk;
             double t = tk - k;
             z = horner3(tab[k].c[0], t);
-            r = horner3(tab[k].c[3], t);
+            r = exp(horner3(tab[k].c[3], t));
         }
     }
     if (z_out) z_out[i] = z;

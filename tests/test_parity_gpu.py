@@ -84,10 +84,11 @@ def test_s2_sample_redshifts_and_weights(P, lam_kw):
         assert np.max(np.abs(z - zr)) < 1e-10
         mism = (wt == 0) != (wr == 0)
         assert np.all(np.maximum(wt, wr)[mism] < 1e-12 * wr.max())
-        # relative to the largest weight (tiny weights deep in the smoothing window carry no mass)
-        assert np.max(np.abs(wt - wr)) < 1e-9 * wr.max()
-        big = wr > 1e-6 * wr.max()
-        assert np.max(np.abs(wt[big] / wr[big] - 1)) < 1e-7
+        # two MUFU.EX2 per weight: relative error <= 2.4e-7 each, also for the tiny weights deep in
+        # the smoothing window; its mean (a common factor of every I_i and of xi) cancels in log L
+        nz = wr > 0
+        assert np.max(np.abs(wt[nz] / wr[nz] - 1)) < 1e-6
+        assert abs(np.mean(wt[nz] / wr[nz] - 1)) < 5e-8
     c.close()
 
 
@@ -101,7 +102,7 @@ def test_s3_bandwidth_and_kde_on_grid(P):
         h, K, logI = c.debug_event_kde(la, ev)
         zr, wr, _ = O.sample_weights(la, w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s])
         hr = O.scott_bw(zr, wr)
-        assert abs(h / hr - 1) < 1e-9
+        assert abs(h / hr - 1) < 1e-7      # weights carry ~1e-7 relative noise; dh/h = 1e-5 moves log I by 5e-8
         Kr = O.kde(zr, wr, hr, w.z_grid[g])
         assert np.max(np.abs(K - Kr)) < 2e-6 * Kr.max()    # fp32 pair loop
         Ir = O.event_integral(la, w.z_grid[g], Kr, w.p_gal[g])
@@ -117,8 +118,9 @@ def test_s5_injection_weights(P):
         s1, s2, sr = O.selection_sums(la, w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw, z_cat_max=w.z_cat_max, return_s=True)
         mism = (s == 0) != (sr == 0)      # underflow deep in the smoothing window may differ: must carry no mass
         assert np.all(np.maximum(s, sr)[mism] < 1e-12 * sr.max())
-        assert np.max(np.abs(s - sr)) < 1e-9 * sr.max()
-        assert abs(s.sum() / s1 - 1) < 1e-9
+        nz = sr > 0
+        assert np.max(np.abs(s[nz] / sr[nz] - 1)) < 1e-6     # two MUFU.EX2 per weight, 2.4e-7 each + fp32 remainders
+        assert abs(s.sum() / s1 - 1) < 5e-8
     c.close()
 
 
@@ -213,6 +215,92 @@ def test_host_entry_point_matches_device_entry_point(P):
     assert np.allclose(out["loglike"].cpu().numpy(), h["loglike"], rtol=1e-12, atol=0)
     assert np.allclose(out["event_logI"].cpu().numpy(), h["event_logI"], rtol=1e-12, atol=0)
     c.close()
+
+
+# ---------------------------------------------------------------- the two formulations of the pair loop
+def test_kde_power_form_and_direct_form_agree_with_the_oracle(P):
+    # equally spaced grids: AUTO takes the power form (Horner in s = 2^(-2 delta u), FFMA2), DIRECT one ex2 per pair
+    w = make_workload("o5_spec", n_events=8, n_lambda=12, n_det=4000)
+    ref = O.loglike_workload(w)
+    ra = _gpu(P, w, kde_method=P.CHIM_KDE_AUTO)
+    rd = _gpu(P, w, kde_method=P.CHIM_KDE_DIRECT)
+    for r in (ra, rd):
+        rel, dtot, _ = _compare(r, ref, w.n_events)
+        assert rel < REL_EVENT and dtot < ABS_TOTAL
+        assert np.max(np.abs(r["event_logI"] - ref["event_logI"])) < 2e-6     # 50x inside the per-event budget
+        st = r["stats"]
+        assert 0 < st["kde_pairs_in_cutoff"] <= st["kde_pairs_evaluated"] < st["kde_pairs_dense"]
+    assert ra["stats"]["kde_pairs_in_cutoff"] == rd["stats"]["kde_pairs_in_cutoff"]
+    assert np.max(np.abs(ra["event_logI"] - rd["event_logI"])) < 2e-6
+
+
+def test_kde_nonuniform_grid_takes_the_direct_form(P):
+    # R14: any strictly increasing grid; the trapezoid uses the true spacings
+    w = make_workload("o5_spec", n_events=5, n_samples=1500, n_grid=400, n_lambda=6, n_det=3000)
+    for i in range(w.n_events):
+        g = slice(w.grid_off[i], w.grid_off[i + 1])
+        lo, hi = w.z_grid[g][0], w.z_grid[g][-1]
+        t = np.linspace(0.0, 1.0, 400)
+        w.z_grid[g] = lo + (hi - lo) * (0.6 * t + 0.4 * t * t)      # p_gal values are just data: keep them
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+
+
+@pytest.mark.parametrize("h_over_dz", [0.4, 1.5, 4.0, 12.0, 60.0])
+def test_kde_bandwidth_regimes_fixed_bw(P, h_over_dz):
+    # h below the grid spacing (direct form), a few spacings (B = 16), many spacings (B = 32)
+    w = make_workload("tiny", n_events=4, n_samples=700, n_grid=300, n_lambda=3, n_inj_draw=2000)
+    dz = np.array([w.z_grid[w.grid_off[i] + 1] - w.z_grid[w.grid_off[i]] for i in range(w.n_events)])
+    fb = h_over_dz * dz
+    ref = O.loglike_workload(w, bw_rule=O.BW_FIXED, fixed_bw=fb)
+    r = _gpu(P, w, fixed_bw=fb, bw_rule=O.BW_FIXED)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    # fp32 coordinates centred on the grid midpoint resolve h to ~1e-4 h when h is below the grid spacing
+    assert np.max(np.abs(r["event_logI"] - ref["event_logI"])) < (5e-5 if h_over_dz < 1 else 5e-6)
+
+
+@pytest.mark.parametrize("ns", [2, 5, 127, 128, 129, 300])
+def test_kde_few_and_widely_spread_samples(P, ns):
+    # warp passes with idle slots, pass boundaries at 128, and a pass whose samples span a gap far wider than h
+    # (p_gal is made smooth here: with a handful of samples sitting in a void of a spiky p_gal the +-t*h cut-off
+    # of R9 would not be negligible -- its bound is relative to sum_j w_j sum_g q_g, R9)
+    w = make_workload("tiny", n_events=3, n_samples=ns, n_grid=257, n_lambda=2, n_inj_draw=1000)
+    w.p_gal = 1.0 + 0.5 * np.sin(40.0 * w.z_grid)
+    s = slice(w.sample_off[1], w.sample_off[2])
+    w.dL[s] = w.dL[s] * np.where(np.arange(ns) % 2 == 0, 0.8, 1.25)     # event 1: two clumps, far apart
+    fb = np.array([0.004, 0.0015, 0.01])
+    ref = O.loglike_workload(w, bw_rule=O.BW_FIXED, fixed_bw=fb)
+    r = _gpu(P, w, fixed_bw=fb, bw_rule=O.BW_FIXED)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+
+
+def test_kde_cutoff_zero_sums_every_pair(P):
+    # two samples in voids of a spiky p_gal: only the full sum (kde_cutoff = 0) matches the oracle's definition
+    # (h is kept wide enough that the nearest galaxy is within ~10 h: a pair below 2^-126 of the event's typical
+    # pair underflows the fp32 loop)
+    w = make_workload("tiny", n_events=3, n_samples=2, n_grid=257, n_lambda=2, n_inj_draw=1000)
+    fb = np.array([0.004, 0.004, 0.01])
+    ref = O.loglike_workload(w, bw_rule=O.BW_FIXED, fixed_bw=fb)
+    r = _gpu(P, w, fixed_bw=fb, bw_rule=O.BW_FIXED, kde_cutoff=0.0)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < 1e-6 and dtot < 1e-4
+    assert r["stats"]["kde_pairs_evaluated"] >= r["stats"]["kde_pairs_dense"]
+
+
+def test_kde_tiny_p_gal_scale_is_factored_out(P):
+    w = make_workload("tiny", n_events=3, n_samples=300, n_grid=100, n_inj_draw=500)
+    ref = O.loglike_workload(w)
+    w.p_gal = w.p_gal * 1e-60          # far below fp32 range: the event's q_g scale must be carried in log space
+    r = _gpu(P, w)
+    assert np.allclose(r["event_logI"] + 60 * math.log(10.0), ref["event_logI"], rtol=0, atol=1e-5)
 
 
 # ---------------------------------------------------------------- degenerate cases and flags
