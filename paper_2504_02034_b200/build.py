@@ -24,7 +24,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return OUT
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + ["-o", OUT] + [os.path.join(CSRC, f) for f in SOURCES]
+    extra = os.environ.get("CHIM_NVCC_EXTRA", "").split()      # developer knob for tuning experiments
+    cmd = [nvcc] + NVCC_FLAGS + extra + ["-o", OUT] + [os.path.join(CSRC, f) for f in SOURCES]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)

@@ -118,6 +118,14 @@ struct MassLookup {
     int lo, cap, n_mass;
 };
 
+// Streaming 128-bit read of a packed sample record: read once per CTA, so it must not evict the table rows from L1.
+__device__ __forceinline__ double2 ldg_stream(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 __device__ __forceinline__ double2 ldg256_lo(const double* p, double2& hi) {   // one 256-bit read-only load
     double2 lo;
     asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(lo.x), "=d"(lo.y), "=d"(hi.x), "=d"(hi.y) : "l"(p));

@@ -24,7 +24,11 @@
 
 namespace chim {
 
-constexpr int kEvThreads = 256;
+#ifndef CHIM_EV_THREADS
+#define CHIM_EV_THREADS 256
+#define CHIM_EV_BLOCKS 3
+#endif
+constexpr int kEvThreads = CHIM_EV_THREADS;   // 256 x 3 CTAs per SM measured faster than 384 x 2 and 512 x 1
 constexpr int kPass = 128;               // samples per warp pass (4 per lane)
 constexpr float kMaxBlockSpan = 4.8f;    // B * delta limit of the power form
 constexpr float kMaxPowExp = 100.f;      // bound on log2 of the largest s^b inside a block (fp32 overflow guard)
@@ -120,7 +124,7 @@ __device__ __forceinline__ void power_pass(const float2* __restrict__ gq, int a_
 }
 
 // shared-memory layout after EvSmem: wbuf double[ns_pad] | zf float[ns_pad] | aux = gq float2[nz_pad] / staged mass rows
-__global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
+__global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKernelParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     EvSmem& S = *reinterpret_cast<EvSmem*>(smem_raw);
     double* wbuf = reinterpret_cast<double*>(smem_raw + ((sizeof(EvSmem) + 15) / 16) * 16);
@@ -181,9 +185,16 @@ __global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
     // ---- S2: weights + centred moments -----------------------------------------------------------------
     double mom[4] = {0.0, 0.0, 0.0, 0.0};   // sum w, sum w^2, sum w z', sum w z'^2
     int oor = 0;
+    // software pipeline: the next sample's table coordinate is read one iteration ahead and its row prefetched to L1
+    double2 A = (tid < ns) ? ldg_stream(P.ev.recA + s0 + tid) : make_double2(1.0, 1.0);
 #pragma unroll 1
     for (int j = tid; j < ns; j += kEvThreads) {
-        double2 A = P.ev.recA[s0 + j], B = P.ev.recB[s0 + j], C = P.ev.recC[s0 + j];
+        const double2 B = ldg_stream(P.ev.recB + s0 + j), C = ldg_stream(P.ev.recC + s0 + j);
+        double2 An = A;
+        if (j + kEvThreads < ns) {
+            An = ldg_stream(P.ev.recA + s0 + j + kEvThreads);
+            prefetch_l1(tab + max(1, min((int)An.x, P.tab_rows - 2)));
+        }
         double z, w;
         bool o;
         sample_weight(L, tab, P.tab_rows, M, L.tkmax_ev, P.z_table_max, A.x, A.y, B.x, B.y, C.x, C.y, z, w, o);
@@ -201,6 +212,7 @@ __global__ void __launch_bounds__(kEvThreads, 3) k_events(EventKernelParams P) {
             P.dbg_z[jo] = z;
             P.dbg_w[jo] = w * exp(P.ln_shift[ev]);
         }
+        A = An;
     }
     block_sum<kEvThreads, 4>(mom, S.red);
     oor = __syncthreads_or(oor);

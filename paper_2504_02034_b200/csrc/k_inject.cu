@@ -46,9 +46,16 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
     int oor = 0;
     if (L.flags == 0) {
         const Row* tab = P.tab + (size_t)l * P.tab_rows;
+        // software pipeline: next sample's table coordinate one iteration ahead, its row prefetched to L1
+        double2 A = (j0 + tid < j1) ? ldg_stream(P.inj.recA + j0 + tid) : make_double2(1.0, 1.0);
 #pragma unroll 1
         for (int64_t j = j0 + tid; j < j1; j += kInjThreads) {
-            const double2 A = P.inj.recA[j], B = P.inj.recB[j], C = P.inj.recC[j];
+            const double2 B = ldg_stream(P.inj.recB + j), C = ldg_stream(P.inj.recC + j);
+            double2 An = A;
+            if (j + kInjThreads < j1) {
+                An = ldg_stream(P.inj.recA + j + kInjThreads);
+                prefetch_l1(tab + max(1, min((int)An.x, P.tab_rows - 2)));
+            }
             double z, s;
             bool o;
             sample_weight(L, tab, P.tab_rows, M, L.tkmax_inj, P.z_table_max, A.x, A.y, B.x, B.y, C.x, C.y, z, s, o);
@@ -57,6 +64,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             acc[0] += s;
             acc[1] = fma(s, s, acc[1]);
             if (P.dbg_s) P.dbg_s[P.inj.perm[j]] = s * P.dbg_scale;
+            A = An;
         }
     }
     acc[0] = warp_sum(acc[0]);
