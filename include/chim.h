@@ -82,17 +82,18 @@ typedef struct chim_config {
     double z_cat_max;    /* z_max of PAPER.md:65 eq. 9: support of the selection-term redshift density (R6)    */
     double z_table_max;  /* extent of the d_C(z) table; samples with z > z_table_max get weight 0 (+ flag)     */
     int32_t n_table;     /* panels of the d_C(z) table on [0, z_table_max] (also the monotonicity check nodes) */
-    int32_t n_dl_table;  /* intervals of the per-lambda z(ln d_L) interpolation tables                         */
+    int32_t n_dl_table;  /* intervals of the per-lambda z(ln d_L) interpolation tables; 0 = spacing ~0.005 in ln d_L */
     int32_t n_win_table; /* panels of the per-lambda window table of int m^beta S(m) dm (M4)                   */
     int32_t lambda_chunk;/* lambdas processed per internal pass (bounds the per-lambda table memory)           */
     double neff_factor;  /* NEFF_LOW is raised if N_eff < neff_factor * N_events (R8)                          */
     int32_t kde_method;  /* CHIM_KDE_AUTO (default) | CHIM_KDE_DIRECT (one MUFU.EX2 per pair on every grid)            */
     int32_t n_mass_table;/* intervals of the per-lambda mass table in ln m1                           */
+    int32_t count_pairs; /* 1: the KDE kernel also counts its (sample, grid point) pairs for chim_get_stats (slower)     */
 } chim_config;
 
 /* Fills *cfg with the defaults: device 0, HOST, NULL stream, ON_SAMPLES, SCOTT, kde_cutoff 6.0,
- * z_cat_max 1.5, z_table_max 10, n_table 2048, n_dl_table 2048, n_win_table 512, lambda_chunk 256,
- * neff_factor 5, kde_method AUTO, n_mass_table 2048. */
+ * z_cat_max 1.5, z_table_max 10, n_table 2048, n_dl_table 0 (auto), n_win_table 512, lambda_chunk 256,
+ * neff_factor 5, kde_method AUTO, n_mass_table 2048, count_pairs 0. */
 void chim_default_config(chim_config *cfg);
 
 /* Creates a context on cfg->device.  cfg == NULL means chim_default_config.  *out is set to NULL on error

@@ -105,6 +105,18 @@ cudaError_t fetch(const chim_ctx* c, const T* src, size_t n, std::vector<T>& dst
     return cudaSuccess;
 }
 
+// number of intervals of a z(ln d_L) table: the configured one, or (n_dl_table = 0) a spacing of ~0.005 in ln d_L,
+// which keeps the interpolation error of the fp32 rows below their rounding
+int choose_dl_intervals(const chim_ctx* ctx, double xmin, double xmax) {
+    if (ctx->cfg.n_dl_table > 0) return std::min(ctx->cfg.n_dl_table, kMaxDlRows);
+    double k = std::ceil((xmax - xmin) / 0.005);
+    return (int)std::min<double>(std::max<double>(k, 64.0), (double)kMaxDlRows);
+}
+
+inline float f_hi(double x) { return (float)x; }
+inline float f_lo(double x) { return (float)(x - (double)(float)x); }
+inline float bits_f(uint32_t u) { float f; std::memcpy(&f, &u, 4); return f; }
+
 DlGrid make_dl_grid(double xmin, double xmax, int K) {
     DlGrid g;
     g.x0 = xmin;
@@ -122,7 +134,7 @@ int ensure_work(chim_ctx* ctx, int nl) {
     CK(dev_alloc(ctx->owned_work, &ctx->Lc, nl));
     CK(dev_alloc(ctx->owned_work, &ctx->tab_ev, (size_t)nl * ctx->ev_grid.rows()));
     CK(dev_alloc(ctx->owned_work, &ctx->tab_inj, (size_t)nl * (ctx->have_inj ? ctx->inj_grid.rows() : 1)));
-    CK(dev_alloc(ctx->owned_work, &ctx->mtab, (size_t)nl * (ctx->cfg.n_mass_table + 2)));
+    CK(dev_alloc(ctx->owned_work, &ctx->mtab, (size_t)nl * 2 * (ctx->cfg.n_mass_table + 2)));
     ctx->dc_tab = nullptr;
     if (need_dc) CK(dev_alloc(ctx->owned_work, &ctx->dc_tab, (size_t)nl * (ctx->cfg.n_table + 1 + kZPad)));
     CK(dev_alloc(ctx->owned_work, &ctx->logI, (size_t)nl * ctx->ev.n_events));
@@ -187,7 +199,7 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t) * nl, st));
     { Bracket b(ctx, 0); CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, st)); }
     EventKernelParams EP = event_params(ctx, nl);
-    { Bracket b(ctx, 1); CK(launch_events(EP, st)); }
+    { Bracket b(ctx, 1); CK(launch_events(EP, ctx->cfg.count_pairs != 0, st)); }
     ctx->launches += 2;
     if (ctx->have_inj) {
         InjKernelParams IP{};
@@ -232,12 +244,13 @@ void chim_default_config(chim_config* cfg) {
     cfg->z_cat_max = 1.5;
     cfg->z_table_max = 10.0;
     cfg->n_table = 2048;
-    cfg->n_dl_table = 2048;
+    cfg->n_dl_table = 0;
     cfg->n_win_table = 512;
     cfg->lambda_chunk = 256;
     cfg->neff_factor = 5.0;
     cfg->kde_method = CHIM_KDE_AUTO;
     cfg->n_mass_table = 2048;
+    cfg->count_pairs = 0;
 }
 
 int chim_version(void) { return CHIM_VERSION; }
@@ -252,7 +265,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     chim_config d;
     chim_default_config(&d);
     if (c.n_table <= 0) c.n_table = d.n_table;
-    if (c.n_dl_table <= 0) c.n_dl_table = d.n_dl_table;
+    if (c.n_dl_table < 0) c.n_dl_table = d.n_dl_table;
     if (c.n_win_table <= 0) c.n_win_table = d.n_win_table;
     if (c.lambda_chunk <= 0) c.lambda_chunk = d.lambda_chunk;
     if (c.n_mass_table <= 0) c.n_mass_table = d.n_mass_table;
@@ -260,7 +273,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     if (!(c.z_cat_max > 0.0)) c.z_cat_max = d.z_cat_max;
     if (!(c.neff_factor >= 0.0)) c.neff_factor = d.neff_factor;
     if (c.kde_cutoff < 0.0 || !std::isfinite(c.kde_cutoff)) return CHIM_EINVAL;
-    if (c.n_table < 16 || c.n_dl_table < 16 || c.n_win_table < 8 || c.n_mass_table < 64 || c.z_cat_max > c.z_table_max) return CHIM_EINVAL;
+    if (c.n_table < 16 || (c.n_dl_table != 0 && c.n_dl_table < 16) || c.n_dl_table > kMaxDlRows || c.n_win_table < 8 || c.n_mass_table < 64 || c.z_cat_max > c.z_table_max) return CHIM_EINVAL;
     if (c.placement != CHIM_ON_SAMPLES && c.placement != CHIM_ON_GRID) return CHIM_EINVAL;
     if (c.bw_rule != CHIM_BW_SCOTT && c.bw_rule != CHIM_BW_FIXED) return CHIM_EINVAL;
     if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT) return CHIM_EINVAL;
@@ -276,7 +289,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     ctx->cfg = c;
     ctx->stream = static_cast<cudaStream_t>(c.stream);
     TableParams TP = table_params(ctx);
-    TP.ev.K = TP.inj.K = c.n_dl_table;
+    TP.ev.K = TP.inj.K = c.n_dl_table > 0 ? c.n_dl_table : kMaxDlRows;
     if (tables_smem_bytes(TP) > kMaxSmemOptin || inject_smem_bytes(c.n_mass_table) > kMaxSmemOptin) { delete ctx; return CHIM_EINVAL; }
     if (upload_gauss_legendre() != cudaSuccess) { delete ctx; return CHIM_ECUDA; }
     *out = ctx;
@@ -347,9 +360,11 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
         if (ctx->cfg.bw_rule == CHIM_BW_FIXED && !(h_bw[i] > 0.0))
             return fail(ctx, CHIM_EINVAL, "chim_init_events: fixed_bw must be > 0");
     }
-    DlGrid grid = make_dl_grid(xmin, xmax, ctx->cfg.n_dl_table);
+    DlGrid grid = make_dl_grid(xmin, xmax, choose_dl_intervals(ctx, xmin, xmax));
 
-    std::vector<double2> rA(NS), rB(NS), rC(NS);
+    std::vector<float4> rA(NS), rB(NS);
+    std::vector<int32_t> k_lo(n_events), k_hi(n_events);
+    const double l2e = 1.4426950408889634074;
     std::vector<int32_t> perm(NS);
     std::vector<double> zc(NG), qg(NG), z0(n_events), shift(n_events), qshift(n_events), udz(n_events);
     std::vector<float> qn(NG);
@@ -370,11 +385,16 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
             const int64_t o = s0 + idx[j];
             lm_lo[i] = std::min(lm_lo[i], std::log(h_m1[o]));
             lm_hi[i] = std::max(lm_hi[i], std::log(h_m1[o]));
-            double q = h_m2[o] / h_m1[o];
-            rA[s0 + j] = make_double2((std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0, h_m1[o]);
-            rB[s0 + j] = make_double2(q, std::log(h_m1[o]));
-            rC[s0 + j] = make_double2(std::log(q), -h_lp[o] - sh);   // ln(1/pi_j) with the event's scale removed
+            const double tk = (std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0;   // in [1, K + 1)
+            const uint32_t tkq_max = ((uint32_t)(grid.K + 1) << kTkFracBits) - 1u;   // rounding must not leave the last interval
+            const uint32_t tkq = std::min((uint32_t)std::min<double>(std::max(tk, 0.0) * (double)(1u << kTkFracBits) + 0.5, 4294967295.0), tkq_max);
+            rA[s0 + j] = make_float4(bits_f(tkq), f_hi(h_m1[o]), f_lo(h_m1[o]), f_hi(h_m2[o]));
+            rB[s0 + j] = make_float4(f_lo(h_m2[o]), (float)std::log(h_m1[o]), (float)std::log(h_m2[o] / h_m1[o]),
+                                     (float)(l2e * (-h_lp[o] - sh)));   // log2(1/pi_j) with the event's scale removed
             perm[s0 + j] = idx[j];
+            const int k = std::min(std::max((int)(tkq >> kTkFracBits), 1), grid.K);
+            if (j == 0) k_lo[i] = k;
+            k_hi[i] = k;
         }
         const int64_t g0 = go[i];
         const int nz = (int)(go[i + 1] - g0);
@@ -406,7 +426,8 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     EventSetDev E{};
     E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz;
     CK(upload(ctx->owned_ev, &E.sample_off, so)); CK(upload(ctx->owned_ev, &E.grid_off, go));
-    CK(upload(ctx->owned_ev, &E.recA, rA)); CK(upload(ctx->owned_ev, &E.recB, rB)); CK(upload(ctx->owned_ev, &E.recC, rC));
+    CK(upload(ctx->owned_ev, &E.recA, rA)); CK(upload(ctx->owned_ev, &E.recB, rB));
+    CK(upload(ctx->owned_ev, &E.k_lo, k_lo)); CK(upload(ctx->owned_ev, &E.k_hi, k_hi));
     CK(upload(ctx->owned_ev, &E.perm, perm)); CK(upload(ctx->owned_ev, &E.zc, zc)); CK(upload(ctx->owned_ev, &E.qn, qn));
     CK(upload(ctx->owned_ev, &E.uni_dz, udz));
     CK(upload(ctx->owned_ev, &E.lnm1_lo, lm_lo)); CK(upload(ctx->owned_ev, &E.lnm1_hi, lm_hi));
@@ -453,17 +474,18 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
         xmax = std::max(xmax, x);
         sh = std::max(sh, -h_lp[j]);
     }
-    DlGrid grid = make_dl_grid(xmin, xmax, ctx->cfg.n_dl_table);
+    DlGrid grid = make_dl_grid(xmin, xmax, choose_dl_intervals(ctx, xmin, xmax));
+    const double l2e = 1.4426950408889634074;
     std::vector<int64_t> idx(N);
     std::iota(idx.begin(), idx.end(), (int64_t)0);
     std::stable_sort(idx.begin(), idx.end(), [&](int64_t a, int64_t b) { return h_dl[a] < h_dl[b]; });
-    std::vector<double2> rA(N), rB(N), rC(N);
+    std::vector<float4> rA(N), rB(N);
     for (size_t j = 0; j < N; ++j) {
         const size_t o = (size_t)idx[j];
-        double q = h_m2[o] / h_m1[o];
-        rA[j] = make_double2((std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0, h_m1[o]);
-        rB[j] = make_double2(q, std::log(h_m1[o]));
-        rC[j] = make_double2(std::log(q), -h_lp[o] - sh);
+        const double tk = (std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0;
+        const int k = std::min(std::max((int)tk, 1), grid.K);
+        rA[j] = make_float4(bits_f((uint32_t)k), (float)(tk - (double)k), (float)h_m1[o], (float)h_m2[o]);
+        rB[j] = make_float4((float)std::log(h_m1[o]), (float)std::log(h_m2[o] / h_m1[o]), (float)(l2e * (-h_lp[o] - sh)), 0.f);
     }
     cudaStreamSynchronize(ctx->stream);
     free_pool(ctx->owned_inj);
@@ -473,7 +495,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     InjSetDev I{};
     I.n_det = n_det;
     I.n_inj_total = (double)n_inj_total;
-    CK(upload(ctx->owned_inj, &I.recA, rA)); CK(upload(ctx->owned_inj, &I.recB, rB)); CK(upload(ctx->owned_inj, &I.recC, rC));
+    CK(upload(ctx->owned_inj, &I.recA, rA)); CK(upload(ctx->owned_inj, &I.recB, rB));
     CK(upload(ctx->owned_inj, &I.perm, idx));
     ctx->inj = I;
     ctx->inj_m_top = m_top;
@@ -635,7 +657,7 @@ static int debug_event(chim_ctx* ctx, const double* lambda, int32_t event, doubl
     EP.dbg_event = event;
     EP.dbg_z = z_out; EP.dbg_w = w_out; EP.dbg_h = h_out; EP.dbg_K = K_out;
     if (K_out) CK(cudaMemsetAsync(K_out, 0, sizeof(double) * (size_t)(ctx->h_grid_off[event + 1] - ctx->h_grid_off[event]), ctx->stream));
-    CK(launch_events(EP, ctx->stream));
+    CK(launch_events(EP, true, ctx->stream));
     if (logI_out) CK(cudaMemcpyAsync(logI_out, ctx->logI, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     return CHIM_OK;

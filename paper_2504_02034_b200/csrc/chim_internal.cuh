@@ -16,6 +16,22 @@ constexpr int kZPad = 32;                  // d_C table panels kept beyond z_tab
 constexpr double kLnFloor = -1.0e4;        // ln of "zero" in the log-space tables (exp underflows to the 1e-307 floor)
 constexpr double kHalfLog2e = 0.72134752044448170368;  // log2(e)/2 : exp(-d^2/2h^2) = 2^(-(d s)^2), s^2 = kHalfLog2e/h^2
 
+// fp32 view of the per-lambda constants used per sample / injection (S2, S5).  Values that enter a difference of
+// nearly equal numbers are carried as an unevaluated sum hi + lo of two floats.
+struct LamF {
+    float mlow_hi, mlow_lo;   // m_low
+    float lm0_hi, lm0_lo;     // ln m_low (origin of the mass table)
+    float delta;              // delta_m
+    float two_dl2e, d2l2e;    // 2 delta log2(e), delta^2 log2(e): log2(e) f = (two_dl2e m' - d2l2e) / (m' (m' - delta))
+    float win_lo, win_hi;     // clamp of m' strictly inside the smoothing window
+    float beta2;              // beta log2(e)
+    float mhigh_p;            // m_high - m_low
+    float tm_scale, tm_max;   // mass-table coordinate tm = (ln m1 - ln m_low) tm_scale + 1, clamped to [1, tm_max]
+    float tkmax_ev, tkmax_inj;// table coordinate beyond which z > z_table_max
+    float zcat_hi, zcat_lo;   // z_cat_max (R6) as hi + lo
+    uint32_t tkmax_ev_q;      // tkmax_ev in the 12.20 fixed point of the event records
+};
+
 // Per-lambda constants written by the table kernel (S1), read by every other kernel.
 struct LamConst {
     double H0, Om, Xi0, n, alpha, beta, delta, m_low, m_high, mu, sigma, lg, gamma, kappa, zp;
@@ -42,14 +58,20 @@ struct LamConst {
     double inv_dlm;
     uint32_t flags;     // CHIM_FLAG_LAMBDA_DOMAIN | CHIM_FLAG_DL_NONMONOTONE
     int32_t beta_is_m1; // |beta + 1| < 1e-12 : log form of the power integral
+    LamF F;             // fp32 constants of the sample kernels (S2, S5)
 };
 
-// One interval of the per-lambda interpolation table in x = ln d_L: cubic (Lagrange through 4 nodes,
-// expanded in the local coordinate t in [0,1)) for 4 columns:
-//   0: z      1: u = ln(1+z)      2: a = 1/(1+z)      3: R = smooth redshift factor of the weight
-// (events: psi/J or 1; injections: psi u_vol / J).  128 B = one cache line.
+// One interval of the per-lambda interpolation table in x = ln d_L, local coordinate t in [0,1), fp32 (64 B):
+//   z(t) = z_hi + (z_lo + t (z1 + t (z2 + t z3)))      redshift: cubic through 4 nodes, leading term as hi + lo
+//   a(t) = a_hi + (a_lo + t (a1 + t (a2 + t a3)))      1/(1+z), same form (feeds the difference m^d a - m_low)
+//   u(t) = u0 + t (u1 + t u2)                           ln(1+z): the cubic with t^3 economised (Chebyshev) away
+//   r(t) = r0 + t (r1 + t r2)                           log2 of the smooth redshift factor of the weight
+// (events: psi/J or 1; injections: psi u_vol / J).
 struct __align__(16) Row {
-    double c[4][4];  // c[col][degree]
+    float z_hi, z_lo, z1, z2;
+    float z3, a_hi, a_lo, a1;
+    float a2, a3, u0, u1;
+    float u2, r0, r1, r2;
 };
 
 // Geometry of a ln d_L table: sample coordinate tk = (ln dL - x0)/dx + 1, interval k = floor(tk) in [1, K],
@@ -69,126 +91,111 @@ struct TableParams {
     DlGrid ev, inj;
 };
 
-// One interval of the per-lambda mass table in y = ln m1: cubics (local coordinate t in [0,1)) of
-//   a: ln[ p(m1)/S(m1) * m1'^2 S(m1)/C(m1) ]  with the power law present (m1 <= m_high),  m1' = m1 - m_low
-//   b: the same with the Gaussian component only (m1 > m_high)
-// i.e. ln of  p(m1) / C(m1) * m1'^2  -- smooth and finite on [m_low, inf) because C/S ~ rho m1'^2 (M3/M4).
-struct __align__(16) MassRow {
-    double a[4], b[4];
-};
+// One interval of the per-lambda mass table in y = ln m1 (local coordinate t in [0,1]): cubic c0 + t(c1 + t(c2 + t c3)),
+// fp32, of  LQ2 = log2[ p(m1)/S(m1) * m1'^2 S(m1)/C(m1) ],  m1' = m1 - m_low  -- i.e. log2 of p(m1)/C(m1) m1'^2,
+// smooth and finite on [m_low, inf) because C/S ~ rho m1'^2 (M3/M4).  Two variants per lambda, stored as two
+// consecutive arrays of n_mass + 2 rows: "a" with the power law present (m1 <= m_high), "b" the Gaussian only.
+typedef float4 MassRow;
 
-// exp(x) for the sample kernels: fp64 range reduction x log2(e) = n + f, |f| <= 1/2 (exact in fp64), MUFU.EX2 on
-// the fp32 remainder (relative error <= 2.4e-7), 2^n through the exponent field.  |x| must stay
-// below ~1e9 (the magic-number rounding) -- every caller bounds its argument; n is clamped so that the result never
-// leaves the normal range: e^-707 ~ 1e-307 stands in for 0.
-__device__ __forceinline__ double exp_mufu(double x) {
-    const double y = x * 1.4426950408889634074;
-    const double t = y + 6755399441055744.0;            // 1.5 * 2^52: round to nearest integer
-    int n = __double2loint(t);
-    const double fn = t - 6755399441055744.0;
-    const float f = (float)(y - fn);
-    float e;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(f));
-    n = max(-1020, min(n, 1020));
-    const double ed = (double)e;                        // in [0.70, 1.42]
-    return __hiloint2double(__double2hiint(ed) + (n << 20), __double2loint(ed));
+// Packed, lambda-independent record of one posterior sample / injection (2 x 16 B).
+//   events:     A = {tkq, m1d_hi, m1d_lo, m2d_hi}   B = {m2d_lo, ln m1d, ln(m2d/m1d), log2(1/prior) - event scale}
+//               tkq = table coordinate in 12.20 fixed point (interval in the upper 12 bits)
+//   injections: A = {k, t, m1d, m2d}                B = {ln m1d, ln(m2d/m1d), log2(1/p_draw) - set scale, 0}
+//               (t kept as a full float: the support cut z <= z_cat_max of R6 is a step)
+constexpr int kTkFracBits = 20;
+constexpr int kMaxDlRows = (1 << (32 - kTkFracBits)) - 3;   // largest n_dl_table the fixed-point coordinate can address
+
+__device__ __forceinline__ float ex2f(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float lg2f(float x) {
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcpf(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 }
 
-// 1/x for finite non-zero normal x: MUFU.RCP64H seed + two Newton steps (error ~1e-16), no special cases.
-__device__ __forceinline__ double fast_rcp(double x) {
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    return fma(r, e, r);
+// 2^y as a double for any float y (the fp32 exponent range is not enough for injection weights carrying an arbitrary
+// draw-density scale): integer part through the exponent field, fraction through MUFU.EX2.  y = -inf gives 0.
+__device__ __forceinline__ double ex2_to_double(float y) {
+    const float yc = fminf(fmaxf(y, -1000.f), 1000.f);
+    const float ti = yc + 12582912.f;                   // 1.5 * 2^23: round to nearest integer
+    const int n = __float_as_int(ti) - 0x4B400000;
+    const float e = ex2f(yc - (ti - 12582912.f));       // in [0.70, 1.42]
+    const double ed = (double)e;
+    const double v = __hiloint2double(__double2hiint(ed) + (n << 20), __double2loint(ed));
+    return (y > -1000.f) ? v : 0.0;
 }
 
-__device__ __forceinline__ double horner3(const double* c, double t) {
-    return fma(fma(fma(c[3], t, c[2]), t, c[1]), t, c[0]);
-}
-
-// Where a thread finds the per-lambda mass table: rows [lo, lo + cap) of the "a" variant staged in shared memory as
-// two split arrays (16-byte halves: the layout with the fewest bank conflicts for scattered rows), everything else
-// (rows outside the staged range, the Gaussian-only "b" variant beyond m_high) in global memory.
+// Where a thread finds the per-lambda mass table: rows [lo, lo + cap) of both variants staged in shared memory
+// (variant "b" at offset cap), everything else in global memory.
 struct MassLookup {
-    const MassRow* g;          // [n_mass + 2] rows of this lambda
-    const double2* sA;         // staged {a[0], a[1]} or null
-    const double2* sB;         // staged {a[2], a[3]}
+    const MassRow* g;          // [2][n_mass + 2] rows of this lambda
+    const MassRow* s;          // staged rows or null
     int lo, cap, n_mass;
 };
 
-// Streaming 128-bit read of a packed sample record: read once per CTA, so it must not evict the table rows from L1.
-__device__ __forceinline__ double2 ldg_stream(const double2* p) {
-    double2 v;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+__device__ __forceinline__ float4 ldg_stream4(const float4* p) {   // streaming 128-bit read (read once per CTA)
+    float4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
     return v;
 }
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
-__device__ __forceinline__ double2 ldg256_lo(const double* p, double2& hi) {   // one 256-bit read-only load
-    double2 lo;
-    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(lo.x), "=d"(lo.y), "=d"(hi.x), "=d"(hi.y) : "l"(p));
-    return lo;
-}
-
-// Steps S2 / S5 for one sample (or injection): redshift from the table, source-frame masses, population weight
+// Steps S2 / S5 for one sample (or injection): redshift from the table, source-frame masses, log2 of the weight
 //   w = p(m1, m2 | lambda_m) * R(z) / prior,   p(m1,m2) = p(m1) m2^beta S(m2) / C(m1)     (M1-M4)
-// assembled in log space from two table look-ups:
-//   ln w' = LQ(ln m1) + beta ln m2 + ln R + ln(1/prior),   w = exp(ln w') S(m2) / m1'^2
-//   LQ   per-lambda mass table (MassRow): ln[p(m1)/C(m1) m1'^2], smooth on [m_low, inf)
+//   log2 w = LQ2(ln m1) + beta log2 m2 + log2 R + log2(1/prior) - 2 log2 m1' - log2(1 + e^f(m2'))
+//   LQ2  per-lambda mass table (MassRow): log2[p(m1)/C(m1) m1'^2], smooth on [m_low, inf)
 //   S(m2) = 1/(1 + exp(delta/m2' + delta/(m2' - delta))) inside the window, 1 above (M1)
-//   ln R, z, ln(1+z), 1/(1+z): the four cubics of the sample's row of the z(ln d_L) table
+//   log2 R, z, ln(1+z), 1/(1+z): the four polynomials of the sample's row of the z(ln d_L) table
 //   PAPER.md:52 (d_L -> z, m = m^d/(1+z)), :195-198 eq. 20 (mass model), :226 eq. 21, :75 eq. 11.
-// Two exponentials (MUFU.EX2 on fp64-reduced arguments) and two reciprocals per sample; selects instead of
-// data-dependent branches, except the (rare) fall-back of the mass row to global memory.
-__device__ __forceinline__ void sample_weight(const LamConst& L, const Row* __restrict__ tab, int n_rows,
-                                              const MassLookup& M, double tkmax, double z_table_max,
-                                              double tk, double m1d, double q, double lnm1d, double lnq, double lnipr,
-                                              double& z, double& w, bool& out_of_range) {
-    out_of_range = !(tk <= tkmax);
-    int k = (int)((tk < (double)(n_rows - 2)) ? tk : (double)(n_rows - 2));
-    k = max(1, k);
-    double t = tk - (double)k;
-    const double* rp = reinterpret_cast<const double*>(tab + k);     // 4 x 256-bit loads of one 128-byte row
-    double2 c0, c1, c2, c3, c4, c5, c6, c7;
-    c0 = ldg256_lo(rp, c1);
-    c2 = ldg256_lo(rp + 4, c3);
-    c4 = ldg256_lo(rp + 8, c5);
-    c6 = ldg256_lo(rp + 12, c7);
-    double zt = fma(fma(fma(c1.y, t, c1.x), t, c0.y), t, c0.x);
-    double u = fma(fma(fma(c3.y, t, c3.x), t, c2.y), t, c2.x);
-    double a = fma(fma(fma(c5.y, t, c5.x), t, c4.y), t, c4.x);
-    double lnR = fma(fma(fma(c7.y, t, c7.x), t, c6.y), t, c6.x);
-    z = out_of_range ? z_table_max : zt;
-    const double m1 = m1d * a, m2 = q * m1;
-    const double lm1 = lnm1d - u, lm2 = lm1 + lnq;
-    const double mp1 = m1 - L.m_low, mp2 = m2 - L.m_low;
-    // mass table
-    double tm = fma(lm1 - L.lm0, L.inv_dlm, 1.0);
-    int km = max(1, min((int)tm, M.n_mass));
-    tm -= (double)km;
-    double2 d0, d1;
+// All fp32; differences of nearly equal numbers (z - z_ref, m^d a - m_low) are formed from hi + lo pairs, so the
+// rounding errors left are ~1e-7 relative, independent from sample to sample.  Five MUFU ops
+// (rcp, ex2, 2 lg2 here; the final ex2 is the caller's), no fp64, no data-dependent branch except the (rare)
+// fall-back of the mass row to global memory.  Returns z - z_ref and log2 w (-inf: weight 0).
+__device__ __forceinline__ void sample_eval(const LamF& F, const float4 q0, const float4 q1, const float4 q2,
+                                            const float4 q3, const float t, const float zref_hi, const float zref_lo,
+                                            const float m1h, const float m1l, const float m2h, const float m2l,
+                                            const float lnm1d, const float lnq, const float ipr2,
+                                            const MassLookup& M, const bool in_range, float& zc, float& l2w) {
+    // row: q0 = {z_hi, z_lo, z1, z2}  q1 = {z3, a_hi, a_lo, a1}  q2 = {a2, a3, u0, u1}  q3 = {u2, r0, r1, r2}
+    zc = (q0.x - zref_hi) + fmaf(fmaf(fmaf(q1.x, t, q0.w), t, q0.z), t, q0.y - zref_lo);
+    const float a_hi = q1.y;
+    const float a_lo = fmaf(fmaf(fmaf(q2.y, t, q2.x), t, q1.w), t, q1.z);
+    const float u = fmaf(fmaf(q3.x, t, q2.w), t, q2.z);
+    const float r = fmaf(fmaf(q3.w, t, q3.z), t, q3.y);
+    // m' = m^d a - m_low for both masses: exact product + low-order terms
+    const float p1 = __fmul_rn(m1h, a_hi), p2 = __fmul_rn(m2h, a_hi);   // never contracted into an FMA
+    const float c1 = fmaf(m1h, a_lo, fmaf(m1l, a_hi, fmaf(m1h, a_hi, -p1) - F.mlow_lo));
+    const float c2 = fmaf(m2h, a_lo, fmaf(m2l, a_hi, fmaf(m2h, a_hi, -p2) - F.mlow_lo));
+    const float mp1 = (p1 - F.mlow_hi) + c1, mp2 = (p2 - F.mlow_hi) + c2;
+    const float lm1 = lnm1d - u, lm2 = lm1 + lnq;
+    // mass table: coordinate, interval by the magic-number floor, cubic
+    float tm = fmaf((lm1 - F.lm0_hi) - F.lm0_lo, F.tm_scale, 1.0f);
+    tm = fminf(fmaxf(tm, 1.0f), F.tm_max);
+    const float ti = (tm - 0.5f) + 12582912.f;
+    const int km = __float_as_int(ti) - 0x4B400000;
+    const float tf = tm - (ti - 12582912.f);
+    const bool gauss_only = mp1 > F.mhigh_p;
     const int ks = km - M.lo;
-    if ((unsigned)ks < (unsigned)M.cap && m1 <= L.m_high) {
-        d0 = M.sA[ks];
-        d1 = M.sB[ks];
-    } else {
-        d0 = ldg256_lo(reinterpret_cast<const double*>(M.g + km) + ((m1 <= L.m_high) ? 0 : 4), d1);
-    }
-    double lnw = fma(fma(fma(d1.y, tm, d1.x), tm, d0.y), tm, d0.x);
-    lnw += fma(L.beta, lm2, lnR + lnipr);
-    // smoothing of m2 (M1): f = delta (2 m' - delta) / (m' (m' - delta)), m' clamped strictly inside the window
-    const double lo = L.delta * 1e-3, hi = L.delta * (1.0 - 1e-12);   // S(m' < 1e-3 delta) < e^-998: "0" either way
-    double mc = (mp2 > lo) ? mp2 : lo;
-    mc = (mc < hi) ? mc : hi;
-    const double f = L.delta * (2.0 * mc - L.delta) * fast_rcp(mc * (mc - L.delta));
-    const double S2 = fast_rcp(1.0 + exp_mufu(f));
-    const double r1 = fast_rcp((mp1 > 0.0) ? mp1 : 1.0);
-    double v = exp_mufu(lnw) * (r1 * r1);
-    v = (mp2 < L.delta) ? v * S2 : v;
-    const bool ok = !out_of_range && (mp2 > 0.0);      // R15 support: m_low < m2 (<= m1)
-    w = ok ? v : 0.0;
+    float4 c;
+    if ((unsigned)ks < (unsigned)M.cap) c = M.s[ks + (gauss_only ? M.cap : 0)];
+    else c = __ldg(M.g + km + (gauss_only ? M.n_mass + 2 : 0));
+    float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x);
+    l += fmaf(F.beta2, lm2, r + ipr2);
+    l = fmaf(-2.f, lg2f(fmaxf(mp1, 1e-30f)), l);
+    // smoothing of m2 (M1): log2(e) f = (2 delta m' - delta^2) log2(e) / (m' (m' - delta)), m' clamped inside the window
+    const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
+    const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
+    const float ls = lg2f(1.0f + ex2f(f2));
+    l -= (mp2 < F.delta) ? ls : 0.f;
+    const bool ok = in_range && (mp2 > 0.f);           // R15 support: m_low < m2 (<= m1)
+    l2w = ok ? l : -INFINITY;
 }
 
 // ---- small reductions ---------------------------------------------------------------------------------
@@ -225,9 +232,8 @@ struct EventSetDev {
     int32_t max_ns, max_nz;
     const int64_t* sample_off;  // [n_events+1]
     const int64_t* grid_off;    // [n_events+1]
-    const double2* recA;        // {tk, m1d}         per sample, sorted by d_L within each event
-    const double2* recB;        // {q = m2d/m1d, ln m1d}
-    const double2* recC;        // {ln q, 1/pi}
+    const float4* recA;         // packed sample records (see above), sorted by d_L within each event
+    const float4* recB;
     const int32_t* perm;        // sorted position -> caller's index within the event
     const double* zc;           // z_g - z0_i  (centred grid)
     const float* qn;            // p_gal(z_g) * trapezoid weight / (the event's largest such product)
@@ -235,6 +241,8 @@ struct EventSetDev {
     const double* z0;           // [n_events] centre of each event's grid
     const double* lnm1_lo;      // [n_events] smallest / largest ln m1d of the event's samples
     const double* lnm1_hi;
+    const int32_t* k_lo;        // [n_events] first / last row of the z(ln d_L) table the event's samples address
+    const int32_t* k_hi;
     const double* fixed_bw;     // [n_events] or null
 };
 
@@ -242,7 +250,7 @@ struct EventKernelParams {
     EventSetDev ev;
     const LamConst* Lc;      // [n_lambda]
     const Row* tab;          // [n_lambda][rows]
-    const MassRow* mtab;     // [n_lambda][n_mass+2]
+    const MassRow* mtab;     // [n_lambda][2][n_mass+2]
     const double* dc_tab;    // [n_lambda][n_table+1+kZPad] (placement ON_GRID only) or null
     int32_t n_lambda, tab_rows, n_mass, n_table;
     int32_t placement, bw_rule, kde_method;
@@ -260,7 +268,7 @@ struct EventKernelParams {
 struct InjSetDev {
     int64_t n_det;
     double n_inj_total;
-    const double2* recA; const double2* recB; const double2* recC;  // sorted by d_L
+    const float4* recA; const float4* recB;   // packed injection records, sorted by d_L
     const int64_t* perm;
 };
 
@@ -288,7 +296,7 @@ struct CombineParams {
 cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P, LamConst* Lc, double* dc_tab,
                           Row* tab_ev, Row* tab_inj, MassRow* mtab, cudaStream_t st);
 
-cudaError_t launch_events(const EventKernelParams& P, cudaStream_t st);
+cudaError_t launch_events(const EventKernelParams& P, bool count_pairs, cudaStream_t st);
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st);
 cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);
 cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, int64_t n, const double* dL,

@@ -1,8 +1,11 @@
 // k_events.cu -- steps S2 + S3 + S4 fused: one CTA per (event, lambda).
 //
-//   S2  per posterior sample: z_j from the per-lambda table, source masses, population weight w_j
-//       (sample_weight, chim_internal.cuh), weighted moments -> Scott bandwidth h (R3), all in fp64.
-//       z_j and w_j never leave shared memory.
+//   S2  per posterior sample: z_j from the per-lambda table, source masses, log2 of the population weight
+//       (sample_eval, chim_internal.cuh), all fp32 with hi + lo pairs where differences cancel.  The slice of the
+//       per-lambda z(ln d_L) table the event addresses and the matching slice of the mass table are brought into
+//       shared memory by TMA bulk copies (cp.async.bulk + mbarrier) issued by one thread; the packed sample records
+//       are streamed from L2 with coalesced 128-bit loads.  A second sweep over shared memory turns log2 w into
+//       w / max w and forms the weighted moments -> Scott bandwidth h (R3).  z_j and w_j never leave shared memory.
 //   S3+S4  I_i = sum_g q_g K(z_g) = (1/(N_s h sqrt(2 pi))) sum_j w_j A_j,  A_j = sum_g q_g exp(-(z_g - z_j)^2 / 2h^2),
 //       q_g = p_gal(z_g) x trapezoid weight (eq. 19 evaluated on the grid, eq. 14).
 //       Samples in lanes (4 per lane, 128 per warp pass, sorted in z), grid points streamed from shared memory;
@@ -32,13 +35,9 @@ constexpr int kEvThreads = CHIM_EV_THREADS;   // 256 x 3 CTAs per SM measured fa
 constexpr int kPass = 128;               // samples per warp pass (4 per lane)
 constexpr float kMaxBlockSpan = 4.8f;    // B * delta limit of the power form
 constexpr float kMaxPowExp = 100.f;      // bound on log2 of the largest s^b inside a block (fp32 overflow guard)
-constexpr int kMassStage = 384;          // mass-table rows staged per CTA during S2 (aliases the grid array of S3)
+constexpr int kRowStage = 224;           // rows of the z(ln d_L) table staged per CTA (14 KB)
+constexpr int kMassStage = 384;          // mass-table rows staged per CTA and variant (2 x 6 KB)
 
-__device__ __forceinline__ float ex2_approx(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
 typedef unsigned long long f32x2;        // two packed floats (lo, hi) for the FFMA2 pipe
 __device__ __forceinline__ f32x2 pack2(float lo, float hi) {
     f32x2 r;
@@ -52,6 +51,40 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
     f32x2 d;
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
     return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+// ---- TMA bulk copy + mbarrier (one-shot: phase 0) ---------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* b) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(b))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok)
+                     : "r"(smem_u32(b)), "r"(parity)
+                     : "memory");
+    } while (!ok);
 }
 
 // psi(z)/J(z) at a grid point for placement ON_GRID (paper eq. 14 literally); d_C from the global table.
@@ -76,26 +109,33 @@ __device__ double grid_factor(const LamConst& L, const double* __restrict__ dc, 
 struct EvSmem {
     LamConst L;
     double red[4 * (kEvThreads / 32)];
+    float fred[kEvThreads / 32];
+    unsigned long long mbar;
     int pass_counter;
-    int pad_;
+    int mass_lo;
 };
 
 __host__ __device__ inline size_t ev_ns_pad(size_t ns) { return (ns + kPass - 1) / kPass * kPass; }
 __host__ __device__ inline size_t ev_nz_pad(size_t nz) { return (nz + 31) / 32 * 32; }
-__host__ __device__ inline size_t ev_aux_bytes(size_t nz) {   // S2: staged mass rows; S3: (q', q') or (x_g, q_g) per grid point
-    size_t a = sizeof(float2) * ev_nz_pad(nz), b = (size_t)kMassStage * 32;
+__host__ __device__ inline size_t ev_aux_bytes(size_t nz) {   // S2: staged table + mass rows; S3: (q', q') or (x_g, q_g) per grid point
+    size_t a = sizeof(float2) * ev_nz_pad(nz), b = (size_t)kRowStage * sizeof(Row) + 2 * (size_t)kMassStage * sizeof(MassRow);
     return a > b ? a : b;
 }
 
 // One block of B grid points for the 4 samples of a lane: tot_k += 2^(-u_k^2) * sum_b q'_b s_k^b (Horner, FFMA2).
 template <int B>
-__device__ __forceinline__ void power_block(const ulonglong2* __restrict__ qp, float xs, float cs, const float (&x)[4],
+__device__ __forceinline__ void power_block(const ulonglong2* __restrict__ qp, f32x2 xs2, f32x2 cs2, f32x2 nx01, f32x2 nx23,
                                             f32x2& tot01, f32x2& tot23) {
-    const float u0 = xs - x[0], u1 = xs - x[1], u2 = xs - x[2], u3 = xs - x[3];
-    const f32x2 s01 = pack2(ex2_approx(cs * u0), ex2_approx(cs * u1));
-    const f32x2 s23 = pack2(ex2_approx(cs * u2), ex2_approx(cs * u3));
-    const f32x2 e01 = pack2(ex2_approx(-u0 * u0), ex2_approx(-u1 * u1));
-    const f32x2 e23 = pack2(ex2_approx(-u2 * u2), ex2_approx(-u3 * u3));
+    const f32x2 u01 = add2(xs2, nx01), u23 = add2(xs2, nx23);          // u = x_a - x_j
+    const f32x2 su01 = mul2(u01, cs2), su23 = mul2(u23, cs2);          // -2 delta u
+    const f32x2 q01 = mul2(u01, u01), q23 = mul2(u23, u23);            // u^2
+    float a, b, c, d;
+    unpack2(su01, a, b);
+    unpack2(su23, c, d);
+    const f32x2 s01 = pack2(ex2f(a), ex2f(b)), s23 = pack2(ex2f(c), ex2f(d));
+    unpack2(q01, a, b);
+    unpack2(q23, c, d);
+    const f32x2 e01 = pack2(ex2f(-a), ex2f(-b)), e23 = pack2(ex2f(-c), ex2f(-d));
     f32x2 a01 = 0ull, a23 = 0ull;     // (+0.f, +0.f)
 #pragma unroll
     for (int i = B / 2 - 1; i >= 0; --i) {
@@ -113,25 +153,66 @@ template <int B>
 __device__ __forceinline__ void power_pass(const float2* __restrict__ gq, int a_lo, int a_hi, float xfirst, float delta,
                                            const float (&x)[4], float (&A)[4]) {
     f32x2 tot01 = 0ull, tot23 = 0ull;
-    const float cs = -2.f * delta;
+    const float cs = -2.f * delta, bd = (float)B * delta;
+    const f32x2 cs2 = pack2(cs, cs), nx01 = pack2(-x[0], -x[1]), nx23 = pack2(-x[2], -x[3]);
+    float af = (float)a_lo;
+    const ulonglong2* qp = reinterpret_cast<const ulonglong2*>(gq + a_lo * B);
 #pragma unroll 1
     for (int a = a_lo; a <= a_hi; ++a) {
-        const float xs = fmaf((float)(a * B), delta, xfirst);
-        power_block<B>(reinterpret_cast<const ulonglong2*>(gq + a * B), xs, cs, x, tot01, tot23);
+        const float xs = fmaf(af, bd, xfirst);     // exact block origin: no drift from block to block
+        power_block<B>(qp, pack2(xs, xs), cs2, nx01, nx23, tot01, tot23);
+        af += 1.0f;
+        qp += B / 2;
     }
     unpack2(tot01, A[0], A[1]);
     unpack2(tot23, A[2], A[3]);
 }
 
-// shared-memory layout after EvSmem: wbuf double[ns_pad] | zf float[ns_pad] | aux = gq float2[nz_pad] / staged mass rows
+// S2 sweep 1 over the event's samples: z_j - z0 and log2 w_j to shared memory; returns the thread's max log2 w.
+template <bool kStaged>
+__device__ __forceinline__ float s2_sweep(const EventKernelParams& P, const LamF& F, const float4* __restrict__ rows,
+                                          int k_base, int tab_rows, const MassLookup& M, int64_t s0, int ns, float z0h, float z0l,
+                                          float* __restrict__ zf, float* __restrict__ wl, int& oor) {
+    float mx = -INFINITY;
+    const int tid = threadIdx.x;
+#pragma unroll 2
+    for (int j = tid; j < ns; j += kEvThreads) {
+        const float4 A = ldg_stream4(P.ev.recA + s0 + j), Bq = ldg_stream4(P.ev.recB + s0 + j);
+        const uint32_t tkq = __float_as_uint(A.x);
+        const int k = min(max((int)(tkq >> kTkFracBits), 1), tab_rows - 2);
+        const float t = __uint_as_float(0x3F800000u | ((tkq << (32 - kTkFracBits)) >> 9)) - 1.0f;
+        const bool in_range = tkq <= F.tkmax_ev_q;
+        float4 q0, q1, q2, q3;
+        if (kStaged) {
+            const float4* r = rows + 4 * (k - k_base);
+            q0 = r[0]; q1 = r[1]; q2 = r[2]; q3 = r[3];
+        } else {
+            const float4* r = rows + 4 * (size_t)k;
+            q0 = __ldg(r); q1 = __ldg(r + 1); q2 = __ldg(r + 2); q3 = __ldg(r + 3);
+        }
+        float zc, l2w;
+        sample_eval(F, q0, q1, q2, q3, t, z0h, z0l, A.y, A.z, A.w, Bq.x, Bq.y, Bq.z, Bq.w, M, in_range, zc, l2w);
+        oor |= (int)!in_range;
+        zf[j] = zc;
+        wl[j] = l2w;
+        mx = fmaxf(mx, l2w);
+    }
+    return mx;
+}
+
+// shared-memory layout after EvSmem: zf float[ns_pad] | wl float[ns_pad] | aux = staged table rows + mass rows (S2) / gq float2[nz_pad] (S3)
+template <bool kStats>
 __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKernelParams P) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     EvSmem& S = *reinterpret_cast<EvSmem*>(smem_raw);
-    double* wbuf = reinterpret_cast<double*>(smem_raw + ((sizeof(EvSmem) + 15) / 16) * 16);
+    float* zf = reinterpret_cast<float*>(smem_raw + ((sizeof(EvSmem) + 127) / 128) * 128);
     const size_t ns_pad = ev_ns_pad(P.ev.max_ns);
-    float* zf = reinterpret_cast<float*>(wbuf + ns_pad);
-    float2* gq = reinterpret_cast<float2*>(zf + ns_pad);
-    const int tid = threadIdx.x, lane = tid & 31;
+    float* wl = zf + ns_pad;
+    unsigned char* aux = reinterpret_cast<unsigned char*>(wl + ns_pad);
+    float2* gq = reinterpret_cast<float2*>(aux);
+    float4* rows_s = reinterpret_cast<float4*>(aux);
+    MassRow* mass_s = reinterpret_cast<MassRow*>(aux + (size_t)kRowStage * sizeof(Row));
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
 
     int l, ev;
     if (P.dbg_event >= 0) { l = blockIdx.x; ev = P.dbg_event; }
@@ -139,13 +220,21 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const int64_t s0 = P.ev.sample_off[ev], g0 = P.ev.grid_off[ev];
     const int ns = (int)(P.ev.sample_off[ev + 1] - s0), nz = (int)(P.ev.grid_off[ev + 1] - g0);
     double* out = (P.dbg_event >= 0) ? P.logI + l : P.logI + (size_t)l * P.ev.n_events + ev;
+    const Row* tab = P.tab + (size_t)l * P.tab_rows;
+    const MassRow* mtab = P.mtab + (size_t)l * 2 * (P.n_mass + 2);
+    const int k_lo = P.ev.k_lo[ev], k_hi = P.ev.k_hi[ev];       // table rows the event's samples address
+    const bool staged = (k_hi - k_lo + 1) <= kRowStage;
+    const int mcap = min(kMassStage, P.n_mass + 2);
 
     {   // stage the per-lambda constants in shared memory
         const int nw = sizeof(LamConst) / 4;
         const uint32_t* src = reinterpret_cast<const uint32_t*>(P.Lc + l);
         uint32_t* dst = reinterpret_cast<uint32_t*>(&S.L);
         for (int i = tid; i < nw; i += kEvThreads) dst[i] = src[i];
-        if (tid == 0) S.pass_counter = 0;
+        if (tid == 0) {
+            S.pass_counter = 0;
+            mbar_init(&S.mbar, 1);
+        }
     }
     __syncthreads();
     const LamConst& L = S.L;
@@ -153,80 +242,87 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         if (tid == 0) *out = NAN;
         return;
     }
-    const Row* tab = P.tab + (size_t)l * P.tab_rows;
     const double z0 = P.ev.z0[ev];
 
-    // ---- stage the mass-table rows this event can address: ln m1 = ln m1d - ln(1+z), z between the event's first and
-    //      last (sorted) sample; rows outside the staged range fall back to global memory inside sample_weight ----------
+    // ---- TMA: the event's slice of the z(ln d_L) table and the mass-table rows it can address: ln m1 = ln m1d - ln(1+z),
+    //      z between the event's first and last (sorted) sample; rows outside the staged range fall back to global
+    //      memory inside sample_eval ----------------------------------------------------------------------------
+    if (tid == 0) {
+        const float u_lo = tab[k_lo].u0, u_hi = tab[min(k_hi + 1, P.tab_rows - 1)].u0;   // ln(1+z) at the bracketing nodes
+        const int ma = max(1, min((int)fma(P.ev.lnm1_lo[ev] - (double)u_hi - L.lm0, L.inv_dlm, 1.0), P.n_mass));
+        const int mb = max(1, min((int)fma(P.ev.lnm1_hi[ev] - (double)u_lo - L.lm0, L.inv_dlm, 1.0), P.n_mass));
+        int mlo = ma - 1 + max(0, (mb - ma + 3 - mcap) / 2);                              // wider than the stage: keep the centre
+        mlo = max(0, min(mlo, P.n_mass + 2 - mcap));
+        S.mass_lo = mlo;
+        const uint32_t rb = staged ? (uint32_t)(k_hi - k_lo + 1) * (uint32_t)sizeof(Row) : 0u, mbytes = (uint32_t)mcap * (uint32_t)sizeof(MassRow);
+        mbar_expect_tx(&S.mbar, rb + 2 * mbytes);
+        if (staged) bulk_g2s(rows_s, tab + k_lo, rb, &S.mbar);
+        bulk_g2s(mass_s, mtab + mlo, mbytes, &S.mbar);
+        bulk_g2s(mass_s + mcap, mtab + (P.n_mass + 2) + mlo, mbytes, &S.mbar);
+    }
+    __syncthreads();     // publishes S.mass_lo
     MassLookup M;
-    M.g = P.mtab + (size_t)l * (P.n_mass + 2);
+    M.g = mtab;
+    M.s = mass_s;
+    M.lo = S.mass_lo;
+    M.cap = mcap;
     M.n_mass = P.n_mass;
-    M.cap = kMassStage;
-    {
-        double2* sA = reinterpret_cast<double2*>(gq);
-        double2* sB = sA + kMassStage;
-        const int ka = max(1, min((int)P.ev.recA[s0].x, P.tab_rows - 2)), kb = max(1, min((int)P.ev.recA[s0 + ns - 1].x, P.tab_rows - 2));
-        const double u_lo = tab[ka].c[1][0], u_hi = tab[kb + 1].c[1][0];      // ln(1+z) at the bracketing nodes
-        const int ma = max(1, min((int)fma(P.ev.lnm1_lo[ev] - u_hi - L.lm0, L.inv_dlm, 1.0), P.n_mass));
-        const int mb = max(1, min((int)fma(P.ev.lnm1_hi[ev] - u_lo - L.lm0, L.inv_dlm, 1.0), P.n_mass));
-        M.lo = ma + max(0, (mb - ma + 1 - kMassStage) / 2);                   // wider than the stage: keep the centre
-        for (int i = tid; i < kMassStage; i += kEvThreads) {
-            const int r = min(M.lo + i, P.n_mass + 1);
-            double2 hi;
-            const double2 lo = ldg256_lo(reinterpret_cast<const double*>(M.g + r), hi);
-            sA[i] = lo;
-            sB[i] = hi;
-        }
-        M.sA = sA;
-        M.sB = sB;
-    }
-    __syncthreads();
+    mbar_wait(&S.mbar, 0);
 
-    // ---- S2: weights + centred moments -----------------------------------------------------------------
-    double mom[4] = {0.0, 0.0, 0.0, 0.0};   // sum w, sum w^2, sum w z', sum w z'^2
+    // ---- S2, sweep 1: z_j - z0 and log2 w_j -------------------------------------------------------------
+    const float z0h = (float)z0, z0l = (float)(z0 - (double)z0h);
     int oor = 0;
-    // software pipeline: the next sample's table coordinate is read one iteration ahead and its row prefetched to L1
-    double2 A = (tid < ns) ? ldg_stream(P.ev.recA + s0 + tid) : make_double2(1.0, 1.0);
-#pragma unroll 1
-    for (int j = tid; j < ns; j += kEvThreads) {
-        const double2 B = ldg_stream(P.ev.recB + s0 + j), C = ldg_stream(P.ev.recC + s0 + j);
-        double2 An = A;
-        if (j + kEvThreads < ns) {
-            An = ldg_stream(P.ev.recA + s0 + j + kEvThreads);
-            prefetch_l1(tab + max(1, min((int)An.x, P.tab_rows - 2)));
-        }
-        double z, w;
-        bool o;
-        sample_weight(L, tab, P.tab_rows, M, L.tkmax_ev, P.z_table_max, A.x, A.y, B.x, B.y, C.x, C.y, z, w, o);
-        oor |= (int)o;
-        double zc = z - z0;
-        zf[j] = (float)zc;
-        wbuf[j] = w;
-        mom[0] += w;
-        mom[1] = fma(w, w, mom[1]);
-        double wz = w * zc;
-        mom[2] += wz;
-        mom[3] = fma(wz, zc, mom[3]);
-        if (P.dbg_z) {
-            int jo = P.ev.perm[s0 + j];
-            P.dbg_z[jo] = z;
-            P.dbg_w[jo] = w * exp(P.ln_shift[ev]);
-        }
-        A = An;
-    }
-    block_sum<kEvThreads, 4>(mom, S.red);
+    float mx;
+    if (staged) mx = s2_sweep<true>(P, L.F, rows_s, k_lo, P.tab_rows, M, s0, ns, z0h, z0l, zf, wl, oor);
+    else mx = s2_sweep<false>(P, L.F, reinterpret_cast<const float4*>(tab), 0, P.tab_rows, M, s0, ns, z0h, z0l, zf, wl, oor);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if (lane == 0) S.fred[wid] = mx;
     oor = __syncthreads_or(oor);
     if (oor && tid == 0) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
-
-    const double sw = mom[0];
-    if (!(sw > 0.0)) {   // all-zero event (R15): I = 0
+#pragma unroll
+    for (int k = 0; k < kEvThreads / 32; ++k) mx = fmaxf(mx, S.fred[k]);
+    if (!(mx > -INFINITY)) {   // all-zero event (R15): I = 0
         if (tid == 0) {
-            *out = isnan(sw) ? NAN : -INFINITY;
+            *out = (mx != mx) ? NAN : -INFINITY;
             atomicOr(P.flags + l, CHIM_FLAG_EVENT_ZERO);
             if (P.dbg_h) *P.dbg_h = NAN;
         }
+        if (P.dbg_z)
+            for (int j = tid; j < ns; j += kEvThreads) {
+                const int jo = P.ev.perm[s0 + j];
+                P.dbg_z[jo] = z0 + (double)zf[j];
+                P.dbg_w[jo] = 0.0;
+            }
         return;
     }
+
+    // ---- S2, sweep 2: w_j / max w, moments about the median sample (sorted: the middle one) -> bandwidth ----------
+    const float zmed = zf[ns >> 1], zlast = zf[ns - 1];
+    float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;   // sum w, sum w^2, sum w z', sum w z'^2
+    const int nsp = (int)ev_ns_pad(ns);
+    for (int j = tid; j < nsp; j += kEvThreads) {
+        if (j < ns) {
+            const float w = ex2f(wl[j] - mx), zc = zf[j] - zmed;
+            wl[j] = w;
+            m0 += w;
+            m1 = fmaf(w, w, m1);
+            const float wz = w * zc;
+            m2 += wz;
+            m3 = fmaf(wz, zc, m3);
+            if (P.dbg_z) {
+                const int jo = P.ev.perm[s0 + j];
+                P.dbg_z[jo] = z0 + (double)zf[j];
+                P.dbg_w[jo] = (double)w * exp2((double)mx) * exp(P.ln_shift[ev]);
+            }
+        } else {                                    // idle slots of the last pass sit on the last sample with weight 0
+            wl[j] = 0.f;
+            zf[j] = zlast;
+        }
+    }
+    double mom[4] = {(double)m0, (double)m1, (double)m2, (double)m3};
+    block_sum<kEvThreads, 4>(mom, S.red);
+    const double sw = mom[0];
     double h;
     if (P.bw_rule == CHIM_BW_FIXED) {
         h = P.ev.fixed_bw[ev];
@@ -249,7 +345,6 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const double sc = sqrt(kHalfLog2e) / h;
     const float scf = (float)sc;
     const double scd = (double)scf;             // samples and grid are scaled by the SAME rounded factor
-    const double wscale = (double)ns / sw;      // weights normalised to mean 1
     const float T = (P.cutoff > 0.0) ? (float)(P.cutoff * sqrt(kHalfLog2e)) : INFINITY;
     const double* zc_g = P.ev.zc + g0;
     const float* qn_g = P.ev.qn + g0;
@@ -262,7 +357,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     }
     const int nzp = (int)ev_nz_pad(nz);
     const bool on_grid = P.placement == CHIM_ON_GRID;
-    for (int g = tid; g < nzp; g += kEvThreads) {
+    for (int g = tid; g < nzp; g += kEvThreads) {   // (the block reduction above fenced the last reads of the staged tables)
         float q = 0.f, xg = 0.f;
         if (g < nz) {
             q = qn_g[g];
@@ -273,7 +368,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         }
         if (Bsel) {
             const float bd = (float)(g & (Bsel - 1)) * delta;
-            q *= ex2_approx(-bd * bd);
+            q *= ex2f(-bd * bd);
             gq[g] = make_float2(q, q);
         } else {
             gq[g] = make_float2(xg, q);
@@ -293,26 +388,12 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         if (pass >= n_pass) break;
         const int j0 = pass * kPass + lane * 4;
         const float4 zz = *reinterpret_cast<const float4*>(zf + j0);
-        const double2 w01 = *reinterpret_cast<const double2*>(wbuf + j0), w23 = *reinterpret_cast<const double2*>(wbuf + j0 + 2);
-        double w[4] = {w01.x, w01.y, w23.x, w23.y};
-        float x[4] = {zz.x * scf, zz.y * scf, zz.z * scf, zz.w * scf};
-        float xmn = INFINITY, xmx = -INFINITY;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const bool valid = (j0 + k < ns) && (w[k] > 0.0);   // zero-weight samples (R15) take no part
-            w[k] = valid ? w[k] * wscale : 0.0;
-            x[k] = valid ? x[k] : NAN;
-            xmn = valid ? fminf(xmn, x[k]) : xmn;
-            xmx = valid ? fmaxf(xmx, x[k]) : xmx;
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            xmn = fminf(xmn, __shfl_xor_sync(0xffffffffu, xmn, o));
-            xmx = fmaxf(xmx, __shfl_xor_sync(0xffffffffu, xmx, o));
-        }
-        if (!(xmn <= xmx)) continue;             // no sample of this pass carries weight
-#pragma unroll
-        for (int k = 0; k < 4; ++k) x[k] = (x[k] == x[k]) ? x[k] : xmn;   // idle slots sit inside the band
+        const float4 ww = *reinterpret_cast<const float4*>(wl + j0);
+        const float w[4] = {ww.x, ww.y, ww.z, ww.w};
+        const float x[4] = {zz.x * scf, zz.y * scf, zz.z * scf, zz.w * scf};
+        // samples are sorted in z: the pass spans [first, last] (idle slots repeat the last sample)
+        const float xa = zf[pass * kPass] * scf, xb = zf[pass * kPass + kPass - 1] * scf;
+        const float xmn = fminf(xa, xb), xmx = fmaxf(xa, xb);
         float A[4] = {0.f, 0.f, 0.f, 0.f};
         bool done = false;
         if (Bsel) {
@@ -324,7 +405,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
                 if (a_hi >= a_lo) {
                     if (Bsel == 32) power_pass<32>(gq, a_lo, a_hi, xfirst, delta, x, A);
                     else power_pass<16>(gq, a_lo, a_hi, xfirst, delta, x, A);
-                    if (lane == 0) pairs_exec += (unsigned long long)(a_hi - a_lo + 1) * Bsel * kPass;
+                    if (kStats && lane == 0) pairs_exec += (unsigned long long)(a_hi - a_lo + 1) * Bsel * kPass;
                 }
                 done = true;
             }
@@ -349,9 +430,9 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
 #pragma unroll 1
                 for (int g = g_lo; g <= g_hi; ++g) {
                     const float bdg = (float)(g & (Bsel - 1)) * delta;
-                    const float xg = fmaf((float)g, delta, xfirst), q = gq[g].x * ex2_approx(bdg * bdg);
+                    const float xg = fmaf((float)g, delta, xfirst), q = gq[g].x * ex2f(bdg * bdg);
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) { const float d = xg - x[k]; A[k] = fmaf(q, ex2_approx(-d * d), A[k]); }
+                    for (int k = 0; k < 4; ++k) { const float d = xg - x[k]; A[k] = fmaf(q, ex2f(-d * d), A[k]); }
                 }
             } else if (P.dbg_K) {
 #pragma unroll 1
@@ -360,9 +441,9 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
                     float kv = 0.f;
 #pragma unroll
                     for (int k = 0; k < 4; ++k) {
-                        const float d = v.x - x[k], e = ex2_approx(-d * d);
+                        const float d = v.x - x[k], e = ex2f(-d * d);
                         A[k] = fmaf(v.y, e, A[k]);
-                        kv = fmaf((float)w[k], e, kv);
+                        kv = fmaf(w[k], e, kv);
                     }
                     double kd = warp_sum((double)kv);
                     if (lane == 0) atomicAdd(P.dbg_K + g, kd);
@@ -372,57 +453,66 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
                 for (int g = g_lo; g <= g_hi; ++g) {
                     const float2 v = gq[g];
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) { const float d = v.x - x[k]; A[k] = fmaf(v.y, ex2_approx(-d * d), A[k]); }
+                    for (int k = 0; k < 4; ++k) { const float d = v.x - x[k]; A[k] = fmaf(v.y, ex2f(-d * d), A[k]); }
                 }
             }
-            if (lane == 0 && g_hi >= g_lo) pairs_exec += (unsigned long long)(g_hi - g_lo + 1) * kPass;
+            if (kStats && lane == 0 && g_hi >= g_lo) pairs_exec += (unsigned long long)(g_hi - g_lo + 1) * kPass;
         }
+        lsum += (double)fmaf(w[0], A[0], fmaf(w[1], A[1], fmaf(w[2], A[2], w[3] * A[3])));
+        if (kStats) {
+            if (udz > 0.0 && T < INFINITY) {   // algorithmic pair count: grid points within the cut-off of each weighted sample
 #pragma unroll
-        for (int k = 0; k < 4; ++k) lsum = fma(w[k], (double)A[k], lsum);
-        if (udz > 0.0 && T < INFINITY) {   // algorithmic pair count: grid points within the cut-off of each weighted sample
+                for (int k = 0; k < 4; ++k)
+                    if (w[k] > 0.f) {
+                        const int a = max(0, (int)ceilf((x[k] - T - xfirst) * inv_delta)), b = min(nz - 1, (int)floorf((x[k] + T - xfirst) * inv_delta));
+                        pairs_cut += (unsigned long long)max(0, b - a + 1);
+                    }
+            } else {
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-                if (w[k] > 0.0) {
-                    const int a = max(0, (int)ceilf((x[k] - T - xfirst) * inv_delta)), b = min(nz - 1, (int)floorf((x[k] + T - xfirst) * inv_delta));
-                    pairs_cut += (unsigned long long)max(0, b - a + 1);
-                }
-        } else if (lane == 0) {
-            pairs_cut += (unsigned long long)nz * min(kPass, ns - pass * kPass);
+                for (int k = 0; k < 4; ++k) pairs_cut += (w[k] > 0.f) ? (unsigned long long)nz : 0ull;
+            }
         }
     }
-    // K(z) = 1/(N_s h sqrt(2 pi)) sum_j w_j exp(..): undo the weight normalisation (sw/ns)
-    const double knorm = (sw / ns) / ((double)ns * h * 2.50662827463100050242);
+    // K(z) = 1/(N_s h sqrt(2 pi)) sum_j w_j exp(..); the weights were divided by 2^mx
+    const double knorm = 1.0 / ((double)ns * h * 2.50662827463100050242);
+    const double ln_wscale = (double)mx * 0.69314718055994530942;
     double tot[3] = {lsum, (double)pairs_exec, (double)pairs_cut};
-    block_sum<kEvThreads, 3>(tot, S.red);
-    if (tid == 0 && P.stats) {
-        if (tot[1] > 0.0) atomicAdd(P.stats, (unsigned long long)tot[1]);
-        if (tot[2] > 0.0) atomicAdd(P.stats + 1, (unsigned long long)tot[2]);
+    if constexpr (kStats) {
+        block_sum<kEvThreads, 3>(tot, S.red);
+        if (tid == 0 && P.stats) {
+            if (tot[1] > 0.0) atomicAdd(P.stats, (unsigned long long)tot[1]);
+            if (tot[2] > 0.0) atomicAdd(P.stats + 1, (unsigned long long)tot[2]);
+        }
+    } else {
+        double t1[1] = {lsum};
+        block_sum<kEvThreads, 1>(t1, S.red);
+        tot[0] = t1[0];
     }
     if (P.dbg_K) {   // diagnostics: turn the accumulated sums into K(z_g)
         __syncthreads();
-        const double ks = knorm * exp(P.ln_shift[ev]);
+        const double ks = knorm * exp(ln_wscale + P.ln_shift[ev]);
         for (int g = tid; g < nz; g += kEvThreads) P.dbg_K[g] *= ks;
     }
     if (tid == 0) {
         double I = tot[0] * knorm;
-        if (I > 0.0) *out = log(I) + P.ln_shift[ev] + P.ln_qscale[ev];
+        if (I > 0.0) *out = log(I) + ln_wscale + P.ln_shift[ev] + P.ln_qscale[ev];
         else if (I == 0.0) { *out = -INFINITY; atomicOr(P.flags + l, CHIM_FLAG_EVENT_ZERO); }
         else *out = NAN;
     }
 }
 
 size_t events_smem_bytes(int max_ns, int max_nz) {
-    return ((sizeof(EvSmem) + 15) / 16) * 16 + (sizeof(double) + sizeof(float)) * ev_ns_pad((size_t)max_ns) +
-           ev_aux_bytes((size_t)max_nz);
+    return ((sizeof(EvSmem) + 127) / 128) * 128 + 2 * sizeof(float) * ev_ns_pad((size_t)max_ns) + ev_aux_bytes((size_t)max_nz);
 }
 
-cudaError_t launch_events(const EventKernelParams& P, cudaStream_t st) {
+cudaError_t launch_events(const EventKernelParams& P, bool count_pairs, cudaStream_t st) {
     size_t smem = events_smem_bytes(P.ev.max_ns, P.ev.max_nz);
-    cudaError_t e = cudaFuncSetAttribute(k_events, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    auto kern = count_pairs ? k_events<true> : k_events<false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     long long nb = (P.dbg_event >= 0) ? P.n_lambda : (long long)P.n_lambda * P.ev.n_events;
     if (nb <= 0) return cudaSuccess;
-    k_events<<<(unsigned)nb, kEvThreads, smem, st>>>(P);
+    kern<<<(unsigned)nb, kEvThreads, smem, st>>>(P);
     return cudaGetLastError();
 }
 

@@ -1,13 +1,14 @@
 // k_inject.cu -- step S5 (selection term, eq. 12-13) and step S6 (combine, eq. 3).
 //
-//   S5  one CTA per (lambda, chunk of detected injections).  The lambda's mass table ("a" variant, 64 KB) is staged
-//       once in shared memory -- the injections' source masses are scattered over the whole table, and scattered
-//       16-byte reads cost an L1 wavefront each from global memory but ~1/3 of that from shared memory -- and the
-//       chunk's packed records are streamed through it with coalesced 128-bit loads (the set is sorted in d_L, so a
-//       warp's rows of the z(ln d_L) table are one or two cache lines).  CTAs in flight share a chunk (lambda is the
-//       fast grid index), so the records come from L2.  Per (injection, lambda): s_j = p_m psi u / J / p_draw via the
-//       same sample_weight() as the events (the injection table's R column carries psi u / J); z_j > z_cat_max gives
-//       s_j = 0 (R6).  Per-CTA fp64 partial sums {sum s, sum s^2}, combined in a fixed order by S6 (deterministic).
+//   S5  one CTA per (lambda, chunk of detected injections).  Both variants of the lambda's mass table (fp32 cubics,
+//       2 x 32 KB) are brought into shared memory by one TMA bulk copy -- the injections' source masses are scattered
+//       over the whole table -- and the chunk's packed records are streamed through it with coalesced 128-bit loads
+//       (the set is sorted in d_L, so a warp's rows of the z(ln d_L) table are one or two L1-resident lines).  CTAs in
+//       flight share a chunk (lambda is the fast grid index), so the records come from L2.  Per (injection, lambda):
+//       log2 s_j = log2[p_m psi u / J / p_draw] via the same sample_eval() as the events (the injection table's r
+//       column carries psi u / J); z_j > z_cat_max gives s_j = 0 (R6; the comparison is made on hi + lo pairs).
+//       s_j is widened to fp64 through the exponent field; per-CTA fp64 partial sums {sum s, sum s^2}, combined in a
+//       fixed order by S6 (deterministic).
 //   S6  log L = sum_i log I_i - N_e log xi, N_eff (eq. 13), flags.
 #include "chim_internal.cuh"
 
@@ -18,53 +19,69 @@ constexpr int kInjThreads = 256;
 struct InjSmem {
     LamConst L;
     double red[2 * (kInjThreads / 32)];
+    unsigned long long mbar;
 };
 
+__device__ __forceinline__ uint32_t inj_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
 __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     InjSmem& S = *reinterpret_cast<InjSmem*>(smem_raw);
-    double2* sA = reinterpret_cast<double2*>(smem_raw + ((sizeof(InjSmem) + 15) / 16) * 16);
-    double2* sB = sA + (P.n_mass + 2);
+    MassRow* mass_s = reinterpret_cast<MassRow*>(smem_raw + ((sizeof(InjSmem) + 127) / 128) * 128);
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int l = blockIdx.x % P.n_lambda, chunk = blockIdx.x / P.n_lambda;
     const int64_t j0 = (int64_t)chunk * P.chunk, j1 = min(j0 + (int64_t)P.chunk, P.inj.n_det);
     const int nw = sizeof(LamConst) / 4;
+    const MassRow* mtab = P.mtab + (size_t)l * 2 * (P.n_mass + 2);
+    if (tid == 0) {   // TMA: the whole mass table of this lambda (both variants are contiguous)
+        const uint32_t mb = inj_smem_u32(&S.mbar), bytes = 2u * (uint32_t)(P.n_mass + 2) * (uint32_t)sizeof(MassRow);
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(inj_smem_u32(mass_s)),
+                     "l"(mtab), "r"(bytes), "r"(mb)
+                     : "memory");
+    }
     for (int i = tid; i < nw; i += kInjThreads)
         reinterpret_cast<uint32_t*>(&S.L)[i] = reinterpret_cast<const uint32_t*>(P.Lc + l)[i];
-    MassLookup M;
-    M.g = P.mtab + (size_t)l * (P.n_mass + 2);
-    M.sA = sA; M.sB = sB; M.lo = 0; M.cap = P.n_mass + 2; M.n_mass = P.n_mass;
-    for (int r = tid; r < P.n_mass + 2; r += kInjThreads) {
-        double2 hi;
-        const double2 lo = ldg256_lo(reinterpret_cast<const double*>(M.g + r), hi);
-        sA[r] = lo;
-        sB[r] = hi;
+    __syncthreads();   // publishes S.L and the initialised barrier
+    {
+        uint32_t ok;
+        do {
+            asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n selp.u32 %0, 1, 0, p;\n}"
+                         : "=r"(ok)
+                         : "r"(inj_smem_u32(&S.mbar))
+                         : "memory");
+        } while (!ok);
     }
-    __syncthreads();
+    MassLookup M;
+    M.g = mtab;
+    M.s = mass_s;
+    M.lo = 0;
+    M.cap = P.n_mass + 2;
+    M.n_mass = P.n_mass;
     const LamConst& L = S.L;
+    const LamF& F = L.F;
     double acc[2] = {0.0, 0.0};
     int oor = 0;
     if (L.flags == 0) {
-        const Row* tab = P.tab + (size_t)l * P.tab_rows;
-        // software pipeline: next sample's table coordinate one iteration ahead, its row prefetched to L1
-        double2 A = (j0 + tid < j1) ? ldg_stream(P.inj.recA + j0 + tid) : make_double2(1.0, 1.0);
-#pragma unroll 1
+        const float4* rows = reinterpret_cast<const float4*>(P.tab + (size_t)l * P.tab_rows);
+#pragma unroll 2
         for (int64_t j = j0 + tid; j < j1; j += kInjThreads) {
-            const double2 B = ldg_stream(P.inj.recB + j), C = ldg_stream(P.inj.recC + j);
-            double2 An = A;
-            if (j + kInjThreads < j1) {
-                An = ldg_stream(P.inj.recA + j + kInjThreads);
-                prefetch_l1(tab + max(1, min((int)An.x, P.tab_rows - 2)));
-            }
-            double z, s;
-            bool o;
-            sample_weight(L, tab, P.tab_rows, M, L.tkmax_inj, P.z_table_max, A.x, A.y, B.x, B.y, C.x, C.y, z, s, o);
-            oor |= (int)o;
-            if (!(z <= P.z_cat_max)) s = 0.0;   // support of the selection-term z density (R6)
+            const float4 A = ldg_stream4(P.inj.recA + j), Bq = ldg_stream4(P.inj.recB + j);
+            const int kraw = __float_as_int(A.x);
+            const int k = min(max(kraw, 1), P.tab_rows - 2);
+            const float t = A.y;
+            const bool in_range = ((float)kraw + t) <= F.tkmax_inj;
+            const float4* r = rows + 4 * (size_t)k;
+            const float4 q0 = __ldg(r), q1 = __ldg(r + 1), q2 = __ldg(r + 2), q3 = __ldg(r + 3);
+            float zc, l2w;
+            sample_eval(F, q0, q1, q2, q3, t, F.zcat_hi, F.zcat_lo, A.z, 0.f, A.w, 0.f, Bq.x, Bq.y, Bq.z, M, in_range, zc, l2w);
+            oor |= (int)!in_range;
+            const double s = (zc <= 0.f) ? ex2_to_double(l2w) : 0.0;   // support of the selection-term z density (R6)
             acc[0] += s;
             acc[1] = fma(s, s, acc[1]);
             if (P.dbg_s) P.dbg_s[P.inj.perm[j]] = s * P.dbg_scale;
-            A = An;
         }
     }
     acc[0] = warp_sum(acc[0]);
@@ -81,7 +98,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
 }
 
 size_t inject_smem_bytes(int n_mass) {
-    return ((sizeof(InjSmem) + 15) / 16) * 16 + 2 * sizeof(double2) * (size_t)(n_mass + 2);
+    return ((sizeof(InjSmem) + 127) / 128) * 128 + 2 * sizeof(MassRow) * (size_t)(n_mass + 2);
 }
 
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st) {

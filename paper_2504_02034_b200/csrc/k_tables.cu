@@ -198,18 +198,28 @@ __device__ void build_dl_table(const DlGrid g, bool is_inj, int placement, const
         s_nodes[3 * NN + idx] = log(R);     // R > 0: psi, J and the volume factor are positive for z > 0
     }
     __syncthreads();
-    // cubic through nodes k-1..k+2 expanded in t = tk - k
+    // cubic through nodes k-1..k+2 expanded in t = tk - k; z and 1/(1+z) keep it (leading term split hi + lo),
+    // ln(1+z) and log2 R drop t^3 by Chebyshev economisation on [0,1]: t^3 ~ 1.5 t^2 - 0.5625 t + 1/32 (error c3/32)
     for (int k = threadIdx.x; k < g.K + 2; k += kTabThreads) {
-        Row r;
+        double cf[4][4];
         int i0 = max(k - 1, 0), i3 = min(k + 2, NN - 1), i2 = min(k + 1, NN - 1);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             double f0 = s_nodes[c * NN + i0], f1 = s_nodes[c * NN + k], f2 = s_nodes[c * NN + i2], f3 = s_nodes[c * NN + i3];
-            r.c[c][0] = f1;
-            r.c[c][1] = -f0 / 3.0 - 0.5 * f1 + f2 - f3 / 6.0;
-            r.c[c][2] = 0.5 * f0 - f1 + 0.5 * f2;
-            r.c[c][3] = (f3 - f0) / 6.0 + 0.5 * (f1 - f2);
+            cf[c][0] = f1;
+            cf[c][1] = -f0 / 3.0 - 0.5 * f1 + f2 - f3 / 6.0;
+            cf[c][2] = 0.5 * f0 - f1 + 0.5 * f2;
+            cf[c][3] = (f3 - f0) / 6.0 + 0.5 * (f1 - f2);
         }
+        Row r;
+        r.z_hi = (float)cf[0][0]; r.z_lo = (float)(cf[0][0] - (double)r.z_hi);
+        r.z1 = (float)cf[0][1]; r.z2 = (float)cf[0][2]; r.z3 = (float)cf[0][3];
+        r.a_hi = (float)cf[2][0]; r.a_lo = (float)(cf[2][0] - (double)r.a_hi);
+        r.a1 = (float)cf[2][1]; r.a2 = (float)cf[2][2]; r.a3 = (float)cf[2][3];
+        r.u0 = (float)(cf[1][0] + cf[1][3] / 32.0); r.u1 = (float)(cf[1][1] - 0.5625 * cf[1][3]); r.u2 = (float)(cf[1][2] + 1.5 * cf[1][3]);
+        const double l2e = 1.4426950408889634074;
+        r.r0 = (float)(l2e * (cf[3][0] + cf[3][3] / 32.0)); r.r1 = (float)(l2e * (cf[3][1] - 0.5625 * cf[3][3]));
+        r.r2 = (float)(l2e * (cf[3][2] + 1.5 * cf[3][3]));
         rows[k] = r;
     }
     __syncthreads();
@@ -266,12 +276,12 @@ __device__ void build_mass_table(const TableParams& P, const TabSmem& S, const d
         s_nodes[NN + idx] = (lnb > kLnFloor) ? lnb : kLnFloor;
     }
     __syncthreads();
+    const double l2e = 1.4426950408889634074;
     for (int k = threadIdx.x; k < K + 2; k += kTabThreads) {
-        MassRow r;
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
             const double* f = s_nodes + c * NN;
-            double* o = c ? r.b : r.a;
+            double o[4];
             if (k <= 1) {   // forward stencil through nodes k..k+3 (k = 0 is never addressed; keep it finite)
                 int b = max(k, 1);
                 double g0 = f[b], g1 = f[b + 1], g2 = f[b + 2], g3 = f[b + 3];
@@ -287,8 +297,8 @@ __device__ void build_mass_table(const TableParams& P, const TabSmem& S, const d
                 o[2] = 0.5 * f0 - f1 + 0.5 * f2;
                 o[3] = (f3 - f0) / 6.0 + 0.5 * (f1 - f2);
             }
+            rows[(size_t)c * (K + 2) + k] = make_float4((float)(l2e * o[0]), (float)(l2e * o[1]), (float)(l2e * o[2]), (float)(l2e * o[3]));
         }
-        rows[k] = r;
     }
     __syncthreads();
 }
@@ -332,7 +342,7 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         L.lm0 = log(L.m_low);
         {   // the mass table spans [ln m_low, max(ln m_top, ln m_low + 1)]
             double top = fmax(P.ln_m_top, L.lm0 + 1.0);
-            L.inv_dlm = (double)P.n_mass / ((top - L.lm0) * (1.0 + 1e-12));
+            L.inv_dlm = (double)(float)((double)P.n_mass / ((top - L.lm0) * (1.0 + 1e-6)));   // exact in fp32 (LamF::tm_scale)
         }
         S.ibad = 0;
     }
@@ -429,9 +439,23 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         double lt = log(L.dl_tabmax);
         L.tkmax_ev = P.ev.K > 0 ? (lt - P.ev.x0) / P.ev.dx + 1.0 : 0.0;
         L.tkmax_inj = P.inj.K > 0 ? (lt - P.inj.x0) / P.inj.dx + 1.0 : 0.0;
+        // fp32 constants of the sample kernels
+        const double l2e = 1.4426950408889634074;
+        LamF& F = L.F;
+        F.mlow_hi = (float)L.m_low; F.mlow_lo = (float)(L.m_low - (double)F.mlow_hi);
+        F.lm0_hi = (float)L.lm0; F.lm0_lo = (float)(L.lm0 - (double)F.lm0_hi);
+        F.delta = (float)L.delta;
+        F.two_dl2e = (float)(2.0 * L.delta * l2e); F.d2l2e = (float)(L.delta * L.delta * l2e);
+        F.win_lo = (float)(L.delta * 1e-3); F.win_hi = (float)(L.delta * (1.0 - 1e-6));   // S(m' < 1e-3 delta) < e^-998: "0" either way
+        F.beta2 = (float)(L.beta * l2e);
+        F.mhigh_p = (float)(L.m_high - L.m_low);
+        F.tm_scale = (float)L.inv_dlm; F.tm_max = (float)P.n_mass + 0.999f;
+        F.tkmax_ev = (float)fmin(L.tkmax_ev, 1e9) * (1.0f - 1e-6f); F.tkmax_inj = (float)fmin(L.tkmax_inj, 1e9) * (1.0f - 1e-6f);
+        F.zcat_hi = (float)P.z_cat_max; F.zcat_lo = (float)(P.z_cat_max - (double)F.zcat_hi);
+        F.tkmax_ev_q = (L.tkmax_ev >= 4095.9) ? 0xFFFFFFFFu : (L.tkmax_ev <= 0.0 ? 0u : (uint32_t)(L.tkmax_ev * (double)(1u << kTkFracBits)));
     }
     __syncthreads();
-    build_mass_table(P, S, s_w, s_nodes, mtab + (size_t)l * (P.n_mass + 2));
+    build_mass_table(P, S, s_w, s_nodes, mtab + (size_t)l * 2 * (P.n_mass + 2));
     if (P.ev.K > 0)
         build_dl_table(P.ev, false, P.placement, S, s_dc, s_dl, dz, nz_nodes, s_nodes, tab_ev + (size_t)l * P.ev.rows());
     if (P.inj.K > 0)
@@ -471,8 +495,10 @@ __global__ void k_table_lookup(const LamConst* __restrict__ Lc, const Row* __res
         else if (tk >= 1.0 && tk < g.K + 1.0) {
             int k = (int)tk;
             double t = tk - k;
-            z = horner3(tab[k].c[0], t);
-            r = exp(horner3(tab[k].c[3], t));
+            const Row& q = tab[k];
+            const double tt = (double)(float)t;
+            z = (double)q.z_hi + ((double)q.z_lo + tt * ((double)q.z1 + tt * ((double)q.z2 + tt * (double)q.z3)));
+            r = exp2((double)q.r0 + tt * ((double)q.r1 + tt * (double)q.r2));
         }
     }
     if (z_out) z_out[i] = z;

@@ -31,6 +31,7 @@ def _ctx(P, w, **kw):
 def _gpu(P, w, lam=None, fixed_bw=None, **kw):
     import torch
     kw.setdefault("z_cat_max", w.z_cat_max)
+    kw.setdefault("count_pairs", 1)
     c = P.Context(**kw)
     c.init_workload(w, fixed_bw=fixed_bw)
     lam = w.lam if lam is None else np.atleast_2d(lam)
@@ -64,10 +65,12 @@ def test_s1_table_inversion_and_ratio(P):
         dl = np.exp(rng.uniform(np.log(w.dL.min()), np.log(w.dL.max()), 4000))
         z, r = c.debug_table_lookup(la, dl)
         zr = O.z_of_dl(la, dl)
-        assert np.max(np.abs(z - zr)) < 1e-10          # budget: systematic dz must stay < 1e-7
+        # fp32 rows: z = hi + lo + cubic with float coefficients (c1 ~ 0.02 rounded to 6e-8 relative; the budget is a
+        # systematic dz < 1e-7); log2 R is a float quadratic of magnitude ~16 (half an ulp = 1e-6)
+        assert np.max(np.abs(z - zr)) < 3e-9
         d = O.distances(la, zr)
         ratio = O.psi(la, zr) / ((1 + zr) ** 3 * np.abs(d["ddl_gw_dz"]))
-        assert np.max(np.abs(r / ratio - 1)) < 1e-9
+        assert np.max(np.abs(r / ratio - 1)) < 2e-6
     c.close()
 
 
@@ -81,14 +84,16 @@ def test_s2_sample_redshifts_and_weights(P, lam_kw):
         s = slice(w.sample_off[ev], w.sample_off[ev + 1])
         z, wt = c.debug_event_samples(la, ev)
         zr, wr, _ = O.sample_weights(la, w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s])
-        assert np.max(np.abs(z - zr)) < 1e-10
+        # z_j - z0 is kept as one float (|z_j - z0| < 0.5: half an ulp is 3e-8)
+        assert np.max(np.abs(z - zr)) < 5e-8
         mism = (wt == 0) != (wr == 0)
         assert np.all(np.maximum(wt, wr)[mism] < 1e-12 * wr.max())
-        # two MUFU.EX2 per weight: relative error <= 2.4e-7 each, also for the tiny weights deep in
-        # the smoothing window; its mean (a common factor of every I_i and of xi) cancels in log L
-        nz = wr > 0
-        assert np.max(np.abs(wt[nz] / wr[nz] - 1)) < 1e-6
-        assert abs(np.mean(wt[nz] / wr[nz] - 1)) < 5e-8
+        # log2 w is a float sum of magnitude ~30-60 (half an ulp = 2e-6 relative in w) + five MUFU ops (DESIGN.md
+        # sec. 7): independent from sample to sample, so the event sum is far more accurate than one weight;
+        # weights below 1e-30 of the largest (deep in the smoothing window) may flush to zero in fp32
+        nz = wr > 1e-30 * wr.max()
+        assert np.max(np.abs(wt[nz] / wr[nz] - 1)) < 2e-5
+        assert abs(np.sum(wt[nz]) / np.sum(wr[nz]) - 1) < 5e-7
     c.close()
 
 
@@ -102,7 +107,7 @@ def test_s3_bandwidth_and_kde_on_grid(P):
         h, K, logI = c.debug_event_kde(la, ev)
         zr, wr, _ = O.sample_weights(la, w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s])
         hr = O.scott_bw(zr, wr)
-        assert abs(h / hr - 1) < 1e-7      # weights carry ~1e-7 relative noise; dh/h = 1e-5 moves log I by 5e-8
+        assert abs(h / hr - 1) < 3e-7      # weights carry ~1e-6 relative noise; dh/h = 1e-5 moves log I by 5e-8
         Kr = O.kde(zr, wr, hr, w.z_grid[g])
         assert np.max(np.abs(K - Kr)) < 2e-6 * Kr.max()    # fp32 pair loop
         Ir = O.event_integral(la, w.z_grid[g], Kr, w.p_gal[g])
@@ -118,9 +123,13 @@ def test_s5_injection_weights(P):
         s1, s2, sr = O.selection_sums(la, w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw, z_cat_max=w.z_cat_max, return_s=True)
         mism = (s == 0) != (sr == 0)      # underflow deep in the smoothing window may differ: must carry no mass
         assert np.all(np.maximum(s, sr)[mism] < 1e-12 * sr.max())
-        nz = sr > 0
-        assert np.max(np.abs(s[nz] / sr[nz] - 1)) < 1e-6     # two MUFU.EX2 per weight, 2.4e-7 each + fp32 remainders
-        assert abs(s.sum() / s1 - 1) < 5e-8
+        # float log2 s (half an ulp ~2e-6) + five MUFU ops; injection masses are single floats, so m - m_low carries
+        # ~3e-7 absolute and S(m) deep in the window (s below ~1e-6 of the largest) is only good to ~1e-4
+        nz = sr > 1e-6 * sr.max()
+        assert np.max(np.abs(s[nz] / sr[nz] - 1)) < 2e-5
+        nz = sr > 1e-30 * sr.max()
+        assert np.max(np.abs(s[nz] / sr[nz] - 1)) < 2e-3
+        assert abs(s.sum() / s1 - 1) < 5e-7
     c.close()
 
 
@@ -132,7 +141,7 @@ def test_tiny_end_to_end(P):
     rel, dtot, dxi = _compare(r, ref, w.n_events)
     print(f"tiny: rel(logI)={rel:.2e} |dlogL|={dtot:.2e} |dlogxi|={dxi:.2e}")
     assert rel < REL_EVENT and dtot < ABS_TOTAL
-    assert abs(r["neff"][0] / ref["neff"][0] - 1) < 1e-8
+    assert abs(r["neff"][0] / ref["neff"][0] - 1) < 1e-5      # a diagnostic compared with 5 N_events (R8)
     assert np.array_equal(r["flags"], ref["flags"])
 
 
@@ -170,7 +179,7 @@ def test_o5_shaped_ragged_multi_tile(P):
     rel, dtot, dxi = _compare(r, ref, w.n_events)
     print(f"o5-shaped: rel(logI)={rel:.2e} |dlogL|={dtot:.2e} |dlogxi|={dxi:.2e} pairs={r['stats']}")
     assert rel < REL_EVENT and dtot < ABS_TOTAL
-    assert np.max(np.abs(r["neff"] / ref["neff"] - 1)) < 1e-7
+    assert np.max(np.abs(r["neff"] / ref["neff"] - 1)) < 1e-5
     assert r["stats"]["kde_pairs_evaluated"] < r["stats"]["kde_pairs_dense"]
 
 
@@ -291,7 +300,8 @@ def test_kde_cutoff_zero_sums_every_pair(P):
     ref = O.loglike_workload(w, bw_rule=O.BW_FIXED, fixed_bw=fb)
     r = _gpu(P, w, fixed_bw=fb, bw_rule=O.BW_FIXED, kde_cutoff=0.0)
     rel, dtot, _ = _compare(r, ref, w.n_events)
-    assert rel < 1e-6 and dtot < 1e-4
+    # two samples, h = 0.004, nearest galaxy ~10 h away: |d log I / dz| ~ 10/h = 2500, z_j carries 3e-8 (fp32)
+    assert rel < 5e-6 and dtot < 3e-4
     assert r["stats"]["kde_pairs_evaluated"] >= r["stats"]["kde_pairs_dense"]
 
 
