@@ -362,7 +362,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     }
     DlGrid grid = make_dl_grid(xmin, xmax, choose_dl_intervals(ctx, xmin, xmax));
 
-    std::vector<float4> rA(NS), rB(NS);
+    std::vector<float4> rec(2 * NS);
     std::vector<int32_t> k_lo(n_events), k_hi(n_events);
     const double l2e = 1.4426950408889634074;
     std::vector<int32_t> perm(NS);
@@ -388,8 +388,8 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
             const double tk = (std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0;   // in [1, K + 1)
             const uint32_t tkq_max = ((uint32_t)(grid.K + 1) << kTkFracBits) - 1u;   // rounding must not leave the last interval
             const uint32_t tkq = std::min((uint32_t)std::min<double>(std::max(tk, 0.0) * (double)(1u << kTkFracBits) + 0.5, 4294967295.0), tkq_max);
-            rA[s0 + j] = make_float4(bits_f(tkq), f_hi(h_m1[o]), f_lo(h_m1[o]), f_hi(h_m2[o]));
-            rB[s0 + j] = make_float4(f_lo(h_m2[o]), (float)std::log(h_m1[o]), (float)std::log(h_m2[o] / h_m1[o]),
+            rec[2 * (s0 + j)] = make_float4(bits_f(tkq), f_hi(h_m1[o]), f_lo(h_m1[o]), f_hi(h_m2[o]));
+            rec[2 * (s0 + j) + 1] = make_float4(f_lo(h_m2[o]), (float)std::log(h_m1[o]), (float)std::log(h_m2[o] / h_m1[o]),
                                      (float)(l2e * (-h_lp[o] - sh)));   // log2(1/pi_j) with the event's scale removed
             perm[s0 + j] = idx[j];
             const int k = std::min(std::max((int)(tkq >> kTkFracBits), 1), grid.K);
@@ -426,7 +426,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     EventSetDev E{};
     E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz;
     CK(upload(ctx->owned_ev, &E.sample_off, so)); CK(upload(ctx->owned_ev, &E.grid_off, go));
-    CK(upload(ctx->owned_ev, &E.recA, rA)); CK(upload(ctx->owned_ev, &E.recB, rB));
+    CK(upload(ctx->owned_ev, &E.rec, rec));
     CK(upload(ctx->owned_ev, &E.k_lo, k_lo)); CK(upload(ctx->owned_ev, &E.k_hi, k_hi));
     CK(upload(ctx->owned_ev, &E.perm, perm)); CK(upload(ctx->owned_ev, &E.zc, zc)); CK(upload(ctx->owned_ev, &E.qn, qn));
     CK(upload(ctx->owned_ev, &E.uni_dz, udz));
@@ -479,13 +479,13 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     std::vector<int64_t> idx(N);
     std::iota(idx.begin(), idx.end(), (int64_t)0);
     std::stable_sort(idx.begin(), idx.end(), [&](int64_t a, int64_t b) { return h_dl[a] < h_dl[b]; });
-    std::vector<float4> rA(N), rB(N);
+    std::vector<float4> rec(2 * N);
     for (size_t j = 0; j < N; ++j) {
         const size_t o = (size_t)idx[j];
         const double tk = (std::log(h_dl[o]) - grid.x0) / grid.dx + 1.0;
         const int k = std::min(std::max((int)tk, 1), grid.K);
-        rA[j] = make_float4(bits_f((uint32_t)k), (float)(tk - (double)k), (float)h_m1[o], (float)h_m2[o]);
-        rB[j] = make_float4((float)std::log(h_m1[o]), (float)std::log(h_m2[o] / h_m1[o]), (float)(l2e * (-h_lp[o] - sh)), 0.f);
+        rec[2 * j] = make_float4(bits_f((uint32_t)k), (float)(tk - (double)k), (float)h_m1[o], (float)h_m2[o]);
+        rec[2 * j + 1] = make_float4((float)std::log(h_m1[o]), (float)std::log(h_m2[o] / h_m1[o]), (float)(l2e * (-h_lp[o] - sh)), 0.f);
     }
     cudaStreamSynchronize(ctx->stream);
     free_pool(ctx->owned_inj);
@@ -495,7 +495,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     InjSetDev I{};
     I.n_det = n_det;
     I.n_inj_total = (double)n_inj_total;
-    CK(upload(ctx->owned_inj, &I.recA, rA)); CK(upload(ctx->owned_inj, &I.recB, rB));
+    CK(upload(ctx->owned_inj, &I.rec, rec));
     CK(upload(ctx->owned_inj, &I.perm, idx));
     ctx->inj = I;
     ctx->inj_m_top = m_top;

@@ -97,7 +97,7 @@ struct TableParams {
 // consecutive arrays of n_mass + 2 rows: "a" with the power law present (m1 <= m_high), "b" the Gaussian only.
 typedef float4 MassRow;
 
-// Packed, lambda-independent record of one posterior sample / injection (2 x 16 B).
+// Packed, lambda-independent record of one posterior sample / injection (32 B = {A, B}, read with one 256-bit load).
 //   events:     A = {tkq, m1d_hi, m1d_lo, m2d_hi}   B = {m2d_lo, ln m1d, ln(m2d/m1d), log2(1/prior) - event scale}
 //               tkq = table coordinate in 12.20 fixed point (interval in the upper 12 bits)
 //   injections: A = {k, t, m1d, m2d}                B = {ln m1d, ln(m2d/m1d), log2(1/p_draw) - set scale, 0}
@@ -141,10 +141,13 @@ struct MassLookup {
     int lo, cap, n_mass;
 };
 
-__device__ __forceinline__ float4 ldg_stream4(const float4* p) {   // streaming 128-bit read (read once per CTA)
-    float4 v;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-    return v;
+struct Rec { float4 A, B; };   // one packed record (32 B, 32-byte aligned)
+__device__ __forceinline__ Rec ldg_stream_rec(const float4* p) {   // streaming 256-bit read (read once per CTA)
+    Rec r;
+    asm volatile("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(r.A.x), "=f"(r.A.y), "=f"(r.A.z), "=f"(r.A.w), "=f"(r.B.x), "=f"(r.B.y), "=f"(r.B.z), "=f"(r.B.w)
+                 : "l"(p));
+    return r;
 }
 
 // Steps S2 / S5 for one sample (or injection): redshift from the table, source-frame masses, log2 of the weight
@@ -232,8 +235,7 @@ struct EventSetDev {
     int32_t max_ns, max_nz;
     const int64_t* sample_off;  // [n_events+1]
     const int64_t* grid_off;    // [n_events+1]
-    const float4* recA;         // packed sample records (see above), sorted by d_L within each event
-    const float4* recB;
+    const float4* rec;          // packed sample records {A, B} (see above), sorted by d_L within each event
     const int32_t* perm;        // sorted position -> caller's index within the event
     const double* zc;           // z_g - z0_i  (centred grid)
     const float* qn;            // p_gal(z_g) * trapezoid weight / (the event's largest such product)
@@ -268,7 +270,7 @@ struct EventKernelParams {
 struct InjSetDev {
     int64_t n_det;
     double n_inj_total;
-    const float4* recA; const float4* recB;   // packed injection records, sorted by d_L
+    const float4* rec;       // packed injection records {A, B}, sorted by d_L
     const int64_t* perm;
 };
 

@@ -113,6 +113,9 @@ struct EvSmem {
     unsigned long long mbar;
     int pass_counter;
     int mass_lo;
+    double h, scd;            // bandwidth and the coordinate scale (as the rounded float, widened)
+    float scf, delta, xfirst; // scale, grid spacing and first grid point in scaled coordinates
+    int Bsel;                 // block size of the power form, 0 = direct form
 };
 
 __host__ __device__ inline size_t ev_ns_pad(size_t ns) { return (ns + kPass - 1) / kPass * kPass; }
@@ -177,9 +180,10 @@ __device__ __forceinline__ float s2_sweep(const EventKernelParams& P, const LamF
     const int tid = threadIdx.x;
 #pragma unroll 2
     for (int j = tid; j < ns; j += kEvThreads) {
-        const float4 A = ldg_stream4(P.ev.recA + s0 + j), Bq = ldg_stream4(P.ev.recB + s0 + j);
+        const Rec R = ldg_stream_rec(P.ev.rec + 2 * (s0 + j));
+        const float4 A = R.A, Bq = R.B;
         const uint32_t tkq = __float_as_uint(A.x);
-        const int k = min(max((int)(tkq >> kTkFracBits), 1), tab_rows - 2);
+        const int k = (int)(tkq >> kTkFracBits);     // in [1, K]: clamped when the records were packed
         const float t = __uint_as_float(0x3F800000u | ((tkq << (32 - kTkFracBits)) >> 9)) - 1.0f;
         const bool in_range = tkq <= F.tkmax_ev_q;
         float4 q0, q1, q2, q3;
@@ -301,37 +305,70 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const float zmed = zf[ns >> 1], zlast = zf[ns - 1];
     float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;   // sum w, sum w^2, sum w z', sum w z'^2
     const int nsp = (int)ev_ns_pad(ns);
-    for (int j = tid; j < nsp; j += kEvThreads) {
-        if (j < ns) {
-            const float w = ex2f(wl[j] - mx), zc = zf[j] - zmed;
-            wl[j] = w;
-            m0 += w;
-            m1 = fmaf(w, w, m1);
-            const float wz = w * zc;
-            m2 += wz;
-            m3 = fmaf(wz, zc, m3);
-            if (P.dbg_z) {
-                const int jo = P.ev.perm[s0 + j];
-                P.dbg_z[jo] = z0 + (double)zf[j];
-                P.dbg_w[jo] = (double)w * exp2((double)mx) * exp(P.ln_shift[ev]);
-            }
-        } else {                                    // idle slots of the last pass sit on the last sample with weight 0
-            wl[j] = 0.f;
-            zf[j] = zlast;
+    for (int j = tid; j < ns; j += kEvThreads) {
+        const float w = ex2f(wl[j] - mx), zc = zf[j] - zmed;
+        wl[j] = w;
+        m0 += w;
+        m1 = fmaf(w, w, m1);
+        const float wz = w * zc;
+        m2 += wz;
+        m3 = fmaf(wz, zc, m3);
+    }
+    for (int j = ns + tid; j < nsp; j += kEvThreads) {   // idle slots of the last pass sit on the last sample with weight 0
+        wl[j] = 0.f;
+        zf[j] = zlast;
+    }
+    if (P.dbg_z)
+        for (int j = tid; j < ns; j += kEvThreads) {
+            const int jo = P.ev.perm[s0 + j];
+            P.dbg_z[jo] = z0 + (double)zf[j];
+            P.dbg_w[jo] = (double)wl[j] * exp2((double)mx) * exp(P.ln_shift[ev]);
         }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        m0 += __shfl_xor_sync(0xffffffffu, m0, o);
+        m1 += __shfl_xor_sync(0xffffffffu, m1, o);
+        m2 += __shfl_xor_sync(0xffffffffu, m2, o);
+        m3 += __shfl_xor_sync(0xffffffffu, m3, o);
     }
-    double mom[4] = {(double)m0, (double)m1, (double)m2, (double)m3};
-    block_sum<kEvThreads, 4>(mom, S.red);
-    const double sw = mom[0];
-    double h;
-    if (P.bw_rule == CHIM_BW_FIXED) {
-        h = P.ev.fixed_bw[ev];
-    } else {   // Scott on the weighted sample (R3, O7)
-        double s2 = mom[1] / (sw * sw), zb = mom[2] / sw;
-        double var = (mom[3] / sw - zb * zb) / (1.0 - s2);
-        h = (1.0 - s2 > 0.0 && var > 0.0) ? sqrt(var) * exp(0.2 * log(s2)) : NAN;   // n_eff^(-1/5) = s2^(1/5)
+    if (lane == 0) { S.red[wid] = m0; S.red[8 + wid] = m1; S.red[16 + wid] = m2; S.red[24 + wid] = m3; }
+    __syncthreads();
+    const double* zc_g = P.ev.zc + g0;
+    const float* qn_g = P.ev.qn + g0;
+    const double udz = P.ev.uni_dz[ev];
+    const float T = (P.cutoff > 0.0) ? (float)(P.cutoff * sqrt(kHalfLog2e)) : INFINITY;
+    if (tid == 0) {   // one thread: fp64 sums over the warps, bandwidth, and every scalar the pair loop needs
+        double mom[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            double a = 0.0;
+#pragma unroll
+            for (int k = 0; k < kEvThreads / 32; ++k) a += S.red[i * 8 + k];
+            mom[i] = a;
+        }
+        const double sw = mom[0];
+        double h;
+        if (P.bw_rule == CHIM_BW_FIXED) {
+            h = P.ev.fixed_bw[ev];
+        } else {   // Scott on the weighted sample (R3, O7)
+            double s2 = mom[1] / (sw * sw), zb = mom[2] / sw;
+            double var = (mom[3] / sw - zb * zb) / (1.0 - s2);
+            h = (1.0 - s2 > 0.0 && var > 0.0) ? sqrt(var) * exp(0.2 * log(s2)) : NAN;   // n_eff^(-1/5) = s2^(1/5)
+        }
+        if (P.dbg_h) *P.dbg_h = h;
+        // scaled coordinates x = z' sqrt(log2(e)/2)/h: exp(-d^2/2h^2) = 2^(-dx^2)
+        const float scf = (float)(sqrt(kHalfLog2e) / h);
+        const double scd = (double)scf;             // samples and grid are scaled by the SAME rounded factor
+        const float delta = (float)(udz * scd);
+        int Bsel = 0;                                // 0 = direct form
+        if (udz > 0.0 && T < INFINITY && P.kde_method == CHIM_KDE_AUTO && !P.dbg_K) {
+            if (delta * 32.f <= 3.3f) Bsel = 32;
+            else if (delta * 16.f <= kMaxBlockSpan) Bsel = 16;
+        }
+        S.h = h; S.scd = scd; S.scf = scf; S.delta = delta; S.xfirst = (float)(zc_g[0] * scd); S.Bsel = Bsel;
     }
-    if (P.dbg_h && tid == 0) *P.dbg_h = h;
+    __syncthreads();
+    const double h = S.h;
     if (!(h > 0.0) || !isfinite(h)) {
         if (tid == 0) {
             *out = NAN;
@@ -340,38 +377,34 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         if (P.dbg_K) for (int g = tid; g < nz; g += kEvThreads) P.dbg_K[g] = NAN;
         return;
     }
-
-    // ---- scaled coordinates x = z' sqrt(log2(e)/2)/h: exp(-d^2/2h^2) = 2^(-dx^2) --------------------------------
-    const double sc = sqrt(kHalfLog2e) / h;
-    const float scf = (float)sc;
-    const double scd = (double)scf;             // samples and grid are scaled by the SAME rounded factor
-    const float T = (P.cutoff > 0.0) ? (float)(P.cutoff * sqrt(kHalfLog2e)) : INFINITY;
-    const double* zc_g = P.ev.zc + g0;
-    const float* qn_g = P.ev.qn + g0;
-    const double udz = P.ev.uni_dz[ev];
-    const float delta = (float)(udz * scd), xfirst = (float)(zc_g[0] * scd);
-    int Bsel = 0;                                // 0 = direct form
-    if (udz > 0.0 && T < INFINITY && P.kde_method == CHIM_KDE_AUTO && !P.dbg_K) {
-        if (delta * 32.f <= 3.3f) Bsel = 32;
-        else if (delta * 16.f <= kMaxBlockSpan) Bsel = 16;
-    }
+    const float scf = S.scf, delta = S.delta, xfirst = S.xfirst;
+    const int Bsel = S.Bsel;
     const int nzp = (int)ev_nz_pad(nz);
     const bool on_grid = P.placement == CHIM_ON_GRID;
-    for (int g = tid; g < nzp; g += kEvThreads) {   // (the block reduction above fenced the last reads of the staged tables)
-        float q = 0.f, xg = 0.f;
-        if (g < nz) {
-            q = qn_g[g];
-            if (on_grid)
-                q = (float)((double)q * grid_factor(L, P.dc_tab + (size_t)l * (P.n_table + 1 + kZPad), P.n_table + 1 + kZPad,
-                                                    P.z_table_max / P.n_table, zc_g[g] + z0));
-            xg = (float)(zc_g[g] * scd);
-        }
-        if (Bsel) {
+    if (Bsel && !on_grid) {   // power form: q'_g = q_g 2^(-(b delta)^2), b = g mod B, duplicated for the packed FMA
+        for (int g = tid; g < nzp; g += kEvThreads) {   // (the barriers above fenced the last reads of the staged tables)
             const float bd = (float)(g & (Bsel - 1)) * delta;
-            q *= ex2f(-bd * bd);
+            const float q = (g < nz) ? qn_g[g] * ex2f(-bd * bd) : 0.f;
             gq[g] = make_float2(q, q);
-        } else {
-            gq[g] = make_float2(xg, q);
+        }
+    } else {
+        const double scd = S.scd;
+        for (int g = tid; g < nzp; g += kEvThreads) {
+            float q = 0.f, xg = 0.f;
+            if (g < nz) {
+                q = qn_g[g];
+                if (on_grid)
+                    q = (float)((double)q * grid_factor(L, P.dc_tab + (size_t)l * (P.n_table + 1 + kZPad), P.n_table + 1 + kZPad,
+                                                        P.z_table_max / P.n_table, zc_g[g] + z0));
+                xg = (float)(zc_g[g] * scd);
+            }
+            if (Bsel) {
+                const float bd = (float)(g & (Bsel - 1)) * delta;
+                q *= ex2f(-bd * bd);
+                gq[g] = make_float2(q, q);
+            } else {
+                gq[g] = make_float2(xg, q);
+            }
         }
     }
     __syncthreads();
@@ -379,6 +412,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     // ---- S3 + S4: warp passes over 128 consecutive (sorted) samples ----------------------------------------
     const int n_pass = (ns + kPass - 1) / kPass;
     const float inv_delta = (udz > 0.0) ? 1.f / delta : 0.f;
+    const float bd = (float)Bsel * delta, inv_bd = Bsel ? 1.f / bd : 0.f;
+    const int a_max = Bsel ? nzp / Bsel - 1 : 0;
     double lsum = 0.0;                          // this lane's sum_j w_j A_j
     unsigned long long pairs_exec = 0, pairs_cut = 0;
     for (;;) {
@@ -397,9 +432,10 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         float A[4] = {0.f, 0.f, 0.f, 0.f};
         bool done = false;
         if (Bsel) {
-            const float bd = (float)Bsel * delta;
-            const int a_lo = max(0, (int)floorf((xmn - T - xfirst) / bd));
-            const int a_hi = min(nzp / Bsel - 1, (int)floorf((xmx + T - xfirst) / bd));
+            // (a product with the rounded 1/bd may land one block early or late at an exact block edge: the pairs
+            // concerned sit at the cut-off distance, where a Gaussian term is below 2^-26 of the peak)
+            const int a_lo = max(0, (int)floorf((xmn - T - xfirst) * inv_bd));
+            const int a_hi = min(a_max, (int)floorf((xmx + T - xfirst) * inv_bd));
             // largest exponent of s^b inside a block: 2 |u| delta (B-1) with |u| <= span + T + B delta
             if (2.f * (xmx - xmn + T + bd) * bd <= kMaxPowExp) {
                 if (a_hi >= a_lo) {

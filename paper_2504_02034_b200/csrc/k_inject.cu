@@ -68,11 +68,11 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
         const float4* rows = reinterpret_cast<const float4*>(P.tab + (size_t)l * P.tab_rows);
 #pragma unroll 2
         for (int64_t j = j0 + tid; j < j1; j += kInjThreads) {
-            const float4 A = ldg_stream4(P.inj.recA + j), Bq = ldg_stream4(P.inj.recB + j);
-            const int kraw = __float_as_int(A.x);
-            const int k = min(max(kraw, 1), P.tab_rows - 2);
+            const Rec R = ldg_stream_rec(P.inj.rec + 2 * j);
+            const float4 A = R.A, Bq = R.B;
+            const int k = __float_as_int(A.x);           // in [1, K]: clamped when the records were packed
             const float t = A.y;
-            const bool in_range = ((float)kraw + t) <= F.tkmax_inj;
+            const bool in_range = ((float)k + t) <= F.tkmax_inj;
             const float4* r = rows + 4 * (size_t)k;
             const float4 q0 = __ldg(r), q1 = __ldg(r + 1), q2 = __ldg(r + 2), q3 = __ldg(r + 3);
             float zc, l2w;
