@@ -161,6 +161,7 @@ __device__ __forceinline__ Rec ldg_stream_rec(const float4* p) {   // streaming 
 // rounding errors left are ~1e-7 relative, independent from sample to sample.  Five MUFU ops
 // (rcp, ex2, 2 lg2 here; the final ex2 is the caller's), no fp64, no data-dependent branch except the (rare)
 // fall-back of the mass row to global memory.  Returns z - z_ref and log2 w (-inf: weight 0).
+// Warp-collective: all 32 lanes must call it together (the rare paths are taken per warp, by vote).
 __device__ __forceinline__ void sample_eval(const LamF& F, const float4 q0, const float4 q1, const float4 q2,
                                             const float4 q3, const float t, const float zref_hi, const float zref_lo,
                                             const float m1h, const float m1l, const float m2h, const float m2l,
@@ -186,17 +187,21 @@ __device__ __forceinline__ void sample_eval(const LamF& F, const float4 q0, cons
     const float tf = tm - (ti - 12582912.f);
     const bool gauss_only = mp1 > F.mhigh_p;
     const int ks = km - M.lo;
-    float4 c;
-    if ((unsigned)ks < (unsigned)M.cap) c = M.s[ks + (gauss_only ? M.cap : 0)];
-    else c = __ldg(M.g + km + (gauss_only ? M.n_mass + 2 : 0));
+    const bool staged = (unsigned)ks < (unsigned)M.cap;
+    float4 c = M.s[(staged ? ks : 0) + (gauss_only ? M.cap : 0)];
+    if (__any_sync(0xffffffffu, !staged)) {            // rare: a source mass outside the staged rows
+        if (!staged) c = __ldg(M.g + km + (gauss_only ? M.n_mass + 2 : 0));
+    }
     float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x);
     l += fmaf(F.beta2, lm2, r + ipr2);
     l = fmaf(-2.f, lg2f(fmaxf(mp1, 1e-30f)), l);
     // smoothing of m2 (M1): log2(e) f = (2 delta m' - delta^2) log2(e) / (m' (m' - delta)), m' clamped inside the window
-    const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
-    const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
-    const float ls = lg2f(1.0f + ex2f(f2));
-    l -= (mp2 < F.delta) ? ls : 0.f;
+    if (__any_sync(0xffffffffu, mp2 < F.delta)) {      // skipped by warps whose secondaries all lie above the window
+        const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
+        const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
+        const float ls = lg2f(1.0f + ex2f(f2));
+        l -= (mp2 < F.delta) ? ls : 0.f;
+    }
     const bool ok = in_range && (mp2 > 0.f);           // R15 support: m_low < m2 (<= m1)
     l2w = ok ? l : -INFINITY;
 }

@@ -31,6 +31,10 @@ namespace chim {
 #define CHIM_EV_THREADS 256
 #define CHIM_EV_BLOCKS 3
 #endif
+#ifndef CHIM_S2_UNROLL
+#define CHIM_S2_UNROLL 2
+#endif
+constexpr int kS2Unroll = CHIM_S2_UNROLL;
 constexpr int kEvThreads = CHIM_EV_THREADS;   // 256 x 3 CTAs per SM measured faster than 384 x 2 and 512 x 1
 constexpr int kPass = 128;               // samples per warp pass (4 per lane)
 constexpr float kMaxBlockSpan = 4.8f;    // B * delta limit of the power form
@@ -127,7 +131,7 @@ __host__ __device__ inline size_t ev_aux_bytes(size_t nz) {   // S2: staged tabl
 
 // One block of B grid points for the 4 samples of a lane: tot_k += 2^(-u_k^2) * sum_b q'_b s_k^b (Horner, FFMA2).
 template <int B>
-__device__ __forceinline__ void power_block(const ulonglong2* __restrict__ qp, f32x2 xs2, f32x2 cs2, f32x2 nx01, f32x2 nx23,
+__device__ __forceinline__ void power_block(const float4* __restrict__ qp, f32x2 xs2, f32x2 cs2, f32x2 nx01, f32x2 nx23,
                                             f32x2& tot01, f32x2& tot23) {
     const f32x2 u01 = add2(xs2, nx01), u23 = add2(xs2, nx23);          // u = x_a - x_j
     const f32x2 su01 = mul2(u01, cs2), su23 = mul2(u23, cs2);          // -2 delta u
@@ -141,31 +145,36 @@ __device__ __forceinline__ void power_block(const ulonglong2* __restrict__ qp, f
     const f32x2 e01 = pack2(ex2f(-a), ex2f(-b)), e23 = pack2(ex2f(-c), ex2f(-d));
     f32x2 a01 = 0ull, a23 = 0ull;     // (+0.f, +0.f)
 #pragma unroll
-    for (int i = B / 2 - 1; i >= 0; --i) {
-        const ulonglong2 v = qp[i];   // {(q'_2i, q'_2i), (q'_2i+1, q'_2i+1)}
-        a01 = fma2(a01, s01, v.y);
-        a23 = fma2(a23, s23, v.y);
-        a01 = fma2(a01, s01, v.x);
-        a23 = fma2(a23, s23, v.x);
+    for (int i = B / 4 - 1; i >= 0; --i) {
+        const float4 v = qp[i];       // q'_4i .. q'_4i+3: one shared-memory wavefront pair feeds 8 packed FMAs
+        const f32x2 q3 = pack2(v.w, v.w), q2 = pack2(v.z, v.z), q1 = pack2(v.y, v.y), q0 = pack2(v.x, v.x);   // (scalar operand of FFMA2)
+        a01 = fma2(a01, s01, q3);
+        a23 = fma2(a23, s23, q3);
+        a01 = fma2(a01, s01, q2);
+        a23 = fma2(a23, s23, q2);
+        a01 = fma2(a01, s01, q1);
+        a23 = fma2(a23, s23, q1);
+        a01 = fma2(a01, s01, q0);
+        a23 = fma2(a23, s23, q0);
     }
     tot01 = fma2(e01, a01, tot01);
     tot23 = fma2(e23, a23, tot23);
 }
 
 template <int B>
-__device__ __forceinline__ void power_pass(const float2* __restrict__ gq, int a_lo, int a_hi, float xfirst, float delta,
+__device__ __forceinline__ void power_pass(const float* __restrict__ gq, int a_lo, int a_hi, float xfirst, float delta,
                                            const float (&x)[4], float (&A)[4]) {
     f32x2 tot01 = 0ull, tot23 = 0ull;
     const float cs = -2.f * delta, bd = (float)B * delta;
     const f32x2 cs2 = pack2(cs, cs), nx01 = pack2(-x[0], -x[1]), nx23 = pack2(-x[2], -x[3]);
     float af = (float)a_lo;
-    const ulonglong2* qp = reinterpret_cast<const ulonglong2*>(gq + a_lo * B);
+    const float4* qp = reinterpret_cast<const float4*>(gq + a_lo * B);
 #pragma unroll 1
     for (int a = a_lo; a <= a_hi; ++a) {
         const float xs = fmaf(af, bd, xfirst);     // exact block origin: no drift from block to block
         power_block<B>(qp, pack2(xs, xs), cs2, nx01, nx23, tot01, tot23);
         af += 1.0f;
-        qp += B / 2;
+        qp += B / 4;
     }
     unpack2(tot01, A[0], A[1]);
     unpack2(tot23, A[2], A[3]);
@@ -173,15 +182,18 @@ __device__ __forceinline__ void power_pass(const float2* __restrict__ gq, int a_
 
 // S2 sweep 1 over the event's samples: z_j - z0 and log2 w_j to shared memory; returns the thread's max log2 w.
 template <bool kStaged>
-__device__ __forceinline__ float s2_sweep(const EventKernelParams& P, const LamF& F, const float4* __restrict__ rows,
-                                          int k_base, int tab_rows, const MassLookup& M, int64_t s0, int ns, float z0h, float z0l,
-                                          float* __restrict__ zf, float* __restrict__ wl, int& oor) {
+__device__ __forceinline__ float s2_sweep(const float4* __restrict__ rec, const LamF& Fs, const float4* __restrict__ rows,
+                                          int k_base, const MassLookup& M, int ns, float z0h, float z0l,
+                                          float* __restrict__ zf, float* __restrict__ wl) {
     float mx = -INFINITY;
     const int tid = threadIdx.x;
-#pragma unroll 2
-    for (int j = tid; j < ns; j += kEvThreads) {
-        const Rec R = ldg_stream_rec(P.ev.rec + 2 * (s0 + j));
+    const LamF F = Fs;                               // registers, not re-read from shared memory after every store
+    const int ns32 = (ns + 31) & ~31;                // whole warps stay in the loop (sample_eval votes)
+    Rec R = ldg_stream_rec(rec + 2 * min(tid, ns - 1));
+#pragma unroll(kS2Unroll)
+    for (int j = tid; j < ns32; j += kEvThreads) {
         const float4 A = R.A, Bq = R.B;
+        if (j + kEvThreads < ns32) R = ldg_stream_rec(rec + 2 * min(j + kEvThreads, ns - 1));   // one iteration ahead
         const uint32_t tkq = __float_as_uint(A.x);
         const int k = (int)(tkq >> kTkFracBits);     // in [1, K]: clamped when the records were packed
         const float t = __uint_as_float(0x3F800000u | ((tkq << (32 - kTkFracBits)) >> 9)) - 1.0f;
@@ -196,10 +208,11 @@ __device__ __forceinline__ float s2_sweep(const EventKernelParams& P, const LamF
         }
         float zc, l2w;
         sample_eval(F, q0, q1, q2, q3, t, z0h, z0l, A.y, A.z, A.w, Bq.x, Bq.y, Bq.z, Bq.w, M, in_range, zc, l2w);
-        oor |= (int)!in_range;
-        zf[j] = zc;
-        wl[j] = l2w;
-        mx = fmaxf(mx, l2w);
+        if (j < ns) {
+            zf[j] = zc;
+            wl[j] = l2w;
+            mx = fmaxf(mx, l2w);
+        }
     }
     return mx;
 }
@@ -213,7 +226,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const size_t ns_pad = ev_ns_pad(P.ev.max_ns);
     float* wl = zf + ns_pad;
     unsigned char* aux = reinterpret_cast<unsigned char*>(wl + ns_pad);
-    float2* gq = reinterpret_cast<float2*>(aux);
+    float2* gq = reinterpret_cast<float2*>(aux);     // direct form: (x_g, q_g)
+    float* gqp = reinterpret_cast<float*>(aux);      // power form: q'_g
     float4* rows_s = reinterpret_cast<float4*>(aux);
     MassRow* mass_s = reinterpret_cast<MassRow*>(aux + (size_t)kRowStage * sizeof(Row));
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -275,15 +289,16 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
 
     // ---- S2, sweep 1: z_j - z0 and log2 w_j -------------------------------------------------------------
     const float z0h = (float)z0, z0l = (float)(z0 - (double)z0h);
-    int oor = 0;
     float mx;
-    if (staged) mx = s2_sweep<true>(P, L.F, rows_s, k_lo, P.tab_rows, M, s0, ns, z0h, z0l, zf, wl, oor);
-    else mx = s2_sweep<false>(P, L.F, reinterpret_cast<const float4*>(tab), 0, P.tab_rows, M, s0, ns, z0h, z0l, zf, wl, oor);
+    const float4* rec = P.ev.rec + 2 * s0;
+    if (staged) mx = s2_sweep<true>(rec, L.F, rows_s, k_lo, M, ns, z0h, z0l, zf, wl);
+    else mx = s2_sweep<false>(rec, L.F, reinterpret_cast<const float4*>(tab), 0, M, ns, z0h, z0l, zf, wl);
+    // samples are sorted in d_L: one of them lies beyond the table iff the last one does
+    if (tid == 0 && __float_as_uint(__ldg(rec + 2 * (size_t)(ns - 1)).x) > L.F.tkmax_ev_q) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
     if (lane == 0) S.fred[wid] = mx;
-    oor = __syncthreads_or(oor);
-    if (oor && tid == 0) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
+    __syncthreads();
 #pragma unroll
     for (int k = 0; k < kEvThreads / 32; ++k) mx = fmaxf(mx, S.fred[k]);
     if (!(mx > -INFINITY)) {   // all-zero event (R15): I = 0
@@ -384,8 +399,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     if (Bsel && !on_grid) {   // power form: q'_g = q_g 2^(-(b delta)^2), b = g mod B, duplicated for the packed FMA
         for (int g = tid; g < nzp; g += kEvThreads) {   // (the barriers above fenced the last reads of the staged tables)
             const float bd = (float)(g & (Bsel - 1)) * delta;
-            const float q = (g < nz) ? qn_g[g] * ex2f(-bd * bd) : 0.f;
-            gq[g] = make_float2(q, q);
+            gqp[g] = (g < nz) ? qn_g[g] * ex2f(-bd * bd) : 0.f;
         }
     } else {
         const double scd = S.scd;
@@ -400,8 +414,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             }
             if (Bsel) {
                 const float bd = (float)(g & (Bsel - 1)) * delta;
-                q *= ex2f(-bd * bd);
-                gq[g] = make_float2(q, q);
+                gqp[g] = q * ex2f(-bd * bd);
             } else {
                 gq[g] = make_float2(xg, q);
             }
@@ -439,8 +452,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             // largest exponent of s^b inside a block: 2 |u| delta (B-1) with |u| <= span + T + B delta
             if (2.f * (xmx - xmn + T + bd) * bd <= kMaxPowExp) {
                 if (a_hi >= a_lo) {
-                    if (Bsel == 32) power_pass<32>(gq, a_lo, a_hi, xfirst, delta, x, A);
-                    else power_pass<16>(gq, a_lo, a_hi, xfirst, delta, x, A);
+                    if (Bsel == 32) power_pass<32>(gqp, a_lo, a_hi, xfirst, delta, x, A);
+                    else power_pass<16>(gqp, a_lo, a_hi, xfirst, delta, x, A);
                     if (kStats && lane == 0) pairs_exec += (unsigned long long)(a_hi - a_lo + 1) * Bsel * kPass;
                 }
                 done = true;
@@ -466,7 +479,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
 #pragma unroll 1
                 for (int g = g_lo; g <= g_hi; ++g) {
                     const float bdg = (float)(g & (Bsel - 1)) * delta;
-                    const float xg = fmaf((float)g, delta, xfirst), q = gq[g].x * ex2f(bdg * bdg);
+                    const float xg = fmaf((float)g, delta, xfirst), q = gqp[g] * ex2f(bdg * bdg);
 #pragma unroll
                     for (int k = 0; k < 4; ++k) { const float d = xg - x[k]; A[k] = fmaf(q, ex2f(-d * d), A[k]); }
                 }

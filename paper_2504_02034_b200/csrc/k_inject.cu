@@ -14,6 +14,10 @@
 
 namespace chim {
 
+#ifndef CHIM_S5_UNROLL
+#define CHIM_S5_UNROLL 2
+#endif
+constexpr int kS5Unroll = CHIM_S5_UNROLL;
 constexpr int kInjThreads = 256;
 
 struct InjSmem {
@@ -66,10 +70,12 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
     int oor = 0;
     if (L.flags == 0) {
         const float4* rows = reinterpret_cast<const float4*>(P.tab + (size_t)l * P.tab_rows);
-#pragma unroll 2
-        for (int64_t j = j0 + tid; j < j1; j += kInjThreads) {
-            const Rec R = ldg_stream_rec(P.inj.rec + 2 * j);
+        const int64_t j1w = j0 + ((j1 - j0 + 31) & ~(int64_t)31);    // whole warps stay in the loop (sample_eval votes)
+        Rec R = ldg_stream_rec(P.inj.rec + 2 * min(j0 + tid, j1 - 1));
+#pragma unroll(kS5Unroll)
+        for (int64_t j = j0 + tid; j < j1w; j += kInjThreads) {
             const float4 A = R.A, Bq = R.B;
+            if (j + kInjThreads < j1w) R = ldg_stream_rec(P.inj.rec + 2 * min(j + kInjThreads, j1 - 1));   // one iteration ahead
             const int k = __float_as_int(A.x);           // in [1, K]: clamped when the records were packed
             const float t = A.y;
             const bool in_range = ((float)k + t) <= F.tkmax_inj;
@@ -78,10 +84,10 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             float zc, l2w;
             sample_eval(F, q0, q1, q2, q3, t, F.zcat_hi, F.zcat_lo, A.z, 0.f, A.w, 0.f, Bq.x, Bq.y, Bq.z, M, in_range, zc, l2w);
             oor |= (int)!in_range;
-            const double s = (zc <= 0.f) ? ex2_to_double(l2w) : 0.0;   // support of the selection-term z density (R6)
+            const double s = (zc <= 0.f && j < j1) ? ex2_to_double(l2w) : 0.0;   // support of the selection-term z density (R6)
             acc[0] += s;
             acc[1] = fma(s, s, acc[1]);
-            if (P.dbg_s) P.dbg_s[P.inj.perm[j]] = s * P.dbg_scale;
+            if (P.dbg_s && j < j1) P.dbg_s[P.inj.perm[j]] = s * P.dbg_scale;
         }
     }
     acc[0] = warp_sum(acc[0]);
