@@ -57,8 +57,11 @@ typedef enum chim_status {
 enum { CHIM_MEM_HOST = 0, CHIM_MEM_DEVICE = 1 };   /* where the pointers given to chim_init_* live     */
 enum { CHIM_ON_SAMPLES = 0, CHIM_ON_GRID = 1 };    /* placement of psi/J (R1): N = per-sample weights  */
 enum { CHIM_BW_SCOTT = 0, CHIM_BW_FIXED = 1 };     /* KDE bandwidth rule (R3)                          */
-enum { CHIM_KDE_AUTO = 0, CHIM_KDE_DIRECT = 1 };   /* pair-loop formulation: AUTO = power
-                                                      form on equally spaced grids, direct form otherwise  */
+enum { CHIM_KDE_AUTO = 0, CHIM_KDE_DIRECT = 1, CHIM_KDE_POWER = 2 };
+                                                   /* KDE formulation.  AUTO: on equally spaced grids
+                                                      the local-expansion form, else (or where it does not fit) the power
+                                                      form, else the direct form; DIRECT: one MUFU.EX2 per pair on every
+                                                      grid; POWER: as AUTO without the local-expansion form              */
 
 /* per-lambda flag bits written to out_flags */
 #define CHIM_FLAG_LAMBDA_DOMAIN 1u   /* H0<=0, Om not in (0,1], Xi0<=0, delta_m<=0, sigma_g<=0, lambda_g not in
@@ -86,7 +89,7 @@ typedef struct chim_config {
     int32_t n_win_table; /* panels of the per-lambda window table of int m^beta S(m) dm (M4)                   */
     int32_t lambda_chunk;/* lambdas processed per internal pass (bounds the per-lambda table memory)           */
     double neff_factor;  /* NEFF_LOW is raised if N_eff < neff_factor * N_events (R8)                          */
-    int32_t kde_method;  /* CHIM_KDE_AUTO (default) | CHIM_KDE_DIRECT (one MUFU.EX2 per pair on every grid)            */
+    int32_t kde_method;  /* CHIM_KDE_AUTO (default) | CHIM_KDE_DIRECT | CHIM_KDE_POWER                                   */
     int32_t n_mass_table;/* intervals of the per-lambda mass table in ln m1                           */
     int32_t count_pairs; /* 1: the KDE kernel also counts its (sample, grid point) pairs for chim_get_stats (slower)     */
 } chim_config;
@@ -146,8 +149,10 @@ int chim_loglike_batch_host(chim_ctx *ctx, int32_t n_lambda, const double *lambd
 
 /* Work counters of the last chim_loglike_batch on this context (valid after the stream is synchronised;
  * the call itself synchronises).  kde_pairs_in_cutoff = (sample, grid point) pairs with |z_g - z_j| <= t*h, the
- * algorithmic work of S3; kde_pairs_evaluated = pairs the kernel executed (the bands are padded to whole
- * blocks and to the widest sample of a warp pass); kde_pairs_dense = sum_i N_s,i N_z,i x n_lambda. */
+ * algorithmic work of S3; kde_pairs_evaluated = fp32 FMA lane-operations the KDE phase executed: in the direct and
+ * power forms one per executed pair (the bands are padded to whole blocks and to the widest sample of a warp
+ * pass), in the local-expansion form the coefficient build plus one polynomial per sample;
+ * kde_pairs_dense = sum_i N_s,i N_z,i x n_lambda.  The first two are only counted when cfg.count_pairs = 1. */
 typedef struct chim_stats {
     uint64_t kde_pairs_evaluated;
     uint64_t kde_pairs_in_cutoff;

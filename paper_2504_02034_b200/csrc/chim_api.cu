@@ -20,6 +20,7 @@ using namespace chim;
 namespace {
 constexpr size_t kMaxSmemOptin = 232448;   // 227 KB per CTA on sm_100
 constexpr int kInjChunk = 8192;            // injections per CTA of k_inject
+constexpr double kPolyMaxHalfRange = 0.45; // half-width in ln d_L up to which an event takes the local polynomials
 }
 
 struct chim_ctx {
@@ -116,6 +117,7 @@ int choose_dl_intervals(const chim_ctx* ctx, double xmin, double xmax) {
 inline float f_hi(double x) { return (float)x; }
 inline float f_lo(double x) { return (float)(x - (double)(float)x); }
 inline float bits_f(uint32_t u) { float f; std::memcpy(&f, &u, 4); return f; }
+inline uint32_t f_bits(float f) { uint32_t u; std::memcpy(&u, &f, 4); return u; }
 
 DlGrid make_dl_grid(double xmin, double xmax, int K) {
     DlGrid g;
@@ -276,7 +278,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     if (c.n_table < 16 || (c.n_dl_table != 0 && c.n_dl_table < 16) || c.n_dl_table > kMaxDlRows || c.n_win_table < 8 || c.n_mass_table < 64 || c.z_cat_max > c.z_table_max) return CHIM_EINVAL;
     if (c.placement != CHIM_ON_SAMPLES && c.placement != CHIM_ON_GRID) return CHIM_EINVAL;
     if (c.bw_rule != CHIM_BW_SCOTT && c.bw_rule != CHIM_BW_FIXED) return CHIM_EINVAL;
-    if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT) return CHIM_EINVAL;
+    if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT && c.kde_method != CHIM_KDE_POWER) return CHIM_EINVAL;
     if (c.mem != CHIM_MEM_HOST && c.mem != CHIM_MEM_DEVICE) return CHIM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device < 0 || c.device >= ndev) return CHIM_ECUDA;
@@ -291,7 +293,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     TableParams TP = table_params(ctx);
     TP.ev.K = TP.inj.K = c.n_dl_table > 0 ? c.n_dl_table : kMaxDlRows;
     if (tables_smem_bytes(TP) > kMaxSmemOptin || inject_smem_bytes(c.n_mass_table) > kMaxSmemOptin) { delete ctx; return CHIM_EINVAL; }
-    if (upload_gauss_legendre() != cudaSuccess) { delete ctx; return CHIM_ECUDA; }
+    if (upload_gauss_legendre() != cudaSuccess || upload_poly_matrices() != cudaSuccess) { delete ctx; return CHIM_ECUDA; }
     *out = ctx;
     return CHIM_OK;
 }
@@ -363,12 +365,20 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     DlGrid grid = make_dl_grid(xmin, xmax, choose_dl_intervals(ctx, xmin, xmax));
 
     std::vector<float4> rec(2 * NS);
+    // records of the event-local-polynomial sweep: {t, m1d, m2d, ln m1d}, {ln m2d, log2(1/prior) - scale, 0, 0}; every
+    // event padded to a multiple of 32 samples with copies of its last one (whole warps read without bounds checks)
+    std::vector<int64_t> poff(n_events + 1, 0);
+    for (int i = 0; i < n_events; ++i) poff[i + 1] = poff[i] + ((so[i + 1] - so[i] + 31) / 32) * 32;
+    std::vector<float4> prec(2 * (size_t)poff[n_events]);
     std::vector<int32_t> k_lo(n_events), k_hi(n_events);
     const double l2e = 1.4426950408889634074;
     std::vector<int32_t> perm(NS);
     std::vector<double> zc(NG), qg(NG), z0(n_events), shift(n_events), qshift(n_events), udz(n_events);
     std::vector<float> qn(NG);
     std::vector<double> lm_lo(n_events), lm_hi(n_events);
+    std::vector<double> tk_c(n_events), tk_h(n_events);
+    std::vector<uint32_t> tkq_c(n_events);
+    std::vector<float> tq_scale(n_events);   // (host-side intermediates of the polynomial coordinate)
     std::vector<int32_t> idx;
     for (int i = 0; i < n_events; ++i) {
         const int64_t s0 = so[i];
@@ -395,6 +405,22 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
             const int k = std::min(std::max((int)(tkq >> kTkFracBits), 1), grid.K);
             if (j == 0) k_lo[i] = k;
             k_hi[i] = k;
+        }
+        {   // event-local polynomials of k_events: centre / half-width of the samples in table coordinates
+            const double fq = (double)(1u << kTkFracBits);
+            const double q_lo = (double)f_bits(rec[2 * s0].x), q_hi = (double)f_bits(rec[2 * (s0 + ns - 1)].x);
+            tkq_c[i] = (uint32_t)(0.5 * (q_lo + q_hi));
+            tk_c[i] = (double)tkq_c[i] / fq;
+            const double half = std::max(q_hi - (double)tkq_c[i], (double)tkq_c[i] - q_lo) / fq + 1e-3;
+            tk_h[i] = (half * grid.dx <= kPolyMaxHalfRange) ? half : 0.0;
+            tq_scale[i] = (float)(1.0 / (half * fq));
+            const int64_t p0 = poff[i], np = poff[i + 1] - p0;
+            for (int64_t j = 0; j < np; ++j) {
+                const int64_t js = s0 + std::min<int64_t>(j, ns - 1), o = s0 + idx[std::min<int64_t>(j, ns - 1)];
+                const double t = ((double)f_bits(rec[2 * js].x) - (double)tkq_c[i]) / (half * fq);
+                prec[2 * (p0 + j)] = make_float4((float)t, (float)h_m1[o], (float)h_m2[o], (float)std::log(h_m1[o]));
+                prec[2 * (p0 + j) + 1] = make_float4((float)std::log(h_m2[o]), rec[2 * js + 1].w, 0.f, 0.f);
+            }
         }
         const int64_t g0 = go[i];
         const int nz = (int)(go[i + 1] - g0);
@@ -432,6 +458,8 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     CK(upload(ctx->owned_ev, &E.uni_dz, udz));
     CK(upload(ctx->owned_ev, &E.lnm1_lo, lm_lo)); CK(upload(ctx->owned_ev, &E.lnm1_hi, lm_hi));
     CK(upload(ctx->owned_ev, &E.z0, z0));
+    CK(upload(ctx->owned_ev, &E.tk_c, tk_c)); CK(upload(ctx->owned_ev, &E.tk_h, tk_h));
+    CK(upload(ctx->owned_ev, &E.poly_off, poff)); CK(upload(ctx->owned_ev, &E.prec, prec));
     if (fixed_bw) CK(upload(ctx->owned_ev, &E.fixed_bw, h_bw));
     CK(upload(ctx->owned_ev, &ctx->ev_ln_shift, shift));
     CK(upload(ctx->owned_ev, &ctx->ev_ln_qscale, qshift));

@@ -30,6 +30,9 @@ struct LamF {
     float tkmax_ev, tkmax_inj;// table coordinate beyond which z > z_table_max
     float zcat_hi, zcat_lo;   // z_cat_max (R6) as hi + lo
     uint32_t tkmax_ev_q;      // tkmax_ev in the 12.20 fixed point of the event records
+    float gk2, cpsi;          // (gamma + kappa) log2(e) and gk2 ln(1 + z_p): log2 psi = gamma2 u - log2(1 + 2^(gk2 u - cpsi));
+                              // placement ON_GRID (no psi in the sample weights): gk2 = 0, cpsi = 100
+    float mlow_tm;            // 1 - ln(m_low) tm_scale: tm = ln(m1) tm_scale + mlow_tm
 };
 
 // Per-lambda constants written by the table kernel (S1), read by every other kernel.
@@ -251,6 +254,12 @@ struct EventSetDev {
     const int32_t* k_lo;        // [n_events] first / last row of the z(ln d_L) table the event's samples address
     const int32_t* k_hi;
     const double* fixed_bw;     // [n_events] or null
+    // event-local polynomials (k_events, S2): centre and half-width of the event's samples in table coordinates
+    // (tk_h = 0: the event's d_L range is too wide for them), and the same centre / scale for the 12.20 fixed point
+    const double* tk_c;         // [n_events]
+    const double* tk_h;         // [n_events]
+    const int64_t* poly_off;    // [n_events+1] offsets into prec (events padded to a multiple of 32 samples)
+    const float4* prec;         // records of the polynomial sweep: {t in [-1,1], m1d, m2d, ln m1d}, {ln m2d, log2(1/prior) - scale, 0, 0}
 };
 
 struct EventKernelParams {
@@ -309,6 +318,7 @@ cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);
 cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, int64_t n, const double* dL,
                                 double z_table_max, double* z_out, double* r_out, cudaStream_t st);
 cudaError_t upload_gauss_legendre();   // fills the __constant__ node tables used by S1
+cudaError_t upload_poly_matrices();    // fills the __constant__ fit matrices of the event-local polynomials (k_events)
 cudaError_t measure_alu_peaks(int n_sm, int reps, cudaStream_t st, double out_g[4]);
 size_t events_smem_bytes(int max_ns, int max_nz);
 size_t tables_smem_bytes(const TableParams& P);

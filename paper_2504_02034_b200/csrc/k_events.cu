@@ -42,6 +42,18 @@ constexpr float kMaxPowExp = 100.f;      // bound on log2 of the largest s^b ins
 constexpr int kRowStage = 224;           // rows of the z(ln d_L) table staged per CTA (14 KB)
 constexpr int kMassStage = 384;          // mass-table rows staged per CTA and variant (2 x 6 KB)
 
+constexpr int kLeP = 12;                 // terms of the local expansion (degree 11)
+constexpr int kLeMaxBox = 96;            // boxes per event the local-expansion form accepts
+constexpr float kLeMaxW = 1.3f;          // largest box width in units of sqrt(2) h (truncation error)
+
+// Event-local polynomials (S2): on an event whose samples span <= 0.9 in ln d_L, z - z0, ln(1+z), 1/(1+z) and the
+// smooth part of log2 of the redshift factor are polynomials in t in [-1, 1] (degree 6, 5, 5, 5; errors < 1e-8, 4e-8,
+// 6e-8 and 1e-8), fitted per (event, lambda) through 7 Chebyshev nodes read from the per-lambda z(ln d_L) table.
+constexpr int kPolyN = 7;
+__constant__ double c_poly_node[kPolyN];          // Chebyshev nodes cos(pi (k + 1/2) / 7)
+__constant__ double c_poly_m7[kPolyN][kPolyN];    // node values -> monomial coefficients, degree 6 (interpolation)
+__constant__ double c_poly_m6[kPolyN][kPolyN];    // node values -> monomial coefficients, degree 5 (discrete least squares; row 6 = 0)
+
 typedef unsigned long long f32x2;        // two packed floats (lo, hi) for the FFMA2 pipe
 __device__ __forceinline__ f32x2 pack2(float lo, float hi) {
     f32x2 r;
@@ -116,10 +128,15 @@ struct EvSmem {
     float fred[kEvThreads / 32];
     unsigned long long mbar;
     int pass_counter;
-    int mass_lo;
+    int mass_lo, mass_fit;
     double h, scd;            // bandwidth and the coordinate scale (as the rounded float, widened)
     float scf, delta, xfirst; // scale, grid spacing and first grid point in scaled coordinates
     int Bsel;                 // block size of the power form, 0 = direct form
+    // local-expansion form (le_nbox > 0): coordinates y = z'/(sqrt(2) h)
+    float scy, dy, yfirst;    // scale, grid spacing and first grid point in y
+    int le_m, le_D, le_blo, le_nbox;   // grid points per box, half-width of the psi table, first box, number of boxes
+    // event-local polynomials of S2 (use_poly != 0): z - z0 [7], ln(1+z) [7], 1/(1+z) [7], smooth log2 factor [7]
+    float poly[4 * kPolyN];
 };
 
 __host__ __device__ inline size_t ev_ns_pad(size_t ns) { return (ns + kPass - 1) / kPass * kPass; }
@@ -180,6 +197,171 @@ __device__ __forceinline__ void power_pass(const float* __restrict__ gq, int a_l
     unpack2(tot23, A[2], A[3]);
 }
 
+// ---- local-expansion form of S3 + S4 (equally spaced grid) -------------------------------------------------
+// With y = z'/(sqrt(2) h):  I ~ sum_j w_j A(y_j),  A(y) = sum_g q_g exp(-(y_g - y)^2).  In units of h the samples are far
+// denser than the grid, and A is entire, so A is expanded about box centres c_b placed on grid points (box = m grid
+// spacings ~ one unit of y):  exp(-(t - s)^2) = sum_n psi_n(t) s^n,  psi_n(t) = exp(-t^2) H_n(t)/n!  (generating function of
+// the Hermite polynomials), t = y_g - c_b, s = y - c_b, |s| <= w/2:
+//     A(y) = sum_{n<P} B_bn s^n + O((w/sqrt 2)^P / sqrt(P!)),   B_bn = sum_{|d| <= D} q_{g_b+d} psi_n(d dy)
+// (grid points beyond the cut-off t*h of the box are dropped: R9).  Because the centres sit on grid points, psi_n(d dy)
+// is ONE table per CTA, shared by all boxes (psi_n(-t) = (-1)^n psi_n(t)).  Per sample: one degree-(P-1) Horner
+// polynomial (packed FFMA2) instead of ~2 t h / dz Gaussian pairs.  P = 12, w <= 1.3: truncation < 1e-8 of A.
+struct LeSmem {
+    float* qs;      // [nzp]  q_g (x grid factor for placement ON_GRID), 0 beyond the grid
+    float* psi;     // [(D+1) * kLeP]
+    float* Bc;      // [nbox * kLeP]
+    int* jst;       // [nbox + 1] first sample of each box (samples are sorted)
+    int* cpre;      // [nbox + 1] prefix sum of the 128-sample chunks per box
+};
+__host__ __device__ inline size_t le_bytes(size_t nzp, int D, int nbox) {
+    return 4 * nzp + 4 * (size_t)kLeP * (D + 1) + 4 * (size_t)kLeP * nbox + 8 * (size_t)(nbox + 1) + 64;
+}
+__device__ __forceinline__ LeSmem le_layout(unsigned char* aux, size_t nzp, int D, int nbox) {
+    LeSmem M;
+    M.qs = reinterpret_cast<float*>(aux);
+    M.psi = M.qs + nzp;
+    M.Bc = M.psi + (size_t)kLeP * (D + 1);
+    M.jst = reinterpret_cast<int*>(M.Bc + (size_t)kLeP * nbox);
+    M.cpre = M.jst + (nbox + 1);
+    return M;
+}
+
+// Called by all threads after qs has been staged (and a barrier).  Returns this lane's sum_j w_j A_j.
+template <bool kStats>
+__device__ double le_phase(const EvSmem& S, const LeSmem& M, const float* __restrict__ zf, const float* __restrict__ wl,
+                           int ns, int nz, float Ty, unsigned long long& fma_ops, unsigned long long& pairs_cut) {
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const float scy = S.scy, dy = S.dy, yfirst = S.yfirst;
+    const int m = S.le_m, D = S.le_D, b_lo = S.le_blo, nbox = S.le_nbox;
+    const float wbox = (float)m * dy;
+    // (a) psi table: thread d computes psi_0..psi_{P-1} at t = d dy by the three-term recurrence
+    for (int d = tid; d <= D; d += kEvThreads) {
+        const float t = (float)d * dy, t2 = 2.f * t;
+        float p0 = ex2f(-t * t * 1.44269504088896341f), p1 = t2 * p0;
+        float* o = M.psi + (size_t)d * kLeP;
+        o[0] = p0;
+        o[1] = p1;
+#pragma unroll
+        for (int n = 1; n < kLeP - 1; ++n) {
+            const float p2 = fmaf(t2, p1, -2.f * p0) * (1.0f / (float)(n + 1));
+            o[n + 1] = p2;
+            p0 = p1;
+            p1 = p2;
+        }
+    }
+    // (b) first sample of every box: y_j >= left edge of box b_lo + i  (binary search on the sorted samples)
+    for (int i = tid; i <= nbox; i += kEvThreads) {
+        int a = 0;
+        if (i == nbox) a = ns;
+        else if (i > 0) {
+            const float edge = fmaf((float)(b_lo + i) - 0.5f, wbox, yfirst);
+            int b = ns;
+            while (a < b) { const int mid = (a + b) >> 1; if (zf[mid] * scy < edge) a = mid + 1; else b = mid; }
+        }
+        M.jst[i] = a;
+    }
+    __syncthreads();
+    // chunk prefix (warp 0; 3 boxes per lane)
+    if (wid == 0) {
+        int c[3], tot = 0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int i = 3 * lane + k;
+            c[k] = (i < nbox) ? (M.jst[i + 1] - M.jst[i] + kPass - 1) / kPass : 0;
+            tot += c[k];
+        }
+        int inc = tot;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+        int ex = inc - tot;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int i = 3 * lane + k;
+            if (i <= nbox) M.cpre[i] = ex;
+            ex += c[k];
+        }
+    }
+    // (c) coefficients: item = (box, quad of n, quarter of the d range); the four quarters sit in adjacent lanes
+    const int H = D >> 1, n_items = nbox * 12;
+    for (int base = 0; base < n_items; base += kEvThreads) {
+        const int id = base + tid;
+        const bool valid = id < n_items;
+        const int i = valid ? id / 12 : 0, rem = id - (id / 12) * 12, quad = rem >> 2, seg = rem & 3;
+        const int gc = (b_lo + i) * m;
+        const bool neg = seg < 2;
+        int d0 = (seg == 0 || seg == 3) ? H + 1 : (seg == 1 ? 1 : 0), d1 = (seg == 0 || seg == 3) ? D : H;
+        // clip to the grid: g = gc -/+ d in [0, nz)
+        if (neg) { d0 = max(d0, gc - (nz - 1)); d1 = min(d1, gc); }
+        else { d0 = max(d0, -gc); d1 = min(d1, nz - 1 - gc); }
+        if (!valid) d1 = d0 - 1;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float* qp = M.qs + gc;
+        const float4* pp = reinterpret_cast<const float4*>(M.psi) + quad;
+#pragma unroll 2
+        for (int d = d0; d <= d1; ++d) {
+            const float q = qp[neg ? -d : d];
+            const float4 v = pp[d * (kLeP / 4)];
+            acc.x = fmaf(q, v.x, acc.x);
+            acc.y = fmaf(q, v.y, acc.y);
+            acc.z = fmaf(q, v.z, acc.z);
+            acc.w = fmaf(q, v.w, acc.w);
+        }
+        if (neg) { acc.y = -acc.y; acc.w = -acc.w; }   // psi_n(-t) = (-1)^n psi_n(t); n = 4 quad + {0,1,2,3}
+#pragma unroll
+        for (int o = 1; o <= 2; o <<= 1) {
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+            acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
+            acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+        }
+        if (valid && seg == 0) reinterpret_cast<float4*>(M.Bc)[i * (kLeP / 4) + quad] = acc;
+        if (kStats && valid) fma_ops += 4ull * (unsigned long long)max(0, d1 - d0 + 1);
+    }
+    __syncthreads();
+    // (d) evaluation: chunk k (128 consecutive samples of one box) goes to warp k mod 8
+    const int n_chunks = M.cpre[nbox];
+    const float inv_dy = 1.0f / dy;
+    double lsum = 0.0;
+    int i = 0;
+    for (int k = wid; k < n_chunks; k += kEvThreads / 32) {
+        while (M.cpre[i + 1] <= k) ++i;
+        const int j_end = M.jst[i + 1], j0 = M.jst[i] + (k - M.cpre[i]) * kPass + lane;
+        const float c = fmaf((float)((b_lo + i) * m), dy, yfirst);
+        const float4* bp = reinterpret_cast<const float4*>(M.Bc) + i * (kLeP / 4);
+        const float4 c0 = bp[0], c1 = bp[1], c2 = bp[2];
+        float sv[4], wv[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int j = j0 + 32 * r;
+            const bool ok = j < j_end;
+            sv[r] = ok ? fmaf(zf[j], scy, -c) : 0.f;
+            wv[r] = ok ? wl[j] : 0.f;
+        }
+        const f32x2 s01 = pack2(sv[0], sv[1]), s23 = pack2(sv[2], sv[3]);
+        f32x2 a01 = pack2(c2.w, c2.w), a23 = a01;
+#define CHIM_LE_STEP(cf) { const f32x2 q_ = pack2(cf, cf); a01 = fma2(a01, s01, q_); a23 = fma2(a23, s23, q_); }
+        CHIM_LE_STEP(c2.z) CHIM_LE_STEP(c2.y) CHIM_LE_STEP(c2.x)
+        CHIM_LE_STEP(c1.w) CHIM_LE_STEP(c1.z) CHIM_LE_STEP(c1.y) CHIM_LE_STEP(c1.x)
+        CHIM_LE_STEP(c0.w) CHIM_LE_STEP(c0.z) CHIM_LE_STEP(c0.y) CHIM_LE_STEP(c0.x)
+#undef CHIM_LE_STEP
+        float A[4];
+        unpack2(a01, A[0], A[1]);
+        unpack2(a23, A[2], A[3]);
+        lsum += (double)fmaf(wv[0], A[0], fmaf(wv[1], A[1], fmaf(wv[2], A[2], wv[3] * A[3])));
+        if (kStats) {
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+                if (wv[r] > 0.f) {
+                    const float y = sv[r] + c;
+                    const int a = max(0, (int)ceilf((y - Ty - yfirst) * inv_dy)), b = min(nz - 1, (int)floorf((y + Ty - yfirst) * inv_dy));
+                    pairs_cut += (unsigned long long)max(0, b - a + 1);
+                    fma_ops += kLeP;
+                }
+        }
+    }
+    return lsum;
+}
+
 // S2 sweep 1 over the event's samples: z_j - z0 and log2 w_j to shared memory; returns the thread's max log2 w.
 template <bool kStaged>
 __device__ __forceinline__ float s2_sweep(const float4* __restrict__ rec, const LamF& Fs, const float4* __restrict__ rows,
@@ -215,6 +397,147 @@ __device__ __forceinline__ float s2_sweep(const float4* __restrict__ rec, const 
         }
     }
     return mx;
+}
+
+// S2 sweep 1 with the event-local polynomials: the same quantities as sample_eval, per sample
+//   t from the record's fixed-point table coordinate; z - z0, u = ln(1+z), a = 1/(1+z), r by Horner;
+//   m' = m^d a - m_low;  log2 w = LQ2(ln m1) + beta2 ln m2^d + r + log2(1/prior) - 2 log2 m1' - log2(1 + 2^(gk2 u - cpsi))
+//                                 - log2(1 + e^f(m2'))      (r carries -beta2 u and everything of log2(psi/J) but the
+//   Madau-Dickinson turnover, whose poles sit too close to the real axis for a low-degree polynomial).
+// PAPER.md:52, :195-198 eq. 20, :226 eq. 21, :75 eq. 11.  Warp-collective like sample_eval.
+// kFit: every mass-table row the event can address is staged (the tm clamp keeps the index inside the stage).
+// All samples of an event on this path lie inside the table (use_poly), so there is no range check.
+template <bool kFit>
+__device__ __forceinline__ float s2_sweep_poly(const float4* __restrict__ prec, const LamF& Fs, const float* __restrict__ pc,
+                                               const MassLookup& M, int ns, float* __restrict__ zf, float* __restrict__ wl) {
+    float mx = -INFINITY;
+    const int tid = threadIdx.x;
+    const LamF F = Fs;
+    float cz[kPolyN], cu[kPolyN - 1], ca[kPolyN - 1], cr[kPolyN - 1];
+#pragma unroll
+    for (int n = 0; n < kPolyN; ++n) cz[n] = pc[n];
+#pragma unroll
+    for (int n = 0; n < kPolyN - 1; ++n) { cu[n] = pc[kPolyN + n]; ca[n] = pc[2 * kPolyN + n]; cr[n] = pc[3 * kPolyN + n]; }
+    const int ns32 = (ns + 31) & ~31;                // the records are padded to ns32 with copies of the last sample
+    // clamp of the mass-table coordinate: the table's range, and (kFit) the staged rows [M.lo, M.lo + M.cap)
+    const float tm_lo = kFit ? fmaxf(1.0f, (float)M.lo) : 1.0f;
+    const float tm_hi = kFit ? fminf(F.tm_max, (float)(M.lo + M.cap) - 0.01f) : F.tm_max;
+    const float4* p = prec + 2 * tid;
+    Rec R;
+    if (tid < ns32) R = ldg_stream_rec(p);
+#pragma unroll 2
+    for (int j = tid; j < ns32; j += kEvThreads) {
+        const float4 A = R.A, Bq = R.B;
+        p += 2 * kEvThreads;
+        if (j + kEvThreads < ns32) R = ldg_stream_rec(p);
+        const float t = A.x;
+        float zc = cz[6], u = cu[5], a = ca[5], r = cr[5];
+#pragma unroll
+        for (int n = 5; n >= 0; --n) zc = fmaf(zc, t, cz[n]);
+#pragma unroll
+        for (int n = 4; n >= 0; --n) { u = fmaf(u, t, cu[n]); a = fmaf(a, t, ca[n]); r = fmaf(r, t, cr[n]); }
+        const float mp1 = fmaf(A.y, a, -F.mlow_hi) - F.mlow_lo, mp2 = fmaf(A.z, a, -F.mlow_hi) - F.mlow_lo;
+        const float lm1 = A.w - u;
+        float tm = fmaf(lm1, F.tm_scale, F.mlow_tm);
+        tm = fminf(fmaxf(tm, tm_lo), tm_hi);
+        const float ti = (tm - 0.5f) + 12582912.f;
+        const int km = __float_as_int(ti) - 0x4B400000;
+        const float tf = tm - (ti - 12582912.f);
+        const bool gauss_only = mp1 > F.mhigh_p;
+        const int ks = km - M.lo;
+        float4 c;
+        if (kFit) {
+            c = M.s[ks + (gauss_only ? M.cap : 0)];
+        } else {
+            const bool staged = (unsigned)ks < (unsigned)M.cap;
+            c = M.s[(staged ? ks : 0) + (gauss_only ? M.cap : 0)];
+            if (__any_sync(0xffffffffu, !staged)) {
+                if (!staged) c = __ldg(M.g + km + (gauss_only ? M.n_mass + 2 : 0));
+            }
+        }
+        float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x);
+        l += fmaf(F.beta2, Bq.x, r + Bq.y);
+        l = fmaf(-2.f, lg2f(fmaxf(mp1, 1e-30f)), l);
+        l -= lg2f(1.0f + ex2f(fminf(fmaf(F.gk2, u, -F.cpsi), 100.f)));
+        if (__any_sync(0xffffffffu, mp2 < F.delta)) {
+            const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
+            const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
+            const float ls = lg2f(1.0f + ex2f(f2));
+            l -= (mp2 < F.delta) ? ls : 0.f;
+        }
+        const float l2w = (mp2 > 0.f) ? l : -INFINITY;      // R15 support: m_low < m2
+        if (j < ns) {
+            zf[j] = zc;
+            wl[j] = l2w;
+            mx = fmaxf(mx, l2w);
+        }
+    }
+    return mx;
+}
+
+// Fit of the event-local polynomials by one warp: lanes 0..6 read the table at the Chebyshev nodes of the event's
+// range (fp64 from the rows' hi + lo terms), then every lane n < 7 forms coefficient n of the four polynomials.
+__device__ __forceinline__ void fit_event_polys(const LamConst& L, const Row* __restrict__ tab, int K, double tk_c, double tk_h,
+                                                double z0, float* __restrict__ out) {
+    const int lane = threadIdx.x & 31;
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
+    if (lane < kPolyN) {
+        const double tk = tk_c + tk_h * c_poly_node[lane];
+        const int k = max(1, min((int)tk, K));
+        const float t = (float)(tk - (double)k);
+        const float4* r = reinterpret_cast<const float4*>(tab + k);
+        const float4 q0 = __ldg(r), q1 = __ldg(r + 1), q3 = __ldg(r + 3);
+        const double z = (double)q0.x + (double)fmaf(fmaf(fmaf(q1.x, t, q0.w), t, q0.z), t, q0.y);
+        const double rr = (double)fmaf(fmaf(q3.w, t, q3.z), t, q3.y);
+        const double u = log1p(z);
+        const double turn = (L.F.gk2 != 0.f) ? log2(1.0 + exp2(1.4426950408889634074 * L.gk * (u - L.ln1pzp))) : 0.0;
+        v0 = z - z0;
+        v1 = u;
+        v2 = 1.0 / (1.0 + z);
+        v3 = rr + turn - 1.4426950408889634074 * L.beta * u;
+    }
+    double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+    const int n = min(lane, kPolyN - 1);
+#pragma unroll
+    for (int k = 0; k < kPolyN; ++k) {
+        const double m7 = c_poly_m7[n][k], m6 = c_poly_m6[n][k];
+        c0 = fma(m7, __shfl_sync(0xffffffffu, v0, k), c0);
+        c1 = fma(m6, __shfl_sync(0xffffffffu, v1, k), c1);
+        c2 = fma(m6, __shfl_sync(0xffffffffu, v2, k), c2);
+        c3 = fma(m6, __shfl_sync(0xffffffffu, v3, k), c3);
+    }
+    if (lane < kPolyN) {
+        out[lane] = (float)c0;
+        out[kPolyN + lane] = (float)c1;
+        out[2 * kPolyN + lane] = (float)c2;
+        out[3 * kPolyN + lane] = (float)c3;
+    }
+}
+
+cudaError_t upload_poly_matrices() {
+    double node[kPolyN], A[kPolyN][kPolyN], C[kPolyN][kPolyN] = {}, m7[kPolyN][kPolyN], m6[kPolyN][kPolyN];
+    const double pi = 3.14159265358979323846;
+    for (int k = 0; k < kPolyN; ++k) node[k] = cos(pi * (k + 0.5) / kPolyN);
+    for (int m = 0; m < kPolyN; ++m)            // Chebyshev coefficient m from the node values (discrete orthogonality)
+        for (int k = 0; k < kPolyN; ++k) A[m][k] = (m == 0 ? 1.0 : 2.0) / kPolyN * cos(m * pi * (k + 0.5) / kPolyN);
+    C[0][0] = 1.0;                              // C[n][m]: coefficient of t^n in T_m
+    C[1][1] = 1.0;
+    for (int m = 2; m < kPolyN; ++m)
+        for (int n = 0; n < kPolyN; ++n) C[n][m] = (n > 0 ? 2.0 * C[n - 1][m - 1] : 0.0) - C[n][m - 2];
+    for (int n = 0; n < kPolyN; ++n)
+        for (int k = 0; k < kPolyN; ++k) {
+            double a7 = 0.0, a6 = 0.0;
+            for (int m = 0; m < kPolyN; ++m) {
+                a7 += C[n][m] * A[m][k];
+                if (m < kPolyN - 1) a6 += C[n][m] * A[m][k];
+            }
+            m7[n][k] = a7;
+            m6[n][k] = (n < kPolyN - 1) ? a6 : 0.0;
+        }
+    cudaError_t e = cudaMemcpyToSymbol(c_poly_node, node, sizeof node);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_poly_m7, m7, sizeof m7);
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_poly_m6, m6, sizeof m6);
+    return e;
 }
 
 // shared-memory layout after EvSmem: zf float[ns_pad] | wl float[ns_pad] | aux = staged table rows + mass rows (S2) / gq float2[nz_pad] (S3)
@@ -261,6 +584,10 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         return;
     }
     const double z0 = P.ev.z0[ev];
+    // event-local polynomials (S2): narrow d_L range and every node inside the table
+    const double tk_h = P.ev.tk_h[ev], tk_c = P.ev.tk_c[ev];
+    const bool use_poly = tk_h > 0.0 && tk_c + tk_h < L.tkmax_ev;
+    if (use_poly && wid == 1) fit_event_polys(L, tab, P.tab_rows - 2, tk_c, tk_h, z0, S.poly);
 
     // ---- TMA: the event's slice of the z(ln d_L) table and the mass-table rows it can address: ln m1 = ln m1d - ln(1+z),
     //      z between the event's first and last (sorted) sample; rows outside the staged range fall back to global
@@ -272,9 +599,10 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         int mlo = ma - 1 + max(0, (mb - ma + 3 - mcap) / 2);                              // wider than the stage: keep the centre
         mlo = max(0, min(mlo, P.n_mass + 2 - mcap));
         S.mass_lo = mlo;
-        const uint32_t rb = staged ? (uint32_t)(k_hi - k_lo + 1) * (uint32_t)sizeof(Row) : 0u, mbytes = (uint32_t)mcap * (uint32_t)sizeof(MassRow);
+        S.mass_fit = (mb - ma + 3 <= mcap) ? 1 : 0;
+        const uint32_t rb = (staged && !use_poly) ? (uint32_t)(k_hi - k_lo + 1) * (uint32_t)sizeof(Row) : 0u, mbytes = (uint32_t)mcap * (uint32_t)sizeof(MassRow);
         mbar_expect_tx(&S.mbar, rb + 2 * mbytes);
-        if (staged) bulk_g2s(rows_s, tab + k_lo, rb, &S.mbar);
+        if (rb) bulk_g2s(rows_s, tab + k_lo, rb, &S.mbar);
         bulk_g2s(mass_s, mtab + mlo, mbytes, &S.mbar);
         bulk_g2s(mass_s + mcap, mtab + (P.n_mass + 2) + mlo, mbytes, &S.mbar);
     }
@@ -291,7 +619,10 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const float z0h = (float)z0, z0l = (float)(z0 - (double)z0h);
     float mx;
     const float4* rec = P.ev.rec + 2 * s0;
-    if (staged) mx = s2_sweep<true>(rec, L.F, rows_s, k_lo, M, ns, z0h, z0l, zf, wl);
+    const float4* prec = P.ev.prec + 2 * P.ev.poly_off[ev];
+    if (use_poly && S.mass_fit) mx = s2_sweep_poly<true>(prec, L.F, S.poly, M, ns, zf, wl);
+    else if (use_poly) mx = s2_sweep_poly<false>(prec, L.F, S.poly, M, ns, zf, wl);
+    else if (staged) mx = s2_sweep<true>(rec, L.F, rows_s, k_lo, M, ns, z0h, z0l, zf, wl);
     else mx = s2_sweep<false>(rec, L.F, reinterpret_cast<const float4*>(tab), 0, M, ns, z0h, z0l, zf, wl);
     // samples are sorted in d_L: one of them lies beyond the table iff the last one does
     if (tid == 0 && __float_as_uint(__ldg(rec + 2 * (size_t)(ns - 1)).x) > L.F.tkmax_ev_q) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
@@ -381,6 +712,24 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             else if (delta * 16.f <= kMaxBlockSpan) Bsel = 16;
         }
         S.h = h; S.scd = scd; S.scf = scf; S.delta = delta; S.xfirst = (float)(zc_g[0] * scd); S.Bsel = Bsel;
+        // local-expansion form: equally spaced grid, a cut-off, boxes of ~1 unit of y = z'/(sqrt(2) h) that fit the stage
+        S.le_nbox = 0; S.le_D = 0;
+        if (udz > 0.0 && T < INFINITY && P.kde_method == CHIM_KDE_AUTO && !P.dbg_K && h > 0.0 && isfinite(h)) {
+            const float scy = (float)(0.70710678118654752440 / h);
+            const float dy = (float)(udz * (double)scy);
+            const int m = max(1, (int)lrintf(1.0f / dy));
+            const float wbox = (float)m * dy, Ty = (float)(P.cutoff * 0.70710678118654752440);
+            const float yfirst = (float)(zc_g[0] * (double)scy);
+            const float fb_lo = floorf((zf[0] * scy - yfirst) / wbox + 0.5f), fb_hi = floorf((zf[ns - 1] * scy - yfirst) / wbox + 0.5f);
+            const float fD = ceilf((Ty + 0.5f * wbox) / dy) + 1.0f;
+            if (wbox <= kLeMaxW && fb_hi - fb_lo < (float)kLeMaxBox && fabsf(fb_lo) < 1e6f && fabsf(fb_hi) < 1e6f && fD < 1e5f &&
+                fabsf(fb_lo) * (float)m < 1e8f && fabsf(fb_hi) * (float)m < 1e8f) {
+                const int D = (int)fD, nbox = (int)(fb_hi - fb_lo) + 1;
+                if (le_bytes(ev_nz_pad(nz), D, nbox) <= ev_aux_bytes(P.ev.max_nz)) {
+                    S.scy = scy; S.dy = dy; S.yfirst = yfirst; S.le_m = m; S.le_D = D; S.le_blo = (int)fb_lo; S.le_nbox = nbox;
+                }
+            }
+        }
     }
     __syncthreads();
     const double h = S.h;
@@ -396,7 +745,20 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const int Bsel = S.Bsel;
     const int nzp = (int)ev_nz_pad(nz);
     const bool on_grid = P.placement == CHIM_ON_GRID;
-    if (Bsel && !on_grid) {   // power form: q'_g = q_g 2^(-(b delta)^2), b = g mod B, duplicated for the packed FMA
+    const int le_nbox = S.le_nbox;
+    LeSmem LM = le_layout(aux, (size_t)nzp, S.le_D, le_nbox);
+    if (le_nbox) {            // local-expansion form: plain q_g (x grid factor)
+        for (int g = tid; g < nzp; g += kEvThreads) {
+            float q = 0.f;
+            if (g < nz) {
+                q = qn_g[g];
+                if (on_grid)
+                    q = (float)((double)q * grid_factor(L, P.dc_tab + (size_t)l * (P.n_table + 1 + kZPad), P.n_table + 1 + kZPad,
+                                                        P.z_table_max / P.n_table, zc_g[g] + z0));
+            }
+            LM.qs[g] = q;
+        }
+    } else if (Bsel && !on_grid) {   // power form: q'_g = q_g 2^(-(b delta)^2), b = g mod B, duplicated for the packed FMA
         for (int g = tid; g < nzp; g += kEvThreads) {   // (the barriers above fenced the last reads of the staged tables)
             const float bd = (float)(g & (Bsel - 1)) * delta;
             gqp[g] = (g < nz) ? qn_g[g] * ex2f(-bd * bd) : 0.f;
@@ -429,7 +791,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const int a_max = Bsel ? nzp / Bsel - 1 : 0;
     double lsum = 0.0;                          // this lane's sum_j w_j A_j
     unsigned long long pairs_exec = 0, pairs_cut = 0;
-    for (;;) {
+    if (le_nbox) lsum = le_phase<kStats>(S, LM, zf, wl, ns, nz, (float)(P.cutoff * 0.70710678118654752440), pairs_exec, pairs_cut);
+    else for (;;) {
         int pass = 0;
         if (lane == 0) pass = atomicAdd(&S.pass_counter, 1);
         pass = __shfl_sync(0xffffffffu, pass, 0);

@@ -452,6 +452,9 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         F.tm_scale = (float)L.inv_dlm; F.tm_max = (float)P.n_mass + 0.999f;
         F.tkmax_ev = (float)fmin(L.tkmax_ev, 1e9) * (1.0f - 1e-6f); F.tkmax_inj = (float)fmin(L.tkmax_inj, 1e9) * (1.0f - 1e-6f);
         F.zcat_hi = (float)P.z_cat_max; F.zcat_lo = (float)(P.z_cat_max - (double)F.zcat_hi);
+        if (P.placement == CHIM_ON_SAMPLES) { F.gk2 = (float)(L.gk * l2e); F.cpsi = (float)(L.gk * l2e * L.ln1pzp); }
+        else { F.gk2 = 0.f; F.cpsi = 100.f; }
+        F.mlow_tm = (float)(1.0 - L.lm0 * L.inv_dlm);
         F.tkmax_ev_q = (L.tkmax_ev >= 4095.9) ? 0xFFFFFFFFu : (L.tkmax_ev <= 0.0 ? 0u : (uint32_t)(L.tkmax_ev * (double)(1u << kTkFracBits)));
     }
     __syncthreads();

@@ -192,6 +192,24 @@ def test_three_catalogs_small(P):
         assert rel < REL_EVENT and dtot < ABS_TOTAL
 
 
+def test_s2_wide_distance_posteriors_take_the_table_path(P):
+    # events whose samples span more than 0.9 in ln d_L are outside the range of the event-local polynomials of S2
+    # and go through the per-lambda z(ln d_L) table rows; both paths in one batch
+    w = make_workload("o5_spec", n_events=6, n_samples=2000, n_grid=600, n_lambda=6, n_det=3000)
+    rng = np.random.default_rng(7)
+    for i in (1, 3, 4):     # widen: d_L -> d_L * exp(0.35 eps), prior recomputed (ln pi = 2 ln d_L)
+        s = slice(w.sample_off[i], w.sample_off[i + 1])
+        w.dL[s] = w.dL[s] * np.exp(0.35 * rng.standard_normal(w.dL[s].size))
+        w.ln_prior[s] = 2.0 * np.log(w.dL[s])
+    rng_ln = [np.ptp(np.log(w.dL[w.sample_off[i]:w.sample_off[i + 1]])) for i in range(w.n_events)]
+    assert min(rng_ln) < 0.9 < max(rng_ln)
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    assert np.max(np.abs(r["event_logI"] - ref["event_logI"])) < 5e-6
+
+
 def test_events_deep_in_the_smoothing_window(P):
     # every sample of the event sits in the lower part of [m_low, m_low + delta_m], where S and C(m1) both vanish
     # faster than any power: the weights are tiny but their ratios decide log I (n_eff can drop to ~1)
@@ -226,21 +244,31 @@ def test_host_entry_point_matches_device_entry_point(P):
     c.close()
 
 
-# ---------------------------------------------------------------- the two formulations of the pair loop
-def test_kde_power_form_and_direct_form_agree_with_the_oracle(P):
-    # equally spaced grids: AUTO takes the power form (Horner in s = 2^(-2 delta u), FFMA2), DIRECT one ex2 per pair
+# ---------------------------------------------------------------- the three formulations of the KDE
+def test_kde_local_expansion_power_and_direct_forms_agree_with_the_oracle(P):
+    # equally spaced grids: AUTO takes the local-expansion form (one degree-11 polynomial per sample), POWER the power
+    # form (Horner in s = 2^(-2 delta u), FFMA2), DIRECT one ex2 per pair
     w = make_workload("o5_spec", n_events=8, n_lambda=12, n_det=4000)
     ref = O.loglike_workload(w)
     ra = _gpu(P, w, kde_method=P.CHIM_KDE_AUTO)
+    rp = _gpu(P, w, kde_method=P.CHIM_KDE_POWER)
     rd = _gpu(P, w, kde_method=P.CHIM_KDE_DIRECT)
-    for r in (ra, rd):
+    for r in (ra, rp, rd):
         rel, dtot, _ = _compare(r, ref, w.n_events)
         assert rel < REL_EVENT and dtot < ABS_TOTAL
-        assert np.max(np.abs(r["event_logI"] - ref["event_logI"])) < 2e-6     # 50x inside the per-event budget
+        assert np.max(np.abs(r["event_logI"] - ref["event_logI"])) < 5e-6     # 600x inside the per-event budget (|log I| ~ 30)
+        assert abs(np.mean(r["event_logI"] - ref["event_logI"])) < 5e-7       # no systematic offset that 300 events would add up
         st = r["stats"]
-        assert 0 < st["kde_pairs_in_cutoff"] <= st["kde_pairs_evaluated"] < st["kde_pairs_dense"]
-    assert ra["stats"]["kde_pairs_in_cutoff"] == rd["stats"]["kde_pairs_in_cutoff"]
+        assert 0 < st["kde_pairs_in_cutoff"] < st["kde_pairs_dense"] and st["kde_pairs_evaluated"] < st["kde_pairs_dense"]
+    for r in (rp, rd):    # pair loops execute every pair inside the cut-off (plus band padding)
+        assert r["stats"]["kde_pairs_in_cutoff"] <= r["stats"]["kde_pairs_evaluated"]
+    # the local expansion replaces the pairs by fewer FMA operations (coefficient build + one polynomial per sample)
+    assert 0 < ra["stats"]["kde_pairs_evaluated"] < ra["stats"]["kde_pairs_in_cutoff"]
+    # the algorithmic pair count does not depend on the formulation (edge pairs may round differently: 1e-4)
+    for r in (ra, rp):
+        assert abs(r["stats"]["kde_pairs_in_cutoff"] / rd["stats"]["kde_pairs_in_cutoff"] - 1.0) < 1e-4
     assert np.max(np.abs(ra["event_logI"] - rd["event_logI"])) < 2e-6
+    assert np.max(np.abs(rp["event_logI"] - rd["event_logI"])) < 2e-6
 
 
 def test_kde_nonuniform_grid_takes_the_direct_form(P):
