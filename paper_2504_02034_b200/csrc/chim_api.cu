@@ -27,7 +27,8 @@ struct chim_ctx {
     chim_config cfg;
     cudaStream_t stream = nullptr;
     std::string err;
-    std::vector<void*> owned_ev, owned_inj, owned_work, owned_host;
+    std::vector<void*> owned_ev, owned_inj, owned_work, owned_host, owned_ctx;
+    const double* poly_mats = nullptr;     // fit matrices of the local polynomials (device)
     // events
     bool have_events = false;
     EventSetDev ev{};
@@ -48,6 +49,7 @@ struct chim_ctx {
     double ev_m_top = 0.0, inj_m_top = 0.0;   // largest detector-frame m1 of each loaded set
     double* dc_tab = nullptr; double* logI = nullptr; double2* partial = nullptr; uint32_t* flags = nullptr;
     unsigned long long* stats = nullptr;
+    float* poly_ev = nullptr; float* poly_inj = nullptr;   // local polynomials per (lambda, event) / (lambda, chunk)
     // staging for the host-pointer entry point
     int host_nl = 0;
     double* st_lam = nullptr; double* st_ll = nullptr; double* st_ev = nullptr; double* st_xi = nullptr;
@@ -143,6 +145,8 @@ int ensure_work(chim_ctx* ctx, int nl) {
     CK(dev_alloc(ctx->owned_work, &ctx->partial, (size_t)nl * std::max(ctx->inj_blocks, 1)));
     CK(dev_alloc(ctx->owned_work, &ctx->flags, nl));
     CK(dev_alloc(ctx->owned_work, &ctx->stats, 4));
+    CK(dev_alloc(ctx->owned_work, &ctx->poly_ev, (size_t)nl * ctx->ev.n_events * 4 * kPolyN));
+    CK(dev_alloc(ctx->owned_work, &ctx->poly_inj, (size_t)nl * std::max(ctx->inj_blocks, 1) * 4 * kPolyN));
     ctx->work_nl = nl;
     ctx->work_has_dc = need_dc;
     return CHIM_OK;
@@ -172,6 +176,7 @@ EventKernelParams event_params(const chim_ctx* ctx, int nl) {
     P.logI = ctx->logI; P.flags = ctx->flags; P.stats = ctx->stats;
     P.ln_shift = ctx->ev_ln_shift;
     P.ln_qscale = ctx->ev_ln_qscale;
+    P.poly = ctx->poly_ev;
     P.dbg_event = -1;
     return P;
 }
@@ -200,6 +205,15 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
     TableParams TP = table_params(ctx);
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t) * nl, st));
     { Bracket b(ctx, 0); CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, st)); }
+    {   // local-polynomial fits (part of S1: per-lambda interpolants)
+        Bracket b(ctx, 0);
+        CK(launch_polyfit(ctx->Lc, ctx->tab_ev, ctx->ev_grid.rows(), nl, ctx->ev.n_events, ctx->ev.tk_c, ctx->ev.tk_h, ctx->ev.z0, 0.0,
+                          false, ctx->poly_mats, ctx->poly_ev, st));
+        if (ctx->have_inj)
+            CK(launch_polyfit(ctx->Lc, ctx->tab_inj, ctx->inj_grid.rows(), nl, ctx->inj_blocks, ctx->inj.tk_c, ctx->inj.tk_h, nullptr,
+                              ctx->cfg.z_cat_max, true, ctx->poly_mats, ctx->poly_inj, st));
+        ctx->launches += ctx->have_inj ? 2 : 1;
+    }
     EventKernelParams EP = event_params(ctx, nl);
     { Bracket b(ctx, 1); CK(launch_events(EP, ctx->cfg.count_pairs != 0, st)); }
     ctx->launches += 2;
@@ -208,7 +222,7 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
         IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.mtab = ctx->mtab;
         IP.n_lambda = nl; IP.tab_rows = ctx->inj_grid.rows(); IP.n_mass = ctx->cfg.n_mass_table; IP.chunk = kInjChunk;
         IP.z_table_max = ctx->cfg.z_table_max; IP.z_cat_max = ctx->cfg.z_cat_max;
-        IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = nullptr;
+        IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = nullptr; IP.poly = ctx->poly_inj; IP.n_chunks = ctx->inj_blocks;
         { Bracket b(ctx, 2); CK(launch_inject(IP, ctx->inj_blocks, st)); }
         ctx->launches += 1;
     }
@@ -223,6 +237,32 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
     { Bracket b(ctx, 3); CK(launch_combine(CP, st)); }
     ctx->launches += 1;
     return CHIM_OK;
+}
+
+// Chebyshev nodes and the node-value -> monomial-coefficient matrices of the local polynomials (chim_internal.cuh)
+cudaError_t upload_poly_matrices(chim_ctx* ctx) {
+    constexpr int N = kPolyN;
+    std::vector<double> h(kPolyMatDoubles, 0.0);
+    double A[N][N], C[N][N] = {};
+    const double pi = 3.14159265358979323846;
+    for (int k = 0; k < N; ++k) h[k] = std::cos(pi * (k + 0.5) / N);
+    for (int m = 0; m < N; ++m)            // Chebyshev coefficient m from the node values (discrete orthogonality)
+        for (int k = 0; k < N; ++k) A[m][k] = (m == 0 ? 1.0 : 2.0) / N * std::cos(m * pi * (k + 0.5) / N);
+    C[0][0] = 1.0;                         // C[n][m]: coefficient of t^n in T_m
+    C[1][1] = 1.0;
+    for (int m = 2; m < N; ++m)
+        for (int n = 0; n < N; ++n) C[n][m] = (n > 0 ? 2.0 * C[n - 1][m - 1] : 0.0) - C[n][m - 2];
+    for (int n = 0; n < N; ++n)
+        for (int k = 0; k < N; ++k) {
+            double a7 = 0.0, a6 = 0.0;
+            for (int m = 0; m < N; ++m) {
+                a7 += C[n][m] * A[m][k];
+                if (m < N - 1) a6 += C[n][m] * A[m][k];
+            }
+            h[N + n * N + k] = a7;
+            h[N + N * N + n * N + k] = (n < N - 1) ? a6 : 0.0;
+        }
+    return upload(ctx->owned_ctx, &ctx->poly_mats, h);
 }
 
 bool all_finite(const std::vector<double>& v) {
@@ -293,7 +333,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     TableParams TP = table_params(ctx);
     TP.ev.K = TP.inj.K = c.n_dl_table > 0 ? c.n_dl_table : kMaxDlRows;
     if (tables_smem_bytes(TP) > kMaxSmemOptin || inject_smem_bytes(c.n_mass_table) > kMaxSmemOptin) { delete ctx; return CHIM_EINVAL; }
-    if (upload_gauss_legendre() != cudaSuccess || upload_poly_matrices() != cudaSuccess) { delete ctx; return CHIM_ECUDA; }
+    if (upload_gauss_legendre() != cudaSuccess || upload_poly_matrices(ctx) != cudaSuccess) { chim_destroy(ctx); return CHIM_ECUDA; }
     *out = ctx;
     return CHIM_OK;
 }
@@ -307,6 +347,7 @@ void chim_destroy(chim_ctx* ctx) {
     free_pool(ctx->owned_inj);
     free_pool(ctx->owned_work);
     free_pool(ctx->owned_host);
+    free_pool(ctx->owned_ctx);
     delete ctx;
 }
 
@@ -369,7 +410,8 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     // event padded to a multiple of 32 samples with copies of its last one (whole warps read without bounds checks)
     std::vector<int64_t> poff(n_events + 1, 0);
     for (int i = 0; i < n_events; ++i) poff[i + 1] = poff[i] + ((so[i + 1] - so[i] + 31) / 32) * 32;
-    std::vector<float4> prec(2 * (size_t)poff[n_events]);
+    std::vector<float4> prec_a((size_t)poff[n_events]);
+    std::vector<float2> prec_b((size_t)poff[n_events]);
     std::vector<int32_t> k_lo(n_events), k_hi(n_events);
     const double l2e = 1.4426950408889634074;
     std::vector<int32_t> perm(NS);
@@ -418,8 +460,8 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
             for (int64_t j = 0; j < np; ++j) {
                 const int64_t js = s0 + std::min<int64_t>(j, ns - 1), o = s0 + idx[std::min<int64_t>(j, ns - 1)];
                 const double t = ((double)f_bits(rec[2 * js].x) - (double)tkq_c[i]) / (half * fq);
-                prec[2 * (p0 + j)] = make_float4((float)t, (float)h_m1[o], (float)h_m2[o], (float)std::log(h_m1[o]));
-                prec[2 * (p0 + j) + 1] = make_float4((float)std::log(h_m2[o]), rec[2 * js + 1].w, 0.f, 0.f);
+                prec_a[p0 + j] = make_float4((float)t, (float)h_m1[o], (float)h_m2[o], (float)std::log(h_m1[o]));
+                prec_b[p0 + j] = make_float2((float)std::log(h_m2[o]), rec[2 * js + 1].w);
             }
         }
         const int64_t g0 = go[i];
@@ -459,7 +501,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     CK(upload(ctx->owned_ev, &E.lnm1_lo, lm_lo)); CK(upload(ctx->owned_ev, &E.lnm1_hi, lm_hi));
     CK(upload(ctx->owned_ev, &E.z0, z0));
     CK(upload(ctx->owned_ev, &E.tk_c, tk_c)); CK(upload(ctx->owned_ev, &E.tk_h, tk_h));
-    CK(upload(ctx->owned_ev, &E.poly_off, poff)); CK(upload(ctx->owned_ev, &E.prec, prec));
+    CK(upload(ctx->owned_ev, &E.poly_off, poff)); CK(upload(ctx->owned_ev, &E.prec_a, prec_a)); CK(upload(ctx->owned_ev, &E.prec_b, prec_b));
     if (fixed_bw) CK(upload(ctx->owned_ev, &E.fixed_bw, h_bw));
     CK(upload(ctx->owned_ev, &ctx->ev_ln_shift, shift));
     CK(upload(ctx->owned_ev, &ctx->ev_ln_qscale, qshift));
@@ -515,6 +557,25 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
         rec[2 * j] = make_float4(bits_f((uint32_t)k), (float)(tk - (double)k), (float)h_m1[o], (float)h_m2[o]);
         rec[2 * j + 1] = make_float4((float)std::log(h_m1[o]), (float)std::log(h_m2[o] / h_m1[o]), (float)(l2e * (-h_lp[o] - sh)), 0.f);
     }
+    // chunk-local polynomials of k_inject: the set is sorted in d_L, so a chunk of kInjChunk injections spans a narrow range
+    const int n_chunks = (int)((n_det + kInjChunk - 1) / kInjChunk);
+    std::vector<float4> prec_a((size_t)n_chunks * kInjChunk);
+    std::vector<float2> prec_b((size_t)n_chunks * kInjChunk);
+    std::vector<double> ctk_c(n_chunks), ctk_h(n_chunks);
+    for (int c = 0; c < n_chunks; ++c) {
+        const size_t a = (size_t)c * kInjChunk, b = std::min<size_t>(a + kInjChunk, N);
+        auto tk_of = [&](size_t j) { return (double)f_bits(rec[2 * j].x) + (double)rec[2 * j].y; };   // k + t
+        const double lo = tk_of(a), hi = tk_of(b - 1);
+        const double half = 0.5 * (hi - lo) * (1.0 + 1e-9) + 1e-3;
+        ctk_c[c] = 0.5 * (lo + hi);
+        ctk_h[c] = (half * grid.dx <= kPolyMaxHalfRange) ? half : 0.0;
+        for (size_t j = a; j < a + kInjChunk; ++j) {
+            const size_t js = std::min(j, b - 1), o = (size_t)idx[js];
+            const double t = (tk_of(js) - ctk_c[c]) / half;
+            prec_a[j] = make_float4((float)t, (float)h_m1[o], (float)h_m2[o], (float)std::log(h_m1[o]));
+            prec_b[j] = make_float2((float)std::log(h_m2[o]), rec[2 * js + 1].z);
+        }
+    }
     cudaStreamSynchronize(ctx->stream);
     free_pool(ctx->owned_inj);
     free_pool(ctx->owned_work);
@@ -525,6 +586,8 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     I.n_inj_total = (double)n_inj_total;
     CK(upload(ctx->owned_inj, &I.rec, rec));
     CK(upload(ctx->owned_inj, &I.perm, idx));
+    CK(upload(ctx->owned_inj, &I.prec_a, prec_a)); CK(upload(ctx->owned_inj, &I.prec_b, prec_b));
+    CK(upload(ctx->owned_inj, &I.tk_c, ctk_c)); CK(upload(ctx->owned_inj, &I.tk_h, ctk_h));
     ctx->inj = I;
     ctx->inj_m_top = m_top;
     ctx->inj_grid = grid;
@@ -663,6 +726,11 @@ static int debug_prepare(chim_ctx* ctx, const double* lambda, const char* who) {
     TableParams TP = table_params(ctx);
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t), ctx->stream));
     CK(launch_tables(lambda, 1, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, ctx->stream));
+    CK(launch_polyfit(ctx->Lc, ctx->tab_ev, ctx->ev_grid.rows(), 1, ctx->ev.n_events, ctx->ev.tk_c, ctx->ev.tk_h, ctx->ev.z0, 0.0, false,
+                      ctx->poly_mats, ctx->poly_ev, ctx->stream));
+    if (ctx->have_inj)
+        CK(launch_polyfit(ctx->Lc, ctx->tab_inj, ctx->inj_grid.rows(), 1, ctx->inj_blocks, ctx->inj.tk_c, ctx->inj.tk_h, nullptr,
+                          ctx->cfg.z_cat_max, true, ctx->poly_mats, ctx->poly_inj, ctx->stream));
     return CHIM_OK;
 }
 
@@ -709,7 +777,7 @@ int chim_debug_injection_weights(chim_ctx* ctx, const double* lambda, double* s_
     IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.mtab = ctx->mtab;
     IP.n_lambda = 1; IP.tab_rows = ctx->inj_grid.rows(); IP.n_mass = ctx->cfg.n_mass_table; IP.chunk = kInjChunk;
     IP.z_table_max = ctx->cfg.z_table_max; IP.z_cat_max = ctx->cfg.z_cat_max;
-    IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = s_out;
+    IP.partial = ctx->partial; IP.flags = ctx->flags; IP.dbg_s = s_out; IP.poly = ctx->poly_inj; IP.n_chunks = ctx->inj_blocks;
     IP.dbg_scale = std::exp(ctx->inj_ln_shift);
     CK(launch_inject(IP, ctx->inj_blocks, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));

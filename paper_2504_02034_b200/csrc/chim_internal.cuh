@@ -33,6 +33,7 @@ struct LamF {
     float gk2, cpsi;          // (gamma + kappa) log2(e) and gk2 ln(1 + z_p): log2 psi = gamma2 u - log2(1 + 2^(gk2 u - cpsi));
                               // placement ON_GRID (no psi in the sample weights): gk2 = 0, cpsi = 100
     float mlow_tm;            // 1 - ln(m_low) tm_scale: tm = ln(m1) tm_scale + mlow_tm
+    float gk2_inj, cpsi_inj;  // the same for the injections (psi is always in s_j)
 };
 
 // Per-lambda constants written by the table kernel (S1), read by every other kernel.
@@ -136,6 +137,15 @@ __device__ __forceinline__ double ex2_to_double(float y) {
     return (y > -1000.f) ? v : 0.0;
 }
 
+// Records of the local-polynomial sweeps, split for 24 B per sample: A = {t, m1d, m2d, ln m1d}, B = {ln m2d, log2(1/prior)}
+struct PRec { float4 A; float2 B; };
+__device__ __forceinline__ PRec ldg_stream_prec(const float4* pa, const float2* pb) {   // streaming reads (once per CTA)
+    PRec r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.A.x), "=f"(r.A.y), "=f"(r.A.z), "=f"(r.A.w) : "l"(pa));
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];" : "=f"(r.B.x), "=f"(r.B.y) : "l"(pb));
+    return r;
+}
+
 // Where a thread finds the per-lambda mass table: rows [lo, lo + cap) of both variants staged in shared memory
 // (variant "b" at offset cap), everything else in global memory.
 struct MassLookup {
@@ -209,6 +219,141 @@ __device__ __forceinline__ void sample_eval(const LamF& F, const float4 q0, cons
     l2w = ok ? l : -INFINITY;
 }
 
+// ---- packed fp32x2 arithmetic (FFMA2 pipe) --------------------------------------------------------------
+typedef unsigned long long f32x2;        // two packed floats (lo, hi) for the FFMA2 pipe
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+// ---- local polynomials in ln d_L (S2 of narrow events, S5 of injection chunks) -------------------------------
+// Over a range of <= 0.9 in ln d_L, z - z_ref, u = ln(1+z), a = 1/(1+z) and the smooth part r of log2 of the redshift factor
+// are polynomials in t in [-1, 1] (degree 6, 5, 5, 6; errors < 1e-8, 4e-8, 6e-8, 1e-9), fitted per (range, lambda)
+// through 7 Chebyshev nodes read from the per-lambda z(ln d_L) table.  The Madau-Dickinson turnover of psi is NOT in r
+// (its poles sit too close to the real axis for a low degree): it is evaluated per sample from u.
+constexpr int kPolyN = 7;
+constexpr int kPolyMatDoubles = kPolyN + 2 * kPolyN * kPolyN;   // nodes[7], m7[7][7] (degree 6), m6[7][7] (degree 5, row 6 = 0)
+
+// Coefficients paired for FFMA2: zr[n] = (z_n, r_n), ua[n] = (u_n, a_n); z and r of degree 6, u and a of degree 5.
+struct PolyCoef { f32x2 zr[kPolyN], ua[kPolyN - 1]; };
+__device__ __forceinline__ void load_poly(PolyCoef& C, const float* __restrict__ pc) {   // pc: float2 zr[7], float2 ua[7]
+    const f32x2* q = reinterpret_cast<const f32x2*>(pc);
+#pragma unroll
+    for (int n = 0; n < kPolyN; ++n) C.zr[n] = q[n];
+#pragma unroll
+    for (int n = 0; n < kPolyN - 1; ++n) C.ua[n] = q[kPolyN + n];
+}
+
+// One warp: lanes 0..6 read the table at the Chebyshev nodes of [tk_c - tk_h, tk_c + tk_h] (table coordinates; fp64 from
+// the rows' hi + lo terms), then lane n < 7 forms coefficient n of the four polynomials; out[4][7] floats.
+//   r = table r + log2(1 + 2^(gk2 u - cpsi)) - beta2 u   (turnover taken out, -beta ln(1+z) of m2^beta folded in)
+__device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restrict__ tab, int K, double tk_c, double tk_h,
+                                          double z_ref, bool turn_on, const double* __restrict__ pm, float* __restrict__ out) {
+    const int lane = threadIdx.x & 31;
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
+    if (lane < kPolyN) {
+        const double tk = tk_c + tk_h * __ldg(pm + lane);
+        const int k = max(1, min((int)tk, K));
+        const float t = (float)(tk - (double)k);
+        const float4* r = reinterpret_cast<const float4*>(tab + k);
+        const float4 q0 = __ldg(r), q1 = __ldg(r + 1), q3 = __ldg(r + 3);
+        const double z = (double)q0.x + (double)fmaf(fmaf(fmaf(q1.x, t, q0.w), t, q0.z), t, q0.y);
+        const double rr = (double)fmaf(fmaf(q3.w, t, q3.z), t, q3.y);
+        const double u = log1p(z);
+        const double turn = turn_on ? log2(1.0 + exp2(1.4426950408889634074 * L.gk * (u - L.ln1pzp))) : 0.0;
+        v0 = z - z_ref;
+        v1 = u;
+        v2 = 1.0 / (1.0 + z);
+        v3 = rr + turn - 1.4426950408889634074 * L.beta * u;
+    }
+    double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+    const int n = min(lane, kPolyN - 1);
+    const double* m7 = pm + kPolyN + n * kPolyN;
+    const double* m6 = m7 + kPolyN * kPolyN;
+#pragma unroll
+    for (int k = 0; k < kPolyN; ++k) {
+        const double a7 = __ldg(m7 + k), a6 = __ldg(m6 + k);
+        c0 = fma(a7, __shfl_sync(0xffffffffu, v0, k), c0);
+        c1 = fma(a6, __shfl_sync(0xffffffffu, v1, k), c1);
+        c2 = fma(a6, __shfl_sync(0xffffffffu, v2, k), c2);
+        c3 = fma(a7, __shfl_sync(0xffffffffu, v3, k), c3);
+    }
+    if (lane < kPolyN) {        // out: float2 zr[7] = (z_n, r_n), float2 ua[7] = (u_n, a_n)
+        out[2 * lane] = (float)c0;
+        out[2 * lane + 1] = (float)c3;
+        out[2 * kPolyN + 2 * lane] = (float)c1;
+        out[2 * kPolyN + 2 * lane + 1] = (float)c2;
+    }
+}
+
+// Steps S2 / S5 for one sample with the local polynomials: the same quantities as sample_eval.  Record
+// A = {t, m1d, m2d, ln m1d}, B = {ln m2d, log2(1/prior or 1/p_draw) - scale, .., ..}:
+//   m' = m^d a - m_low;  log2 w = LQ2(ln m1) + beta2 ln m2^d + r + B.y - 2 log2 m1' - log2(1 + 2^(gk2 u - cpsi)) - log2(1 + e^f(m2'))
+// PAPER.md:52, :195-198 eq. 20, :226 eq. 21, :75 eq. 11.  Warp-collective like sample_eval.
+template <bool kFit>
+__device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, const float cpsi, const PolyCoef& C, const float4 A,
+                                            const float2 Bq, const MassLookup& M, const float tm_lo, const float tm_hi,
+                                            float& zc, float& l2w) {
+    const f32x2 t2 = pack2(A.x, A.x);
+    f32x2 zr = C.zr[6], ua = C.ua[5];
+#pragma unroll
+    for (int n = 5; n >= 0; --n) zr = fma2(zr, t2, C.zr[n]);
+#pragma unroll
+    for (int n = 4; n >= 0; --n) ua = fma2(ua, t2, C.ua[n]);
+    float r, u, a, mp1, mp2;
+    unpack2(zr, zc, r);
+    unpack2(ua, u, a);
+    unpack2(fma2(pack2(A.y, A.z), pack2(a, a), pack2(-F.mlow_hi, -F.mlow_hi)), mp1, mp2);   // m' = m^d a - m_low
+    const float lm1 = A.w - u;
+    float tm = fmaf(lm1, F.tm_scale, F.mlow_tm);
+    tm = fminf(fmaxf(tm, tm_lo), tm_hi);
+    const float ti = (tm - 0.5f) + 12582912.f;
+    const int km = __float_as_int(ti) - 0x4B400000;
+    const float tf = tm - (ti - 12582912.f);
+    const bool gauss_only = mp1 > F.mhigh_p;
+    const int ks = km - M.lo;
+    float4 c;
+    if (kFit) {
+        c = M.s[ks + (gauss_only ? M.cap : 0)];
+    } else {
+        const bool staged = (unsigned)ks < (unsigned)M.cap;
+        c = M.s[(staged ? ks : 0) + (gauss_only ? M.cap : 0)];
+        if (__any_sync(0xffffffffu, !staged)) {
+            if (!staged) c = __ldg(M.g + km + (gauss_only ? M.n_mass + 2 : 0));
+        }
+    }
+    float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x);
+    l += fmaf(F.beta2, Bq.x, r + Bq.y);
+    l = fmaf(-2.f, lg2f(mp1), l);            // m1' <= 0 implies m2' <= 0: discarded below
+    l -= lg2f(1.0f + ex2f(fmaf(gk2, u, -cpsi)));   // overflow -> l = -inf, the limit (psi -> 0)
+    if (__any_sync(0xffffffffu, mp2 < F.delta)) {
+        const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
+        const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
+        const float ls = lg2f(1.0f + ex2f(f2));
+        l -= (mp2 < F.delta) ? ls : 0.f;
+    }
+    l2w = (mp2 > 0.f) ? l : -INFINITY;      // R15 support: m_low < m2
+}
+
 // ---- small reductions ---------------------------------------------------------------------------------
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -259,7 +404,8 @@ struct EventSetDev {
     const double* tk_c;         // [n_events]
     const double* tk_h;         // [n_events]
     const int64_t* poly_off;    // [n_events+1] offsets into prec (events padded to a multiple of 32 samples)
-    const float4* prec;         // records of the polynomial sweep: {t in [-1,1], m1d, m2d, ln m1d}, {ln m2d, log2(1/prior) - scale, 0, 0}
+    const float4* prec_a;       // records of the polynomial sweep: {t in [-1,1], m1d, m2d, ln m1d}
+    const float2* prec_b;       //                                  {ln m2d, log2(1/prior) - scale}
 };
 
 struct EventKernelParams {
@@ -276,6 +422,7 @@ struct EventKernelParams {
     unsigned long long* stats;  // [0] executed pairs (incl. band padding), [1] pairs inside the cut-off
     const double* ln_shift;  // [n_events] prior scale factored out of the weights, added back to log I
     const double* ln_qscale; // [n_events] ln of the event's largest q_g (qn = q / that), added back to log I
+    const float* poly;       // [n_lambda][n_events][4 kPolyN] event-local polynomials fitted by k_polyfit
     // diagnostics (single event, single lambda) -- null in the hot path
     int32_t dbg_event;       // >= 0: blockIdx.x addresses lambda only, event = dbg_event
     double* dbg_z; double* dbg_w; double* dbg_h; double* dbg_K;
@@ -286,6 +433,12 @@ struct InjSetDev {
     double n_inj_total;
     const float4* rec;       // packed injection records {A, B}, sorted by d_L
     const int64_t* perm;
+    // chunk-local polynomials (k_inject): records {t, m1d, m2d, ln m1d}, {ln m2d, log2(1/p_draw) - scale} padded to
+    // whole chunks, centre / half-width of each chunk in table coordinates (tk_h = 0: range too wide -> table path)
+    const float4* prec_a;
+    const float2* prec_b;
+    const double* tk_c;      // [n_chunks]
+    const double* tk_h;      // [n_chunks]
 };
 
 struct InjKernelParams {
@@ -295,6 +448,8 @@ struct InjKernelParams {
     double z_table_max, z_cat_max;
     double2* partial;        // [n_blocks][n_lambda] {sum s, sum s^2}
     uint32_t* flags;
+    const float* poly;       // [n_lambda][n_chunks][4 kPolyN] chunk-local polynomials fitted by k_polyfit
+    int32_t n_chunks;
     double* dbg_s;           // diagnostics: per-injection s_j (caller order), single lambda
     double dbg_scale;        // exp(ln_shift) to undo the draw-density scale in dbg_s
 };
@@ -312,13 +467,15 @@ struct CombineParams {
 cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P, LamConst* Lc, double* dc_tab,
                           Row* tab_ev, Row* tab_inj, MassRow* mtab, cudaStream_t st);
 
+cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int n_lambda, int n_ranges, const double* tk_c,
+                           const double* tk_h, const double* z_ref, double z_ref_const, bool is_inj, const double* pm,
+                           float* out, cudaStream_t st);
 cudaError_t launch_events(const EventKernelParams& P, bool count_pairs, cudaStream_t st);
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st);
 cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);
 cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, int64_t n, const double* dL,
                                 double z_table_max, double* z_out, double* r_out, cudaStream_t st);
 cudaError_t upload_gauss_legendre();   // fills the __constant__ node tables used by S1
-cudaError_t upload_poly_matrices();    // fills the __constant__ fit matrices of the event-local polynomials (k_events)
 cudaError_t measure_alu_peaks(int n_sm, int reps, cudaStream_t st, double out_g[4]);
 size_t events_smem_bytes(int max_ns, int max_nz);
 size_t tables_smem_bytes(const TableParams& P);

@@ -46,39 +46,6 @@ constexpr int kLeP = 12;                 // terms of the local expansion (degree
 constexpr int kLeMaxBox = 96;            // boxes per event the local-expansion form accepts
 constexpr float kLeMaxW = 1.3f;          // largest box width in units of sqrt(2) h (truncation error)
 
-// Event-local polynomials (S2): on an event whose samples span <= 0.9 in ln d_L, z - z0, ln(1+z), 1/(1+z) and the
-// smooth part of log2 of the redshift factor are polynomials in t in [-1, 1] (degree 6, 5, 5, 5; errors < 1e-8, 4e-8,
-// 6e-8 and 1e-8), fitted per (event, lambda) through 7 Chebyshev nodes read from the per-lambda z(ln d_L) table.
-constexpr int kPolyN = 7;
-__constant__ double c_poly_node[kPolyN];          // Chebyshev nodes cos(pi (k + 1/2) / 7)
-__constant__ double c_poly_m7[kPolyN][kPolyN];    // node values -> monomial coefficients, degree 6 (interpolation)
-__constant__ double c_poly_m6[kPolyN][kPolyN];    // node values -> monomial coefficients, degree 5 (discrete least squares; row 6 = 0)
-
-typedef unsigned long long f32x2;        // two packed floats (lo, hi) for the FFMA2 pipe
-__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
-    f32x2 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
-    f32x2 d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
-    f32x2 d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
-    f32x2 d;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-
 // ---- TMA bulk copy + mbarrier (one-shot: phase 0) ---------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
@@ -136,7 +103,7 @@ struct EvSmem {
     float scy, dy, yfirst;    // scale, grid spacing and first grid point in y
     int le_m, le_D, le_blo, le_nbox;   // grid points per box, half-width of the psi table, first box, number of boxes
     // event-local polynomials of S2 (use_poly != 0): z - z0 [7], ln(1+z) [7], 1/(1+z) [7], smooth log2 factor [7]
-    float poly[4 * kPolyN];
+    alignas(16) float poly[4 * kPolyN];
 };
 
 __host__ __device__ inline size_t ev_ns_pad(size_t ns) { return (ns + kPass - 1) / kPass * kPass; }
@@ -399,73 +366,35 @@ __device__ __forceinline__ float s2_sweep(const float4* __restrict__ rec, const 
     return mx;
 }
 
-// S2 sweep 1 with the event-local polynomials: the same quantities as sample_eval, per sample
-//   t from the record's fixed-point table coordinate; z - z0, u = ln(1+z), a = 1/(1+z), r by Horner;
-//   m' = m^d a - m_low;  log2 w = LQ2(ln m1) + beta2 ln m2^d + r + log2(1/prior) - 2 log2 m1' - log2(1 + 2^(gk2 u - cpsi))
-//                                 - log2(1 + e^f(m2'))      (r carries -beta2 u and everything of log2(psi/J) but the
-//   Madau-Dickinson turnover, whose poles sit too close to the real axis for a low-degree polynomial).
-// PAPER.md:52, :195-198 eq. 20, :226 eq. 21, :75 eq. 11.  Warp-collective like sample_eval.
+// S2 sweep 1 with the event-local polynomials (poly_sample, chim_internal.cuh): z_j - z0 and log2 w_j to shared memory.
 // kFit: every mass-table row the event can address is staged (the tm clamp keeps the index inside the stage).
 // All samples of an event on this path lie inside the table (use_poly), so there is no range check.
 template <bool kFit>
-__device__ __forceinline__ float s2_sweep_poly(const float4* __restrict__ prec, const LamF& Fs, const float* __restrict__ pc,
-                                               const MassLookup& M, int ns, float* __restrict__ zf, float* __restrict__ wl) {
+__device__ __forceinline__ float s2_sweep_poly(const float4* __restrict__ pa, const float2* __restrict__ pb, const LamF& Fs,
+                                               const float* __restrict__ pc, const MassLookup& M, int ns,
+                                               float* __restrict__ zf, float* __restrict__ wl) {
     float mx = -INFINITY;
     const int tid = threadIdx.x;
     const LamF F = Fs;
-    float cz[kPolyN], cu[kPolyN - 1], ca[kPolyN - 1], cr[kPolyN - 1];
-#pragma unroll
-    for (int n = 0; n < kPolyN; ++n) cz[n] = pc[n];
-#pragma unroll
-    for (int n = 0; n < kPolyN - 1; ++n) { cu[n] = pc[kPolyN + n]; ca[n] = pc[2 * kPolyN + n]; cr[n] = pc[3 * kPolyN + n]; }
+    PolyCoef C;
+    load_poly(C, pc);
     const int ns32 = (ns + 31) & ~31;                // the records are padded to ns32 with copies of the last sample
     // clamp of the mass-table coordinate: the table's range, and (kFit) the staged rows [M.lo, M.lo + M.cap)
     const float tm_lo = kFit ? fmaxf(1.0f, (float)M.lo) : 1.0f;
     const float tm_hi = kFit ? fminf(F.tm_max, (float)(M.lo + M.cap) - 0.01f) : F.tm_max;
-    const float4* p = prec + 2 * tid;
-    Rec R;
-    if (tid < ns32) R = ldg_stream_rec(p);
+    pa += tid;
+    pb += tid;
+    PRec R;
+    if (tid < ns32) R = ldg_stream_prec(pa, pb);
 #pragma unroll 2
     for (int j = tid; j < ns32; j += kEvThreads) {
-        const float4 A = R.A, Bq = R.B;
-        p += 2 * kEvThreads;
-        if (j + kEvThreads < ns32) R = ldg_stream_rec(p);
-        const float t = A.x;
-        float zc = cz[6], u = cu[5], a = ca[5], r = cr[5];
-#pragma unroll
-        for (int n = 5; n >= 0; --n) zc = fmaf(zc, t, cz[n]);
-#pragma unroll
-        for (int n = 4; n >= 0; --n) { u = fmaf(u, t, cu[n]); a = fmaf(a, t, ca[n]); r = fmaf(r, t, cr[n]); }
-        const float mp1 = fmaf(A.y, a, -F.mlow_hi) - F.mlow_lo, mp2 = fmaf(A.z, a, -F.mlow_hi) - F.mlow_lo;
-        const float lm1 = A.w - u;
-        float tm = fmaf(lm1, F.tm_scale, F.mlow_tm);
-        tm = fminf(fmaxf(tm, tm_lo), tm_hi);
-        const float ti = (tm - 0.5f) + 12582912.f;
-        const int km = __float_as_int(ti) - 0x4B400000;
-        const float tf = tm - (ti - 12582912.f);
-        const bool gauss_only = mp1 > F.mhigh_p;
-        const int ks = km - M.lo;
-        float4 c;
-        if (kFit) {
-            c = M.s[ks + (gauss_only ? M.cap : 0)];
-        } else {
-            const bool staged = (unsigned)ks < (unsigned)M.cap;
-            c = M.s[(staged ? ks : 0) + (gauss_only ? M.cap : 0)];
-            if (__any_sync(0xffffffffu, !staged)) {
-                if (!staged) c = __ldg(M.g + km + (gauss_only ? M.n_mass + 2 : 0));
-            }
-        }
-        float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x);
-        l += fmaf(F.beta2, Bq.x, r + Bq.y);
-        l = fmaf(-2.f, lg2f(fmaxf(mp1, 1e-30f)), l);
-        l -= lg2f(1.0f + ex2f(fminf(fmaf(F.gk2, u, -F.cpsi), 100.f)));
-        if (__any_sync(0xffffffffu, mp2 < F.delta)) {
-            const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
-            const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
-            const float ls = lg2f(1.0f + ex2f(f2));
-            l -= (mp2 < F.delta) ? ls : 0.f;
-        }
-        const float l2w = (mp2 > 0.f) ? l : -INFINITY;      // R15 support: m_low < m2
+        const float4 A = R.A;
+        const float2 Bq = R.B;
+        pa += kEvThreads;
+        pb += kEvThreads;
+        if (j + kEvThreads < ns32) R = ldg_stream_prec(pa, pb);
+        float zc, l2w;
+        poly_sample<kFit>(F, F.gk2, F.cpsi, C, A, Bq, M, tm_lo, tm_hi, zc, l2w);
         if (j < ns) {
             zf[j] = zc;
             wl[j] = l2w;
@@ -473,71 +402,6 @@ __device__ __forceinline__ float s2_sweep_poly(const float4* __restrict__ prec, 
         }
     }
     return mx;
-}
-
-// Fit of the event-local polynomials by one warp: lanes 0..6 read the table at the Chebyshev nodes of the event's
-// range (fp64 from the rows' hi + lo terms), then every lane n < 7 forms coefficient n of the four polynomials.
-__device__ __forceinline__ void fit_event_polys(const LamConst& L, const Row* __restrict__ tab, int K, double tk_c, double tk_h,
-                                                double z0, float* __restrict__ out) {
-    const int lane = threadIdx.x & 31;
-    double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
-    if (lane < kPolyN) {
-        const double tk = tk_c + tk_h * c_poly_node[lane];
-        const int k = max(1, min((int)tk, K));
-        const float t = (float)(tk - (double)k);
-        const float4* r = reinterpret_cast<const float4*>(tab + k);
-        const float4 q0 = __ldg(r), q1 = __ldg(r + 1), q3 = __ldg(r + 3);
-        const double z = (double)q0.x + (double)fmaf(fmaf(fmaf(q1.x, t, q0.w), t, q0.z), t, q0.y);
-        const double rr = (double)fmaf(fmaf(q3.w, t, q3.z), t, q3.y);
-        const double u = log1p(z);
-        const double turn = (L.F.gk2 != 0.f) ? log2(1.0 + exp2(1.4426950408889634074 * L.gk * (u - L.ln1pzp))) : 0.0;
-        v0 = z - z0;
-        v1 = u;
-        v2 = 1.0 / (1.0 + z);
-        v3 = rr + turn - 1.4426950408889634074 * L.beta * u;
-    }
-    double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
-    const int n = min(lane, kPolyN - 1);
-#pragma unroll
-    for (int k = 0; k < kPolyN; ++k) {
-        const double m7 = c_poly_m7[n][k], m6 = c_poly_m6[n][k];
-        c0 = fma(m7, __shfl_sync(0xffffffffu, v0, k), c0);
-        c1 = fma(m6, __shfl_sync(0xffffffffu, v1, k), c1);
-        c2 = fma(m6, __shfl_sync(0xffffffffu, v2, k), c2);
-        c3 = fma(m6, __shfl_sync(0xffffffffu, v3, k), c3);
-    }
-    if (lane < kPolyN) {
-        out[lane] = (float)c0;
-        out[kPolyN + lane] = (float)c1;
-        out[2 * kPolyN + lane] = (float)c2;
-        out[3 * kPolyN + lane] = (float)c3;
-    }
-}
-
-cudaError_t upload_poly_matrices() {
-    double node[kPolyN], A[kPolyN][kPolyN], C[kPolyN][kPolyN] = {}, m7[kPolyN][kPolyN], m6[kPolyN][kPolyN];
-    const double pi = 3.14159265358979323846;
-    for (int k = 0; k < kPolyN; ++k) node[k] = cos(pi * (k + 0.5) / kPolyN);
-    for (int m = 0; m < kPolyN; ++m)            // Chebyshev coefficient m from the node values (discrete orthogonality)
-        for (int k = 0; k < kPolyN; ++k) A[m][k] = (m == 0 ? 1.0 : 2.0) / kPolyN * cos(m * pi * (k + 0.5) / kPolyN);
-    C[0][0] = 1.0;                              // C[n][m]: coefficient of t^n in T_m
-    C[1][1] = 1.0;
-    for (int m = 2; m < kPolyN; ++m)
-        for (int n = 0; n < kPolyN; ++n) C[n][m] = (n > 0 ? 2.0 * C[n - 1][m - 1] : 0.0) - C[n][m - 2];
-    for (int n = 0; n < kPolyN; ++n)
-        for (int k = 0; k < kPolyN; ++k) {
-            double a7 = 0.0, a6 = 0.0;
-            for (int m = 0; m < kPolyN; ++m) {
-                a7 += C[n][m] * A[m][k];
-                if (m < kPolyN - 1) a6 += C[n][m] * A[m][k];
-            }
-            m7[n][k] = a7;
-            m6[n][k] = (n < kPolyN - 1) ? a6 : 0.0;
-        }
-    cudaError_t e = cudaMemcpyToSymbol(c_poly_node, node, sizeof node);
-    if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_poly_m7, m7, sizeof m7);
-    if (e == cudaSuccess) e = cudaMemcpyToSymbol(c_poly_m6, m6, sizeof m6);
-    return e;
 }
 
 // shared-memory layout after EvSmem: zf float[ns_pad] | wl float[ns_pad] | aux = staged table rows + mass rows (S2) / gq float2[nz_pad] (S3)
@@ -587,7 +451,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     // event-local polynomials (S2): narrow d_L range and every node inside the table
     const double tk_h = P.ev.tk_h[ev], tk_c = P.ev.tk_c[ev];
     const bool use_poly = tk_h > 0.0 && tk_c + tk_h < L.tkmax_ev;
-    if (use_poly && wid == 1) fit_event_polys(L, tab, P.tab_rows - 2, tk_c, tk_h, z0, S.poly);
+    if (use_poly && tid < 4 * kPolyN) S.poly[tid] = P.poly[((size_t)l * P.ev.n_events + ev) * (4 * kPolyN) + tid];   // fitted by k_polyfit
 
     // ---- TMA: the event's slice of the z(ln d_L) table and the mass-table rows it can address: ln m1 = ln m1d - ln(1+z),
     //      z between the event's first and last (sorted) sample; rows outside the staged range fall back to global
@@ -619,9 +483,9 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const float z0h = (float)z0, z0l = (float)(z0 - (double)z0h);
     float mx;
     const float4* rec = P.ev.rec + 2 * s0;
-    const float4* prec = P.ev.prec + 2 * P.ev.poly_off[ev];
-    if (use_poly && S.mass_fit) mx = s2_sweep_poly<true>(prec, L.F, S.poly, M, ns, zf, wl);
-    else if (use_poly) mx = s2_sweep_poly<false>(prec, L.F, S.poly, M, ns, zf, wl);
+    const int64_t p0 = P.ev.poly_off[ev];
+    if (use_poly && S.mass_fit) mx = s2_sweep_poly<true>(P.ev.prec_a + p0, P.ev.prec_b + p0, L.F, S.poly, M, ns, zf, wl);
+    else if (use_poly) mx = s2_sweep_poly<false>(P.ev.prec_a + p0, P.ev.prec_b + p0, L.F, S.poly, M, ns, zf, wl);
     else if (staged) mx = s2_sweep<true>(rec, L.F, rows_s, k_lo, M, ns, z0h, z0l, zf, wl);
     else mx = s2_sweep<false>(rec, L.F, reinterpret_cast<const float4*>(tab), 0, M, ns, z0h, z0l, zf, wl);
     // samples are sorted in d_L: one of them lies beyond the table iff the last one does

@@ -7,6 +7,8 @@
 //       flight share a chunk (lambda is the fast grid index), so the records come from L2.  Per (injection, lambda):
 //       log2 s_j = log2[p_m psi u / J / p_draw] via the same sample_eval() as the events (the injection table's r
 //       column carries psi u / J); z_j > z_cat_max gives s_j = 0 (R6; the comparison is made on hi + lo pairs).
+//       Chunks that span <= 0.9 in ln d_L (all of them for a dense set: it is sorted) replace the table rows by
+//       chunk-local polynomials fitted per (chunk, lambda) (fit_polys / poly_sample, chim_internal.cuh).
 //       s_j is widened to fp64 through the exponent field; per-CTA fp64 partial sums {sum s, sum s^2}, combined in a
 //       fixed order by S6 (deterministic).
 //   S6  log L = sum_i log I_i - N_e log xi, N_eff (eq. 13), flags.
@@ -24,6 +26,7 @@ struct InjSmem {
     LamConst L;
     double red[2 * (kInjThreads / 32)];
     unsigned long long mbar;
+    alignas(16) float poly[4 * kPolyN];   // chunk-local polynomials (chim_internal.cuh)
 };
 
 __device__ __forceinline__ uint32_t inj_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -68,7 +71,35 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
     const LamF& F = L.F;
     double acc[2] = {0.0, 0.0};
     int oor = 0;
-    if (L.flags == 0) {
+    const double tk_h = P.inj.tk_h[chunk], tk_c = P.inj.tk_c[chunk];
+    const bool use_poly = L.flags == 0 && tk_h > 0.0 && tk_c + tk_h < L.tkmax_inj && !P.dbg_s;
+    if (use_poly) {
+        // chunk-local polynomials: the chunk's (sorted) injections span a narrow range of ln d_L; z is taken relative to
+        // z_cat_max, so the support cut of R6 is the sign of the polynomial
+        if (tid < 4 * kPolyN) S.poly[tid] = P.poly[((size_t)l * P.n_chunks + chunk) * (4 * kPolyN) + tid];   // fitted by k_polyfit
+        __syncthreads();
+        PolyCoef C;
+        load_poly(C, S.poly);
+        const float4* pa = P.inj.prec_a + j0 + tid;          // padded to whole chunks with copies of the last injection
+        const float2* pb = P.inj.prec_b + j0 + tid;
+        const int n = (int)(j1 - j0), n32 = (n + 31) & ~31;
+        const float tm_hi = F.tm_max;
+        PRec R;
+        if (tid < n32) R = ldg_stream_prec(pa, pb);
+#pragma unroll 2
+        for (int j = tid; j < n32; j += kInjThreads) {
+            const float4 A = R.A;
+            const float2 Bq = R.B;
+            pa += kInjThreads;
+            pb += kInjThreads;
+            if (j + kInjThreads < n32) R = ldg_stream_prec(pa, pb);
+            float zc, l2w;
+            poly_sample<true>(F, F.gk2_inj, F.cpsi_inj, C, A, Bq, M, 1.0f, tm_hi, zc, l2w);
+            const double s = (zc <= 0.f && j < n) ? ex2_to_double(l2w) : 0.0;
+            acc[0] += s;
+            acc[1] = fma(s, s, acc[1]);
+        }
+    } else if (L.flags == 0) {
         const float4* rows = reinterpret_cast<const float4*>(P.tab + (size_t)l * P.tab_rows);
         const int64_t j1w = j0 + ((j1 - j0 + 31) & ~(int64_t)31);    // whole warps stay in the loop (sample_eval votes)
         Rec R = ldg_stream_rec(P.inj.rec + 2 * min(j0 + tid, j1 - 1));

@@ -455,6 +455,7 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         if (P.placement == CHIM_ON_SAMPLES) { F.gk2 = (float)(L.gk * l2e); F.cpsi = (float)(L.gk * l2e * L.ln1pzp); }
         else { F.gk2 = 0.f; F.cpsi = 100.f; }
         F.mlow_tm = (float)(1.0 - L.lm0 * L.inv_dlm);
+        F.gk2_inj = (float)(L.gk * l2e); F.cpsi_inj = (float)(L.gk * l2e * L.ln1pzp);
         F.tkmax_ev_q = (L.tkmax_ev >= 4095.9) ? 0xFFFFFFFFu : (L.tkmax_ev <= 0.0 ? 0u : (uint32_t)(L.tkmax_ev * (double)(1u << kTkFracBits)));
     }
     __syncthreads();
@@ -485,6 +486,34 @@ cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P,
 }
 
 // Diagnostics: evaluate the event table at arbitrary d_L (single lambda).
+// Local-polynomial fits for k_events (per (event, lambda)) and k_inject (per (chunk, lambda)): one warp per item.
+// out[(l * n_ranges + r) * 4 * kPolyN ..]; items whose range is too wide (tk_h = 0), beyond the table or whose lambda is
+// invalid are left untouched (the consumers test the same conditions and take the table path).
+__global__ void __launch_bounds__(256) k_polyfit(const LamConst* __restrict__ Lc, const Row* __restrict__ tab, int tab_rows,
+                                                 int n_lambda, int n_ranges, const double* __restrict__ tk_c,
+                                                 const double* __restrict__ tk_h, const double* __restrict__ z_ref,
+                                                 double z_ref_const, int is_inj, const double* __restrict__ pm,
+                                                 float* __restrict__ out) {
+    const long long item = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (item >= (long long)n_lambda * n_ranges) return;
+    const int l = (int)(item % n_lambda), r = (int)(item / n_lambda);
+    const LamConst& L = Lc[l];
+    const double h = tk_h[r], c = tk_c[r];
+    if (L.flags || !(h > 0.0) || !(c + h < (is_inj ? L.tkmax_inj : L.tkmax_ev))) return;
+    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, is_inj || L.F.gk2 != 0.f, pm,
+              out + ((size_t)l * n_ranges + r) * (4 * kPolyN));
+}
+
+cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int n_lambda, int n_ranges, const double* tk_c,
+                           const double* tk_h, const double* z_ref, double z_ref_const, bool is_inj, const double* pm,
+                           float* out, cudaStream_t st) {
+    const long long items = (long long)n_lambda * n_ranges;
+    if (items <= 0) return cudaSuccess;
+    k_polyfit<<<(unsigned)((items + 7) / 8), 256, 0, st>>>(Lc, tab, tab_rows, n_lambda, n_ranges, tk_c, tk_h, z_ref, z_ref_const,
+                                                            is_inj ? 1 : 0, pm, out);
+    return cudaGetLastError();
+}
+
 __global__ void k_table_lookup(const LamConst* __restrict__ Lc, const Row* __restrict__ tab, DlGrid g, int64_t n,
                                const double* __restrict__ dL, double z_table_max, double* __restrict__ z_out,
                                double* __restrict__ r_out) {

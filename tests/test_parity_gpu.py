@@ -134,6 +134,18 @@ def test_s5_injection_weights(P):
 
 
 # ---------------------------------------------------------------- T3: end to end
+def test_s5_dense_injection_set_takes_the_chunk_local_polynomials(P):
+    # 10^5 sorted injections: chunks of 8192 span < 0.9 in ln d_L and are evaluated with chunk-local polynomials
+    # (the sparse ends of the set still go through the table rows); log xi and N_eff against the oracle
+    w = make_workload("o5_spec", n_events=3, n_samples=600, n_grid=300, n_lambda=4, n_det=100_000)
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w)
+    rel, dtot, dxi = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    assert dxi < 1e-6                                   # N_e log xi is part of the 1e-3 total: 300 x 1e-6
+    assert np.max(np.abs(r["neff"] / ref["neff"] - 1.0)) < 1e-5
+
+
 def test_tiny_end_to_end(P):
     w = make_workload("tiny")
     ref = O.loglike_workload(w)
