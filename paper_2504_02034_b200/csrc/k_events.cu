@@ -177,35 +177,25 @@ struct LeSmem {
     float* qs;      // [nzp]  q_g (x grid factor for placement ON_GRID), 0 beyond the grid
     float* psi;     // [(D+1) * kLeP]
     float* Bc;      // [nbox * kLeP]
-    int* jst;       // [nbox + 1] first sample of each box (samples are sorted)
-    int* cpre;      // [nbox + 1] prefix sum of the 128-sample chunks per box
 };
 __host__ __device__ inline size_t le_bytes(size_t nzp, int D, int nbox) {
-    return 4 * nzp + 4 * (size_t)kLeP * (D + 1) + 4 * (size_t)kLeP * nbox + 8 * (size_t)(nbox + 1) + 64;
+    return 4 * nzp + 4 * (size_t)kLeP * (D + 1) + 4 * (size_t)kLeP * nbox + 64;
 }
 __device__ __forceinline__ LeSmem le_layout(unsigned char* aux, size_t nzp, int D, int nbox) {
     LeSmem M;
     M.qs = reinterpret_cast<float*>(aux);
     M.psi = M.qs + nzp;
     M.Bc = M.psi + (size_t)kLeP * (D + 1);
-    M.jst = reinterpret_cast<int*>(M.Bc + (size_t)kLeP * nbox);
-    M.cpre = M.jst + (nbox + 1);
     return M;
 }
 
-// Called by all threads after qs has been staged (and a barrier).  Returns this lane's sum_j w_j A_j.
-template <bool kStats>
-__device__ double le_phase(const EvSmem& S, const LeSmem& M, const float* __restrict__ zf, const float* __restrict__ wl,
-                           int ns, int nz, float Ty, unsigned long long& fma_ops, unsigned long long& pairs_cut) {
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const float scy = S.scy, dy = S.dy, yfirst = S.yfirst;
-    const int m = S.le_m, D = S.le_D, b_lo = S.le_blo, nbox = S.le_nbox;
-    const float wbox = (float)m * dy;
-    // (a) psi table: thread d computes psi_0..psi_{P-1} at t = d dy by the three-term recurrence
-    for (int d = tid; d <= D; d += kEvThreads) {
+// psi table of the local-expansion form: thread d computes psi_0..psi_{P-1} at t = d dy by the three-term recurrence
+// (threads from the top of the CTA, so that the warps staging q_g and the warps building psi overlap)
+__device__ __forceinline__ void le_psi_table(float* __restrict__ psi, int D, float dy) {
+    for (int d = kEvThreads - 1 - (int)threadIdx.x; d <= D; d += kEvThreads) {
         const float t = (float)d * dy, t2 = 2.f * t;
         float p0 = ex2f(-t * t * 1.44269504088896341f), p1 = t2 * p0;
-        float* o = M.psi + (size_t)d * kLeP;
+        float* o = psi + (size_t)d * kLeP;
         o[0] = p0;
         o[1] = p1;
 #pragma unroll
@@ -216,39 +206,17 @@ __device__ double le_phase(const EvSmem& S, const LeSmem& M, const float* __rest
             p1 = p2;
         }
     }
-    // (b) first sample of every box: y_j >= left edge of box b_lo + i  (binary search on the sorted samples)
-    for (int i = tid; i <= nbox; i += kEvThreads) {
-        int a = 0;
-        if (i == nbox) a = ns;
-        else if (i > 0) {
-            const float edge = fmaf((float)(b_lo + i) - 0.5f, wbox, yfirst);
-            int b = ns;
-            while (a < b) { const int mid = (a + b) >> 1; if (zf[mid] * scy < edge) a = mid + 1; else b = mid; }
-        }
-        M.jst[i] = a;
-    }
-    __syncthreads();
-    // chunk prefix (warp 0; 3 boxes per lane)
-    if (wid == 0) {
-        int c[3], tot = 0;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const int i = 3 * lane + k;
-            c[k] = (i < nbox) ? (M.jst[i + 1] - M.jst[i] + kPass - 1) / kPass : 0;
-            tot += c[k];
-        }
-        int inc = tot;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-        int ex = inc - tot;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const int i = 3 * lane + k;
-            if (i <= nbox) M.cpre[i] = ex;
-            ex += c[k];
-        }
-    }
-    // (c) coefficients: item = (box, quad of n, quarter of the d range); the four quarters sit in adjacent lanes
+}
+
+// Called by all threads after qs and psi have been staged (and a barrier).  Returns this lane's sum_j w_j A_j.
+template <bool kStats>
+__device__ double le_phase(const EvSmem& S, const LeSmem& M, const float* __restrict__ zf, const float* __restrict__ wl,
+                           int ns, int nz, float Ty, unsigned long long& fma_ops, unsigned long long& pairs_cut) {
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const float scy = S.scy, dy = S.dy, yfirst = S.yfirst;
+    const int m = S.le_m, D = S.le_D, b_lo = S.le_blo, nbox = S.le_nbox;
+    const float wbox = (float)m * dy;
+    // (b) coefficients: item = (box, quad of n, quarter of the d range); the four quarters sit in adjacent lanes
     const int H = D >> 1, n_items = nbox * 12;
     for (int base = 0; base < n_items; base += kEvThreads) {
         const int id = base + tid;
@@ -262,16 +230,33 @@ __device__ double le_phase(const EvSmem& S, const LeSmem& M, const float* __rest
         else { d0 = max(d0, -gc); d1 = min(d1, nz - 1 - gc); }
         if (!valid) d1 = d0 - 1;
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        const float* qp = M.qs + gc;
-        const float4* pp = reinterpret_cast<const float4*>(M.psi) + quad;
-#pragma unroll 2
-        for (int d = d0; d <= d1; ++d) {
-            const float q = qp[neg ? -d : d];
-            const float4 v = pp[d * (kLeP / 4)];
+        const float* qp = M.qs + gc + (neg ? -d0 : d0);
+        const int qstep = neg ? -1 : 1;
+        const float4* pp = reinterpret_cast<const float4*>(M.psi) + quad + d0 * (kLeP / 4);
+        int n = d1 - d0 + 1;
+#pragma unroll 1
+        for (; n >= 4; n -= 4) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const float q = qp[k * qstep];
+                const float4 v = pp[k * (kLeP / 4)];
+                acc.x = fmaf(q, v.x, acc.x);
+                acc.y = fmaf(q, v.y, acc.y);
+                acc.z = fmaf(q, v.z, acc.z);
+                acc.w = fmaf(q, v.w, acc.w);
+            }
+            qp += 4 * qstep;
+            pp += 4 * (kLeP / 4);
+        }
+        for (; n > 0; --n) {
+            const float q = *qp;
+            const float4 v = *pp;
             acc.x = fmaf(q, v.x, acc.x);
             acc.y = fmaf(q, v.y, acc.y);
             acc.z = fmaf(q, v.z, acc.z);
             acc.w = fmaf(q, v.w, acc.w);
+            qp += qstep;
+            pp += kLeP / 4;
         }
         if (neg) { acc.y = -acc.y; acc.w = -acc.w; }   // psi_n(-t) = (-1)^n psi_n(t); n = 4 quad + {0,1,2,3}
 #pragma unroll
@@ -285,42 +270,53 @@ __device__ double le_phase(const EvSmem& S, const LeSmem& M, const float* __rest
         if (kStats && valid) fma_ops += 4ull * (unsigned long long)max(0, d1 - d0 + 1);
     }
     __syncthreads();
-    // (d) evaluation: chunk k (128 consecutive samples of one box) goes to warp k mod 8
-    const int n_chunks = M.cpre[nbox];
-    const float inv_dy = 1.0f / dy;
+    // (c) evaluation: a warp pass = 128 consecutive (sorted) samples, 4 per lane; the boxes the pass touches are visited in
+    //     turn (usually one or two), each lane keeping the value of the box its sample lies in
+    const float inv_w = 1.0f / wbox, inv_dy = 1.0f / dy;
+    const int n_pass = (ns + kPass - 1) / kPass;
     double lsum = 0.0;
-    int i = 0;
-    for (int k = wid; k < n_chunks; k += kEvThreads / 32) {
-        while (M.cpre[i + 1] <= k) ++i;
-        const int j_end = M.jst[i + 1], j0 = M.jst[i] + (k - M.cpre[i]) * kPass + lane;
-        const float c = fmaf((float)((b_lo + i) * m), dy, yfirst);
-        const float4* bp = reinterpret_cast<const float4*>(M.Bc) + i * (kLeP / 4);
-        const float4 c0 = bp[0], c1 = bp[1], c2 = bp[2];
-        float sv[4], wv[4];
+    for (int pass = wid; pass < n_pass; pass += kEvThreads / 32) {
+        const int j0 = pass * kPass + lane * 4;
+        const float4 zz = *reinterpret_cast<const float4*>(zf + j0);     // padded: idle slots repeat the last sample, w = 0
+        const float4 ww = *reinterpret_cast<const float4*>(wl + j0);
+        const float y[4] = {zz.x * scy, zz.y * scy, zz.z * scy, zz.w * scy};
+        int bx[4];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int j = j0 + 32 * r;
-            const bool ok = j < j_end;
-            sv[r] = ok ? fmaf(zf[j], scy, -c) : 0.f;
-            wv[r] = ok ? wl[j] : 0.f;
-        }
-        const f32x2 s01 = pack2(sv[0], sv[1]), s23 = pack2(sv[2], sv[3]);
-        f32x2 a01 = pack2(c2.w, c2.w), a23 = a01;
+        for (int r = 0; r < 4; ++r) bx[r] = min(max((int)floorf(fmaf(y[r] - yfirst, inv_w, 0.5f)) - b_lo, 0), nbox - 1);
+        // the samples are sorted (up to fp32 rounding, which at worst moves a sample to the neighbouring box, where the
+        // expansion is still valid): the pass spans the boxes of its first and last sample
+        const int bmin = __shfl_sync(0xffffffffu, bx[0], 0), bmax = __shfl_sync(0xffffffffu, bx[3], 31);
+        bx[0] = min(max(bx[0], bmin), bmax);
+        bx[3] = min(max(bx[3], bx[0]), bmax);
+        bx[1] = min(max(bx[1], bx[0]), bx[3]);
+        bx[2] = min(max(bx[2], bx[0]), bx[3]);
+        float A[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int i = bmin; i <= bmax; ++i) {
+            const bool mine = (bx[0] <= i) & (bx[3] >= i);               // sorted within the lane as well
+            if (!__any_sync(0xffffffffu, mine)) continue;                 // empty box inside the pass
+            const float c = fmaf((float)((b_lo + i) * m), dy, yfirst);
+            const float4* bp = reinterpret_cast<const float4*>(M.Bc) + i * (kLeP / 4);
+            const float4 c0 = bp[0], c1 = bp[1], c2 = bp[2];
+            const f32x2 s01 = pack2(y[0] - c, y[1] - c), s23 = pack2(y[2] - c, y[3] - c);
+            f32x2 a01 = pack2(c2.w, c2.w), a23 = a01;
 #define CHIM_LE_STEP(cf) { const f32x2 q_ = pack2(cf, cf); a01 = fma2(a01, s01, q_); a23 = fma2(a23, s23, q_); }
-        CHIM_LE_STEP(c2.z) CHIM_LE_STEP(c2.y) CHIM_LE_STEP(c2.x)
-        CHIM_LE_STEP(c1.w) CHIM_LE_STEP(c1.z) CHIM_LE_STEP(c1.y) CHIM_LE_STEP(c1.x)
-        CHIM_LE_STEP(c0.w) CHIM_LE_STEP(c0.z) CHIM_LE_STEP(c0.y) CHIM_LE_STEP(c0.x)
+            CHIM_LE_STEP(c2.z) CHIM_LE_STEP(c2.y) CHIM_LE_STEP(c2.x)
+            CHIM_LE_STEP(c1.w) CHIM_LE_STEP(c1.z) CHIM_LE_STEP(c1.y) CHIM_LE_STEP(c1.x)
+            CHIM_LE_STEP(c0.w) CHIM_LE_STEP(c0.z) CHIM_LE_STEP(c0.y) CHIM_LE_STEP(c0.x)
 #undef CHIM_LE_STEP
-        float A[4];
-        unpack2(a01, A[0], A[1]);
-        unpack2(a23, A[2], A[3]);
-        lsum += (double)fmaf(wv[0], A[0], fmaf(wv[1], A[1], fmaf(wv[2], A[2], wv[3] * A[3])));
+            float v[4];
+            unpack2(a01, v[0], v[1]);
+            unpack2(a23, v[2], v[3]);
+#pragma unroll
+            for (int r = 0; r < 4; ++r) A[r] = (bx[r] == i) ? v[r] : A[r];
+        }
+        lsum += (double)fmaf(ww.x, A[0], fmaf(ww.y, A[1], fmaf(ww.z, A[2], ww.w * A[3])));
         if (kStats) {
+            const float wv[4] = {ww.x, ww.y, ww.z, ww.w};
 #pragma unroll
             for (int r = 0; r < 4; ++r)
                 if (wv[r] > 0.f) {
-                    const float y = sv[r] + c;
-                    const int a = max(0, (int)ceilf((y - Ty - yfirst) * inv_dy)), b = min(nz - 1, (int)floorf((y + Ty - yfirst) * inv_dy));
+                    const int a = max(0, (int)ceilf((y[r] - Ty - yfirst) * inv_dy)), b = min(nz - 1, (int)floorf((y[r] + Ty - yfirst) * inv_dy));
                     pairs_cut += (unsigned long long)max(0, b - a + 1);
                     fma_ops += kLeP;
                 }
@@ -563,7 +559,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         } else {   // Scott on the weighted sample (R3, O7)
             double s2 = mom[1] / (sw * sw), zb = mom[2] / sw;
             double var = (mom[3] / sw - zb * zb) / (1.0 - s2);
-            h = (1.0 - s2 > 0.0 && var > 0.0) ? sqrt(var) * exp(0.2 * log(s2)) : NAN;   // n_eff^(-1/5) = s2^(1/5)
+            h = (1.0 - s2 > 0.0 && var > 0.0) ? sqrt(var) * (double)exp2f(0.2f * log2f((float)s2)) : NAN;   // n_eff^(-1/5) = s2^(1/5); fp32: dh/h ~ 1e-7 moves log I by ~1e-9
         }
         if (P.dbg_h) *P.dbg_h = h;
         // scaled coordinates x = z' sqrt(log2(e)/2)/h: exp(-d^2/2h^2) = 2^(-dx^2)
@@ -622,6 +618,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             }
             LM.qs[g] = q;
         }
+        le_psi_table(LM.psi, S.le_D, S.dy);
     } else if (Bsel && !on_grid) {   // power form: q'_g = q_g 2^(-(b delta)^2), b = g mod B, duplicated for the packed FMA
         for (int g = tid; g < nzp; g += kEvThreads) {   // (the barriers above fenced the last reads of the staged tables)
             const float bd = (float)(g & (Bsel - 1)) * delta;
