@@ -233,6 +233,21 @@ def run_ours(args):
             pairs_cut += cst["kde_pairs_in_cutoff"]
         alu = cctx.alu_peaks()
         cctx.close()
+    # ---- S2 alone (CHIM_KDE_NONE: the same kernel with the KDE phase skipped), to split the fused kernel's time ------
+    ev_ms_s2 = None
+    if rank == 0:
+        sctx = pkg.Context(device=local, stream=stream, z_cat_max=w.z_cat_max, kde_cutoff=args.cutoff,
+                           lambda_chunk=args.lambda_chunk, kde_method=pkg.CHIM_KDE_NONE)
+        sctx.init_events(w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal)
+        sout = sctx.alloc_outputs(w.n_lambda, event_logI=False)
+        sctx.loglike_batch(lam_dev[0], out=sout)
+        sctx.set_profiling(True)
+        ev_ms_s2 = 0.0
+        for i in range(K):
+            flush.fill_(i & 0xFF)
+            sctx.loglike_batch(lam_dev[W + i], out=sout)
+            ev_ms_s2 += sctx.kernel_times()["events_ms"]
+        sctx.close()
 
     # ---- end-to-end arm: host buffers through chim_loglike_batch_host -----------------------------------
     lam_pin = [torch.as_tensor(l).contiguous().pin_memory() for l in lams[W:W + K]]
@@ -296,6 +311,12 @@ def run_ours(args):
                          "traffic": None, "algorithmic_ops_per_launch": pairs_cut / n_launch,
                          "executed_ops_per_launch": pairs_eval / n_launch,
                          "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
+                         "kde_phase": (None if ev_ms_s2 is None else {
+                             "what": "k_events timed again with the KDE phase skipped (CHIM_KDE_NONE); the difference is S3+S4",
+                             "s2_only_ms_per_launch": ev_ms_s2 / n_launch,
+                             "kde_ms_per_launch": (ktimes["events_ms"] - ev_ms_s2) / n_launch,
+                             "achieved": pairs_cut / max((ktimes["events_ms"] - ev_ms_s2) / 1e3, 1e-9) / 1e9,
+                             "frac": pairs_cut / max((ktimes["events_ms"] - ev_ms_s2) / 1e3, 1e-9) / 1e9 / peak_g}),
                          "measured_alu_peaks_gops": alu,
                          "peak_source": f"148 SM x 128 fp32 FMA lanes/clk x {clk_max:.0f} MHz ({peak_src} sm_max_mhz); "
                                         "achieved = pairs inside the t*h cut-off / k_events device time (which also holds S2, S4); "

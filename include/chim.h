@@ -57,11 +57,14 @@ typedef enum chim_status {
 enum { CHIM_MEM_HOST = 0, CHIM_MEM_DEVICE = 1 };   /* where the pointers given to chim_init_* live     */
 enum { CHIM_ON_SAMPLES = 0, CHIM_ON_GRID = 1 };    /* placement of psi/J (R1): N = per-sample weights  */
 enum { CHIM_BW_SCOTT = 0, CHIM_BW_FIXED = 1 };     /* KDE bandwidth rule (R3)                          */
-enum { CHIM_KDE_AUTO = 0, CHIM_KDE_DIRECT = 1, CHIM_KDE_POWER = 2 };
+enum { CHIM_KDE_AUTO = 0, CHIM_KDE_DIRECT = 1, CHIM_KDE_POWER = 2, CHIM_KDE_NONE = 3 };
                                                    /* KDE formulation.  AUTO: on equally spaced grids
                                                       the local-expansion form, else (or where it does not fit) the power
                                                       form, else the direct form; DIRECT: one MUFU.EX2 per pair on every
-                                                      grid; POWER: as AUTO without the local-expansion form              */
+                                                      grid; POWER: as AUTO without the local-expansion form; NONE
+                                                      (diagnostic): S3/S4 skipped, I_i = mean sample weight, i.e. the
+                                                      integral against a flat p_gal = 1 on an unbounded grid -- times
+                                                      S2 alone and serves as a closed-form check                          */
 
 /* per-lambda flag bits written to out_flags */
 #define CHIM_FLAG_LAMBDA_DOMAIN 1u   /* H0<=0, Om not in (0,1], Xi0<=0, delta_m<=0, sigma_g<=0, lambda_g not in
@@ -89,7 +92,7 @@ typedef struct chim_config {
     int32_t n_win_table; /* panels of the per-lambda window table of int m^beta S(m) dm (M4)                   */
     int32_t lambda_chunk;/* lambdas processed per internal pass (bounds the per-lambda table memory)           */
     double neff_factor;  /* NEFF_LOW is raised if N_eff < neff_factor * N_events (R8)                          */
-    int32_t kde_method;  /* CHIM_KDE_AUTO (default) | CHIM_KDE_DIRECT | CHIM_KDE_POWER                                   */
+    int32_t kde_method;  /* CHIM_KDE_AUTO (default) | CHIM_KDE_DIRECT | CHIM_KDE_POWER | CHIM_KDE_NONE                              */
     int32_t n_mass_table;/* intervals of the per-lambda mass table in ln m1                           */
     int32_t count_pairs; /* 1: the KDE kernel also counts its (sample, grid point) pairs for chim_get_stats (slower)     */
 } chim_config;

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CHIM_MEM_HOST, CHIM_MEM_DEVICE = 0, 1
 CHIM_ON_SAMPLES, CHIM_ON_GRID = 0, 1
 CHIM_BW_SCOTT, CHIM_BW_FIXED = 0, 1
-CHIM_KDE_AUTO, CHIM_KDE_DIRECT, CHIM_KDE_POWER = 0, 1, 2
+CHIM_KDE_AUTO, CHIM_KDE_DIRECT, CHIM_KDE_POWER, CHIM_KDE_NONE = 0, 1, 2, 3
 CHIM_FLAG_LAMBDA_DOMAIN, CHIM_FLAG_DL_NONMONOTONE, CHIM_FLAG_EVENT_ZERO, CHIM_FLAG_XI_ZERO = 1, 2, 4, 8
 CHIM_FLAG_NEFF_LOW, CHIM_FLAG_TABLE_RANGE, CHIM_FLAG_BW_DEGENERATE = 16, 32, 64
 N_LAMBDA_PARAMS = 15

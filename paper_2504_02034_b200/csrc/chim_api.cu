@@ -318,7 +318,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     if (c.n_table < 16 || (c.n_dl_table != 0 && c.n_dl_table < 16) || c.n_dl_table > kMaxDlRows || c.n_win_table < 8 || c.n_mass_table < 64 || c.z_cat_max > c.z_table_max) return CHIM_EINVAL;
     if (c.placement != CHIM_ON_SAMPLES && c.placement != CHIM_ON_GRID) return CHIM_EINVAL;
     if (c.bw_rule != CHIM_BW_SCOTT && c.bw_rule != CHIM_BW_FIXED) return CHIM_EINVAL;
-    if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT && c.kde_method != CHIM_KDE_POWER) return CHIM_EINVAL;
+    if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT && c.kde_method != CHIM_KDE_POWER && c.kde_method != CHIM_KDE_NONE) return CHIM_EINVAL;
     if (c.mem != CHIM_MEM_HOST && c.mem != CHIM_MEM_DEVICE) return CHIM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device < 0 || c.device >= ndev) return CHIM_ECUDA;

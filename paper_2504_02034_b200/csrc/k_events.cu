@@ -1,23 +1,27 @@
 // k_events.cu -- steps S2 + S3 + S4 fused: one CTA per (event, lambda).
 //
-//   S2  per posterior sample: z_j from the per-lambda table, source masses, log2 of the population weight
-//       (sample_eval, chim_internal.cuh), all fp32 with hi + lo pairs where differences cancel.  The slice of the
-//       per-lambda z(ln d_L) table the event addresses and the matching slice of the mass table are brought into
-//       shared memory by TMA bulk copies (cp.async.bulk + mbarrier) issued by one thread; the packed sample records
-//       are streamed from L2 with coalesced 128-bit loads.  A second sweep over shared memory turns log2 w into
-//       w / max w and forms the weighted moments -> Scott bandwidth h (R3).  z_j and w_j never leave shared memory.
+//   S2  per posterior sample: z_j, source masses, log2 of the population weight, all fp32.
+//       Narrow events (samples spanning <= 0.9 in ln d_L; every BASELINE config): event-local polynomials in ln d_L fitted
+//       per (event, lambda) by k_polyfit (poly_sample, chim_internal.cuh); 24-byte records streamed from L2 with
+//       coalesced 128 + 64-bit loads, the event's slice of the per-lambda mass table staged by a TMA bulk copy.
+//       Wide events: the per-lambda z(ln d_L) table rows (sample_eval; rows staged by TMA when they fit, hi + lo pairs
+//       where differences cancel).  A second sweep over shared memory turns log2 w into w / max w and forms the weighted
+//       moments -> Scott bandwidth h (R3).  z_j and w_j never leave shared memory.
 //   S3+S4  I_i = sum_g q_g K(z_g) = (1/(N_s h sqrt(2 pi))) sum_j w_j A_j,  A_j = sum_g q_g exp(-(z_g - z_j)^2 / 2h^2),
 //       q_g = p_gal(z_g) x trapezoid weight (eq. 19 evaluated on the grid, eq. 14).
-//       Samples in lanes (4 per lane, 128 per warp pass, sorted in z), grid points streamed from shared memory;
-//       a pass visits the grid band within t*h of its samples (R9).  Two formulations of the Gaussian:
+//       Three formulations:
 //
-//       power form (equally spaced grid): with x = z sqrt(log2(e)/2)/h, delta the grid spacing in
-//       x, block start x_a, u = x_a - x_j and g = aB + b:
+//       local-expansion form (equally spaced grid; the default): A(y) is expanded about box centres
+//       placed on grid points -- Hermite generating function, 12 terms, one coefficient table per CTA -- and every
+//       sample costs one degree-11 polynomial (packed FFMA2) instead of ~2 t h / dz Gaussian pairs (le_phase).
+//
+//       power form (equally spaced grid; when the expansion does not fit): with x = z sqrt(log2(e)/2)/h, delta the
+//       grid spacing in x, block start x_a, u = x_a - x_j and g = aB + b:
 //           2^-(x_g - x_j)^2 = 2^(-u^2) * (2^(-2 delta u))^b * 2^(-b^2 delta^2)
 //       so per block of B grid points  sum_b q_g E_gj = e0 * sum_b q'_b s^b  with q'_b = q_g 2^(-b^2 delta^2)
 //       precomputed per CTA: a Horner polynomial in s -- ONE fp32 FMA per pair, issued as packed FFMA2 (two
-//       samples per instruction), and two MUFU.EX2 (e0, s) per sample and block.  Exact up to fp32 rounding
-//       (no recurrence across blocks: every block restarts from fresh exponentials).
+//       samples per instruction), and two MUFU.EX2 (e0, s) per sample and block.  Samples in lanes (4 per lane, 128 per
+//       warp pass, sorted in z); a pass visits the grid band within t*h of its samples (R9).
 //
 //       direct form (any grid; also bandwidths below ~3 grid spacings, no cut-off, diagnostics):
 //           A_j += q_g * ex2(-(x_g - x_j)^2)   FADD, FMUL, MUFU.EX2, FFMA per pair.
@@ -592,6 +596,15 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         }
     }
     __syncthreads();
+    if (P.kde_method == CHIM_KDE_NONE) {   // diagnostic: S3 skipped; flat p_gal on a wide grid: I = mean weight (pin P5)
+        if (tid == 0) {
+            double sw = 0.0;
+#pragma unroll
+            for (int k = 0; k < kEvThreads / 32; ++k) sw += S.red[k];
+            *out = log(sw / (double)ns) + (double)mx * 0.69314718055994530942 + P.ln_shift[ev];
+        }
+        return;
+    }
     const double h = S.h;
     if (!(h > 0.0) || !isfinite(h)) {
         if (tid == 0) {

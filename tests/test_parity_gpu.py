@@ -283,6 +283,17 @@ def test_kde_local_expansion_power_and_direct_forms_agree_with_the_oracle(P):
     assert np.max(np.abs(rp["event_logI"] - rd["event_logI"])) < 2e-6
 
 
+def test_kde_none_is_the_mean_sample_weight(P):
+    # CHIM_KDE_NONE (diagnostic, times S2 alone): I_i = (1/N_s) sum_j w_j -- the flat-p_gal limit of eq. 14 (pin P5)
+    w = make_workload("tiny", n_events=4, n_samples=700, n_grid=64, n_lambda=3, n_inj_draw=500)
+    r = _gpu(P, w, kde_method=P.CHIM_KDE_NONE, count_pairs=0)
+    for l in range(3):
+        for i in range(w.n_events):
+            s = slice(w.sample_off[i], w.sample_off[i + 1])
+            _, wo, _ = O.sample_weights(w.lam[l], w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s])
+            assert abs(r["event_logI"][l, i] - math.log(np.mean(wo))) < 2e-6
+
+
 def test_kde_nonuniform_grid_takes_the_direct_form(P):
     # R14: any strictly increasing grid; the trapezoid uses the true spacings
     w = make_workload("o5_spec", n_events=5, n_samples=1500, n_grid=400, n_lambda=6, n_det=3000)
