@@ -10,6 +10,7 @@ from . import build as _build
 
 PLACE_SAMPLES, PLACE_GRID = 0, 1
 BW_SCOTT, BW_FIXED = 0, 1
+KERNEL_GAUSS, KERNEL_EPANECHNIKOV = 0, 1
 F_LAMBDA_DOMAIN, F_DL_NONMONOTONE, F_EVENT_ZERO, F_XI_ZERO = 1, 2, 4, 8
 F_NEFF_LOW, F_TABLE_RANGE, F_BW_DEGENERATE = 16, 32, 64
 
@@ -129,13 +130,22 @@ def kde(z, w, h, zg):
     return K
 
 
+def kde_epanechnikov(z, w, h, zg):
+    """O8': Epanechnikov kernel with the same standard deviation h as the Gaussian one (h_E = sqrt(5) h, reading R19)."""
+    z, w, zg = _d(z), _d(w), _d(zg)
+    K = np.empty_like(zg)
+    lib().chimo_kde_epan(C.c_int(z.size), _p(z), _p(w), C.c_double(h), C.c_int(zg.size), _p(zg), _p(K))
+    return K
+
+
 def event_integral(lam, zg, K, pgal, placement=PLACE_SAMPLES):
     lam, zg, K, pgal = _lam(lam), _d(zg), _d(K), _d(pgal)
     return float(lib().chimo_event_integral(_p(lam), C.c_int(placement), C.c_int(zg.size), _p(zg), _p(K), _p(pgal)))
 
 
 def event_logI(lam, dl, m1d, m2d, ln_prior, zg, pgal, placement=PLACE_SAMPLES, bw_rule=BW_SCOTT,
-               fixed_bw=float("nan"), z_table_max=10.0):
+               fixed_bw=float("nan"), z_table_max=10.0, kernel=KERNEL_GAUSS):
+    lib().chimo_set_kernel(C.c_int(kernel))
     lam, dl, m1d, m2d, lp, zg, pgal = _lam(lam), _d(dl), _d(m1d), _d(m2d), _d(ln_prior), _d(zg), _d(pgal)
     h = C.c_double(0.0)
     fl = C.c_uint32(0)
@@ -163,8 +173,9 @@ def neff(sum_s, sum_s2, n_inj_total):
 
 def loglike_batch(lam, sample_off, dl, m1d, m2d, ln_prior, grid_off, zg, pgal, *, fixed_bw=None,
                   inj=None, n_inj_total=0, placement=PLACE_SAMPLES, bw_rule=BW_SCOTT, z_cat_max=1.5,
-                  z_table_max=10.0, n_table=2048, neff_factor=5.0):
+                  z_table_max=10.0, n_table=2048, neff_factor=5.0, kernel=KERNEL_GAUSS):
     """inj = (dL, m1d, m2d, ln_pdraw) of the detected set or None.  Returns a dict of arrays."""
+    lib().chimo_set_kernel(C.c_int(kernel))
     lam = np.atleast_2d(_lam(lam))
     nl = lam.shape[0]
     so = np.ascontiguousarray(sample_off, dtype=np.int64)

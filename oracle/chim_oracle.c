@@ -394,6 +394,25 @@ void chimo_kde(int n, const double *z, const double *w, double h, int ng, const 
     }
 }
 
+/* O8' Epanechnikov variant ("Epanechnikov kernel", no formula given; reading R19 of DESIGN.md):
+ * K(z_g) = (1/N_s) sum_j w_j (3/(4 h_E)) max(0, 1 - ((z_g - z_j)/h_E)^2),  h_E = sqrt(5) h,
+ * so that the kernel has the same standard deviation h as the Gaussian one (the bandwidth rule is unchanged). */
+void chimo_kde_epan(int n, const double *z, const double *w, double h, int ng, const double *zg, double *K) {
+    double hE = sqrt(5.0) * h, norm = 0.75 / ((double)n * hE);
+    for (int g = 0; g < ng; ++g) {
+        long double s = 0.0L;
+        for (int j = 0; j < n; ++j) {
+            double u = (zg[g] - z[j]) / hE, k = 1.0 - u * u;
+            if (k > 0.0) s += w[j] * k;
+        }
+        K[g] = (double)s * norm;
+    }
+}
+
+static int chimo_kernel_kind = 0; /* 0 Gaussian (default), 1 Epanechnikov: selects O8 / O8' in chimo_event_logI */
+void chimo_set_kernel(int kind) { chimo_kernel_kind = kind; }
+int chimo_get_kernel(void) { return chimo_kernel_kind; }
+
 /* -------------------------------------------------------------------- O9 event integral ----- */
 /* I_i = composite trapezoid of y_g = K(z_g) G(z_g) p_gal(z_g) on the given grid (PAPER.md:97,
  * eq. 14 with N_pix = 1, R13).  G = 1 (placement N) or psi/J at the grid point (placement P). */
@@ -436,7 +455,8 @@ double chimo_event_logI(const double *lam, int placement, int bw_rule, double fi
             fl |= CHIMO_F_BW_DEGENERATE;
             logI = NAN;
         } else {
-            chimo_kde(ns, z, w, h, ng, zg, K);
+            if (chimo_kernel_kind == 1) chimo_kde_epan(ns, z, w, h, ng, zg, K);
+            else chimo_kde(ns, z, w, h, ng, zg, K);
             double I = chimo_event_integral(lam, placement, ng, zg, K, pgal);
             if (I > 0.0) logI = log(I);
             else { fl |= CHIMO_F_EVENT_ZERO; logI = -INFINITY; }

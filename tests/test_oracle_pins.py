@@ -418,6 +418,55 @@ def test_p11_trapezoid_against_simpson_on_refined_grid():
     assert abs(I / Is - 1) < 1e-9
 
 
+# ------------------------------------------------------------------ Epanechnikov variant (NEXT-2; reading R19)
+def test_epanechnikov_single_sample_shape_mass_and_variance():
+    # one sample: K(z) = w (3/(4 hE)) (1 - u^2) on |u| <= 1, hE = sqrt(5) h: integrates to w, variance h^2 (R19), support 2 hE
+    z0, w0, h = 0.5, 2.0, 0.02
+    hE = math.sqrt(5.0) * h
+    zg = np.array([z0, z0 + 0.5 * hE, z0 - 0.5 * hE, z0 + hE, z0 + 1.0001 * hE, z0 - 3 * hE])
+    K = O.kde_epanechnikov(np.array([z0]), np.array([w0]), h, zg)
+    assert np.allclose(K[:3], w0 * 0.75 / hE * np.array([1.0, 0.75, 0.75]), rtol=1e-14)
+    assert abs(K[3]) < 1e-12 * K[0] and K[4] == 0.0 and K[5] == 0.0
+    mass = integrate.quad(lambda x: O.kde_epanechnikov(np.array([z0]), np.array([w0]), h, np.array([x]))[0],
+                          z0 - hE, z0 + hE, epsabs=1e-13)[0]
+    var = integrate.quad(lambda x: (x - z0) ** 2 * O.kde_epanechnikov(np.array([z0]), np.array([w0]), h, np.array([x]))[0],
+                         z0 - hE, z0 + hE, epsabs=1e-15)[0] / mass
+    assert abs(mass - w0) < 1e-12 and abs(var / h ** 2 - 1) < 1e-10
+
+
+def test_epanechnikov_flat_p_gal_gives_mean_weight_and_brute_force():
+    # flat p_gal on a wide grid: I = (1/N_s) sum w_j up to the trapezoid error of a piecewise quadratic (O(dz^2/hE^2));
+    # and the grid sum against the hand-expanded double sum
+    rng = np.random.default_rng(5)
+    z, w = 0.6 + 0.03 * rng.standard_normal(40), rng.random(40)
+    h = 0.01
+    hE = math.sqrt(5.0) * h
+    zg = np.linspace(0.3, 0.9, 60001)
+    I = O.event_integral(lam(), zg, O.kde_epanechnikov(z, w, h, zg), np.ones_like(zg))
+    assert abs(I / np.mean(w) - 1) < 1e-6
+    zg2 = np.linspace(0.45, 0.75, 31)
+    K = O.kde_epanechnikov(z, w, h, zg2)
+    brute = [sum(wj * 0.75 / hE * max(0.0, 1 - ((g - zj) / hE) ** 2) for zj, wj in zip(z, w)) / 40 for g in zg2]
+    assert np.allclose(K, brute, rtol=1e-13, atol=1e-300)
+
+
+def test_epanechnikov_end_to_end_uses_the_same_bandwidth_rule():
+    # kernel=EPANECHNIKOV swaps O8 only: same z_j, w_j, h; log I from the Epanechnikov KDE on the event grid
+    w = make_workload("tiny", n_events=2, n_samples=200, n_grid=150, n_inj_draw=200)
+    la = w.lam[0]
+    rg = O.loglike_workload(w, lam=la)
+    re = O.loglike_workload(w, lam=la, kernel=O.KERNEL_EPANECHNIKOV)
+    assert np.array_equal(rg["h"], re["h"]) and rg["logxi"][0] == re["logxi"][0]
+    for i in range(2):
+        s, g = slice(w.sample_off[i], w.sample_off[i + 1]), slice(w.grid_off[i], w.grid_off[i + 1])
+        zj, wj, _ = O.sample_weights(la, w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s])
+        K = O.kde_epanechnikov(zj, wj, re["h"][0, i], w.z_grid[g])
+        I = O.event_integral(la, w.z_grid[g], K, w.p_gal[g])
+        assert abs(re["event_logI"][0, i] - math.log(I)) < 1e-13
+    assert np.max(np.abs(re["event_logI"] - rg["event_logI"])) < 0.5     # same estimator up to the kernel shape
+    O.loglike_workload(w, lam=la)                                        # (leaves the oracle on the Gaussian kernel)
+
+
 # ------------------------------------------------------------------ flags / degenerate cases
 def test_flags_and_degenerate_cases():
     w = make_workload("tiny", n_events=2, n_samples=50, n_grid=60, n_inj_draw=200)
