@@ -30,6 +30,7 @@ sys.path.insert(0, ROOT)
 METRIC = "event-likelihoods/sec (events x lambda) on the O5-spectroscopic workload"
 UNIT = "event-likelihoods/s"
 SM_COUNT = 148
+ORACLE_KERNEL = [0]           # oracle kernel id of the timed oracle legs (set from --kde-kernel)
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
@@ -121,7 +122,7 @@ def lambda_batches(w, n_batches, rank):
 def oracle_step(O, w, lam):
     inj = (w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw)
     return O.loglike_batch(lam, w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal, inj=inj,
-                           n_inj_total=w.n_inj_total, z_cat_max=w.z_cat_max)
+                           n_inj_total=w.n_inj_total, z_cat_max=w.z_cat_max, kernel=ORACLE_KERNEL[0])
 
 
 def run_reference(args):
@@ -154,7 +155,7 @@ def workload_config(w, args):
     nz = int(np.diff(w.grid_off).max())
     return {"workload": f"{w.name} (BASELINE.json configs[{w.meta['index']}]), catalog {w.meta['catalog']}",
             "n_events": int(w.n_events), "n_samples": ns, "n_grid": nz, "n_lambda_per_gpu": int(w.n_lambda),
-            "n_injections_detected": int(w.n_det), "n_injections_drawn": int(w.n_inj_total),
+            "n_injections_detected": int(w.n_det), "n_injections_drawn": int(w.n_inj_total), "kde_kernel": args.kde_kernel,
             "l2": "flushed between timed steps (256 MiB write)", "fresh_lambda_batch_per_step": True,
             "parallelism": f"lambda-sharded replicas x{args.gpus}, no data-path collective"}
 
@@ -178,8 +179,9 @@ def run_ours(args):
     K, W = args.steps, max(args.warmup, 3)
     lams = lambda_batches(w, K + W, rank)
     stream = torch.cuda.current_stream(dev)
+    kk = pkg.CHIM_KERNEL_EPANECHNIKOV if args.kde_kernel == "epanechnikov" else pkg.CHIM_KERNEL_GAUSS
     ctx = pkg.Context(device=local, stream=stream, z_cat_max=w.z_cat_max, kde_cutoff=args.cutoff,
-                      lambda_chunk=args.lambda_chunk)
+                      lambda_chunk=args.lambda_chunk, kde_kernel=kk)
     ctx.init_workload(w)                        # inputs resident in HBM from here on
     lam_dev = [torch.as_tensor(l, device=dev).contiguous() for l in lams]
     out = ctx.alloc_outputs(w.n_lambda, event_logI=False)
@@ -356,9 +358,12 @@ def main():
     ap.add_argument("--n-events", type=int, default=0, help="override (debug only; invalidates the number)")
     ap.add_argument("--n-det", type=int, default=0, help="override (debug only)")
     ap.add_argument("--n-lambda", type=int, default=0, help="override (debug only)")
+    ap.add_argument("--kde-kernel", default="gauss", choices=["gauss", "epanechnikov"],
+                    help="KDE kernel shape (the headline metric is quoted on gauss; epanechnikov is the NEXT-2 variant)")
     ap.add_argument("--cpu-lambdas", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    ORACLE_KERNEL[0] = 1 if args.kde_kernel == "epanechnikov" else 0
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -66,6 +66,13 @@ enum { CHIM_KDE_AUTO = 0, CHIM_KDE_DIRECT = 1, CHIM_KDE_POWER = 2, CHIM_KDE_NONE
                                                       integral against a flat p_gal = 1 on an unbounded grid -- times
                                                       S2 alone and serves as a closed-form check                          */
 
+enum { CHIM_KERNEL_GAUSS = 0, CHIM_KERNEL_EPANECHNIKOV = 1 };
+                                                   /* KDE kernel shape.  EPANECHNIKOV: K(u) = 3/4 (1 - u^2) on |u| <= 1 with
+                                                      u = (z - z_j)/h_E, h_E = sqrt(5) h: the same standard deviation h (and
+                                                      bandwidth rule) as the Gaussian kernel.  Exact on any grid through
+                                                      prefix sums of q_g, q_g z_g, q_g z_g^2 (no pair loop, no cut-off);
+                                                      kde_method and kde_cutoff are ignored; needs placement ON_SAMPLES     */
+
 /* per-lambda flag bits written to out_flags */
 #define CHIM_FLAG_LAMBDA_DOMAIN 1u   /* H0<=0, Om not in (0,1], Xi0<=0, delta_m<=0, sigma_g<=0, lambda_g not in
                                         [0,1], m_low<=0, m_high<=m_low, z_p<=-1, non-finite -> loglike = NaN    */
@@ -95,11 +102,12 @@ typedef struct chim_config {
     int32_t kde_method;  /* CHIM_KDE_AUTO (default) | CHIM_KDE_DIRECT | CHIM_KDE_POWER | CHIM_KDE_NONE                              */
     int32_t n_mass_table;/* intervals of the per-lambda mass table in ln m1                           */
     int32_t count_pairs; /* 1: the KDE kernel also counts its (sample, grid point) pairs for chim_get_stats (slower)     */
+    int32_t kde_kernel;  /* CHIM_KERNEL_GAUSS (default) | CHIM_KERNEL_EPANECHNIKOV (reading R19)        */
 } chim_config;
 
 /* Fills *cfg with the defaults: device 0, HOST, NULL stream, ON_SAMPLES, SCOTT, kde_cutoff 6.0,
  * z_cat_max 1.5, z_table_max 10, n_table 2048, n_dl_table 0 (auto), n_win_table 512, lambda_chunk 256,
- * neff_factor 5, kde_method AUTO, n_mass_table 2048, count_pairs 0. */
+ * neff_factor 5, kde_method AUTO, n_mass_table 2048, count_pairs 0, kde_kernel GAUSS. */
 void chim_default_config(chim_config *cfg);
 
 /* Creates a context on cfg->device.  cfg == NULL means chim_default_config.  *out is set to NULL on error
@@ -199,7 +207,8 @@ int chim_debug_table_lookup(chim_ctx *ctx, const double *lambda, int64_t n, cons
 int chim_debug_event_samples(chim_ctx *ctx, const double *lambda, int32_t event, double *z_out,
                              double *w_out);
 /* Steps S2-S4: bandwidth h (1 double), KDE on the event grid K_out [N_z] (no cut-off applied to the
- * returned K if kde_cutoff == 0; otherwise the skipped pairs are missing from it), and log I. */
+ * returned K if kde_cutoff == 0; otherwise the skipped pairs are missing from it), and log I.
+ * K_out is available for the Gaussian kernel only (NaN with CHIM_KERNEL_EPANECHNIKOV). */
 int chim_debug_event_kde(chim_ctx *ctx, const double *lambda, int32_t event, double *h_out, double *K_out,
                          double *logI_out);
 /* Step S5: per-injection s_j in the caller's order [n_det]. */

@@ -12,6 +12,7 @@ CHIM_MEM_HOST, CHIM_MEM_DEVICE = 0, 1
 CHIM_ON_SAMPLES, CHIM_ON_GRID = 0, 1
 CHIM_BW_SCOTT, CHIM_BW_FIXED = 0, 1
 CHIM_KDE_AUTO, CHIM_KDE_DIRECT, CHIM_KDE_POWER, CHIM_KDE_NONE = 0, 1, 2, 3
+CHIM_KERNEL_GAUSS, CHIM_KERNEL_EPANECHNIKOV = 0, 1
 CHIM_FLAG_LAMBDA_DOMAIN, CHIM_FLAG_DL_NONMONOTONE, CHIM_FLAG_EVENT_ZERO, CHIM_FLAG_XI_ZERO = 1, 2, 4, 8
 CHIM_FLAG_NEFF_LOW, CHIM_FLAG_TABLE_RANGE, CHIM_FLAG_BW_DEGENERATE = 16, 32, 64
 N_LAMBDA_PARAMS = 15
@@ -28,7 +29,8 @@ class ChimConfig(C.Structure):
                 ("bw_rule", C.c_int32), ("kde_cutoff", C.c_double), ("z_cat_max", C.c_double),
                 ("z_table_max", C.c_double), ("n_table", C.c_int32), ("n_dl_table", C.c_int32),
                 ("n_win_table", C.c_int32), ("lambda_chunk", C.c_int32), ("neff_factor", C.c_double),
-                ("kde_method", C.c_int32), ("n_mass_table", C.c_int32), ("count_pairs", C.c_int32)]
+                ("kde_method", C.c_int32), ("n_mass_table", C.c_int32), ("count_pairs", C.c_int32),
+                ("kde_kernel", C.c_int32)]
 
 
 class ChimStats(C.Structure):
@@ -175,7 +177,8 @@ class Context:
 
     def __init__(self, device=0, stream=None, placement=CHIM_ON_SAMPLES, bw_rule=CHIM_BW_SCOTT, kde_cutoff=None,
                  z_cat_max=None, z_table_max=None, n_table=None, n_dl_table=None, n_win_table=None,
-                 lambda_chunk=None, neff_factor=None, kde_method=None, n_mass_table=None, count_pairs=None):
+                 lambda_chunk=None, neff_factor=None, kde_method=None, n_mass_table=None, count_pairs=None,
+                 kde_kernel=None):
         import torch
         if not torch.cuda.is_available():
             raise ChimError(-3, "no CUDA device: libchim has no CPU fallback")
@@ -192,7 +195,7 @@ class Context:
         for k, v in dict(kde_cutoff=kde_cutoff, z_cat_max=z_cat_max, z_table_max=z_table_max, n_table=n_table,
                          n_dl_table=n_dl_table, n_win_table=n_win_table, lambda_chunk=lambda_chunk,
                          neff_factor=neff_factor, kde_method=kde_method, n_mass_table=n_mass_table,
-                         count_pairs=count_pairs).items():
+                         count_pairs=count_pairs, kde_kernel=kde_kernel).items():
             if v is not None:
                 setattr(cfg, k, v)
         self.cfg = cfg

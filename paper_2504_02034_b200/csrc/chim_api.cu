@@ -171,7 +171,7 @@ EventKernelParams event_params(const chim_ctx* ctx, int nl) {
     P.ev = ctx->ev;
     P.Lc = ctx->Lc; P.tab = ctx->tab_ev; P.mtab = ctx->mtab; P.dc_tab = ctx->dc_tab;
     P.n_lambda = nl; P.tab_rows = ctx->ev_grid.rows(); P.n_mass = ctx->cfg.n_mass_table; P.n_table = ctx->cfg.n_table;
-    P.placement = ctx->cfg.placement; P.bw_rule = ctx->cfg.bw_rule; P.kde_method = ctx->cfg.kde_method;
+    P.placement = ctx->cfg.placement; P.bw_rule = ctx->cfg.bw_rule; P.kde_method = ctx->cfg.kde_method; P.kde_kernel = ctx->cfg.kde_kernel;
     P.z_table_max = ctx->cfg.z_table_max; P.cutoff = ctx->cfg.kde_cutoff;
     P.logI = ctx->logI; P.flags = ctx->flags; P.stats = ctx->stats;
     P.ln_shift = ctx->ev_ln_shift;
@@ -293,6 +293,7 @@ void chim_default_config(chim_config* cfg) {
     cfg->kde_method = CHIM_KDE_AUTO;
     cfg->n_mass_table = 2048;
     cfg->count_pairs = 0;
+    cfg->kde_kernel = CHIM_KERNEL_GAUSS;
 }
 
 int chim_version(void) { return CHIM_VERSION; }
@@ -320,6 +321,8 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     if (c.bw_rule != CHIM_BW_SCOTT && c.bw_rule != CHIM_BW_FIXED) return CHIM_EINVAL;
     if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT && c.kde_method != CHIM_KDE_POWER && c.kde_method != CHIM_KDE_NONE) return CHIM_EINVAL;
     if (c.mem != CHIM_MEM_HOST && c.mem != CHIM_MEM_DEVICE) return CHIM_EINVAL;
+    if (c.kde_kernel != CHIM_KERNEL_GAUSS && c.kde_kernel != CHIM_KERNEL_EPANECHNIKOV) return CHIM_EINVAL;
+    if (c.kde_kernel == CHIM_KERNEL_EPANECHNIKOV && c.placement != CHIM_ON_SAMPLES) return CHIM_EINVAL;   // lambda-independent q_g needed
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device < 0 || c.device >= ndev) return CHIM_ECUDA;
     cudaDeviceProp prop;
@@ -417,6 +420,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     std::vector<int32_t> perm(NS);
     std::vector<double> zc(NG), qg(NG), z0(n_events), shift(n_events), qshift(n_events), udz(n_events);
     std::vector<float> qn(NG);
+    std::vector<double> ep0(NG + n_events), ep1(NG + n_events), ep2(NG + n_events);   // Epanechnikov prefix sums
     std::vector<double> lm_lo(n_events), lm_hi(n_events);
     std::vector<double> tk_c(n_events), tk_h(n_events);
     std::vector<uint32_t> tkq_c(n_events);
@@ -479,6 +483,16 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
         if (!(qmax > 0.0)) qmax = 1.0;
         qshift[i] = std::log(qmax);
         for (int g = 0; g < nz; ++g) qn[g0 + g] = (float)(qg[g0 + g] / qmax);
+        {
+            long double a0 = 0.0L, a1 = 0.0L, a2 = 0.0L;
+            const size_t e0 = (size_t)g0 + i;
+            ep0[e0] = ep1[e0] = ep2[e0] = 0.0;
+            for (int g = 0; g < nz; ++g) {
+                const long double q = qg[g0 + g] / qmax, zz = zc[g0 + g];
+                a0 += q; a1 += q * zz; a2 += q * zz * zz;
+                ep0[e0 + g + 1] = (double)a0; ep1[e0 + g + 1] = (double)a1; ep2[e0 + g + 1] = (double)a2;
+            }
+        }
         // equally spaced grid?  then the KDE pair loop may take the power form
         const double dz = (h_z[g0 + nz - 1] - h_z[g0]) / (nz - 1);
         bool uniform = true;
@@ -498,6 +512,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     CK(upload(ctx->owned_ev, &E.k_lo, k_lo)); CK(upload(ctx->owned_ev, &E.k_hi, k_hi));
     CK(upload(ctx->owned_ev, &E.perm, perm)); CK(upload(ctx->owned_ev, &E.zc, zc)); CK(upload(ctx->owned_ev, &E.qn, qn));
     CK(upload(ctx->owned_ev, &E.uni_dz, udz));
+    CK(upload(ctx->owned_ev, &E.ep_q0, ep0)); CK(upload(ctx->owned_ev, &E.ep_q1, ep1)); CK(upload(ctx->owned_ev, &E.ep_q2, ep2));
     CK(upload(ctx->owned_ev, &E.lnm1_lo, lm_lo)); CK(upload(ctx->owned_ev, &E.lnm1_hi, lm_hi));
     CK(upload(ctx->owned_ev, &E.z0, z0));
     CK(upload(ctx->owned_ev, &E.tk_c, tk_c)); CK(upload(ctx->owned_ev, &E.tk_h, tk_h));

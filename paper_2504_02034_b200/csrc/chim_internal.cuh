@@ -399,6 +399,9 @@ struct EventSetDev {
     const int32_t* k_lo;        // [n_events] first / last row of the z(ln d_L) table the event's samples address
     const int32_t* k_hi;
     const double* fixed_bw;     // [n_events] or null
+    // Epanechnikov kernel: prefix sums over the event grid (N_z + 1 entries per event, offset grid_off[i] + i) of
+    // q_g, q_g z'_g, q_g z'_g^2 (z' = z_g - z0, q as in qn but fp64)
+    const double* ep_q0; const double* ep_q1; const double* ep_q2;
     // event-local polynomials (k_events, S2): centre and half-width of the event's samples in table coordinates
     // (tk_h = 0: the event's d_L range is too wide for them), and the same centre / scale for the 12.20 fixed point
     const double* tk_c;         // [n_events]
@@ -415,7 +418,7 @@ struct EventKernelParams {
     const MassRow* mtab;     // [n_lambda][2][n_mass+2]
     const double* dc_tab;    // [n_lambda][n_table+1+kZPad] (placement ON_GRID only) or null
     int32_t n_lambda, tab_rows, n_mass, n_table;
-    int32_t placement, bw_rule, kde_method;
+    int32_t placement, bw_rule, kde_method, kde_kernel;
     double z_table_max, cutoff;
     double* logI;            // [n_lambda][n_events]
     uint32_t* flags;         // [n_lambda]

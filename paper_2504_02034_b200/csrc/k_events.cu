@@ -614,6 +614,49 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         if (P.dbg_K) for (int g = tid; g < nz; g += kEvThreads) P.dbg_K[g] = NAN;
         return;
     }
+    if (P.kde_kernel == CHIM_KERNEL_EPANECHNIKOV) {
+        // Epanechnikov kernel (R19), exact on any grid without a pair loop: with the prefix sums
+        // Q_k[g] = sum_{g' < g} q_g' z'^k over the event grid,
+        //   A_j = sum_{|z_g - z_j| <= hE} q_g (1 - (z_g - z_j)^2 / hE^2) = dQ0 - (dQ2 - 2 z_j dQ1 + z_j^2 dQ0) / hE^2
+        // over the index range [a, b] of the support; I = 3/(4 hE N_s) sum_j w_j A_j.  fp64 (the bracket cancels ~1e3).
+        // A grid point that rounding puts on the wrong side of the support edge contributes ~1e-16 (the kernel is 0 there).
+        const double hE = 2.2360679774997896964 * h, ihE2 = 1.0 / (hE * hE);
+        const double* q0 = P.ev.ep_q0 + g0 + ev;
+        const double* q1 = P.ev.ep_q1 + g0 + ev;
+        const double* q2 = P.ev.ep_q2 + g0 + ev;
+        const double zfirst = zc_g[0], idz = (udz > 0.0) ? 1.0 / udz : 0.0;
+        double lsum = 0.0;
+        for (int j = tid; j < ns; j += kEvThreads) {
+            const double zj = (double)zf[j], lo = zj - hE, hi = zj + hE;
+            int a, b;
+            if (udz > 0.0) {
+                a = (int)fmax(0.0, ceil((lo - zfirst) * idz));
+                b = (int)fmin((double)(nz - 1), floor((hi - zfirst) * idz));
+            } else {
+                int x = 0, y = nz;
+                while (x < y) { const int mid = (x + y) >> 1; if (zc_g[mid] < lo) x = mid + 1; else y = mid; }
+                a = x;
+                y = nz;
+                while (x < y) { const int mid = (x + y) >> 1; if (zc_g[mid] <= hi) x = mid + 1; else y = mid; }
+                b = x - 1;
+            }
+            if (b >= a) {
+                const double d0 = q0[b + 1] - q0[a], d1 = q1[b + 1] - q1[a], d2 = q2[b + 1] - q2[a];
+                const double A = d0 - (d2 - 2.0 * zj * d1 + zj * zj * d0) * ihE2;
+                lsum = fma((double)wl[j], fmax(A, 0.0), lsum);
+            }
+        }
+        double t1[1] = {lsum};
+        block_sum<kEvThreads, 1>(t1, S.red);
+        if (P.dbg_K) for (int g = tid; g < nz; g += kEvThreads) P.dbg_K[g] = NAN;
+        if (tid == 0) {
+            const double I = t1[0] * 0.75 / ((double)ns * hE);
+            if (I > 0.0) *out = log(I) + (double)mx * 0.69314718055994530942 + P.ln_shift[ev] + P.ln_qscale[ev];
+            else if (I == 0.0) { *out = -INFINITY; atomicOr(P.flags + l, CHIM_FLAG_EVENT_ZERO); }
+            else *out = NAN;
+        }
+        return;
+    }
     const float scf = S.scf, delta = S.delta, xfirst = S.xfirst;
     const int Bsel = S.Bsel;
     const int nzp = (int)ev_nz_pad(nz);

@@ -294,6 +294,41 @@ def test_kde_none_is_the_mean_sample_weight(P):
             assert abs(r["event_logI"][l, i] - math.log(np.mean(wo))) < 2e-6
 
 
+# ---------------------------------------------------------------- Epanechnikov kernel (NEXT-2; reading R19)
+@pytest.mark.parametrize("shape", ["o5", "tiny_fixed", "nonuniform"])
+def test_epanechnikov_kernel_matches_the_oracle(P, shape):
+    kw, okw = {}, {}
+    if shape == "o5":
+        w = make_workload("o5_spec", n_events=6, n_lambda=8, n_det=4000)
+    elif shape == "tiny_fixed":
+        w = make_workload("tiny", n_events=5, n_samples=333, n_grid=97, n_lambda=3, n_inj_draw=2000)
+        fb = np.array([0.002, 0.004, 0.008, 0.02, 0.0007])          # from below the grid spacing to many spacings
+        kw, okw = dict(fixed_bw=fb, bw_rule=O.BW_FIXED), dict(fixed_bw=fb, bw_rule=O.BW_FIXED)
+    else:
+        w = make_workload("o5_spec", n_events=4, n_samples=1500, n_grid=400, n_lambda=4, n_det=3000)
+        for i in range(w.n_events):
+            g = slice(w.grid_off[i], w.grid_off[i + 1])
+            lo, hi = w.z_grid[g][0], w.z_grid[g][-1]
+            t = np.linspace(0.0, 1.0, 400)
+            w.z_grid[g] = lo + (hi - lo) * (0.6 * t + 0.4 * t * t)
+    ref = O.loglike_workload(w, kernel=O.KERNEL_EPANECHNIKOV, **okw)
+    O.loglike_workload(w, lam=w.lam[:1], **okw)          # (leaves the oracle on the Gaussian kernel)
+    r = _gpu(P, w, kde_kernel=P.CHIM_KERNEL_EPANECHNIKOV, count_pairs=0, **kw)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    assert np.nanmax(np.abs(r["event_logI"] - ref["event_logI"])) < 2e-5
+    # the kernel shape matters: the Gaussian result differs
+    rg = _gpu(P, w, count_pairs=0, **kw)
+    assert np.nanmax(np.abs(rg["event_logI"] - r["event_logI"])) > 1e-4
+
+
+def test_epanechnikov_needs_placement_on_samples(P):
+    cfg = P.chim_default_config()
+    cfg.kde_kernel, cfg.placement = P.CHIM_KERNEL_EPANECHNIKOV, P.CHIM_ON_GRID
+    with pytest.raises(P.ChimError):
+        P.chim_create(cfg)
+
+
 def test_kde_nonuniform_grid_takes_the_direct_form(P):
     # R14: any strictly increasing grid; the trapezoid uses the true spacings
     w = make_workload("o5_spec", n_events=5, n_samples=1500, n_grid=400, n_lambda=6, n_det=3000)
