@@ -173,7 +173,7 @@ def neff(sum_s, sum_s2, n_inj_total):
 
 def loglike_batch(lam, sample_off, dl, m1d, m2d, ln_prior, grid_off, zg, pgal, *, fixed_bw=None,
                   inj=None, n_inj_total=0, placement=PLACE_SAMPLES, bw_rule=BW_SCOTT, z_cat_max=1.5,
-                  z_table_max=10.0, n_table=2048, neff_factor=5.0, kernel=KERNEL_GAUSS):
+                  z_table_max=10.0, n_table=2048, neff_factor=5.0, kernel=KERNEL_GAUSS, group_off=None, ln_factor=None):
     """inj = (dL, m1d, m2d, ln_pdraw) of the detected set or None.  Returns a dict of arrays."""
     lib().chimo_set_kernel(C.c_int(kernel))
     lam = np.atleast_2d(_lam(lam))
@@ -190,11 +190,19 @@ def loglike_batch(lam, sample_off, dl, m1d, m2d, ln_prior, grid_off, zg, pgal, *
         nd = i0.size
     out = dict(loglike=np.empty(nl), event_logI=np.empty((nl, ne)), logxi=np.empty(nl), neff=np.empty(nl),
                h=np.empty((nl, ne)), flags=np.zeros(nl, dtype=np.uint32))
-    lib().chimo_loglike_batch(
+    if group_off is not None:
+        gof = np.ascontiguousarray(group_off, dtype=np.int64)
+        lnf = _d(ln_factor)
+        assert gof[0] == 0 and gof[-1] == ne and lnf.size == ne
+        ng, gp, fp = gof.size - 1, gof.ctypes.data_as(_ip), _p(lnf)
+    else:
+        ng, gp, fp = 0, None, None
+    lib().chimo_loglike_batch_grouped(
         C.c_int(nl), _p(lam), C.c_int(placement), C.c_int(bw_rule), C.c_double(z_cat_max),
         C.c_double(z_table_max), C.c_int(n_table), C.c_double(neff_factor), C.c_int(ne),
         so.ctypes.data_as(_ip), _p(dl), _p(m1d), _p(m2d), _p(lp), go.ctypes.data_as(_ip), _p(zg), _p(pgal),
         _p(fb), C.c_int64(nd), C.c_double(float(n_inj_total)), _p(i0), _p(i1), _p(i2), _p(i3),
+        C.c_int(ng), gp, fp,
         _p(out["loglike"]), _p(out["event_logI"]), _p(out["logxi"]), _p(out["neff"]), _p(out["h"]),
         out["flags"].ctypes.data_as(C.POINTER(C.c_uint32)))
     return out
@@ -205,5 +213,8 @@ def loglike_workload(w, lam=None, **kw):
     lam = w.lam if lam is None else lam
     inj = (w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw) if w.n_det > 0 else None
     kw.setdefault("z_cat_max", w.z_cat_max)
+    if getattr(w, "group_off", None) is not None:
+        kw.setdefault("group_off", w.group_off)
+        kw.setdefault("ln_factor", w.ln_factor)
     return loglike_batch(lam, w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal,
                          inj=inj, n_inj_total=w.n_inj_total, **kw)

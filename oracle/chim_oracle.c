@@ -505,6 +505,17 @@ double chimo_neff(double sum_s, double sum_s2, double n_inj_total) {
 }
 
 /* ------------------------------------------------------------------------- O11 log L -------- */
+void chimo_loglike_batch_grouped(int n_lambda, const double *lam, int placement, int bw_rule,
+                         double z_cat_max, double z_table_max, int n_table, double neff_factor,
+                         int n_events, const int64_t *sample_off, const double *dl,
+                         const double *m1d, const double *m2d, const double *ln_prior,
+                         const int64_t *grid_off, const double *zg, const double *pgal,
+                         const double *fixed_bw, int64_t n_det, double n_inj_total,
+                         const double *inj_dl, const double *inj_m1d, const double *inj_m2d,
+                         const double *inj_ln_pdraw, int n_groups, const int64_t *group_off,
+                         const double *ln_factor, double *out_loglike, double *out_event_logI,
+                         double *out_logxi, double *out_neff, double *out_h, uint32_t *out_flags);
+
 /* log L = sum_i log I_i - N_e log xi   (eq. 3) for a batch of lambda.
  * event_lo/hi select a sub-range of events (for bounded timing samples); out arrays may be NULL. */
 void chimo_loglike_batch(int n_lambda, const double *lam, int placement, int bw_rule,
@@ -516,7 +527,30 @@ void chimo_loglike_batch(int n_lambda, const double *lam, int placement, int bw_
                          const double *inj_dl, const double *inj_m1d, const double *inj_m2d,
                          const double *inj_ln_pdraw, double *out_loglike, double *out_event_logI,
                          double *out_logxi, double *out_neff, double *out_h, uint32_t *out_flags) {
+    chimo_loglike_batch_grouped(n_lambda, lam, placement, bw_rule, z_cat_max, z_table_max, n_table, neff_factor,
+                                n_events, sample_off, dl, m1d, m2d, ln_prior, grid_off, zg, pgal, fixed_bw, n_det,
+                                n_inj_total, inj_dl, inj_m1d, inj_m2d, inj_ln_pdraw, 0, NULL, NULL, out_loglike,
+                                out_event_logI, out_logxi, out_neff, out_h, out_flags);
+}
+
+/* "many-1d" kernel (eq. 18; eq. 14's sum over pixels; reading R20 of DESIGN.md): the n_events
+ * entries are (event, pixel) SUB-events -- the N_k PE samples that fall in pixel k, the pixel's own grid and p_gal --
+ * and physical event g owns the sub-events [group_off[g], group_off[g+1]):
+ *     I_g = sum_k F_k I_k,   I_k = int KDE[{z_j | w_j}_{j in pixel k}](z) p_gal,k(z) dz  (O8-O9 per pixel, 1/N_k, own Scott h),
+ * F_k = exp(ln_factor[k]) the hyperparameter-independent factor of eq. 18 (2-d sky KDE at the pixel centre x pixel area).
+ * log L = sum_g log I_g - N_groups log xi.  n_groups = 0: every sub-event is its own event (single-1d). */
+void chimo_loglike_batch_grouped(int n_lambda, const double *lam, int placement, int bw_rule,
+                         double z_cat_max, double z_table_max, int n_table, double neff_factor,
+                         int n_events, const int64_t *sample_off, const double *dl,
+                         const double *m1d, const double *m2d, const double *ln_prior,
+                         const int64_t *grid_off, const double *zg, const double *pgal,
+                         const double *fixed_bw, int64_t n_det, double n_inj_total,
+                         const double *inj_dl, const double *inj_m1d, const double *inj_m2d,
+                         const double *inj_ln_pdraw, int n_groups, const int64_t *group_off,
+                         const double *ln_factor, double *out_loglike, double *out_event_logI,
+                         double *out_logxi, double *out_neff, double *out_h, uint32_t *out_flags) {
     gl_init();
+    const int n_phys = (n_groups > 0) ? n_groups : n_events;   /* N_obs of eq. 3 */
     for (int l = 0; l < n_lambda; ++l) {
         const double *la = lam + (size_t)l * CHIMO_NLAM;
         const lam_t *L = (const lam_t *)la;
@@ -548,8 +582,25 @@ void chimo_loglike_batch(int n_lambda, const double *lam, int placement, int bw_
             if (out_event_logI) out_event_logI[(size_t)l * n_events + i] = li[i];
             if (out_h) out_h[(size_t)l * n_events + i] = h;
         }
+        if (n_groups > 0) {   /* pixel sum of eq. 14 in log space; a pixel with I = 0 is not an empty event */
+            efl &= ~CHIMO_F_EVENT_ZERO;
+            for (int g = 0; g < n_groups; ++g) {
+                double mx = -INFINITY, acc = 0.0;
+                int nan = 0;
+                for (int64_t k = group_off[g]; k < group_off[g + 1]; ++k) {
+                    double v = li[k] + ln_factor[k];
+                    if (isnan(v)) nan = 1;
+                    else if (v > mx) mx = v;
+                }
+                if (nan) { total = NAN; continue; }
+                if (mx == -INFINITY) { efl |= CHIMO_F_EVENT_ZERO; total += -INFINITY; continue; }
+                for (int64_t k = group_off[g]; k < group_off[g + 1]; ++k) acc += exp(li[k] + ln_factor[k] - mx);
+                total += mx + log(acc);
+            }
+        } else {
+            for (int i = 0; i < n_events; ++i) total += li[i];
+        }
         fl |= efl;
-        for (int i = 0; i < n_events; ++i) total += li[i];
         free(li);
         if (n_det > 0) {
             double S1, S2;
@@ -562,8 +613,8 @@ void chimo_loglike_batch(int n_lambda, const double *lam, int placement, int bw_
             if (!(xi > 0.0)) { fl |= CHIMO_F_XI_ZERO; logxi = NAN; total = NAN; }
             else {
                 logxi = log(xi);
-                if (neff < neff_factor * n_events) fl |= CHIMO_F_NEFF_LOW; /* R8: report only */
-                total -= n_events * logxi;
+                if (neff < neff_factor * n_phys) fl |= CHIMO_F_NEFF_LOW; /* R8: report only */
+                total -= n_phys * logxi;
             }
         }
         out_loglike[l] = total;

@@ -8,7 +8,7 @@ import pytest
 from scipy import integrate, optimize, special
 
 import oracle as O
-from workloads import lambda_vector, make_workload
+from workloads import lambda_vector, make_workload, split_into_pixels
 
 C = 299792.458
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
@@ -465,6 +465,42 @@ def test_epanechnikov_end_to_end_uses_the_same_bandwidth_rule():
         assert abs(re["event_logI"][0, i] - math.log(I)) < 1e-13
     assert np.max(np.abs(re["event_logI"] - rg["event_logI"])) < 0.5     # same estimator up to the kernel shape
     O.loglike_workload(w, lam=la)                                        # (leaves the oracle on the Gaussian kernel)
+
+
+# ------------------------------------------------------------------ many-1d kernel (NEXT-1; eq. 18, reading R20)
+def test_many1d_singleton_groups_are_single1d():
+    w = make_workload("tiny", n_events=3, n_samples=120, n_grid=90, n_inj_draw=300)
+    r0 = O.loglike_workload(w)
+    r1 = O.loglike_workload(w, group_off=np.arange(4), ln_factor=np.zeros(3))
+    assert r1["loglike"][0] == r0["loglike"][0] and np.array_equal(r1["event_logI"], r0["event_logI"])
+
+
+def test_many1d_pixel_sum_is_logsumexp_of_the_pixel_integrals():
+    # I_g = sum_k F_k I_k (eq. 14's pixel sum with eq. 18's kernel): the total from the per-pixel log I of the same run
+    w = split_into_pixels(make_workload("tiny", n_events=3, n_samples=400, n_grid=120, n_inj_draw=300), n_pix=4)
+    r = O.loglike_workload(w)
+    tot = 0.0
+    for g in range(3):
+        k = slice(w.group_off[g], w.group_off[g + 1])
+        tot += math.log(np.sum(np.exp(w.ln_factor[k]) * np.exp(r["event_logI"][0, k])))
+    assert abs(r["loglike"][0] - (tot - 3 * r["logxi"][0])) < 1e-10
+    # a pixel without weight is not an empty event; an event whose pixels are all empty is
+    lam2 = w.lam[0].copy()
+    lam2[7], lam2[8] = 200.0, 300.0                                   # m_low above every source mass: all weights 0
+    r2 = O.loglike_batch(lam2, w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal,
+                         group_off=w.group_off, ln_factor=w.ln_factor)            # (no injections: xi would be 0 too)
+    assert r2["loglike"][0] == -np.inf and (r2["flags"][0] & O.F_EVENT_ZERO)
+
+
+def test_many1d_with_shared_p_gal_and_fixed_bandwidth_equals_single1d():
+    # pins the normalisation reading R20: per-pixel KDE divided by N_k, pixel factor N_k/N_s.  The KDE is linear in the
+    # samples, so with one p_gal for all pixels and one fixed h the pixel sum IS the single-1d integral.
+    w1 = make_workload("tiny", n_events=2, n_samples=500, n_grid=150, n_inj_draw=300)
+    wp = split_into_pixels(w1, n_pix=5, same_p_gal=True)
+    h = 0.01
+    r1 = O.loglike_workload(w1, bw_rule=O.BW_FIXED, fixed_bw=np.full(2, h))
+    rp = O.loglike_workload(wp, bw_rule=O.BW_FIXED, fixed_bw=np.full(10, h))
+    assert abs(rp["loglike"][0] - r1["loglike"][0]) < 1e-10
 
 
 # ------------------------------------------------------------------ flags / degenerate cases

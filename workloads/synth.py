@@ -142,6 +142,10 @@ class Workload:
     n_inj_total: int
     z_cat_max: float = Z_EVENT_MAX
     meta: Optional[Dict] = None
+    # "many-1d" kernel: the entries above are (event, pixel) sub-events; physical event g owns the
+    # sub-events [group_off[g], group_off[g+1]) and ln_factor[k] = ln of the hyperparameter-independent pixel factor
+    group_off: Optional[np.ndarray] = None
+    ln_factor: Optional[np.ndarray] = None
 
     @property
     def n_events(self):
@@ -304,3 +308,44 @@ def make_workload(name: str = "tiny", catalog: int = 0, *, n_events=None, n_samp
         inj_dL=inj[0], inj_m1d=inj[1], inj_m2d=inj[2], inj_ln_pdraw=inj[3],
         n_inj_total=int(inj[4]), meta=dict(cfg, catalog=catalog),
     )
+
+
+def split_into_pixels(w: Workload, n_pix: int = 8, rho: float = 0.4, min_samples: int = 24, same_p_gal: bool = False,
+                      seed_offset: int = 0) -> Workload:
+    """Stand-in for the paper's sky pixelisation (the sky posteriors are not in the container):
+    every event's samples are distributed over n_pix pixels of unequal population, with a sky coordinate correlated
+    (coefficient rho) with the sample's distance; each pixel keeps the event's grid and gets its own p_gal (the event's
+    one modulated smoothly along z, non-negative); the pixel factor is the fraction of the samples it holds (what a sky
+    KDE at the pixel centre times the pixel area estimates).  Returns a workload of sub-events with group_off / ln_factor."""
+    rng = np.random.default_rng(np.random.SeedSequence([w.seed, 77, seed_offset]))
+    so, dl, m1, m2, lp, go, zg, pg, lnf, goff = [0], [], [], [], [], [0], [], [], [], [0]
+    for i in range(w.n_events):
+        s = slice(w.sample_off[i], w.sample_off[i + 1])
+        g = slice(w.grid_off[i], w.grid_off[i + 1])
+        ns = s.stop - s.start
+        x = np.log(w.dL[s])
+        key = rho * (x - x.mean()) / (x.std() + 1e-300) + np.sqrt(1 - rho * rho) * rng.standard_normal(ns)
+        frac = rng.dirichlet(np.full(n_pix, 3.0))
+        cnt = np.maximum(min_samples, np.floor(frac * ns).astype(int))
+        while cnt.sum() > ns:
+            cnt[np.argmax(cnt)] -= 1
+        cnt[np.argmax(cnt)] += ns - cnt.sum()
+        order = np.argsort(key, kind="stable")
+        z = w.z_grid[g]
+        start = 0
+        for k in range(n_pix):
+            idx = np.sort(order[start:start + cnt[k]])          # keep the caller's sample order inside the pixel
+            start += cnt[k]
+            dl.append(w.dL[s][idx]); m1.append(w.m1d[s][idx]); m2.append(w.m2d[s][idx]); lp.append(w.ln_prior[s][idx])
+            so.append(so[-1] + idx.size)
+            zg.append(z)
+            mod = 1.0 if same_p_gal else 1.0 + 0.6 * np.cos(2 * np.pi * (k / n_pix + 3.0 * (z - z[0]) / (z[-1] - z[0])))
+            pg.append(w.p_gal[g] * mod)
+            go.append(go[-1] + z.size)
+            lnf.append(np.log(idx.size / ns))
+        goff.append(goff[-1] + n_pix)
+    return dataclasses.replace(
+        w, sample_off=np.array(so, dtype=np.int64), dL=np.concatenate(dl), m1d=np.concatenate(m1), m2d=np.concatenate(m2),
+        ln_prior=np.concatenate(lp), grid_off=np.array(go, dtype=np.int64), z_grid=np.concatenate(zg),
+        p_gal=np.concatenate(pg), group_off=np.array(goff, dtype=np.int64), ln_factor=np.array(lnf),
+        meta=dict(w.meta or {}, n_pix=n_pix))
