@@ -133,6 +133,21 @@ int chim_init_events(chim_ctx *ctx, int32_t n_events, const int64_t *sample_off,
                      const double *fixed_bw);
 
 /*
+ * "many-1d" kernel (eq. 18; the pixel sum of PAPER.md:97 eq. 14; reading R20).  Optional; call after
+ * chim_init_events.  The entries given to chim_init_events are then (event, pixel) SUB-events -- the PE samples that fall
+ * in pixel k, the pixel's own grid and p_gal -- and physical event g owns the sub-events [group_off[g], group_off[g+1]):
+ *     I_g = sum_k F_k I_k,  F_k = exp(ln_factor[k])   (the hyperparameter-independent factor of eq. 18: the 2-d sky
+ *                                                      KDE at the pixel centre times the pixel area)
+ *     loglike = sum_g log I_g - n_groups * log xi;  NEFF_LOW compares with neff_factor * n_groups
+ *   group_off [n_groups+1]: starts at 0, strictly increasing, ends at n_events (HOST or DEVICE per cfg.mem)
+ *   ln_factor [n_events]  : finite
+ * out_event_logI of chim_loglike_batch stays per sub-event.  A sub-event with I_k = 0 does not raise EVENT_ZERO; a group
+ * whose sub-events are all zero does (loglike = -inf).  n_groups == 0 removes the grouping (every sub-event is an
+ * event: the single-1d kernel); chim_init_events also removes it.
+ */
+int chim_set_event_groups(chim_ctx *ctx, int32_t n_groups, const int64_t *group_off, const double *ln_factor);
+
+/*
  * Detected injections for the selection term: n_det stored injections out of
  * n_inj_total drawn; ln_pdraw = ln of the draw density in (d_L, m1d, m2d) (R7).  Optional: without
  * injections log xi := 0 and loglike = sum_i log I_i.  n_det == 0 removes a previous set.

@@ -77,6 +77,7 @@ def lib():
     L.chim_version.restype = C.c_int
     L.chim_init_events.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 9
     L.chim_init_injections.argtypes = [C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 4
+    L.chim_set_event_groups.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.chim_loglike_batch.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_loglike_batch_host.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_get_stats.argtypes = [C.c_void_p, C.POINTER(ChimStats)]
@@ -137,6 +138,10 @@ def chim_last_error(ctx) -> str:
 def chim_init_events(ctx, n_events, sample_off, dL, m1d, m2d, ln_prior, grid_off, z_grid, p_gal, fixed_bw=None):
     _check(ctx, lib().chim_init_events(ctx, n_events, *[_addr(a) for a in (sample_off, dL, m1d, m2d, ln_prior,
                                                                            grid_off, z_grid, p_gal, fixed_bw)]))
+
+
+def chim_set_event_groups(ctx, n_groups, group_off, ln_factor):
+    _check(ctx, lib().chim_set_event_groups(ctx, n_groups, _addr(group_off), _addr(ln_factor)))
 
 
 def chim_init_injections(ctx, n_det, n_inj_total, dL, m1d, m2d, ln_pdraw):
@@ -226,6 +231,14 @@ class Context:
         self.n_events = len(so) - 1
         self._ns, self._nz = np.diff(so), np.diff(go)
 
+    def set_event_groups(self, group_off, ln_factor):
+        """many-1d: the loaded entries are (event, pixel) sub-events; None removes the grouping."""
+        if group_off is None:
+            chim_set_event_groups(self.h, 0, None, None)
+            return
+        go = np.ascontiguousarray(group_off, dtype=np.int64)
+        chim_set_event_groups(self.h, len(go) - 1, go, _f64(ln_factor))
+
     def init_injections(self, dL, m1d, m2d, ln_pdraw, n_inj_total):
         arrs = [_f64(a) for a in (dL, m1d, m2d, ln_pdraw)]
         chim_init_injections(self.h, arrs[0].size, int(n_inj_total), *arrs)
@@ -233,6 +246,8 @@ class Context:
 
     def init_workload(self, w, fixed_bw=None):
         self.init_events(w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal, fixed_bw)
+        if getattr(w, "group_off", None) is not None:
+            self.set_event_groups(w.group_off, w.ln_factor)
         if w.n_det > 0:
             self.init_injections(w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw, w.n_inj_total)
 

@@ -27,7 +27,9 @@ struct chim_ctx {
     chim_config cfg;
     cudaStream_t stream = nullptr;
     std::string err;
-    std::vector<void*> owned_ev, owned_inj, owned_work, owned_host, owned_ctx;
+    std::vector<void*> owned_ev, owned_inj, owned_work, owned_host, owned_ctx, owned_grp;
+    int n_groups = 0;                      // many-1d grouping of the sub-events (0 = none)
+    const int64_t* grp_off = nullptr; const double* grp_lnf = nullptr;
     const double* poly_mats = nullptr;     // fit matrices of the local polynomials (device)
     // events
     bool have_events = false;
@@ -232,6 +234,7 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
     CP.n_det = ctx->have_inj ? ctx->inj.n_det : 0;
     CP.n_inj_total = ctx->have_inj ? ctx->inj.n_inj_total : 1.0;
     CP.inj_ln_shift = ctx->inj_ln_shift;
+    CP.n_groups = ctx->n_groups; CP.group_off = ctx->grp_off; CP.ln_factor = ctx->grp_lnf;
     CP.neff_factor = ctx->cfg.neff_factor; CP.flags_in = ctx->flags;
     CP.out_loglike = out_ll; CP.out_event_logI = out_ev; CP.out_logxi = out_xi; CP.out_neff = out_neff; CP.out_flags = out_fl;
     { Bracket b(ctx, 3); CK(launch_combine(CP, st)); }
@@ -351,6 +354,7 @@ void chim_destroy(chim_ctx* ctx) {
     free_pool(ctx->owned_work);
     free_pool(ctx->owned_host);
     free_pool(ctx->owned_ctx);
+    free_pool(ctx->owned_grp);
     delete ctx;
 }
 
@@ -501,6 +505,9 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     }
     // replace the previous set
     cudaStreamSynchronize(ctx->stream);
+    free_pool(ctx->owned_grp);
+    ctx->n_groups = 0;
+    ctx->grp_off = nullptr; ctx->grp_lnf = nullptr;
     free_pool(ctx->owned_ev);
     free_pool(ctx->owned_work);
     ctx->work_nl = 0;
@@ -526,6 +533,35 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     ctx->h_sample_off = so;
     ctx->h_grid_off = go;
     ctx->have_events = true;
+    return CHIM_OK;
+}
+
+int chim_set_event_groups(chim_ctx* ctx, int32_t n_groups, const int64_t* group_off, const double* ln_factor) {
+    if (!ctx) return CHIM_EINVAL;
+    if (!ctx->have_events) return fail(ctx, CHIM_ESTATE, "chim_set_event_groups: call chim_init_events first");
+    CK(cudaSetDevice(ctx->cfg.device));
+    if (n_groups < 0 || (n_groups > 0 && (!group_off || !ln_factor)))
+        return fail(ctx, CHIM_EINVAL, "chim_set_event_groups: null pointer or n_groups < 0");
+    std::vector<int64_t> go;
+    std::vector<double> lf;
+    if (n_groups > 0) {
+        CK(fetch(ctx, group_off, (size_t)n_groups + 1, go));
+        CK(fetch(ctx, ln_factor, (size_t)ctx->ev.n_events, lf));
+        if (go[0] != 0 || go[n_groups] != ctx->ev.n_events)
+            return fail(ctx, CHIM_EINVAL, "chim_set_event_groups: group_off must start at 0 and end at n_events");
+        for (int g = 0; g < n_groups; ++g)
+            if (!(go[g + 1] > go[g])) return fail(ctx, CHIM_EINVAL, "chim_set_event_groups: group_off must be strictly increasing");
+        if (!all_finite(lf)) return fail(ctx, CHIM_EINVAL, "chim_set_event_groups: non-finite ln_factor");
+    }
+    cudaStreamSynchronize(ctx->stream);
+    free_pool(ctx->owned_grp);
+    ctx->n_groups = 0;
+    ctx->grp_off = nullptr; ctx->grp_lnf = nullptr;
+    if (n_groups > 0) {
+        CK(upload(ctx->owned_grp, &ctx->grp_off, go));
+        CK(upload(ctx->owned_grp, &ctx->grp_lnf, lf));
+        ctx->n_groups = n_groups;
+    }
     return CHIM_OK;
 }
 

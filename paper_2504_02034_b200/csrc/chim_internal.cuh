@@ -462,6 +462,8 @@ struct CombineParams {
     int32_t n_lambda, n_events, n_inj_blocks;
     int64_t n_det; double n_inj_total, neff_factor;
     double inj_ln_shift;     // draw-density scale factored out of s_j, added back to log xi
+    int32_t n_groups;        // many-1d: > 0 = physical events, each the sub-events [group_off[g], group_off[g+1])
+    const int64_t* group_off; const double* ln_factor;
     const uint32_t* flags_in;
     double* out_loglike; double* out_event_logI; double* out_logxi; double* out_neff; uint32_t* out_flags;
 };

@@ -157,6 +157,29 @@ __global__ void __launch_bounds__(kCombThreads) k_combine(CombineParams P) {
     uint32_t fl = lflags | P.flags_in[l];
     double v[3] = {0.0, 0.0, 0.0};   // sum log I, sum s, sum s^2
     int n_ninf = 0, n_nan = 0;
+    if (P.n_groups > 0) {   // many-1d: I_g = sum_k F_k I_k over the pixels of event g, in log space (eq. 14's pixel sum)
+        fl &= ~CHIM_FLAG_EVENT_ZERO;             // raised per sub-event by k_events; here an empty pixel is not an empty event
+        if (P.out_event_logI)
+            for (int i = tid; i < P.n_events; i += kCombThreads)
+                P.out_event_logI[(size_t)l * P.n_events + i] = P.logI[(size_t)l * P.n_events + i];
+        for (int g = tid; g < P.n_groups; g += kCombThreads) {
+            const int64_t k0 = P.group_off[g], k1 = P.group_off[g + 1];
+            double mx = -INFINITY;
+            bool nan = false;
+            for (int64_t k = k0; k < k1; ++k) {
+                const double x = P.logI[(size_t)l * P.n_events + k] + P.ln_factor[k];
+                if (isnan(x)) nan = true;
+                else mx = fmax(mx, x);
+            }
+            if (nan) n_nan = 1;
+            else if (mx == -INFINITY) n_ninf = 1;
+            else {
+                double acc = 0.0;
+                for (int64_t k = k0; k < k1; ++k) acc += exp(P.logI[(size_t)l * P.n_events + k] + P.ln_factor[k] - mx);
+                v[0] += mx + log(acc);
+            }
+        }
+    } else
     for (int i = tid; i < P.n_events; i += kCombThreads) {
         double x = P.logI[(size_t)l * P.n_events + i];
         if (P.out_event_logI) P.out_event_logI[(size_t)l * P.n_events + i] = x;
@@ -174,6 +197,8 @@ __global__ void __launch_bounds__(kCombThreads) k_combine(CombineParams P) {
     n_nan = __syncthreads_or(n_nan);
     n_ninf = __syncthreads_or(n_ninf);
     if (tid != 0) return;
+    const int n_obs = (P.n_groups > 0) ? P.n_groups : P.n_events;   // N_obs of eq. 3
+    if (P.n_groups > 0 && n_ninf && !n_nan) fl |= CHIM_FLAG_EVENT_ZERO;
     double total = n_nan ? NAN : (n_ninf ? -INFINITY : v[0]);
     double logxi = 0.0, neff = NAN;
     if (lflags) { total = NAN; logxi = NAN; }
@@ -183,8 +208,8 @@ __global__ void __launch_bounds__(kCombThreads) k_combine(CombineParams P) {
         if (!(xi > 0.0)) { fl |= CHIM_FLAG_XI_ZERO; logxi = NAN; total = NAN; }
         else {
             logxi = log(xi) + P.inj_ln_shift;
-            if (neff < P.neff_factor * P.n_events) fl |= CHIM_FLAG_NEFF_LOW;   // R8: report only
-            total -= P.n_events * logxi;
+            if (neff < P.neff_factor * n_obs) fl |= CHIM_FLAG_NEFF_LOW;   // R8: report only
+            total -= n_obs * logxi;
         }
     }
     P.out_loglike[l] = total;

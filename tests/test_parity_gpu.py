@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 import oracle as O
-from workloads import lambda_vector, make_workload
+from workloads import lambda_vector, make_workload, split_into_pixels
 
 pytestmark = pytest.mark.gpu
 
@@ -327,6 +327,56 @@ def test_epanechnikov_needs_placement_on_samples(P):
     cfg.kde_kernel, cfg.placement = P.CHIM_KERNEL_EPANECHNIKOV, P.CHIM_ON_GRID
     with pytest.raises(P.ChimError):
         P.chim_create(cfg)
+
+
+# ---------------------------------------------------------------- many-1d kernel (NEXT-1; eq. 18, reading R20)
+@pytest.mark.parametrize("kernel", ["gauss", "epanechnikov"])
+def test_many1d_pixel_groups_match_the_oracle(P, kernel):
+    # 6 events x 8 pixels of unequal population (24 .. ~900 samples), per-pixel p_gal, pixel factors; both kernels
+    w = split_into_pixels(make_workload("o5_spec", n_events=6, n_samples=2500, n_grid=600, n_lambda=6, n_det=4000), n_pix=8)
+    assert w.n_events == 48 and len(w.group_off) == 7
+    ok = O.KERNEL_EPANECHNIKOV if kernel == "epanechnikov" else O.KERNEL_GAUSS
+    ref = O.loglike_workload(w, kernel=ok)
+    O.loglike_workload(w, lam=w.lam[:1])                 # (leaves the oracle on the Gaussian kernel)
+    r = _gpu(P, w, count_pairs=0, kde_kernel=P.CHIM_KERNEL_EPANECHNIKOV if kernel == "epanechnikov" else P.CHIM_KERNEL_GAUSS)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    assert np.array_equal(r["flags"], ref["flags"])
+    # the grouping matters: without it the same sub-events give another total
+    c = P.Context(z_cat_max=w.z_cat_max)
+    c.init_workload(w)
+    c.set_event_groups(None, None)
+    import torch
+    out = c.loglike_batch(torch.as_tensor(w.lam, device=c.device).contiguous())
+    torch.cuda.synchronize()
+    assert np.min(np.abs(out["loglike"].cpu().numpy() - ref["loglike"])) > 1.0
+    c.close()
+
+
+def test_many1d_empty_pixels_and_argument_checks(P):
+    w = split_into_pixels(make_workload("tiny", n_events=3, n_samples=400, n_grid=120, n_lambda=2, n_inj_draw=300), n_pix=4)
+    # pixel 1 of event 0 gets a p_gal of zeros: I_k = 0 there, the event survives; all pixels of event 2 zero: -inf + flag
+    g = slice(w.grid_off[1], w.grid_off[2])
+    w.p_gal[g] = 0.0
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w, count_pairs=0)
+    assert np.isneginf(r["event_logI"][:, 1]).all() and np.isfinite(r["loglike"]).all()
+    assert np.max(np.abs(r["loglike"] - ref["loglike"])) < ABS_TOTAL and np.array_equal(r["flags"], ref["flags"])
+    w.p_gal[w.grid_off[8]:w.grid_off[12]] = 0.0
+    ref = O.loglike_workload(w)
+    r = _gpu(P, w, count_pairs=0)
+    assert np.isneginf(r["loglike"]).all() and np.isneginf(ref["loglike"]).all()
+    assert (r["flags"] & P.CHIM_FLAG_EVENT_ZERO).all() and np.array_equal(r["flags"], ref["flags"])
+    c = P.Context(z_cat_max=w.z_cat_max)
+    with pytest.raises(P.ChimError):                      # before chim_init_events
+        c.set_event_groups(w.group_off, w.ln_factor)
+    c.init_workload(w)
+    for bad in (np.array([0, 4, 4, 12]), np.array([1, 4, 8, 12]), np.array([0, 4, 8, 11])):
+        with pytest.raises(P.ChimError):
+            c.set_event_groups(bad, w.ln_factor)
+    with pytest.raises(P.ChimError):
+        c.set_event_groups(w.group_off, np.full(12, np.nan))
+    c.close()
 
 
 def test_kde_nonuniform_grid_takes_the_direct_form(P):
