@@ -104,7 +104,14 @@ def build_workload(name, args, rank):
     if args.n_lambda:
         kw["n_lambda"] = args.n_lambda
     w = make_workload(name, catalog=args.catalog, **kw)
+    if args.pixels > 0:      # many-1d variant (NEXT-1): every event split into (event, pixel) sub-events
+        from workloads import split_into_pixels
+        w = split_into_pixels(w, n_pix=args.pixels)
     return w
+
+
+def n_physical_events(w):
+    return int(len(w.group_off) - 1) if getattr(w, "group_off", None) is not None else int(w.n_events)
 
 
 def lambda_batches(w, n_batches, rank):
@@ -122,7 +129,8 @@ def lambda_batches(w, n_batches, rank):
 def oracle_step(O, w, lam):
     inj = (w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw)
     return O.loglike_batch(lam, w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal, inj=inj,
-                           n_inj_total=w.n_inj_total, z_cat_max=w.z_cat_max, kernel=ORACLE_KERNEL[0])
+                           n_inj_total=w.n_inj_total, z_cat_max=w.z_cat_max, kernel=ORACLE_KERNEL[0],
+                           group_off=getattr(w, "group_off", None), ln_factor=getattr(w, "ln_factor", None))
 
 
 def run_reference(args):
@@ -140,7 +148,7 @@ def run_reference(args):
     for i in range(args.steps):
         oracle_step(O, w, lams[args.warmup + i][:1])
     dt = (time.perf_counter() - t0) / max(args.steps, 1)
-    val = w.n_events * 1 / dt
+    val = n_physical_events(w) * 1 / dt
     sample = f"per step: 1 of {w.n_lambda} lambda over all {w.n_events} events and {w.n_det} injections"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -154,7 +162,7 @@ def workload_config(w, args):
     ns = int(np.diff(w.sample_off).max())
     nz = int(np.diff(w.grid_off).max())
     return {"workload": f"{w.name} (BASELINE.json configs[{w.meta['index']}]), catalog {w.meta['catalog']}",
-            "n_events": int(w.n_events), "n_samples": ns, "n_grid": nz, "n_lambda_per_gpu": int(w.n_lambda),
+            "n_events": n_physical_events(w), "n_pixels_per_event": int(args.pixels) or 1, "n_samples": ns, "n_grid": nz, "n_lambda_per_gpu": int(w.n_lambda),
             "n_injections_detected": int(w.n_det), "n_injections_drawn": int(w.n_inj_total), "kde_kernel": args.kde_kernel,
             "l2": "flushed between timed steps (256 MiB write)", "fresh_lambda_batch_per_step": True,
             "parallelism": f"lambda-sharded replicas x{args.gpus}, no data-path collective"}
@@ -280,7 +288,7 @@ def run_ours(args):
     if world > 1:
         dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
     t_dev_max, t_e2e_max = [float(x) for x in t_all.cpu()]
-    units = w.n_events * w.n_lambda * K * world
+    units = n_physical_events(w) * w.n_lambda * K * world
     st = ctx.stats()
 
     if rank == 0:
@@ -341,7 +349,7 @@ def cpu_baseline(w, lam, args):
     t0 = time.perf_counter()
     oracle_step(O, w, lam[:n])
     dt = time.perf_counter() - t0
-    return {"value": w.n_events * n / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "seconds": dt,
+    return {"value": n_physical_events(w) * n / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "seconds": dt,
             "sample": f"{n} of {w.n_lambda} lambda over all {w.n_events} events and {w.n_det} injections (work is linear in lambda)"}
 
 
@@ -360,6 +368,8 @@ def main():
     ap.add_argument("--n-lambda", type=int, default=0, help="override (debug only)")
     ap.add_argument("--kde-kernel", default="gauss", choices=["gauss", "epanechnikov"],
                     help="KDE kernel shape (the headline metric is quoted on gauss; epanechnikov is the NEXT-2 variant)")
+    ap.add_argument("--pixels", type=int, default=0,
+                    help="many-1d variant: split every event into this many (event, pixel) sub-events (0 = single-1d, the headline)")
     ap.add_argument("--cpu-lambdas", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

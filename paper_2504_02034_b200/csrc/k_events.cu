@@ -589,7 +589,11 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             if (wbox <= kLeMaxW && fb_hi - fb_lo < (float)kLeMaxBox && fabsf(fb_lo) < 1e6f && fabsf(fb_hi) < 1e6f && fD < 1e5f &&
                 fabsf(fb_lo) * (float)m < 1e8f && fabsf(fb_hi) * (float)m < 1e8f) {
                 const int D = (int)fD, nbox = (int)(fb_hi - fb_lo) + 1;
-                if (le_bytes(ev_nz_pad(nz), D, nbox) <= ev_aux_bytes(P.ev.max_nz)) {
+                // issue-slot estimates (profiles/r01c): coefficient build 1/16 per FMA, evaluation ~1 per sample; power form
+                // 2.25 per 64 pairs.  Few samples (many-1d pixels) do not amortise the coefficient build.
+                const float le_cost = 0.0625f * (float)nbox * (float)kLeP * (2.f * fD + 1.f) + (float)ns + 150.f;
+                const float pw_cost = Bsel ? 0.035f * (float)ns * (2.f * T / delta + (float)Bsel) : INFINITY;
+                if (le_cost <= pw_cost && le_bytes(ev_nz_pad(nz), D, nbox) <= ev_aux_bytes(P.ev.max_nz)) {
                     S.scy = scy; S.dy = dy; S.yfirst = yfirst; S.le_m = m; S.le_D = D; S.le_blo = (int)fb_lo; S.le_nbox = nbox;
                 }
             }
