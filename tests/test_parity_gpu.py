@@ -135,7 +135,7 @@ def test_s5_injection_weights(P):
 
 # ---------------------------------------------------------------- T3: end to end
 def test_s5_dense_injection_set_takes_the_chunk_local_polynomials(P):
-    # 10^5 sorted injections: chunks of 8192 span < 0.9 in ln d_L and are evaluated with chunk-local polynomials
+    # 10^5 sorted injections: chunks of 16384 span < 0.9 in ln d_L and are evaluated with chunk-local polynomials
     # (the sparse ends of the set still go through the table rows); log xi and N_eff against the oracle
     w = make_workload("o5_spec", n_events=3, n_samples=600, n_grid=300, n_lambda=4, n_det=100_000)
     ref = O.loglike_workload(w)
