@@ -372,7 +372,9 @@ double chimo_scott_bw(int n, const double *z, const double *w) {
         long double wh = w[j] / sw, d = z[j] - zb;
         var += wh * d * d;
     }
-    if (!(1.0L - s2 > 0.0L)) return NAN;
+    /* R21: one sample carries the event.  As n_eff -> 1 the rule divides 0 by 0 (sigma^2 -> d^2/2 for two
+     * samples however small the second weight): the bandwidth is declared undefined once n_eff < 1/(1 - 1e-4). */
+    if (!(1.0L - s2 > 1.0e-4L)) return NAN;
     var /= (1.0L - s2);
     if (!(var > 0.0L)) return NAN;
     double neff = (double)(1.0L / s2);

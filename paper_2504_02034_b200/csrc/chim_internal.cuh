@@ -212,7 +212,7 @@ __device__ __forceinline__ void sample_eval(const LamF& F, const float4 q0, cons
     if (__any_sync(0xffffffffu, mp2 < F.delta)) {      // skipped by warps whose secondaries all lie above the window
         const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
         const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
-        const float ls = lg2f(1.0f + ex2f(f2));
+        const float ls = (f2 > 64.f) ? f2 : lg2f(1.0f + ex2f(f2));   // deep in the window 2^f2 overflows; log2(1 + 2^f) = f there
         l -= (mp2 < F.delta) ? ls : 0.f;
     }
     const bool ok = in_range && (mp2 > 0.f);           // R15 support: m_low < m2 (<= m1)
@@ -348,7 +348,7 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
     if (__any_sync(0xffffffffu, mp2 < F.delta)) {
         const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
         const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
-        const float ls = lg2f(1.0f + ex2f(f2));
+        const float ls = (f2 > 64.f) ? f2 : lg2f(1.0f + ex2f(f2));   // deep in the window 2^f2 overflows; log2(1 + 2^f) = f there
         l -= (mp2 < F.delta) ? ls : 0.f;
     }
     l2w = (mp2 > 0.f) ? l : -INFINITY;      // R15 support: m_low < m2

@@ -563,7 +563,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         } else {   // Scott on the weighted sample (R3, O7)
             double s2 = mom[1] / (sw * sw), zb = mom[2] / sw;
             double var = (mom[3] / sw - zb * zb) / (1.0 - s2);
-            h = (1.0 - s2 > 0.0 && var > 0.0) ? sqrt(var) * (double)exp2f(0.2f * log2f((float)s2)) : NAN;   // n_eff^(-1/5) = s2^(1/5); fp32: dh/h ~ 1e-7 moves log I by ~1e-9
+            h = (1.0 - s2 > 1.0e-4 && var > 0.0) ? sqrt(var) * (double)exp2f(0.2f * log2f((float)s2)) : NAN;   // n_eff^(-1/5) = s2^(1/5); fp32: dh/h ~ 1e-7 moves log I by ~1e-9.  R21: undefined once one sample carries the event
         }
         if (P.dbg_h) *P.dbg_h = h;
         // scaled coordinates x = z' sqrt(log2(e)/2)/h: exp(-d^2/2h^2) = 2^(-dx^2)

@@ -341,6 +341,18 @@ def test_scott_bandwidth_reduces_to_textbook_for_equal_weights():
     assert math.isnan(O.scott_bw([0.3], [1.0])) and math.isnan(O.scott_bw(z, np.zeros(200)))
 
 
+def test_scott_bandwidth_two_samples_closed_form_and_degenerate_threshold():
+    # two samples d apart, weights (1, eps): sum w^2 = (1 + eps^2)/(1 + eps)^2, sigma^2 = d^2/2 for EVERY eps (the 0/0 of
+    # R21), h = d/sqrt(2) n_eff^(-1/5); undefined once 1 - sum w^2 <= 1e-4 (eps ~ 5e-5)
+    d = 0.04
+    for eps in (1.0, 0.1, 1e-3, 1e-4):
+        s2 = (1 + eps ** 2) / (1 + eps) ** 2
+        h = O.scott_bw([0.5, 0.5 + d], [1.0, eps])
+        assert abs(h / (d / math.sqrt(2) * s2 ** 0.2) - 1) < 1e-12
+    for eps in (4e-5, 1e-6, 1e-12, 0.0):
+        assert math.isnan(O.scott_bw([0.5, 0.5 + d], [1.0, eps]))
+
+
 # ------------------------------------------------------------------ P11: brute force, independent route
 def _brute_loglike(la, events, inj, n_inj_total, z_cat_max, fixed_h=None):
     """Independent re-computation with scipy (quad / brentq) on tiny inputs; placement N."""

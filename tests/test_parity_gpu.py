@@ -56,6 +56,54 @@ def _compare(r, ref, n_events):
     return rel, dtot, dxi
 
 
+# ---------------------------------------------------------------- full size, in the configuration bench.py times
+def test_full_size_o5_spectroscopic_sampled_outputs(P):
+    """BASELINE.json configs[1] at full size (300 events x 5000 samples x 1000 grid points, 1024 lambda, 10^6
+    injections), launched as bench.py launches it (default config, lambda_chunk 256, no pair counting).  The oracle
+    cannot run 307 200 units in a test, so: 40 sampled (event, lambda) outputs one by one, log xi / N_eff / the total
+    for 2 lambdas, and properties over the whole batch."""
+    import torch
+    w = make_workload("o5_spec")
+    assert (w.n_events, w.n_lambda, w.n_det) == (300, 1024, 1_000_000)
+    c = P.Context(z_cat_max=w.z_cat_max)
+    c.init_workload(w)
+    out = c.loglike_batch(torch.as_tensor(w.lam, device=c.device).contiguous())
+    torch.cuda.synchronize()
+    r = {k: v.cpu().numpy() for k, v in out.items()}
+    c.close()
+    # properties at any size: total = sum of the parts (eq. 3); flags clear wherever every unit is finite
+    assert np.isfinite(r["logxi"]).all() and (r["neff"] > 5 * 300).all() and (r["neff"] < w.n_det).all()
+    fin = np.isfinite(r["event_logI"]).all(axis=1)
+    assert fin.sum() >= 1000 and (r["flags"][fin] == 0).all() and (r["flags"][~fin] != 0).all()
+    assert np.max(np.abs(r["loglike"][fin] - (r["event_logI"][fin].sum(axis=1) - 300 * r["logxi"][fin]))) < 1e-8
+    assert not np.isfinite(r["loglike"][~fin]).any()
+    # the few non-finite units (an extreme lambda whose m_low leaves an event one or no sample: R15 / R21) one by one:
+    # -inf where the oracle has -inf, NaN where it has NaN
+    bad = np.argwhere(~np.isfinite(r["event_logI"]))
+    assert len(bad) < 200
+    for l, i in bad:
+        s, g = slice(w.sample_off[i], w.sample_off[i + 1]), slice(w.grid_off[i], w.grid_off[i + 1])
+        ref, _, fl = O.event_logI(w.lam[l], w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s], w.z_grid[g], w.p_gal[g])
+        assert (np.isnan(ref) and np.isnan(r["event_logI"][l, i])) or (ref == -np.inf and r["event_logI"][l, i] == -np.inf), (l, i, ref)
+        assert fl & (P.CHIM_FLAG_EVENT_ZERO | P.CHIM_FLAG_BW_DEGENERATE) & int(r["flags"][l])
+    # sampled units against the oracle, one by one
+    rng = np.random.default_rng(123)
+    worst = 0.0
+    for l, i in zip(rng.choice(np.flatnonzero(fin), 40), rng.integers(0, 300, 40)):
+        s, g = slice(w.sample_off[i], w.sample_off[i + 1]), slice(w.grid_off[i], w.grid_off[i + 1])
+        ref, _, fl = O.event_logI(w.lam[l], w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s], w.z_grid[g], w.p_gal[g])
+        assert fl == 0 and abs(r["event_logI"][l, i] - ref) < REL_EVENT * abs(ref)
+        worst = max(worst, abs(r["event_logI"][l, i] - ref))
+    assert worst < 5e-6
+    # selection term and total for two lambdas (the fiducial and a random one)
+    ls = [0, 777]
+    ref = O.loglike_workload(w, lam=w.lam[ls])
+    assert np.max(np.abs(r["logxi"][ls] - ref["logxi"])) < 1e-6
+    assert np.max(np.abs(r["neff"][ls] / ref["neff"] - 1)) < 1e-5
+    assert np.max(np.abs(r["loglike"][ls] - ref["loglike"])) < ABS_TOTAL
+    assert np.max(np.abs(r["event_logI"][ls] - ref["event_logI"]) / np.abs(ref["event_logI"])) < REL_EVENT
+
+
 # ---------------------------------------------------------------- T2: intermediates, step by step
 def test_s1_table_inversion_and_ratio(P):
     w = make_workload("tiny")
