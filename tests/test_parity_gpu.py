@@ -104,6 +104,36 @@ def test_full_size_o5_spectroscopic_sampled_outputs(P):
     assert np.max(np.abs(r["event_logI"][ls] - ref["event_logI"]) / np.abs(ref["event_logI"])) < REL_EVENT
 
 
+@pytest.mark.parametrize("name,kw", [("o5_photo", dict(n_lambda=48)),
+                                     ("full_pop", dict(n_events=400, n_lambda=32)),
+                                     ("sel_heavy", dict(n_events=40, n_lambda=24, n_det=2_000_000))])
+def test_other_config_shapes_sampled_outputs(P, name, kw):
+    """The per-unit shapes of BASELINE.json configs[2..4] (4096-point photometric grids with 2000 galaxies; 4096 samples x
+    512 grid points; the 10^7-injection reference pdf at 2 x 10^6) with fewer lambdas / events than the full configs:
+    sampled (event, lambda) units one by one, log xi for two lambdas."""
+    import torch
+    w = make_workload(name, **kw)
+    c = P.Context(z_cat_max=w.z_cat_max)
+    c.init_workload(w)
+    out = c.loglike_batch(torch.as_tensor(w.lam, device=c.device).contiguous())
+    torch.cuda.synchronize()
+    r = {k: v.cpu().numpy() for k, v in out.items()}
+    c.close()
+    fin = np.isfinite(r["event_logI"]).all(axis=1)
+    assert fin.sum() >= 0.9 * w.n_lambda and (r["flags"][fin] == 0).all()
+    rng = np.random.default_rng(321)
+    for l, i in zip(rng.choice(np.flatnonzero(fin), 10), rng.integers(0, w.n_events, 10)):
+        s, g = slice(w.sample_off[i], w.sample_off[i + 1]), slice(w.grid_off[i], w.grid_off[i + 1])
+        ref, _, fl = O.event_logI(w.lam[l], w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s], w.z_grid[g], w.p_gal[g])
+        assert fl == 0 and abs(r["event_logI"][l, i] - ref) < 5e-6
+    ls = [int(np.flatnonzero(fin)[0]), int(np.flatnonzero(fin)[-1])]
+    inj = (w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw)
+    for l in ls:
+        s1, s2 = O.selection_sums(w.lam[l], *inj, z_cat_max=w.z_cat_max)
+        assert abs(r["logxi"][l] - math.log(s1 / w.n_inj_total)) < 1e-6
+        assert abs(r["neff"][l] / O.neff(s1, s2, w.n_inj_total) - 1) < 1e-5
+
+
 # ---------------------------------------------------------------- T2: intermediates, step by step
 def test_s1_table_inversion_and_ratio(P):
     w = make_workload("tiny")
