@@ -155,6 +155,15 @@ def event_logI(lam, dl, m1d, m2d, ln_prior, zg, pgal, placement=PLACE_SAMPLES, b
     return float(v), float(h.value), int(fl.value)
 
 
+def pcat(lam, z_gal, sigma_gal, zg, w_gal=None):
+    """PAPER.md:62 eq. 8 for one line of sight: catalogue redshift density on the grid zg (reading R22)."""
+    lam, zt, st, zg = _lam(lam), _d(z_gal), _d(sigma_gal), _d(zg)
+    wg = None if w_gal is None else _d(w_gal)
+    out = np.empty_like(zg)
+    lib().chimo_pcat(_p(lam), C.c_int(zt.size), _p(zt), _p(st), _p(wg), C.c_int(zg.size), _p(zg), _p(out))
+    return out
+
+
 def selection_sums(lam, dl, m1d, m2d, ln_pdraw, z_cat_max=1.5, z_table_max=10.0, return_s=False):
     lam, dl, m1d, m2d, lp = _lam(lam), _d(dl), _d(m1d), _d(m2d), _d(ln_pdraw)
     s1, s2 = C.c_double(0), C.c_double(0)

@@ -506,6 +506,43 @@ double chimo_neff(double sum_s, double sum_s2, double n_inj_total) {
     return sum_s * sum_s / (sum_s2 - sum_s * sum_s / n_inj_total);
 }
 
+/* -------------------------------------------------------------- p_cat from a galaxy list ---- */
+/* PAPER.md:62 eq. 8 for one line of sight (the step before the hot path; reading R22 of DESIGN.md):
+ *   p_cat(z) = (1/sum_g w_g) sum_g w_g N(z; zt_g, st_g) dVc/dz(z) / Z_g,   Z_g = int_0^inf N(z; zt_g, st_g) dVc/dz dz,
+ * dV_c/dz at the fixed cosmology lam (computed once, fixed for the whole inference); Z_g by Gauss-Legendre on
+ * [max(0, zt - 10 st), zt + 10 st].  w == NULL: unit weights. */
+typedef struct { const lam_t *L; double zt, st; } pcat_ctx;
+static double pcat_integrand(double z, const void *ctx) {
+    const pcat_ctx *c = (const pcat_ctx *)ctx;
+    double u = (z - c->zt) / c->st;
+    return exp(-0.5 * u * u) / (c->st * sqrt(2.0 * M_PI)) * dVc_dz(z, c->L);
+}
+void chimo_pcat(const double *lam, int n_gal, const double *zt, const double *st, const double *w, int ng,
+                const double *zg, double *out) {
+    gl_init();
+    const lam_t *L = (const lam_t *)lam;
+    double *coef = (double *)malloc(sizeof(double) * (n_gal > 0 ? n_gal : 1));
+    long double sw = 0.0L;
+    for (int g = 0; g < n_gal; ++g) {
+        pcat_ctx c = {L, zt[g], st[g]};
+        double lo = zt[g] - 10.0 * st[g], hi = zt[g] + 10.0 * st[g];
+        if (lo < 0.0) lo = 0.0;
+        double Z = gl_integrate(pcat_integrand, &c, lo, hi, 8);
+        double wg = w ? w[g] : 1.0;
+        coef[g] = wg / Z;
+        sw += wg;
+    }
+    for (int i = 0; i < ng; ++i) {
+        long double acc = 0.0L;
+        for (int g = 0; g < n_gal; ++g) {
+            double u = (zg[i] - zt[g]) / st[g];
+            acc += coef[g] * exp(-0.5 * u * u) / (st[g] * sqrt(2.0 * M_PI));
+        }
+        out[i] = (double)(acc / sw) * dVc_dz(zg[i], L);
+    }
+    free(coef);
+}
+
 /* ------------------------------------------------------------------------- O11 log L -------- */
 void chimo_loglike_batch_grouped(int n_lambda, const double *lam, int placement, int bw_rule,
                          double z_cat_max, double z_table_max, int n_table, double neff_factor,

@@ -515,6 +515,37 @@ def test_many1d_with_shared_p_gal_and_fixed_bandwidth_equals_single1d():
     assert abs(rp["loglike"][0] - r1["loglike"][0]) < 1e-10
 
 
+# ------------------------------------------------------------------ p_cat from a galaxy list (NEXT-3; eq. 8, R22)
+def test_pcat_against_scipy_quadrature_and_unit_mass():
+    la = lam(H0=67.0, Om=0.31)
+    rng = np.random.default_rng(3)
+    zt = rng.uniform(0.2, 0.6, 7)
+    st = 0.01 * (1 + zt) * rng.uniform(0.5, 2.0, 7)
+    wg = rng.uniform(0.5, 2.0, 7)
+    dv = lambda z: O.volume(la, np.array([z]))[0][0]                      # dV_c/dz, itself pinned by eq. 23
+    gauss = lambda z, m, s: math.exp(-0.5 * ((z - m) / s) ** 2) / (s * math.sqrt(2 * math.pi))
+    Z = [integrate.quad(lambda z: gauss(z, m, s) * dv(z), max(0.0, m - 12 * s), m + 12 * s, epsabs=0, epsrel=1e-13)[0]
+         for m, s in zip(zt, st)]
+    zg = np.linspace(0.1, 0.8, 29)
+    ref = [sum(w * gauss(z, m, s) / zz for w, m, s, zz in zip(wg, zt, st, Z)) * dv(z) / wg.sum() for z in zg]
+    assert np.allclose(O.pcat(la, zt, st, zg, wg), ref, rtol=1e-11, atol=1e-300)
+    # each galaxy contributes unit mass: p_cat integrates to 1 over a grid that covers the catalogue; unit weights = w None
+    zf = np.linspace(0.0, 1.2, 24001)
+    assert abs(np.trapezoid(O.pcat(la, zt, st, zf, wg), zf) - 1) < 1e-9
+    assert np.allclose(O.pcat(la, zt, st, zg), O.pcat(la, zt, st, zg, np.ones(7)), rtol=1e-15)
+
+
+def test_pcat_narrow_galaxies_reduce_to_the_gaussian_mixture_and_h0_cancels():
+    # sigma -> 0: dV_c/dz is constant across a galaxy, so it cancels against Z_g and p_cat -> sum_g w_g N / sum_g w_g
+    la = lam(H0=70.0, Om=0.3)
+    zt, st = np.array([0.5, 0.9]), np.array([1e-5, 2e-5])
+    zg = np.array([0.5 - 1e-5, 0.5, 0.5 + 2e-5, 0.9, 0.9 + 3e-5])
+    mix = 0.5 * sum(np.exp(-0.5 * ((zg - m) / s) ** 2) / (s * math.sqrt(2 * math.pi)) for m, s in zip(zt, st))
+    assert np.allclose(O.pcat(la, zt, st, zg), mix, rtol=2e-4)
+    z2 = np.linspace(0.3, 1.1, 9)
+    assert np.allclose(O.pcat(la, zt, np.array([0.02, 0.03]), z2), O.pcat(lam(H0=35.0, Om=0.3), zt, np.array([0.02, 0.03]), z2), rtol=1e-13)
+
+
 # ------------------------------------------------------------------ flags / degenerate cases
 def test_flags_and_degenerate_cases():
     w = make_workload("tiny", n_events=2, n_samples=50, n_grid=60, n_inj_draw=200)
