@@ -148,6 +148,21 @@ int chim_init_events(chim_ctx *ctx, int32_t n_events, const int64_t *sample_off,
 int chim_set_event_groups(chim_ctx *ctx, int32_t n_groups, const int64_t *group_off, const double *ln_factor);
 
 /*
+ * The step before the path (one-off): the catalogue term p_cat of PAPER.md:62 eq. 8 on redshift grids, from galaxy lists,
+ * at a fixed cosmology (computed once for the whole inference; only Omega_m matters, H0 cancels; R22).
+ * For each of n_los lines of sight (an event, or an event's pixel):
+ *     p_cat(z) = (1/sum_g w_g) sum_g w_g N(z; z_gal_g, sigma_gal_g) dVc/dz(z) / Z_g,  Z_g = int N(z; z_gal_g, sigma_gal_g) dVc/dz dz
+ *   gal_off  [n_los+1] CSR offsets into z_gal / sigma_gal / w_gal (>= 1 galaxy per line of sight)
+ *   z_gal >= 0, sigma_gal > 0, w_gal > 0 or NULL (unit weights)
+ *   grid_off [n_los+1] CSR offsets into z_grid / p_cat_out;  z_grid >= 0
+ * All pointers live where cfg.mem says (p_cat_out too); synchronous.  The result can be passed to chim_init_events as p_gal
+ * (complete catalogue, as in the paper's runs; the completeness terms of eq. 7, 9, 10 are not built).
+ */
+int chim_build_pcat(chim_ctx *ctx, double omega_m, int32_t n_los, const int64_t *gal_off, const double *z_gal,
+                    const double *sigma_gal, const double *w_gal, const int64_t *grid_off, const double *z_grid,
+                    double *p_cat_out);
+
+/*
  * Detected injections for the selection term: n_det stored injections out of
  * n_inj_total drawn; ln_pdraw = ln of the draw density in (d_L, m1d, m2d) (R7).  Optional: without
  * injections log xi := 0 and loglike = sum_i log I_i.  n_det == 0 removes a previous set.

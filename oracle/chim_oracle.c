@@ -13,7 +13,7 @@
  * CUDA path's tables are checked rather than shared.  No blocking, truncation or reordering:
  * the KDE is the full N_s x N_z sum.
  *
- * Citations are PAPER.md:<line> (section / equation).  Readings R1..R20 and the mass-model
+ * Citations are PAPER.md:<line> (section / equation).  Readings R1..R22 and the mass-model
  * reading M1..M4 are SURVEY.md sec. 8(c), restated in DESIGN.md.
  *
  * Pins (tests/test_oracle_pins.py): every function below is pinned except the *choices*

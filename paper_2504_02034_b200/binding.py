@@ -78,6 +78,7 @@ def lib():
     L.chim_init_events.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 9
     L.chim_init_injections.argtypes = [C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 4
     L.chim_set_event_groups.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    L.chim_build_pcat.argtypes = [C.c_void_p, C.c_double, C.c_int32] + [C.c_void_p] * 7
     L.chim_loglike_batch.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_loglike_batch_host.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_get_stats.argtypes = [C.c_void_p, C.POINTER(ChimStats)]
@@ -142,6 +143,11 @@ def chim_init_events(ctx, n_events, sample_off, dL, m1d, m2d, ln_prior, grid_off
 
 def chim_set_event_groups(ctx, n_groups, group_off, ln_factor):
     _check(ctx, lib().chim_set_event_groups(ctx, n_groups, _addr(group_off), _addr(ln_factor)))
+
+
+def chim_build_pcat(ctx, omega_m, n_los, gal_off, z_gal, sigma_gal, w_gal, grid_off, z_grid, p_cat_out):
+    _check(ctx, lib().chim_build_pcat(ctx, omega_m, n_los, *[_addr(a) for a in (gal_off, z_gal, sigma_gal, w_gal, grid_off,
+                                                                               z_grid, p_cat_out)]))
 
 
 def chim_init_injections(ctx, n_det, n_inj_total, dL, m1d, m2d, ln_pdraw):
@@ -230,6 +236,16 @@ class Context:
         chim_init_events(self.h, len(so) - 1, so, *arrs, go, zg, pg, fb)
         self.n_events = len(so) - 1
         self._ns, self._nz = np.diff(so), np.diff(go)
+
+    def build_pcat(self, omega_m, gal_off, z_gal, sigma_gal, grid_off, z_grid, w_gal=None):
+        """PAPER.md:62 eq. 8 on the given grids (host arrays in, host array out)."""
+        go = np.ascontiguousarray(gal_off, dtype=np.int64)
+        po = np.ascontiguousarray(grid_off, dtype=np.int64)
+        zg = _f64(z_grid)
+        out = np.empty_like(zg)
+        chim_build_pcat(self.h, float(omega_m), len(go) - 1, go, _f64(z_gal), _f64(sigma_gal),
+                        None if w_gal is None else _f64(w_gal), po, zg, out)
+        return out
 
     def set_event_groups(self, group_off, ln_factor):
         """many-1d: the loaded entries are (event, pixel) sub-events; None removes the grouping."""

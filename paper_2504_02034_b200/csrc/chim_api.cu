@@ -565,6 +565,51 @@ int chim_set_event_groups(chim_ctx* ctx, int32_t n_groups, const int64_t* group_
     return CHIM_OK;
 }
 
+int chim_build_pcat(chim_ctx* ctx, double omega_m, int32_t n_los, const int64_t* gal_off, const double* z_gal,
+                    const double* sigma_gal, const double* w_gal, const int64_t* grid_off, const double* z_grid,
+                    double* p_cat_out) {
+    if (!ctx) return CHIM_EINVAL;
+    if (n_los < 1 || !gal_off || !z_gal || !sigma_gal || !grid_off || !z_grid || !p_cat_out || !(omega_m > 0.0) || !(omega_m <= 1.0))
+        return fail(ctx, CHIM_EINVAL, "chim_build_pcat: null pointer, n_los < 1 or omega_m outside (0, 1]");
+    CK(cudaSetDevice(ctx->cfg.device));
+    std::vector<int64_t> go, po;
+    CK(fetch(ctx, gal_off, (size_t)n_los + 1, go));
+    CK(fetch(ctx, grid_off, (size_t)n_los + 1, po));
+    if (go[0] != 0 || po[0] != 0) return fail(ctx, CHIM_EINVAL, "chim_build_pcat: offsets must start at 0");
+    for (int i = 0; i < n_los; ++i)
+        if (go[i + 1] <= go[i] || po[i + 1] < po[i])
+            return fail(ctx, CHIM_EINVAL, "chim_build_pcat: every line of sight needs >= 1 galaxy; offsets must not decrease");
+    const size_t NG = (size_t)go[n_los], NP = (size_t)po[n_los];
+    std::vector<double> hz, hs, hw, hg;
+    CK(fetch(ctx, z_gal, NG, hz)); CK(fetch(ctx, sigma_gal, NG, hs)); CK(fetch(ctx, z_grid, NP, hg));
+    if (w_gal) CK(fetch(ctx, w_gal, NG, hw));
+    if (!all_finite(hz) || !all_finite(hs) || !all_finite(hw) || !all_finite(hg)) return fail(ctx, CHIM_EINVAL, "chim_build_pcat: non-finite input");
+    for (size_t g = 0; g < NG; ++g)
+        if (hz[g] < 0.0 || !(hs[g] > 0.0) || (w_gal && !(hw[g] > 0.0)))
+            return fail(ctx, CHIM_EINVAL, "chim_build_pcat: need z_gal >= 0, sigma_gal > 0, w_gal > 0");
+    for (size_t i = 0; i < NP; ++i)
+        if (hg[i] < 0.0) return fail(ctx, CHIM_EINVAL, "chim_build_pcat: z_grid must be >= 0");
+    std::vector<void*> pool;
+    const int64_t *d_go = nullptr, *d_po = nullptr;
+    const double *d_z = nullptr, *d_s = nullptr, *d_w = nullptr, *d_g = nullptr;
+    double *d_coef = nullptr, *d_out = nullptr;
+    cudaError_t e = upload(pool, &d_go, go);
+    if (e == cudaSuccess) e = upload(pool, &d_po, po);
+    if (e == cudaSuccess) e = upload(pool, &d_z, hz);
+    if (e == cudaSuccess) e = upload(pool, &d_s, hs);
+    if (e == cudaSuccess && w_gal) e = upload(pool, &d_w, hw);
+    if (e == cudaSuccess) e = upload(pool, &d_g, hg);
+    if (e == cudaSuccess) e = dev_alloc(pool, &d_coef, NG);
+    if (e == cudaSuccess) e = dev_alloc(pool, &d_out, NP);
+    if (e == cudaSuccess) e = launch_pcat(omega_m, n_los, d_go, d_z, d_s, d_w, d_po, d_g, d_coef, d_out, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e == cudaSuccess && NP > 0)
+        e = cudaMemcpy(p_cat_out, d_out, NP * sizeof(double), ctx->cfg.mem == CHIM_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost);
+    free_pool(pool);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "chim_build_pcat");
+    return CHIM_OK;
+}
+
 int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, const double* dL, const double* m1d,
                          const double* m2d, const double* ln_pdraw) {
     if (!ctx) return CHIM_EINVAL;

@@ -514,6 +514,76 @@ cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int
     return cudaGetLastError();
 }
 
+// ---- p_cat from galaxy lists (eq. 8; one-off, before the hot path; R22) -----------------------
+// One CTA per line of sight (event or pixel).  dV_c/dz is needed up to a constant only (it cancels against the per-galaxy
+// normalisation): V(z) = I(z)^2 / E(z), I(z) = int_0^z dz'/E by one 32-node Gauss-Legendre panel.  fp64 throughout.
+__device__ __forceinline__ double pcat_vol(double z, double Om) {
+    double I = 0.0;
+    const double hz = 0.5 * z;
+#pragma unroll 4
+    for (int q = 0; q < kGLWin; ++q) {
+        const double a = 1.0 + hz * (1.0 + c_glw_x[q]);
+        I += c_glw_w[q] * rsqrt(Om * a * a * a + 1.0 - Om);
+    }
+    I *= hz;
+    const double a = 1.0 + z;
+    return I * I * rsqrt(Om * a * a * a + 1.0 - Om);
+}
+
+__global__ void __launch_bounds__(256) k_pcat(double Om, const int64_t* __restrict__ gal_off, const double* __restrict__ zt,
+                                              const double* __restrict__ st, const double* __restrict__ wg,
+                                              const int64_t* __restrict__ grid_off, const double* __restrict__ zg,
+                                              double* __restrict__ coef, double* __restrict__ out) {
+    __shared__ double red[256 / 32];
+    __shared__ double s_sw;
+    const int e = blockIdx.x, tid = threadIdx.x;
+    const int64_t g0 = gal_off[e], g1 = gal_off[e + 1], p0 = grid_off[e], p1 = grid_off[e + 1];
+    // per galaxy: Z_g = int N(z; zt, st) V(z) dz over [max(0, zt - 10 st), zt + 10 st], 8 panels of 32 nodes
+    double sw = 0.0;
+    for (int64_t g = g0 + tid; g < g1; g += 256) {
+        const double m = zt[g], s = st[g], w = wg ? wg[g] : 1.0;
+        const double lo = fmax(0.0, m - 10.0 * s), hi = m + 10.0 * s, hw = 0.5 * (hi - lo) / 8.0;
+        double Z = 0.0;
+        for (int p = 0; p < 8; ++p) {
+            const double mid = lo + (2 * p + 1) * hw;
+            double acc = 0.0;
+            for (int q = 0; q < kGLWin; ++q) {
+                const double z = mid + hw * c_glw_x[q], u = (z - m) / s;
+                acc += c_glw_w[q] * exp(-0.5 * u * u) * pcat_vol(z, Om);
+            }
+            Z += acc * hw;
+        }
+        coef[g] = w / Z;          // (the Gaussian's 1/(s sqrt(2 pi)) is common to N and Z_g: it cancels)
+        sw += w;
+    }
+    sw = warp_sum(sw);
+    if ((tid & 31) == 0) red[tid >> 5] = sw;
+    __syncthreads();              // also publishes coef[] (same CTA)
+    if (tid == 0) {
+        double a = 0.0;
+        for (int k = 0; k < 256 / 32; ++k) a += red[k];
+        s_sw = a;
+    }
+    __syncthreads();
+    const double inv_sw = 1.0 / s_sw;
+    for (int64_t i = p0 + tid; i < p1; i += 256) {
+        const double z = zg[i];
+        double acc = 0.0;
+        for (int64_t g = g0; g < g1; ++g) {
+            const double u = (z - zt[g]) / st[g];
+            if (fabs(u) < 39.0) acc += coef[g] * exp(-0.5 * u * u);      // exp(-760) underflows fp64
+        }
+        out[i] = acc * inv_sw * pcat_vol(z, Om);
+    }
+}
+
+cudaError_t launch_pcat(double Om, int n_los, const int64_t* gal_off, const double* zt, const double* st, const double* wg,
+                        const int64_t* grid_off, const double* zg, double* coef, double* out, cudaStream_t st_) {
+    if (n_los <= 0) return cudaSuccess;
+    k_pcat<<<n_los, 256, 0, st_>>>(Om, gal_off, zt, st, wg, grid_off, zg, coef, out);
+    return cudaGetLastError();
+}
+
 __global__ void k_table_lookup(const LamConst* __restrict__ Lc, const Row* __restrict__ tab, DlGrid g, int64_t n,
                                const double* __restrict__ dL, double z_table_max, double* __restrict__ z_out,
                                double* __restrict__ r_out) {

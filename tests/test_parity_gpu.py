@@ -457,6 +457,49 @@ def test_many1d_empty_pixels_and_argument_checks(P):
     c.close()
 
 
+# ---------------------------------------------------------------- p_cat from galaxy lists (NEXT-3; eq. 8, R22)
+def test_build_pcat_matches_the_oracle_and_feeds_the_path(P):
+    rng = np.random.default_rng(17)
+    n_los, om = 5, 0.31
+    ngal = [1, 50, 500, 333, 7]
+    gal_off = np.concatenate([[0], np.cumsum(ngal)])
+    z_gal = np.concatenate([rng.uniform(0.05, 1.4, n) for n in ngal])
+    sig = np.where(rng.random(z_gal.size) < 0.5, 0.001, 0.03) * (1 + z_gal)          # spectroscopic and photometric widths
+    wg = rng.uniform(0.3, 3.0, z_gal.size)
+    nz = [300, 1000, 257, 4096, 2]
+    grid_off = np.concatenate([[0], np.cumsum(nz)])
+    z_grid = np.concatenate([np.linspace(lo, lo + 0.9, n) for lo, n in zip((0.0, 0.1, 0.3, 0.2, 0.5), nz)])
+    c = P.Context()
+    for w_in in (wg, None):
+        got = c.build_pcat(om, gal_off, z_gal, sig, grid_off, z_grid, w_gal=w_in)
+        for i in range(n_los):
+            g, p = slice(gal_off[i], gal_off[i + 1]), slice(grid_off[i], grid_off[i + 1])
+            ref = O.pcat(lambda_vector(H0=70.0, Om=om), z_gal[g], sig[g], z_grid[p], None if w_in is None else wg[g])
+            assert np.allclose(got[p], ref, rtol=1e-10, atol=1e-290), i
+    # argument checks
+    with pytest.raises(P.ChimError):
+        c.build_pcat(om, gal_off, z_gal, np.zeros_like(sig), grid_off, z_grid)
+    with pytest.raises(P.ChimError):
+        c.build_pcat(1.5, gal_off, z_gal, sig, grid_off, z_grid)
+    with pytest.raises(P.ChimError):
+        c.build_pcat(om, np.array([0, 0, 3]), z_gal[:3], sig[:3], np.array([0, 2, 4]), z_grid[:4])
+    c.close()
+    # end to end: p_gal built on the GPU from galaxy lists, then the path; the oracle gets its own p_cat
+    w = make_workload("tiny", n_events=3, n_samples=400, n_grid=160, n_lambda=2, n_inj_draw=500)
+    go = np.arange(4) * 40
+    zgal = np.concatenate([rng.uniform(w.z_grid[w.grid_off[i]], w.z_grid[w.grid_off[i + 1] - 1], 40) for i in range(3)])
+    sg = 0.002 * (1 + zgal)
+    c = P.Context(z_cat_max=w.z_cat_max)
+    w.p_gal = c.build_pcat(0.3, go, zgal, sg, w.grid_off, w.z_grid)
+    c.close()
+    r = _gpu(P, w, count_pairs=0)
+    w.p_gal = np.concatenate([O.pcat(lambda_vector(Om=0.3), zgal[go[i]:go[i + 1]], sg[go[i]:go[i + 1]],
+                                     w.z_grid[w.grid_off[i]:w.grid_off[i + 1]]) for i in range(3)])
+    ref = O.loglike_workload(w)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+
+
 def test_kde_nonuniform_grid_takes_the_direct_form(P):
     # R14: any strictly increasing grid; the trapezoid uses the true spacings
     w = make_workload("o5_spec", n_events=5, n_samples=1500, n_grid=400, n_lambda=6, n_det=3000)
