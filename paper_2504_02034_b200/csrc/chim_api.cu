@@ -294,7 +294,7 @@ void chim_default_config(chim_config* cfg) {
     cfg->lambda_chunk = 256;
     cfg->neff_factor = 5.0;
     cfg->kde_method = CHIM_KDE_AUTO;
-    cfg->n_mass_table = 2048;
+    cfg->n_mass_table = 1024;
     cfg->count_pairs = 0;
     cfg->kde_kernel = CHIM_KERNEL_GAUSS;
 }

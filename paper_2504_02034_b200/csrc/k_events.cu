@@ -464,7 +464,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         mlo = max(0, min(mlo, P.n_mass + 2 - mcap));
         S.mass_lo = mlo;
         S.mass_fit = (mb - ma + 3 <= mcap) ? 1 : 0;
-        const uint32_t rb = (staged && !use_poly) ? (uint32_t)(k_hi - k_lo + 1) * (uint32_t)sizeof(Row) : 0u, mbytes = (uint32_t)mcap * (uint32_t)sizeof(MassRow);
+        const uint32_t rb = (staged && !use_poly) ? (uint32_t)(k_hi - k_lo + 1) * (uint32_t)sizeof(Row) : 0u, mbytes = (uint32_t)min(mcap, mb + 3 - mlo) * (uint32_t)sizeof(MassRow);   // rows mlo .. mb + 2: what the event can address (+ margin), not the whole stage
         mbar_expect_tx(&S.mbar, rb + 2 * mbytes);
         if (rb) bulk_g2s(rows_s, tab + k_lo, rb, &S.mbar);
         bulk_g2s(mass_s, mtab + mlo, mbytes, &S.mbar);
