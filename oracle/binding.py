@@ -138,14 +138,23 @@ def kde_epanechnikov(z, w, h, zg):
     return K
 
 
+def bin_samples(z, w, n_bins):
+    """R23: equal-width bins on [min z, max z]; pseudo-samples (weighted mean z, sum of weights)."""
+    z, w = _d(z), _d(w)
+    zb, wb = np.empty(n_bins), np.empty(n_bins)
+    n = lib().chimo_bin_samples(C.c_int(z.size), _p(z), _p(w), C.c_int(n_bins), _p(zb), _p(wb))
+    return zb[:n], wb[:n]
+
+
 def event_integral(lam, zg, K, pgal, placement=PLACE_SAMPLES):
     lam, zg, K, pgal = _lam(lam), _d(zg), _d(K), _d(pgal)
     return float(lib().chimo_event_integral(_p(lam), C.c_int(placement), C.c_int(zg.size), _p(zg), _p(K), _p(pgal)))
 
 
 def event_logI(lam, dl, m1d, m2d, ln_prior, zg, pgal, placement=PLACE_SAMPLES, bw_rule=BW_SCOTT,
-               fixed_bw=float("nan"), z_table_max=10.0, kernel=KERNEL_GAUSS):
+               fixed_bw=float("nan"), z_table_max=10.0, kernel=KERNEL_GAUSS, n_bins=0):
     lib().chimo_set_kernel(C.c_int(kernel))
+    lib().chimo_set_bins(C.c_int(n_bins))
     lam, dl, m1d, m2d, lp, zg, pgal = _lam(lam), _d(dl), _d(m1d), _d(m2d), _d(ln_prior), _d(zg), _d(pgal)
     h = C.c_double(0.0)
     fl = C.c_uint32(0)
@@ -182,9 +191,10 @@ def neff(sum_s, sum_s2, n_inj_total):
 
 def loglike_batch(lam, sample_off, dl, m1d, m2d, ln_prior, grid_off, zg, pgal, *, fixed_bw=None,
                   inj=None, n_inj_total=0, placement=PLACE_SAMPLES, bw_rule=BW_SCOTT, z_cat_max=1.5,
-                  z_table_max=10.0, n_table=2048, neff_factor=5.0, kernel=KERNEL_GAUSS, group_off=None, ln_factor=None):
+                  z_table_max=10.0, n_table=2048, neff_factor=5.0, kernel=KERNEL_GAUSS, group_off=None, ln_factor=None, n_bins=0):
     """inj = (dL, m1d, m2d, ln_pdraw) of the detected set or None.  Returns a dict of arrays."""
     lib().chimo_set_kernel(C.c_int(kernel))
+    lib().chimo_set_bins(C.c_int(n_bins))
     lam = np.atleast_2d(_lam(lam))
     nl = lam.shape[0]
     so = np.ascontiguousarray(sample_off, dtype=np.int64)

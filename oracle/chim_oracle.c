@@ -411,6 +411,30 @@ void chimo_kde_epan(int n, const double *z, const double *w, double h, int ng, c
     }
 }
 
+/* Sample binning ("the weighted PE samples ... are binned" to a fixed-size dataset; no recipe given;
+ * reading R23 of DESIGN.md): n_bins equal-width bins on [min_j z_j, max_j z_j]; every bin becomes one pseudo-sample at the
+ * weighted mean redshift of its members carrying the sum of their weights (an empty bin: weight 0).  The bandwidth is the one
+ * of the ORIGINAL samples and the KDE keeps its 1/N_s, so binning approximates the unbinned estimator to O((bin width / h)^2).
+ * zb, wb: [n_bins].  Returns the number of bins written (n_bins; 1 if all z_j coincide). */
+int chimo_bin_samples(int n, const double *z, const double *w, int n_bins, double *zb, double *wb) {
+    double lo = INFINITY, hi = -INFINITY;
+    for (int j = 0; j < n; ++j) { if (z[j] < lo) lo = z[j]; if (z[j] > hi) hi = z[j]; }
+    if (!(hi > lo)) n_bins = 1;
+    double width = (hi - lo) / n_bins;
+    for (int b = 0; b < n_bins; ++b) { zb[b] = 0.0; wb[b] = 0.0; }
+    for (int j = 0; j < n; ++j) {
+        int b = (hi > lo) ? (int)((z[j] - lo) / width) : 0;
+        if (b > n_bins - 1) b = n_bins - 1;
+        wb[b] += w[j];
+        zb[b] += w[j] * (z[j] - lo);
+    }
+    for (int b = 0; b < n_bins; ++b) zb[b] = (wb[b] > 0.0) ? lo + zb[b] / wb[b] : lo + (b + 0.5) * width;
+    return n_bins;
+}
+
+static int chimo_n_bins = 0; /* 0 = no binning (default) */
+void chimo_set_bins(int n_bins) { chimo_n_bins = n_bins; }
+
 static int chimo_kernel_kind = 0; /* 0 Gaussian (default), 1 Epanechnikov: selects O8 / O8' in chimo_event_logI */
 void chimo_set_kernel(int kind) { chimo_kernel_kind = kind; }
 int chimo_get_kernel(void) { return chimo_kernel_kind; }
@@ -457,8 +481,19 @@ double chimo_event_logI(const double *lam, int placement, int bw_rule, double fi
             fl |= CHIMO_F_BW_DEGENERATE;
             logI = NAN;
         } else {
-            if (chimo_kernel_kind == 1) chimo_kde_epan(ns, z, w, h, ng, zg, K);
-            else chimo_kde(ns, z, w, h, ng, zg, K);
+            int nk = ns;
+            const double *zk = z, *wk = w;
+            double *zb = NULL, *wb = NULL;
+            if (chimo_n_bins > 0) {   /* R23: pseudo-samples; h stays the one of the original samples, 1/N_s stays */
+                zb = (double *)malloc(sizeof(double) * chimo_n_bins);
+                wb = (double *)malloc(sizeof(double) * chimo_n_bins);
+                nk = chimo_bin_samples(ns, z, w, chimo_n_bins, zb, wb);
+                zk = zb; wk = wb;
+            }
+            if (chimo_kernel_kind == 1) chimo_kde_epan(nk, zk, wk, h, ng, zg, K);
+            else chimo_kde(nk, zk, wk, h, ng, zg, K);
+            if (nk != ns) { double f = (double)nk / (double)ns; for (int g = 0; g < ng; ++g) K[g] *= f; }   /* keep 1/N_s */
+            free(zb); free(wb);
             double I = chimo_event_integral(lam, placement, ng, zg, K, pgal);
             if (I > 0.0) logI = log(I);
             else { fl |= CHIMO_F_EVENT_ZERO; logI = -INFINITY; }

@@ -546,6 +546,41 @@ def test_pcat_narrow_galaxies_reduce_to_the_gaussian_mixture_and_h0_cancels():
     assert np.allclose(O.pcat(la, zt, np.array([0.02, 0.03]), z2), O.pcat(lam(H0=35.0, Om=0.3), zt, np.array([0.02, 0.03]), z2), rtol=1e-13)
 
 
+# ------------------------------------------------------------------ sample binning (NEXT-2; reading R23)
+def test_binning_conserves_moments_and_reduces_to_the_unbinned_kde():
+    rng = np.random.default_rng(9)
+    z, w = 0.5 + 0.05 * rng.standard_normal(300), rng.random(300)
+    zb, wb = O.bin_samples(z, w, 37)
+    assert len(zb) == 37 and abs(wb.sum() - w.sum()) < 1e-12 and abs((wb * zb).sum() - (w * z).sum()) < 1e-12
+    assert np.all(np.diff(zb) > 0) and zb[0] >= z.min() and zb[-1] <= z.max()
+    edges = np.linspace(z.min(), z.max(), 38)
+    k = np.minimum(((z - z.min()) / ((z.max() - z.min()) / 37)).astype(int), 36)
+    for b in (0, 5, 36):
+        m = k == b
+        assert abs(wb[b] - w[m].sum()) < 1e-13 and abs(zb[b] - (w[m] * z[m]).sum() / w[m].sum()) < 1e-13
+        assert edges[b] - 1e-12 <= zb[b] <= edges[b + 1] + 1e-12
+    z1, w1 = O.bin_samples(z, w, 1)
+    assert abs(z1[0] - (w * z).sum() / w.sum()) < 1e-13 and abs(w1[0] - w.sum()) < 1e-12
+    # one sample per bin at most (bins far narrower than the sample spacing): the binned estimator IS the unbinned one
+    zs = np.sort(0.4 + 0.2 * rng.random(12))
+    ws = rng.random(12)
+    zb, wb = O.bin_samples(zs, ws, 200000)
+    assert np.allclose(zb[wb > 0], zs, rtol=0, atol=1e-15) and np.allclose(wb[wb > 0], ws)
+
+
+def test_binning_end_to_end_converges_quadratically_and_keeps_h_and_the_normalisation():
+    w = make_workload("tiny", n_events=3, n_samples=1500, n_grid=200, n_inj_draw=300)
+    r0 = O.loglike_workload(w)
+    err = []
+    for nb in (32, 64, 128, 256):
+        r = O.loglike_workload(w, n_bins=nb)
+        assert np.array_equal(r["h"], r0["h"]) and r["logxi"][0] == r0["logxi"][0]
+        err.append(np.max(np.abs(r["event_logI"] - r0["event_logI"])))
+    assert err[0] > err[1] > err[2] > err[3] and err[3] < 2e-3
+    assert 2.5 < err[1] / err[2] < 6.0 and 2.5 < err[2] / err[3] < 6.0          # O(bin width^2)
+    O.loglike_workload(w, lam=w.lam[:1])                                          # (leaves the oracle unbinned)
+
+
 # ------------------------------------------------------------------ flags / degenerate cases
 def test_flags_and_degenerate_cases():
     w = make_workload("tiny", n_events=2, n_samples=50, n_grid=60, n_inj_draw=200)
