@@ -103,11 +103,15 @@ typedef struct chim_config {
     int32_t n_mass_table;/* intervals of the per-lambda mass table in ln m1                           */
     int32_t count_pairs; /* 1: the KDE kernel also counts its (sample, grid point) pairs for chim_get_stats (slower)     */
     int32_t kde_kernel;  /* CHIM_KERNEL_GAUSS (default) | CHIM_KERNEL_EPANECHNIKOV (reading R19)        */
+    int32_t n_bins;      /* sample binning (reading R23): 0 = off (default, exact); > 0: per (event, lambda)
+                            the weighted samples are reduced to n_bins pseudo-samples (equal-width bins on their redshift
+                            range; weighted mean z, summed weight) before the KDE; bandwidth and 1/N_s stay those of the
+                            original samples.  An approximation, O((bin width/h)^2).  n_bins <= 2048 and <= the largest N_s  */
 } chim_config;
 
 /* Fills *cfg with the defaults: device 0, HOST, NULL stream, ON_SAMPLES, SCOTT, kde_cutoff 6.0,
  * z_cat_max 1.5, z_table_max 10, n_table 2048, n_dl_table 0 (auto), n_win_table 512, lambda_chunk 256,
- * neff_factor 5, kde_method AUTO, n_mass_table 1024, count_pairs 0, kde_kernel GAUSS. */
+ * neff_factor 5, kde_method AUTO, n_mass_table 1024, count_pairs 0, kde_kernel GAUSS, n_bins 0. */
 void chim_default_config(chim_config *cfg);
 
 /* Creates a context on cfg->device.  cfg == NULL means chim_default_config.  *out is set to NULL on error

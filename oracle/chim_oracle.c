@@ -13,13 +13,13 @@
  * CUDA path's tables are checked rather than shared.  No blocking, truncation or reordering:
  * the KDE is the full N_s x N_z sum.
  *
- * Citations are PAPER.md:<line> (section / equation).  Readings R1..R22 and the mass-model
+ * Citations are PAPER.md:<line> (section / equation).  Readings R1..R23 and the mass-model
  * reading M1..M4 are SURVEY.md sec. 8(c), restated in DESIGN.md.
  *
  * Pins (tests/test_oracle_pins.py): every function below is pinned except the *choices*
  * "bandwidth rule = Scott" (R3), "placement default = on samples" (R1), "u(z) in xi" (R6),
- * "m_low fiducial" (R11), "Epanechnikov bandwidth h_E = sqrt(5) h" (R19) and "per-pixel bandwidth of
- * many-1d" (R20), which the paper does not fix: for those, parity is unpinned by the paper and pinned only by DESIGN.md.
+ * "m_low fiducial" (R11), "Epanechnikov bandwidth h_E = sqrt(5) h" (R19), "per-pixel bandwidth of
+ * many-1d" (R20) and "binning recipe" (R23), which the paper does not fix: for those, parity is unpinned by the paper and pinned only by DESIGN.md.
  *
  * lambda layout (15 doubles): H0, Om, Xi0, n, alpha, beta, delta_m, m_low, m_high, mu_g,
  * sigma_g, lambda_g, gamma, kappa, z_p   (Table 1; m_low per R11).

@@ -30,7 +30,7 @@ class ChimConfig(C.Structure):
                 ("z_table_max", C.c_double), ("n_table", C.c_int32), ("n_dl_table", C.c_int32),
                 ("n_win_table", C.c_int32), ("lambda_chunk", C.c_int32), ("neff_factor", C.c_double),
                 ("kde_method", C.c_int32), ("n_mass_table", C.c_int32), ("count_pairs", C.c_int32),
-                ("kde_kernel", C.c_int32)]
+                ("kde_kernel", C.c_int32), ("n_bins", C.c_int32)]
 
 
 class ChimStats(C.Structure):
@@ -189,7 +189,7 @@ class Context:
     def __init__(self, device=0, stream=None, placement=CHIM_ON_SAMPLES, bw_rule=CHIM_BW_SCOTT, kde_cutoff=None,
                  z_cat_max=None, z_table_max=None, n_table=None, n_dl_table=None, n_win_table=None,
                  lambda_chunk=None, neff_factor=None, kde_method=None, n_mass_table=None, count_pairs=None,
-                 kde_kernel=None):
+                 kde_kernel=None, n_bins=None):
         import torch
         if not torch.cuda.is_available():
             raise ChimError(-3, "no CUDA device: libchim has no CPU fallback")
@@ -206,7 +206,7 @@ class Context:
         for k, v in dict(kde_cutoff=kde_cutoff, z_cat_max=z_cat_max, z_table_max=z_table_max, n_table=n_table,
                          n_dl_table=n_dl_table, n_win_table=n_win_table, lambda_chunk=lambda_chunk,
                          neff_factor=neff_factor, kde_method=kde_method, n_mass_table=n_mass_table,
-                         count_pairs=count_pairs, kde_kernel=kde_kernel).items():
+                         count_pairs=count_pairs, kde_kernel=kde_kernel, n_bins=n_bins).items():
             if v is not None:
                 setattr(cfg, k, v)
         self.cfg = cfg

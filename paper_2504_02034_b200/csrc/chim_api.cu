@@ -173,7 +173,7 @@ EventKernelParams event_params(const chim_ctx* ctx, int nl) {
     P.ev = ctx->ev;
     P.Lc = ctx->Lc; P.tab = ctx->tab_ev; P.mtab = ctx->mtab; P.dc_tab = ctx->dc_tab;
     P.n_lambda = nl; P.tab_rows = ctx->ev_grid.rows(); P.n_mass = ctx->cfg.n_mass_table; P.n_table = ctx->cfg.n_table;
-    P.placement = ctx->cfg.placement; P.bw_rule = ctx->cfg.bw_rule; P.kde_method = ctx->cfg.kde_method; P.kde_kernel = ctx->cfg.kde_kernel;
+    P.placement = ctx->cfg.placement; P.bw_rule = ctx->cfg.bw_rule; P.kde_method = ctx->cfg.kde_method; P.kde_kernel = ctx->cfg.kde_kernel; P.n_bins = ctx->cfg.n_bins;
     P.z_table_max = ctx->cfg.z_table_max; P.cutoff = ctx->cfg.kde_cutoff;
     P.logI = ctx->logI; P.flags = ctx->flags; P.stats = ctx->stats;
     P.ln_shift = ctx->ev_ln_shift;
@@ -297,6 +297,7 @@ void chim_default_config(chim_config* cfg) {
     cfg->n_mass_table = 1024;
     cfg->count_pairs = 0;
     cfg->kde_kernel = CHIM_KERNEL_GAUSS;
+    cfg->n_bins = 0;
 }
 
 int chim_version(void) { return CHIM_VERSION; }
@@ -325,6 +326,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT && c.kde_method != CHIM_KDE_POWER && c.kde_method != CHIM_KDE_NONE) return CHIM_EINVAL;
     if (c.mem != CHIM_MEM_HOST && c.mem != CHIM_MEM_DEVICE) return CHIM_EINVAL;
     if (c.kde_kernel != CHIM_KERNEL_GAUSS && c.kde_kernel != CHIM_KERNEL_EPANECHNIKOV) return CHIM_EINVAL;
+    if (c.n_bins < 0 || c.n_bins > 2048) return CHIM_EINVAL;
     if (c.kde_kernel == CHIM_KERNEL_EPANECHNIKOV && c.placement != CHIM_ON_SAMPLES) return CHIM_EINVAL;   // lambda-independent q_g needed
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device < 0 || c.device >= ndev) return CHIM_ECUDA;
@@ -379,6 +381,8 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
         max_ns = std::max<int>(max_ns, (int)ns);
         max_nz = std::max<int>(max_nz, (int)nz);
     }
+    if (ctx->cfg.n_bins > max_ns)
+        return fail(ctx, CHIM_EINVAL, "chim_init_events: cfg.n_bins exceeds the largest N_s (the pseudo-samples reuse the sample stage)");
     if (events_smem_bytes(max_ns, max_nz) > kMaxSmemOptin) {
         char b[160];
         std::snprintf(b, sizeof b, "chim_init_events: N_s = %d exceeds the shared-memory staging limit (%d samples per event)",

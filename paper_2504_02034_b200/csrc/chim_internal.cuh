@@ -418,7 +418,7 @@ struct EventKernelParams {
     const MassRow* mtab;     // [n_lambda][2][n_mass+2]
     const double* dc_tab;    // [n_lambda][n_table+1+kZPad] (placement ON_GRID only) or null
     int32_t n_lambda, tab_rows, n_mass, n_table;
-    int32_t placement, bw_rule, kde_method, kde_kernel;
+    int32_t placement, bw_rule, kde_method, kde_kernel, n_bins;
     double z_table_max, cutoff;
     double* logI;            // [n_lambda][n_events]
     uint32_t* flags;         // [n_lambda]

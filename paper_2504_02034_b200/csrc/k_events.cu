@@ -591,8 +591,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
                 const int D = (int)fD, nbox = (int)(fb_hi - fb_lo) + 1;
                 // issue-slot estimates (profiles/r01c): coefficient build 1/16 per FMA, evaluation ~1 per sample; power form
                 // 2.25 per 64 pairs.  Few samples (many-1d pixels) do not amortise the coefficient build.
-                const float le_cost = 0.0625f * (float)nbox * (float)kLeP * (2.f * fD + 1.f) + (float)ns + 150.f;
-                const float pw_cost = Bsel ? 0.035f * (float)ns * (2.f * T / delta + (float)Bsel) : INFINITY;
+                const float le_cost = 0.0625f * (float)nbox * (float)kLeP * (2.f * fD + 1.f) + (float)(P.n_bins > 0 ? P.n_bins : ns) + 150.f;
+                const float pw_cost = Bsel ? 0.035f * (float)(P.n_bins > 0 ? P.n_bins : ns) * (2.f * T / delta + (float)Bsel) : INFINITY;
                 if (le_cost <= pw_cost && le_bytes(ev_nz_pad(nz), D, nbox) <= ev_aux_bytes(P.ev.max_nz)) {
                     S.scy = scy; S.dy = dy; S.yfirst = yfirst; S.le_m = m; S.le_D = D; S.le_blo = (int)fb_lo; S.le_nbox = nbox;
                 }
@@ -618,6 +618,47 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         if (P.dbg_K) for (int g = tid; g < nz; g += kEvThreads) P.dbg_K[g] = NAN;
         return;
     }
+    int ns3 = ns;            // samples S3 works on: the pseudo-samples when binning is on
+    if (P.n_bins > 0) {
+        // Sample binning (R23): n_bins equal-width bins on [z_first, z_last] (sorted samples); a bin becomes
+        // one pseudo-sample at the weighted mean redshift of its members with the sum of their weights (empty: weight 0, bin
+        // centre).  h and 1/N_s stay those of the original samples.  The pseudo-samples overwrite zf / wl (sorted by
+        // construction); bins are accumulated in the stage with shared-memory atomics (order-dependent at the fp32 level).
+        const int nb = (zf[ns - 1] > zf[0]) ? P.n_bins : 1;
+        float* bw = reinterpret_cast<float*>(aux);
+        float* bz = bw + P.n_bins;
+        const float zlo = zf[0], width = (zf[ns - 1] - zlo) / (float)nb, inv_width = (nb > 1) ? 1.0f / width : 0.f;
+        for (int b = tid; b < nb; b += kEvThreads) { bw[b] = 0.f; bz[b] = 0.f; }
+        __syncthreads();
+        {   // every thread walks a contiguous run of the (sorted) samples and flushes a bin when the index changes:
+            // 2-3 atomics per thread instead of one per sample, and neighbours rarely meet in a bin
+            const int chunk = ((ns + kEvThreads - 1) / kEvThreads) | 1;          // odd: spreads the lanes over the banks
+            const int j0 = tid * chunk, j1 = min(j0 + chunk, ns);
+            int cur = -1;
+            float aw = 0.f, az = 0.f;
+            for (int j = j0; j < j1; ++j) {
+                const float w = wl[j], dz = zf[j] - zlo;
+                const int b = min(max((int)(dz * inv_width), 0), nb - 1);
+                if (b != cur) {
+                    if (aw > 0.f) { atomicAdd(bw + cur, aw); atomicAdd(bz + cur, az); }
+                    cur = b; aw = 0.f; az = 0.f;
+                }
+                aw += w;
+                az = fmaf(w, dz, az);
+            }
+            if (aw > 0.f) { atomicAdd(bw + cur, aw); atomicAdd(bz + cur, az); }
+        }
+        __syncthreads();
+        const int nbp = (int)ev_ns_pad(nb);
+        for (int b = tid; b < nbp; b += kEvThreads) {
+            const int bb = min(b, nb - 1);
+            const float W = bw[bb];
+            zf[b] = (W > 0.f) ? zlo + bz[bb] / W : zlo + ((float)bb + 0.5f) * width;
+            wl[b] = (b < nb) ? W : 0.f;                          // idle slots of the last pass: last pseudo-sample, weight 0
+        }
+        __syncthreads();
+        ns3 = nb;
+    }
     if (P.kde_kernel == CHIM_KERNEL_EPANECHNIKOV) {
         // Epanechnikov kernel (R19), exact on any grid without a pair loop: with the prefix sums
         // Q_k[g] = sum_{g' < g} q_g' z'^k over the event grid,
@@ -630,7 +671,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         const double* q2 = P.ev.ep_q2 + g0 + ev;
         const double zfirst = zc_g[0], idz = (udz > 0.0) ? 1.0 / udz : 0.0;
         double lsum = 0.0;
-        for (int j = tid; j < ns; j += kEvThreads) {
+        for (int j = tid; j < ns3; j += kEvThreads) {
             const double zj = (double)zf[j], lo = zj - hE, hi = zj + hE;
             int a, b;
             if (udz > 0.0) {
@@ -706,13 +747,13 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     __syncthreads();
 
     // ---- S3 + S4: warp passes over 128 consecutive (sorted) samples ----------------------------------------
-    const int n_pass = (ns + kPass - 1) / kPass;
+    const int n_pass = (ns3 + kPass - 1) / kPass;
     const float inv_delta = (udz > 0.0) ? 1.f / delta : 0.f;
     const float bd = (float)Bsel * delta, inv_bd = Bsel ? 1.f / bd : 0.f;
     const int a_max = Bsel ? nzp / Bsel - 1 : 0;
     double lsum = 0.0;                          // this lane's sum_j w_j A_j
     unsigned long long pairs_exec = 0, pairs_cut = 0;
-    if (le_nbox) lsum = le_phase<kStats>(S, LM, zf, wl, ns, nz, (float)(P.cutoff * 0.70710678118654752440), pairs_exec, pairs_cut);
+    if (le_nbox) lsum = le_phase<kStats>(S, LM, zf, wl, ns3, nz, (float)(P.cutoff * 0.70710678118654752440), pairs_exec, pairs_cut);
     else for (;;) {
         int pass = 0;
         if (lane == 0) pass = atomicAdd(&S.pass_counter, 1);

@@ -500,6 +500,35 @@ def test_build_pcat_matches_the_oracle_and_feeds_the_path(P):
     assert rel < REL_EVENT and dtot < ABS_TOTAL
 
 
+# ---------------------------------------------------------------- sample binning (NEXT-2; reading R23)
+@pytest.mark.parametrize("kernel,nb", [("gauss", 256), ("gauss", 64), ("epanechnikov", 512)])
+def test_binned_samples_match_the_binned_oracle(P, kernel, nb):
+    w = make_workload("o5_spec", n_events=6, n_samples=3000, n_grid=700, n_lambda=6, n_det=3000)
+    ok = O.KERNEL_EPANECHNIKOV if kernel == "epanechnikov" else O.KERNEL_GAUSS
+    ref = O.loglike_workload(w, kernel=ok, n_bins=nb)
+    exact = O.loglike_workload(w, kernel=ok)
+    O.loglike_workload(w, lam=w.lam[:1])                 # (leaves the oracle unbinned, Gaussian)
+    r = _gpu(P, w, count_pairs=0, n_bins=nb, kde_kernel=P.CHIM_KERNEL_EPANECHNIKOV if kernel == "epanechnikov" else P.CHIM_KERNEL_GAUSS)
+    rel, dtot, _ = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    # a sample within fp32 rounding of a bin edge may sit in the neighbouring bin: the effect is far below the binning error
+    assert np.max(np.abs(r["event_logI"] - ref["event_logI"])) < 2e-5
+    if nb <= 64:      # coarse bins: the approximation itself is visible, the parity error is not
+        assert np.max(np.abs(ref["event_logI"] - exact["event_logI"])) > 10 * np.max(np.abs(r["event_logI"] - ref["event_logI"]))
+
+
+def test_binning_argument_checks(P):
+    w = make_workload("tiny", n_events=2, n_samples=100, n_grid=50, n_inj_draw=100)
+    cfg = P.chim_default_config()
+    cfg.n_bins = 4096
+    with pytest.raises(P.ChimError):
+        P.chim_create(cfg)
+    c = P.Context(n_bins=512)
+    with pytest.raises(P.ChimError):                      # more bins than samples
+        c.init_workload(w)
+    c.close()
+
+
 def test_kde_nonuniform_grid_takes_the_direct_form(P):
     # R14: any strictly increasing grid; the trapezoid uses the true spacings
     w = make_workload("o5_spec", n_events=5, n_samples=1500, n_grid=400, n_lambda=6, n_det=3000)
