@@ -108,6 +108,8 @@ struct EvSmem {
     int le_m, le_D, le_blo, le_nbox;   // grid points per box, half-width of the psi table, first box, number of boxes
     // event-local polynomials of S2 (use_poly != 0): z - z0 [7], ln(1+z) [7], 1/(1+z) [7], smooth log2 factor [7]
     alignas(16) float poly[4 * kPolyN];
+    // lambda-independent scalars of the event, fetched once beside the constants (one L2 latency instead of one per use)
+    double ev_udz, ev_zfirst, ev_ln_out;   // grid spacing (0: not equally spaced), first centred grid point, ln_shift + ln_qscale
 };
 
 __host__ __device__ inline size_t ev_ns_pad(size_t ns) { return (ns + kPass - 1) / kPass * kPass; }
@@ -440,6 +442,10 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             S.pass_counter = 0;
             mbar_init(&S.mbar, 1);
         }
+        if (tid == 32) {
+            const double a = P.ev.uni_dz[ev], b = P.ev.zc[g0], c = P.ln_shift[ev], d = P.ln_qscale[ev];
+            S.ev_udz = a; S.ev_zfirst = b; S.ev_ln_out = c + d;
+        }
     }
     __syncthreads();
     const LamConst& L = S.L;
@@ -545,7 +551,14 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     __syncthreads();
     const double* zc_g = P.ev.zc + g0;
     const float* qn_g = P.ev.qn + g0;
-    const double udz = P.ev.uni_dz[ev];
+    // q_g of the first 1024 grid points: requested now, consumed after the bandwidth step (their L2 latency hides behind it)
+    float qpre[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int g = tid + k * kEvThreads;
+        qpre[k] = (g < nz) ? __ldg(qn_g + g) : 0.f;
+    }
+    const double udz = S.ev_udz;
     const float T = (P.cutoff > 0.0) ? (float)(P.cutoff * sqrt(kHalfLog2e)) : INFINITY;
     if (tid == 0) {   // one thread: fp64 sums over the warps, bandwidth, and every scalar the pair loop needs
         double mom[4];
@@ -575,7 +588,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             if (delta * 32.f <= 3.3f) Bsel = 32;
             else if (delta * 16.f <= kMaxBlockSpan) Bsel = 16;
         }
-        S.h = h; S.scd = scd; S.scf = scf; S.delta = delta; S.xfirst = (float)(zc_g[0] * scd); S.Bsel = Bsel;
+        S.h = h; S.scd = scd; S.scf = scf; S.delta = delta; S.xfirst = (float)(S.ev_zfirst * scd); S.Bsel = Bsel;
         // local-expansion form: equally spaced grid, a cut-off, boxes of ~1 unit of y = z'/(sqrt(2) h) that fit the stage
         S.le_nbox = 0; S.le_D = 0;
         if (udz > 0.0 && T < INFINITY && P.kde_method == CHIM_KDE_AUTO && !P.dbg_K && h > 0.0 && isfinite(h)) {
@@ -583,7 +596,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             const float dy = (float)(udz * (double)scy);
             const int m = max(1, (int)lrintf(1.0f / dy));
             const float wbox = (float)m * dy, Ty = (float)(P.cutoff * 0.70710678118654752440);
-            const float yfirst = (float)(zc_g[0] * (double)scy);
+            const float yfirst = (float)(S.ev_zfirst * (double)scy);
             const float fb_lo = floorf((zf[0] * scy - yfirst) / wbox + 0.5f), fb_hi = floorf((zf[ns - 1] * scy - yfirst) / wbox + 0.5f);
             const float fD = ceilf((Ty + 0.5f * wbox) / dy) + 1.0f;
             if (wbox <= kLeMaxW && fb_hi - fb_lo < (float)kLeMaxBox && fabsf(fb_lo) < 1e6f && fabsf(fb_hi) < 1e6f && fD < 1e5f &&
@@ -669,7 +682,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         const double* q0 = P.ev.ep_q0 + g0 + ev;
         const double* q1 = P.ev.ep_q1 + g0 + ev;
         const double* q2 = P.ev.ep_q2 + g0 + ev;
-        const double zfirst = zc_g[0], idz = (udz > 0.0) ? 1.0 / udz : 0.0;
+        const double zfirst = S.ev_zfirst, idz = (udz > 0.0) ? 1.0 / udz : 0.0;
         double lsum = 0.0;
         for (int j = tid; j < ns3; j += kEvThreads) {
             const double zj = (double)zf[j], lo = zj - hE, hi = zj + hE;
@@ -696,7 +709,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         if (P.dbg_K) for (int g = tid; g < nz; g += kEvThreads) P.dbg_K[g] = NAN;
         if (tid == 0) {
             const double I = t1[0] * 0.75 / ((double)ns * hE);
-            if (I > 0.0) *out = log(I) + (double)mx * 0.69314718055994530942 + P.ln_shift[ev] + P.ln_qscale[ev];
+            if (I > 0.0) *out = log(I) + (double)mx * 0.69314718055994530942 + S.ev_ln_out;
             else if (I == 0.0) { *out = -INFINITY; atomicOr(P.flags + l, CHIM_FLAG_EVENT_ZERO); }
             else *out = NAN;
         }
@@ -709,7 +722,18 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     const int le_nbox = S.le_nbox;
     LeSmem LM = le_layout(aux, (size_t)nzp, S.le_D, le_nbox);
     if (le_nbox) {            // local-expansion form: plain q_g (x grid factor)
-        for (int g = tid; g < nzp; g += kEvThreads) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {           // the prefetched part
+            const int g = tid + k * kEvThreads;
+            if (g < nzp) {
+                float q = qpre[k];
+                if (on_grid && g < nz)
+                    q = (float)((double)q * grid_factor(L, P.dc_tab + (size_t)l * (P.n_table + 1 + kZPad), P.n_table + 1 + kZPad,
+                                                        P.z_table_max / P.n_table, zc_g[g] + z0));
+                LM.qs[g] = q;
+            }
+        }
+        for (int g = tid + 4 * kEvThreads; g < nzp; g += kEvThreads) {
             float q = 0.f;
             if (g < nz) {
                 q = qn_g[g];
@@ -869,7 +893,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     }
     if (tid == 0) {
         double I = tot[0] * knorm;
-        if (I > 0.0) *out = log(I) + ln_wscale + P.ln_shift[ev] + P.ln_qscale[ev];
+        if (I > 0.0) *out = log(I) + ln_wscale + S.ev_ln_out;
         else if (I == 0.0) { *out = -INFINITY; atomicOr(P.flags + l, CHIM_FLAG_EVENT_ZERO); }
         else *out = NAN;
     }
