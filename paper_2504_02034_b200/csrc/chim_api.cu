@@ -210,10 +210,11 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
     {   // local-polynomial fits (part of S1: per-lambda interpolants)
         Bracket b(ctx, 0);
         CK(launch_polyfit(ctx->Lc, ctx->tab_ev, ctx->ev_grid.rows(), nl, ctx->ev.n_events, ctx->ev.tk_c, ctx->ev.tk_h, ctx->ev.z0, 0.0,
-                          false, ctx->poly_mats, ctx->poly_ev, st));
+                          false, ctx->poly_mats, ctx->ev.lnm1_lo, ctx->ev.lnm1_hi, ctx->cfg.n_mass_table,
+                          events_mass_stage_rows(ctx->cfg.n_mass_table), ctx->poly_ev, st));
         if (ctx->have_inj)
             CK(launch_polyfit(ctx->Lc, ctx->tab_inj, ctx->inj_grid.rows(), nl, ctx->inj_blocks, ctx->inj.tk_c, ctx->inj.tk_h, nullptr,
-                              ctx->cfg.z_cat_max, true, ctx->poly_mats, ctx->poly_inj, st));
+                              ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->poly_inj, st));
         ctx->launches += ctx->have_inj ? 2 : 1;
     }
     EventKernelParams EP = event_params(ctx, nl);
@@ -827,10 +828,11 @@ static int debug_prepare(chim_ctx* ctx, const double* lambda, const char* who) {
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t), ctx->stream));
     CK(launch_tables(lambda, 1, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, ctx->stream));
     CK(launch_polyfit(ctx->Lc, ctx->tab_ev, ctx->ev_grid.rows(), 1, ctx->ev.n_events, ctx->ev.tk_c, ctx->ev.tk_h, ctx->ev.z0, 0.0, false,
-                      ctx->poly_mats, ctx->poly_ev, ctx->stream));
+                      ctx->poly_mats, ctx->ev.lnm1_lo, ctx->ev.lnm1_hi, ctx->cfg.n_mass_table,
+                      events_mass_stage_rows(ctx->cfg.n_mass_table), ctx->poly_ev, ctx->stream));
     if (ctx->have_inj)
         CK(launch_polyfit(ctx->Lc, ctx->tab_inj, ctx->inj_grid.rows(), 1, ctx->inj_blocks, ctx->inj.tk_c, ctx->inj.tk_h, nullptr,
-                          ctx->cfg.z_cat_max, true, ctx->poly_mats, ctx->poly_inj, ctx->stream));
+                          ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->poly_inj, ctx->stream));
     return CHIM_OK;
 }
 

@@ -474,7 +474,8 @@ cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P,
 
 cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int n_lambda, int n_ranges, const double* tk_c,
                            const double* tk_h, const double* z_ref, double z_ref_const, bool is_inj, const double* pm,
-                           float* out, cudaStream_t st);
+                           const double* lnm1_lo, const double* lnm1_hi, int n_mass, int mcap, float* out, cudaStream_t st);
+int events_mass_stage_rows(int n_mass);   // rows of the mass table a k_events CTA stages per variant
 cudaError_t launch_events(const EventKernelParams& P, bool count_pairs, cudaStream_t st);
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st);
 cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);

@@ -99,7 +99,7 @@ struct EvSmem {
     float fred[kEvThreads / 32];
     unsigned long long mbar;
     int pass_counter;
-    int mass_lo, mass_fit;
+    int mass_lo, mass_fit, early_tma;
     double h, scd;            // bandwidth and the coordinate scale (as the rounded float, widened)
     float scf, delta, xfirst; // scale, grid spacing and first grid point in scaled coordinates
     int Bsel;                 // block size of the power form, 0 = direct form
@@ -441,6 +441,22 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         if (tid == 0) {
             S.pass_counter = 0;
             mbar_init(&S.mbar, 1);
+            // polynomial path: the stage bounds were computed by k_polyfit, so the TMA copy of the mass rows starts now and
+            // runs beside the staging of the constants (the same test as use_poly below, on the global copy of the constants)
+            const double h0 = P.ev.tk_h[ev], c0 = P.ev.tk_c[ev];
+            const float* pr = P.poly + ((size_t)l * P.ev.n_events + ev) * (4 * kPolyN);
+            int early = 0;
+            if (h0 > 0.0 && P.Lc[l].flags == 0 && c0 + h0 < P.Lc[l].tkmax_ev) {
+                const int mlo = __float_as_int(__ldg(pr + 26)), nr = __float_as_int(__ldg(pr + 27));
+                const uint32_t mbytes = (uint32_t)abs(nr) * (uint32_t)sizeof(MassRow);
+                S.mass_lo = mlo;
+                S.mass_fit = nr > 0 ? 1 : 0;
+                mbar_expect_tx(&S.mbar, 2 * mbytes);
+                bulk_g2s(mass_s, mtab + mlo, mbytes, &S.mbar);
+                bulk_g2s(mass_s + mcap, mtab + (P.n_mass + 2) + mlo, mbytes, &S.mbar);
+                early = 1;
+            }
+            S.early_tma = early;
         }
         if (tid == 32) {
             const double a = P.ev.uni_dz[ev], b = P.ev.zc[g0], c = P.ln_shift[ev], d = P.ln_qscale[ev];
@@ -462,7 +478,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     // ---- TMA: the event's slice of the z(ln d_L) table and the mass-table rows it can address: ln m1 = ln m1d - ln(1+z),
     //      z between the event's first and last (sorted) sample; rows outside the staged range fall back to global
     //      memory inside sample_eval ----------------------------------------------------------------------------
-    if (tid == 0) {
+    if (tid == 0 && !S.early_tma) {
         const float u_lo = tab[k_lo].u0, u_hi = tab[min(k_hi + 1, P.tab_rows - 1)].u0;   // ln(1+z) at the bracketing nodes
         const int ma = max(1, min((int)fma(P.ev.lnm1_lo[ev] - (double)u_hi - L.lm0, L.inv_dlm, 1.0), P.n_mass));
         const int mb = max(1, min((int)fma(P.ev.lnm1_hi[ev] - (double)u_lo - L.lm0, L.inv_dlm, 1.0), P.n_mass));
@@ -898,6 +914,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         else *out = NAN;
     }
 }
+
+int events_mass_stage_rows(int n_mass) { return min(kMassStage, n_mass + 2); }
 
 size_t events_smem_bytes(int max_ns, int max_nz) {
     return ((sizeof(EvSmem) + 127) / 128) * 128 + 2 * sizeof(float) * ev_ns_pad((size_t)max_ns) + ev_aux_bytes((size_t)max_nz);

@@ -493,24 +493,46 @@ __global__ void __launch_bounds__(256) k_polyfit(const LamConst* __restrict__ Lc
                                                  int n_lambda, int n_ranges, const double* __restrict__ tk_c,
                                                  const double* __restrict__ tk_h, const double* __restrict__ z_ref,
                                                  double z_ref_const, int is_inj, const double* __restrict__ pm,
-                                                 float* __restrict__ out) {
+                                                 const double* __restrict__ lnm1_lo, const double* __restrict__ lnm1_hi,
+                                                 int n_mass, int mcap, float* __restrict__ out) {
     const long long item = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (item >= (long long)n_lambda * n_ranges) return;
     const int l = (int)(item % n_lambda), r = (int)(item / n_lambda);
     const LamConst& L = Lc[l];
     const double h = tk_h[r], c = tk_c[r];
     if (L.flags || !(h > 0.0) || !(c + h < (is_inj ? L.tkmax_inj : L.tkmax_ev))) return;
-    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, is_inj || L.F.gk2 != 0.f, pm,
-              out + ((size_t)l * n_ranges + r) * (4 * kPolyN));
+    float* o = out + ((size_t)l * n_ranges + r) * (4 * kPolyN);
+    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, is_inj || L.F.gk2 != 0.f, pm, o);
+    if (lnm1_lo) {
+        // k_events: the rows of the mass table the event can address, ln m1 = ln m1d - u, u = ln(1+z) between the ends of the
+        // event's range (the fitted polynomial at t = -1, +1), so that the CTA can issue its TMA copy at once.  Slots 26, 27 of
+        // the record (the unused degree-6 terms of u and a): first staged row, and the row count (negative: does not fit)
+        __syncwarp();
+        const int lane = threadIdx.x & 31;
+        const float cu = (lane < kPolyN - 1) ? o[2 * kPolyN + 2 * lane] : 0.f;          // u_n
+        float up = cu, um = (lane & 1) ? -cu : cu;
+#pragma unroll
+        for (int k = 16; k > 0; k >>= 1) { up += __shfl_xor_sync(0xffffffffu, up, k); um += __shfl_xor_sync(0xffffffffu, um, k); }
+        if (lane == 0) {
+            const double u_lo = fmin((double)um, (double)up) - 1e-4, u_hi = fmax((double)um, (double)up) + 1e-4;
+            const int ma = max(1, min((int)fma(lnm1_lo[r] - u_hi - L.lm0, L.inv_dlm, 1.0), n_mass));
+            const int mb = max(1, min((int)fma(lnm1_hi[r] - u_lo - L.lm0, L.inv_dlm, 1.0), n_mass));
+            int mlo = ma - 1 + max(0, (mb - ma + 3 - mcap) / 2);                          // wider than the stage: keep the centre
+            mlo = max(0, min(mlo, n_mass + 2 - mcap));
+            const int nrow = min(mcap, mb + 3 - mlo);
+            o[26] = __int_as_float(mlo);
+            o[27] = __int_as_float((mb - ma + 3 <= mcap) ? nrow : -nrow);
+        }
+    }
 }
 
 cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int n_lambda, int n_ranges, const double* tk_c,
                            const double* tk_h, const double* z_ref, double z_ref_const, bool is_inj, const double* pm,
-                           float* out, cudaStream_t st) {
+                           const double* lnm1_lo, const double* lnm1_hi, int n_mass, int mcap, float* out, cudaStream_t st) {
     const long long items = (long long)n_lambda * n_ranges;
     if (items <= 0) return cudaSuccess;
     k_polyfit<<<(unsigned)((items + 7) / 8), 256, 0, st>>>(Lc, tab, tab_rows, n_lambda, n_ranges, tk_c, tk_h, z_ref, z_ref_const,
-                                                            is_inj ? 1 : 0, pm, out);
+                                                            is_inj ? 1 : 0, pm, lnm1_lo, lnm1_hi, n_mass, mcap, out);
     return cudaGetLastError();
 }
 
