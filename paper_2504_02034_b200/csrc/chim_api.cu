@@ -422,8 +422,9 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     // event padded to a multiple of 32 samples with copies of its last one (whole warps read without bounds checks)
     std::vector<int64_t> poff(n_events + 1, 0);
     for (int i = 0; i < n_events; ++i) poff[i + 1] = poff[i] + ((so[i + 1] - so[i] + 31) / 32) * 32;
-    std::vector<float4> prec_a((size_t)poff[n_events]);
-    std::vector<float2> prec_b((size_t)poff[n_events]);
+    constexpr size_t kRecTail = 1024;   // spare records: the sweeps prefetch one iteration (256 records) past their range
+    std::vector<float4> prec_a((size_t)poff[n_events] + kRecTail, make_float4(0.f, 1.f, 1.f, 0.f));
+    std::vector<float2> prec_b((size_t)poff[n_events] + kRecTail, make_float2(0.f, 0.f));
     std::vector<int32_t> k_lo(n_events), k_hi(n_events);
     const double l2e = 1.4426950408889634074;
     std::vector<int32_t> perm(NS);
@@ -660,8 +661,8 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     }
     // chunk-local polynomials of k_inject: the set is sorted in d_L, so a chunk of kInjChunk injections spans a narrow range
     const int n_chunks = (int)((n_det + kInjChunk - 1) / kInjChunk);
-    std::vector<float4> prec_a((size_t)n_chunks * kInjChunk);
-    std::vector<float2> prec_b((size_t)n_chunks * kInjChunk);
+    std::vector<float4> prec_a((size_t)n_chunks * kInjChunk + 1024, make_float4(0.f, 1.f, 1.f, 0.f));   // + spare tail (prefetch)
+    std::vector<float2> prec_b((size_t)n_chunks * kInjChunk + 1024, make_float2(0.f, 0.f));
     std::vector<double> ctk_c(n_chunks), ctk_h(n_chunks);
     for (int c = 0; c < n_chunks; ++c) {
         const size_t a = (size_t)c * kInjChunk, b = std::min<size_t>(a + kInjChunk, N);

@@ -386,15 +386,14 @@ __device__ __forceinline__ float s2_sweep_poly(const float4* __restrict__ pa, co
     const float tm_hi = kFit ? fminf(F.tm_max, (float)(M.lo + M.cap) - 0.01f) : F.tm_max;
     pa += tid;
     pb += tid;
-    PRec R;
-    if (tid < ns32) R = ldg_stream_prec(pa, pb);
+    PRec R = ldg_stream_prec(pa, pb);                // unconditional: the record arrays carry a tail of 2 x 256 spare records
 #pragma unroll 2
     for (int j = tid; j < ns32; j += kEvThreads) {
         const float4 A = R.A;
         const float2 Bq = R.B;
         pa += kEvThreads;
         pb += kEvThreads;
-        if (j + kEvThreads < ns32) R = ldg_stream_prec(pa, pb);
+        R = ldg_stream_prec(pa, pb);                 // one iteration ahead (past the event: read and dropped)
         float zc, l2w;
         poly_sample<kFit>(F, F.gk2, F.cpsi, C, A, Bq, M, tm_lo, tm_hi, zc, l2w);
         if (j < ns) {

@@ -84,15 +84,14 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
         const float2* pb = P.inj.prec_b + j0 + tid;
         const int n = (int)(j1 - j0), n32 = (n + 31) & ~31;
         const float tm_hi = F.tm_max;
-        PRec R;
-        if (tid < n32) R = ldg_stream_prec(pa, pb);
+        PRec R = ldg_stream_prec(pa, pb);                    // unconditional: the record arrays carry a tail of spare records
 #pragma unroll 2
         for (int j = tid; j < n32; j += kInjThreads) {
             const float4 A = R.A;
             const float2 Bq = R.B;
             pa += kInjThreads;
             pb += kInjThreads;
-            if (j + kInjThreads < n32) R = ldg_stream_prec(pa, pb);
+            R = ldg_stream_prec(pa, pb);                     // one iteration ahead (past the chunk: read and dropped)
             float zc, l2w;
             poly_sample<true>(F, F.gk2_inj, F.cpsi_inj, C, A, Bq, M, 1.0f, tm_hi, zc, l2w);
             const double s = (zc <= 0.f && j < n) ? ex2_to_double(l2w) : 0.0;
