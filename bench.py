@@ -305,7 +305,7 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": t_dev_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32 (sample weights with hi+lo pairs, KDE pair loop) + f64 (tables, reductions)", "data": "synthetic",
+            "dtype": "f32 (sample weights, KDE) + f64 (tables, fits, reductions)", "data": "synthetic",
             "config": workload_config(w, args),
             "kde_pairs_per_s_dense_equivalent": st["kde_pairs_dense"] * K * world / t_dev_max,
             "kde_pairs_per_s_evaluated": pairs_eval * world / t_dev_max,
