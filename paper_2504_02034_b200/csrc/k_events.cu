@@ -235,35 +235,36 @@ __device__ double le_phase(const EvSmem& S, const LeSmem& M, const float* __rest
         if (neg) { d0 = max(d0, gc - (nz - 1)); d1 = min(d1, gc); }
         else { d0 = max(d0, -gc); d1 = min(d1, nz - 1 - gc); }
         if (!valid) d1 = d0 - 1;
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        f32x2 axy = 0ull, azw = 0ull;      // (+0.f, +0.f): accumulators of n = 4 quad + {0, 1} and + {2, 3}, packed for FFMA2
         const float* qp = M.qs + gc + (neg ? -d0 : d0);
         const int qstep = neg ? -1 : 1;
-        const float4* pp = reinterpret_cast<const float4*>(M.psi) + quad + d0 * (kLeP / 4);
+        const ulonglong2* pp = reinterpret_cast<const ulonglong2*>(M.psi) + quad + d0 * (kLeP / 4);
         int n = d1 - d0 + 1;
 #pragma unroll 1
         for (; n >= 4; n -= 4) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const float q = qp[k * qstep];
-                const float4 v = pp[k * (kLeP / 4)];
-                acc.x = fmaf(q, v.x, acc.x);
-                acc.y = fmaf(q, v.y, acc.y);
-                acc.z = fmaf(q, v.z, acc.z);
-                acc.w = fmaf(q, v.w, acc.w);
+                const ulonglong2 v = pp[k * (kLeP / 4)];
+                const f32x2 q2 = pack2(q, q);
+                axy = fma2(q2, v.x, axy);
+                azw = fma2(q2, v.y, azw);
             }
             qp += 4 * qstep;
             pp += 4 * (kLeP / 4);
         }
         for (; n > 0; --n) {
             const float q = *qp;
-            const float4 v = *pp;
-            acc.x = fmaf(q, v.x, acc.x);
-            acc.y = fmaf(q, v.y, acc.y);
-            acc.z = fmaf(q, v.z, acc.z);
-            acc.w = fmaf(q, v.w, acc.w);
+            const ulonglong2 v = *pp;
+            const f32x2 q2 = pack2(q, q);
+            axy = fma2(q2, v.x, axy);
+            azw = fma2(q2, v.y, azw);
             qp += qstep;
             pp += kLeP / 4;
         }
+        float4 acc;
+        unpack2(axy, acc.x, acc.y);
+        unpack2(azw, acc.z, acc.w);
         if (neg) { acc.y = -acc.y; acc.w = -acc.w; }   // psi_n(-t) = (-1)^n psi_n(t); n = 4 quad + {0,1,2,3}
 #pragma unroll
         for (int o = 1; o <= 2; o <<= 1) {
