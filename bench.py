@@ -34,6 +34,14 @@ ORACLE_KERNEL = [0, 0]        # oracle kernel id and bin count of the timed orac
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
+NCU_TRAFFIC_BYTES = 56.63e6 + 2.69e6   # k_events, O5-spectroscopic, 256-lambda launch (profiles/r01e)
+
+
+def default_workload(args):
+    return (args.config == "o5_spec" and args.catalog == 0 and not (args.n_events or args.n_det or args.n_lambda)
+            and args.pixels == 0 and args.bins == 0 and args.kde_kernel == "gauss" and args.lambda_chunk == 256)
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -319,7 +327,12 @@ def run_ours(args):
                          "achieved": achieved, "peak": peak_g, "unit": "G pairs/s (1 fp32 FMA lane-op per Gaussian pair)",
                          "frac": achieved / peak_g, "frac_at_sampled_clock": achieved / (peak_g * clk_run / clk_max),
                          "achieved_executed": executed, "frac_executed": executed / peak_g,
-                         "traffic": None, "algorithmic_ops_per_launch": pairs_cut / n_launch,
+                         # DRAM bytes per k_events launch from the committed ncu --set full capture of this workload
+                         # (dram__bytes_read.sum + dram__bytes_write.sum); not measurable from inside bench.py
+                         "traffic": (NCU_TRAFFIC_BYTES if default_workload(args) else None),
+                         "traffic_source": ("profiles/r01e_k_events_k_inject_ncu_full.md" if default_workload(args) else None),
+                         "algorithmic_bytes_per_launch": 24 * int(w.sample_off[-1]) * min(w.n_lambda, args.lambda_chunk),
+                         "algorithmic_ops_per_launch": pairs_cut / n_launch,
                          "executed_ops_per_launch": pairs_eval / n_launch,
                          "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
                          "kde_phase": (None if ev_ms_s2 is None else {
