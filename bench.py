@@ -331,7 +331,8 @@ def run_ours(args):
                          # (dram__bytes_read.sum + dram__bytes_write.sum); not measurable from inside bench.py
                          "traffic": (NCU_TRAFFIC_BYTES if default_workload(args) else None),
                          "traffic_source": ("profiles/r01e_k_events_k_inject_ncu_full.md" if default_workload(args) else None),
-                         "algorithmic_bytes_per_launch": 24 * int(w.sample_off[-1]) * min(w.n_lambda, args.lambda_chunk),
+                         # what a launch must bring from HBM once (records, 24 B per sample; the lambdas of a chunk share them in L2)
+                         "algorithmic_dram_bytes_per_launch": 24 * int(w.sample_off[-1]),
                          "algorithmic_ops_per_launch": pairs_cut / n_launch,
                          "executed_ops_per_launch": pairs_eval / n_launch,
                          "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
