@@ -24,6 +24,7 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(_build.build())
         _lib.chimo_scott_bw.restype = C.c_double
+        _lib.chimo_scott_bw_log.restype = C.c_double
         _lib.chimo_event_integral.restype = C.c_double
         _lib.chimo_event_logI.restype = C.c_double
         _lib.chimo_neff.restype = C.c_double
@@ -102,6 +103,27 @@ def mass_pdf(lam, m1, m2):
     return o
 
 
+def ln_smoothing(lam, m):
+    lam, m = _lam(lam), _d(np.atleast_1d(m))
+    o = np.empty_like(m)
+    lib().chimo_ln_smoothing(_p(lam), C.c_int(m.size), _p(m), _p(o))
+    return o
+
+
+def ln_p_m2_given_m1(lam, m1, m2):
+    lam, m1, m2 = _lam(lam), _d(np.atleast_1d(m1)), _d(np.atleast_1d(m2))
+    o = np.empty_like(m1)
+    lib().chimo_ln_p_m2_given_m1(_p(lam), C.c_int(m1.size), _p(m1), _p(m2), _p(o))
+    return o
+
+
+def ln_mass_pdf(lam, m1, m2):
+    lam, m1, m2 = _lam(lam), _d(np.atleast_1d(m1)), _d(np.atleast_1d(m2))
+    o = np.empty_like(m1)
+    lib().chimo_ln_mass_pdf(_p(lam), C.c_int(m1.size), _p(m1), _p(m2), _p(o))
+    return o
+
+
 def psi(lam, z):
     lam, z = _lam(lam), _d(np.atleast_1d(z))
     o = np.empty_like(z)
@@ -116,6 +138,22 @@ def sample_weights(lam, dl, m1d, m2d, ln_prior, placement=PLACE_SAMPLES, z_table
     lib().chimo_sample_weights(_p(lam), C.c_int(placement), C.c_double(z_table_max), C.c_int(dl.size),
                                _p(dl), _p(m1d), _p(m2d), _p(lp), _p(z), _p(w), C.byref(rf))
     return z, w, bool(rf.value)
+
+
+def sample_log_weights(lam, dl, m1d, m2d, ln_prior, placement=PLACE_SAMPLES, z_table_max=10.0):
+    """O6 in log space: (z_j, ln w_j, range flag); ln w = -inf where the weight is 0."""
+    lam, dl, m1d, m2d, lp = _lam(lam), _d(dl), _d(m1d), _d(m2d), _d(ln_prior)
+    z, lw = np.empty_like(dl), np.empty_like(dl)
+    rf = C.c_int(0)
+    lib().chimo_sample_log_weights(_p(lam), C.c_int(placement), C.c_double(z_table_max), C.c_int(dl.size),
+                                   _p(dl), _p(m1d), _p(m2d), _p(lp), _p(z), _p(lw), C.byref(rf))
+    return z, lw, bool(rf.value)
+
+
+def scott_bw_log(z, lw):
+    """O7 from log weights (the form the event path uses)."""
+    z, lw = _d(z), _d(lw)
+    return float(lib().chimo_scott_bw_log(C.c_int(z.size), _p(z), _p(lw)))
 
 
 def scott_bw(z, w):

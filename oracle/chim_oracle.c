@@ -19,7 +19,7 @@
  * Pins (tests/test_oracle_pins.py): every function below is pinned except the *choices*
  * "bandwidth rule = Scott" (R3), "placement default = on samples" (R1), "u(z) in xi" (R6),
  * "m_low fiducial" (R11), "Epanechnikov bandwidth h_E = sqrt(5) h" (R19), "per-pixel bandwidth of
- * many-1d" (R20) and "binning recipe" (R23), which the paper does not fix: for those, parity is unpinned by the paper and pinned only by DESIGN.md.
+ * many-1d" (R20), "binning recipe" (R23) and "sparse pixels are left out" (R24), which the paper does not fix: for those, parity is unpinned by the paper and pinned only by DESIGN.md.
  *
  * lambda layout (15 doubles): H0, Om, Xi0, n, alpha, beta, delta_m, m_low, m_high, mu_g,
  * sigma_g, lambda_g, gamma, kappa, z_p   (Table 1; m_low per R11).
@@ -226,34 +226,49 @@ void chimo_z_of_dl(const double *lam, double z_table_max, int n, const double *d
 }
 
 /* --------------------------------------------------------------------- O4 mass function ----- */
-/* M1: low-mass smoothing S(m) (PAPER.md:198 "smoothed using delta_m"; form: the published
- * power-law+peak definition the paper cites at :224) */
-static double smooth_S(double m, const lam_t *L) {
-    if (m < L->m_low) return 0.0;
-    if (m >= L->m_low + L->delta_m) return 1.0;
-    double mp = m - L->m_low;
-    if (mp <= 0.0) return 0.0;
-    double f = L->delta_m / mp + L->delta_m / (mp - L->delta_m);
-    return 1.0 / (1.0 + exp(f)); /* exp(+inf) = inf -> 0 ; exp(-inf) = 0 -> 1 */
+/* The mass function is evaluated in LOG space (ln S, ln p(m1), ln C, ln p(m1,m2)) and the linear-valued functions the
+ * pins call are exp() of these: deep in the smoothing window S(m) = e^(-delta/m') leaves the fp64 range (m' < delta/709)
+ * although ln S is an ordinary number, and an event whose only supported samples sit there has a well-defined log I
+ * (R21: with linear weights the oracle used to return I = 0 there -- an fp64 artefact, not the definition). */
+static double logaddexp(double a, double b) {
+    if (a == -INFINITY) return b;
+    if (b == -INFINITY) return a;
+    double mx = a > b ? a : b, mn = a > b ? b : a;
+    return mx + log1p(exp(mn - mx));
 }
+/* M1: low-mass smoothing S(m) (PAPER.md:198 "smoothed using delta_m"; form: the published
+ * power-law+peak definition the paper cites at :224):  S = 1/(1 + e^f), f = delta/m' + delta/(m' - delta), m' = m - m_low;
+ * ln S = -ln(1 + e^f) = -f - ln(1 + e^-f) for f > 0. */
+static double ln_smooth_S(double m, const lam_t *L) {
+    if (m < L->m_low) return -INFINITY;
+    if (m >= L->m_low + L->delta_m) return 0.0;
+    double mp = m - L->m_low;
+    if (mp <= 0.0) return -INFINITY;
+    double f = L->delta_m / mp + L->delta_m / (mp - L->delta_m);
+    return (f > 0.0) ? -(f + log1p(exp(-f))) : -log1p(exp(f));
+}
+static double smooth_S(double m, const lam_t *L) { return exp(ln_smooth_S(m, L)); }
 /* normalised truncated power law m^-alpha on [m_low, m_high] (closed interval, R15) */
-static double powerlaw_pdf(double m, const lam_t *L) {
-    if (m < L->m_low || m > L->m_high) return 0.0;
+static double ln_powerlaw_pdf(double m, const lam_t *L) {
+    if (m < L->m_low || m > L->m_high) return -INFINITY;
     double norm;
     if (fabs(L->alpha - 1.0) < 1e-12) norm = log(L->m_high / L->m_low);
     else norm = (pow(L->m_high, 1.0 - L->alpha) - pow(L->m_low, 1.0 - L->alpha)) / (1.0 - L->alpha);
-    return pow(m, -L->alpha) / norm;
+    return -L->alpha * log(m) - log(norm);
 }
-static double gauss_pdf(double m, double mu, double sig) {
+static double ln_gauss_pdf(double m, double mu, double sig) {
     double d = (m - mu) / sig;
-    return exp(-0.5 * d * d) / (sig * sqrt(2.0 * M_PI));
+    return -0.5 * d * d - log(sig * sqrt(2.0 * M_PI));
 }
 /* M2: un-normalised primary density [ (1-lg) PL + lg N ] S */
-static double p1_unnorm(double m, const void *ctx) {
-    const lam_t *L = (const lam_t *)ctx;
-    return ((1.0 - L->lambda_g) * powerlaw_pdf(m, L) + L->lambda_g * gauss_pdf(m, L->mu_g, L->sigma_g)) *
-           smooth_S(m, L);
+static double ln_p1_unnorm(double m, const lam_t *L) {
+    double a = (L->lambda_g < 1.0) ? log(1.0 - L->lambda_g) + ln_powerlaw_pdf(m, L) : -INFINITY;
+    double b = (L->lambda_g > 0.0) ? log(L->lambda_g) + ln_gauss_pdf(m, L->mu_g, L->sigma_g) : -INFINITY;
+    double s = ln_smooth_S(m, L);
+    if (s == -INFINITY) return -INFINITY;
+    return logaddexp(a, b) + s;
 }
+static double p1_unnorm(double m, const void *ctx) { return exp(ln_p1_unnorm(m, (const lam_t *)ctx)); }
 /* Z1 = int_{m_low}^{inf} p1_unnorm dm.  Pieces: the smoothing window (split at m_high if the
  * power law ends inside it), the plateau up to m_high, and the Gaussian beyond (to +40 sigma). */
 static double Z1_norm(const lam_t *L) {
@@ -271,30 +286,50 @@ static double Z1_norm(const lam_t *L) {
     }
     return z;
 }
+/* integrand of C(m1) with S(m1') factored out: m^beta S(m)/S(m_ref), S(m)/S(m_ref) = exp(ln S(m) - ln S(m_ref)) <= 1 */
+typedef struct { const lam_t *L; double ln_s_ref; } m2_ctx;
 static double m2_kernel(double m, const void *ctx) {
-    const lam_t *L = (const lam_t *)ctx;
-    return pow(m, L->beta) * smooth_S(m, L);
+    const m2_ctx *c = (const m2_ctx *)ctx;
+    double ls = ln_smooth_S(m, c->L);
+    if (ls == -INFINITY) return 0.0;
+    return pow(m, c->L->beta) * exp(ls - c->ln_s_ref);
 }
-/* M3/M4: C(m1) = int_{m_low}^{m1} m^beta S(m) dm.  Window part by quadrature; above the window
- * S = 1 and the integrand is a pure power (closed form, beta = -1 -> log). */
-static double C_norm(double m1, const lam_t *L) {
+/* M3/M4: C(m1) = int_{m_low}^{m1} m^beta S(m) dm, returned as ln C.  Above the window S = 1 and the integrand is a pure power
+ * (closed form, beta = -1 -> log) on top of the full-window integral.  Inside the window S(m1) is factored out (it may be
+ * e^-1000) and the rest -- which piles up at the upper end over a width ~ m1'^2/delta -- is integrated on panels that halve
+ * towards m1 (13 panels of GLN nodes: resolves m1'/delta down to ~1e-4). */
+static double ln_C_norm(double m1, const lam_t *L) {
     double a = L->m_low, c = L->m_low + L->delta_m;
-    if (m1 <= a) return 0.0;
-    if (m1 <= c) return gl_integrate(m2_kernel, L, a, m1, 8);
-    double w = gl_integrate(m2_kernel, L, a, c, 8);
+    if (m1 <= a) return -INFINITY;
+    if (m1 < c) {
+        m2_ctx k = {L, ln_smooth_S(m1, L)};
+        if (k.ln_s_ref == -INFINITY) return -INFINITY;
+        double sum = 0.0, lo = a, w = m1 - a;
+        for (int p = 0; p <= 12; ++p) {            /* panels [a, m1 - w/2], [m1 - w/2, m1 - w/4], ..., [m1 - w/4096, m1] */
+            double hi = (p < 12) ? m1 - w / (double)(2 << p) : m1;
+            sum += gl_integrate(m2_kernel, &k, lo, hi, 1);
+            lo = hi;
+        }
+        return k.ln_s_ref + log(sum);
+    }
+    m2_ctx k = {L, 0.0};
+    double w = gl_integrate(m2_kernel, &k, a, c, 8);
     double bp = L->beta + 1.0;
-    if (fabs(bp) < 1e-12) return w + log(m1 / c);
-    return w + (pow(m1, bp) - pow(c, bp)) / bp;
+    if (fabs(bp) < 1e-12) return log(w + log(m1 / c));
+    return log(w + (pow(m1, bp) - pow(c, bp)) / bp);
 }
-/* p(m1,m2) = p(m1) p(m2|m1)  (eq. 20) */
-static double mass_pdf(double m1, double m2, const lam_t *L, double Z1) {
-    if (m2 < L->m_low || m2 > m1) return 0.0;
-    double p1 = p1_unnorm(m1, L) / Z1;
-    if (p1 == 0.0) return 0.0;
-    double C = C_norm(m1, L);
-    if (!(C > 0.0)) return 0.0;
-    return p1 * pow(m2, L->beta) * smooth_S(m2, L) / C;
+/* ln p(m1,m2), p(m1,m2) = p(m1) p(m2|m1)  (eq. 20); ln_Z1 = ln of Z1_norm */
+static double ln_mass_pdf(double m1, double m2, const lam_t *L, double ln_Z1) {
+    if (m2 < L->m_low || m2 > m1) return -INFINITY;
+    double lp1 = ln_p1_unnorm(m1, L);
+    if (lp1 == -INFINITY) return -INFINITY;
+    double ls2 = ln_smooth_S(m2, L);
+    if (ls2 == -INFINITY) return -INFINITY;
+    double lC = ln_C_norm(m1, L);
+    if (lC == -INFINITY) return -INFINITY;
+    return lp1 - ln_Z1 + L->beta * log(m2) + ls2 - lC;
 }
+static double mass_pdf(double m1, double m2, const lam_t *L, double Z1) { return exp(ln_mass_pdf(m1, m2, L, log(Z1))); }
 
 void chimo_smoothing(const double *lam, int n, const double *m, double *out) {
     for (int i = 0; i < n; ++i) out[i] = smooth_S(m[i], (const lam_t *)lam);
@@ -310,9 +345,27 @@ void chimo_p_m2_given_m1(const double *lam, int n, const double *m1, const doubl
     const lam_t *L = (const lam_t *)lam;
     for (int i = 0; i < n; ++i) {
         if (m2[i] < L->m_low || m2[i] > m1[i]) { out[i] = 0.0; continue; }
-        double C = C_norm(m1[i], L);
-        out[i] = (C > 0.0) ? pow(m2[i], L->beta) * smooth_S(m2[i], L) / C : 0.0;
+        double lC = ln_C_norm(m1[i], L), ls = ln_smooth_S(m2[i], L);
+        out[i] = (lC > -INFINITY && ls > -INFINITY) ? exp(L->beta * log(m2[i]) + ls - lC) : 0.0;
     }
+}
+/* log-valued entries (finite where the linear ones underflow) */
+void chimo_ln_smoothing(const double *lam, int n, const double *m, double *out) {
+    for (int i = 0; i < n; ++i) out[i] = ln_smooth_S(m[i], (const lam_t *)lam);
+}
+void chimo_ln_p_m2_given_m1(const double *lam, int n, const double *m1, const double *m2, double *out) {
+    gl_init();
+    const lam_t *L = (const lam_t *)lam;
+    for (int i = 0; i < n; ++i) {
+        double lC = ln_C_norm(m1[i], L), ls = ln_smooth_S(m2[i], L);
+        out[i] = (m2[i] >= L->m_low && m2[i] <= m1[i] && lC > -INFINITY && ls > -INFINITY) ? L->beta * log(m2[i]) + ls - lC : -INFINITY;
+    }
+}
+void chimo_ln_mass_pdf(const double *lam, int n, const double *m1, const double *m2, double *out) {
+    gl_init();
+    const lam_t *L = (const lam_t *)lam;
+    double ln_Z1 = log(Z1_norm(L));
+    for (int i = 0; i < n; ++i) out[i] = ln_mass_pdf(m1[i], m2[i], L, ln_Z1);
 }
 void chimo_mass_pdf(const double *lam, int n, const double *m1, const double *m2, double *out) {
     gl_init();
@@ -332,53 +385,83 @@ void chimo_psi(const double *lam, int n, const double *z, double *out) {
 }
 
 /* -------------------------------------------------------------------------- O6 weights ------ */
-/* Per-sample redshift and weight (PAPER.md:52; :112 eq. 16 weights; :75 eq. 11; R1, R10).
+/* Per-sample redshift and LOG weight (PAPER.md:52; :112 eq. 16 weights; :75 eq. 11; R1, R10).
  *   placement N: w = p_m(m1,m2) psi(z)/J(z) / pi ;  placement P: w = p_m / pi.
- * Samples beyond the table range (z = NaN) get z = z_table_max, w = 0 and raise *range_flag. */
-void chimo_sample_weights(const double *lam, int placement, double z_table_max, int n,
-                          const double *dl, const double *m1d, const double *m2d,
-                          const double *ln_prior, double *z_out, double *w_out, int *range_flag) {
+ * ln w = -inf where the weight is 0 (R15).  Samples beyond the table range (z = NaN) get z = z_table_max, w = 0 and
+ * raise *range_flag. */
+void chimo_sample_log_weights(const double *lam, int placement, double z_table_max, int n,
+                              const double *dl, const double *m1d, const double *m2d,
+                              const double *ln_prior, double *z_out, double *lw_out, int *range_flag) {
     gl_init();
     const lam_t *L = (const lam_t *)lam;
-    double Z1 = Z1_norm(L);
+    double ln_Z1 = log(Z1_norm(L));
     int rf = 0;
     for (int j = 0; j < n; ++j) {
         double z = z_of_dL(dl[j], L, z_table_max);
-        if (isnan(z)) { z_out[j] = z_table_max; w_out[j] = 0.0; rf = 1; continue; }
+        if (isnan(z)) { z_out[j] = z_table_max; lw_out[j] = -INFINITY; rf = 1; continue; }
         double m1 = m1d[j] / (1.0 + z), m2 = m2d[j] / (1.0 + z);
-        double w = mass_pdf(m1, m2, L, Z1) / exp(ln_prior[j]);
-        if (placement == CHIMO_PLACE_SAMPLES && w != 0.0) w *= psi_rate(z, L) / jac(z, L);
+        double lw = ln_mass_pdf(m1, m2, L, ln_Z1);
+        if (lw > -INFINITY) {
+            lw -= ln_prior[j];
+            if (placement == CHIMO_PLACE_SAMPLES) lw += log(psi_rate(z, L)) - log(jac(z, L));
+        }
         z_out[j] = z;
-        w_out[j] = w;
+        lw_out[j] = lw;
     }
     if (range_flag) *range_flag = rf;
 }
+/* the same as linear weights w = exp(ln w) (may underflow to 0 for ln w < -745: the step-by-step pins use it) */
+void chimo_sample_weights(const double *lam, int placement, double z_table_max, int n,
+                          const double *dl, const double *m1d, const double *m2d,
+                          const double *ln_prior, double *z_out, double *w_out, int *range_flag) {
+    chimo_sample_log_weights(lam, placement, z_table_max, n, dl, m1d, m2d, ln_prior, z_out, w_out, range_flag);
+    for (int j = 0; j < n; ++j) w_out[j] = exp(w_out[j]);
+}
 
 /* ------------------------------------------------------------------------ O7 bandwidth ------ */
-/* Scott's rule on the weighted sample (R3): w^ = w/sum w, n_eff = 1/sum w^2,
- * var = sum w^(z-zbar)^2 / (1 - sum w^^2), h = sqrt(var) n_eff^(-1/5).  NaN if degenerate. */
-double chimo_scott_bw(int n, const double *z, const double *w) {
-    long double sw = 0.0L;
-    for (int j = 0; j < n; ++j) sw += w[j];
-    if (!(sw > 0.0L)) return NAN;
-    long double s2 = 0.0L, zb = 0.0L;
+/* Scott's rule on the weighted sample (R3): w^ = w/sum w, n_eff = 1/sum w^^2,
+ * var = sum w^(z-zbar)^2 / (1 - sum w^^2), h = sqrt(var) n_eff^(-1/5).
+ *
+ * Input: LOG weights.  The rule is evaluated in an algebraically identical form that neither cancels nor underflows when one
+ * sample d carries (almost) the whole event -- both sums of the definition then tend to 0 together (R21).  With
+ * d = argmax ln w, l2 = the largest ln w among the others, s = exp(l2 - ln w_d) in (0, 1], e_j = exp(ln w_j - l2),
+ * u_j = z_j - z_d and, over j != d,  W = sum e_j, Q = sum e_j^2, A = sum e_j u_j^2, B = sum e_j u_j:
+ *     sum w / w_d = 1 + sW,     1 - sum w^^2 = [2sW + s^2 (W^2 - Q)] / (1 + sW)^2,
+ *     sum w^(z-zbar)^2 = [sA(1 + sW) - s^2 B^2] / (1 + sW)^2
+ *  => var = [A(1 + sW) - s B^2] / [2W + s (W^2 - Q)],   n_eff = (1 + sW)^2 / (1 + s^2 Q).
+ * Undefined (NaN, BW_DEGENERATE) iff fewer than two samples have non-zero weight -- then 1 - sum w^^2 = 0 exactly -- or
+ * var = 0 (all weighted samples at one redshift).  Two samples d apart give var = d^2/2 for every weight ratio. */
+double chimo_scott_bw_log(int n, const double *z, const double *lw) {
+    int d = -1;
+    for (int j = 0; j < n; ++j)
+        if (lw[j] > -INFINITY && (d < 0 || lw[j] > lw[d])) d = j;
+    if (d < 0) return NAN;
+    double l2 = -INFINITY;
+    for (int j = 0; j < n; ++j)
+        if (j != d && lw[j] > l2) l2 = lw[j];
+    if (l2 == -INFINITY) return NAN;
+    long double s = expl((long double)l2 - (long double)lw[d]);
+    long double W = 0.0L, Q = 0.0L, A = 0.0L, B = 0.0L;
     for (int j = 0; j < n; ++j) {
-        long double wh = w[j] / sw;
-        s2 += wh * wh;
-        zb += wh * z[j];
+        if (j == d || lw[j] == -INFINITY) continue;
+        long double e = expl((long double)lw[j] - (long double)l2), u = (long double)z[j] - (long double)z[d];
+        W += e;
+        Q += e * e;
+        A += e * u * u;
+        B += e * u;
     }
-    long double var = 0.0L;
-    for (int j = 0; j < n; ++j) {
-        long double wh = w[j] / sw, d = z[j] - zb;
-        var += wh * d * d;
-    }
-    /* R21: one sample carries the event.  As n_eff -> 1 the rule divides 0 by 0 (sigma^2 -> d^2/2 for two
-     * samples however small the second weight): the bandwidth is declared undefined once n_eff < 1/(1 - 1e-4). */
-    if (!(1.0L - s2 > 1.0e-4L)) return NAN;
-    var /= (1.0L - s2);
+    long double var = (A * (1.0L + s * W) - s * B * B) / (2.0L * W + s * (W * W - Q));
     if (!(var > 0.0L)) return NAN;
-    double neff = (double)(1.0L / s2);
-    return sqrt((double)var) * pow(neff, -0.2);
+    long double neff = (1.0L + s * W) * (1.0L + s * W) / (1.0L + s * s * Q);
+    return sqrt((double)var) * pow((double)neff, -0.2);
+}
+/* linear-weight entry (w >= 0): ln w = log(w), log(0) = -inf */
+double chimo_scott_bw(int n, const double *z, const double *w) {
+    double *lw = (double *)malloc(sizeof(double) * (n > 0 ? n : 1));
+    for (int j = 0; j < n; ++j) lw[j] = (w[j] > 0.0) ? log(w[j]) : -INFINITY;
+    double h = chimo_scott_bw_log(n, z, lw);
+    free(lw);
+    return h;
 }
 
 /* ------------------------------------------------------------------------------ O8 KDE ------ */
@@ -458,25 +541,29 @@ double chimo_event_integral(const double *lam, int placement, int ng, const doub
     return (double)I;
 }
 
-/* One event end to end: O2..O9.  Returns log I_i; optional outputs h, flags. */
+/* One event end to end: O2..O9.  Returns log I_i; optional outputs h, flags.
+ * The weights are carried as ln w_j and enter O8-O9 as w_j / w_max (P10: w -> c w gives I -> c I with the same h), ln w_max
+ * is added back to log I: an event whose weights all lie below the fp64 range is small, not empty. */
 double chimo_event_logI(const double *lam, int placement, int bw_rule, double fixed_bw,
                         double z_table_max, int ns, const double *dl, const double *m1d,
                         const double *m2d, const double *ln_prior, int ng, const double *zg,
                         const double *pgal, double *h_out, uint32_t *flags) {
-    double *z = (double *)malloc(sizeof(double) * ns), *w = (double *)malloc(sizeof(double) * ns);
+    double *z = (double *)malloc(sizeof(double) * ns), *lw = (double *)malloc(sizeof(double) * ns);
+    double *w = (double *)malloc(sizeof(double) * ns);
     double *K = (double *)malloc(sizeof(double) * ng);
     int rf = 0;
     uint32_t fl = 0;
-    chimo_sample_weights(lam, placement, z_table_max, ns, dl, m1d, m2d, ln_prior, z, w, &rf);
+    chimo_sample_log_weights(lam, placement, z_table_max, ns, dl, m1d, m2d, ln_prior, z, lw, &rf);
     if (rf) fl |= CHIMO_F_TABLE_RANGE;
-    double sw = 0.0, h, logI;
-    for (int j = 0; j < ns; ++j) sw += w[j];
-    if (!(sw > 0.0)) { /* all-zero event: I = 0 (R15) */
+    double lmax = -INFINITY, h, logI;
+    for (int j = 0; j < ns; ++j) if (lw[j] > lmax) lmax = lw[j];
+    if (lmax == -INFINITY) { /* all-zero event: I = 0 (R15) */
         fl |= CHIMO_F_EVENT_ZERO;
         h = NAN;
         logI = -INFINITY;
     } else {
-        h = (bw_rule == CHIMO_BW_FIXED) ? fixed_bw : chimo_scott_bw(ns, z, w);
+        for (int j = 0; j < ns; ++j) w[j] = exp(lw[j] - lmax);
+        h = (bw_rule == CHIMO_BW_FIXED) ? fixed_bw : chimo_scott_bw_log(ns, z, lw);
         if (!(h > 0.0) || !isfinite(h)) {
             fl |= CHIMO_F_BW_DEGENERATE;
             logI = NAN;
@@ -495,13 +582,13 @@ double chimo_event_logI(const double *lam, int placement, int bw_rule, double fi
             if (nk != ns) { double f = (double)nk / (double)ns; for (int g = 0; g < ng; ++g) K[g] *= f; }   /* keep 1/N_s */
             free(zb); free(wb);
             double I = chimo_event_integral(lam, placement, ng, zg, K, pgal);
-            if (I > 0.0) logI = log(I);
+            if (I > 0.0) logI = log(I) + lmax;
             else { fl |= CHIMO_F_EVENT_ZERO; logI = -INFINITY; }
         }
     }
     if (h_out) *h_out = h;
     if (flags) *flags |= fl;
-    free(z); free(w); free(K);
+    free(z); free(lw); free(w); free(K);
     return logI;
 }
 
@@ -514,7 +601,7 @@ void chimo_selection_sums(const double *lam, double z_cat_max, double z_table_ma
                           int *range_flag) {
     gl_init();
     const lam_t *L = (const lam_t *)lam;
-    double Z1 = Z1_norm(L);
+    double ln_Z1 = log(Z1_norm(L));
     double Vmax = V_c(z_cat_max, L);
     long double S1 = 0.0L, S2 = 0.0L;
     int rf = 0;
@@ -525,8 +612,8 @@ void chimo_selection_sums(const double *lam, double z_cat_max, double z_table_ma
         if (isnan(z)) rf |= 1;
         else if (z <= z_cat_max) {
             double m1 = m1d[j] / (1.0 + z), m2 = m2d[j] / (1.0 + z);
-            double pm = mass_pdf(m1, m2, L, Z1);
-            if (pm != 0.0) s = pm * psi_rate(z, L) * (dVc_dz(z, L) / Vmax) / jac(z, L) / exp(ln_pdraw[j]);
+            double lpm = ln_mass_pdf(m1, m2, L, ln_Z1);
+            if (lpm > -INFINITY) s = exp(lpm - ln_pdraw[j]) * psi_rate(z, L) * (dVc_dz(z, L) / Vmax) / jac(z, L);
         }
         if (s_out) s_out[j] = s;
         S1 += s;
@@ -612,7 +699,9 @@ void chimo_loglike_batch(int n_lambda, const double *lam, int placement, int bw_
  * and physical event g owns the sub-events [group_off[g], group_off[g+1]):
  *     I_g = sum_k F_k I_k,   I_k = int KDE[{z_j | w_j}_{j in pixel k}](z) p_gal,k(z) dz  (O8-O9 per pixel, 1/N_k, own Scott h),
  * F_k = exp(ln_factor[k]) the hyperparameter-independent factor of eq. 18 (2-d sky KDE at the pixel centre x pixel area).
- * log L = sum_g log I_g - N_groups log xi.  n_groups = 0: every sub-event is its own event (single-1d). */
+ * log L = sum_g log I_g - N_groups log xi.  n_groups = 0: every sub-event is its own event (single-1d).
+ * Sparse pixels (reading R24 of DESIGN.md; PAPER.md:167-169 notes "less populated pixels" but gives no rule): a pixel whose
+ * Scott bandwidth is undefined under this lambda (fewer than two samples with non-zero weight) is left out of the sum. */
 void chimo_loglike_batch_grouped(int n_lambda, const double *lam, int placement, int bw_rule,
                          double z_cat_max, double z_table_max, int n_table, double neff_factor,
                          int n_events, const int64_t *sample_off, const double *dl,
@@ -659,6 +748,8 @@ void chimo_loglike_batch_grouped(int n_lambda, const double *lam, int placement,
         if (n_groups > 0) {   /* pixel sum of eq. 14 in log space; a pixel with I = 0 is not an empty event */
             efl &= ~CHIMO_F_EVENT_ZERO;
             for (int g = 0; g < n_groups; ++g) {
+                /* R24: a pixel whose bandwidth is undefined (log I_k = NaN, BW_DEGENERATE stays raised) is left out of the
+                 * pixel sum; an event none of whose pixels has I_k > 0 is NaN if a pixel was left out, else empty (-inf) */
                 double mx = -INFINITY, acc = 0.0;
                 int nan = 0;
                 for (int64_t k = group_off[g]; k < group_off[g + 1]; ++k) {
@@ -666,9 +757,15 @@ void chimo_loglike_batch_grouped(int n_lambda, const double *lam, int placement,
                     if (isnan(v)) nan = 1;
                     else if (v > mx) mx = v;
                 }
-                if (nan) { total = NAN; continue; }
-                if (mx == -INFINITY) { efl |= CHIMO_F_EVENT_ZERO; total += -INFINITY; continue; }
-                for (int64_t k = group_off[g]; k < group_off[g + 1]; ++k) acc += exp(li[k] + ln_factor[k] - mx);
+                if (mx == -INFINITY) {
+                    if (nan) total = NAN;
+                    else { efl |= CHIMO_F_EVENT_ZERO; total += -INFINITY; }
+                    continue;
+                }
+                for (int64_t k = group_off[g]; k < group_off[g + 1]; ++k) {
+                    double v = li[k] + ln_factor[k];
+                    if (!isnan(v)) acc += exp(v - mx);
+                }
                 total += mx + log(acc);
             }
         } else {

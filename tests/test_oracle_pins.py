@@ -8,7 +8,7 @@ import pytest
 from scipy import integrate, optimize, special
 
 import oracle as O
-from workloads import lambda_vector, make_workload, split_into_pixels
+from workloads import append_pixels, lambda_vector, make_workload, split_into_pixels
 
 C = 299792.458
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
@@ -341,16 +341,101 @@ def test_scott_bandwidth_reduces_to_textbook_for_equal_weights():
     assert math.isnan(O.scott_bw([0.3], [1.0])) and math.isnan(O.scott_bw(z, np.zeros(200)))
 
 
-def test_scott_bandwidth_two_samples_closed_form_and_degenerate_threshold():
-    # two samples d apart, weights (1, eps): sum w^2 = (1 + eps^2)/(1 + eps)^2, sigma^2 = d^2/2 for EVERY eps (the 0/0 of
-    # R21), h = d/sqrt(2) n_eff^(-1/5); undefined once 1 - sum w^2 <= 1e-4 (eps ~ 5e-5)
+def test_scott_bandwidth_two_samples_closed_form_for_every_weight_ratio():
+    # two samples d apart, weights (1, eps): sum w^2 = (1 + eps^2)/(1 + eps)^2 and sigma^2 = d^2/2 for EVERY eps > 0 (both sums
+    # of the rule tend to 0 together: R21), so h = d/sqrt(2) n_eff^(-1/5); undefined only when the second weight IS zero
     d = 0.04
-    for eps in (1.0, 0.1, 1e-3, 1e-4):
+    for eps in (1.0, 0.1, 1e-3, 1e-4, 4e-5, 1e-12, 1e-30, 1e-300):
         s2 = (1 + eps ** 2) / (1 + eps) ** 2
         h = O.scott_bw([0.5, 0.5 + d], [1.0, eps])
-        assert abs(h / (d / math.sqrt(2) * s2 ** 0.2) - 1) < 1e-12
-    for eps in (4e-5, 1e-6, 1e-12, 0.0):
-        assert math.isnan(O.scott_bw([0.5, 0.5 + d], [1.0, eps]))
+        assert abs(h / (d / math.sqrt(2) * s2 ** 0.2) - 1) < 1e-12, eps
+        assert abs(O.scott_bw([0.5 + d, 0.5], [eps, 1.0]) / h - 1) < 1e-12               # order of the samples
+    for lr in (-800.0, -5000.0, -1e6):                                                      # ratios below the fp64 range
+        assert abs(O.scott_bw_log([0.5, 0.5 + d], [3.0, 3.0 + lr]) / (d / math.sqrt(2)) - 1) < 1e-12
+    assert math.isnan(O.scott_bw([0.5, 0.5 + d], [1.0, 0.0]))
+    assert math.isnan(O.scott_bw_log([0.5, 0.5 + d], [-np.inf, -np.inf]))
+    assert math.isnan(O.scott_bw([0.5, 0.5, 0.5], [1.0, 0.3, 0.2]))                        # zero variance
+
+
+def test_scott_bandwidth_is_the_plain_rule_in_high_precision():
+    # O7 as SURVEY writes it -- w^ = w/sum w, n_eff = 1/sum w^^2, var = sum w^(z - zbar)^2/(1 - sum w^^2) -- typed out with
+    # 1000-digit arithmetic (mpmath: 1 - sum w^^2 is 10^-869 in the last case), against the oracle's cancellation-free rearrangement, on weights spanning 10^-40 .. 1,
+    # on one dominant sample plus a sprinkle at 10^-25, and on weights that only exist as logs (e^-3000)
+    import mpmath as mp
+    mp.mp.dps = 1000
+    rng = np.random.default_rng(11)
+
+    def plain(z, lw):
+        lw = [mp.mpf(float(x)) for x in lw]
+        m = max(lw)
+        w = [mp.e ** (x - m) for x in lw]
+        sw = mp.fsum(w)
+        wh = [x / sw for x in w]
+        s2 = mp.fsum(x * x for x in wh)
+        zb = mp.fsum(x * mp.mpf(float(t)) for x, t in zip(wh, z))
+        var = mp.fsum(x * (mp.mpf(float(t)) - zb) ** 2 for x, t in zip(wh, z)) / (1 - s2)
+        return float(mp.sqrt(var) * (1 / s2) ** mp.mpf(-0.2))
+    z = 0.7 + 0.05 * rng.standard_normal(60)
+    cases = [rng.uniform(-92.0, 0.0, 60),                                    # 40 decades
+             np.concatenate([[0.0], rng.uniform(-60.0, -55.0, 59)]),         # one sample carries the event
+             rng.uniform(-3000.0, -2990.0, 60),                              # all far below the fp64 range
+             np.concatenate([[-700.0], rng.uniform(-2800.0, -2700.0, 59)])]  # both
+    for lw in cases:
+        assert abs(O.scott_bw_log(z, lw) / plain(z, lw) - 1) < 1e-12
+    lw = cases[0]
+    assert abs(O.scott_bw(z, np.exp(lw)) / plain(z, lw) - 1) < 1e-12       # the linear-weight entry is the same rule
+    assert abs(O.scott_bw_log(z + 3.0, lw + 123.0) / O.scott_bw_log(z, lw) - 1) < 1e-12   # shift / scale invariance
+
+
+def test_mass_function_in_log_space_matches_high_precision_deep_in_the_window():
+    # ln S and ln p(m2|m1) where S itself leaves the fp64 range (m' < delta/709), against the definitions M1, M3 in
+    # 40-digit arithmetic: S = 1/(1 + e^f), C(m1) = int m^beta S dm by mpmath's adaptive quadrature
+    import mpmath as mp
+    mp.mp.dps = 40
+    la = lam()
+    ml, dm, be = la[7], la[6], la[5]
+
+    def S(m):
+        mpr = mp.mpf(m) - mp.mpf(ml)
+        return 1 / (1 + mp.e ** (mp.mpf(dm) / mpr + mp.mpf(dm) / (mpr - mp.mpf(dm))))
+    for frac in (0.3, 0.02, 1.0 / 900.0, 1.0 / 3000.0):
+        m = ml + frac * dm
+        assert abs(O.ln_smoothing(la, [m])[0] / float(mp.log(S(m))) - 1) < 1e-12
+        if frac > 1.0 / 700.0:
+            assert abs(O.smoothing(la, [m])[0] / float(S(m)) - 1) < 1e-10            # the linear entry, where it exists
+    for frac1, frac2 in ((0.5, 0.3), (0.05, 0.04), (1.0 / 500.0, 1.0 / 550.0), (1.0 / 2000.0, 1.0 / 2500.0), (3.0, 1.0 / 1500.0)):
+        m1, m2 = ml + frac1 * dm, ml + frac2 * dm
+        top = min(m1, ml + dm)
+        pts = [mp.mpf(ml)] + [mp.mpf(top) - (mp.mpf(top) - mp.mpf(ml)) / 2 ** k for k in range(1, 30)] + [mp.mpf(top)]
+        Cw = mp.quad(lambda x: x ** mp.mpf(be) * S(x), pts)
+        Cm = Cw + ((mp.mpf(m1) ** (be + 1) - mp.mpf(top) ** (be + 1)) / (be + 1) if m1 > top else 0)
+        ref = float(mp.mpf(be) * mp.log(m2) + mp.log(S(m2)) - mp.log(Cm))
+        got = O.ln_p_m2_given_m1(la, [m1], [m2])[0]
+        assert abs(got - ref) < 1e-9 * max(1.0, abs(ref)), (frac1, frac2, got, ref)
+    # the joint density where the linear one underflows: ln p = ln p(m1) + ln p(m2|m1)
+    m1, m2 = 30.0, ml + dm / 1500.0
+    assert O.mass_pdf(la, [m1], [m2])[0] == 0.0 and O.ln_mass_pdf(la, [m1], [m2])[0] < -1400.0
+    assert abs(O.ln_mass_pdf(la, [m1], [m2])[0] - (math.log(O.p_m1(la, [m1])[0]) + O.ln_p_m2_given_m1(la, [m1], [m2])[0])) < 1e-9
+
+
+def test_p10_weight_scaling_at_the_edge_of_the_fp64_range():
+    # P10 where linear weights die: ln_prior -> ln_prior + c multiplies every weight by e^-c; h must not move and log I must
+    # shift by exactly -c, also when the weights sit near 1e-300 and when they lie far below the smallest double
+    w = make_workload("tiny", n_samples=300)
+    la = w.lam[0]
+    dl, m1, m2, lp, zg, pg = _one_event(w, 2)
+    a, h, fa = O.event_logI(la, dl, m1, m2, lp, zg, pg)
+    assert fa == 0 and -60 < a < 0
+    for c in (650.0, 1350.0, 5000.0):
+        b, h2, fb = O.event_logI(la, dl, m1, m2, lp + c, zg, pg)
+        assert fb == 0 and abs(b - (a - c)) < 1e-9 and abs(h2 / h - 1) < 1e-12, c
+    # an event carried by secondaries deep in the smoothing window (S(m2) < 2^-1024 for all of them) is small, not empty
+    z = O.z_of_dl(la, dl)
+    m2deep = (la[7] + la[6] / np.linspace(900.0, 4000.0, dl.size)) * (1 + z)
+    v, hd, fd = O.event_logI(la, dl, np.maximum(m1, m2deep), m2deep, lp, zg, pg)
+    assert fd == 0 and np.isfinite(v) and v < -900 and hd > 0
+    _, wlin, _ = O.sample_weights(la, dl, np.maximum(m1, m2deep), m2deep, lp)
+    assert np.all(wlin == 0.0)                                                          # (what the linear weights see)
 
 
 # ------------------------------------------------------------------ P11: brute force, independent route
@@ -513,6 +598,28 @@ def test_many1d_with_shared_p_gal_and_fixed_bandwidth_equals_single1d():
     r1 = O.loglike_workload(w1, bw_rule=O.BW_FIXED, fixed_bw=np.full(2, h))
     rp = O.loglike_workload(wp, bw_rule=O.BW_FIXED, fixed_bw=np.full(10, h))
     assert abs(rp["loglike"][0] - r1["loglike"][0]) < 1e-10
+
+
+def test_many1d_sparse_pixels_are_left_out_of_the_pixel_sum():
+    # R24: a pixel with one sample (or one sample left with weight under this lambda) has no Scott bandwidth; it is left out
+    # of the pixel sum -- the result is the one of the same event without that pixel -- and BW_DEGENERATE is raised
+    w = split_into_pixels(make_workload("tiny", n_events=3, n_samples=400, n_grid=120, n_inj_draw=300), n_pix=4)
+    ref = O.loglike_workload(w)
+    s = slice(w.sample_off[0], w.sample_off[0] + 2)
+    one = (w.dL[s][:1], w.m1d[s][:1], w.m2d[s][:1], w.ln_prior[s][:1], math.log(0.01))
+    below = (w.dL[s], w.m1d[s], np.array([w.m2d[s][0], 1.0]), w.ln_prior[s], math.log(0.02))   # second sample below m_low
+    w2 = append_pixels(w, 1, [one, below])
+    assert w2.n_events == w.n_events + 2 and w2.group_off[-1] == w2.n_events
+    r = O.loglike_workload(w2)
+    assert abs(r["loglike"][0] - ref["loglike"][0]) < 1e-12
+    assert r["flags"][0] == ref["flags"][0] | O.F_BW_DEGENERATE
+    k = int(w.group_off[2])
+    assert np.isnan(r["event_logI"][0, k]) and np.isnan(r["event_logI"][0, k + 1])
+    # an event made of sparse pixels only has support but no estimate: NaN (as the single-1d kernel with one sample)
+    w3 = append_pixels(w, 2, [one])
+    w3.group_off = np.append(w3.group_off[:-1], [w3.n_events - 1, w3.n_events])      # ... as a fourth event of its own
+    r3 = O.loglike_workload(w3)
+    assert np.isnan(r3["loglike"][0]) and (r3["flags"][0] & O.F_BW_DEGENERATE)
 
 
 # ------------------------------------------------------------------ p_cat from a galaxy list (NEXT-3; eq. 8, R22)

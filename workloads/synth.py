@@ -349,3 +349,24 @@ def split_into_pixels(w: Workload, n_pix: int = 8, rho: float = 0.4, min_samples
         ln_prior=np.concatenate(lp), grid_off=np.array(go, dtype=np.int64), z_grid=np.concatenate(zg),
         p_gal=np.concatenate(pg), group_off=np.array(goff, dtype=np.int64), ln_factor=np.array(lnf),
         meta=dict(w.meta or {}, n_pix=n_pix))
+
+
+def append_pixels(w: Workload, g: int, pixels) -> Workload:
+    """Append (event, pixel) sub-events to physical event g of a many-1d workload (test helper for sparse pixels).
+    pixels = [(dL, m1d, m2d, ln_prior, ln_factor), ...]; the new pixels reuse the grid and p_gal of the event's first one."""
+    so, go = w.sample_off, w.grid_off
+    cut = lambda a, off: [a[off[i]:off[i + 1]] for i in range(len(off) - 1)]
+    dl, m1, m2, lp = cut(w.dL, so), cut(w.m1d, so), cut(w.m2d, so), cut(w.ln_prior, so)
+    zg, pg = cut(w.z_grid, go), cut(w.p_gal, go)
+    lnf = list(w.ln_factor)
+    k0, k1 = int(w.group_off[g]), int(w.group_off[g + 1])
+    for n, (a, b, c, d, f) in enumerate(pixels):
+        for lst, v in ((dl, a), (m1, b), (m2, c), (lp, d), (zg, zg[k0]), (pg, pg[k0])):
+            lst.insert(k1 + n, np.asarray(v, dtype=np.float64))
+        lnf.insert(k1 + n, float(f))
+    goff = w.group_off.copy()
+    goff[g + 1:] += len(pixels)
+    off = lambda parts: np.concatenate([[0], np.cumsum([len(x) for x in parts])]).astype(np.int64)
+    return dataclasses.replace(w, sample_off=off(dl), dL=np.concatenate(dl), m1d=np.concatenate(m1), m2d=np.concatenate(m2),
+                               ln_prior=np.concatenate(lp), grid_off=off(zg), z_grid=np.concatenate(zg), p_gal=np.concatenate(pg),
+                               group_off=goff, ln_factor=np.array(lnf))
