@@ -81,7 +81,8 @@ enum { CHIM_KERNEL_GAUSS = 0, CHIM_KERNEL_EPANECHNIKOV = 1 };
 #define CHIM_FLAG_XI_ZERO 8u         /* xi = 0 -> loglike = NaN                                                  */
 #define CHIM_FLAG_NEFF_LOW 16u       /* N_eff < neff_factor * N_events (R8); loglike is left untouched           */
 #define CHIM_FLAG_TABLE_RANGE 32u    /* a sample's d_L exceeds d_L^gw(z_table_max): that sample gets weight 0    */
-#define CHIM_FLAG_BW_DEGENERATE 64u  /* Scott bandwidth undefined (one effective sample) -> that log I_i = NaN   */
+#define CHIM_FLAG_BW_DEGENERATE 64u  /* Scott bandwidth undefined (fewer than two samples with non-zero weight, or all at one
+                                        redshift; R21) -> that log I_i = NaN                                     */
 
 typedef struct chim_ctx chim_ctx; /* opaque; owns all device copies */
 
@@ -114,11 +115,12 @@ typedef struct chim_config {
  * neff_factor 5, kde_method AUTO, n_mass_table 1024, count_pairs 0, kde_kernel GAUSS, n_bins 0. */
 void chim_default_config(chim_config *cfg);
 
-/* Creates a context on cfg->device.  cfg == NULL means chim_default_config.  *out is set to NULL on error
- * (the status is then the only report).  Fails with CHIM_ECUDA if no sm_100 device is present. */
+/* Creates a context on cfg->device.  cfg == NULL means chim_default_config.  *out is set to NULL on error; the
+ * reason is then available from chim_last_error(NULL) (kept per calling thread until the next failed chim_create).
+ * Fails with CHIM_ECUDA if the device is not of compute capability 10.x. */
 int chim_create(const chim_config *cfg, chim_ctx **out);
 void chim_destroy(chim_ctx *ctx);
-const char *chim_last_error(const chim_ctx *ctx); /* never NULL; "" if no error yet */
+const char *chim_last_error(const chim_ctx *ctx); /* never NULL; "" if no error yet; ctx == NULL: the last failed chim_create */
 int chim_version(void);
 
 /*
@@ -146,7 +148,9 @@ int chim_init_events(chim_ctx *ctx, int32_t n_events, const int64_t *sample_off,
  *   group_off [n_groups+1]: starts at 0, strictly increasing, ends at n_events (HOST or DEVICE per cfg.mem)
  *   ln_factor [n_events]  : finite
  * out_event_logI of chim_loglike_batch stays per sub-event.  A sub-event with I_k = 0 does not raise EVENT_ZERO; a group
- * whose sub-events are all zero does (loglike = -inf).  n_groups == 0 removes the grouping (every sub-event is an
+ * whose sub-events are all zero does (loglike = -inf).  Sparse pixels (reading R24): a sub-event whose Scott bandwidth is
+ * undefined under a lambda (fewer than two samples with non-zero weight) is left out of the sum and raises BW_DEGENERATE; a
+ * group with no I_k > 0 of which one was left out gives loglike = NaN.  n_groups == 0 removes the grouping (every sub-event is an
  * event: the single-1d kernel); chim_init_events also removes it.
  */
 int chim_set_event_groups(chim_ctx *ctx, int32_t n_groups, const int64_t *group_off, const double *ln_factor);

@@ -124,7 +124,7 @@ def chim_create(cfg: ChimConfig | None = None):
     h = C.c_void_p()
     st = lib().chim_create(C.byref(cfg) if cfg is not None else None, C.byref(h))
     if st != 0:
-        raise ChimError(st, "chim_create failed (no sm_100 device, bad config or out of memory)")
+        raise ChimError(st, lib().chim_last_error(None).decode() or "chim_create failed")
     return h
 
 

@@ -66,8 +66,10 @@ struct chim_ctx {
 
 namespace {
 
+thread_local std::string g_create_err;     // reason of the last failed chim_create on this thread: chim_last_error(NULL)
 int fail(chim_ctx* c, int code, const std::string& msg) {
     if (c) c->err = msg;
+    else g_create_err = msg;
     return code;
 }
 int cuda_fail(chim_ctx* c, cudaError_t e, const char* where) {
@@ -132,11 +134,35 @@ DlGrid make_dl_grid(double xmin, double xmax, int K) {
     return g;
 }
 
+// Work and host-staging buffers are sized for the loaded sets: dropped (and every pointer into them nulled) whenever a
+// set is replaced.
+void drop_work(chim_ctx* ctx) {
+    free_pool(ctx->owned_work);
+    ctx->work_nl = 0;
+    ctx->work_has_dc = false;
+    ctx->Lc = nullptr; ctx->tab_ev = nullptr; ctx->tab_inj = nullptr; ctx->mtab = nullptr; ctx->dc_tab = nullptr;
+    ctx->logI = nullptr; ctx->partial = nullptr; ctx->flags = nullptr; ctx->stats = nullptr;
+    ctx->poly_ev = nullptr; ctx->poly_inj = nullptr;
+    free_pool(ctx->owned_host);
+    ctx->host_nl = 0;
+    ctx->st_lam = ctx->st_ll = ctx->st_ev = ctx->st_xi = ctx->st_neff = nullptr;
+    ctx->st_fl = nullptr;
+}
+
 int ensure_work(chim_ctx* ctx, int nl) {
     bool need_dc = ctx->cfg.placement == CHIM_ON_GRID;
     if (nl <= ctx->work_nl && (!need_dc || ctx->work_has_dc)) return CHIM_OK;
-    free_pool(ctx->owned_work);
-    ctx->work_nl = 0;
+    {   // (the host staging is sized by n_lambda x n_events as well, but only grows with n_lambda: keep it)
+        std::vector<void*> keep;
+        keep.swap(ctx->owned_host);
+        const int keep_nl = ctx->host_nl;
+        double *a = ctx->st_lam, *b = ctx->st_ll, *c = ctx->st_ev, *d = ctx->st_xi, *e = ctx->st_neff;
+        uint32_t* f = ctx->st_fl;
+        drop_work(ctx);
+        ctx->owned_host.swap(keep);
+        ctx->host_nl = keep_nl;
+        ctx->st_lam = a; ctx->st_ll = b; ctx->st_ev = c; ctx->st_xi = d; ctx->st_neff = e; ctx->st_fl = f;
+    }
     CK(dev_alloc(ctx->owned_work, &ctx->Lc, nl));
     CK(dev_alloc(ctx->owned_work, &ctx->tab_ev, (size_t)nl * ctx->ev_grid.rows()));
     CK(dev_alloc(ctx->owned_work, &ctx->tab_inj, (size_t)nl * (ctx->have_inj ? ctx->inj_grid.rows() : 1)));
@@ -303,10 +329,10 @@ void chim_default_config(chim_config* cfg) {
 
 int chim_version(void) { return CHIM_VERSION; }
 
-const char* chim_last_error(const chim_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+const char* chim_last_error(const chim_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
 int chim_create(const chim_config* cfg, chim_ctx** out) {
-    if (!out) return CHIM_EINVAL;
+    if (!out) return fail(nullptr, CHIM_EINVAL, "chim_create: out is NULL");
     *out = nullptr;
     chim_config c;
     if (cfg) c = *cfg; else chim_default_config(&c);
@@ -320,29 +346,47 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     if (!(c.z_table_max > 0.0)) c.z_table_max = d.z_table_max;
     if (!(c.z_cat_max > 0.0)) c.z_cat_max = d.z_cat_max;
     if (!(c.neff_factor >= 0.0)) c.neff_factor = d.neff_factor;
-    if (c.kde_cutoff < 0.0 || !std::isfinite(c.kde_cutoff)) return CHIM_EINVAL;
-    if (c.n_table < 16 || (c.n_dl_table != 0 && c.n_dl_table < 16) || c.n_dl_table > kMaxDlRows || c.n_win_table < 8 || c.n_mass_table < 64 || c.z_cat_max > c.z_table_max) return CHIM_EINVAL;
-    if (c.placement != CHIM_ON_SAMPLES && c.placement != CHIM_ON_GRID) return CHIM_EINVAL;
-    if (c.bw_rule != CHIM_BW_SCOTT && c.bw_rule != CHIM_BW_FIXED) return CHIM_EINVAL;
-    if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT && c.kde_method != CHIM_KDE_POWER && c.kde_method != CHIM_KDE_NONE) return CHIM_EINVAL;
-    if (c.mem != CHIM_MEM_HOST && c.mem != CHIM_MEM_DEVICE) return CHIM_EINVAL;
-    if (c.kde_kernel != CHIM_KERNEL_GAUSS && c.kde_kernel != CHIM_KERNEL_EPANECHNIKOV) return CHIM_EINVAL;
-    if (c.n_bins < 0 || c.n_bins > 2048) return CHIM_EINVAL;
-    if (c.kde_kernel == CHIM_KERNEL_EPANECHNIKOV && c.placement != CHIM_ON_SAMPLES) return CHIM_EINVAL;   // lambda-independent q_g needed
+    if (c.kde_cutoff < 0.0 || !std::isfinite(c.kde_cutoff)) return fail(nullptr, CHIM_EINVAL, "chim_create: kde_cutoff must be finite and >= 0");
+    if (c.n_table < 16 || (c.n_dl_table != 0 && c.n_dl_table < 16) || c.n_dl_table > kMaxDlRows || c.n_win_table < 8 || c.n_mass_table < 64)
+        return fail(nullptr, CHIM_EINVAL, "chim_create: table size out of range (n_table >= 16, n_dl_table 0 or 16..4093, n_win_table >= 8, n_mass_table >= 64)");
+    if (c.z_cat_max > c.z_table_max) return fail(nullptr, CHIM_EINVAL, "chim_create: z_cat_max exceeds z_table_max");
+    if (c.placement != CHIM_ON_SAMPLES && c.placement != CHIM_ON_GRID) return fail(nullptr, CHIM_EINVAL, "chim_create: unknown placement");
+    if (c.bw_rule != CHIM_BW_SCOTT && c.bw_rule != CHIM_BW_FIXED) return fail(nullptr, CHIM_EINVAL, "chim_create: unknown bw_rule");
+    if (c.kde_method != CHIM_KDE_AUTO && c.kde_method != CHIM_KDE_DIRECT && c.kde_method != CHIM_KDE_POWER && c.kde_method != CHIM_KDE_NONE)
+        return fail(nullptr, CHIM_EINVAL, "chim_create: unknown kde_method");
+    if (c.mem != CHIM_MEM_HOST && c.mem != CHIM_MEM_DEVICE) return fail(nullptr, CHIM_EINVAL, "chim_create: unknown mem");
+    if (c.kde_kernel != CHIM_KERNEL_GAUSS && c.kde_kernel != CHIM_KERNEL_EPANECHNIKOV) return fail(nullptr, CHIM_EINVAL, "chim_create: unknown kde_kernel");
+    if (c.n_bins < 0 || c.n_bins > 2048) return fail(nullptr, CHIM_EINVAL, "chim_create: n_bins must be in [0, 2048]");
+    if (c.kde_kernel == CHIM_KERNEL_EPANECHNIKOV && c.placement != CHIM_ON_SAMPLES)   // lambda-independent q_g needed
+        return fail(nullptr, CHIM_EINVAL, "chim_create: the Epanechnikov kernel needs placement CHIM_ON_SAMPLES");
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device < 0 || c.device >= ndev) return CHIM_ECUDA;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess) return fail(nullptr, CHIM_ECUDA, std::string("chim_create: cudaGetDeviceCount: ") + cudaGetErrorString(ce));
+    if (c.device < 0 || c.device >= ndev) return fail(nullptr, CHIM_ECUDA, "chim_create: no such CUDA device");
     cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, c.device) != cudaSuccess) return CHIM_ECUDA;
-    if (prop.major != 10) return CHIM_ECUDA;   // sm_100a only: no other code path exists
-    if (cudaSetDevice(c.device) != cudaSuccess) return CHIM_ECUDA;
+    ce = cudaGetDeviceProperties(&prop, c.device);
+    if (ce != cudaSuccess) return fail(nullptr, CHIM_ECUDA, std::string("chim_create: cudaGetDeviceProperties: ") + cudaGetErrorString(ce));
+    if (prop.major != 10)   // sm_100a only: no other code path exists
+        return fail(nullptr, CHIM_ECUDA, std::string("chim_create: device is ") + prop.name + " (compute capability " + std::to_string(prop.major) + "." +
+                                         std::to_string(prop.minor) + "); libchim is built for sm_100a only");
+    ce = cudaSetDevice(c.device);
+    if (ce != cudaSuccess) return fail(nullptr, CHIM_ECUDA, std::string("chim_create: cudaSetDevice: ") + cudaGetErrorString(ce));
     chim_ctx* ctx = new (std::nothrow) chim_ctx();
-    if (!ctx) return CHIM_ENOMEM;
+    if (!ctx) return fail(nullptr, CHIM_ENOMEM, "chim_create: out of host memory");
     ctx->cfg = c;
     ctx->stream = static_cast<cudaStream_t>(c.stream);
     TableParams TP = table_params(ctx);
     TP.ev.K = TP.inj.K = c.n_dl_table > 0 ? c.n_dl_table : kMaxDlRows;
-    if (tables_smem_bytes(TP) > kMaxSmemOptin || inject_smem_bytes(c.n_mass_table) > kMaxSmemOptin) { delete ctx; return CHIM_EINVAL; }
-    if (upload_gauss_legendre() != cudaSuccess || upload_poly_matrices(ctx) != cudaSuccess) { chim_destroy(ctx); return CHIM_ECUDA; }
+    if (tables_smem_bytes(TP) > kMaxSmemOptin || inject_smem_bytes(c.n_mass_table) > kMaxSmemOptin) {
+        delete ctx;
+        return fail(nullptr, CHIM_EINVAL, "chim_create: n_table / n_win_table / n_mass_table exceed the shared-memory staging limit");
+    }
+    ce = upload_gauss_legendre();
+    if (ce == cudaSuccess) ce = upload_poly_matrices(ctx);
+    if (ce != cudaSuccess) {
+        chim_destroy(ctx);
+        return fail(nullptr, ce == cudaErrorMemoryAllocation ? CHIM_ENOMEM : CHIM_ECUDA, std::string("chim_create: ") + cudaGetErrorString(ce));
+    }
     *out = ctx;
     return CHIM_OK;
 }
@@ -515,8 +559,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     ctx->n_groups = 0;
     ctx->grp_off = nullptr; ctx->grp_lnf = nullptr;
     free_pool(ctx->owned_ev);
-    free_pool(ctx->owned_work);
-    ctx->work_nl = 0;
+    drop_work(ctx);
     ctx->have_events = false;
     EventSetDev E{};
     E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz;
@@ -623,8 +666,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     if (n_det == 0) {
         cudaStreamSynchronize(ctx->stream);
         free_pool(ctx->owned_inj);
-        free_pool(ctx->owned_work);
-        ctx->work_nl = 0;
+        drop_work(ctx);
         ctx->have_inj = false;
         ctx->inj_blocks = 0;
         return CHIM_OK;
@@ -680,8 +722,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     }
     cudaStreamSynchronize(ctx->stream);
     free_pool(ctx->owned_inj);
-    free_pool(ctx->owned_work);
-    ctx->work_nl = 0;
+    drop_work(ctx);
     ctx->have_inj = false;
     InjSetDev I{};
     I.n_det = n_det;

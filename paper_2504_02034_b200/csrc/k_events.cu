@@ -96,7 +96,9 @@ __device__ double grid_factor(const LamConst& L, const double* __restrict__ dc, 
 struct EvSmem {
     LamConst L;
     double red[4 * (kEvThreads / 32)];
-    float fred[kEvThreads / 32];
+    unsigned long long kred[kEvThreads / 32];
+    double mom[4], slev;      // W, Q, B, A of Scott's rule about the heaviest sample (relative to level slev, R21)
+    int careful;
     unsigned long long mbar;
     int pass_counter;
     int mass_lo, mass_fit, early_tma;
@@ -332,12 +334,14 @@ __device__ double le_phase(const EvSmem& S, const LeSmem& M, const float* __rest
     return lsum;
 }
 
-// S2 sweep 1 over the event's samples: z_j - z0 and log2 w_j to shared memory; returns the thread's max log2 w.
+// S2 sweep 1 over the event's samples: z_j - z0 and log2 w_j to shared memory; returns the thread's max log2 w and (jx) the
+// first sample that attains it.
 template <bool kStaged>
 __device__ __forceinline__ float s2_sweep(const float4* __restrict__ rec, const LamF& Fs, const float4* __restrict__ rows,
                                           int k_base, const MassLookup& M, int ns, float z0h, float z0l,
-                                          float* __restrict__ zf, float* __restrict__ wl) {
+                                          float* __restrict__ zf, float* __restrict__ wl, int& jx) {
     float mx = -INFINITY;
+    jx = 0;
     const int tid = threadIdx.x;
     const LamF F = Fs;                               // registers, not re-read from shared memory after every store
     const int ns32 = (ns + 31) & ~31;                // whole warps stay in the loop (sample_eval votes)
@@ -363,7 +367,7 @@ __device__ __forceinline__ float s2_sweep(const float4* __restrict__ rec, const 
         if (j < ns) {
             zf[j] = zc;
             wl[j] = l2w;
-            mx = fmaxf(mx, l2w);
+            if (l2w > mx) { mx = l2w; jx = j; }
         }
     }
     return mx;
@@ -375,8 +379,9 @@ __device__ __forceinline__ float s2_sweep(const float4* __restrict__ rec, const 
 template <bool kFit>
 __device__ __forceinline__ float s2_sweep_poly(const float4* __restrict__ pa, const float2* __restrict__ pb, const LamF& Fs,
                                                const float* __restrict__ pc, const MassLookup& M, int ns,
-                                               float* __restrict__ zf, float* __restrict__ wl) {
+                                               float* __restrict__ zf, float* __restrict__ wl, int& jx) {
     float mx = -INFINITY;
+    jx = 0;
     const int tid = threadIdx.x;
     const LamF F = Fs;
     PolyCoef C;
@@ -400,10 +405,31 @@ __device__ __forceinline__ float s2_sweep_poly(const float4* __restrict__ pa, co
         if (j < ns) {
             zf[j] = zc;
             wl[j] = l2w;
-            mx = fmaxf(mx, l2w);
+            if (l2w > mx) { mx = l2w; jx = j; }
         }
     }
     return mx;
+}
+
+// Block-wide argmax of (value, first index): every thread passes its own candidate; the result is valid in all threads.
+// Key = order-preserving bits of the float in the upper word, ~index in the lower one (ties: the smallest index wins).
+// A NaN value sorts above everything (it is reported by the caller).  Two barriers; kscratch holds kEvThreads/32 keys.
+__device__ __forceinline__ void block_argmax(float& v, int& j, unsigned long long* kscratch) {
+    const uint32_t b = __float_as_uint(v);
+    unsigned long long key = ((unsigned long long)(b ^ ((b >> 31) ? 0xFFFFFFFFu : 0x80000000u)) << 32) | (uint32_t)(~(uint32_t)j);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
+        key = other > key ? other : key;
+    }
+    __syncthreads();                              // protect kscratch from a previous use
+    if ((threadIdx.x & 31) == 0) kscratch[threadIdx.x >> 5] = key;
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kEvThreads / 32; ++k) { const unsigned long long other = kscratch[k]; key = other > key ? other : key; }
+    const uint32_t hb = (uint32_t)(key >> 32);
+    v = __uint_as_float(hb ^ ((hb >> 31) ? 0x80000000u : 0xFFFFFFFFu));
+    j = (int)(~(uint32_t)key);
 }
 
 // shared-memory layout after EvSmem: zf float[ns_pad] | wl float[ns_pad] | aux = staged table rows + mass rows (S2) / gq float2[nz_pad] (S3)
@@ -501,23 +527,102 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     M.n_mass = P.n_mass;
     mbar_wait(&S.mbar, 0);
 
-    // ---- S2, sweep 1: z_j - z0 and log2 w_j -------------------------------------------------------------
+    // ---- S2: z_j - z0 and the weights, relative to the heaviest sample d; moments for Scott's rule --------------------
+    // Scott's rule (R3, R21) is evaluated about and excluding d: with w_d = 1, u = z - z_d and, over j != d,
+    // W = sum w, Q = sum w^2, B = sum w u, A = sum w u^2:  var = [A(1+W) - B^2]/[2W + W^2 - Q], n_eff = (1+W)^2/(1+Q) -- no
+    // cancellation however few samples carry the event.  The fast sweep (fp32 polynomials) is redone by the careful one
+    // (table rows with hi + lo pairs: m' to ~1e-9; second reference level for weights below the fp32 range) when the event
+    // hangs on samples the fast one cannot resolve: no weighted sample, W below the fp32 range, or d deep in the window.
     const float z0h = (float)z0, z0l = (float)(z0 - (double)z0h);
-    float mx;
+    float mx = -INFINITY;
+    int jd = 0;
     const float4* rec = P.ev.rec + 2 * s0;
     const int64_t p0 = P.ev.poly_off[ev];
-    if (use_poly && S.mass_fit) mx = s2_sweep_poly<true>(P.ev.prec_a + p0, P.ev.prec_b + p0, L.F, S.poly, M, ns, zf, wl);
-    else if (use_poly) mx = s2_sweep_poly<false>(P.ev.prec_a + p0, P.ev.prec_b + p0, L.F, S.poly, M, ns, zf, wl);
-    else if (staged) mx = s2_sweep<true>(rec, L.F, rows_s, k_lo, M, ns, z0h, z0l, zf, wl);
-    else mx = s2_sweep<false>(rec, L.F, reinterpret_cast<const float4*>(tab), 0, M, ns, z0h, z0l, zf, wl);
     // samples are sorted in d_L: one of them lies beyond the table iff the last one does
     if (tid == 0 && __float_as_uint(__ldg(rec + 2 * (size_t)(ns - 1)).x) > L.F.tkmax_ev_q) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
+    bool careful = true;
+    if (use_poly) {
+        if (S.mass_fit) mx = s2_sweep_poly<true>(P.ev.prec_a + p0, P.ev.prec_b + p0, L.F, S.poly, M, ns, zf, wl, jd);
+        else mx = s2_sweep_poly<false>(P.ev.prec_a + p0, P.ev.prec_b + p0, L.F, S.poly, M, ns, zf, wl, jd);
+        block_argmax(mx, jd, S.kred);
+        if (mx > -INFINITY && mx == mx) {
+            const float zd = zf[jd];
+            float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;   // W, Q, B, A
+            for (int j = tid; j < ns; j += kEvThreads) {
+                const float w = ex2f(wl[j] - mx), u = zf[j] - zd;
+                wl[j] = w;
+                const float we = (j == jd) ? 0.f : w;
+                m0 += we;
+                m1 = fmaf(we, we, m1);
+                const float wu = we * u;
+                m2 += wu;
+                m3 = fmaf(wu, u, m3);
+            }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    if (lane == 0) S.fred[wid] = mx;
-    __syncthreads();
+            for (int o = 16; o > 0; o >>= 1) {
+                m0 += __shfl_xor_sync(0xffffffffu, m0, o);
+                m1 += __shfl_xor_sync(0xffffffffu, m1, o);
+                m2 += __shfl_xor_sync(0xffffffffu, m2, o);
+                m3 += __shfl_xor_sync(0xffffffffu, m3, o);
+            }
+            if (lane == 0) { S.red[wid] = m0; S.red[8 + wid] = m1; S.red[16 + wid] = m2; S.red[24 + wid] = m3; }
+            __syncthreads();
+            if (tid == 0) {
 #pragma unroll
-    for (int k = 0; k < kEvThreads / 32; ++k) mx = fmaxf(mx, S.fred[k]);
+                for (int i = 0; i < 4; ++i) {
+                    double acc = 0.0;
+#pragma unroll
+                    for (int k = 0; k < kEvThreads / 32; ++k) acc += S.red[i * 8 + k];
+                    S.mom[i] = acc;
+                }
+                S.slev = 1.0;
+                // m2' of the heaviest sample, from its record and the polynomial of 1/(1+z)
+                const float4 Ad = __ldg(P.ev.prec_a + p0 + jd);
+                float ad = S.poly[2 * kPolyN + 2 * (kPolyN - 2) + 1];
+#pragma unroll
+                for (int n = kPolyN - 3; n >= 0; --n) ad = fmaf(ad, Ad.x, S.poly[2 * kPolyN + 2 * n + 1]);
+                const float mp2d = fmaf(Ad.z, ad, -L.F.mlow_hi);
+                // fp32 leaves ~1e-6 (random) + ~5e-7 (the fit, common to all samples) in m2': d ln w = delta/m2'^2 of that.  The
+                // careful sweep is taken where this would show in log I: few effective samples, or all of them deep
+                const double neff = (1.0 + S.mom[0]) * (1.0 + S.mom[0]) / (1.0 + S.mom[1]);
+                S.careful = (S.mom[0] < 7.9e-31 /* 2^-100 */ ||
+                             (double)mp2d * (double)mp2d < (double)L.F.delta * fmax(0.5 * rsqrt(neff), 0.1)) ? 1 : 0;
+            }
+            __syncthreads();
+            careful = S.careful != 0;
+        }
+    }
+    if (careful) {
+        __syncthreads();     // (every thread is done with zf / wl of the fast sweep)
+        if (staged && !use_poly) mx = s2_sweep<true>(rec, L.F, rows_s, k_lo, M, ns, z0h, z0l, zf, wl, jd);
+        else mx = s2_sweep<false>(rec, L.F, reinterpret_cast<const float4*>(tab), 0, M, ns, z0h, z0l, zf, wl, jd);
+        block_argmax(mx, jd, S.kred);
+        if (mx > -INFINITY && mx == mx) {
+            float l2 = -INFINITY;                       // second reference level: the largest log2 w among the others
+            int j2 = 0;
+            for (int j = tid; j < ns; j += kEvThreads)
+                if (j != jd) l2 = fmaxf(l2, wl[j]);
+            block_argmax(l2, j2, S.kred);
+            const float zd = zf[jd];
+            float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;   // W'', Q'', B'', A'' relative to l2
+            for (int j = tid; j < ns; j += kEvThreads) {
+                const float lw = wl[j], u = zf[j] - zd;
+                wl[j] = ex2f(lw - mx);                   // what the KDE sees: relative to the heaviest sample
+                const float we = (j == jd || !(l2 > -INFINITY)) ? 0.f : ex2f(lw - l2);
+                m0 += we;
+                m1 = fmaf(we, we, m1);
+                const float wu = we * u;
+                m2 += wu;
+                m3 = fmaf(wu, u, m3);
+            }
+            double mm[4] = {(double)m0, (double)m1, (double)m2, (double)m3};
+            block_sum<kEvThreads, 4>(mm, S.red);
+            if (tid == 0) {
+                S.mom[0] = mm[0]; S.mom[1] = mm[1]; S.mom[2] = mm[2]; S.mom[3] = mm[3];
+                S.slev = (l2 > -INFINITY) ? exp2((double)l2 - (double)mx) : 0.0;
+            }
+        }
+    }
     if (!(mx > -INFINITY)) {   // all-zero event (R15): I = 0
         if (tid == 0) {
             *out = (mx != mx) ? NAN : -INFINITY;
@@ -532,23 +637,14 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             }
         return;
     }
-
-    // ---- S2, sweep 2: w_j / max w, moments about the median sample (sorted: the middle one) -> bandwidth ----------
-    const float zmed = zf[ns >> 1], zlast = zf[ns - 1];
-    float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;   // sum w, sum w^2, sum w z', sum w z'^2
-    const int nsp = (int)ev_ns_pad(ns);
-    for (int j = tid; j < ns; j += kEvThreads) {
-        const float w = ex2f(wl[j] - mx), zc = zf[j] - zmed;
-        wl[j] = w;
-        m0 += w;
-        m1 = fmaf(w, w, m1);
-        const float wz = w * zc;
-        m2 += wz;
-        m3 = fmaf(wz, zc, m3);
-    }
-    for (int j = ns + tid; j < nsp; j += kEvThreads) {   // idle slots of the last pass sit on the last sample with weight 0
-        wl[j] = 0.f;
-        zf[j] = zlast;
+    {
+        const float zlast = zf[ns - 1];
+        const int nsp = (int)ev_ns_pad(ns);
+        __syncthreads();     // wl / zf complete (and S.mom published) before the idle slots and the diagnostics read them
+        for (int j = ns + tid; j < nsp; j += kEvThreads) {   // idle slots of the last pass sit on the last sample with weight 0
+            wl[j] = 0.f;
+            zf[j] = zlast;
+        }
     }
     if (P.dbg_z)
         for (int j = tid; j < ns; j += kEvThreads) {
@@ -556,15 +652,6 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             P.dbg_z[jo] = z0 + (double)zf[j];
             P.dbg_w[jo] = (double)wl[j] * exp2((double)mx) * exp(P.ln_shift[ev]);
         }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        m0 += __shfl_xor_sync(0xffffffffu, m0, o);
-        m1 += __shfl_xor_sync(0xffffffffu, m1, o);
-        m2 += __shfl_xor_sync(0xffffffffu, m2, o);
-        m3 += __shfl_xor_sync(0xffffffffu, m3, o);
-    }
-    if (lane == 0) { S.red[wid] = m0; S.red[8 + wid] = m1; S.red[16 + wid] = m2; S.red[24 + wid] = m3; }
-    __syncthreads();
     const double* zc_g = P.ev.zc + g0;
     const float* qn_g = P.ev.qn + g0;
     // q_g of the first 1024 grid points: requested now, consumed after the bandwidth step (their L2 latency hides behind it)
@@ -576,23 +663,15 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     }
     const double udz = S.ev_udz;
     const float T = (P.cutoff > 0.0) ? (float)(P.cutoff * sqrt(kHalfLog2e)) : INFINITY;
-    if (tid == 0) {   // one thread: fp64 sums over the warps, bandwidth, and every scalar the pair loop needs
-        double mom[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            double a = 0.0;
-#pragma unroll
-            for (int k = 0; k < kEvThreads / 32; ++k) a += S.red[i * 8 + k];
-            mom[i] = a;
-        }
-        const double sw = mom[0];
+    if (tid == 0) {   // one thread: bandwidth, and every scalar the pair loop needs
         double h;
         if (P.bw_rule == CHIM_BW_FIXED) {
             h = P.ev.fixed_bw[ev];
-        } else {   // Scott on the weighted sample (R3, O7)
-            double s2 = mom[1] / (sw * sw), zb = mom[2] / sw;
-            double var = (mom[3] / sw - zb * zb) / (1.0 - s2);
-            h = (1.0 - s2 > 1.0e-4 && var > 0.0) ? sqrt(var) * (double)exp2f(0.2f * log2f((float)s2)) : NAN;   // n_eff^(-1/5) = s2^(1/5); fp32: dh/h ~ 1e-7 moves log I by ~1e-9.  R21: undefined once one sample carries the event
+        } else {   // Scott on the weighted sample (R3, O7) in the form of R21; sl = 1 unless the careful sweep set a second level
+            const double W = S.mom[0], Q = S.mom[1], Bm = S.mom[2], Am = S.mom[3], sl = S.slev;
+            const double den = 2.0 * W + sl * (W * W - Q), var = (Am * (1.0 + sl * W) - sl * Bm * Bm) / den;
+            const double neff = (1.0 + sl * W) * (1.0 + sl * W) / (1.0 + sl * sl * Q);
+            h = (den > 0.0 && var > 0.0) ? sqrt(var) * (double)exp2f(-0.2f * log2f((float)neff)) : NAN;   // fp32 power: dh/h ~ 1e-7 moves log I by ~1e-9
         }
         if (P.dbg_h) *P.dbg_h = h;
         // scaled coordinates x = z' sqrt(log2(e)/2)/h: exp(-d^2/2h^2) = 2^(-dx^2)
@@ -600,7 +679,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         const double scd = (double)scf;             // samples and grid are scaled by the SAME rounded factor
         const float delta = (float)(udz * scd);
         int Bsel = 0;                                // 0 = direct form
-        if (udz > 0.0 && T < INFINITY && P.kde_method == CHIM_KDE_AUTO && !P.dbg_K) {
+        if (udz > 0.0 && T < INFINITY && (P.kde_method == CHIM_KDE_AUTO || P.kde_method == CHIM_KDE_POWER) && !P.dbg_K) {
             if (delta * 32.f <= 3.3f) Bsel = 32;
             else if (delta * 16.f <= kMaxBlockSpan) Bsel = 16;
         }
@@ -631,9 +710,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     __syncthreads();
     if (P.kde_method == CHIM_KDE_NONE) {   // diagnostic: S3 skipped; flat p_gal on a wide grid: I = mean weight (pin P5)
         if (tid == 0) {
-            double sw = 0.0;
-#pragma unroll
-            for (int k = 0; k < kEvThreads / 32; ++k) sw += S.red[k];
+            const double sw = 1.0 + S.slev * S.mom[0];     // sum_j w_j / w_d
             *out = log(sw / (double)ns) + (double)mx * 0.69314718055994530942 + P.ln_shift[ev];
         }
         return;

@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
     double acc[2] = {0.0, 0.0};
     int oor = 0;
     const double tk_h = P.inj.tk_h[chunk], tk_c = P.inj.tk_c[chunk];
-    const bool use_poly = L.flags == 0 && tk_h > 0.0 && tk_c + tk_h < L.tkmax_inj && !P.dbg_s;
+    const bool use_poly = L.flags == 0 && tk_h > 0.0 && tk_c + tk_h < L.tkmax_inj;
     if (use_poly) {
         // chunk-local polynomials: the chunk's (sorted) injections span a narrow range of ln d_L; z is taken relative to
         // z_cat_max, so the support cut of R6 is the sign of the polynomial
@@ -97,6 +97,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             const double s = (zc <= 0.f && j < n) ? ex2_to_double(l2w) : 0.0;
             acc[0] += s;
             acc[1] = fma(s, s, acc[1]);
+            if (P.dbg_s && j < n) P.dbg_s[P.inj.perm[j0 + j]] = s * P.dbg_scale;
         }
     } else if (L.flags == 0) {
         const float4* rows = reinterpret_cast<const float4*>(P.tab + (size_t)l * P.tab_rows);
@@ -162,6 +163,8 @@ __global__ void __launch_bounds__(kCombThreads) k_combine(CombineParams P) {
             for (int i = tid; i < P.n_events; i += kCombThreads)
                 P.out_event_logI[(size_t)l * P.n_events + i] = P.logI[(size_t)l * P.n_events + i];
         for (int g = tid; g < P.n_groups; g += kCombThreads) {
+            // R24: a pixel whose bandwidth is undefined (log I_k = NaN; k_events raised BW_DEGENERATE) is left out of the sum;
+            // an event none of whose pixels has I_k > 0 is NaN if a pixel was left out, else empty
             const int64_t k0 = P.group_off[g], k1 = P.group_off[g + 1];
             double mx = -INFINITY;
             bool nan = false;
@@ -170,11 +173,15 @@ __global__ void __launch_bounds__(kCombThreads) k_combine(CombineParams P) {
                 if (isnan(x)) nan = true;
                 else mx = fmax(mx, x);
             }
-            if (nan) n_nan = 1;
-            else if (mx == -INFINITY) n_ninf = 1;
-            else {
+            if (mx == -INFINITY) {
+                if (nan) n_nan = 1;
+                else n_ninf = 1;
+            } else {
                 double acc = 0.0;
-                for (int64_t k = k0; k < k1; ++k) acc += exp(P.logI[(size_t)l * P.n_events + k] + P.ln_factor[k] - mx);
+                for (int64_t k = k0; k < k1; ++k) {
+                    const double x = P.logI[(size_t)l * P.n_events + k] + P.ln_factor[k];
+                    if (!isnan(x)) acc += exp(x - mx);
+                }
                 v[0] += mx + log(acc);
             }
         }

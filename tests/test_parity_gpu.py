@@ -1,12 +1,13 @@
 """GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on the same
 seeded inputs.  Tolerances are north_star's: per-event log I relative 1e-4, total log L absolute 1e-3."""
 import math
+import os
 
 import numpy as np
 import pytest
 
 import oracle as O
-from workloads import lambda_vector, make_workload, split_into_pixels
+from workloads import append_pixels, lambda_vector, make_workload, split_into_pixels
 
 pytestmark = pytest.mark.gpu
 
@@ -57,81 +58,137 @@ def _compare(r, ref, n_events):
 
 
 # ---------------------------------------------------------------- full size, in the configuration bench.py times
-def test_full_size_o5_spectroscopic_sampled_outputs(P):
-    """BASELINE.json configs[1] at full size (300 events x 5000 samples x 1000 grid points, 1024 lambda, 10^6
-    injections), launched as bench.py launches it (default config, lambda_chunk 256, no pair counting).  The oracle
-    cannot run 307 200 units in a test, so: 40 sampled (event, lambda) outputs one by one, log xi / N_eff / the total
-    for 2 lambdas, and properties over the whole batch."""
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _run_full(P, w, lam=None, **kw):
+    """The workload at full size, launched as bench.py launches it (default config, lambda_chunk 256, no pair counting)."""
     import torch
-    w = make_workload("o5_spec")
-    assert (w.n_events, w.n_lambda, w.n_det) == (300, 1024, 1_000_000)
-    c = P.Context(z_cat_max=w.z_cat_max)
+    c = P.Context(z_cat_max=w.z_cat_max, **kw)
     c.init_workload(w)
-    out = c.loglike_batch(torch.as_tensor(w.lam, device=c.device).contiguous())
+    lam = w.lam if lam is None else lam
+    out = c.loglike_batch(torch.as_tensor(np.ascontiguousarray(lam), device=c.device).contiguous())
     torch.cuda.synchronize()
     r = {k: v.cpu().numpy() for k, v in out.items()}
+    r["flags"] = r["flags"].astype(np.uint32)
     c.close()
-    # properties at any size: total = sum of the parts (eq. 3); flags clear wherever every unit is finite
+    return r
+
+
+def _oracle_units(w, units):
+    """log I of the oracle for a list of (lambda row, event) units, grouped by lambda so that the events of one lambda
+    run on all host cores (the oracle is OpenMP-parallel over events).  Returns {(l, i): log I}."""
+    out = {}
+    by_l = {}
+    for l, i in units:
+        by_l.setdefault(int(l), []).append(int(i))
+    for l, ev in by_l.items():
+        so = np.concatenate([[0], np.cumsum([w.sample_off[i + 1] - w.sample_off[i] for i in ev])])
+        go = np.concatenate([[0], np.cumsum([w.grid_off[i + 1] - w.grid_off[i] for i in ev])])
+        cat = lambda a, off: np.concatenate([a[off[i]:off[i + 1]] for i in ev])
+        r = O.loglike_batch(w.lam[l], so, cat(w.dL, w.sample_off), cat(w.m1d, w.sample_off), cat(w.m2d, w.sample_off),
+                            cat(w.ln_prior, w.sample_off), go, cat(w.z_grid, w.grid_off), cat(w.p_gal, w.grid_off))
+        for k, i in enumerate(ev):
+            out[(l, i)] = float(r["event_logI"][0, k])
+    return out
+
+
+def _same_class(a, b):
+    return (np.isnan(a) and np.isnan(b)) or (np.isneginf(a) and np.isneginf(b)) or (np.isfinite(a) and np.isfinite(b))
+
+
+def _golden(name, w):
+    import hashlib
+    g = np.load(os.path.join(GOLD, f"ref_{name}.npz"))
+    h = hashlib.sha256()
+    for a in (w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal, w.inj_dL, w.inj_m1d, w.inj_m2d,
+              w.inj_ln_pdraw, w.lam):
+        h.update(np.ascontiguousarray(a).tobytes())
+    h.update(str(int(w.n_inj_total)).encode())
+    assert h.hexdigest() == str(g["input_sha256"]), "the cached oracle reference belongs to other inputs: rerun tests/golden/make_reference.py"
+    return g
+
+
+def _compare_with_golden(P, w, r, g, n_events):
+    """Every unit and every total of the cached oracle run (tests/golden/make_reference.py) against the CUDA path: rows of the
+    batch are read out of the full-size launch `r`; the box corners (not in the batch) get a launch of their own."""
+    idx = g["lam_index"]
+    inb = idx >= 0
+    got = {k: np.empty_like(g[k]) for k in ("loglike", "event_logI", "logxi", "neff")}
+    fl = np.zeros(len(idx), dtype=np.uint32)
+    for k in got:
+        got[k][inb] = r[k][idx[inb]]
+    fl[inb] = r["flags"][idx[inb]]
+    assert np.array_equal(w.lam[idx[inb]], g["lam"][inb])
+    if (~inb).any():
+        rc = _run_full(P, w, lam=g["lam"][~inb])
+        for k in got:
+            got[k][~inb] = rc[k]
+        fl[~inb] = rc["flags"]
+    a, b = got["event_logI"], g["event_logI"]
+    # classes: finite / -inf / NaN unit by unit, zero disagreements
+    assert np.array_equal(np.isnan(a), np.isnan(b)), np.argwhere(np.isnan(a) != np.isnan(b))[:10]
+    assert np.array_equal(np.isneginf(a), np.isneginf(b)), np.argwhere(np.isneginf(a) != np.isneginf(b))[:10]
+    fin = np.isfinite(b)
+    rel = np.abs(a[fin] - b[fin]) / np.abs(b[fin])
+    assert rel.max() < REL_EVENT, rel.max()
+    # rows where every unit is finite and ordinary (log I > -100: not hanging on a handful of samples deep in the smoothing
+    # window, where |log I| of hundreds lets rel 1e-4 be several 1e-2): the error statistics DESIGN.md sec. 7 quotes
+    ok = np.isfinite(g["loglike"])
+    assert ok.sum() >= 0.5 * len(idx)
+    err = (a - b)[ok]
+    ordinary = b[ok] > -100.0
+    assert np.abs(err[ordinary]).max() < 5e-6, np.abs(err[ordinary]).max()
+    assert abs(err[ordinary].mean()) < 5e-7
+    assert np.max(np.abs(got["logxi"][ok] - g["logxi"][ok])) < 1e-6
+    assert np.max(np.abs(got["neff"][ok] / g["neff"][ok] - 1)) < 1e-5
+    dtot = np.abs(got["loglike"][ok] - g["loglike"][ok])
+    assert dtot.max() < ABS_TOTAL, (dtot.max(), int(np.argmax(dtot)))
+    assert np.array_equal(np.isnan(got["loglike"]), np.isnan(g["loglike"])) and np.array_equal(np.isneginf(got["loglike"]), np.isneginf(g["loglike"]))
+    assert np.array_equal(fl, g["flags"].astype(np.uint32)), np.flatnonzero(fl != g["flags"])[:10]
+    return dict(max_rel=float(rel.max()), max_abs=float(np.abs(err[ordinary]).max()), mean=float(err[ordinary].mean()), max_total=float(dtot.max()),
+                n_units=int(a.size), n_nonfinite=int((~fin).sum()))
+
+
+@pytest.mark.parametrize("catalog", [0, 1, 2])
+def test_full_size_o5_spectroscopic_every_catalog(P, catalog):
+    """BASELINE.json configs[1] at full size (300 events x 5000 samples x 1000 grid points, 1024 lambda, 10^6 injections),
+    each of its three catalogs, launched as bench.py launches it.
+    (1) properties over the whole batch; (2) EVERY non-finite unit of the batch one by one against the oracle: the class
+    (-inf / NaN) must agree -- zero disagreements; (3) all 300 events x 64 lambda of the cached oracle run (the fiducial, 31
+    random rows, the 16 rows with the largest m_low -- where events lose their support -- and the 16 box corners): every
+    unit's class and value, log xi, N_eff, every total, the flags."""
+    w = make_workload("o5_spec", catalog=catalog)
+    assert (w.n_events, w.n_lambda, w.n_det) == (300, 1024, 1_000_000)
+    r = _run_full(P, w)
     assert np.isfinite(r["logxi"]).all() and (r["neff"] > 5 * 300).all() and (r["neff"] < w.n_det).all()
     fin = np.isfinite(r["event_logI"]).all(axis=1)
-    assert fin.sum() >= 1000 and (r["flags"][fin] == 0).all() and (r["flags"][~fin] != 0).all()
+    assert fin.sum() >= 800 and (r["flags"][fin] == 0).all() and (r["flags"][~fin] != 0).all()
     assert np.max(np.abs(r["loglike"][fin] - (r["event_logI"][fin].sum(axis=1) - 300 * r["logxi"][fin]))) < 1e-8
     assert not np.isfinite(r["loglike"][~fin]).any()
-    # the few non-finite units (an extreme lambda whose m_low leaves an event one or no sample: R15 / R21) one by one:
-    # -inf where the oracle has -inf, NaN where it has NaN
     bad = np.argwhere(~np.isfinite(r["event_logI"]))
-    assert len(bad) < 200
+    ref = _oracle_units(w, bad)
+    wrong = [(int(l), int(i), ref[(int(l), int(i))], float(r["event_logI"][l, i])) for l, i in bad
+             if not _same_class(ref[(int(l), int(i))], r["event_logI"][l, i])]
+    assert not wrong, (len(wrong), len(bad), wrong[:10])
     for l, i in bad:
-        s, g = slice(w.sample_off[i], w.sample_off[i + 1]), slice(w.grid_off[i], w.grid_off[i + 1])
-        ref, _, fl = O.event_logI(w.lam[l], w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s], w.z_grid[g], w.p_gal[g])
-        assert (np.isnan(ref) and np.isnan(r["event_logI"][l, i])) or (ref == -np.inf and r["event_logI"][l, i] == -np.inf), (l, i, ref)
-        assert fl & (P.CHIM_FLAG_EVENT_ZERO | P.CHIM_FLAG_BW_DEGENERATE) & int(r["flags"][l])
-    # sampled units against the oracle, one by one
-    rng = np.random.default_rng(123)
-    worst = 0.0
-    for l, i in zip(rng.choice(np.flatnonzero(fin), 40), rng.integers(0, 300, 40)):
-        s, g = slice(w.sample_off[i], w.sample_off[i + 1]), slice(w.grid_off[i], w.grid_off[i + 1])
-        ref, _, fl = O.event_logI(w.lam[l], w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s], w.z_grid[g], w.p_gal[g])
-        assert fl == 0 and abs(r["event_logI"][l, i] - ref) < REL_EVENT * abs(ref)
-        worst = max(worst, abs(r["event_logI"][l, i] - ref))
-    assert worst < 5e-6
-    # selection term and total for two lambdas (the fiducial and a random one)
-    ls = [0, 777]
-    ref = O.loglike_workload(w, lam=w.lam[ls])
-    assert np.max(np.abs(r["logxi"][ls] - ref["logxi"])) < 1e-6
-    assert np.max(np.abs(r["neff"][ls] / ref["neff"] - 1)) < 1e-5
-    assert np.max(np.abs(r["loglike"][ls] - ref["loglike"])) < ABS_TOTAL
-    assert np.max(np.abs(r["event_logI"][ls] - ref["event_logI"]) / np.abs(ref["event_logI"])) < REL_EVENT
+        assert int(r["flags"][l]) & (P.CHIM_FLAG_EVENT_ZERO | P.CHIM_FLAG_BW_DEGENERATE)
+    st = _compare_with_golden(P, w, r, _golden(f"o5_spec_cat{catalog}", w), 300)
+    print(f"catalog {catalog}: {len(bad)} non-finite units of 307200, all of the oracle's class; golden: {st}")
 
 
-@pytest.mark.parametrize("name,kw", [("o5_photo", dict(n_lambda=48)),
-                                     ("full_pop", dict(n_events=400, n_lambda=32)),
-                                     ("sel_heavy", dict(n_events=40, n_lambda=24, n_det=2_000_000))])
-def test_other_config_shapes_sampled_outputs(P, name, kw):
-    """The per-unit shapes of BASELINE.json configs[2..4] (4096-point photometric grids with 2000 galaxies; 4096 samples x
-    512 grid points; the 10^7-injection reference pdf at 2 x 10^6) with fewer lambdas / events than the full configs:
-    sampled (event, lambda) units one by one, log xi for two lambdas."""
-    import torch
-    w = make_workload(name, **kw)
-    c = P.Context(z_cat_max=w.z_cat_max)
-    c.init_workload(w)
-    out = c.loglike_batch(torch.as_tensor(w.lam, device=c.device).contiguous())
-    torch.cuda.synchronize()
-    r = {k: v.cpu().numpy() for k, v in out.items()}
-    c.close()
+@pytest.mark.parametrize("name", ["o5_photo", "full_pop", "sel_heavy"])
+def test_full_size_other_configs_against_the_cached_oracle(P, name):
+    """BASELINE.json configs[2..4] at FULL size (4096-point photometric grids with 2000 galaxies, 1024 lambda; 5000 events x
+    4096 samples x 512 grid points, 256 lambda; 4096 lambda with 10^7 injections): every unit, log xi, N_eff and every total of
+    the cached oracle rows (16 / 4 / 4 lambda over all events and all injections)."""
+    w = make_workload(name)
+    r = _run_full(P, w)
     fin = np.isfinite(r["event_logI"]).all(axis=1)
-    assert fin.sum() >= 0.9 * w.n_lambda and (r["flags"][fin] == 0).all()
-    rng = np.random.default_rng(321)
-    for l, i in zip(rng.choice(np.flatnonzero(fin), 10), rng.integers(0, w.n_events, 10)):
-        s, g = slice(w.sample_off[i], w.sample_off[i + 1]), slice(w.grid_off[i], w.grid_off[i + 1])
-        ref, _, fl = O.event_logI(w.lam[l], w.dL[s], w.m1d[s], w.m2d[s], w.ln_prior[s], w.z_grid[g], w.p_gal[g])
-        assert fl == 0 and abs(r["event_logI"][l, i] - ref) < 5e-6
-    ls = [int(np.flatnonzero(fin)[0]), int(np.flatnonzero(fin)[-1])]
-    inj = (w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw)
-    for l in ls:
-        s1, s2 = O.selection_sums(w.lam[l], *inj, z_cat_max=w.z_cat_max)
-        assert abs(r["logxi"][l] - math.log(s1 / w.n_inj_total)) < 1e-6
-        assert abs(r["neff"][l] / O.neff(s1, s2, w.n_inj_total) - 1) < 1e-5
+    assert fin.sum() >= 0.75 * w.n_lambda and (r["flags"][fin] == 0).all()
+    assert np.max(np.abs(r["loglike"][fin] - (r["event_logI"][fin].sum(axis=1) - w.n_events * r["logxi"][fin]))) < 1e-7
+    st = _compare_with_golden(P, w, r, _golden(name, w), w.n_events)
+    print(f"{name}: golden {st}")
 
 
 # ---------------------------------------------------------------- T2: intermediates, step by step
@@ -352,6 +409,9 @@ def test_kde_local_expansion_power_and_direct_forms_agree_with_the_oracle(P):
         assert 0 < st["kde_pairs_in_cutoff"] < st["kde_pairs_dense"] and st["kde_pairs_evaluated"] < st["kde_pairs_dense"]
     for r in (rp, rd):    # pair loops execute every pair inside the cut-off (plus band padding)
         assert r["stats"]["kde_pairs_in_cutoff"] <= r["stats"]["kde_pairs_evaluated"]
+    # POWER really took the power form: its bands are padded to whole blocks of 16 / 32 grid points (and to the widest
+    # sample of a 128-sample pass), the direct form's only to the pass
+    assert rp["stats"]["kde_pairs_evaluated"] > 1.02 * rd["stats"]["kde_pairs_evaluated"]
     # the local expansion replaces the pairs by fewer FMA operations (coefficient build + one polynomial per sample)
     assert 0 < ra["stats"]["kde_pairs_evaluated"] < ra["stats"]["kde_pairs_in_cutoff"]
     # the algorithmic pair count does not depend on the formulation (edge pairs may round differently: 1e-4)
@@ -701,3 +761,100 @@ def test_replacing_sets_and_reuse(P):
         ref = O.loglike_workload(w)
         assert abs(h["loglike"][0] - ref["loglike"][0]) < ABS_TOTAL
     c.close()
+
+
+def test_reinit_with_a_larger_event_set_then_host_call_with_event_logI(P):
+    # the device staging of chim_loglike_batch_host is sized n_lambda x n_events: a larger set after a smaller one must not
+    # reuse the smaller buffer; chim_get_stats between re-init and the next batch reports ESTATE instead of reading freed memory
+    w1 = make_workload("tiny", n_events=3, n_samples=120, n_grid=50, n_lambda=4, n_inj_draw=400)
+    w2 = make_workload("tiny", n_events=40, n_samples=90, n_grid=70, n_lambda=4, n_inj_draw=300, seed_offset=7)
+    c = P.Context(z_cat_max=1.5)
+    c.init_workload(w1)
+    h1 = c.loglike_batch_host(np.ascontiguousarray(w1.lam), event_logI=True)
+    c.init_workload(w2)
+    with pytest.raises(P.ChimError) as e:
+        c.stats()
+    assert e.value.status == -2
+    h2 = c.loglike_batch_host(np.ascontiguousarray(w2.lam), event_logI=True)
+    ref = O.loglike_workload(w2)
+    assert h2["event_logI"].shape == (4, 40)
+    assert np.max(np.abs(h2["event_logI"] - ref["event_logI"]) / np.abs(ref["event_logI"])) < REL_EVENT
+    assert np.max(np.abs(h2["loglike"] - ref["loglike"])) < ABS_TOTAL
+    assert np.max(np.abs(h1["loglike"] - O.loglike_workload(w1)["loglike"])) < ABS_TOTAL
+    c.close()
+
+
+def test_chim_create_reports_why_it_failed(P):
+    cfg = P.chim_default_config()
+    cfg.n_bins = 4096
+    with pytest.raises(P.ChimError) as e:
+        P.chim_create(cfg)
+    assert e.value.status == -1 and "n_bins" in str(e.value)
+    cfg = P.chim_default_config()
+    cfg.device = 99
+    with pytest.raises(P.ChimError) as e:
+        P.chim_create(cfg)
+    assert e.value.status == -3 and "device" in str(e.value)
+
+
+# ---------------------------------------------------------------- events that hang on one or two samples (R21, R24)
+def _few_sample_workload():
+    """Events whose secondaries all lie below m_low except a chosen few, placed eps above it (source frame, fiducial lambda):
+    none (-inf), one (Scott undefined: NaN), two and more at depths where S(m2) leaves the fp32 and the fp64 range."""
+    w = make_workload("o5_spec", n_events=8, n_samples=2000, n_grid=500, n_lambda=4, n_det=3000)
+    la = w.lam[0].copy()
+    cases = [(), (0.5,), (0.5, 0.4), (0.004, 0.002), (0.01, 0.0099, 0.002), tuple(np.linspace(0.02, 0.2, 12)), (0.003, 1.0)]
+    rng = np.random.default_rng(42)
+    for i, eps in enumerate(cases):
+        s = slice(w.sample_off[i], w.sample_off[i + 1])
+        z = O.z_of_dl(la, w.dL[s])
+        m2d = 0.5 * la[7] * (1 + z)
+        mid = np.argsort(w.dL[s])[900:1100]                          # samples near the middle of the distance posterior
+        for j, e in zip(rng.choice(mid, len(eps), replace=False), eps):
+            m2d[j] = (la[7] + e) * (1 + z[j])
+        w.m2d[s] = m2d
+        w.m1d[s] = np.maximum(w.m1d[s], m2d * 1.5)
+    lam = np.stack([la, la, la])
+    lam[1, 7] -= 1e-3
+    lam[2, 7] -= 1e-2
+    return w, lam
+
+
+def test_events_carried_by_one_or_two_samples_agree_with_the_oracle(P):
+    w, lam = _few_sample_workload()
+    ref = O.loglike_batch(lam, w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal)
+    c = P.Context(z_cat_max=w.z_cat_max)
+    c.init_events(w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal)
+    got = c.loglike_batch_host(np.ascontiguousarray(lam), event_logI=True)
+    c.close()
+    a, b = got["event_logI"], ref["event_logI"]
+    assert np.isneginf(b[:, 0]).all() and np.isnan(b[:, 1]).all() and np.isfinite(b[:, 2:]).all() and (b[:, 3] < -300).all()
+    assert np.array_equal(np.isnan(a), np.isnan(b)) and np.array_equal(np.isneginf(a), np.isneginf(b)), (a, b)
+    fin = np.isfinite(b)
+    assert np.max(np.abs(a[fin] - b[fin]) / np.abs(b[fin])) < REL_EVENT, (a, b)
+    assert np.max(np.abs(a[:, 7] - b[:, 7])) < 5e-6                                          # the ordinary event of the set
+    assert np.array_equal(got["flags"].astype(np.uint32), ref["flags"])
+
+
+def test_many1d_sparse_pixels_match_the_oracle(P):
+    # pixels of 1, 2 and 3 samples (R24): the one-sample pixel has no Scott bandwidth and is left out of the pixel sum; a pixel
+    # whose second sample lies below m_low likewise; 2 and 3 samples give a (wide) bandwidth.  Flags bit by bit.
+    w = split_into_pixels(make_workload("tiny", n_events=3, n_samples=400, n_grid=120, n_lambda=2, n_inj_draw=300), n_pix=4)
+    s = slice(w.sample_off[0], w.sample_off[0] + 3)
+    px = lambda n, f: (w.dL[s][:n], w.m1d[s][:n], w.m2d[s][:n], w.ln_prior[s][:n], math.log(f))
+    below = (w.dL[s][:2], w.m1d[s][:2], np.array([w.m2d[s][0], 1.0]), w.ln_prior[s][:2], math.log(0.02))
+    w2 = append_pixels(w, 1, [px(1, 0.01), px(2, 0.02), px(3, 0.03), below])
+    ref = O.loglike_workload(w2)
+    r = _gpu(P, w2, count_pairs=0)
+    assert np.isfinite(ref["loglike"]).all() and (ref["flags"] & O.F_BW_DEGENERATE).all()
+    assert np.array_equal(np.isnan(r["event_logI"]), np.isnan(ref["event_logI"]))
+    fin = np.isfinite(ref["event_logI"])
+    assert np.max(np.abs(r["event_logI"][fin] - ref["event_logI"][fin]) / np.abs(ref["event_logI"][fin])) < REL_EVENT
+    assert np.max(np.abs(r["loglike"] - ref["loglike"])) < ABS_TOTAL
+    assert np.array_equal(r["flags"], ref["flags"])
+    # an event made of a sparse pixel only: NaN on both sides
+    w3 = append_pixels(w, 2, [px(1, 1.0)])
+    w3.group_off = np.append(w3.group_off[:-1], [w3.n_events - 1, w3.n_events])
+    ref = O.loglike_workload(w3)
+    r = _gpu(P, w3, count_pairs=0)
+    assert np.isnan(ref["loglike"]).all() and np.isnan(r["loglike"]).all() and np.array_equal(r["flags"], ref["flags"])
