@@ -472,7 +472,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     std::vector<int32_t> k_lo(n_events), k_hi(n_events);
     const double l2e = 1.4426950408889634074;
     std::vector<int32_t> perm(NS);
-    std::vector<double> zc(NG), qg(NG), z0(n_events), shift(n_events), qshift(n_events), udz(n_events);
+    std::vector<double> zc(NG), qg(NG), z0(n_events), shift(n_events), qshift(n_events), udz(n_events), maxdz(n_events);
     std::vector<float> qn(NG);
     std::vector<double> ep0(NG + n_events), ep1(NG + n_events), ep2(NG + n_events);   // Epanechnikov prefix sums
     std::vector<double> lm_lo(n_events), lm_hi(n_events);
@@ -552,6 +552,8 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
         bool uniform = true;
         for (int g = 0; g < nz && uniform; ++g) uniform = std::fabs(h_z[g0 + g] - (h_z[g0] + g * dz)) <= 1e-7 * dz;
         udz[i] = uniform ? dz : 0.0;
+        maxdz[i] = 0.0;
+        for (int g = 1; g < nz; ++g) maxdz[i] = std::max(maxdz[i], h_z[g0 + g] - h_z[g0 + g - 1]);
     }
     // replace the previous set
     cudaStreamSynchronize(ctx->stream);
@@ -567,7 +569,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     CK(upload(ctx->owned_ev, &E.rec, rec));
     CK(upload(ctx->owned_ev, &E.k_lo, k_lo)); CK(upload(ctx->owned_ev, &E.k_hi, k_hi));
     CK(upload(ctx->owned_ev, &E.perm, perm)); CK(upload(ctx->owned_ev, &E.zc, zc)); CK(upload(ctx->owned_ev, &E.qn, qn));
-    CK(upload(ctx->owned_ev, &E.uni_dz, udz));
+    CK(upload(ctx->owned_ev, &E.uni_dz, udz)); CK(upload(ctx->owned_ev, &E.max_dz, maxdz));
     CK(upload(ctx->owned_ev, &E.ep_q0, ep0)); CK(upload(ctx->owned_ev, &E.ep_q1, ep1)); CK(upload(ctx->owned_ev, &E.ep_q2, ep2));
     CK(upload(ctx->owned_ev, &E.lnm1_lo, lm_lo)); CK(upload(ctx->owned_ev, &E.lnm1_hi, lm_hi));
     CK(upload(ctx->owned_ev, &E.z0, z0));

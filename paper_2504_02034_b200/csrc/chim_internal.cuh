@@ -393,6 +393,7 @@ struct EventSetDev {
     const double* zc;           // z_g - z0_i  (centred grid)
     const float* qn;            // p_gal(z_g) * trapezoid weight / (the event's largest such product)
     const double* uni_dz;       // [n_events] grid spacing if the event's grid is equally spaced, else 0
+    const double* max_dz;       // [n_events] largest grid spacing of the event
     const double* z0;           // [n_events] centre of each event's grid
     const double* lnm1_lo;      // [n_events] smallest / largest ln m1d of the event's samples
     const double* lnm1_hi;

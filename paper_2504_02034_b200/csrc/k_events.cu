@@ -112,6 +112,8 @@ struct EvSmem {
     alignas(16) float poly[4 * kPolyN];
     // lambda-independent scalars of the event, fetched once beside the constants (one L2 latency instead of one per use)
     double ev_udz, ev_zfirst, ev_ln_out;   // grid spacing (0: not equally spaced), first centred grid point, ln_shift + ln_qscale
+    double ev_maxdz;          // largest grid spacing of the event
+    int exact;                // S3 in log space without cut-off (exact_log2_kde)
 };
 
 __host__ __device__ inline size_t ev_ns_pad(size_t ns) { return (ns + kPass - 1) / kPass * kPass; }
@@ -432,6 +434,51 @@ __device__ __forceinline__ void block_argmax(float& v, int& j, unsigned long lon
     j = (int)(~(uint32_t)key);
 }
 
+// S3 + S4 without cut-off and in log space, for the units the fp32 pair loop cannot represent (R9, R21): an event left with a
+// few samples within ~1e-4 of each other has a bandwidth far below the grid spacing, so that no grid point lies within t h
+// of any sample and the nearest ones contribute e^-100 -- small, not zero.  Returns log2 of
+//     sum_j w_j sum_g q_g exp(-(z_g - z_j)^2 / 2h^2)
+// (block-uniform; -inf if every term is zero) by two passes over all (weighted sample, grid point) pairs: the largest
+// exponent, then the sum relative to it.  Slow by design: only taken when t h < half a grid spacing or the fast sum is 0.
+__device__ __noinline__ double exact_log2_kde(const LamConst& L, const double* __restrict__ dc_row, int dc_nodes, double dc_dz,
+                                              const float* __restrict__ zf, const float* __restrict__ wl, int ns3,
+                                              const double* __restrict__ zc_g, const float* __restrict__ qn_g, int nz, double z0,
+                                              double h, double* red, unsigned long long* kred) {
+    const int tid = threadIdx.x;
+    const double sc = sqrt(kHalfLog2e) / h;
+    const bool on_grid = dc_row != nullptr;     // placement ON_GRID: psi/J on the grid points
+    float mxt = -INFINITY;
+    int dummy = 0;
+    double sum = 0.0;
+    float M = 0.f;
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+        for (int g = tid; g < nz; g += kEvThreads) {
+            double q = (double)qn_g[g];
+            if (on_grid && q > 0.0) q *= grid_factor(L, dc_row, dc_nodes, dc_dz, zc_g[g] + z0);
+            if (!(q > 0.0)) continue;
+            const float lq = (float)log2(q);
+            const double xg = zc_g[g] * sc;
+            for (int j = 0; j < ns3; ++j) {
+                const float w = wl[j];
+                if (!(w > 0.f)) continue;
+                const double d = xg - (double)zf[j] * sc;
+                const float term = lg2f(w) + lq - (float)(d * d);
+                if (pass == 0) mxt = fmaxf(mxt, term);
+                else sum += (double)ex2f(term - M);
+            }
+        }
+        if (pass == 0) {
+            block_argmax(mxt, dummy, kred);
+            M = mxt;
+            if (!(M > -INFINITY)) return -INFINITY;
+        }
+    }
+    double t1[1] = {sum};
+    block_sum<kEvThreads, 1>(t1, red);
+    return (double)M + log2(t1[0]);
+}
+
 // shared-memory layout after EvSmem: zf float[ns_pad] | wl float[ns_pad] | aux = staged table rows + mass rows (S2) / gq float2[nz_pad] (S3)
 template <bool kStats>
 __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKernelParams P) {
@@ -485,8 +532,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             S.early_tma = early;
         }
         if (tid == 32) {
-            const double a = P.ev.uni_dz[ev], b = P.ev.zc[g0], c = P.ln_shift[ev], d = P.ln_qscale[ev];
-            S.ev_udz = a; S.ev_zfirst = b; S.ev_ln_out = c + d;
+            const double a = P.ev.uni_dz[ev], b = P.ev.zc[g0], c = P.ln_shift[ev], d = P.ln_qscale[ev], e = P.ev.max_dz[ev];
+            S.ev_udz = a; S.ev_zfirst = b; S.ev_ln_out = c + d; S.ev_maxdz = e;
         }
     }
     __syncthreads();
@@ -583,9 +630,9 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
                 for (int n = kPolyN - 3; n >= 0; --n) ad = fmaf(ad, Ad.x, S.poly[2 * kPolyN + 2 * n + 1]);
                 const float mp2d = fmaf(Ad.z, ad, -L.F.mlow_hi);
                 // fp32 leaves ~1e-6 (random) + ~5e-7 (the fit, common to all samples) in m2': d ln w = delta/m2'^2 of that.  The
-                // careful sweep is taken where this would show in log I: few effective samples, or all of them deep
+                // careful sweep is taken where this would show in log I: few effective samples (n_eff < 64), or all of them deep
                 const double neff = (1.0 + S.mom[0]) * (1.0 + S.mom[0]) / (1.0 + S.mom[1]);
-                S.careful = (S.mom[0] < 7.9e-31 /* 2^-100 */ ||
+                S.careful = (S.mom[0] < 7.9e-31 /* 2^-100 */ || neff < 64.0 ||
                              (double)mp2d * (double)mp2d < (double)L.F.delta * fmax(0.5 * rsqrt(neff), 0.1)) ? 1 : 0;
             }
             __syncthreads();
@@ -684,6 +731,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
             else if (delta * 16.f <= kMaxBlockSpan) Bsel = 16;
         }
         S.h = h; S.scd = scd; S.scf = scf; S.delta = delta; S.xfirst = (float)(S.ev_zfirst * scd); S.Bsel = Bsel;
+        // t h below half the (largest) grid spacing: a sample may have no grid point inside its cut-off -> exact evaluation
+        S.exact = (P.kde_kernel == CHIM_KERNEL_GAUSS && P.cutoff > 0.0 && h > 0.0 && P.cutoff * h < 0.5 * S.ev_maxdz) ? 1 : 0;
         // local-expansion form: equally spaced grid, a cut-off, boxes of ~1 unit of y = z'/(sqrt(2) h) that fit the stage
         S.le_nbox = 0; S.le_D = 0;
         if (udz > 0.0 && T < INFINITY && P.kde_method == CHIM_KDE_AUTO && !P.dbg_K && h > 0.0 && isfinite(h)) {
@@ -983,6 +1032,15 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         __syncthreads();
         const double ks = knorm * exp(ln_wscale + P.ln_shift[ev]);
         for (int g = tid; g < nz; g += kEvThreads) P.dbg_K[g] *= ks;
+    }
+    if ((S.exact || tot[0] == 0.0) && !P.dbg_K) {   // (block-uniform) units outside the reach of the fp32 pair loop
+        const double l2s = exact_log2_kde(L, on_grid ? P.dc_tab + (size_t)l * (P.n_table + 1 + kZPad) : nullptr, P.n_table + 1 + kZPad,
+                                          P.z_table_max / P.n_table, zf, wl, ns3, zc_g, qn_g, nz, z0, h, S.red, S.kred);
+        if (tid == 0) {
+            if (l2s > -INFINITY) *out = l2s * 0.69314718055994530942 + log(knorm) + ln_wscale + S.ev_ln_out;
+            else { *out = -INFINITY; atomicOr(P.flags + l, CHIM_FLAG_EVENT_ZERO); }
+        }
+        return;
     }
     if (tid == 0) {
         double I = tot[0] * knorm;

@@ -446,7 +446,7 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         F.lm0_hi = (float)L.lm0; F.lm0_lo = (float)(L.lm0 - (double)F.lm0_hi);
         F.delta = (float)L.delta;
         F.two_dl2e = (float)(2.0 * L.delta * l2e); F.d2l2e = (float)(L.delta * L.delta * l2e);
-        F.win_lo = (float)(L.delta * 1e-3); F.win_hi = (float)(L.delta * (1.0 - 1e-6));   // S(m' < 1e-3 delta) < e^-998: "0" either way
+        F.win_lo = (float)(L.delta * 1e-12); F.win_hi = (float)(L.delta * (1.0 - 1e-6));   // keeps f finite: log2 S down to -1e12 (the weights are carried as logs, R21)
         F.beta2 = (float)(L.beta * l2e);
         F.mhigh_p = (float)(L.m_high - L.m_low);
         F.tm_scale = (float)L.inv_dlm; F.tm_max = (float)P.n_mass + 0.999f;
