@@ -215,10 +215,14 @@ int chim_get_stats(chim_ctx *ctx, chim_stats *out);
 /* Per-kernel device times of the last chim_loglike_batch: when profiling is enabled, CUDA events are recorded on
  * cfg.stream around every kernel launch of the batch (no host synchronisation is added to the batch call);
  * chim_get_kernel_times synchronises the stream and sums the elapsed times per kernel kind.  S1 = table
- * builder, S2-S4 = fused sample-weight + KDE + integral kernel, S5 = injection reduction, S6 = combine. */
+ * builder and polynomial fits; S2-S4 = the fused sample-weight + KDE + integral step, split into k_events_fast (events_*: the
+ * regular units) and k_events (events_general_*: every other unit -- all of them when the configuration is not the default
+ * one); S5 = injection reduction; S6 = combine. */
 typedef struct chim_kernel_times {
     double tables_ms, events_ms, inject_ms, combine_ms;
     uint32_t tables_launches, events_launches, inject_launches, combine_launches;
+    double events_general_ms;
+    uint32_t events_general_launches, reserved;
 } chim_kernel_times;
 int chim_set_profiling(chim_ctx *ctx, int32_t enable);
 int chim_get_kernel_times(chim_ctx *ctx, chim_kernel_times *out);

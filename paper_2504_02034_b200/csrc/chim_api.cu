@@ -52,6 +52,10 @@ struct chim_ctx {
     double* dc_tab = nullptr; double* logI = nullptr; double2* partial = nullptr; uint32_t* flags = nullptr;
     unsigned long long* stats = nullptr;
     float* poly_ev = nullptr; float* poly_inj = nullptr;   // local polynomials per (lambda, event) / (lambda, chunk)
+    // k_events_fast: the events it takes / leaves to k_events, and the per-chunk work list of the units it hands over
+    const int32_t* fast_ev = nullptr; const int32_t* slow_ev = nullptr;
+    int n_fast = 0, n_slow = 0;
+    uint32_t* worklist = nullptr; unsigned int* work_count = nullptr;
     // staging for the host-pointer entry point
     int host_nl = 0;
     double* st_lam = nullptr; double* st_ll = nullptr; double* st_ev = nullptr; double* st_xi = nullptr;
@@ -60,6 +64,7 @@ struct chim_ctx {
     uint64_t launches = 0;
     // optional per-kernel timing (CUDA events around each launch of the last batch)
     bool profiling = false;
+    int sm_count = 148;
     std::vector<cudaEvent_t> ev_pool;          // reused across batches
     std::vector<int> ev_kind;                  // kind of the launch bracketed by events [2i, 2i+1]
 };
@@ -143,6 +148,7 @@ void drop_work(chim_ctx* ctx) {
     ctx->Lc = nullptr; ctx->tab_ev = nullptr; ctx->tab_inj = nullptr; ctx->mtab = nullptr; ctx->dc_tab = nullptr;
     ctx->logI = nullptr; ctx->partial = nullptr; ctx->flags = nullptr; ctx->stats = nullptr;
     ctx->poly_ev = nullptr; ctx->poly_inj = nullptr;
+    ctx->worklist = nullptr; ctx->work_count = nullptr;
     free_pool(ctx->owned_host);
     ctx->host_nl = 0;
     ctx->st_lam = ctx->st_ll = ctx->st_ev = ctx->st_xi = ctx->st_neff = nullptr;
@@ -175,6 +181,8 @@ int ensure_work(chim_ctx* ctx, int nl) {
     CK(dev_alloc(ctx->owned_work, &ctx->stats, 4));
     CK(dev_alloc(ctx->owned_work, &ctx->poly_ev, (size_t)nl * ctx->ev.n_events * 4 * kPolyN));
     CK(dev_alloc(ctx->owned_work, &ctx->poly_inj, (size_t)nl * std::max(ctx->inj_blocks, 1) * 4 * kPolyN));
+    CK(dev_alloc(ctx->owned_work, &ctx->worklist, (size_t)nl * ctx->ev.n_events));
+    CK(dev_alloc(ctx->owned_work, &ctx->work_count, 4));
     ctx->work_nl = nl;
     ctx->work_has_dc = need_dc;
     return CHIM_OK;
@@ -209,7 +217,7 @@ EventKernelParams event_params(const chim_ctx* ctx, int nl) {
     return P;
 }
 
-// profiling brackets: record an event pair around a launch of kind k (0 tables, 1 events, 2 inject, 3 combine)
+// profiling brackets: record an event pair around a launch of kind k (0 tables, 1 k_events_fast, 2 inject, 3 combine, 4 k_events)
 struct Bracket {
     chim_ctx* ctx; bool on; size_t slot;
     Bracket(chim_ctx* c, int kind) : ctx(c), on(c->profiling), slot(0) {
@@ -243,9 +251,37 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
                               ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->poly_inj, st));
         ctx->launches += ctx->have_inj ? 2 : 1;
     }
+    ctx->launches += 1;   // (k_tables)
     EventKernelParams EP = event_params(ctx, nl);
-    { Bracket b(ctx, 1); CK(launch_events(EP, ctx->cfg.count_pairs != 0, st)); }
-    ctx->launches += 2;
+    const chim_config& cf = ctx->cfg;
+    // the regular units go to k_events_fast: default configuration (Gaussian kernel, local-expansion form, weights on the samples,
+    // no binning, no pair counting) and events with a narrow d_L range on an equally spaced grid; the rest, and every unit the
+    // fast kernel hands over through the work list, to k_events
+    const bool fast = ctx->n_fast > 0 && cf.placement == CHIM_ON_SAMPLES && cf.kde_kernel == CHIM_KERNEL_GAUSS && cf.n_bins == 0 &&
+                      cf.kde_method == CHIM_KDE_AUTO && cf.kde_cutoff > 0.0 && cf.count_pairs == 0;
+    if (fast) {
+        FastEventParams FP{};
+        FP.ev = ctx->ev; FP.Lc = ctx->Lc; FP.mtab = ctx->mtab; FP.poly = ctx->poly_ev;
+        FP.n_lambda = nl; FP.n_mass = cf.n_mass_table; FP.bw_rule = cf.bw_rule; FP.cutoff = cf.kde_cutoff;
+        FP.logI = ctx->logI; FP.ln_shift = ctx->ev_ln_shift; FP.ln_qscale = ctx->ev_ln_qscale;
+        FP.fast_events = ctx->fast_ev; FP.worklist = ctx->worklist; FP.work_count = ctx->work_count;
+        CK(cudaMemsetAsync(ctx->work_count, 0, sizeof(unsigned int), st));
+        { Bracket b(ctx, 1); CK(launch_events_fast(FP, ctx->n_fast, st)); }
+        ctx->launches += 1;
+        if (ctx->n_slow > 0) {
+            EP.ev_list = ctx->slow_ev; EP.n_ev_list = ctx->n_slow;
+            { Bracket b(ctx, 4); CK(launch_events(EP, false, st)); }
+            ctx->launches += 1;
+        }
+        EP.ev_list = nullptr; EP.n_ev_list = 0;
+        EP.worklist = ctx->worklist; EP.work_count = ctx->work_count;
+        EP.worklist_ctas = (int)std::min<long long>((long long)nl * ctx->n_fast, 3LL * ctx->sm_count);
+        { Bracket b(ctx, 4); CK(launch_events(EP, false, st)); }
+        ctx->launches += 1;
+    } else {
+        { Bracket b(ctx, 4); CK(launch_events(EP, cf.count_pairs != 0, st)); }
+        ctx->launches += 1;
+    }
     if (ctx->have_inj) {
         InjKernelParams IP{};
         IP.inj = ctx->inj; IP.Lc = ctx->Lc; IP.tab = ctx->tab_inj; IP.mtab = ctx->mtab;
@@ -374,6 +410,7 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     chim_ctx* ctx = new (std::nothrow) chim_ctx();
     if (!ctx) return fail(nullptr, CHIM_ENOMEM, "chim_create: out of host memory");
     ctx->cfg = c;
+    ctx->sm_count = prop.multiProcessorCount;
     ctx->stream = static_cast<cudaStream_t>(c.stream);
     TableParams TP = table_params(ctx);
     TP.ev.K = TP.inj.K = c.n_dl_table > 0 ? c.n_dl_table : kMaxDlRows;
@@ -555,6 +592,16 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
         maxdz[i] = 0.0;
         for (int g = 1; g < nz; ++g) maxdz[i] = std::max(maxdz[i], h_z[g0 + g] - h_z[g0 + g - 1]);
     }
+    // k_events_fast: q_g once more with 16-byte aligned, zero-padded slices (the source of its TMA copy), and the events it takes:
+    // narrow d_L range (event-local polynomials) on an equally spaced grid, if its stage fits the shared memory at all
+    std::vector<int64_t> q4off(n_events);
+    int64_t q4n = 0;
+    for (int i = 0; i < n_events; ++i) { q4off[i] = q4n; q4n += ((go[i + 1] - go[i] + 3) / 4) * 4; }
+    std::vector<float> qn4((size_t)q4n + 4, 0.f);
+    for (int i = 0; i < n_events; ++i) std::copy(qn.begin() + go[i], qn.begin() + go[i + 1], qn4.begin() + q4off[i]);
+    std::vector<int32_t> fast_ev, slow_ev;
+    const bool fast_fits = events_fast_smem_bytes(max_ns, max_nz) <= kMaxSmemOptin;
+    for (int i = 0; i < n_events; ++i) (fast_fits && tk_h[i] > 0.0 && udz[i] > 0.0 ? fast_ev : slow_ev).push_back(i);
     // replace the previous set
     cudaStreamSynchronize(ctx->stream);
     free_pool(ctx->owned_grp);
@@ -576,6 +623,9 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     CK(upload(ctx->owned_ev, &E.tk_c, tk_c)); CK(upload(ctx->owned_ev, &E.tk_h, tk_h));
     CK(upload(ctx->owned_ev, &E.poly_off, poff)); CK(upload(ctx->owned_ev, &E.prec_a, prec_a)); CK(upload(ctx->owned_ev, &E.prec_b, prec_b));
     if (fixed_bw) CK(upload(ctx->owned_ev, &E.fixed_bw, h_bw));
+    CK(upload(ctx->owned_ev, &E.qn4, qn4)); CK(upload(ctx->owned_ev, &E.q4_off, q4off));
+    CK(upload(ctx->owned_ev, &ctx->fast_ev, fast_ev)); CK(upload(ctx->owned_ev, &ctx->slow_ev, slow_ev));
+    ctx->n_fast = (int)fast_ev.size(); ctx->n_slow = (int)slow_ev.size();
     CK(upload(ctx->owned_ev, &ctx->ev_ln_shift, shift));
     CK(upload(ctx->owned_ev, &ctx->ev_ln_qscale, qshift));
     ctx->ev = E;
@@ -836,8 +886,8 @@ int chim_get_kernel_times(chim_ctx* ctx, chim_kernel_times* out) {
     CK(cudaSetDevice(ctx->cfg.device));
     CK(cudaStreamSynchronize(ctx->stream));
     std::memset(out, 0, sizeof(*out));
-    double* ms[4] = {&out->tables_ms, &out->events_ms, &out->inject_ms, &out->combine_ms};
-    uint32_t* nl[4] = {&out->tables_launches, &out->events_launches, &out->inject_launches, &out->combine_launches};
+    double* ms[5] = {&out->tables_ms, &out->events_ms, &out->inject_ms, &out->combine_ms, &out->events_general_ms};
+    uint32_t* nl[5] = {&out->tables_launches, &out->events_launches, &out->inject_launches, &out->combine_launches, &out->events_general_launches};
     for (size_t i = 0; i < ctx->ev_kind.size(); ++i) {
         float t = 0.f;
         CK(cudaEventElapsedTime(&t, ctx->ev_pool[2 * i], ctx->ev_pool[2 * i + 1]));

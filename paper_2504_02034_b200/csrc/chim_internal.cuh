@@ -312,14 +312,14 @@ __device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restri
 template <bool kFit>
 __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, const float cpsi, const PolyCoef& C, const float4 A,
                                             const float2 Bq, const MassLookup& M, const float tm_lo, const float tm_hi,
-                                            float& zc, float& l2w) {
+                                            float& zc, float& l2w, float& mp2) {
     const f32x2 t2 = pack2(A.x, A.x);
     f32x2 zr = C.zr[6], ua = C.ua[5];
 #pragma unroll
     for (int n = 5; n >= 0; --n) zr = fma2(zr, t2, C.zr[n]);
 #pragma unroll
     for (int n = 4; n >= 0; --n) ua = fma2(ua, t2, C.ua[n]);
-    float r, u, a, mp1, mp2;
+    float r, u, a, mp1;
     unpack2(zr, zc, r);
     unpack2(ua, u, a);
     unpack2(fma2(pack2(A.y, A.z), pack2(a, a), pack2(-F.mlow_hi, -F.mlow_hi)), mp1, mp2);   // m' = m^d a - m_low
@@ -352,6 +352,37 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
         l -= (mp2 < F.delta) ? ls : 0.f;
     }
     l2w = (mp2 > 0.f) ? l : -INFINITY;      // R15 support: m_low < m2
+}
+template <bool kFit>
+__device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, const float cpsi, const PolyCoef& C, const float4 A,
+                                            const float2 Bq, const MassLookup& M, const float tm_lo, const float tm_hi,
+                                            float& zc, float& l2w) {
+    float mp2;
+    poly_sample<kFit>(F, gk2, cpsi, C, A, Bq, M, tm_lo, tm_hi, zc, l2w, mp2);
+}
+
+// ---- TMA bulk copy + mbarrier  ---------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* b) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(b))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok)
+                     : "r"(smem_u32(b)), "r"(parity)
+                     : "memory");
+    } while (!ok);
 }
 
 // ---- small reductions ---------------------------------------------------------------------------------
@@ -410,6 +441,9 @@ struct EventSetDev {
     const int64_t* poly_off;    // [n_events+1] offsets into prec (events padded to a multiple of 32 samples)
     const float4* prec_a;       // records of the polynomial sweep: {t in [-1,1], m1d, m2d, ln m1d}
     const float2* prec_b;       //                                  {ln m2d, log2(1/prior) - scale}
+    // k_events_fast: qn again with every event's slice starting at a multiple of 4 floats and zero-padded to one (TMA source)
+    const float* qn4;
+    const int64_t* q4_off;      // [n_events]
 };
 
 struct EventKernelParams {
@@ -427,9 +461,28 @@ struct EventKernelParams {
     const double* ln_shift;  // [n_events] prior scale factored out of the weights, added back to log I
     const double* ln_qscale; // [n_events] ln of the event's largest q_g (qn = q / that), added back to log I
     const float* poly;       // [n_lambda][n_events][4 kPolyN] event-local polynomials fitted by k_polyfit
+    const int32_t* ev_list;  // null, or the events this launch covers (n_ev_list of them; the others belong to k_events_fast)
+    int32_t n_ev_list;
+    const uint32_t* worklist;      // null, or the units (lambda * n_events + event) handed over by k_events_fast ...
+    const unsigned int* work_count;// ... and their number; worklist_ctas CTAs loop over them
+    int32_t worklist_ctas;
     // diagnostics (single event, single lambda) -- null in the hot path
     int32_t dbg_event;       // >= 0: blockIdx.x addresses lambda only, event = dbg_event
     double* dbg_z; double* dbg_w; double* dbg_h; double* dbg_K;
+};
+
+// k_events_fast (k_events_fast.cu): the regular units; everything else goes to k_events through the work list
+struct FastEventParams {
+    EventSetDev ev;
+    const LamConst* Lc;
+    const MassRow* mtab;     // [n_lambda][2][n_mass+2]
+    const float* poly;       // [n_lambda][n_events][4 kPolyN]
+    int32_t n_lambda, n_mass, bw_rule;
+    double cutoff;
+    double* logI;            // [n_lambda][n_events]
+    const double* ln_shift; const double* ln_qscale;
+    const int32_t* fast_events;   // the events this kernel takes (narrow d_L range, equally spaced grid)
+    uint32_t* worklist; unsigned int* work_count;
 };
 
 struct InjSetDev {
@@ -478,6 +531,8 @@ cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int
                            const double* lnm1_lo, const double* lnm1_hi, int n_mass, int mcap, float* out, cudaStream_t st);
 int events_mass_stage_rows(int n_mass);   // rows of the mass table a k_events CTA stages per variant
 cudaError_t launch_events(const EventKernelParams& P, bool count_pairs, cudaStream_t st);
+cudaError_t launch_events_fast(const FastEventParams& P, int n_fast, cudaStream_t st);
+size_t events_fast_smem_bytes(int max_ns, int max_nz);
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st);
 cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);
 cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, int64_t n, const double* dL,

@@ -50,30 +50,6 @@ constexpr int kLeP = 12;                 // terms of the local expansion (degree
 constexpr int kLeMaxBox = 96;            // boxes per event the local-expansion form accepts
 constexpr float kLeMaxW = 1.3f;          // largest box width in units of sqrt(2) h (truncation error)
 
-// ---- TMA bulk copy + mbarrier (one-shot: phase 0) ---------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* b) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(b))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok)
-                     : "r"(smem_u32(b)), "r"(parity)
-                     : "memory");
-    } while (!ok);
-}
-
 // psi(z)/J(z) at a grid point for placement ON_GRID (paper eq. 14 literally); d_C from the global table.
 __device__ double grid_factor(const LamConst& L, const double* __restrict__ dc, int n_nodes, double dz, double z) {
     double x = z / dz;
@@ -480,9 +456,10 @@ __device__ __noinline__ double exact_log2_kde(const LamConst& L, const double* _
 }
 
 // shared-memory layout after EvSmem: zf float[ns_pad] | wl float[ns_pad] | aux = staged table rows + mass rows (S2) / gq float2[nz_pad] (S3)
+// One (event, lambda) unit.  Block-uniform returns only.  again: the CTA has processed a unit before (work-list mode): the
+// one-shot mbarrier is invalidated and initialised anew.
 template <bool kStats>
-__global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKernelParams P) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
+__device__ __forceinline__ void events_unit(const EventKernelParams& P, const int l, const int ev, unsigned char* smem_raw, const bool again) {
     EvSmem& S = *reinterpret_cast<EvSmem*>(smem_raw);
     float* zf = reinterpret_cast<float*>(smem_raw + ((sizeof(EvSmem) + 127) / 128) * 128);
     const size_t ns_pad = ev_ns_pad(P.ev.max_ns);
@@ -494,9 +471,6 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     MassRow* mass_s = reinterpret_cast<MassRow*>(aux + (size_t)kRowStage * sizeof(Row));
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
 
-    int l, ev;
-    if (P.dbg_event >= 0) { l = blockIdx.x; ev = P.dbg_event; }
-    else { l = blockIdx.x % P.n_lambda; ev = blockIdx.x / P.n_lambda; }   // lambda fastest: CTAs in flight share an event
     const int64_t s0 = P.ev.sample_off[ev], g0 = P.ev.grid_off[ev];
     const int ns = (int)(P.ev.sample_off[ev + 1] - s0), nz = (int)(P.ev.grid_off[ev + 1] - g0);
     double* out = (P.dbg_event >= 0) ? P.logI + l : P.logI + (size_t)l * P.ev.n_events + ev;
@@ -513,6 +487,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         for (int i = tid; i < nw; i += kEvThreads) dst[i] = src[i];
         if (tid == 0) {
             S.pass_counter = 0;
+            if (again) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&S.mbar)) : "memory");
             mbar_init(&S.mbar, 1);
             // polynomial path: the stage bounds were computed by k_polyfit, so the TMA copy of the mass rows starts now and
             // runs beside the staging of the constants (the same test as use_poly below, on the global copy of the constants)
@@ -1050,6 +1025,32 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
     }
 }
 
+// Grid: (events x lambdas) with lambda fastest [optionally through ev_list: the events k_events_fast does not take], or --
+// work-list mode -- a fixed number of CTAs that loop over the units k_events_fast handed over in this batch.
+template <bool kStats>
+__global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKernelParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    if (P.worklist) {
+        const unsigned n = *P.work_count;
+        bool again = false;
+        for (unsigned u = blockIdx.x; u < n; u += gridDim.x) {
+            const uint32_t unit = P.worklist[u];
+            events_unit<kStats>(P, (int)(unit / (uint32_t)P.ev.n_events), (int)(unit % (uint32_t)P.ev.n_events), smem_raw, again);
+            again = true;
+            __syncthreads();
+        }
+        return;
+    }
+    int l, ev;
+    if (P.dbg_event >= 0) { l = blockIdx.x; ev = P.dbg_event; }
+    else {   // lambda fastest: CTAs in flight share an event
+        l = blockIdx.x % P.n_lambda;
+        ev = blockIdx.x / P.n_lambda;
+        if (P.ev_list) ev = P.ev_list[ev];
+    }
+    events_unit<kStats>(P, l, ev, smem_raw, false);
+}
+
 int events_mass_stage_rows(int n_mass) { return min(kMassStage, n_mass + 2); }
 
 size_t events_smem_bytes(int max_ns, int max_nz) {
@@ -1061,7 +1062,8 @@ cudaError_t launch_events(const EventKernelParams& P, bool count_pairs, cudaStre
     auto kern = count_pairs ? k_events<true> : k_events<false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    long long nb = (P.dbg_event >= 0) ? P.n_lambda : (long long)P.n_lambda * P.ev.n_events;
+    long long nb = (P.dbg_event >= 0) ? P.n_lambda : (long long)P.n_lambda * (P.ev_list ? P.n_ev_list : P.ev.n_events);
+    if (P.worklist) nb = P.worklist_ctas;
     if (nb <= 0) return cudaSuccess;
     kern<<<(unsigned)nb, kEvThreads, smem, st>>>(P);
     return cudaGetLastError();

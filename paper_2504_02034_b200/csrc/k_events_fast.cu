@@ -1,0 +1,413 @@
+// k_events_fast.cu -- steps S2 + S3 + S4 for the regular case, one CTA per (event, lambda): narrow distance posterior
+// (event-local polynomials), equally spaced redshift grid, Gaussian kernel in the local-expansion
+// form, placement ON_SAMPLES.  Everything else -- wide events, other kernels / forms / placements,
+// binning, diagnostics -- and every unit this kernel finds outside its reach (no or few effective samples, the heaviest
+// sample deep in the smoothing window, a bandwidth the expansion cannot take: DESIGN.md R21) is left to k_events: the unit
+// is appended to a work list that k_events processes in the same batch call.
+//
+// Structure (what differs from k_events): after one barrier the eight warps are independent.  Warp w owns a contiguous chunk
+// of the (d_L-sorted) samples and runs S2 on it alone -- sweep 1 with the 26 polynomial coefficients in registers, its own
+// maximum, sweep 2 relative to that -- leaving chunk statistics {max, heaviest sample, W, Q, B, A about and excluding it}.
+// One barrier; every warp combines the eight chunk statistics in fp64 (exactly: Scott's rule in the cancellation-free form
+// of R21), derives bandwidth and expansion geometry redundantly, the psi table is built once per CTA; one barrier; every
+// warp then builds the expansion coefficients of the boxes ITS samples fall in and evaluates its samples -- no further
+// block-wide step until the eight partial sums are added.  q_g and the mass-table rows arrive by TMA bulk copies issued
+// before the first barrier.
+#include "chim_internal.cuh"
+
+namespace chim {
+
+#ifndef CHIM_FAST_BLOCKS
+#define CHIM_FAST_BLOCKS 3
+#endif
+#ifndef CHIM_FAST_UNROLL
+#define CHIM_FAST_UNROLL 2
+#endif
+constexpr int kFUnroll = CHIM_FAST_UNROLL;
+constexpr int kFT = 256;             // threads per CTA
+constexpr int kFW = kFT / 32;        // warps = sample chunks
+constexpr int kFPass = 128;          // samples per warp pass (4 per lane)
+constexpr int kFLeP = 12;            // terms of the local expansion
+constexpr int kFMaxBox = 96;         // boxes per event
+constexpr float kFMaxW = 1.3f;       // largest box width in units of sqrt(2) h
+constexpr int kFMaxD = 160;          // largest half-width of the psi table (grid points)
+constexpr int kFQPad = 2 * kFMaxD;   // zeros on both sides of the staged q_g: the coefficient build reads g_b +- d unchecked
+constexpr int kFMassStage = 384;     // mass-table rows staged per variant (= events_mass_stage_rows: k_polyfit sizes the slice)
+
+struct FastSmem {
+    unsigned long long mbar_mass, mbar_q;
+    float c_mx[kFW], c_zr[kFW];      // per chunk: largest log2 w; z - z0 of the chunk's first sample (reference of its moments)
+    float c_mp2[kFW];                // per chunk: largest m2' = m2 - m_low among its samples
+    float c_mom[kFW][4];             // sum w, sum w^2, sum w u, sum w u^2 with w relative to the chunk's largest, u = z - c_zr
+    double c_sum[kFW];               // per chunk: sum_j w_j A_j relative to the event's heaviest sample
+};
+
+__host__ __device__ inline int fast_chunk(int ns) { return ((ns + kFW * kFPass - 1) / (kFW * kFPass)) * kFPass; }
+__host__ __device__ inline size_t fast_nz4(size_t nz) { return (nz + 3) / 4 * 4; }
+__host__ __device__ inline size_t fast_aux_bytes() {
+    const size_t a = 2 * (size_t)kFMassStage * sizeof(MassRow);
+    const size_t b = 4 * (size_t)kFLeP * ((size_t)(kFMaxD + 1) + (size_t)(kFMaxBox + kFW));
+    return a > b ? a : b;
+}
+size_t events_fast_smem_bytes(int max_ns, int max_nz) {
+    return ((sizeof(FastSmem) + 127) / 128) * 128 + 2 * sizeof(float) * (size_t)kFW * fast_chunk(max_ns) +
+           sizeof(float) * (2 * (size_t)kFQPad + fast_nz4((size_t)max_nz)) + fast_aux_bytes();
+}
+
+__global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEventParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    FastSmem& S = *reinterpret_cast<FastSmem*>(smem_raw);
+    float2* zw = reinterpret_cast<float2*>(smem_raw + ((sizeof(FastSmem) + 127) / 128) * 128);   // (z_j - z0, log2 w_j -> w_j)
+    float* qs = reinterpret_cast<float*>(zw + (size_t)kFW * fast_chunk(P.ev.max_ns));            // [kFQPad | nz4 | kFQPad]
+    unsigned char* aux = reinterpret_cast<unsigned char*>(qs + 2 * (size_t)kFQPad + fast_nz4((size_t)P.ev.max_nz));
+    MassRow* mass_s = reinterpret_cast<MassRow*>(aux);                  // S2: both variants of the event's slice of the mass table
+    float* psi = reinterpret_cast<float*>(aux);                         // S3: psi table [(D+1) x 12] ...
+    float* Bc = psi + (size_t)kFLeP * (kFMaxD + 1);                     // ... and the expansion coefficients [box][12]
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+
+    const int l = blockIdx.x % P.n_lambda;                              // lambda fastest: CTAs in flight share an event
+    const int ev = P.fast_events[blockIdx.x / P.n_lambda];
+    const int64_t s0 = P.ev.sample_off[ev], g0 = P.ev.grid_off[ev];
+    const int ns = (int)(P.ev.sample_off[ev + 1] - s0), nz = (int)(P.ev.grid_off[ev + 1] - g0);
+    double* out = P.logI + (size_t)l * P.ev.n_events + ev;
+    const LamConst* Lg = P.Lc + l;
+    if (__ldg(&Lg->flags)) {   // invalid lambda: NaN
+        if (tid == 0) *out = NAN;
+        return;
+    }
+    const float* pr = P.poly + ((size_t)l * P.ev.n_events + ev) * (4 * kPolyN);
+    // the event-local polynomials exist (k_polyfit) iff the whole d_L range of the event lies inside the table
+    int mlo = 0, nr = 0;
+    {
+        const double tk_h = __ldg(P.ev.tk_h + ev), tk_c = __ldg(P.ev.tk_c + ev);
+        if (tk_h > 0.0 && tk_c + tk_h < __ldg(&Lg->tkmax_ev)) {
+            mlo = __float_as_int(__ldg(pr + 26));
+            nr = __float_as_int(__ldg(pr + 27));    // > 0: every mass-table row the event can address fits the stage
+        }
+    }
+#define CHIM_FAST_HANDOVER()                                                    \
+    do {                                                                        \
+        if (tid == 0) {                                                         \
+            const unsigned k_ = atomicAdd(P.work_count, 1u);                    \
+            P.worklist[k_] = (uint32_t)l * (uint32_t)P.ev.n_events + (uint32_t)ev; \
+        }                                                                       \
+        return;                                                                 \
+    } while (0)
+    if (nr <= 0) CHIM_FAST_HANDOVER();
+
+    const size_t nz4 = fast_nz4((size_t)nz);
+    const MassRow* mtab = P.mtab + (size_t)l * 2 * (P.n_mass + 2);
+    if (tid == 0) {
+        mbar_init(&S.mbar_mass, 1);
+        mbar_init(&S.mbar_q, 1);
+        const uint32_t mbytes = (uint32_t)nr * (uint32_t)sizeof(MassRow);
+        mbar_expect_tx(&S.mbar_mass, 2 * mbytes);
+        bulk_g2s(mass_s, mtab + mlo, mbytes, &S.mbar_mass);
+        bulk_g2s(mass_s + kFMassStage, mtab + (P.n_mass + 2) + mlo, mbytes, &S.mbar_mass);
+        const uint32_t qbytes = (uint32_t)nz4 * 4u;
+        mbar_expect_tx(&S.mbar_q, qbytes);
+        bulk_g2s(qs + kFQPad, P.ev.qn4 + P.ev.q4_off[ev], qbytes, &S.mbar_q);
+    }
+    for (int i = tid; i < kFQPad; i += kFT) {
+        qs[i] = 0.f;
+        qs[kFQPad + nz4 + i] = 0.f;
+    }
+    // per-thread copies: the 26 polynomial coefficients and the fp32 constants of S2
+    PolyCoef Cf;
+    {
+        const f32x2* q = reinterpret_cast<const f32x2*>(pr);
+#pragma unroll
+        for (int n = 0; n < kPolyN; ++n) Cf.zr[n] = __ldg(q + n);
+#pragma unroll
+        for (int n = 0; n < kPolyN - 1; ++n) Cf.ua[n] = __ldg(q + kPolyN + n);
+    }
+    const LamF F = Lg->F;
+    __syncthreads();                                                    // (1) the barriers are initialised
+    MassLookup M;
+    M.g = mtab;
+    M.s = mass_s;
+    M.lo = mlo;
+    M.cap = kFMassStage;
+    M.n_mass = P.n_mass;
+    const float tm_lo = fmaxf(1.0f, (float)mlo), tm_hi = fminf(F.tm_max, (float)(mlo + nr) - 0.01f);
+
+    // ---- S2 on the warp's chunk [c0, c1): (z_j - z0, log2 w_j) pairs to shared memory, then w_j relative to the chunk's largest ---------
+    const int C = fast_chunk(ns);
+    const int c0 = wid * C, c1 = min(c0 + C, ns);
+    const int64_t p0 = P.ev.poly_off[ev];
+    float mx = -INFINITY, mp2x = -INFINITY;
+    mbar_wait(&S.mbar_mass, 0);
+    if (c0 < ns) {
+        const float4* pa = P.ev.prec_a + p0;
+        const float2* pb = P.ev.prec_b + p0;
+        const int nfull = c0 + ((c1 - c0) & ~31);                       // end of the whole blocks of 32 samples
+        int j = c0 + lane;
+        PRec R = ldg_stream_prec(pa + j, pb + j);                       // the record arrays carry a spare tail: unconditional
+#pragma unroll(kFUnroll)
+        for (; j < nfull; j += 32) {
+            const float4 A = R.A;
+            const float2 Bq = R.B;
+            R = ldg_stream_prec(pa + j + 32, pb + j + 32);              // one iteration ahead
+            float zc, l2w, mp2;
+            poly_sample<true>(F, F.gk2, F.cpsi, Cf, A, Bq, M, tm_lo, tm_hi, zc, l2w, mp2);
+            zw[j] = make_float2(zc, l2w);
+            mx = fmaxf(mx, l2w);
+            mp2x = fmaxf(mp2x, mp2);
+        }
+        if (nfull < c1) {   // the ragged end of the event (its records are padded to whole warps: poly_sample votes)
+            float zc, l2w, mp2;
+            poly_sample<true>(F, F.gk2, F.cpsi, Cf, R.A, R.B, M, tm_lo, tm_hi, zc, l2w, mp2);
+            if (j < c1) {
+                zw[j] = make_float2(zc, l2w);
+                mx = fmaxf(mx, l2w);
+                mp2x = fmaxf(mp2x, mp2);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            mp2x = fmaxf(mp2x, __shfl_xor_sync(0xffffffffu, mp2x, o));
+        }
+        __syncwarp();
+        // sweep 2: w = 2^(log2 w - chunk max); plain weighted moments about the chunk's first sample (the cancellation-free form of
+        // R21 is only needed below n_eff ~ 1, and such units are handed over); idle slots of the last pass sit on the chunk's last
+        // sample with weight 0
+        const float mref = (mx > -INFINITY) ? mx : 0.f, zr = zw[c0].x, zlast = zw[c1 - 1].x;
+        float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;
+        const int pend = c0 + ((c1 - c0 + kFPass - 1) / kFPass) * kFPass;
+        for (int j4 = c0 + 4 * lane; j4 < pend; j4 += kFPass) {
+            float4 ab = *reinterpret_cast<const float4*>(zw + j4), cd4 = *reinterpret_cast<const float4*>(zw + j4 + 2);
+            float zv[4] = {ab.x, ab.z, cd4.x, cd4.z};
+            const float lv[4] = {ab.y, ab.w, cd4.y, cd4.w};
+            float wv[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const bool valid = j4 + r < c1;
+                const float w = valid ? ex2f(lv[r] - mref) : 0.f;
+                zv[r] = valid ? zv[r] : zlast;
+                wv[r] = w;
+                const float u = zv[r] - zr, wu = w * u;
+                m0 += w;
+                m1 = fmaf(w, w, m1);
+                m2 += wu;
+                m3 = fmaf(wu, u, m3);
+            }
+            *reinterpret_cast<float4*>(zw + j4) = make_float4(zv[0], wv[0], zv[1], wv[1]);
+            *reinterpret_cast<float4*>(zw + j4 + 2) = make_float4(zv[2], wv[2], zv[3], wv[3]);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            m0 += __shfl_xor_sync(0xffffffffu, m0, o);
+            m1 += __shfl_xor_sync(0xffffffffu, m1, o);
+            m2 += __shfl_xor_sync(0xffffffffu, m2, o);
+            m3 += __shfl_xor_sync(0xffffffffu, m3, o);
+        }
+        if (lane == 0) {
+            S.c_mx[wid] = mx; S.c_zr[wid] = zr; S.c_mp2[wid] = mp2x;
+            S.c_mom[wid][0] = m0; S.c_mom[wid][1] = m1; S.c_mom[wid][2] = m2; S.c_mom[wid][3] = m3;
+        }
+    } else if (lane == 0) {
+        S.c_mx[wid] = -INFINITY; S.c_zr[wid] = 0.f; S.c_mp2[wid] = -INFINITY;
+        S.c_mom[wid][0] = 0.f; S.c_mom[wid][1] = 0.f; S.c_mom[wid][2] = 0.f; S.c_mom[wid][3] = 0.f;
+    }
+    __syncthreads();                                                    // (2) chunk statistics and the samples are complete
+
+    // ---- every warp: the event's moments from the eight chunks (lane c takes chunk c), bandwidth, expansion geometry -------------
+    // fp32 throughout: all sums are sums of positive terms (the second moment is taken about the weighted mean in a second
+    // step), n_eff >= 64 on this path, and dh/h = 1e-6 moves log I by ~5e-9
+    const float cm = (lane < kFW) ? S.c_mx[lane] : -INFINITY;
+    float gmx = cm, gmp2 = (lane < kFW) ? S.c_mp2[lane] : -INFINITY;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) {
+        gmx = fmaxf(gmx, __shfl_xor_sync(0xffffffffu, gmx, o));
+        gmp2 = fmaxf(gmp2, __shfl_xor_sync(0xffffffffu, gmp2, o));
+    }
+    gmx = __shfl_sync(0xffffffffu, gmx, 0);
+    gmp2 = __shfl_sync(0xffffffffu, gmp2, 0);
+    mbar_wait(&S.mbar_q, 0);                                            // q_g has landed (also: no copy in flight at any exit below)
+    if (!(gmx > -INFINITY) || gmx != gmx) CHIM_FAST_HANDOVER();         // no weighted sample on this path: k_events decides
+    const bool live = lane < kFW && cm > -INFINITY;
+    const float f = live ? ex2f(cm - gmx) : 0.f;                        // chunk-relative weights -> relative to the event's largest
+    const float dl = live ? S.c_zr[lane] - S.c_zr[0] : 0.f;             // chunk reference relative to the first chunk's
+    const float wc = live ? S.c_mom[lane][0] : 0.f, qc = live ? S.c_mom[lane][1] : 0.f;
+    const float bc = live ? S.c_mom[lane][2] : 0.f, ac = live ? S.c_mom[lane][3] : 0.f;
+    float SW = f * wc, SQ = f * f * qc, SB = f * fmaf(dl, wc, bc);
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) {
+        SW += __shfl_xor_sync(0xffffffffu, SW, o);
+        SQ += __shfl_xor_sync(0xffffffffu, SQ, o);
+        SB += __shfl_xor_sync(0xffffffffu, SB, o);
+    }
+    SW = __shfl_sync(0xffffffffu, SW, 0);
+    SQ = __shfl_sync(0xffffffffu, SQ, 0);
+    SB = __shfl_sync(0xffffffffu, SB, 0);
+    const float ubar = SB / SW, de = dl - ubar;                         // weighted mean (relative to the first chunk's reference)
+    float SA = f * fmaf(de, fmaf(de, wc, 2.f * bc), ac);                // sum w (u + de)^2 >= 0 per chunk
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) SA += __shfl_xor_sync(0xffffffffu, SA, o);
+    SA = __shfl_sync(0xffffffffu, SA, 0);
+    const float s2 = SQ / (SW * SW), neff = 1.0f / s2;                  // sum w^2, Kish n_eff
+    double h;
+    if (P.bw_rule == CHIM_BW_FIXED) {
+        h = __ldg(P.ev.fixed_bw + ev);
+    } else {   // Scott on the weighted sample (R3, O7): sigma^2 = sum w^(z - zbar)^2 / (1 - sum w^^2), h = sigma n_eff^(-1/5)
+        const float var = SA / (SW * (1.0f - s2));
+        h = (var > 0.f) ? (double)(sqrtf(var) * exp2f(0.2f * log2f(s2))) : NAN;
+    }
+    // handed over: no bandwidth; few effective samples (fp32 weights, moments and the plain form of Scott's rule are good for
+    // n_eff >> 1 only); every supported secondary deep in the smoothing window (m2' < ~0.3 sqrt(delta): d ln w = delta/m2'^2 x 1e-6)
+    bool hand = !(h > 0.0) || !isfinite(h) || !(neff >= 64.0f) || gmp2 * gmp2 < 0.1f * F.delta;
+    // local-expansion geometry: y = z'/(sqrt(2) h), boxes of m grid spacings centred on grid points
+    const double udz = __ldg(P.ev.uni_dz + ev), zfirst = __ldg(P.ev.zc + g0);
+    const float scy = (float)(0.70710678118654752440 / h);
+    const float dy = (float)(udz * (double)scy);
+    const int m = max(1, (int)lrintf(1.0f / dy));
+    const float wbox = (float)m * dy, Ty = (float)(P.cutoff * 0.70710678118654752440);
+    const float yfirst = (float)(zfirst * (double)scy), inv_w = 1.0f / wbox;
+    const float fb_lo = floorf((zw[0].x * scy - yfirst) * inv_w + 0.5f), fb_hi = floorf((zw[ns - 1].x * scy - yfirst) * inv_w + 0.5f);
+    const float fD = ceilf((Ty + 0.5f * wbox) / dy) + 1.0f;
+    hand = hand || !(wbox <= kFMaxW) || !(fb_hi - fb_lo < (float)kFMaxBox) || !(fabsf(fb_lo) < 1e6f) || !(fabsf(fb_hi) < 1e6f) ||
+           !(fD <= (float)kFMaxD) || !(fabsf(fb_lo) * (float)m < 1e8f) || !(fabsf(fb_hi) * (float)m < 1e8f);
+    if (hand) CHIM_FAST_HANDOVER();
+    const int D = (int)fD, b_lo = (int)fb_lo, nbox = (int)(fb_hi - fb_lo) + 1;
+    // psi table: psi_n(d dy) = exp(-t^2) H_n(t)/n!, t = d dy, by the three-term recurrence (one d per thread)
+    for (int d = tid; d <= D; d += kFT) {
+        const float t = (float)d * dy, t2 = 2.f * t;
+        float p0v = ex2f(-t * t * 1.44269504088896341f), p1v = t2 * p0v;
+        float* o = psi + (size_t)d * kFLeP;
+        o[0] = p0v;
+        o[1] = p1v;
+#pragma unroll
+        for (int n = 1; n < kFLeP - 1; ++n) {
+            const float p2v = fmaf(t2, p1v, -2.f * p0v) * (1.0f / (float)(n + 1));
+            o[n + 1] = p2v;
+            p0v = p1v;
+            p1v = p2v;
+        }
+    }
+    __syncthreads();                                                    // (3) psi table (the staged mass rows are dead)
+
+    // ---- S3 + S4 on the warp's chunk: coefficients of its own boxes, then one degree-11 polynomial per sample ------------------
+    double lsum = 0.0;
+    if (c0 < ns) {
+        const int bw0 = min(max((int)floorf((zw[c0].x * scy - yfirst) * inv_w + 0.5f) - b_lo, 0), nbox - 1);
+        const int bw1 = min(max((int)floorf((zw[c1 - 1].x * scy - yfirst) * inv_w + 0.5f) - b_lo, bw0), nbox - 1);
+        const int nbw = bw1 - bw0 + 1;
+        float* Bw = Bc + (size_t)(bw0 + wid) * kFLeP;                    // (neighbouring chunks share at most one box: shifted by wid)
+        // coefficients B_bn = sum_{|d| <= D} q_{g_b+d} psi_n(d dy): lane = (half of the d range, box, quad of n), five boxes per
+        // round; psi_n(-t) = (-1)^n psi_n(t), so even n take (q_+ + q_-) psi_n and odd n (q_+ - q_-) psi_n -- the pairs (n, n+1)
+        // of a packed FMA
+        const int half = lane >= 15 ? 1 : 0, sub = lane - 15 * half, quad = sub % 3, bsub = sub / 3;
+        const int Dh = D >> 1, d_lo = half ? Dh + 1 : 1, d_hi = half ? D : Dh;
+        for (int base = 0; base < nbw; base += 5) {
+            const int bi = base + bsub;
+            const bool valid = lane < 30 && bi < nbw;
+            const int gc = (b_lo + bw0 + (valid ? bi : 0)) * m;         // grid index of the box centre
+            const bool reach = valid && gc > -D - 1 && gc < nz + D;     // else no grid point within the box's cut-off: B = 0
+            const float* qp = qs + kFQPad + (reach ? gc : 0) + d_lo;
+            const float* qm = qs + kFQPad + (reach ? gc : 0) - d_lo;
+            const float4* pp = reinterpret_cast<const float4*>(psi) + quad + d_lo * (kFLeP / 4);
+            f32x2 a01 = 0ull, a23 = 0ull;
+            if (reach && !half) {   // d = 0: psi_odd(0) = 0
+                const float q0 = qp[-d_lo];
+                const float4 v = reinterpret_cast<const float4*>(psi)[quad];
+                a01 = pack2(q0 * v.x, 0.f);
+                a23 = pack2(q0 * v.z, 0.f);
+            }
+            int n = reach ? d_hi - d_lo + 1 : 0;
+#pragma unroll 1
+            for (; n >= 4; n -= 4) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const float a = qp[k], b = qm[-k];
+                    const float4 v = pp[k * (kFLeP / 4)];
+                    const f32x2 qeo = pack2(a + b, a - b);
+                    a01 = fma2(qeo, pack2(v.x, v.y), a01);
+                    a23 = fma2(qeo, pack2(v.z, v.w), a23);
+                }
+                qp += 4;
+                qm -= 4;
+                pp += 4 * (kFLeP / 4);
+            }
+            for (; n > 0; --n) {
+                const float a = *qp, b = *qm;
+                const float4 v = *pp;
+                const f32x2 qeo = pack2(a + b, a - b);
+                a01 = fma2(qeo, pack2(v.x, v.y), a01);
+                a23 = fma2(qeo, pack2(v.z, v.w), a23);
+                ++qp;
+                --qm;
+                pp += kFLeP / 4;
+            }
+            float4 acc;
+            unpack2(a01, acc.x, acc.y);
+            unpack2(a23, acc.z, acc.w);
+            acc.x += __shfl_down_sync(0xffffffffu, acc.x, 15);          // the two halves of the d range
+            acc.y += __shfl_down_sync(0xffffffffu, acc.y, 15);
+            acc.z += __shfl_down_sync(0xffffffffu, acc.z, 15);
+            acc.w += __shfl_down_sync(0xffffffffu, acc.w, 15);
+            if (valid && !half) reinterpret_cast<float4*>(Bw + (size_t)bi * kFLeP)[quad] = acc;
+        }
+        __syncwarp();
+        // evaluation: passes of 128 consecutive (sorted) samples, 4 per lane; the boxes a pass touches are visited in turn
+        const int bofs = b_lo + bw0;
+        const int pend = c0 + ((c1 - c0 + kFPass - 1) / kFPass) * kFPass;
+        for (int j0 = c0 + 4 * lane; j0 < pend; j0 += kFPass) {
+            const float4 ab = *reinterpret_cast<const float4*>(zw + j0), cd4 = *reinterpret_cast<const float4*>(zw + j0 + 2);
+            const float y[4] = {ab.x * scy, ab.z * scy, cd4.x * scy, cd4.z * scy};
+            int bx[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) bx[r] = min(max((int)floorf(fmaf(y[r] - yfirst, inv_w, 0.5f)) - bofs, 0), nbw - 1);
+            const int bmin = __reduce_min_sync(0xffffffffu, min(min(bx[0], bx[1]), min(bx[2], bx[3])));
+            const int bmax = __reduce_max_sync(0xffffffffu, max(max(bx[0], bx[1]), max(bx[2], bx[3])));
+            float A[4] = {0.f, 0.f, 0.f, 0.f};
+            for (int i = bmin; i <= bmax; ++i) {
+                const float c = fmaf((float)((bofs + i) * m), dy, yfirst);
+                const float4* bp = reinterpret_cast<const float4*>(Bw + (size_t)i * kFLeP);
+                const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
+                const f32x2 s01 = pack2(y[0] - c, y[1] - c), s23 = pack2(y[2] - c, y[3] - c);
+                f32x2 a01 = pack2(k2.w, k2.w), a23 = a01;
+#define CHIM_LE_STEP(cf) { const f32x2 q_ = pack2(cf, cf); a01 = fma2(a01, s01, q_); a23 = fma2(a23, s23, q_); }
+                CHIM_LE_STEP(k2.z) CHIM_LE_STEP(k2.y) CHIM_LE_STEP(k2.x)
+                CHIM_LE_STEP(k1.w) CHIM_LE_STEP(k1.z) CHIM_LE_STEP(k1.y) CHIM_LE_STEP(k1.x)
+                CHIM_LE_STEP(k0.w) CHIM_LE_STEP(k0.z) CHIM_LE_STEP(k0.y) CHIM_LE_STEP(k0.x)
+#undef CHIM_LE_STEP
+                float v[4];
+                unpack2(a01, v[0], v[1]);
+                unpack2(a23, v[2], v[3]);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) A[r] = (bx[r] == i) ? v[r] : A[r];
+            }
+            lsum += (double)fmaf(ab.y, A[0], fmaf(ab.w, A[1], fmaf(cd4.y, A[2], cd4.w * A[3])));
+        }
+        lsum = warp_sum(lsum) * (double)exp2f(S.c_mx[wid] - gmx);       // chunk-relative weights -> relative to the event's largest
+    }
+    if (lane == 0) S.c_sum[wid] = lsum;
+    __syncthreads();                                                    // (4)
+    if (tid == 0) {
+        double tot = 0.0;
+#pragma unroll
+        for (int k = 0; k < kFW; ++k) tot += S.c_sum[k];                // fixed order: deterministic
+        // K(z) = 1/(N_s h sqrt(2 pi)) sum_j w_j exp(..); the weights were divided by 2^gmx, the prior and q_g scales factored out
+        const double I = tot / ((double)ns * h * 2.50662827463100050242);
+        if (I > 0.0 && isfinite(I)) {
+            *out = log(I) + (double)gmx * 0.69314718055994530942 + __ldg(P.ln_shift + ev) + __ldg(P.ln_qscale + ev);
+        } else {   // nothing within the cut-off (or not a number): k_events evaluates the unit in log space
+            const unsigned k_ = atomicAdd(P.work_count, 1u);
+            P.worklist[k_] = (uint32_t)l * (uint32_t)P.ev.n_events + (uint32_t)ev;
+        }
+    }
+#undef CHIM_FAST_HANDOVER
+}
+
+cudaError_t launch_events_fast(const FastEventParams& P, int n_fast, cudaStream_t st) {
+    const long long nb = (long long)P.n_lambda * n_fast;
+    if (nb <= 0) return cudaSuccess;
+    const size_t smem = events_fast_smem_bytes(P.ev.max_ns, P.ev.max_nz);
+    cudaError_t e = cudaFuncSetAttribute(k_events_fast, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_events_fast<<<(unsigned)nb, kFT, smem, st>>>(P);
+    return cudaGetLastError();
+}
+
+}  // namespace chim

@@ -32,7 +32,7 @@ def _ctx(P, w, **kw):
 def _gpu(P, w, lam=None, fixed_bw=None, **kw):
     import torch
     kw.setdefault("z_cat_max", w.z_cat_max)
-    kw.setdefault("count_pairs", 1)
+    kw.setdefault("count_pairs", 0)      # (1: every unit goes through k_events with the pair counters compiled in)
     c = P.Context(**kw)
     c.init_workload(w, fixed_bw=fixed_bw)
     lam = w.lam if lam is None else np.atleast_2d(lam)
@@ -328,6 +328,9 @@ def test_o5_shaped_ragged_multi_tile(P):
     ref = O.loglike_workload(w)
     r = _gpu(P, w, lambda_chunk=16)
     rel, dtot, dxi = _compare(r, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    r = _gpu(P, w, lambda_chunk=16, count_pairs=1)
+    rel, dtot, dxi = _compare(r, ref, w.n_events)
     print(f"o5-shaped: rel(logI)={rel:.2e} |dlogL|={dtot:.2e} |dlogxi|={dxi:.2e} pairs={r['stats']}")
     assert rel < REL_EVENT and dtot < ABS_TOTAL
     assert np.max(np.abs(r["neff"] / ref["neff"] - 1)) < 1e-5
@@ -401,9 +404,13 @@ def test_kde_local_expansion_power_and_direct_forms_agree_with_the_oracle(P):
     # form (Horner in s = 2^(-2 delta u), FFMA2), DIRECT one ex2 per pair
     w = make_workload("o5_spec", n_events=8, n_lambda=12, n_det=4000)
     ref = O.loglike_workload(w)
-    ra = _gpu(P, w, kde_method=P.CHIM_KDE_AUTO)
-    rp = _gpu(P, w, kde_method=P.CHIM_KDE_POWER)
-    rd = _gpu(P, w, kde_method=P.CHIM_KDE_DIRECT)
+    ra = _gpu(P, w, kde_method=P.CHIM_KDE_AUTO, count_pairs=1)
+    rp = _gpu(P, w, kde_method=P.CHIM_KDE_POWER, count_pairs=1)
+    rd = _gpu(P, w, kde_method=P.CHIM_KDE_DIRECT, count_pairs=1)
+    rf = _gpu(P, w)                        # the default configuration: k_events_fast (+ work list)
+    rel, dtot, _ = _compare(rf, ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL and np.max(np.abs(rf["event_logI"] - ref["event_logI"])) < 5e-6
+    assert np.max(np.abs(rf["event_logI"] - ra["event_logI"])) < 2e-6      # same expansion, other summation order
     for r in (ra, rp, rd):
         rel, dtot, _ = _compare(r, ref, w.n_events)
         assert rel < REL_EVENT and dtot < ABS_TOTAL
@@ -648,7 +655,7 @@ def test_kde_cutoff_zero_sums_every_pair(P):
     w = make_workload("tiny", n_events=3, n_samples=2, n_grid=257, n_lambda=2, n_inj_draw=1000)
     fb = np.array([0.004, 0.004, 0.01])
     ref = O.loglike_workload(w, bw_rule=O.BW_FIXED, fixed_bw=fb)
-    r = _gpu(P, w, fixed_bw=fb, bw_rule=O.BW_FIXED, kde_cutoff=0.0)
+    r = _gpu(P, w, fixed_bw=fb, bw_rule=O.BW_FIXED, kde_cutoff=0.0, count_pairs=1)
     rel, dtot, _ = _compare(r, ref, w.n_events)
     # two samples, h = 0.004, nearest galaxy ~10 h away: |d log I / dz| ~ 10/h = 2500, z_j carries 3e-8 (fp32)
     assert rel < 5e-6 and dtot < 3e-4
