@@ -18,23 +18,37 @@ constexpr double kHalfLog2e = 0.72134752044448170368;  // log2(e)/2 : exp(-d^2/2
 
 // fp32 view of the per-lambda constants used per sample / injection (S2, S5).  Values that enter a difference of
 // nearly equal numbers are carried as an unevaluated sum hi + lo of two floats.
-struct LamF {
-    float mlow_hi, mlow_lo;   // m_low
-    float lm0_hi, lm0_lo;     // ln m_low (origin of the mass table)
-    float delta;              // delta_m
-    float two_dl2e, d2l2e;    // 2 delta log2(e), delta^2 log2(e): log2(e) f = (two_dl2e m' - d2l2e) / (m' (m' - delta))
-    float win_lo, win_hi;     // clamp of m' strictly inside the smoothing window
-    float beta2;              // beta log2(e)
+struct alignas(16) LamF {
+    // the 16 constants of poly_sample first, as four 16-byte groups (k_events_fast / k_inject read them with four loads)
+    float mlow_hi;            // m_low (leading float)
+    float tm_scale;           // mass-table coordinate tm = ln(m1) tm_scale + mlow_tm, clamped to [1, tm_max]
+    float mlow_tm;            // 1 - ln(m_low) tm_scale
     float mhigh_p;            // m_high - m_low
-    float tm_scale, tm_max;   // mass-table coordinate tm = (ln m1 - ln m_low) tm_scale + 1, clamped to [1, tm_max]
+    float beta2;              // beta log2(e)
+    float delta;              // delta_m
+    float win_lo, win_hi;     // clamp of m' strictly inside the smoothing window
+    float two_dl2e, d2l2e;    // 2 delta log2(e), delta^2 log2(e): log2(e) f = (two_dl2e m' - d2l2e) / (m' (m' - delta))
+    float gk2, cpsi;          // (gamma + kappa) log2(e) and gk2 ln(1 + z_p): log2 psi = gamma2 u - log2(1 + 2^(gk2 u - cpsi));
+                              // placement ON_GRID (no psi in the sample weights): gk2 = 0, cpsi = 100
+    float tm_max;
+    float gk2_inj, cpsi_inj;  // gk2, cpsi for the injections (psi is always in s_j)
+    float pad0;
+    // the rest (table path, hi + lo pairs)
+    float mlow_lo;            // m_low - mlow_hi
+    float lm0_hi, lm0_lo;     // ln m_low (origin of the mass table)
     float tkmax_ev, tkmax_inj;// table coordinate beyond which z > z_table_max
     float zcat_hi, zcat_lo;   // z_cat_max (R6) as hi + lo
     uint32_t tkmax_ev_q;      // tkmax_ev in the 12.20 fixed point of the event records
-    float gk2, cpsi;          // (gamma + kappa) log2(e) and gk2 ln(1 + z_p): log2 psi = gamma2 u - log2(1 + 2^(gk2 u - cpsi));
-                              // placement ON_GRID (no psi in the sample weights): gk2 = 0, cpsi = 100
-    float mlow_tm;            // 1 - ln(m_low) tm_scale: tm = ln(m1) tm_scale + mlow_tm
-    float gk2_inj, cpsi_inj;  // the same for the injections (psi is always in s_j)
 };
+// the first 64 bytes of LamF through four 128-bit loads
+__device__ __forceinline__ void load_lamf_hot(LamF& F, const LamF* __restrict__ g) {
+    const float4* q = reinterpret_cast<const float4*>(g);
+    const float4 a = __ldg(q), b = __ldg(q + 1), c = __ldg(q + 2), d = __ldg(q + 3);
+    F.mlow_hi = a.x; F.tm_scale = a.y; F.mlow_tm = a.z; F.mhigh_p = a.w;
+    F.beta2 = b.x; F.delta = b.y; F.win_lo = b.z; F.win_hi = b.w;
+    F.two_dl2e = c.x; F.d2l2e = c.y; F.gk2 = c.z; F.cpsi = c.w;
+    F.tm_max = d.x; F.gk2_inj = d.y; F.cpsi_inj = d.z; F.pad0 = 0.f;
+}
 
 // Per-lambda constants written by the table kernel (S1), read by every other kernel.
 struct LamConst {

@@ -1,18 +1,21 @@
 // k_events_fast.cu -- steps S2 + S3 + S4 for the regular case, one CTA per (event, lambda): narrow distance posterior
 // (event-local polynomials), equally spaced redshift grid, Gaussian kernel in the local-expansion
 // form, placement ON_SAMPLES.  Everything else -- wide events, other kernels / forms / placements,
-// binning, diagnostics -- and every unit this kernel finds outside its reach (no or few effective samples, the heaviest
-// sample deep in the smoothing window, a bandwidth the expansion cannot take: DESIGN.md R21) is left to k_events: the unit
+// binning, diagnostics -- and every unit this kernel finds outside its reach (no or few effective samples, every supported
+// secondary deep in the smoothing window, a bandwidth the expansion cannot take: DESIGN.md R21) is left to k_events: the unit
 // is appended to a work list that k_events processes in the same batch call.
 //
-// Structure (what differs from k_events): after one barrier the eight warps are independent.  Warp w owns a contiguous chunk
-// of the (d_L-sorted) samples and runs S2 on it alone -- sweep 1 with the 26 polynomial coefficients in registers, its own
-// maximum, sweep 2 relative to that -- leaving chunk statistics {max, heaviest sample, W, Q, B, A about and excluding it}.
-// One barrier; every warp combines the eight chunk statistics in fp64 (exactly: Scott's rule in the cancellation-free form
-// of R21), derives bandwidth and expansion geometry redundantly, the psi table is built once per CTA; one barrier; every
-// warp then builds the expansion coefficients of the boxes ITS samples fall in and evaluates its samples -- no further
-// block-wide step until the eight partial sums are added.  q_g and the mass-table rows arrive by TMA bulk copies issued
-// before the first barrier.
+// Structure (what differs from k_events): between its four barriers the eight warps are independent.
+//   S2   warp w owns a contiguous chunk of the (d_L-sorted) samples: sweep 1 with the 26 polynomial coefficients in registers
+//        and the records two blocks ahead, its own maximum, sweep 2 relative to that; it leaves chunk statistics
+//        {max log2 w, sum w, sum w^2, sum w u, sum w u^2}.                                                       [barrier]
+//        Every warp combines the eight chunk statistics (lane c takes chunk c; sums of positive terms, fp32), derives
+//        bandwidth and expansion geometry redundantly; the psi table and the first sample of every box are found once per
+//        CTA (one thread per entry).                                                                              [barrier]
+//   S3+S4 warp w owns the boxes w, w + 8, ...: it builds their expansion coefficients and evaluates the samples that fall in
+//        them (a contiguous range each, coefficients in registers) -- the boxes of the sparse tails and of the dense centre
+//        alternate over the warps, so the warps finish together.                                                  [barrier]
+// q_g and the mass-table rows arrive by TMA bulk copies issued before the first barrier.
 #include "chim_internal.cuh"
 
 namespace chim {
@@ -20,37 +23,36 @@ namespace chim {
 #ifndef CHIM_FAST_BLOCKS
 #define CHIM_FAST_BLOCKS 3
 #endif
-#ifndef CHIM_FAST_UNROLL
-#define CHIM_FAST_UNROLL 2
-#endif
-constexpr int kFUnroll = CHIM_FAST_UNROLL;
 constexpr int kFT = 256;             // threads per CTA
 constexpr int kFW = kFT / 32;        // warps = sample chunks
 constexpr int kFPass = 128;          // samples per warp pass (4 per lane)
 constexpr int kFLeP = 12;            // terms of the local expansion
 constexpr int kFMaxBox = 96;         // boxes per event
+constexpr int kFBoxPerWarp = kFMaxBox / kFW;
 constexpr float kFMaxW = 1.3f;       // largest box width in units of sqrt(2) h
 constexpr int kFMaxD = 160;          // largest half-width of the psi table (grid points)
 constexpr int kFQPad = 2 * kFMaxD;   // zeros on both sides of the staged q_g: the coefficient build reads g_b +- d unchecked
-constexpr int kFMassStage = 384;     // mass-table rows staged per variant (= events_mass_stage_rows: k_polyfit sizes the slice)
+constexpr int kFMassStage = 384;     // mass-table rows staged per variant (>= events_mass_stage_rows: k_polyfit sizes the slice)
 
 struct FastSmem {
     unsigned long long mbar_mass, mbar_q;
     float c_mx[kFW], c_zr[kFW];      // per chunk: largest log2 w; z - z0 of the chunk's first sample (reference of its moments)
     float c_mp2[kFW];                // per chunk: largest m2' = m2 - m_low among its samples
     float c_mom[kFW][4];             // sum w, sum w^2, sum w u, sum w u^2 with w relative to the chunk's largest, u = z - c_zr
-    double c_sum[kFW];               // per chunk: sum_j w_j A_j relative to the event's heaviest sample
+    float c_f[kFW];                  // 2^(chunk max - event max): chunk-relative weights -> relative to the event's largest
+    double c_sum[kFW];               // per warp: sum_j w_j A_j over its boxes, relative to the event's largest weight
+    int bnd[kFMaxBox + 1];           // first sample of every box (samples are sorted)
 };
 
 __host__ __device__ inline int fast_chunk(int ns) { return ((ns + kFW * kFPass - 1) / (kFW * kFPass)) * kFPass; }
 __host__ __device__ inline size_t fast_nz4(size_t nz) { return (nz + 3) / 4 * 4; }
 __host__ __device__ inline size_t fast_aux_bytes() {
     const size_t a = 2 * (size_t)kFMassStage * sizeof(MassRow);
-    const size_t b = 4 * (size_t)kFLeP * ((size_t)(kFMaxD + 1) + (size_t)(kFMaxBox + kFW));
+    const size_t b = 4 * (size_t)kFLeP * ((size_t)(kFMaxD + 1) + (size_t)kFMaxBox);
     return a > b ? a : b;
 }
 size_t events_fast_smem_bytes(int max_ns, int max_nz) {
-    return ((sizeof(FastSmem) + 127) / 128) * 128 + 2 * sizeof(float) * (size_t)kFW * fast_chunk(max_ns) +
+    return ((sizeof(FastSmem) + 127) / 128) * 128 + sizeof(float2) * (size_t)kFW * fast_chunk(max_ns) +
            sizeof(float) * (2 * (size_t)kFQPad + fast_nz4((size_t)max_nz)) + fast_aux_bytes();
 }
 
@@ -62,7 +64,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     unsigned char* aux = reinterpret_cast<unsigned char*>(qs + 2 * (size_t)kFQPad + fast_nz4((size_t)P.ev.max_nz));
     MassRow* mass_s = reinterpret_cast<MassRow*>(aux);                  // S2: both variants of the event's slice of the mass table
     float* psi = reinterpret_cast<float*>(aux);                         // S3: psi table [(D+1) x 12] ...
-    float* Bc = psi + (size_t)kFLeP * (kFMaxD + 1);                     // ... and the expansion coefficients [box][12]
+    float* Bc = psi + (size_t)kFLeP * (kFMaxD + 1);                     // ... and the expansion coefficients [warp][box][12]
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
 
     const int l = blockIdx.x % P.n_lambda;                              // lambda fastest: CTAs in flight share an event
@@ -93,7 +95,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         }                                                                       \
         return;                                                                 \
     } while (0)
-    if (nr <= 0) CHIM_FAST_HANDOVER();
+    if (nr <= 0 || nr > kFMassStage) CHIM_FAST_HANDOVER();
 
     const size_t nz4 = fast_nz4((size_t)nz);
     const MassRow* mtab = P.mtab + (size_t)l * 2 * (P.n_mass + 2);
@@ -112,16 +114,21 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         qs[i] = 0.f;
         qs[kFQPad + nz4 + i] = 0.f;
     }
-    // per-thread copies: the 26 polynomial coefficients and the fp32 constants of S2
+    // per-thread copies: the 26 polynomial coefficients (seven 128-bit loads) and the fp32 constants of S2 (four)
     PolyCoef Cf;
     {
-        const f32x2* q = reinterpret_cast<const f32x2*>(pr);
+        const float4* q = reinterpret_cast<const float4*>(pr);
+        float4 v[7];
 #pragma unroll
-        for (int n = 0; n < kPolyN; ++n) Cf.zr[n] = __ldg(q + n);
+        for (int k = 0; k < 7; ++k) v[k] = __ldg(q + k);
+        const float* f = reinterpret_cast<const float*>(v);
 #pragma unroll
-        for (int n = 0; n < kPolyN - 1; ++n) Cf.ua[n] = __ldg(q + kPolyN + n);
+        for (int n = 0; n < kPolyN; ++n) Cf.zr[n] = pack2(f[2 * n], f[2 * n + 1]);
+#pragma unroll
+        for (int n = 0; n < kPolyN - 1; ++n) Cf.ua[n] = pack2(f[2 * kPolyN + 2 * n], f[2 * kPolyN + 2 * n + 1]);
     }
-    const LamF F = Lg->F;
+    LamF F;
+    load_lamf_hot(F, &Lg->F);
     __syncthreads();                                                    // (1) the barriers are initialised
     MassLookup M;
     M.g = mtab;
@@ -142,27 +149,34 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         const float2* pb = P.ev.prec_b + p0;
         const int nfull = c0 + ((c1 - c0) & ~31);                       // end of the whole blocks of 32 samples
         int j = c0 + lane;
-        PRec R = ldg_stream_prec(pa + j, pb + j);                       // the record arrays carry a spare tail: unconditional
-#pragma unroll(kFUnroll)
-        for (; j < nfull; j += 32) {
-            const float4 A = R.A;
-            const float2 Bq = R.B;
-            R = ldg_stream_prec(pa + j + 32, pb + j + 32);              // one iteration ahead
-            float zc, l2w, mp2;
-            poly_sample<true>(F, F.gk2, F.cpsi, Cf, A, Bq, M, tm_lo, tm_hi, zc, l2w, mp2);
-            zw[j] = make_float2(zc, l2w);
-            mx = fmaxf(mx, l2w);
-            mp2x = fmaxf(mp2x, mp2);
+#define CHIM_FAST_SAMPLE(REC, JJ, STORE)                                                                          \
+        {                                                                                                         \
+            float zc_, l2w_, mp2_;                                                                                \
+            poly_sample<true>(F, F.gk2, F.cpsi, Cf, (REC).A, (REC).B, M, tm_lo, tm_hi, zc_, l2w_, mp2_);          \
+            if (STORE) {                                                                                          \
+                zw[JJ] = make_float2(zc_, l2w_);                                                                  \
+                mx = fmaxf(mx, l2w_);                                                                             \
+                mp2x = fmaxf(mp2x, mp2_);                                                                         \
+            }                                                                                                     \
         }
-        if (nfull < c1) {   // the ragged end of the event (its records are padded to whole warps: poly_sample votes)
-            float zc, l2w, mp2;
-            poly_sample<true>(F, F.gk2, F.cpsi, Cf, R.A, R.B, M, tm_lo, tm_hi, zc, l2w, mp2);
-            if (j < c1) {
-                zw[j] = make_float2(zc, l2w);
-                mx = fmaxf(mx, l2w);
-                mp2x = fmaxf(mp2x, mp2);
-            }
+        // the records are streamed two blocks ahead (one doubled iteration ~ 140 instructions x 6 warps per scheduler: the L2
+        // latency); the record arrays carry a spare tail, so the loads are unconditional
+        PRec R0 = ldg_stream_prec(pa + j, pb + j), R1 = ldg_stream_prec(pa + j + 32, pb + j + 32);
+#pragma unroll 1
+        for (; j + 32 < nfull; j += 64) {
+            const PRec A0 = R0, A1 = R1;
+            R0 = ldg_stream_prec(pa + j + 64, pb + j + 64);
+            R1 = ldg_stream_prec(pa + j + 96, pb + j + 96);
+            CHIM_FAST_SAMPLE(A0, j, true)
+            CHIM_FAST_SAMPLE(A1, j + 32, true)
         }
+        if (j < nfull) {
+            CHIM_FAST_SAMPLE(R0, j, true)
+            j += 32;
+            R0 = R1;
+        }
+        if (nfull < c1) CHIM_FAST_SAMPLE(R0, j, j < c1)   // the ragged end of the event (records padded to whole warps: poly_sample votes)
+#undef CHIM_FAST_SAMPLE
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
@@ -170,13 +184,13 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         }
         __syncwarp();
         // sweep 2: w = 2^(log2 w - chunk max); plain weighted moments about the chunk's first sample (the cancellation-free form of
-        // R21 is only needed below n_eff ~ 1, and such units are handed over); idle slots of the last pass sit on the chunk's last
+        // R21 is only needed near n_eff = 1, and such units are handed over); idle slots of the last pass sit on the chunk's last
         // sample with weight 0
         const float mref = (mx > -INFINITY) ? mx : 0.f, zr = zw[c0].x, zlast = zw[c1 - 1].x;
         float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;
         const int pend = c0 + ((c1 - c0 + kFPass - 1) / kFPass) * kFPass;
         for (int j4 = c0 + 4 * lane; j4 < pend; j4 += kFPass) {
-            float4 ab = *reinterpret_cast<const float4*>(zw + j4), cd4 = *reinterpret_cast<const float4*>(zw + j4 + 2);
+            const float4 ab = *reinterpret_cast<const float4*>(zw + j4), cd4 = *reinterpret_cast<const float4*>(zw + j4 + 2);
             float zv[4] = {ab.x, ab.z, cd4.x, cd4.z};
             const float lv[4] = {ab.y, ab.w, cd4.y, cd4.w};
             float wv[4];
@@ -231,6 +245,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     const float dl = live ? S.c_zr[lane] - S.c_zr[0] : 0.f;             // chunk reference relative to the first chunk's
     const float wc = live ? S.c_mom[lane][0] : 0.f, qc = live ? S.c_mom[lane][1] : 0.f;
     const float bc = live ? S.c_mom[lane][2] : 0.f, ac = live ? S.c_mom[lane][3] : 0.f;
+    if (wid == 0 && lane < kFW) S.c_f[lane] = f;
     float SW = f * wc, SQ = f * f * qc, SB = f * fmaf(dl, wc, bc);
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1) {
@@ -246,7 +261,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1) SA += __shfl_xor_sync(0xffffffffu, SA, o);
     SA = __shfl_sync(0xffffffffu, SA, 0);
-    const float s2 = SQ / (SW * SW), neff = 1.0f / s2;                  // sum w^2, Kish n_eff
+    const float s2 = SQ / (SW * SW), neff = 1.0f / s2;                  // sum w^^2, Kish n_eff
     double h;
     if (P.bw_rule == CHIM_BW_FIXED) {
         h = __ldg(P.ev.fixed_bw + ev);
@@ -270,8 +285,24 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
            !(fD <= (float)kFMaxD) || !(fabsf(fb_lo) * (float)m < 1e8f) || !(fabsf(fb_hi) * (float)m < 1e8f);
     if (hand) CHIM_FAST_HANDOVER();
     const int D = (int)fD, b_lo = (int)fb_lo, nbox = (int)(fb_hi - fb_lo) + 1;
-    // psi table: psi_n(d dy) = exp(-t^2) H_n(t)/n!, t = d dy, by the three-term recurrence (one d per thread)
-    for (int d = tid; d <= D; d += kFT) {
+    // once per CTA, one thread per entry: the first sample of every box (binary search in the sorted samples; box b holds the
+    // samples with y in [c_b - w/2, c_b + w/2), c_b = yfirst + (b_lo + b) w) from the low threads, and from the high ones the
+    // psi table psi_n(d dy) = exp(-t^2) H_n(t)/n!, t = d dy, by the three-term recurrence
+    if (tid <= nbox) {
+        int lo = 0, hi = ns;
+        if (tid == 0) hi = 0;
+        else if (tid == nbox) lo = ns;
+        else {
+            const float zb = (yfirst + ((float)(b_lo + tid) - 0.5f) * wbox) / scy;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (zw[mid].x < zb) lo = mid + 1;
+                else hi = mid;
+            }
+        }
+        S.bnd[tid] = lo;
+    }
+    for (int d = kFT - 1 - tid; d <= D; d += kFT) {
         const float t = (float)d * dy, t2 = 2.f * t;
         float p0v = ex2f(-t * t * 1.44269504088896341f), p1v = t2 * p0v;
         float* o = psi + (size_t)d * kFLeP;
@@ -285,15 +316,13 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
             p1v = p2v;
         }
     }
-    __syncthreads();                                                    // (3) psi table (the staged mass rows are dead)
+    __syncthreads();                                                    // (3) psi table, box ranges (the staged mass rows are dead)
 
-    // ---- S3 + S4 on the warp's chunk: coefficients of its own boxes, then one degree-11 polynomial per sample ------------------
+    // ---- S3 + S4, warp w on the boxes w, w + 8, ...: their coefficients, then one degree-11 polynomial per sample ------------------
     double lsum = 0.0;
-    if (c0 < ns) {
-        const int bw0 = min(max((int)floorf((zw[c0].x * scy - yfirst) * inv_w + 0.5f) - b_lo, 0), nbox - 1);
-        const int bw1 = min(max((int)floorf((zw[c1 - 1].x * scy - yfirst) * inv_w + 0.5f) - b_lo, bw0), nbox - 1);
-        const int nbw = bw1 - bw0 + 1;
-        float* Bw = Bc + (size_t)(bw0 + wid) * kFLeP;                    // (neighbouring chunks share at most one box: shifted by wid)
+    const int nbw = (wid < nbox) ? (nbox - wid + kFW - 1) / kFW : 0;    // boxes of this warp
+    if (nbw > 0) {
+        float* Bw = Bc + (size_t)wid * kFBoxPerWarp * kFLeP;
         // coefficients B_bn = sum_{|d| <= D} q_{g_b+d} psi_n(d dy): lane = (half of the d range, box, quad of n), five boxes per
         // round; psi_n(-t) = (-1)^n psi_n(t), so even n take (q_+ + q_-) psi_n and odd n (q_+ - q_-) psi_n -- the pairs (n, n+1)
         // of a packed FMA
@@ -302,7 +331,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         for (int base = 0; base < nbw; base += 5) {
             const int bi = base + bsub;
             const bool valid = lane < 30 && bi < nbw;
-            const int gc = (b_lo + bw0 + (valid ? bi : 0)) * m;         // grid index of the box centre
+            const int gc = (b_lo + wid + kFW * (valid ? bi : 0)) * m;   // grid index of the box centre
             const bool reach = valid && gc > -D - 1 && gc < nz + D;     // else no grid point within the box's cut-off: B = 0
             const float* qp = qs + kFQPad + (reach ? gc : 0) + d_lo;
             const float* qm = qs + kFQPad + (reach ? gc : 0) - d_lo;
@@ -349,23 +378,19 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
             if (valid && !half) reinterpret_cast<float4*>(Bw + (size_t)bi * kFLeP)[quad] = acc;
         }
         __syncwarp();
-        // evaluation: passes of 128 consecutive (sorted) samples, 4 per lane; the boxes a pass touches are visited in turn
-        const int bofs = b_lo + bw0;
-        const int pend = c0 + ((c1 - c0 + kFPass - 1) / kFPass) * kFPass;
-        for (int j0 = c0 + 4 * lane; j0 < pend; j0 += kFPass) {
-            const float4 ab = *reinterpret_cast<const float4*>(zw + j0), cd4 = *reinterpret_cast<const float4*>(zw + j0 + 2);
-            const float y[4] = {ab.x * scy, ab.z * scy, cd4.x * scy, cd4.z * scy};
-            int bx[4];
-#pragma unroll
-            for (int r = 0; r < 4; ++r) bx[r] = min(max((int)floorf(fmaf(y[r] - yfirst, inv_w, 0.5f)) - bofs, 0), nbw - 1);
-            const int bmin = __reduce_min_sync(0xffffffffu, min(min(bx[0], bx[1]), min(bx[2], bx[3])));
-            const int bmax = __reduce_max_sync(0xffffffffu, max(max(bx[0], bx[1]), max(bx[2], bx[3])));
-            float A[4] = {0.f, 0.f, 0.f, 0.f};
-            for (int i = bmin; i <= bmax; ++i) {
-                const float c = fmaf((float)((bofs + i) * m), dy, yfirst);
-                const float4* bp = reinterpret_cast<const float4*>(Bw + (size_t)i * kFLeP);
-                const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
-                const f32x2 s01 = pack2(y[0] - c, y[1] - c), s23 = pack2(y[2] - c, y[3] - c);
+        // evaluation box by box: the samples [bnd[b], bnd[b+1]) in passes of 128 (4 consecutive per lane, aligned to 4; lanes beyond
+        // the range masked), the box's 12 coefficients in registers, s = y - c_b
+        const int Cq = C >> 2;                                          // chunk length in groups of 4 samples
+        for (int k = 0; k < nbw; ++k) {
+            const int b = wid + kFW * k;
+            const int j_lo = S.bnd[b], j_hi = S.bnd[b + 1];
+            if (j_hi <= j_lo) continue;
+            const float cb = fmaf((float)((b_lo + b) * m), dy, yfirst);
+            const float4* bp = reinterpret_cast<const float4*>(Bw + (size_t)k * kFLeP);
+            const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
+            for (int j0 = (j_lo & ~3) + 4 * lane; j0 < j_hi; j0 += kFPass) {
+                const float4 ab = *reinterpret_cast<const float4*>(zw + j0), cd4 = *reinterpret_cast<const float4*>(zw + j0 + 2);
+                const f32x2 s01 = pack2(fmaf(ab.x, scy, -cb), fmaf(ab.z, scy, -cb)), s23 = pack2(fmaf(cd4.x, scy, -cb), fmaf(cd4.z, scy, -cb));
                 f32x2 a01 = pack2(k2.w, k2.w), a23 = a01;
 #define CHIM_LE_STEP(cf) { const f32x2 q_ = pack2(cf, cf); a01 = fma2(a01, s01, q_); a23 = fma2(a23, s23, q_); }
                 CHIM_LE_STEP(k2.z) CHIM_LE_STEP(k2.y) CHIM_LE_STEP(k2.x)
@@ -375,12 +400,14 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
                 float v[4];
                 unpack2(a01, v[0], v[1]);
                 unpack2(a23, v[2], v[3]);
+                const float wv[4] = {ab.y, ab.w, cd4.y, cd4.w};
+                float acc = 0.f;
 #pragma unroll
-                for (int r = 0; r < 4; ++r) A[r] = (bx[r] == i) ? v[r] : A[r];
+                for (int r = 0; r < 4; ++r) acc = fmaf((j0 + r >= j_lo && j0 + r < j_hi) ? wv[r] : 0.f, v[r], acc);
+                lsum += (double)(acc * S.c_f[(j0 >> 2) / Cq]);          // the weights are relative to their chunk's largest
             }
-            lsum += (double)fmaf(ab.y, A[0], fmaf(ab.w, A[1], fmaf(cd4.y, A[2], cd4.w * A[3])));
         }
-        lsum = warp_sum(lsum) * (double)exp2f(S.c_mx[wid] - gmx);       // chunk-relative weights -> relative to the event's largest
+        lsum = warp_sum(lsum);
     }
     if (lane == 0) S.c_sum[wid] = lsum;
     __syncthreads();                                                    // (4)
