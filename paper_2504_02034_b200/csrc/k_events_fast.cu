@@ -164,11 +164,10 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         PRec R0 = ldg_stream_prec(pa + j, pb + j), R1 = ldg_stream_prec(pa + j + 32, pb + j + 32);
 #pragma unroll 1
         for (; j + 32 < nfull; j += 64) {
-            const PRec A0 = R0, A1 = R1;
+            CHIM_FAST_SAMPLE(R0, j, true)
             R0 = ldg_stream_prec(pa + j + 64, pb + j + 64);
+            CHIM_FAST_SAMPLE(R1, j + 32, true)
             R1 = ldg_stream_prec(pa + j + 96, pb + j + 96);
-            CHIM_FAST_SAMPLE(A0, j, true)
-            CHIM_FAST_SAMPLE(A1, j + 32, true)
         }
         if (j < nfull) {
             CHIM_FAST_SAMPLE(R0, j, true)
@@ -189,14 +188,14 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         const float mref = (mx > -INFINITY) ? mx : 0.f, zr = zw[c0].x, zlast = zw[c1 - 1].x;
         float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;
         const int pend = c0 + ((c1 - c0 + kFPass - 1) / kFPass) * kFPass;
-        for (int j4 = c0 + 4 * lane; j4 < pend; j4 += kFPass) {
-            const float4 ab = *reinterpret_cast<const float4*>(zw + j4), cd4 = *reinterpret_cast<const float4*>(zw + j4 + 2);
+        for (int jb = c0 + 2 * lane; jb < pend; jb += kFPass) {         // lane: samples jb, jb + 1, jb + 64, jb + 65 (16-byte lane stride)
+            const float4 ab = *reinterpret_cast<const float4*>(zw + jb), cd4 = *reinterpret_cast<const float4*>(zw + jb + 64);
             float zv[4] = {ab.x, ab.z, cd4.x, cd4.z};
             const float lv[4] = {ab.y, ab.w, cd4.y, cd4.w};
             float wv[4];
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
-                const bool valid = j4 + r < c1;
+                const bool valid = jb + (r & 1) + 64 * (r >> 1) < c1;
                 const float w = valid ? ex2f(lv[r] - mref) : 0.f;
                 zv[r] = valid ? zv[r] : zlast;
                 wv[r] = w;
@@ -206,8 +205,8 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
                 m2 += wu;
                 m3 = fmaf(wu, u, m3);
             }
-            *reinterpret_cast<float4*>(zw + j4) = make_float4(zv[0], wv[0], zv[1], wv[1]);
-            *reinterpret_cast<float4*>(zw + j4 + 2) = make_float4(zv[2], wv[2], zv[3], wv[3]);
+            *reinterpret_cast<float4*>(zw + jb) = make_float4(zv[0], wv[0], zv[1], wv[1]);
+            *reinterpret_cast<float4*>(zw + jb + 64) = make_float4(zv[2], wv[2], zv[3], wv[3]);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -380,7 +379,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         __syncwarp();
         // evaluation box by box: the samples [bnd[b], bnd[b+1]) in passes of 128 (4 consecutive per lane, aligned to 4; lanes beyond
         // the range masked), the box's 12 coefficients in registers, s = y - c_b
-        const int Cq = C >> 2;                                          // chunk length in groups of 4 samples
+        const float invC = 1.0f / (float)C;                             // chunk of a pair of samples: floor((jb + 1) / C), exact in fp32 (jb even, C a multiple of 128)
         for (int k = 0; k < nbw; ++k) {
             const int b = wid + kFW * k;
             const int j_lo = S.bnd[b], j_hi = S.bnd[b + 1];
@@ -388,8 +387,9 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
             const float cb = fmaf((float)((b_lo + b) * m), dy, yfirst);
             const float4* bp = reinterpret_cast<const float4*>(Bw + (size_t)k * kFLeP);
             const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
-            for (int j0 = (j_lo & ~3) + 4 * lane; j0 < j_hi; j0 += kFPass) {
-                const float4 ab = *reinterpret_cast<const float4*>(zw + j0), cd4 = *reinterpret_cast<const float4*>(zw + j0 + 2);
+            const int jsafe = (ns - 1) & ~1;                                // (lanes beyond the range read a valid pair; their weights are masked)
+            for (int jb = (j_lo & ~1) + 2 * lane; jb - 2 * lane < j_hi; jb += kFPass) {   // lane: samples jb, jb + 1, jb + 64, jb + 65
+                const float4 ab = *reinterpret_cast<const float4*>(zw + min(jb, jsafe)), cd4 = *reinterpret_cast<const float4*>(zw + min(jb + 64, jsafe));
                 const f32x2 s01 = pack2(fmaf(ab.x, scy, -cb), fmaf(ab.z, scy, -cb)), s23 = pack2(fmaf(cd4.x, scy, -cb), fmaf(cd4.z, scy, -cb));
                 f32x2 a01 = pack2(k2.w, k2.w), a23 = a01;
 #define CHIM_LE_STEP(cf) { const f32x2 q_ = pack2(cf, cf); a01 = fma2(a01, s01, q_); a23 = fma2(a23, s23, q_); }
@@ -401,10 +401,12 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
                 unpack2(a01, v[0], v[1]);
                 unpack2(a23, v[2], v[3]);
                 const float wv[4] = {ab.y, ab.w, cd4.y, cd4.w};
-                float acc = 0.f;
-#pragma unroll
-                for (int r = 0; r < 4; ++r) acc = fmaf((j0 + r >= j_lo && j0 + r < j_hi) ? wv[r] : 0.f, v[r], acc);
-                lsum += (double)(acc * S.c_f[(j0 >> 2) / Cq]);          // the weights are relative to their chunk's largest
+                const unsigned rel = (unsigned)(jb - j_lo), span = (unsigned)(j_hi - j_lo);   // sample jb + o is in the box iff rel + o < span (unsigned)
+                // the two pairs may lie in different chunks: the weights are relative to their chunk's largest
+                const float f01 = S.c_f[min(__float2int_rd((float)(jb + 1) * invC), kFW - 1)], f23 = S.c_f[min(__float2int_rd((float)(jb + 65) * invC), kFW - 1)];   // (clamped: masked lanes may point past the last chunk)
+                const float a0 = fmaf((rel < span) ? wv[0] : 0.f, v[0], ((rel + 1u < span) ? wv[1] : 0.f) * v[1]);
+                const float a1 = fmaf((rel + 64u < span) ? wv[2] : 0.f, v[2], ((rel + 65u < span) ? wv[3] : 0.f) * v[3]);
+                lsum += (double)fmaf(a0, f01, a1 * f23);
             }
         }
         lsum = warp_sum(lsum);
