@@ -245,10 +245,10 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
         Bracket b(ctx, 0);
         CK(launch_polyfit(ctx->Lc, ctx->tab_ev, ctx->ev_grid.rows(), nl, ctx->ev.n_events, ctx->ev.tk_c, ctx->ev.tk_h, ctx->ev.z0, 0.0,
                           false, ctx->poly_mats, ctx->ev.lnm1_lo, ctx->ev.lnm1_hi, ctx->cfg.n_mass_table,
-                          events_mass_stage_rows(ctx->cfg.n_mass_table), ctx->poly_ev, st));
+                          events_mass_stage_rows(ctx->cfg.n_mass_table), ctx->ev_grid.dx, ctx->poly_ev, st));
         if (ctx->have_inj)
             CK(launch_polyfit(ctx->Lc, ctx->tab_inj, ctx->inj_grid.rows(), nl, ctx->inj_blocks, ctx->inj.tk_c, ctx->inj.tk_h, nullptr,
-                              ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->poly_inj, st));
+                              ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->inj_grid.dx, ctx->poly_inj, st));
         ctx->launches += ctx->have_inj ? 2 : 1;
     }
     ctx->launches += 1;   // (k_tables)
@@ -755,16 +755,39 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     }
     // chunk-local polynomials of k_inject: the set is sorted in d_L, so a chunk of kInjChunk injections spans a narrow range
     const int n_chunks = (int)((n_det + kInjChunk - 1) / kInjChunk);
-    std::vector<float4> prec_a((size_t)n_chunks * kInjChunk + 1024, make_float4(0.f, 1.f, 1.f, 0.f));   // + spare tail (prefetch)
-    std::vector<float2> prec_b((size_t)n_chunks * kInjChunk + 1024, make_float2(0.f, 0.f));
+    std::vector<float4> prec_a((size_t)n_chunks * kInjChunk + 2048, make_float4(0.f, 1.f, 1.f, 0.f));   // + spare tail (prefetch)
+    std::vector<float2> prec_b((size_t)n_chunks * kInjChunk + 2048, make_float2(0.f, 0.f));
     std::vector<double> ctk_c(n_chunks), ctk_h(n_chunks);
+    std::vector<float> blk_m2d((size_t)n_chunks * (kInjChunk / 256), INFINITY);
     for (int c = 0; c < n_chunks; ++c) {
         const size_t a = (size_t)c * kInjChunk, b = std::min<size_t>(a + kInjChunk, N);
         auto tk_of = [&](size_t j) { return (double)f_bits(rec[2 * j].x) + (double)rec[2 * j].y; };   // k + t
-        const double lo = tk_of(a), hi = tk_of(b - 1);
+        const double lo = tk_of(a), hi = tk_of(b - 1);                // (still in d_L order here)
+        {   // inside the chunk the order is free: by m2d, so that the warps of k_inject are uniform in "m2 below m_low" and
+            // "m2 inside the smoothing window" (1 + z varies by a few percent over a chunk)
+            std::vector<size_t> ord(b - a);
+            std::iota(ord.begin(), ord.end(), a);
+            std::stable_sort(ord.begin(), ord.end(), [&](size_t x, size_t y) { return h_m2[(size_t)idx[x]] < h_m2[(size_t)idx[y]]; });
+            // ... and inside every block of 256 by m1d: the 32 lanes of a warp then address neighbouring rows of the mass table
+            // (shared-memory bank conflicts of the 16-byte row loads: 9 -> ~4 wavefronts)
+            for (size_t q = 0; q < ord.size(); q += 256)
+                std::stable_sort(ord.begin() + q, ord.begin() + std::min(q + 256, ord.size()),
+                                 [&](size_t x, size_t y) { return h_m1[(size_t)idx[x]] < h_m1[(size_t)idx[y]]; });
+            std::vector<float4> r2(2 * (b - a));
+            std::vector<int64_t> i2(b - a);
+            for (size_t k = 0; k < b - a; ++k) { r2[2 * k] = rec[2 * ord[k]]; r2[2 * k + 1] = rec[2 * ord[k] + 1]; i2[k] = idx[ord[k]]; }
+            std::copy(r2.begin(), r2.end(), rec.begin() + 2 * a);
+            std::copy(i2.begin(), i2.end(), idx.begin() + a);
+        }
         const double half = 0.5 * (hi - lo) * (1.0 + 1e-9) + 1e-3;
         ctk_c[c] = 0.5 * (lo + hi);
         ctk_h[c] = (half * grid.dx <= kPolyMaxHalfRange) ? half : 0.0;
+        for (int k = 0; k < kInjChunk / 256; ++k) {   // largest m2d of every block of 256 (rounded up: the test in k_inject is conservative)
+            const size_t e = std::min<size_t>(a + (size_t)(k + 1) * 256, b);
+            float mxb = 0.f;
+            for (size_t q = a + (size_t)k * 256; q < e; ++q) mxb = std::max(mxb, (float)h_m2[(size_t)idx[q]]);
+            blk_m2d[(size_t)c * (kInjChunk / 256) + k] = (e > a + (size_t)k * 256) ? std::nextafter(mxb, INFINITY) : INFINITY;
+        }
         for (size_t j = a; j < a + kInjChunk; ++j) {
             const size_t js = std::min(j, b - 1), o = (size_t)idx[js];
             const double t = (tk_of(js) - ctk_c[c]) / half;
@@ -783,6 +806,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     CK(upload(ctx->owned_inj, &I.perm, idx));
     CK(upload(ctx->owned_inj, &I.prec_a, prec_a)); CK(upload(ctx->owned_inj, &I.prec_b, prec_b));
     CK(upload(ctx->owned_inj, &I.tk_c, ctk_c)); CK(upload(ctx->owned_inj, &I.tk_h, ctk_h));
+    CK(upload(ctx->owned_inj, &I.blk_m2d, blk_m2d));
     ctx->inj = I;
     ctx->inj_m_top = m_top;
     ctx->inj_grid = grid;
@@ -923,10 +947,10 @@ static int debug_prepare(chim_ctx* ctx, const double* lambda, const char* who) {
     CK(launch_tables(lambda, 1, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, ctx->stream));
     CK(launch_polyfit(ctx->Lc, ctx->tab_ev, ctx->ev_grid.rows(), 1, ctx->ev.n_events, ctx->ev.tk_c, ctx->ev.tk_h, ctx->ev.z0, 0.0, false,
                       ctx->poly_mats, ctx->ev.lnm1_lo, ctx->ev.lnm1_hi, ctx->cfg.n_mass_table,
-                      events_mass_stage_rows(ctx->cfg.n_mass_table), ctx->poly_ev, ctx->stream));
+                      events_mass_stage_rows(ctx->cfg.n_mass_table), ctx->ev_grid.dx, ctx->poly_ev, ctx->stream));
     if (ctx->have_inj)
         CK(launch_polyfit(ctx->Lc, ctx->tab_inj, ctx->inj_grid.rows(), 1, ctx->inj_blocks, ctx->inj.tk_c, ctx->inj.tk_h, nullptr,
-                          ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->poly_inj, ctx->stream));
+                          ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->inj_grid.dx, ctx->poly_inj, ctx->stream));
     return CHIM_OK;
 }
 

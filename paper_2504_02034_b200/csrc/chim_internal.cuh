@@ -323,7 +323,7 @@ __device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restri
 // A = {t, m1d, m2d, ln m1d}, B = {ln m2d, log2(1/prior or 1/p_draw) - scale, .., ..}:
 //   m' = m^d a - m_low;  log2 w = LQ2(ln m1) + beta2 ln m2^d + r + B.y - 2 log2 m1' - log2(1 + 2^(gk2 u - cpsi)) - log2(1 + e^f(m2'))
 // PAPER.md:52, :195-198 eq. 20, :226 eq. 21, :75 eq. 11.  Warp-collective like sample_eval.
-template <bool kFit>
+template <bool kFit, bool kTurn = true>
 __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, const float cpsi, const PolyCoef& C, const float4 A,
                                             const float2 Bq, const MassLookup& M, const float tm_lo, const float tm_hi,
                                             float& zc, float& l2w, float& mp2) {
@@ -358,7 +358,7 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
     float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x);
     l += fmaf(F.beta2, Bq.x, r + Bq.y);
     l = fmaf(-2.f, lg2f(mp1), l);            // m1' <= 0 implies m2' <= 0: discarded below
-    l -= lg2f(1.0f + ex2f(fmaf(gk2, u, -cpsi)));   // overflow -> l = -inf, the limit (psi -> 0)
+    if (kTurn) l -= lg2f(1.0f + ex2f(fmaf(gk2, u, -cpsi)));   // overflow -> l = -inf, the limit (psi -> 0).  !kTurn: the turnover is part of r
     if (__any_sync(0xffffffffu, mp2 < F.delta)) {
         const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
         const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
@@ -510,6 +510,7 @@ struct InjSetDev {
     const float2* prec_b;
     const double* tk_c;      // [n_chunks]
     const double* tk_h;      // [n_chunks]
+    const float* blk_m2d;    // [n_chunks][64] largest m2d of every block of 256 injections (chunks are ordered by m2d)
 };
 
 struct InjKernelParams {
@@ -542,7 +543,7 @@ cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P,
 
 cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int n_lambda, int n_ranges, const double* tk_c,
                            const double* tk_h, const double* z_ref, double z_ref_const, bool is_inj, const double* pm,
-                           const double* lnm1_lo, const double* lnm1_hi, int n_mass, int mcap, float* out, cudaStream_t st);
+                           const double* lnm1_lo, const double* lnm1_hi, int n_mass, int mcap, double dx_tab, float* out, cudaStream_t st);
 int events_mass_stage_rows(int n_mass);   // rows of the mass table a k_events CTA stages per variant
 cudaError_t launch_events(const EventKernelParams& P, bool count_pairs, cudaStream_t st);
 cudaError_t launch_events_fast(const FastEventParams& P, int n_fast, cudaStream_t st);

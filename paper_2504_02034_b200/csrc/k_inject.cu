@@ -21,6 +21,7 @@ namespace chim {
 #endif
 constexpr int kS5Unroll = CHIM_S5_UNROLL;
 constexpr int kInjThreads = 256;
+constexpr int kInjChunkBlocks = 64;       // blocks of kInjThreads injections per chunk (chim_api.cu: kInjChunk = 16384)
 
 struct InjSmem {
     LamConst L;
@@ -72,33 +73,76 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
     double acc[2] = {0.0, 0.0};
     int oor = 0;
     const double tk_h = P.inj.tk_h[chunk], tk_c = P.inj.tk_c[chunk];
-    const bool use_poly = L.flags == 0 && tk_h > 0.0 && tk_c + tk_h < L.tkmax_inj;
+    const bool use_poly = L.flags == 0 && tk_h > 0.0 && tk_c + tk_h < L.tkmax_inj;   // (block-uniform)
     if (use_poly) {
-        // chunk-local polynomials: the chunk's (sorted) injections span a narrow range of ln d_L; z is taken relative to
-        // z_cat_max, so the support cut of R6 is the sign of the polynomial
-        if (tid < 4 * kPolyN) S.poly[tid] = P.poly[((size_t)l * P.n_chunks + chunk) * (4 * kPolyN) + tid];   // fitted by k_polyfit
-        __syncthreads();
+        // chunk-local polynomials: the chunk's injections span a narrow range of ln d_L; z is taken relative to z_cat_max, so the
+        // support cut of R6 is the sign of the polynomial.  The chunk is ordered by m2d (chim_init_injections): warps whose
+        // secondaries all lie below m_low (5-25 % of a reference set that starts at 5 Msun) leave after the 1/(1+z) polynomial,
+        // and the warps above the smoothing window skip its three MUFU (vote).  For chunks narrower than 0.2 in ln d_L the
+        // Madau-Dickinson turnover is part of the fitted polynomial r (k_polyfit; slot 26 of the record says so).
+        const float* pr = P.poly + ((size_t)l * P.n_chunks + chunk) * (4 * kPolyN);
         PolyCoef C;
-        load_poly(C, S.poly);
-        const float4* pa = P.inj.prec_a + j0 + tid;          // padded to whole chunks with copies of the last injection
-        const float2* pb = P.inj.prec_b + j0 + tid;
+        {
+            const float4* q = reinterpret_cast<const float4*>(pr);
+            float4 v[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v[k] = __ldg(q + k);
+            const float* f = reinterpret_cast<const float*>(v);
+#pragma unroll
+            for (int n = 0; n < kPolyN; ++n) C.zr[n] = pack2(f[2 * n], f[2 * n + 1]);
+#pragma unroll
+            for (int n = 0; n < kPolyN - 1; ++n) C.ua[n] = pack2(f[2 * kPolyN + 2 * n], f[2 * kPolyN + 2 * n + 1]);
+        }
+        const bool turn_folded = __float_as_int(__ldg(pr + 26)) != 0;
+        const float4* pa = P.inj.prec_a + j0;                // padded to whole chunks with copies of the chunk's last injection
+        const float2* pb = P.inj.prec_b + j0;
         const int n = (int)(j1 - j0), n32 = (n + 31) & ~31;
         const float tm_hi = F.tm_max;
-        PRec R = ldg_stream_prec(pa, pb);                    // unconditional: the record arrays carry a tail of spare records
-#pragma unroll 2
-        for (int j = tid; j < n32; j += kInjThreads) {
-            const float4 A = R.A;
-            const float2 Bq = R.B;
-            pa += kInjThreads;
-            pb += kInjThreads;
-            R = ldg_stream_prec(pa, pb);                     // one iteration ahead (past the chunk: read and dropped)
-            float zc, l2w;
-            poly_sample<true>(F, F.gk2_inj, F.cpsi_inj, C, A, Bq, M, 1.0f, tm_hi, zc, l2w);
-            const double s = (zc <= 0.f && j < n) ? ex2_to_double(l2w) : 0.0;
-            acc[0] += s;
-            acc[1] = fma(s, s, acc[1]);
-            if (P.dbg_s && j < n) P.dbg_s[P.inj.perm[j0 + j]] = s * P.dbg_scale;
+        // the blocks of 256 injections whose secondaries ALL lie below m_low (the chunk is ordered by m2d; blk_m2d holds the
+        // largest m2d of every block, 1/(1+z) is largest at the near end t = -1) contribute nothing (R15): the sweep starts
+        // behind them
+        int k0 = 0;
+        {
+            float amax = 0.f, sg = 1.f;
+#pragma unroll
+            for (int k = 0; k < kPolyN - 1; ++k) {
+                float un, an;
+                unpack2(C.ua[k], un, an);
+                amax = fmaf(sg, an, amax);
+                sg = -sg;
+            }
+            amax *= 1.0f + 1e-5f;
+            const float* bm = P.inj.blk_m2d + (size_t)chunk * (kInjChunkBlocks);
+            const int nblk = (n + kInjThreads - 1) / kInjThreads;
+            for (; k0 < nblk - 1 && __ldg(bm + k0) * amax < F.mlow_hi; ++k0) {}
         }
+#define CHIM_INJ_SAMPLE(TURN, REC, JJ)                                                                                \
+        {                                                                                                             \
+            float zc, l2w, mp2_;                                                                                      \
+            poly_sample<true, TURN>(F, F.gk2_inj, F.cpsi_inj, C, (REC).A, (REC).B, M, 1.0f, tm_hi, zc, l2w, mp2_);    \
+            const double s = (zc <= 0.f && (JJ) < n) ? ex2_to_double(l2w) : 0.0;                                      \
+            acc[0] += s;                                                                                              \
+            acc[1] = fma(s, s, acc[1]);                                                                               \
+            if (P.dbg_s && (JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale;                                \
+        }
+#define CHIM_INJ_SWEEP(TURN)                                                                                          \
+        {                                                                                                             \
+            int j = tid + k0 * kInjThreads;                                                                           \
+            PRec R0 = ldg_stream_prec(pa + j, pb + j), R1 = ldg_stream_prec(pa + j + kInjThreads, pb + j + kInjThreads); \
+            _Pragma("unroll 1") for (; j + kInjThreads < n32; j += 2 * kInjThreads) {                                 \
+                CHIM_INJ_SAMPLE(TURN, R0, j)                                                                          \
+                R0 = ldg_stream_prec(pa + j + 2 * kInjThreads, pb + j + 2 * kInjThreads);                             \
+                CHIM_INJ_SAMPLE(TURN, R1, j + kInjThreads)                                                            \
+                R1 = ldg_stream_prec(pa + j + 3 * kInjThreads, pb + j + 3 * kInjThreads);                             \
+            }                                                                                                         \
+            if (j < n32) CHIM_INJ_SAMPLE(TURN, R0, j)                                                                 \
+        }
+        if (P.dbg_s)
+            for (int j = tid; j < min(k0 * kInjThreads, n); j += kInjThreads) P.dbg_s[P.inj.perm[j0 + j]] = 0.0;
+        if (turn_folded) CHIM_INJ_SWEEP(false)
+        else CHIM_INJ_SWEEP(true)
+#undef CHIM_INJ_SWEEP
+#undef CHIM_INJ_SAMPLE
     } else if (L.flags == 0) {
         const float4* rows = reinterpret_cast<const float4*>(P.tab + (size_t)l * P.tab_rows);
         const int64_t j1w = j0 + ((j1 - j0 + 31) & ~(int64_t)31);    // whole warps stay in the loop (sample_eval votes)

@@ -494,7 +494,7 @@ __global__ void __launch_bounds__(256) k_polyfit(const LamConst* __restrict__ Lc
                                                  const double* __restrict__ tk_h, const double* __restrict__ z_ref,
                                                  double z_ref_const, int is_inj, const double* __restrict__ pm,
                                                  const double* __restrict__ lnm1_lo, const double* __restrict__ lnm1_hi,
-                                                 int n_mass, int mcap, float* __restrict__ out) {
+                                                 int n_mass, int mcap, double dx_tab, float* __restrict__ out) {
     const long long item = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (item >= (long long)n_lambda * n_ranges) return;
     const int l = (int)(item % n_lambda), r = (int)(item / n_lambda);
@@ -502,7 +502,15 @@ __global__ void __launch_bounds__(256) k_polyfit(const LamConst* __restrict__ Lc
     const double h = tk_h[r], c = tk_c[r];
     if (L.flags || !(h > 0.0) || !(c + h < (is_inj ? L.tkmax_inj : L.tkmax_ev))) return;
     float* o = out + ((size_t)l * n_ranges + r) * (4 * kPolyN);
-    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, is_inj || L.F.gk2 != 0.f, pm, o);
+    // the Madau-Dickinson turnover log2(1 + ((1+z)/(1+z_p))^(gamma+kappa)) is kept out of the fitted polynomial r (its poles sit
+    // ~0.5 from the real axis in ln(1+z)) -- except for injection chunks narrower than 0.2 in ln d_L, where degree 6 takes it
+    // to < 1e-9 and k_inject saves two MUFU per injection (slot 26 of the record: 1 = folded)
+    const bool fold = is_inj && h * dx_tab <= 0.1;
+    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, !fold && (is_inj || L.F.gk2 != 0.f), pm, o);
+    if (is_inj) {
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) o[26] = __int_as_float(fold ? 1 : 0);
+    }
     if (lnm1_lo) {
         // k_events: the rows of the mass table the event can address, ln m1 = ln m1d - u, u = ln(1+z) between the ends of the
         // event's range (the fitted polynomial at t = -1, +1), so that the CTA can issue its TMA copy at once.  Slots 26, 27 of
@@ -528,11 +536,11 @@ __global__ void __launch_bounds__(256) k_polyfit(const LamConst* __restrict__ Lc
 
 cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int n_lambda, int n_ranges, const double* tk_c,
                            const double* tk_h, const double* z_ref, double z_ref_const, bool is_inj, const double* pm,
-                           const double* lnm1_lo, const double* lnm1_hi, int n_mass, int mcap, float* out, cudaStream_t st) {
+                           const double* lnm1_lo, const double* lnm1_hi, int n_mass, int mcap, double dx_tab, float* out, cudaStream_t st) {
     const long long items = (long long)n_lambda * n_ranges;
     if (items <= 0) return cudaSuccess;
     k_polyfit<<<(unsigned)((items + 7) / 8), 256, 0, st>>>(Lc, tab, tab_rows, n_lambda, n_ranges, tk_c, tk_h, z_ref, z_ref_const,
-                                                            is_inj ? 1 : 0, pm, lnm1_lo, lnm1_hi, n_mass, mcap, out);
+                                                            is_inj ? 1 : 0, pm, lnm1_lo, lnm1_hi, n_mass, mcap, dx_tab, out);
     return cudaGetLastError();
 }
 
