@@ -34,7 +34,7 @@ ORACLE_KERNEL = [0, 0]        # oracle kernel id and bin count of the timed orac
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
-NCU_TRAFFIC_BYTES = 56.63e6 + 2.69e6   # k_events, O5-spectroscopic, 256-lambda launch (profiles/r01e)
+NCU_TRAFFIC_BYTES = 53.27e6 + 1.68e6   # k_events_fast, O5-spectroscopic, 256-lambda launch: dram read + write (profiles/r02)
 
 
 def default_workload(args):
@@ -176,6 +176,157 @@ def workload_config(w, args):
             "parallelism": f"lambda-sharded replicas x{args.gpus}, no data-path collective"}
 
 
+def load_instruction_counts():
+    """Per-unit instruction counts of the two hot kernels from the committed ncu captures (profiles/r02_instruction_counts.csv;
+    the .md beside it names the commands): {(workload, kernel): row}.  Absent file -> {} and the recipe entries read null."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "r02_instruction_counts.csv")
+    out = {}
+    if os.path.exists(p):
+        with open(p) as f:
+            for r in csv.DictReader(f):
+                out[(r["workload"], r["kernel"])] = r
+    return out
+
+
+def recipe_entry(counts, workload, kernel, units_per_step, ms_per_step, clk_hz):
+    """t_min = max(n_x / P_sfu, n_f / P_fp32) with the kernel's executed instruction counts (ncu), P_sfu = 148 x 16
+    lanes/clk, P_fp32 = 148 x 128 lanes/clk; fraction = t_min / t_measured (live).  Beside it the issue-slot fraction: warp
+    instructions / (148 SM x 4 schedulers x clock) / t_measured."""
+    r = counts.get((workload, kernel))
+    if r is None or ms_per_step <= 0:
+        return None
+    n_x = float(r["sfu_thread_inst_per_unit"]) * units_per_step
+    n_f = float(r["fp32_lane_ops_per_unit"]) * units_per_step
+    n_i = float(r["warp_inst_per_unit"]) * units_per_step
+    p_sfu, p_fp32, p_issue = SM_COUNT * 16 * clk_hz, SM_COUNT * FMA_LANES_PER_CLK_PER_SM * clk_hz, SM_COUNT * 4 * clk_hz
+    t = ms_per_step / 1e3
+    return {"t_min_ms": 1e3 * max(n_x / p_sfu, n_f / p_fp32), "frac": max(n_x / p_sfu, n_f / p_fp32) / t,
+            "sfu_frac": n_x / p_sfu / t, "fp32_frac": n_f / p_fp32 / t, "issue_slot_frac": n_i / p_issue / t,
+            "sfu_thread_inst_per_unit": float(r["sfu_thread_inst_per_unit"]), "fp32_lane_ops_per_unit": float(r["fp32_lane_ops_per_unit"]),
+            "warp_inst_per_unit": float(r["warp_inst_per_unit"]), "capture": r["capture"]}
+
+
+def measure(pkg, torch, dist, args, name, catalog, pixels, K, W, rank, world, local, want_pairs, want_e2e):
+    """W warm-up + K timed steps of the whole hot path on one workload; returns a dict of raw measurements."""
+    dev = torch.device("cuda", local)
+    t0 = time.perf_counter()
+    sub = argparse.Namespace(**vars(args))
+    sub.config, sub.catalog, sub.pixels = name, catalog, pixels
+    w = build_workload(name, sub, rank)
+    t_gen = time.perf_counter() - t0
+    lams = lambda_batches(w, K + W, rank)
+    stream = torch.cuda.current_stream(dev)
+    kk = pkg.CHIM_KERNEL_EPANECHNIKOV if args.kde_kernel == "epanechnikov" else pkg.CHIM_KERNEL_GAUSS
+    ctx = pkg.Context(device=local, stream=stream, z_cat_max=w.z_cat_max, kde_cutoff=args.cutoff,
+                      lambda_chunk=args.lambda_chunk, kde_kernel=kk, n_bins=args.bins)
+    t0 = time.perf_counter()
+    ctx.init_events(w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal)
+    if getattr(w, "group_off", None) is not None:
+        ctx.set_event_groups(w.group_off, w.ln_factor)
+    t_init_ev = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    if w.n_det > 0:
+        ctx.init_injections(w.inj_dL, w.inj_m1d, w.inj_m2d, w.inj_ln_pdraw, w.n_inj_total)
+    t_init_inj = time.perf_counter() - t0
+    lam_dev = [torch.as_tensor(l, device=dev).contiguous() for l in lams]
+    out = ctx.alloc_outputs(w.n_lambda, event_logI=False)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for i in range(W):
+        ctx.loglike_batch(lam_dev[i], out=out)
+    barrier()
+    ctx.set_profiling(True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    keys = ("tables_ms", "events_ms", "events_general_ms", "inject_ms", "combine_ms", "events_launches", "events_general_launches",
+            "inject_launches")
+    ktimes = {k: 0.0 for k in keys}
+    barrier()
+    t_wall0 = time.perf_counter()
+    for i in range(K):
+        flush.fill_(i & 0xFF)                   # evict L2 between timed steps
+        evs[i][0].record(stream)
+        ctx.loglike_batch(lam_dev[W + i], out=out)
+        evs[i][1].record(stream)
+        kt = ctx.kernel_times()                 # synchronises; outside the event bracket
+        for k in keys:
+            ktimes[k] += kt[k]
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop() if rank == 0 else None
+    ctx.set_profiling(False)
+    t_dev = float(np.sum([a.elapsed_time(b) for a, b in evs])) / 1e3
+    ll_last = out["loglike"].cpu().numpy()
+    fl_last = out["flags"].cpu().numpy()
+    st = ctx.stats()
+    r = dict(w=w, lams=lams, K=K, W=W, t_dev=t_dev, t_wall=t_wall, clocks=clocks, ktimes=ktimes, stats=st, ll_last=ll_last,
+             nonfinite_lambda=int((~np.isfinite(ll_last)).sum()), flagged_lambda=int((fl_last != 0).sum()),
+             t_gen=t_gen, t_init_ev=t_init_ev, t_init_inj=t_init_inj, pairs_eval=0, pairs_cut=0, t_e2e=None)
+
+    # ---- work counters: the first timed batch once more through k_events with its pair counters compiled in (untimed) ------
+    if want_pairs and rank == 0 and pixels == 0:
+        cctx = pkg.Context(device=local, stream=stream, z_cat_max=w.z_cat_max, kde_cutoff=args.cutoff,
+                           lambda_chunk=args.lambda_chunk, count_pairs=1)
+        cctx.init_events(w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal)
+        cout = cctx.alloc_outputs(w.n_lambda, event_logI=False)
+        cctx.loglike_batch(lam_dev[W], out=cout)
+        cst = cctx.stats()
+        r["pairs_eval"], r["pairs_cut"] = cst["kde_pairs_evaluated"], cst["kde_pairs_in_cutoff"]    # per batch
+        r["alu"] = cctx.alu_peaks()
+        cctx.close()
+
+    # ---- end-to-end arm: host buffers through chim_loglike_batch_host ---------------------------------------
+    if want_e2e:
+        lam_pin = [torch.as_tensor(l).contiguous().pin_memory() for l in lams[W:W + K]]
+        o_pin = {k: torch.empty(w.n_lambda, dtype=torch.float64).pin_memory() for k in ("loglike", "logxi", "neff")}
+        o_pin["flags"] = torch.empty(w.n_lambda, dtype=torch.int32).pin_memory()
+        ctx.loglike_batch_host(lam_pin[0], out=o_pin)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(K):
+            flush.fill_(i & 0xFF)
+            ctx.loglike_batch_host(lam_pin[i], out=o_pin)
+        barrier()
+        t_e2e = time.perf_counter() - t0
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)   # the flush is not part of the step
+        a.record(stream)
+        for i in range(K):
+            flush.fill_(i & 0xFF)
+        b.record(stream)
+        torch.cuda.synchronize(dev)
+        r["t_e2e"] = t_e2e - a.elapsed_time(b) / 1e3
+        # same kernels, same inputs: identical up to the order of fp64 sums (binning adds fp32 shared-memory atomics)
+        assert np.allclose(o_pin["loglike"].numpy(), ll_last, rtol=0, atol=1e-9 if args.bins == 0 else 1e-4, equal_nan=True)
+    ctx.close()
+    del flush
+    torch.cuda.empty_cache()
+    return r
+
+
+def kernel_block(r, counts, workload_key, clk_hz):
+    """Per-config summary: step time, per-kernel times, and the roofline entries of k_events_fast and k_inject."""
+    w, K, kt = r["w"], r["K"], r["ktimes"]
+    units = n_physical_events(w) * w.n_lambda
+    ev_ms, inj_ms = kt["events_ms"] / K, kt["inject_ms"] / K
+    n_sub = int(w.n_events) * w.n_lambda                       # (event, lambda) units of S2-S4 per step (sub-events for many-1d)
+    n_inj = int(w.n_det) * w.n_lambda                          # (injection, lambda) units of S5 per step
+    return {"ms_per_step": r["t_dev"] / K * 1e3, "value": units * K / r["t_dev"], "steps": K, "warmup": r["W"],
+            "kernel_ms_per_step": {"tables_ms": kt["tables_ms"] / K, "events_fast_ms": ev_ms, "events_general_ms": kt["events_general_ms"] / K,
+                                   "inject_ms": inj_ms, "combine_ms": kt["combine_ms"] / K},
+            "nonfinite_lambda": r["nonfinite_lambda"], "flagged_lambda": r["flagged_lambda"],
+            "roofline_k_events_fast": recipe_entry(counts, workload_key, "k_events_fast", n_sub, ev_ms, clk_hz),
+            "roofline_k_inject": recipe_entry(counts, workload_key, "k_inject", n_inj, inj_ms, clk_hz),
+            "init_s": {"generate_inputs": r["t_gen"], "chim_init_events": r["t_init_ev"], "chim_init_injections": r["t_init_inj"]}}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -188,117 +339,35 @@ def run_ours(args):
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
     pkg.lib()                                   # fails loudly without libchim.so: no fallback
-
-    w = build_workload(args.config, args, rank)
     K, W = args.steps, max(args.warmup, 3)
-    lams = lambda_batches(w, K + W, rank)
-    stream = torch.cuda.current_stream(dev)
-    kk = pkg.CHIM_KERNEL_EPANECHNIKOV if args.kde_kernel == "epanechnikov" else pkg.CHIM_KERNEL_GAUSS
-    ctx = pkg.Context(device=local, stream=stream, z_cat_max=w.z_cat_max, kde_cutoff=args.cutoff,
-                      lambda_chunk=args.lambda_chunk, kde_kernel=kk, n_bins=args.bins)
-    ctx.init_workload(w)                        # inputs resident in HBM from here on
-    lam_dev = [torch.as_tensor(l, device=dev).contiguous() for l in lams]
-    out = ctx.alloc_outputs(w.n_lambda, event_logI=False)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize(dev)
-
-    # ---- device-resident arm ---------------------------------------------------------------------------
-    for i in range(W):
-        ctx.loglike_batch(lam_dev[i], out=out)
-    barrier()
-    ctx.set_profiling(True)
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-    ktimes = dict(tables_ms=0.0, events_ms=0.0, inject_ms=0.0, combine_ms=0.0, events_launches=0)
-    barrier()
-    t_wall0 = time.perf_counter()
-    for i in range(K):
-        flush.fill_(i & 0xFF)                   # evict L2 between timed steps
-        evs[i][0].record(stream)
-        ctx.loglike_batch(lam_dev[W + i], out=out)
-        evs[i][1].record(stream)
-        kt = ctx.kernel_times()                 # synchronises; outside the event bracket
-        for k in ktimes:
-            ktimes[k] += kt[k]
-    barrier()
-    t_wall = time.perf_counter() - t_wall0
-    clocks = sampler.stop() if rank == 0 else None
-    ctx.set_profiling(False)
-    ms = [a.elapsed_time(b) for a, b in evs]
-    t_dev = float(np.sum(ms)) / 1e3
-    ll_last = out["loglike"].cpu().numpy()
-
-    # ---- work counters of the timed batches: the same kernels with pair counting compiled in, untimed ------
-    pairs_eval = pairs_cut = 0
-    alu = None
-    if rank == 0:
-        cctx = pkg.Context(device=local, stream=stream, z_cat_max=w.z_cat_max, kde_cutoff=args.cutoff,
-                           lambda_chunk=args.lambda_chunk, count_pairs=1)
-        cctx.init_events(w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal)
-        cout = cctx.alloc_outputs(w.n_lambda, event_logI=False)
-        for i in range(K):
-            cctx.loglike_batch(lam_dev[W + i], out=cout)
-            cst = cctx.stats()
-            pairs_eval += cst["kde_pairs_evaluated"]
-            pairs_cut += cst["kde_pairs_in_cutoff"]
-        alu = cctx.alu_peaks()
-        cctx.close()
-    # ---- S2 alone (CHIM_KDE_NONE: the same kernel with the KDE phase skipped), to split the fused kernel's time ------
-    ev_ms_s2 = None
-    if rank == 0:
-        sctx = pkg.Context(device=local, stream=stream, z_cat_max=w.z_cat_max, kde_cutoff=args.cutoff,
-                           lambda_chunk=args.lambda_chunk, kde_method=pkg.CHIM_KDE_NONE)
-        sctx.init_events(w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal)
-        sout = sctx.alloc_outputs(w.n_lambda, event_logI=False)
-        sctx.loglike_batch(lam_dev[0], out=sout)
-        sctx.set_profiling(True)
-        ev_ms_s2 = 0.0
-        for i in range(K):
-            flush.fill_(i & 0xFF)
-            sctx.loglike_batch(lam_dev[W + i], out=sout)
-            ev_ms_s2 += sctx.kernel_times()["events_ms"]
-        sctx.close()
-
-    # ---- end-to-end arm: host buffers through chim_loglike_batch_host -----------------------------------
-    lam_pin = [torch.as_tensor(l).contiguous().pin_memory() for l in lams[W:W + K]]
-    o_pin = {k: torch.empty(w.n_lambda, dtype=torch.float64).pin_memory() for k in ("loglike", "logxi", "neff")}
-    o_pin["flags"] = torch.empty(w.n_lambda, dtype=torch.int32).pin_memory()
-    ctx.loglike_batch_host(lam_pin[0], out=o_pin)
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(K):
-        flush.fill_(i & 0xFF)
-        ctx.loglike_batch_host(lam_pin[i], out=o_pin)
-    barrier()
-    t_e2e = time.perf_counter() - t0
-    # the flush is not part of the step: subtract its measured cost
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record(stream)
-    for i in range(K):
-        flush.fill_(i & 0xFF)
-    b.record(stream)
-    torch.cuda.synchronize(dev)
-    t_e2e -= a.elapsed_time(b) / 1e3
-    h2d = w.n_lambda * 15 * 8
-    d2h = w.n_lambda * (8 * 3 + 4)
-    # same kernels, same inputs: identical up to the order of fp64 sums (binning adds fp32 shared-memory atomics)
-    assert np.allclose(o_pin["loglike"].numpy(), ll_last, rtol=0, atol=1e-9 if args.bins == 0 else 1e-4, equal_nan=True)
+    counts = load_instruction_counts()
+    r = measure(pkg, torch, dist, args, args.config, args.catalog, args.pixels, K, W, rank, world, local, True, True)
+    w, ktimes, st, clocks = r["w"], r["ktimes"], r["stats"], r["clocks"]
 
     # ---- max over ranks ---------------------------------------------------------------------------------
-    t_all = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
+    t_all = torch.tensor([r["t_dev"], r["t_e2e"]], dtype=torch.float64, device=torch.device("cuda", local))
     if world > 1:
         dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
     t_dev_max, t_e2e_max = [float(x) for x in t_all.cpu()]
     units = n_physical_events(w) * w.n_lambda * K * world
-    st = ctx.stats()
+
+    # ---- the other BASELINE configs (rank 0, N = 1, default workload only): fewer steps each ------------------------
+    others = {}
+    if rank == 0 and world == 1 and default_workload(args) and not args.no_other_configs:
+        peaks0, _ = load_peaks()
+        clk0 = float(peaks0.get("sm_max_mhz", 1965.0)) * 1e6
+        for key, (name, cat, pix) in {"o5_spec_catalog1": ("o5_spec", 1, 0), "o5_spec_catalog2": ("o5_spec", 2, 0),
+                                      "o5_photo": ("o5_photo", 0, 0), "full_pop": ("full_pop", 0, 0), "sel_heavy": ("sel_heavy", 0, 0),
+                                      "o5_spec_many1d_8pixels": ("o5_spec", 0, 8)}.items():
+            try:
+                ro = measure(pkg, torch, dist, args, name, cat, pix, args.other_steps, 3, 0, 1, local, False, False)
+                wk = {"o5_spec": "o5_spec", "o5_photo": "o5_photo", "full_pop": "full_pop", "sel_heavy": "sel_heavy"}[name] if pix == 0 else "many1d"
+                others[key] = kernel_block(ro, counts, wk, clk0)
+                others[key]["workload"] = workload_config(ro["w"], argparse.Namespace(**dict(vars(args), pixels=pix)))["workload"]
+                del ro
+            except Exception as e:                       # a config that does not fit must not take the headline down
+                others[key] = {"error": repr(e)}
 
     if rank == 0:
         peaks, peak_src = load_peaks()
@@ -307,51 +376,55 @@ def run_ours(args):
         ev_s = ktimes["events_ms"] / 1e3
         clk_max = float(peaks.get("sm_max_mhz", 1965.0))
         peak_g = SM_COUNT * FMA_LANES_PER_CLK_PER_SM * clk_max * 1e6 / 1e9
+        pairs_cut, pairs_eval = r["pairs_cut"] * K, r["pairs_eval"] * K          # counted on one batch, scaled to the K timed ones
         achieved = pairs_cut / ev_s / 1e9 if ev_s > 0 else 0.0
-        executed = pairs_eval / ev_s / 1e9 if ev_s > 0 else 0.0
         clk_run = (clocks or {}).get("sm_mhz") or clk_max
+        kb = kernel_block(r, counts, "o5_spec" if default_workload(args) else "-", clk_max * 1e6)
+        h2d = w.n_lambda * 15 * 8
+        d2h = w.n_lambda * (8 * 3 + 4)
+        ns_tot, nz_tot = int(w.sample_off[-1]), int(w.grid_off[-1])
+        # what a k_events_fast launch (one lambda chunk) must bring from HBM once: the 24-byte sample records and q_g; the slices
+        # of the per-lambda mass table the events address (2 variants x ~200 rows x 16 B per unit) and the 112-byte polynomial
+        # records are written by S1 in the same chunk and come back from L2, but count as the kernel's own input
+        chunk = min(args.lambda_chunk, w.n_lambda)
+        alg_bytes = 24 * ns_tot + 4 * nz_tot + chunk * int(w.n_events) * (112 + 2 * 200 * 16)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": t_dev_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 (sample weights, KDE) + f64 (tables, fits, reductions)", "data": "synthetic",
             "config": workload_config(w, args),
             "kde_pairs_per_s_dense_equivalent": st["kde_pairs_dense"] * K * world / t_dev_max,
-            "kde_pairs_per_s_evaluated": pairs_eval * world / t_dev_max,
+            "kde_pairs_per_s_in_cutoff": pairs_cut * world / t_dev_max,
             "kde_cutoff_t": args.cutoff,
-            "kernel_ms_per_step": {k: ktimes[k] / K for k in ("tables_ms", "events_ms", "inject_ms", "combine_ms")},
-            "wall_ms_per_step_incl_flush_and_sync": t_wall / K * 1e3,
+            "kernel_ms_per_step": kb["kernel_ms_per_step"],
+            "wall_ms_per_step_incl_flush_and_sync": r["t_wall"] / K * 1e3,
             "e2e": {"value": units / t_e2e_max, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(st["kernel_launches"]) * K,
             "clocks": clocks,
-            "roofline": {"bound": "alu", "kernel": "k_events (S2-S4: weights + KDE + integral)",
+            "init_s": kb["init_s"],
+            "roofline": {"bound": "alu", "kernel": "k_events_fast (S2-S4: weights + KDE + integral)",
+                         # headline figure: the method's work -- Gaussian (sample, grid point) pairs inside the t*h cut-off, one fp32
+                         # FMA lane-op each in the cheapest exact formulation -- over the kernel's live-measured time
                          "achieved": achieved, "peak": peak_g, "unit": "G pairs/s (1 fp32 FMA lane-op per Gaussian pair)",
                          "frac": achieved / peak_g, "frac_at_sampled_clock": achieved / (peak_g * clk_run / clk_max),
-                         "achieved_executed": executed, "frac_executed": executed / peak_g,
-                         # DRAM bytes per k_events launch from the committed ncu --set full capture of this workload
-                         # (dram__bytes_read.sum + dram__bytes_write.sum); not measurable from inside bench.py
+                         "algorithmic_ops_per_launch": pairs_cut / n_launch, "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
+                         # SURVEY 8(d) recipe on what the kernel executes (ncu instruction counts x live time), and the issue slots
+                         "executed": kb["roofline_k_events_fast"],
                          "traffic": (NCU_TRAFFIC_BYTES if default_workload(args) else None),
-                         "traffic_source": ("profiles/r01e_k_events_k_inject_ncu_full.md" if default_workload(args) else None),
-                         # what a launch must bring from HBM once (records, 24 B per sample; the lambdas of a chunk share them in L2)
-                         "algorithmic_dram_bytes_per_launch": 24 * int(w.sample_off[-1]),
-                         "algorithmic_ops_per_launch": pairs_cut / n_launch,
-                         "executed_ops_per_launch": pairs_eval / n_launch,
-                         "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
-                         "kde_phase": (None if ev_ms_s2 is None else {
-                             "what": "k_events timed again with the KDE phase skipped (CHIM_KDE_NONE); the difference is S3+S4",
-                             "s2_only_ms_per_launch": ev_ms_s2 / n_launch,
-                             "kde_ms_per_launch": (ktimes["events_ms"] - ev_ms_s2) / n_launch,
-                             "achieved": pairs_cut / max((ktimes["events_ms"] - ev_ms_s2) / 1e3, 1e-9) / 1e9,
-                             "frac": pairs_cut / max((ktimes["events_ms"] - ev_ms_s2) / 1e3, 1e-9) / 1e9 / peak_g}),
-                         "measured_alu_peaks_gops": alu,
-                         "peak_source": f"148 SM x 128 fp32 FMA lanes/clk x {clk_max:.0f} MHz ({peak_src} sm_max_mhz); "
-                                        "achieved = pairs inside the t*h cut-off / k_events device time (which also holds S2, S4); "
-                                        "executed = incl. band padding; see DESIGN.md sec. 6"},
-            "loglike_sample": [float(x) for x in ll_last[:3]],
+                         "traffic_source": ("profiles/r02_k_events_fast_k_inject_ncu_full.md" if default_workload(args) else None),
+                         "algorithmic_dram_bytes_per_launch": alg_bytes,
+                         "measured_alu_peaks_gops": r.get("alu"),
+                         "peak_source": f"148 SM x 128 fp32 FMA lanes/clk x {clk_max:.0f} MHz ({peak_src} sm_max_mhz); see DESIGN.md sec. 6"},
+            "roofline_k_inject": dict(kb["roofline_k_inject"] or {}, kernel="k_inject (S5)",
+                                      evals_per_s=int(w.n_det) * w.n_lambda * K / max(ktimes["inject_ms"] / 1e3, 1e-12),
+                                      ms_per_step=ktimes["inject_ms"] / K),
+            "nonfinite_lambda": kb["nonfinite_lambda"],
+            "other_configs": others,
+            "loglike_sample": [float(x) for x in r["ll_last"][:3]],
         }
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(w, lams[0], args)
+            line["cpu_baseline"] = cpu_baseline(w, r["lams"][0], args)
         print(json.dumps(line))
-    ctx.close()
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -388,6 +461,8 @@ def main():
     ap.add_argument("--pixels", type=int, default=0,
                     help="many-1d variant: split every event into this many (event, pixel) sub-events (0 = single-1d, the headline)")
     ap.add_argument("--cpu-lambdas", type=int, default=2)
+    ap.add_argument("--other-steps", type=int, default=3, help="timed steps for each of the other configs in `other_configs`")
+    ap.add_argument("--no-other-configs", action="store_true", help="only the headline workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     ORACLE_KERNEL[0] = 1 if args.kde_kernel == "epanechnikov" else 0

@@ -30,7 +30,7 @@ constexpr int kFLeP = 12;            // terms of the local expansion
 constexpr int kFMaxBox = 96;         // boxes per event
 constexpr int kFBoxPerWarp = kFMaxBox / kFW;
 constexpr float kFMaxW = 1.3f;       // largest box width in units of sqrt(2) h
-constexpr int kFMaxD = 160;          // largest half-width of the psi table (grid points)
+constexpr int kFMaxD = 256;          // largest half-width of the psi table (grid points; ~60 on the spectroscopic, ~240 on the 4096-point photometric grids)
 constexpr int kFQPad = 2 * kFMaxD;   // zeros on both sides of the staged q_g: the coefficient build reads g_b +- d unchecked
 constexpr int kFMassStage = 384;     // mass-table rows staged per variant (>= events_mass_stage_rows: k_polyfit sizes the slice)
 

@@ -32,6 +32,8 @@ struct InjSmem {
 
 __device__ __forceinline__ uint32_t inj_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// kDbg: the diagnostic instantiation also writes every s_j (chim_debug_injection_weights)
+template <bool kDbg>
 __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     InjSmem& S = *reinterpret_cast<InjSmem*>(smem_raw);
@@ -114,7 +116,11 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             amax *= 1.0f + 1e-5f;
             const float* bm = P.inj.blk_m2d + (size_t)chunk * (kInjChunkBlocks);
             const int nblk = (n + kInjThreads - 1) / kInjThreads;
-            for (; k0 < nblk - 1 && __ldg(bm + k0) * amax < F.mlow_hi; ++k0) {}
+            // (one round trip: lane L looks at blocks L and L + 32; the block maxima increase with the block index)
+            const unsigned lo = __ballot_sync(0xffffffffu, !(__ldg(bm + lane) * amax < F.mlow_hi));
+            const unsigned hi = __ballot_sync(0xffffffffu, !(__ldg(bm + 32 + lane) * amax < F.mlow_hi));
+            k0 = lo ? __ffs(lo) - 1 : (hi ? 32 + __ffs(hi) - 1 : kInjChunkBlocks);
+            k0 = max(0, min(k0, nblk - 1));
         }
 #define CHIM_INJ_SAMPLE(TURN, REC, JJ)                                                                                \
         {                                                                                                             \
@@ -123,7 +129,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             const double s = (zc <= 0.f && (JJ) < n) ? ex2_to_double(l2w) : 0.0;                                      \
             acc[0] += s;                                                                                              \
             acc[1] = fma(s, s, acc[1]);                                                                               \
-            if (P.dbg_s && (JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale;                                \
+            if (kDbg && (JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale;                                   \
         }
 #define CHIM_INJ_SWEEP(TURN)                                                                                          \
         {                                                                                                             \
@@ -137,7 +143,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             }                                                                                                         \
             if (j < n32) CHIM_INJ_SAMPLE(TURN, R0, j)                                                                 \
         }
-        if (P.dbg_s)
+        if (kDbg)
             for (int j = tid; j < min(k0 * kInjThreads, n); j += kInjThreads) P.dbg_s[P.inj.perm[j0 + j]] = 0.0;
         if (turn_folded) CHIM_INJ_SWEEP(false)
         else CHIM_INJ_SWEEP(true)
@@ -162,7 +168,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             const double s = (zc <= 0.f && j < j1) ? ex2_to_double(l2w) : 0.0;   // support of the selection-term z density (R6)
             acc[0] += s;
             acc[1] = fma(s, s, acc[1]);
-            if (P.dbg_s && j < j1) P.dbg_s[P.inj.perm[j]] = s * P.dbg_scale;
+            if (kDbg && j < j1) P.dbg_s[P.inj.perm[j]] = s * P.dbg_scale;
         }
     }
     acc[0] = warp_sum(acc[0]);
@@ -185,9 +191,10 @@ size_t inject_smem_bytes(int n_mass) {
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st) {
     if (n_blocks <= 0) return cudaSuccess;
     size_t smem = inject_smem_bytes(P.n_mass);
-    cudaError_t e = cudaFuncSetAttribute(k_inject, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    auto kern = P.dbg_s ? k_inject<true> : k_inject<false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_inject<<<(unsigned)((long long)n_blocks * P.n_lambda), kInjThreads, smem, st>>>(P);
+    kern<<<(unsigned)((long long)n_blocks * P.n_lambda), kInjThreads, smem, st>>>(P);
     return cudaGetLastError();
 }
 
