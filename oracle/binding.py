@@ -28,6 +28,7 @@ def lib():
         _lib.chimo_event_integral.restype = C.c_double
         _lib.chimo_event_logI.restype = C.c_double
         _lib.chimo_neff.restype = C.c_double
+        _lib.chimo_pgal.restype = C.c_double
         _lib.chimo_init()
     return _lib
 
@@ -209,6 +210,16 @@ def pcat(lam, z_gal, sigma_gal, zg, w_gal=None):
     out = np.empty_like(zg)
     lib().chimo_pcat(_p(lam), C.c_int(zt.size), _p(zt), _p(st), _p(wg), C.c_int(zg.size), _p(zg), _p(out))
     return out
+
+
+def pgal(lam, z_max, z_gal, sigma_gal, z_compl, p_compl, zg, w_gal=None):
+    """PAPER.md:58 eq. 7 with eq. 9-10 for one line of sight (reading R25): returns (p_gal on zg, f_R)."""
+    lam, zt, st, zc, pc, zg = _lam(lam), _d(z_gal), _d(sigma_gal), _d(z_compl), _d(p_compl), _d(zg)
+    wg = None if w_gal is None else _d(w_gal)
+    out = np.empty_like(zg)
+    fr = lib().chimo_pgal(_p(lam), C.c_double(z_max), C.c_int(zt.size), _p(zt), _p(st), _p(wg), C.c_int(zc.size), _p(zc), _p(pc),
+                          C.c_int(zg.size), _p(zg), _p(out))
+    return out, float(fr)
 
 
 def selection_sums(lam, dl, m1d, m2d, ln_pdraw, z_cat_max=1.5, z_table_max=10.0, return_s=False):

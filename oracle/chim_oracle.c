@@ -665,6 +665,46 @@ void chimo_pcat(const double *lam, int n_gal, const double *zt, const double *st
     free(coef);
 }
 
+/* ---------------------------------------------------- p_gal with the completeness terms ---- */
+/* PAPER.md:58 eq. 7, :65 eq. 9, :67 eq. 10 for one line of sight (reading R25 of DESIGN.md):
+ *   p_gal(z) = f_R p_cat(z) + (1 - f_R) p_miss(z),   (1 - f_R) p_miss(z) = [1 - P_compl(z)] u(z),
+ *   u(z) = (dV_c/dz)(z) / V_c(z_max) on [0, z_max], 0 beyond (the homogeneous density of eq. 9; the same u as in xi, R6),
+ *   f_R = (1/V_c(z_max)) int dV_c P_compl = int_0^{z_max} P_compl(z) u(z) dz                                   (eq. 10)
+ * The completeness P_compl(z) of the line of sight is given at nc nodes zc (increasing), linear in between and constant
+ * beyond the first / last node.  f_R: Gauss-Legendre on every stretch between consecutive nodes (and 0, z_max).
+ * p_cat: chimo_pcat (eq. 8).  Returns f_R. */
+typedef struct { const lam_t *L; int nc; const double *zc, *pc; double vmax; } compl_ctx;
+static double compl_at(const compl_ctx *c, double z) {
+    if (z <= c->zc[0]) return c->pc[0];
+    if (z >= c->zc[c->nc - 1]) return c->pc[c->nc - 1];
+    int k = 0;
+    while (k + 2 < c->nc && z >= c->zc[k + 1]) ++k;
+    double t = (z - c->zc[k]) / (c->zc[k + 1] - c->zc[k]);
+    return c->pc[k] + t * (c->pc[k + 1] - c->pc[k]);
+}
+static double compl_integrand(double z, const void *ctx) {
+    const compl_ctx *c = (const compl_ctx *)ctx;
+    return compl_at(c, z) * dVc_dz(z, c->L) / c->vmax;
+}
+double chimo_pgal(const double *lam, double z_max, int n_gal, const double *zt, const double *st, const double *w, int nc,
+                  const double *zc, const double *pc, int ng, const double *zg, double *out) {
+    gl_init();
+    const lam_t *L = (const lam_t *)lam;
+    compl_ctx c = {L, nc, zc, pc, V_c(z_max, L)};
+    double fR = 0.0, a = 0.0;
+    for (int k = 0; k <= nc; ++k) {   /* stretches [0, zc_0], [zc_0, zc_1], ..., [zc_last, z_max], clipped to [0, z_max] */
+        double b = (k < nc) ? zc[k] : z_max;
+        if (b > z_max) b = z_max;
+        if (b > a) { fR += gl_integrate(compl_integrand, &c, a, b, 1 + (int)((b - a) / 0.25)); a = b; }
+    }
+    chimo_pcat(lam, n_gal, zt, st, w, ng, zg, out);
+    for (int i = 0; i < ng; ++i) {
+        double u = (zg[i] <= z_max) ? dVc_dz(zg[i], L) / c.vmax : 0.0;
+        out[i] = fR * out[i] + (1.0 - compl_at(&c, zg[i])) * u;
+    }
+    return fR;
+}
+
 /* ------------------------------------------------------------------------- O11 log L -------- */
 void chimo_loglike_batch_grouped(int n_lambda, const double *lam, int placement, int bw_rule,
                          double z_cat_max, double z_table_max, int n_table, double neff_factor,

@@ -653,6 +653,40 @@ def test_pcat_narrow_galaxies_reduce_to_the_gaussian_mixture_and_h0_cancels():
     assert np.allclose(O.pcat(la, zt, np.array([0.02, 0.03]), z2), O.pcat(lam(H0=35.0, Om=0.3), zt, np.array([0.02, 0.03]), z2), rtol=1e-13)
 
 
+# ------------------------------------------------------------------ completeness terms (NEXT-3; eq. 7, 9, 10; R25)
+def test_pgal_completeness_limits_fR_against_scipy_and_unit_mass():
+    la = lam(H0=67.0, Om=0.31)
+    rng = np.random.default_rng(4)
+    zt = rng.uniform(0.2, 1.0, 9)
+    st = 0.01 * (1 + zt)
+    zmax = 1.5
+    zg = np.linspace(0.0, 1.6, 33)
+    pcat = O.pcat(la, zt, st, zg)
+    dv = lambda z: O.volume(la, np.array([z]))[0][0]
+    vmax = O.volume(la, np.array([zmax]))[1][0]
+    u = np.array([dv(z) / vmax if z <= zmax else 0.0 for z in zg])
+    # P_compl = 1: complete catalogue -> p_gal = p_cat, f_R = 1;  P_compl = 0: nothing catalogued -> p_gal = u(z) of R6, f_R = 0
+    p1, f1 = O.pgal(la, zmax, zt, st, [0.0, 2.0], [1.0, 1.0], zg)
+    assert abs(f1 - 1) < 1e-12 and np.allclose(p1, pcat, rtol=1e-12, atol=1e-300)
+    p0, f0 = O.pgal(la, zmax, zt, st, [0.0, 2.0], [0.0, 0.0], zg)
+    assert f0 == 0 and np.allclose(p0, u, rtol=1e-12, atol=1e-300)
+    # a completeness falling with z (piecewise linear, constant beyond its nodes): f_R = int P u dz by scipy, eq. 7 term by term
+    zc, pc = np.array([0.1, 0.4, 0.9, 1.2]), np.array([0.95, 0.8, 0.3, 0.05])
+    P = lambda z: float(np.interp(z, zc, pc))
+    fr_ref = sum(integrate.quad(lambda z: P(z) * dv(z) / vmax, a, b, epsabs=0, epsrel=1e-12)[0]
+                 for a, b in zip([0.0, 0.1, 0.4, 0.9, 1.2], [0.1, 0.4, 0.9, 1.2, zmax]))
+    pg, fr = O.pgal(la, zmax, zt, st, zc, pc, zg)
+    assert abs(fr - fr_ref) < 1e-11 and 0.1 < fr < 0.6
+    assert np.allclose(pg, fr * pcat + (1 - np.array([P(z) for z in zg])) * u, rtol=1e-12, atol=1e-300)
+    # unit mass: f_R + int (1 - P) u = 1 (all galaxies inside the grid)
+    zf = np.linspace(0.0, zmax, 30001)
+    pf, _ = O.pgal(la, zmax, zt, st, zc, pc, zf)
+    assert abs(np.trapezoid(pf, zf) - 1) < 1e-8
+    # only the shape of the cosmology matters (H0 cancels in u and in p_cat)
+    p2, f2 = O.pgal(lam(H0=90.0, Om=0.31), zmax, zt, st, zc, pc, zg)
+    assert abs(f2 - fr) < 1e-13 and np.allclose(p2, pg, rtol=1e-12, atol=1e-300)
+
+
 # ------------------------------------------------------------------ sample binning (NEXT-2; reading R23)
 def test_binning_conserves_moments_and_reduces_to_the_unbinned_kde():
     rng = np.random.default_rng(9)
