@@ -164,11 +164,27 @@ int chim_set_event_groups(chim_ctx *ctx, int32_t n_groups, const int64_t *group_
  *   z_gal >= 0, sigma_gal > 0, w_gal > 0 or NULL (unit weights)
  *   grid_off [n_los+1] CSR offsets into z_grid / p_cat_out;  z_grid >= 0
  * All pointers live where cfg.mem says (p_cat_out too); synchronous.  The result can be passed to chim_init_events as p_gal
- * (complete catalogue, as in the paper's runs; the completeness terms of eq. 7, 9, 10 are not built).
+ * (complete catalogue, as in the paper's runs; for an incomplete one see chim_build_pgal).
  */
 int chim_build_pcat(chim_ctx *ctx, double omega_m, int32_t n_los, const int64_t *gal_off, const double *z_gal,
                     const double *sigma_gal, const double *w_gal, const int64_t *grid_off, const double *z_grid,
                     double *p_cat_out);
+
+/*
+ * The same with the completeness terms (PAPER.md:58 eq. 7, :65 eq. 9, :67 eq. 10; reading R25): per line of sight
+ *     p_gal(z) = f_R p_cat(z) + [1 - P_compl(z)] u(z),  u(z) = (dVc/dz)(z) / Vc(z_max) on [0, z_max], 0 beyond,
+ *     f_R = int_0^z_max P_compl(z) u(z) dz                       (= (1/Vc(z_max)) int dVc P_compl, eq. 10)
+ * i.e. eq. 7 with the homogeneously distributed missing galaxies of eq. 9, (1 - f_R) p_miss = (1 - P_compl) u.
+ *   compl_off [n_los+1] CSR offsets into z_compl / p_compl (>= 2 nodes per line of sight)
+ *   z_compl strictly increasing and >= 0 per line of sight; 0 <= p_compl <= 1: the completeness P_compl at the nodes,
+ *           linear in between, constant beyond the first / last node
+ *   z_max > 0: the z_max of eq. 9-10 (use cfg.z_cat_max for consistency with the selection term, R6)
+ *   f_R_out [n_los] or NULL
+ * Everything else as chim_build_pcat.  P_compl = 1 gives p_cat and f_R = 1; P_compl = 0 gives u(z) and f_R = 0.
+ */
+int chim_build_pgal(chim_ctx *ctx, double omega_m, double z_max, int32_t n_los, const int64_t *gal_off, const double *z_gal,
+                    const double *sigma_gal, const double *w_gal, const int64_t *compl_off, const double *z_compl,
+                    const double *p_compl, const int64_t *grid_off, const double *z_grid, double *p_gal_out, double *f_R_out);
 
 /*
  * Detected injections for the selection term: n_det stored injections out of

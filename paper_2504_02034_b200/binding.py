@@ -80,6 +80,7 @@ def lib():
     L.chim_init_injections.argtypes = [C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 4
     L.chim_set_event_groups.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.chim_build_pcat.argtypes = [C.c_void_p, C.c_double, C.c_int32] + [C.c_void_p] * 7
+    L.chim_build_pgal.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int32] + [C.c_void_p] * 11
     L.chim_loglike_batch.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_loglike_batch_host.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_get_stats.argtypes = [C.c_void_p, C.POINTER(ChimStats)]
@@ -149,6 +150,13 @@ def chim_set_event_groups(ctx, n_groups, group_off, ln_factor):
 def chim_build_pcat(ctx, omega_m, n_los, gal_off, z_gal, sigma_gal, w_gal, grid_off, z_grid, p_cat_out):
     _check(ctx, lib().chim_build_pcat(ctx, omega_m, n_los, *[_addr(a) for a in (gal_off, z_gal, sigma_gal, w_gal, grid_off,
                                                                                z_grid, p_cat_out)]))
+
+
+def chim_build_pgal(ctx, omega_m, z_max, n_los, gal_off, z_gal, sigma_gal, w_gal, compl_off, z_compl, p_compl, grid_off, z_grid,
+                    p_gal_out, f_r_out=None):
+    _check(ctx, lib().chim_build_pgal(ctx, omega_m, z_max, n_los, *[_addr(a) for a in (gal_off, z_gal, sigma_gal, w_gal, compl_off,
+                                                                                       z_compl, p_compl, grid_off, z_grid, p_gal_out,
+                                                                                       f_r_out)]))
 
 
 def chim_init_injections(ctx, n_det, n_inj_total, dL, m1d, m2d, ln_pdraw):
@@ -247,6 +255,17 @@ class Context:
         chim_build_pcat(self.h, float(omega_m), len(go) - 1, go, _f64(z_gal), _f64(sigma_gal),
                         None if w_gal is None else _f64(w_gal), po, zg, out)
         return out
+
+    def build_pgal(self, omega_m, z_max, gal_off, z_gal, sigma_gal, compl_off, z_compl, p_compl, grid_off, z_grid, w_gal=None):
+        """PAPER.md:58 eq. 7 with eq. 9-10 on the given grids (host arrays in); returns (p_gal, f_R per line of sight)."""
+        go = np.ascontiguousarray(gal_off, dtype=np.int64)
+        co = np.ascontiguousarray(compl_off, dtype=np.int64)
+        po = np.ascontiguousarray(grid_off, dtype=np.int64)
+        zg = _f64(z_grid)
+        out, fr = np.empty_like(zg), np.empty(len(go) - 1)
+        chim_build_pgal(self.h, float(omega_m), float(z_max), len(go) - 1, go, _f64(z_gal), _f64(sigma_gal),
+                        None if w_gal is None else _f64(w_gal), co, _f64(z_compl), _f64(p_compl), po, zg, out, fr)
+        return out, fr
 
     def set_event_groups(self, group_off, ln_factor):
         """many-1d: the loaded entries are (event, pixel) sub-events; None removes the grouping."""

@@ -666,34 +666,50 @@ int chim_set_event_groups(chim_ctx* ctx, int32_t n_groups, const int64_t* group_
     return CHIM_OK;
 }
 
-int chim_build_pcat(chim_ctx* ctx, double omega_m, int32_t n_los, const int64_t* gal_off, const double* z_gal,
-                    const double* sigma_gal, const double* w_gal, const int64_t* grid_off, const double* z_grid,
-                    double* p_cat_out) {
+// eq. 8 (and, with a completeness map, eq. 7, 9, 10) on redshift grids; shared by chim_build_pcat / chim_build_pgal
+static int build_pgal_impl(chim_ctx* ctx, const char* who, double omega_m, double z_max, int32_t n_los, const int64_t* gal_off,
+                           const double* z_gal, const double* sigma_gal, const double* w_gal, const int64_t* compl_off,
+                           const double* z_compl, const double* p_compl, const int64_t* grid_off, const double* z_grid,
+                           double* p_out, double* f_r_out) {
+    const std::string W(who);
     if (!ctx) return CHIM_EINVAL;
-    if (n_los < 1 || !gal_off || !z_gal || !sigma_gal || !grid_off || !z_grid || !p_cat_out || !(omega_m > 0.0) || !(omega_m <= 1.0))
-        return fail(ctx, CHIM_EINVAL, "chim_build_pcat: null pointer, n_los < 1 or omega_m outside (0, 1]");
+    if (n_los < 1 || !gal_off || !z_gal || !sigma_gal || !grid_off || !z_grid || !p_out || !(omega_m > 0.0) || !(omega_m <= 1.0))
+        return fail(ctx, CHIM_EINVAL, W + ": null pointer, n_los < 1 or omega_m outside (0, 1]");
+    const bool with_compl = compl_off != nullptr;
+    if (with_compl && (!z_compl || !p_compl || !(z_max > 0.0) || !std::isfinite(z_max)))
+        return fail(ctx, CHIM_EINVAL, W + ": null completeness arrays or z_max <= 0");
     CK(cudaSetDevice(ctx->cfg.device));
-    std::vector<int64_t> go, po;
+    std::vector<int64_t> go, po, co;
     CK(fetch(ctx, gal_off, (size_t)n_los + 1, go));
     CK(fetch(ctx, grid_off, (size_t)n_los + 1, po));
-    if (go[0] != 0 || po[0] != 0) return fail(ctx, CHIM_EINVAL, "chim_build_pcat: offsets must start at 0");
-    for (int i = 0; i < n_los; ++i)
+    if (with_compl) CK(fetch(ctx, compl_off, (size_t)n_los + 1, co));
+    if (go[0] != 0 || po[0] != 0 || (with_compl && co[0] != 0)) return fail(ctx, CHIM_EINVAL, W + ": offsets must start at 0");
+    for (int i = 0; i < n_los; ++i) {
         if (go[i + 1] <= go[i] || po[i + 1] < po[i])
-            return fail(ctx, CHIM_EINVAL, "chim_build_pcat: every line of sight needs >= 1 galaxy; offsets must not decrease");
-    const size_t NG = (size_t)go[n_los], NP = (size_t)po[n_los];
-    std::vector<double> hz, hs, hw, hg;
+            return fail(ctx, CHIM_EINVAL, W + ": every line of sight needs >= 1 galaxy; offsets must not decrease");
+        if (with_compl && co[i + 1] - co[i] < 2) return fail(ctx, CHIM_EINVAL, W + ": every line of sight needs >= 2 completeness nodes");
+    }
+    const size_t NG = (size_t)go[n_los], NP = (size_t)po[n_los], NC = with_compl ? (size_t)co[n_los] : 0;
+    std::vector<double> hz, hs, hw, hg, hzc, hpc;
     CK(fetch(ctx, z_gal, NG, hz)); CK(fetch(ctx, sigma_gal, NG, hs)); CK(fetch(ctx, z_grid, NP, hg));
     if (w_gal) CK(fetch(ctx, w_gal, NG, hw));
-    if (!all_finite(hz) || !all_finite(hs) || !all_finite(hw) || !all_finite(hg)) return fail(ctx, CHIM_EINVAL, "chim_build_pcat: non-finite input");
+    if (with_compl) { CK(fetch(ctx, z_compl, NC, hzc)); CK(fetch(ctx, p_compl, NC, hpc)); }
+    if (!all_finite(hz) || !all_finite(hs) || !all_finite(hw) || !all_finite(hg) || !all_finite(hzc) || !all_finite(hpc))
+        return fail(ctx, CHIM_EINVAL, W + ": non-finite input");
     for (size_t g = 0; g < NG; ++g)
         if (hz[g] < 0.0 || !(hs[g] > 0.0) || (w_gal && !(hw[g] > 0.0)))
-            return fail(ctx, CHIM_EINVAL, "chim_build_pcat: need z_gal >= 0, sigma_gal > 0, w_gal > 0");
+            return fail(ctx, CHIM_EINVAL, W + ": need z_gal >= 0, sigma_gal > 0, w_gal > 0");
     for (size_t i = 0; i < NP; ++i)
-        if (hg[i] < 0.0) return fail(ctx, CHIM_EINVAL, "chim_build_pcat: z_grid must be >= 0");
+        if (hg[i] < 0.0) return fail(ctx, CHIM_EINVAL, W + ": z_grid must be >= 0");
+    if (with_compl)
+        for (int i = 0; i < n_los; ++i)
+            for (int64_t k = co[i]; k < co[i + 1]; ++k)
+                if (hpc[k] < 0.0 || hpc[k] > 1.0 || hzc[k] < 0.0 || (k > co[i] && !(hzc[k] > hzc[k - 1])))
+                    return fail(ctx, CHIM_EINVAL, W + ": need 0 <= P_compl <= 1 on strictly increasing z_compl >= 0");
     std::vector<void*> pool;
-    const int64_t *d_go = nullptr, *d_po = nullptr;
-    const double *d_z = nullptr, *d_s = nullptr, *d_w = nullptr, *d_g = nullptr;
-    double *d_coef = nullptr, *d_out = nullptr;
+    const int64_t *d_go = nullptr, *d_po = nullptr, *d_co = nullptr;
+    const double *d_z = nullptr, *d_s = nullptr, *d_w = nullptr, *d_g = nullptr, *d_zc = nullptr, *d_pc = nullptr;
+    double *d_coef = nullptr, *d_out = nullptr, *d_fr = nullptr;
     cudaError_t e = upload(pool, &d_go, go);
     if (e == cudaSuccess) e = upload(pool, &d_po, po);
     if (e == cudaSuccess) e = upload(pool, &d_z, hz);
@@ -702,13 +718,34 @@ int chim_build_pcat(chim_ctx* ctx, double omega_m, int32_t n_los, const int64_t*
     if (e == cudaSuccess) e = upload(pool, &d_g, hg);
     if (e == cudaSuccess) e = dev_alloc(pool, &d_coef, NG);
     if (e == cudaSuccess) e = dev_alloc(pool, &d_out, NP);
+    if (e == cudaSuccess && with_compl) e = upload(pool, &d_co, co);
+    if (e == cudaSuccess && with_compl) e = upload(pool, &d_zc, hzc);
+    if (e == cudaSuccess && with_compl) e = upload(pool, &d_pc, hpc);
+    if (e == cudaSuccess && with_compl) e = dev_alloc(pool, &d_fr, (size_t)n_los);
     if (e == cudaSuccess) e = launch_pcat(omega_m, n_los, d_go, d_z, d_s, d_w, d_po, d_g, d_coef, d_out, ctx->stream);
+    if (e == cudaSuccess && with_compl) e = launch_pgal(omega_m, z_max, n_los, d_co, d_zc, d_pc, d_po, d_g, d_out, d_fr, ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-    if (e == cudaSuccess && NP > 0)
-        e = cudaMemcpy(p_cat_out, d_out, NP * sizeof(double), ctx->cfg.mem == CHIM_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost);
+    const cudaMemcpyKind back = ctx->cfg.mem == CHIM_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (e == cudaSuccess && NP > 0) e = cudaMemcpy(p_out, d_out, NP * sizeof(double), back);
+    if (e == cudaSuccess && with_compl && f_r_out) e = cudaMemcpy(f_r_out, d_fr, (size_t)n_los * sizeof(double), back);
     free_pool(pool);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "chim_build_pcat");
+    if (e != cudaSuccess) return cuda_fail(ctx, e, who);
     return CHIM_OK;
+}
+
+int chim_build_pcat(chim_ctx* ctx, double omega_m, int32_t n_los, const int64_t* gal_off, const double* z_gal,
+                    const double* sigma_gal, const double* w_gal, const int64_t* grid_off, const double* z_grid,
+                    double* p_cat_out) {
+    return build_pgal_impl(ctx, "chim_build_pcat", omega_m, 0.0, n_los, gal_off, z_gal, sigma_gal, w_gal, nullptr, nullptr, nullptr,
+                           grid_off, z_grid, p_cat_out, nullptr);
+}
+
+int chim_build_pgal(chim_ctx* ctx, double omega_m, double z_max, int32_t n_los, const int64_t* gal_off, const double* z_gal,
+                    const double* sigma_gal, const double* w_gal, const int64_t* compl_off, const double* z_compl,
+                    const double* p_compl, const int64_t* grid_off, const double* z_grid, double* p_gal_out, double* f_r_out) {
+    if (ctx && !compl_off) return fail(ctx, CHIM_EINVAL, "chim_build_pgal: compl_off is NULL (use chim_build_pcat for a complete catalogue)");
+    return build_pgal_impl(ctx, "chim_build_pgal", omega_m, z_max, n_los, gal_off, z_gal, sigma_gal, w_gal, compl_off, z_compl, p_compl,
+                           grid_off, z_grid, p_gal_out, f_r_out);
 }
 
 int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, const double* dL, const double* m1d,

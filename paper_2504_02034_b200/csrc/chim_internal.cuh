@@ -554,6 +554,8 @@ cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, in
                                 double z_table_max, double* z_out, double* r_out, cudaStream_t st);
 cudaError_t launch_pcat(double Om, int n_los, const int64_t* gal_off, const double* zt, const double* st, const double* wg,
                         const int64_t* grid_off, const double* zg, double* coef, double* out, cudaStream_t st_);
+cudaError_t launch_pgal(double Om, double zmax, int n_los, const int64_t* compl_off, const double* zc, const double* pc,
+                        const int64_t* grid_off, const double* zg, double* out, double* fr_out, cudaStream_t st_);
 cudaError_t upload_gauss_legendre();   // fills the __constant__ node tables used by S1
 cudaError_t measure_alu_peaks(int n_sm, int reps, cudaStream_t st, double out_g[4]);
 size_t events_smem_bytes(int max_ns, int max_nz);

@@ -614,6 +614,75 @@ cudaError_t launch_pcat(double Om, int n_los, const int64_t* gal_off, const doub
     return cudaGetLastError();
 }
 
+// ---- completeness terms of p_gal (PAPER.md:58 eq. 7, :65 eq. 9, :67 eq. 10; one-off, R25) --------------------
+// One CTA per line of sight, after k_pcat has written p_cat into `out`:
+//   f_R = int_0^zmax P_compl(z) u(z) dz,  u = (dV_c/dz)/V_c(zmax) = 3 I(z)^2 / (E(z) I(zmax)^3),  I(z) = int_0^z dz'/E
+//   p_gal(z) = f_R p_cat(z) + [1 - P_compl(z)] u(z)  (u = 0 beyond zmax)
+// P_compl: nc nodes per line of sight, linear in between, constant beyond the ends.  f_R: one 32-node Gauss-Legendre panel on
+// every stretch between consecutive nodes (the integrand is a linear function times a smooth one there).  fp64 throughout.
+__device__ __forceinline__ double pcat_I(double z, double Om) {
+    double I = 0.0;
+    const double hz = 0.5 * z;
+#pragma unroll 4
+    for (int q = 0; q < kGLWin; ++q) {
+        const double a = 1.0 + hz * (1.0 + c_glw_x[q]);
+        I += c_glw_w[q] * rsqrt(Om * a * a * a + 1.0 - Om);
+    }
+    return I * hz;
+}
+__device__ __forceinline__ double compl_at(const double* __restrict__ zc, const double* __restrict__ pc, int nc, double z) {
+    if (z <= zc[0]) return pc[0];
+    if (z >= zc[nc - 1]) return pc[nc - 1];
+    int lo = 0, hi = nc - 1;                       // zc[lo] <= z < zc[hi]
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (zc[mid] <= z) lo = mid; else hi = mid; }
+    const double t = (z - zc[lo]) / (zc[lo + 1] - zc[lo]);
+    return pc[lo] + t * (pc[lo + 1] - pc[lo]);
+}
+__global__ void __launch_bounds__(256) k_pgal(double Om, double zmax, const int64_t* __restrict__ compl_off,
+                                              const double* __restrict__ zc_all, const double* __restrict__ pc_all,
+                                              const int64_t* __restrict__ grid_off, const double* __restrict__ zg,
+                                              double* __restrict__ out, double* __restrict__ fr_out) {
+    __shared__ double red[256 / 32];
+    __shared__ double s_fr;
+    const int e = blockIdx.x, tid = threadIdx.x;
+    const int64_t c0 = compl_off[e], p0 = grid_off[e], p1 = grid_off[e + 1];
+    const int nc = (int)(compl_off[e + 1] - c0);
+    const double* zc = zc_all + c0;
+    const double* pc = pc_all + c0;
+    const double Im = pcat_I(zmax, Om), inv_v = 3.0 / (Im * Im * Im);
+    double acc = 0.0;
+    for (int idx = tid; idx < (nc + 1) * kGLWin; idx += 256) {
+        const int k = idx / kGLWin, q = idx - k * kGLWin;
+        const double a = fmin((k == 0) ? 0.0 : zc[k - 1], zmax), b = fmin((k < nc) ? zc[k] : zmax, zmax);
+        if (b > a) {
+            const double hw = 0.5 * (b - a), z = a + hw * (1.0 + c_glw_x[q]);
+            acc += c_glw_w[q] * hw * compl_at(zc, pc, nc, z) * pcat_vol(z, Om) * inv_v;
+        }
+    }
+    acc = warp_sum(acc);
+    if ((tid & 31) == 0) red[tid >> 5] = acc;
+    __syncthreads();
+    if (tid == 0) {
+        double a = 0.0;
+        for (int k = 0; k < 256 / 32; ++k) a += red[k];
+        s_fr = a;
+        if (fr_out) fr_out[e] = a;
+    }
+    __syncthreads();
+    const double fr = s_fr;
+    for (int64_t i = p0 + tid; i < p1; i += 256) {
+        const double z = zg[i], u = (z <= zmax) ? pcat_vol(z, Om) * inv_v : 0.0;
+        out[i] = fr * out[i] + (1.0 - compl_at(zc, pc, nc, z)) * u;
+    }
+}
+
+cudaError_t launch_pgal(double Om, double zmax, int n_los, const int64_t* compl_off, const double* zc, const double* pc,
+                        const int64_t* grid_off, const double* zg, double* out, double* fr_out, cudaStream_t st_) {
+    if (n_los <= 0) return cudaSuccess;
+    k_pgal<<<n_los, 256, 0, st_>>>(Om, zmax, compl_off, zc, pc, grid_off, zg, out, fr_out);
+    return cudaGetLastError();
+}
+
 __global__ void k_table_lookup(const LamConst* __restrict__ Lc, const Row* __restrict__ tab, DlGrid g, int64_t n,
                                const double* __restrict__ dL, double z_table_max, double* __restrict__ z_out,
                                double* __restrict__ r_out) {

@@ -577,6 +577,49 @@ def test_build_pcat_matches_the_oracle_and_feeds_the_path(P):
     assert rel < REL_EVENT and dtot < ABS_TOTAL
 
 
+# ---------------------------------------------------------------- completeness terms (NEXT-3; eq. 7, 9, 10, R25)
+def test_build_pgal_matches_the_oracle_and_its_limits(P):
+    rng = np.random.default_rng(23)
+    om, zmax = 0.29, 1.5
+    ngal = [3, 80, 400, 1]
+    gal_off = np.concatenate([[0], np.cumsum(ngal)])
+    z_gal = np.concatenate([rng.uniform(0.05, 1.3, n) for n in ngal])
+    sig = np.where(rng.random(z_gal.size) < 0.5, 0.001, 0.03) * (1 + z_gal)
+    nz = [300, 1000, 4096, 57]
+    grid_off = np.concatenate([[0], np.cumsum(nz)])
+    z_grid = np.concatenate([np.linspace(lo, hi, n) for lo, hi, n in zip((0.0, 0.1, 0.3, 1.2), (1.0, 1.6, 1.2, 1.9), nz)])
+    # completeness maps: falling with z; two nodes only; many nodes; beyond z_max
+    zcs = [np.array([0.1, 0.4, 0.9, 1.2]), np.array([0.0, 1.5]), np.sort(rng.uniform(0.0, 1.7, 40)), np.array([0.2, 0.6, 1.0])]
+    pcs = [np.array([0.95, 0.8, 0.3, 0.05]), np.array([1.0, 0.0]), None, np.array([0.5, 0.5, 0.1])]
+    pcs[2] = np.clip(1.0 - zcs[2] / 1.4 + 0.05 * rng.standard_normal(40), 0.0, 1.0)
+    compl_off = np.concatenate([[0], np.cumsum([len(z) for z in zcs])])
+    c = P.Context()
+    got, fr = c.build_pgal(om, zmax, gal_off, z_gal, sig, compl_off, np.concatenate(zcs), np.concatenate(pcs), grid_off, z_grid)
+    la = lambda_vector(H0=70.0, Om=om)
+    for i in range(4):
+        g, p = slice(gal_off[i], gal_off[i + 1]), slice(grid_off[i], grid_off[i + 1])
+        ref, fr_ref = O.pgal(la, zmax, z_gal[g], sig[g], zcs[i], pcs[i], z_grid[p])
+        assert abs(fr[i] - fr_ref) < 1e-11, (i, fr[i], fr_ref)
+        assert np.allclose(got[p], ref, rtol=1e-10, atol=1e-290), i
+    # limits: P_compl = 1 -> the complete-catalogue p_cat and f_R = 1; P_compl = 0 -> f_R = 0 and no galaxy term at all
+    two = np.tile([0.0, 2.0], 4)
+    off2 = np.arange(5) * 2
+    pc1, f1 = c.build_pgal(om, zmax, gal_off, z_gal, sig, off2, two, np.ones(8), grid_off, z_grid)
+    assert np.allclose(f1, 1.0, atol=1e-12) and np.allclose(pc1, c.build_pcat(om, gal_off, z_gal, sig, grid_off, z_grid), rtol=1e-11, atol=1e-290)
+    pc0, f0 = c.build_pgal(om, zmax, gal_off, z_gal, sig, off2, two, np.zeros(8), grid_off, z_grid)
+    assert np.all(f0 == 0.0) and np.all(pc0[z_grid > zmax] == 0.0)
+    pc0b, _ = c.build_pgal(om, zmax, gal_off, z_gal + 0.01, 2 * sig, off2, two, np.zeros(8), grid_off, z_grid)
+    assert np.array_equal(pc0, pc0b)
+    # argument checks
+    with pytest.raises(P.ChimError):
+        c.build_pgal(om, zmax, gal_off, z_gal, sig, off2, two, np.full(8, 1.5), grid_off, z_grid)          # P_compl > 1
+    with pytest.raises(P.ChimError):
+        c.build_pgal(om, zmax, gal_off, z_gal, sig, off2, np.tile([0.5, 0.5], 4), np.ones(8), grid_off, z_grid)   # nodes not increasing
+    with pytest.raises(P.ChimError):
+        c.build_pgal(om, -1.0, gal_off, z_gal, sig, off2, two, np.ones(8), grid_off, z_grid)
+    c.close()
+
+
 # ---------------------------------------------------------------- sample binning (NEXT-2; reading R23)
 @pytest.mark.parametrize("kernel,nb", [("gauss", 256), ("gauss", 64), ("epanechnikov", 512)])
 def test_binned_samples_match_the_binned_oracle(P, kernel, nb):
