@@ -209,6 +209,9 @@ EventKernelParams event_params(const chim_ctx* ctx, int nl) {
     P.n_lambda = nl; P.tab_rows = ctx->ev_grid.rows(); P.n_mass = ctx->cfg.n_mass_table; P.n_table = ctx->cfg.n_table;
     P.placement = ctx->cfg.placement; P.bw_rule = ctx->cfg.bw_rule; P.kde_method = ctx->cfg.kde_method; P.kde_kernel = ctx->cfg.kde_kernel; P.n_bins = ctx->cfg.n_bins;
     P.z_table_max = ctx->cfg.z_table_max; P.cutoff = ctx->cfg.kde_cutoff;
+    // fp32 weights leave ~2e-5 / sqrt(n_eff) in log I: 64 keeps an event below 3e-6; the pixels of many-1d enter the event through a
+    // sum over pixels (a 600-sample pixel has n_eff ~ 100), so a lower bar keeps them on the fast sweep
+    P.neff_min = ctx->n_groups > 0 ? 24.f : 64.f;
     P.logI = ctx->logI; P.flags = ctx->flags; P.stats = ctx->stats;
     P.ln_shift = ctx->ev_ln_shift;
     P.ln_qscale = ctx->ev_ln_qscale;
@@ -262,7 +265,7 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
     if (fast) {
         FastEventParams FP{};
         FP.ev = ctx->ev; FP.Lc = ctx->Lc; FP.mtab = ctx->mtab; FP.poly = ctx->poly_ev;
-        FP.n_lambda = nl; FP.n_mass = cf.n_mass_table; FP.bw_rule = cf.bw_rule; FP.cutoff = cf.kde_cutoff;
+        FP.n_lambda = nl; FP.n_mass = cf.n_mass_table; FP.bw_rule = cf.bw_rule; FP.cutoff = cf.kde_cutoff; FP.neff_min = EP.neff_min;
         FP.logI = ctx->logI; FP.ln_shift = ctx->ev_ln_shift; FP.ln_qscale = ctx->ev_ln_qscale;
         FP.fast_events = ctx->fast_ev; FP.worklist = ctx->worklist; FP.work_count = ctx->work_count;
         CK(cudaMemsetAsync(ctx->work_count, 0, sizeof(unsigned int), st));

@@ -468,6 +468,7 @@ struct EventKernelParams {
     const double* dc_tab;    // [n_lambda][n_table+1+kZPad] (placement ON_GRID only) or null
     int32_t n_lambda, tab_rows, n_mass, n_table;
     int32_t placement, bw_rule, kde_method, kde_kernel, n_bins;
+    float neff_min;          // below this Kish n_eff the fp32 polynomial sweep is redone by the careful one
     double z_table_max, cutoff;
     double* logI;            // [n_lambda][n_events]
     uint32_t* flags;         // [n_lambda]
@@ -492,6 +493,7 @@ struct FastEventParams {
     const MassRow* mtab;     // [n_lambda][2][n_mass+2]
     const float* poly;       // [n_lambda][n_events][4 kPolyN]
     int32_t n_lambda, n_mass, bw_rule;
+    float neff_min;          // units with a Kish n_eff below this are handed over (k_events takes its careful sweep there)
     double cutoff;
     double* logI;            // [n_lambda][n_events]
     const double* ln_shift; const double* ln_qscale;

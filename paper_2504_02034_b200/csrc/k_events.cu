@@ -605,9 +605,9 @@ __device__ __forceinline__ void events_unit(const EventKernelParams& P, const in
                 for (int n = kPolyN - 3; n >= 0; --n) ad = fmaf(ad, Ad.x, S.poly[2 * kPolyN + 2 * n + 1]);
                 const float mp2d = fmaf(Ad.z, ad, -L.F.mlow_hi);
                 // fp32 leaves ~1e-6 (random) + ~5e-7 (the fit, common to all samples) in m2': d ln w = delta/m2'^2 of that.  The
-                // careful sweep is taken where this would show in log I: few effective samples (n_eff < 200), or all of them deep
+                // careful sweep is taken where this would show in log I: few effective samples (n_eff < neff_min), or all of them deep
                 const double neff = (1.0 + S.mom[0]) * (1.0 + S.mom[0]) / (1.0 + S.mom[1]);
-                S.careful = (S.mom[0] < 7.9e-31 /* 2^-100 */ || neff < 200.0 ||
+                S.careful = (S.mom[0] < 7.9e-31 /* 2^-100 */ || neff < (double)P.neff_min ||
                              (double)mp2d * (double)mp2d < (double)L.F.delta * fmax(0.5 * rsqrt(neff), 0.1)) ? 1 : 0;
             }
             __syncthreads();

@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
 
     // ---- every warp: the event's moments from the eight chunks (lane c takes chunk c), bandwidth, expansion geometry -------------
     // fp32 throughout: all sums are sums of positive terms (the second moment is taken about the weighted mean in a second
-    // step), n_eff >= 200 on this path, and dh/h = 1e-6 moves log I by ~5e-9
+    // step), n_eff >= neff_min (64; 24 for many-1d pixels) on this path, and dh/h = 1e-6 moves log I by ~5e-9
     const float cm = (lane < kFW) ? S.c_mx[lane] : -INFINITY;
     float gmx = cm, gmp2 = (lane < kFW) ? S.c_mp2[lane] : -INFINITY;
 #pragma unroll
@@ -270,7 +270,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     }
     // handed over: no bandwidth; few effective samples (fp32 weights, moments and the plain form of Scott's rule are good for
     // n_eff >> 1 only); every supported secondary deep in the smoothing window (m2' < ~0.3 sqrt(delta): d ln w = delta/m2'^2 x 1e-6)
-    bool hand = !(h > 0.0) || !isfinite(h) || !(neff >= 200.0f) || gmp2 * gmp2 < 0.1f * F.delta;
+    bool hand = !(h > 0.0) || !isfinite(h) || !(neff >= P.neff_min) || gmp2 * gmp2 < 0.1f * F.delta;
     // local-expansion geometry: y = z'/(sqrt(2) h), boxes of m grid spacings centred on grid points
     const double udz = __ldg(P.ev.uni_dz + ev), zfirst = __ldg(P.ev.zc + g0);
     const float scy = (float)(0.70710678118654752440 / h);
