@@ -286,3 +286,27 @@ def loglike_workload(w, lam=None, **kw):
         kw.setdefault("ln_factor", w.ln_factor)
     return loglike_batch(lam, w.sample_off, w.dL, w.m1d, w.m2d, w.ln_prior, w.grid_off, w.z_grid, w.p_gal,
                          inj=inj, n_inj_total=w.n_inj_total, **kw)
+
+
+def loglike_grad(w, lam, rel_step=1e-2, **kw):
+    """Gradient of log L with respect to the 15 hyper-parameters at ONE lambda, by its definition as a limit of difference
+    quotients: central differences of the fp64 oracle with one Richardson step,
+        g_k = [4 D(h_k / 2) - D(h_k)] / 3,  D(h) = [logL(lam + h e_k) - logL(lam - h e_k)] / 2h,  h_k = rel_step |lam_k| (rel_step if 0).
+    Returns (logL(lam), g[15])."""
+    lam = _lam(lam).reshape(15)
+    rows = [lam]
+    hs = []
+    for k in range(15):
+        h = rel_step * abs(lam[k]) if lam[k] != 0.0 else rel_step
+        hs.append(h)
+        for d in (1.0, -1.0, 0.5, -0.5):
+            r = lam.copy()
+            r[k] += d * h
+            rows.append(r)
+    f = loglike_workload(w, lam=np.array(rows), **kw)["loglike"]
+    g = np.empty(15)
+    for k in range(15):
+        d1 = (f[1 + 4 * k] - f[2 + 4 * k]) / (2.0 * hs[k])
+        d2 = (f[3 + 4 * k] - f[4 + 4 * k]) / hs[k]
+        g[k] = (4.0 * d2 - d1) / 3.0
+    return float(f[0]), g

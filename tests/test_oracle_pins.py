@@ -653,6 +653,40 @@ def test_pcat_narrow_galaxies_reduce_to_the_gaussian_mixture_and_h0_cancels():
     assert np.allclose(O.pcat(la, zt, np.array([0.02, 0.03]), z2), O.pcat(lam(H0=35.0, Om=0.3), zt, np.array([0.02, 0.03]), z2), rtol=1e-13)
 
 
+# ------------------------------------------------------------------ lambda-gradients (NEXT-4)
+def test_gradient_zero_directions_h0_scaling_identity_and_step_independence():
+    import dataclasses
+    w = make_workload("tiny", n_events=3, n_samples=150, n_grid=60, n_inj_draw=400)
+    la = w.lam[0].copy()
+    la[2], la[3] = 1.3, 1.7                                            # Xi0 != 1 so that n matters
+    f0, g = O.loglike_grad(w, la, rel_step=1e-2)
+    assert abs(f0 - O.loglike_workload(w, lam=la)["loglike"][0]) < 1e-12
+    # directions that provably do not matter: Xi0 = 1 -> n drops out of eq. 2; lambda_g = 0 -> mu_g, sigma_g drop out of eq. 20
+    lb = la.copy(); lb[2] = 1.0
+    assert abs(O.loglike_grad(w, lb)[1][3]) < 1e-9
+    lc = la.copy(); lc[11] = 0.0
+    gc = O.loglike_grad(w, lc)[1]
+    assert abs(gc[9]) < 1e-9 and abs(gc[10]) < 1e-9
+    # log L depends on H0 and on the distance scale of the data (events and injections, priors held fixed) through H0 x d_L only:
+    # z_j = Z(H0 d_L,j) and every weight carries the same 1/|d d_L/dz| ~ H0, which cancels between sum_i log I_i and N log xi.
+    # So H0 dlogL/dH0 = dlogL/dln(a) at a = 1 with all d_L -> a d_L -- the right side differentiates the DATA, not lambda
+    def f_scaled(a):
+        w2 = dataclasses.replace(w, dL=w.dL * a, inj_dL=w.inj_dL * a)
+        return O.loglike_workload(w2, lam=la)["loglike"][0]
+    e = 1e-2
+    d1 = (f_scaled(1 + e) - f_scaled(1 - e)) / (2 * e)
+    d2 = (f_scaled(1 + e / 2) - f_scaled(1 - e / 2)) / e
+    assert abs(la[0] * g[0] - (4 * d2 - d1) / 3) < 1e-5 * max(1.0, abs(la[0] * g[0]))
+    # the Richardson value does not hang on the step (O(h^4)): half the step, same gradient
+    _, g2 = O.loglike_grad(w, la, rel_step=5e-3)
+    scale = np.max(np.abs(g * la))
+    assert np.max(np.abs((g - g2) * la)) < 1e-5 * scale
+    # and agrees with a five-point stencil typed out here for one parameter (alpha)
+    h = 1e-2 * la[4]
+    fv = O.loglike_workload(w, lam=np.array([la + d * h * np.eye(15)[4] for d in (-2, -1, 1, 2)]))["loglike"]
+    assert abs(g[4] - (fv[0] - 8 * fv[1] + 8 * fv[2] - fv[3]) / (12 * h)) < 1e-5 * scale / la[4]
+
+
 # ------------------------------------------------------------------ completeness terms (NEXT-3; eq. 7, 9, 10; R25)
 def test_pgal_completeness_limits_fR_against_scipy_and_unit_mass():
     la = lam(H0=67.0, Om=0.31)
