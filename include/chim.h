@@ -212,6 +212,23 @@ int chim_loglike_batch_host(chim_ctx *ctx, int32_t n_lambda, const double *lambd
                             double *out_event_logI, double *out_logxi, double *out_neff,
                             uint32_t *out_flags);
 
+/*
+ * Gradient of log L with respect to the 15 hyper-parameters (the paper's stated direction: gradient-based samplers,
+ * PAPER.md:132, :175).  Central differences with one Richardson step,
+ *     dlogL/dlambda_k = [4 D(h_k/2) - D(h_k)] / 3,  D(h) = [logL(lambda + h e_k) - logL(lambda - h e_k)] / 2h,
+ *     h_k = rel_step |lambda_k| (rel_step where lambda_k = 0),
+ * evaluated on the device through the batched hot path itself: the 60 displaced points of every lambda are 60 more rows of
+ * one chim_loglike_batch (61 n_lambda rows in all).  DEVICE pointers, enqueue-only like chim_loglike_batch.
+ *   rel_step in (0, 0.5); 5e-3 .. 2e-2 keeps both the O(h^4) truncation and the fp32 noise of the path (~1e-5 in log L)
+ *            below 1e-3 of the gradient's scale
+ *   out_loglike [n_lambda]       log L at lambda itself
+ *   out_grad    [n_lambda x 15]  row-major; NaN / inf where a displaced point is not finite (the derivative is undefined there)
+ *   out_flags   [n_lambda] or NULL: OR of the flags of the 61 rows
+ * log L is smooth in lambda except where a sample crosses a support edge (m1 = m_high, z = z_cat_max for an injection).
+ */
+int chim_loglike_grad_batch(chim_ctx *ctx, int32_t n_lambda, const double *lambda, double rel_step, double *out_loglike,
+                            double *out_grad, uint32_t *out_flags);
+
 /* Work counters of the last chim_loglike_batch on this context (valid after the stream is synchronised;
  * the call itself synchronises).  kde_pairs_in_cutoff = (sample, grid point) pairs with |z_g - z_j| <= t*h, the
  * algorithmic work of S3; kde_pairs_evaluated = fp32 FMA lane-operations the KDE phase executed: in the direct and

@@ -83,6 +83,7 @@ def lib():
     L.chim_build_pgal.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int32] + [C.c_void_p] * 11
     L.chim_loglike_batch.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_loglike_batch_host.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
+    L.chim_loglike_grad_batch.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
     L.chim_get_stats.argtypes = [C.c_void_p, C.POINTER(ChimStats)]
     L.chim_set_profiling.argtypes = [C.c_void_p, C.c_int32]
     L.chim_get_kernel_times.argtypes = [C.c_void_p, C.POINTER(ChimKernelTimes)]
@@ -173,6 +174,10 @@ def chim_loglike_batch_host(ctx, n_lambda, lam, out_loglike, out_event_logI=None
                             out_flags=None):
     _check(ctx, lib().chim_loglike_batch_host(ctx, n_lambda, *[_addr(a) for a in (lam, out_loglike, out_event_logI,
                                                                                    out_logxi, out_neff, out_flags)]))
+
+
+def chim_loglike_grad_batch(ctx, n_lambda, lam, rel_step, out_loglike, out_grad, out_flags=None):
+    _check(ctx, lib().chim_loglike_grad_batch(ctx, n_lambda, _addr(lam), rel_step, _addr(out_loglike), _addr(out_grad), _addr(out_flags)))
 
 
 def chim_get_stats(ctx) -> ChimStats:
@@ -316,6 +321,16 @@ class Context:
             if event_logI:
                 out["event_logI"] = np.empty((n, self.n_events))
         chim_loglike_batch_host(self.h, n, lam, out["loglike"], out.get("event_logI"), out["logxi"], out["neff"], out["flags"])
+        return out
+
+    def loglike_grad_batch(self, lam, rel_step=1e-2):
+        """lam: torch CUDA float64 [n_lambda, 15] -> dict(loglike [n], grad [n, 15], flags [n]) of device tensors."""
+        t = self.torch
+        assert lam.is_cuda and lam.dtype == t.float64 and lam.is_contiguous() and lam.shape[-1] == N_LAMBDA_PARAMS
+        n = lam.shape[0]
+        out = dict(loglike=t.empty(n, dtype=t.float64, device=self.device), grad=t.empty((n, N_LAMBDA_PARAMS), dtype=t.float64, device=self.device),
+                   flags=t.empty(n, dtype=t.int32, device=self.device))
+        chim_loglike_grad_batch(self.h, n, lam, float(rel_step), out["loglike"], out["grad"], out["flags"])
         return out
 
     def stats(self):

@@ -60,6 +60,10 @@ struct chim_ctx {
     int host_nl = 0;
     double* st_lam = nullptr; double* st_ll = nullptr; double* st_ev = nullptr; double* st_xi = nullptr;
     double* st_neff = nullptr; uint32_t* st_fl = nullptr;
+    // chim_loglike_grad_batch: the displaced lambda rows and their results
+    int grad_nl = 0;
+    double* g_lam = nullptr; double* g_ll = nullptr; uint32_t* g_fl = nullptr;
+    std::vector<void*> owned_grad;
     chim_stats last{};
     uint64_t launches = 0;
     // optional per-kernel timing (CUDA events around each launch of the last batch)
@@ -442,6 +446,7 @@ void chim_destroy(chim_ctx* ctx) {
     free_pool(ctx->owned_host);
     free_pool(ctx->owned_ctx);
     free_pool(ctx->owned_grp);
+    free_pool(ctx->owned_grad);
     delete ctx;
 }
 
@@ -922,6 +927,34 @@ int chim_loglike_batch_host(chim_ctx* ctx, int32_t n_lambda, const double* lambd
     if (out_neff) CK(cudaMemcpyAsync(out_neff, ctx->st_neff, sizeof(double) * n_lambda, cudaMemcpyDeviceToHost, st));
     if (out_flags) CK(cudaMemcpyAsync(out_flags, ctx->st_fl, sizeof(uint32_t) * n_lambda, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    return CHIM_OK;
+}
+
+int chim_loglike_grad_batch(chim_ctx* ctx, int32_t n_lambda, const double* lambda, double rel_step, double* out_loglike,
+                            double* out_grad, uint32_t* out_flags) {
+    if (!ctx) return CHIM_EINVAL;
+    if (!ctx->have_events) return fail(ctx, CHIM_ESTATE, "chim_loglike_grad_batch: call chim_init_events first");
+    if (n_lambda < 0 || (n_lambda > 0 && (!lambda || !out_loglike || !out_grad)))
+        return fail(ctx, CHIM_EINVAL, "chim_loglike_grad_batch: null lambda / out_loglike / out_grad or n_lambda < 0");
+    if (!(rel_step > 0.0) || !(rel_step < 0.5)) return fail(ctx, CHIM_EINVAL, "chim_loglike_grad_batch: rel_step must be in (0, 0.5)");
+    if (n_lambda == 0) return CHIM_OK;
+    const int R = grad_rows();
+    if ((long long)n_lambda * R > (1LL << 30)) return fail(ctx, CHIM_EINVAL, "chim_loglike_grad_batch: n_lambda too large");
+    CK(cudaSetDevice(ctx->cfg.device));
+    if (n_lambda > ctx->grad_nl) {
+        cudaStreamSynchronize(ctx->stream);
+        free_pool(ctx->owned_grad);
+        ctx->grad_nl = 0;
+        CK(dev_alloc(ctx->owned_grad, &ctx->g_lam, (size_t)n_lambda * R * CHIM_N_LAMBDA_PARAMS));
+        CK(dev_alloc(ctx->owned_grad, &ctx->g_ll, (size_t)n_lambda * R));
+        CK(dev_alloc(ctx->owned_grad, &ctx->g_fl, (size_t)n_lambda * R));
+        ctx->grad_nl = n_lambda;
+    }
+    CK(launch_grad_expand(lambda, n_lambda, rel_step, ctx->g_lam, ctx->stream));
+    int rc = chim_loglike_batch(ctx, n_lambda * R, ctx->g_lam, ctx->g_ll, nullptr, nullptr, nullptr, ctx->g_fl);
+    if (rc != CHIM_OK) return rc;
+    CK(launch_grad_combine(lambda, n_lambda, rel_step, ctx->g_ll, ctx->g_fl, out_loglike, out_grad, out_flags, ctx->stream));
+    ctx->last.kernel_launches += 2;
     return CHIM_OK;
 }
 

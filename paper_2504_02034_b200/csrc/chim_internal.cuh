@@ -558,6 +558,10 @@ cudaError_t launch_pcat(double Om, int n_los, const int64_t* gal_off, const doub
                         const int64_t* grid_off, const double* zg, double* coef, double* out, cudaStream_t st_);
 cudaError_t launch_pgal(double Om, double zmax, int n_los, const int64_t* compl_off, const double* zc, const double* pc,
                         const int64_t* grid_off, const double* zg, double* out, double* fr_out, cudaStream_t st_);
+cudaError_t launch_grad_expand(const double* lam, int n_lambda, double rel, double* ext, cudaStream_t st);
+cudaError_t launch_grad_combine(const double* lam, int n_lambda, double rel, const double* ll, const uint32_t* fl, double* out_ll,
+                                double* out_grad, uint32_t* out_fl, cudaStream_t st);
+int grad_rows();
 cudaError_t upload_gauss_legendre();   // fills the __constant__ node tables used by S1
 cudaError_t measure_alu_peaks(int n_sm, int reps, cudaStream_t st, double out_g[4]);
 size_t events_smem_bytes(int max_ns, int max_nz);

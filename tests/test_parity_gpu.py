@@ -918,3 +918,52 @@ def test_many1d_sparse_pixels_match_the_oracle(P):
     ref = O.loglike_workload(w3)
     r = _gpu(P, w3, count_pairs=0)
     assert np.isnan(ref["loglike"]).all() and np.isnan(r["loglike"]).all() and np.array_equal(r["flags"], ref["flags"])
+
+
+# ---------------------------------------------------------------- lambda-gradients (NEXT-4)
+@pytest.mark.parametrize("shape", ["tiny", "o5"])
+def test_loglike_gradients_match_the_oracle_differences(P, shape):
+    # chim_loglike_grad_batch (central differences + Richardson through the batched path, on the device) against the same
+    # difference quotients of the fp64 oracle.  Compared in d/dln(lambda) units against the gradient's own scale: rel 1e-3
+    # (a component 1000x below the largest is noise for a sampler's leapfrog step as well)
+    import torch
+    if shape == "tiny":
+        w = make_workload("tiny", n_lambda=2)
+        lams = np.stack([w.lam[0], lambda_vector(H0=64, Om=0.35, Xi0=1.3, n=1.7, alpha=3.1, m_low=5.3, gamma=2.4)])
+    else:
+        w = make_workload("o5_spec", n_events=8, n_lambda=4, n_det=20_000)
+        lams = w.lam[:4].copy()
+    c = P.Context(z_cat_max=w.z_cat_max)
+    c.init_workload(w)
+    out = c.loglike_grad_batch(torch.as_tensor(lams, device=c.device).contiguous(), rel_step=1e-2)
+    torch.cuda.synchronize()
+    ll, g, fl = out["loglike"].cpu().numpy(), out["grad"].cpu().numpy(), out["flags"].cpu().numpy()
+    plain = c.loglike_batch(torch.as_tensor(lams, device=c.device).contiguous())["loglike"].cpu().numpy()
+    c.close()
+    assert np.array_equal(ll, plain) and np.isfinite(g).all()
+    for i, la in enumerate(lams):
+        f0, gr = O.loglike_grad(w, la, rel_step=1e-2)
+        assert abs(ll[i] - f0) < ABS_TOTAL
+        scale = np.max(np.abs(gr * la))
+        err = np.abs((g[i] - gr) * la)
+        assert err.max() < 1e-3 * scale, (i, err / scale, g[i], gr)
+
+
+def test_loglike_gradient_argument_checks_and_undefined_points(P):
+    import torch
+    w = make_workload("tiny", n_events=2, n_samples=100, n_grid=50, n_inj_draw=200)
+    c = P.Context(z_cat_max=w.z_cat_max)
+    lam = torch.as_tensor(w.lam, device="cuda").contiguous()
+    with pytest.raises(P.ChimError) as e:
+        c.loglike_grad_batch(lam)
+    assert e.value.status == -2                                   # before chim_init_events
+    c.init_workload(w)
+    with pytest.raises(P.ChimError):
+        c.loglike_grad_batch(lam, rel_step=0.0)
+    bad = w.lam.copy()
+    bad[0, 1] = 1.5                                               # Om out of domain: log L and its derivatives are NaN, flagged
+    out = c.loglike_grad_batch(torch.as_tensor(bad, device="cuda").contiguous())
+    torch.cuda.synchronize()
+    assert np.isnan(out["loglike"].cpu().numpy()[0]) and np.isnan(out["grad"].cpu().numpy()[0]).all()
+    assert int(out["flags"].cpu().numpy()[0]) & P.CHIM_FLAG_LAMBDA_DOMAIN
+    c.close()
