@@ -507,12 +507,12 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     DlGrid grid = make_dl_grid(xmin, xmax, choose_dl_intervals(ctx, xmin, xmax));
 
     std::vector<float4> rec(2 * NS);
-    // records of the event-local-polynomial sweep: {t, m1d, m2d, ln m1d}, {ln m2d, log2(1/prior) - scale, 0, 0}; every
+    // records of the event-local-polynomial sweep: {m1d, m2d, t, ln m1d}, {ln m2d, log2(1/prior) - scale, 0, 0}; every
     // event padded to a multiple of 32 samples with copies of its last one (whole warps read without bounds checks)
     std::vector<int64_t> poff(n_events + 1, 0);
     for (int i = 0; i < n_events; ++i) poff[i + 1] = poff[i] + ((so[i + 1] - so[i] + 31) / 32) * 32;
     constexpr size_t kRecTail = 1024;   // spare records: the sweeps prefetch one iteration (256 records) past their range
-    std::vector<float4> prec_a((size_t)poff[n_events] + kRecTail, make_float4(0.f, 1.f, 1.f, 0.f));
+    std::vector<float4> prec_a((size_t)poff[n_events] + kRecTail, make_float4(1.f, 1.f, 0.f, 0.f));
     std::vector<float2> prec_b((size_t)poff[n_events] + kRecTail, make_float2(0.f, 0.f));
     std::vector<int32_t> k_lo(n_events), k_hi(n_events);
     const double l2e = 1.4426950408889634074;
@@ -563,7 +563,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
             for (int64_t j = 0; j < np; ++j) {
                 const int64_t js = s0 + std::min<int64_t>(j, ns - 1), o = s0 + idx[std::min<int64_t>(j, ns - 1)];
                 const double t = ((double)f_bits(rec[2 * js].x) - (double)tkq_c[i]) / (half * fq);
-                prec_a[p0 + j] = make_float4((float)t, (float)h_m1[o], (float)h_m2[o], (float)std::log(h_m1[o]));
+                prec_a[p0 + j] = make_float4((float)h_m1[o], (float)h_m2[o], (float)t, (float)std::log(h_m1[o]));
                 prec_b[p0 + j] = make_float2((float)std::log(h_m2[o]), rec[2 * js + 1].w);
             }
         }
@@ -800,7 +800,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
     }
     // chunk-local polynomials of k_inject: the set is sorted in d_L, so a chunk of kInjChunk injections spans a narrow range
     const int n_chunks = (int)((n_det + kInjChunk - 1) / kInjChunk);
-    std::vector<float4> prec_a((size_t)n_chunks * kInjChunk + 2048, make_float4(0.f, 1.f, 1.f, 0.f));   // + spare tail (prefetch)
+    std::vector<float4> prec_a((size_t)n_chunks * kInjChunk + 2048, make_float4(1.f, 1.f, 0.f, 0.f));   // + spare tail (prefetch)
     std::vector<float2> prec_b((size_t)n_chunks * kInjChunk + 2048, make_float2(0.f, 0.f));
     std::vector<double> ctk_c(n_chunks), ctk_h(n_chunks);
     std::vector<float> blk_m2d((size_t)n_chunks * (kInjChunk / 256), INFINITY);
@@ -836,7 +836,7 @@ int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, cons
         for (size_t j = a; j < a + kInjChunk; ++j) {
             const size_t js = std::min(j, b - 1), o = (size_t)idx[js];
             const double t = (tk_of(js) - ctk_c[c]) / half;
-            prec_a[j] = make_float4((float)t, (float)h_m1[o], (float)h_m2[o], (float)std::log(h_m1[o]));
+            prec_a[j] = make_float4((float)h_m1[o], (float)h_m2[o], (float)t, (float)std::log(h_m1[o]));
             prec_b[j] = make_float2((float)std::log(h_m2[o]), rec[2 * js + 1].z);
         }
     }

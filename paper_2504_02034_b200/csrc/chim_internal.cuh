@@ -151,7 +151,8 @@ __device__ __forceinline__ double ex2_to_double(float y) {
     return (y > -1000.f) ? v : 0.0;
 }
 
-// Records of the local-polynomial sweeps, split for 24 B per sample: A = {t, m1d, m2d, ln m1d}, B = {ln m2d, log2(1/prior)}
+// Records of the local-polynomial sweeps, split for 24 B per sample: A = {m1d, m2d, t, ln m1d}, B = {ln m2d, log2(1/prior)}
+// (the masses first: they enter one packed FMA, and a 128-bit load fills aligned register pairs)
 struct PRec { float4 A; float2 B; };
 __device__ __forceinline__ PRec ldg_stream_prec(const float4* pa, const float2* pb) {   // streaming reads (once per CTA)
     PRec r;
@@ -167,6 +168,23 @@ struct MassLookup {
     const MassRow* s;          // staged rows or null
     int lo, cap, n_mass;
 };
+
+// The two halves separately, for the doubly prefetched sweeps (k_events_fast, k_inject).  Half A is first touched at the top of
+// a sample and dead after its polynomials, so its next load may move up into the sample; half B enters a sample's last two
+// operations (poly_sample), and `after` (any value computed from them) pins the load of the NEXT B behind them -- otherwise the
+// compiler issues it early into a second register pair and copies it over later, and that copy waits for the load.
+__device__ __forceinline__ float4 ldg_stream_a(const float4* pa) {
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(pa));
+    return r;
+}
+__device__ __forceinline__ void ldg_stream_b(float2& r, const float2* pb, float after) {
+    // (predicated on `after` being a number or +-inf -- a true dependency the assembler cannot remove; a NaN weight leaves the
+    // previous values in place, and its unit is not-a-number anyway)
+    asm volatile("{\n .reg .pred p;\n setp.le.f32 p, %3, 0f7F800000;\n @p ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];\n}"
+                 : "+f"(r.x), "+f"(r.y)
+                 : "l"(pb), "f"(after));
+}
 
 struct Rec { float4 A, B; };   // one packed record (32 B, 32-byte aligned)
 __device__ __forceinline__ Rec ldg_stream_rec(const float4* p) {   // streaming 256-bit read (read once per CTA)
@@ -320,14 +338,14 @@ __device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restri
 }
 
 // Steps S2 / S5 for one sample with the local polynomials: the same quantities as sample_eval.  Record
-// A = {t, m1d, m2d, ln m1d}, B = {ln m2d, log2(1/prior or 1/p_draw) - scale, .., ..}:
+// A = {m1d, m2d, t, ln m1d}, B = {ln m2d, log2(1/prior or 1/p_draw) - scale, .., ..}:
 //   m' = m^d a - m_low;  log2 w = LQ2(ln m1) + beta2 ln m2^d + r + B.y - 2 log2 m1' - log2(1 + 2^(gk2 u - cpsi)) - log2(1 + e^f(m2'))
 // PAPER.md:52, :195-198 eq. 20, :226 eq. 21, :75 eq. 11.  Warp-collective like sample_eval.
 template <bool kFit, bool kTurn = true>
 __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, const float cpsi, const PolyCoef& C, const float4 A,
                                             const float2 Bq, const MassLookup& M, const float tm_lo, const float tm_hi,
                                             float& zc, float& l2w, float& mp2) {
-    const f32x2 t2 = pack2(A.x, A.x);
+    const f32x2 t2 = pack2(A.z, A.z);
     f32x2 zr = C.zr[6], ua = C.ua[5];
 #pragma unroll
     for (int n = 5; n >= 0; --n) zr = fma2(zr, t2, C.zr[n]);
@@ -336,7 +354,7 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
     float r, u, a, mp1;
     unpack2(zr, zc, r);
     unpack2(ua, u, a);
-    unpack2(fma2(pack2(A.y, A.z), pack2(a, a), pack2(-F.mlow_hi, -F.mlow_hi)), mp1, mp2);   // m' = m^d a - m_low
+    unpack2(fma2(pack2(A.x, A.y), pack2(a, a), pack2(-F.mlow_hi, -F.mlow_hi)), mp1, mp2);   // m' = m^d a - m_low
     const float lm1 = A.w - u;
     float tm = fmaf(lm1, F.tm_scale, F.mlow_tm);
     tm = fminf(fmaxf(tm, tm_lo), tm_hi);
@@ -355,8 +373,7 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
             if (!staged) c = __ldg(M.g + km + (gauss_only ? M.n_mass + 2 : 0));
         }
     }
-    float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x);
-    l += fmaf(F.beta2, Bq.x, r + Bq.y);
+    float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x) + r;
     l = fmaf(-2.f, lg2f(mp1), l);            // m1' <= 0 implies m2' <= 0: discarded below
     if (kTurn) l -= lg2f(1.0f + ex2f(fmaf(gk2, u, -cpsi)));   // overflow -> l = -inf, the limit (psi -> 0).  !kTurn: the turnover is part of r
     if (__any_sync(0xffffffffu, mp2 < F.delta)) {
@@ -365,6 +382,9 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
         const float ls = (f2 > 64.f) ? f2 : lg2f(1.0f + ex2f(f2));   // deep in the window 2^f2 overflows; log2(1 + 2^f) = f there
         l -= (mp2 < F.delta) ? ls : 0.f;
     }
+    // the B half of the record enters last (both terms depend on everything above): a streamed record is first touched as late
+    // as possible, which is what the prefetch distance of the sweeps is measured against
+    l = fmaf(F.beta2, Bq.x, l) + Bq.y;
     l2w = (mp2 > 0.f) ? l : -INFINITY;      // R15 support: m_low < m2
 }
 template <bool kFit>
@@ -453,7 +473,7 @@ struct EventSetDev {
     const double* tk_c;         // [n_events]
     const double* tk_h;         // [n_events]
     const int64_t* poly_off;    // [n_events+1] offsets into prec (events padded to a multiple of 32 samples)
-    const float4* prec_a;       // records of the polynomial sweep: {t in [-1,1], m1d, m2d, ln m1d}
+    const float4* prec_a;       // records of the polynomial sweep: {m1d, m2d, t in [-1,1], ln m1d}
     const float2* prec_b;       //                                  {ln m2d, log2(1/prior) - scale}
     // k_events_fast: qn again with every event's slice starting at a multiple of 4 floats and zero-padded to one (TMA source)
     const float* qn4;
@@ -506,7 +526,7 @@ struct InjSetDev {
     double n_inj_total;
     const float4* rec;       // packed injection records {A, B}, sorted by d_L
     const int64_t* perm;
-    // chunk-local polynomials (k_inject): records {t, m1d, m2d, ln m1d}, {ln m2d, log2(1/p_draw) - scale} padded to
+    // chunk-local polynomials (k_inject): records {m1d, m2d, t, ln m1d}, {ln m2d, log2(1/p_draw) - scale} padded to
     // whole chunks, centre / half-width of each chunk in table coordinates (tk_h = 0: range too wide -> table path)
     const float4* prec_a;
     const float2* prec_b;

@@ -602,8 +602,8 @@ __device__ __forceinline__ void events_unit(const EventKernelParams& P, const in
                 const float4 Ad = __ldg(P.ev.prec_a + p0 + jd);
                 float ad = S.poly[2 * kPolyN + 2 * (kPolyN - 2) + 1];
 #pragma unroll
-                for (int n = kPolyN - 3; n >= 0; --n) ad = fmaf(ad, Ad.x, S.poly[2 * kPolyN + 2 * n + 1]);
-                const float mp2d = fmaf(Ad.z, ad, -L.F.mlow_hi);
+                for (int n = kPolyN - 3; n >= 0; --n) ad = fmaf(ad, Ad.z, S.poly[2 * kPolyN + 2 * n + 1]);
+                const float mp2d = fmaf(Ad.y, ad, -L.F.mlow_hi);
                 // fp32 leaves ~1e-6 (random) + ~5e-7 (the fit, common to all samples) in m2': d ln w = delta/m2'^2 of that.  The
                 // careful sweep is taken where this would show in log I: few effective samples (n_eff < neff_min), or all of them deep
                 const double neff = (1.0 + S.mom[0]) * (1.0 + S.mom[0]) / (1.0 + S.mom[1]);

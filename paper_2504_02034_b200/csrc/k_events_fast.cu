@@ -129,6 +129,18 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     }
     LamF F;
     load_lamf_hot(F, &Lg->F);
+    // the warp's chunk [c0, c1) of the (d_L-sorted) samples; its first two blocks of records are requested here, ahead of the
+    // barrier and of the wait for the mass rows
+    const int C = fast_chunk(ns);
+    const int c0 = wid * C, c1 = min(c0 + C, ns);
+    const float4* pa = P.ev.prec_a + P.ev.poly_off[ev];
+    const float2* pb = P.ev.prec_b + P.ev.poly_off[ev];
+    PRec R0, R1;
+    {
+        const int jf = min(c0, ns - 1) + lane;                          // (warps beyond the event read its last block and drop it)
+        R0 = ldg_stream_prec(pa + jf, pb + jf);
+        R1 = ldg_stream_prec(pa + jf + 32, pb + jf + 32);
+    }
     __syncthreads();                                                    // (1) the barriers are initialised
     MassLookup M;
     M.g = mtab;
@@ -138,20 +150,16 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     M.n_mass = P.n_mass;
     const float tm_lo = fmaxf(1.0f, (float)mlo), tm_hi = fminf(F.tm_max, (float)(mlo + nr) - 0.01f);
 
-    // ---- S2 on the warp's chunk [c0, c1): (z_j - z0, log2 w_j) pairs to shared memory, then w_j relative to the chunk's largest ---------
-    const int C = fast_chunk(ns);
-    const int c0 = wid * C, c1 = min(c0 + C, ns);
-    const int64_t p0 = P.ev.poly_off[ev];
+    // ---- S2 on the warp's chunk: (z_j - z0, log2 w_j) pairs to shared memory, then w_j relative to the chunk's largest ----------------
     float mx = -INFINITY, mp2x = -INFINITY;
     mbar_wait(&S.mbar_mass, 0);
     if (c0 < ns) {
-        const float4* pa = P.ev.prec_a + p0;
-        const float2* pb = P.ev.prec_b + p0;
         const int nfull = c0 + ((c1 - c0) & ~31);                       // end of the whole blocks of 32 samples
         int j = c0 + lane;
+        float l2w_;
 #define CHIM_FAST_SAMPLE(REC, JJ, STORE)                                                                          \
         {                                                                                                         \
-            float zc_, l2w_, mp2_;                                                                                \
+            float zc_, mp2_;                                                                                      \
             poly_sample<true>(F, F.gk2, F.cpsi, Cf, (REC).A, (REC).B, M, tm_lo, tm_hi, zc_, l2w_, mp2_);          \
             if (STORE) {                                                                                          \
                 zw[JJ] = make_float2(zc_, l2w_);                                                                  \
@@ -160,14 +168,16 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
             }                                                                                                     \
         }
         // the records are streamed two blocks ahead (one doubled iteration ~ 140 instructions x 6 warps per scheduler: the L2
-        // latency); the record arrays carry a spare tail, so the loads are unconditional
-        PRec R0 = ldg_stream_prec(pa + j, pb + j), R1 = ldg_stream_prec(pa + j + 32, pb + j + 32);
+        // latency); the record arrays carry a spare tail, so the loads are unconditional.  Half A may be requested as soon as the
+        // sample's polynomials are done, half B only behind its use at the very end of the sample (ldg_stream_b)
 #pragma unroll 1
         for (; j + 32 < nfull; j += 64) {
             CHIM_FAST_SAMPLE(R0, j, true)
-            R0 = ldg_stream_prec(pa + j + 64, pb + j + 64);
+            R0.A = ldg_stream_a(pa + j + 64);
+            ldg_stream_b(R0.B, pb + j + 64, l2w_);
             CHIM_FAST_SAMPLE(R1, j + 32, true)
-            R1 = ldg_stream_prec(pa + j + 96, pb + j + 96);
+            R1.A = ldg_stream_a(pa + j + 96);
+            ldg_stream_b(R1.B, pb + j + 96, l2w_);
         }
         if (j < nfull) {
             CHIM_FAST_SAMPLE(R0, j, true)

@@ -124,22 +124,26 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
         }
 #define CHIM_INJ_SAMPLE(TURN, REC, JJ)                                                                                \
         {                                                                                                             \
-            float zc, l2w, mp2_;                                                                                      \
+            float zc, mp2_;                                                                                           \
             poly_sample<true, TURN>(F, F.gk2_inj, F.cpsi_inj, C, (REC).A, (REC).B, M, 1.0f, tm_hi, zc, l2w, mp2_);    \
             const double s = (zc <= 0.f && (JJ) < n) ? ex2_to_double(l2w) : 0.0;                                      \
             acc[0] += s;                                                                                              \
             acc[1] = fma(s, s, acc[1]);                                                                               \
             if (kDbg && (JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale;                                   \
         }
+        // records two blocks ahead; half B of a record is requested behind its use at the end of the sample (ldg_stream_b)
 #define CHIM_INJ_SWEEP(TURN)                                                                                          \
         {                                                                                                             \
             int j = tid + k0 * kInjThreads;                                                                           \
+            float l2w;                                                                                                \
             PRec R0 = ldg_stream_prec(pa + j, pb + j), R1 = ldg_stream_prec(pa + j + kInjThreads, pb + j + kInjThreads); \
             _Pragma("unroll 1") for (; j + kInjThreads < n32; j += 2 * kInjThreads) {                                 \
                 CHIM_INJ_SAMPLE(TURN, R0, j)                                                                          \
-                R0 = ldg_stream_prec(pa + j + 2 * kInjThreads, pb + j + 2 * kInjThreads);                             \
+                R0.A = ldg_stream_a(pa + j + 2 * kInjThreads);                                                        \
+                ldg_stream_b(R0.B, pb + j + 2 * kInjThreads, l2w);                                                    \
                 CHIM_INJ_SAMPLE(TURN, R1, j + kInjThreads)                                                            \
-                R1 = ldg_stream_prec(pa + j + 3 * kInjThreads, pb + j + 3 * kInjThreads);                             \
+                R1.A = ldg_stream_a(pa + j + 3 * kInjThreads);                                                        \
+                ldg_stream_b(R1.B, pb + j + 3 * kInjThreads, l2w);                                                    \
             }                                                                                                         \
             if (j < n32) CHIM_INJ_SAMPLE(TURN, R0, j)                                                                 \
         }
