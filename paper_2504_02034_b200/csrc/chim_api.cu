@@ -521,6 +521,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     std::vector<float> qn(NG);
     std::vector<double> ep0(NG + n_events), ep1(NG + n_events), ep2(NG + n_events);   // Epanechnikov prefix sums
     std::vector<double> lm_lo(n_events), lm_hi(n_events);
+    std::vector<float2> chunk_top((size_t)n_events * kFastWarps, make_float2(0.f, 1.f));   // k_events_fast: per chunk {largest m2d, t of its last sample}
     std::vector<double> tk_c(n_events), tk_h(n_events);
     std::vector<uint32_t> tkq_c(n_events);
     std::vector<float> tq_scale(n_events);   // (host-side intermediates of the polynomial coordinate)
@@ -564,6 +565,11 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
                 const int64_t js = s0 + std::min<int64_t>(j, ns - 1), o = s0 + idx[std::min<int64_t>(j, ns - 1)];
                 const double t = ((double)f_bits(rec[2 * js].x) - (double)tkq_c[i]) / (half * fq);
                 prec_a[p0 + j] = make_float4((float)h_m1[o], (float)h_m2[o], (float)t, (float)std::log(h_m1[o]));
+                if (j < ns) {
+                    float2& ct = chunk_top[(size_t)i * kFastWarps + std::min<int64_t>(j / fast_chunk((int)ns), kFastWarps - 1)];
+                    ct.x = std::max(ct.x, (float)h_m2[o]);
+                    ct.y = (float)t;                                   // (samples in d_L order: the last one written is the chunk's last)
+                }
                 prec_b[p0 + j] = make_float2((float)std::log(h_m2[o]), rec[2 * js + 1].w);
             }
         }
@@ -626,7 +632,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     CK(upload(ctx->owned_ev, &E.perm, perm)); CK(upload(ctx->owned_ev, &E.zc, zc)); CK(upload(ctx->owned_ev, &E.qn, qn));
     CK(upload(ctx->owned_ev, &E.uni_dz, udz)); CK(upload(ctx->owned_ev, &E.max_dz, maxdz));
     CK(upload(ctx->owned_ev, &E.ep_q0, ep0)); CK(upload(ctx->owned_ev, &E.ep_q1, ep1)); CK(upload(ctx->owned_ev, &E.ep_q2, ep2));
-    CK(upload(ctx->owned_ev, &E.lnm1_lo, lm_lo)); CK(upload(ctx->owned_ev, &E.lnm1_hi, lm_hi));
+    CK(upload(ctx->owned_ev, &E.lnm1_lo, lm_lo)); CK(upload(ctx->owned_ev, &E.lnm1_hi, lm_hi)); CK(upload(ctx->owned_ev, &E.chunk_top, chunk_top));
     CK(upload(ctx->owned_ev, &E.z0, z0));
     CK(upload(ctx->owned_ev, &E.tk_c, tk_c)); CK(upload(ctx->owned_ev, &E.tk_h, tk_h));
     CK(upload(ctx->owned_ev, &E.poly_off, poff)); CK(upload(ctx->owned_ev, &E.prec_a, prec_a)); CK(upload(ctx->owned_ev, &E.prec_b, prec_b));

@@ -341,10 +341,10 @@ __device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restri
 // A = {m1d, m2d, t, ln m1d}, B = {ln m2d, log2(1/prior or 1/p_draw) - scale, .., ..}:
 //   m' = m^d a - m_low;  log2 w = LQ2(ln m1) + beta2 ln m2^d + r + B.y - 2 log2 m1' - log2(1 + 2^(gk2 u - cpsi)) - log2(1 + e^f(m2'))
 // PAPER.md:52, :195-198 eq. 20, :226 eq. 21, :75 eq. 11.  Warp-collective like sample_eval.
-template <bool kFit, bool kTurn = true>
+template <bool kFit, bool kTurn = true, bool kWinS = false>
 __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, const float cpsi, const PolyCoef& C, const float4 A,
                                             const float2 Bq, const MassLookup& M, const float tm_lo, const float tm_hi,
-                                            float& zc, float& l2w, float& mp2) {
+                                            float& zc, float& l2w, float& mp2, const float4* __restrict__ win_s = nullptr) {
     const f32x2 t2 = pack2(A.z, A.z);
     f32x2 zr = C.zr[6], ua = C.ua[5];
 #pragma unroll
@@ -377,8 +377,10 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
     l = fmaf(-2.f, lg2f(mp1), l);            // m1' <= 0 implies m2' <= 0: discarded below
     if (kTurn) l -= lg2f(1.0f + ex2f(fmaf(gk2, u, -cpsi)));   // overflow -> l = -inf, the limit (psi -> 0).  !kTurn: the turnover is part of r
     if (__any_sync(0xffffffffu, mp2 < F.delta)) {
-        const float mc = fminf(fmaxf(mp2, F.win_lo), F.win_hi);
-        const float f2 = fmaf(F.two_dl2e, mc, -F.d2l2e) * rcpf(mc * (mc - F.delta));
+        // (kWinS: the four window constants {win_lo, win_hi, two_dl2e, d2l2e} from shared memory instead of registers)
+        const float4 wc = kWinS ? *win_s : make_float4(F.win_lo, F.win_hi, F.two_dl2e, F.d2l2e);
+        const float mc = fminf(fmaxf(mp2, wc.x), wc.y);
+        const float f2 = fmaf(wc.z, mc, -wc.w) * rcpf(mc * (mc - F.delta));
         const float ls = (f2 > 64.f) ? f2 : lg2f(1.0f + ex2f(f2));   // deep in the window 2^f2 overflows; log2(1 + 2^f) = f there
         l -= (mp2 < F.delta) ? ls : 0.f;
     }
@@ -394,6 +396,11 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
     float mp2;
     poly_sample<kFit>(F, gk2, cpsi, C, A, Bq, M, tm_lo, tm_hi, zc, l2w, mp2);
 }
+
+// k_events_fast: eight warps, each on a contiguous chunk of the event's (d_L-sorted) samples; chunks are whole passes of 128
+constexpr int kFastWarps = 8;
+constexpr int kFastPass = 128;
+__host__ __device__ inline int fast_chunk(int ns) { return ((ns + kFastWarps * kFastPass - 1) / (kFastWarps * kFastPass)) * kFastPass; }
 
 // ---- TMA bulk copy + mbarrier  ---------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -462,6 +469,7 @@ struct EventSetDev {
     const double* z0;           // [n_events] centre of each event's grid
     const double* lnm1_lo;      // [n_events] smallest / largest ln m1d of the event's samples
     const double* lnm1_hi;
+    const float2* chunk_top;    // [n_events][kFastWarps] k_events_fast: {largest m2d, t of the last sample} of every warp's chunk
     const int32_t* k_lo;        // [n_events] first / last row of the z(ln d_L) table the event's samples address
     const int32_t* k_hi;
     const double* fixed_bw;     // [n_events] or null

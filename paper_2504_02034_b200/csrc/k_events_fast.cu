@@ -23,9 +23,9 @@ namespace chim {
 #ifndef CHIM_FAST_BLOCKS
 #define CHIM_FAST_BLOCKS 3
 #endif
-constexpr int kFT = 256;             // threads per CTA
-constexpr int kFW = kFT / 32;        // warps = sample chunks
-constexpr int kFPass = 128;          // samples per warp pass (4 per lane)
+constexpr int kFT = 32 * kFastWarps;  // threads per CTA
+constexpr int kFW = kFastWarps;      // warps = sample chunks
+constexpr int kFPass = kFastPass;    // samples per warp pass (4 per lane)
 constexpr int kFLeP = 12;            // terms of the local expansion
 constexpr int kFMaxBox = 96;         // boxes per event
 constexpr int kFBoxPerWarp = kFMaxBox / kFW;
@@ -36,15 +36,14 @@ constexpr int kFMassStage = 384;     // mass-table rows staged per variant (>= e
 
 struct FastSmem {
     unsigned long long mbar_mass, mbar_q;
-    float c_mx[kFW], c_zr[kFW];      // per chunk: largest log2 w; z - z0 of the chunk's first sample (reference of its moments)
-    float c_mp2[kFW];                // per chunk: largest m2' = m2 - m_low among its samples
-    float c_mom[kFW][4];             // sum w, sum w^2, sum w u, sum w u^2 with w relative to the chunk's largest, u = z - c_zr
-    float c_f[kFW];                  // 2^(chunk max - event max): chunk-relative weights -> relative to the event's largest
+    float4 win;                      // the window constants of S(m2) {win_lo, win_hi, two_dl2e, d2l2e} (read inside the vote only)
+    float c_ref[kFW];                // per chunk: the reference log2 w of its weights (-inf: no weighted sample)
+    float c_mom[kFW][4];             // sum w, sum w^2, sum w u, sum w u^2 with w relative to c_ref, u = z - z_mid
+    float c_f[kFW];                  // 2^(c_ref - largest c_ref): chunk-relative weights -> one scale for the event
     double c_sum[kFW];               // per warp: sum_j w_j A_j over its boxes, relative to the event's largest weight
     int bnd[kFMaxBox + 1];           // first sample of every box (samples are sorted)
 };
 
-__host__ __device__ inline int fast_chunk(int ns) { return ((ns + kFW * kFPass - 1) / (kFW * kFPass)) * kFPass; }
 __host__ __device__ inline size_t fast_nz4(size_t nz) { return (nz + 3) / 4 * 4; }
 __host__ __device__ inline size_t fast_aux_bytes() {
     const size_t a = 2 * (size_t)kFMassStage * sizeof(MassRow);
@@ -129,6 +128,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     }
     LamF F;
     load_lamf_hot(F, &Lg->F);
+    if (tid == 0) S.win = make_float4(F.win_lo, F.win_hi, F.two_dl2e, F.d2l2e);
     // the warp's chunk [c0, c1) of the (d_L-sorted) samples; its first two blocks of records are requested here, ahead of the
     // barrier and of the wait for the mass rows
     const int C = fast_chunk(ns);
@@ -150,74 +150,75 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     M.n_mass = P.n_mass;
     const float tm_lo = fmaxf(1.0f, (float)mlo), tm_hi = fminf(F.tm_max, (float)(mlo + nr) - 0.01f);
 
-    // ---- S2 on the warp's chunk: (z_j - z0, log2 w_j) pairs to shared memory, then w_j relative to the chunk's largest ----------------
-    float mx = -INFINITY, mp2x = -INFINITY;
+    // ---- S2 on the warp's chunk, one sweep: (z_j - z0, w_j) pairs to shared memory and the chunk's moments ---------------------------
+    // w_j = 2^(log2 w_j - ref), ref = the largest log2 w of the first block of the chunk that has a weighted sample (any reference
+    // within ~2^100 of the chunk's largest weight serves; one that is not shows up as inf/NaN moments and the unit is handed over).
+    // Moments about z_mid = z at the centre of the event's d_L range (the constant term of the z polynomial): sums of positive
+    // terms; the variance is taken about the weighted mean afterwards.
+    float ref = 0.f;
+    bool ref_unset = true;
+    float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;
+    float zmid, r0_unused;
+    unpack2(Cf.zr[0], zmid, r0_unused);
     mbar_wait(&S.mbar_mass, 0);
     if (c0 < ns) {
-        const int nfull = c0 + ((c1 - c0) & ~31);                       // end of the whole blocks of 32 samples
-        int j = c0 + lane;
+        // running pointers (records, results) and a block count instead of an index: fewer live registers in the loop
+        int nblk = (c1 - c0) >> 5;                                      // whole blocks of 32 samples
+        const bool ragged = ((c1 - c0) & 31) != 0;
+        const float4* pa_t = pa + c0 + lane;
+        const float2* pb_t = pb + c0 + lane;
+        float2* zw_t = zw + c0 + lane;
         float l2w_;
-#define CHIM_FAST_SAMPLE(REC, JJ, STORE)                                                                          \
+#define CHIM_FAST_SAMPLE(REC, OFF, IN, SEARCH)                                                                    \
         {                                                                                                         \
             float zc_, mp2_;                                                                                      \
-            poly_sample<true>(F, F.gk2, F.cpsi, Cf, (REC).A, (REC).B, M, tm_lo, tm_hi, zc_, l2w_, mp2_);          \
-            if (STORE) {                                                                                          \
-                zw[JJ] = make_float2(zc_, l2w_);                                                                  \
-                mx = fmaxf(mx, l2w_);                                                                             \
-                mp2x = fmaxf(mp2x, mp2_);                                                                         \
+            poly_sample<true, true, true>(F, F.gk2, F.cpsi, Cf, (REC).A, (REC).B, M, tm_lo, tm_hi, zc_, l2w_, mp2_, &S.win); \
+            const float lw_ = (IN) ? l2w_ : -INFINITY;                                                            \
+            if ((SEARCH) && ref_unset) {   /* (warp-uniform) */                                                   \
+                float b_ = lw_;                                                                                   \
+                _Pragma("unroll") for (int o = 16; o > 0; o >>= 1) b_ = fmaxf(b_, __shfl_xor_sync(0xffffffffu, b_, o)); \
+                if (b_ > -INFINITY) {                                                                             \
+                    ref = b_;                                                                                     \
+                    ref_unset = false;                                                                            \
+                }                                                                                                 \
             }                                                                                                     \
+            const float w_ = ex2f(lw_ - ref), u_ = zc_ - zmid, wu_ = w_ * u_;                                     \
+            m0 += w_;                                                                                             \
+            m1 = fmaf(w_, w_, m1);                                                                                \
+            m2 += wu_;                                                                                            \
+            m3 = fmaf(wu_, u_, m3);                                                                               \
+            zw_t[OFF] = make_float2(zc_, w_);                                                                     \
         }
-        // the records are streamed two blocks ahead (one doubled iteration ~ 140 instructions x 6 warps per scheduler: the L2
+#define CHIM_FAST_PAIR(SEARCH)                                                                                    \
+        {                                                                                                         \
+            CHIM_FAST_SAMPLE(R0, 0, true, SEARCH)                                                                 \
+            R0.A = ldg_stream_a(pa_t + 64);                                                                       \
+            ldg_stream_b(R0.B, pb_t + 64, l2w_);                                                                  \
+            CHIM_FAST_SAMPLE(R1, 32, true, SEARCH)                                                                \
+            R1.A = ldg_stream_a(pa_t + 96);                                                                       \
+            ldg_stream_b(R1.B, pb_t + 96, l2w_);                                                                  \
+            pa_t += 64;                                                                                           \
+            pb_t += 64;                                                                                           \
+            zw_t += 64;                                                                                           \
+        }
+        // the records are streamed two blocks ahead (one doubled iteration ~ 160 instructions x 6 warps per scheduler: the L2
         // latency); the record arrays carry a spare tail, so the loads are unconditional.  Half A may be requested as soon as the
-        // sample's polynomials are done, half B only behind its use at the very end of the sample (ldg_stream_b)
+        // sample's polynomials are done, half B only behind its use at the very end of the sample (ldg_stream_b).  The first loop
+        // runs until the chunk's reference is set (normally one iteration), the second is the plain one.
 #pragma unroll 1
-        for (; j + 32 < nfull; j += 64) {
-            CHIM_FAST_SAMPLE(R0, j, true)
-            R0.A = ldg_stream_a(pa + j + 64);
-            ldg_stream_b(R0.B, pb + j + 64, l2w_);
-            CHIM_FAST_SAMPLE(R1, j + 32, true)
-            R1.A = ldg_stream_a(pa + j + 96);
-            ldg_stream_b(R1.B, pb + j + 96, l2w_);
-        }
-        if (j < nfull) {
-            CHIM_FAST_SAMPLE(R0, j, true)
-            j += 32;
+        for (; nblk >= 2 && ref_unset; nblk -= 2) CHIM_FAST_PAIR(true)
+#pragma unroll 1
+        for (; nblk >= 2; nblk -= 2) CHIM_FAST_PAIR(false)
+        if (nblk) {
+            CHIM_FAST_SAMPLE(R0, 0, true, true)
+            zw_t += 32;
             R0 = R1;
         }
-        if (nfull < c1) CHIM_FAST_SAMPLE(R0, j, j < c1)   // the ragged end of the event (records padded to whole warps: poly_sample votes)
+        // the ragged end of the event (records padded to whole warps with copies of the last sample: poly_sample votes); the lanes
+        // beyond it store that sample's redshift with weight 0 -- S3 reads the pair of the last sample unmasked
+        if (ragged) CHIM_FAST_SAMPLE(R0, 0, (int)(zw_t - zw) < c1, true)
+#undef CHIM_FAST_PAIR
 #undef CHIM_FAST_SAMPLE
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-            mp2x = fmaxf(mp2x, __shfl_xor_sync(0xffffffffu, mp2x, o));
-        }
-        __syncwarp();
-        // sweep 2: w = 2^(log2 w - chunk max); plain weighted moments about the chunk's first sample (the cancellation-free form of
-        // R21 is only needed near n_eff = 1, and such units are handed over); idle slots of the last pass sit on the chunk's last
-        // sample with weight 0
-        const float mref = (mx > -INFINITY) ? mx : 0.f, zr = zw[c0].x, zlast = zw[c1 - 1].x;
-        float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f;
-        const int pend = c0 + ((c1 - c0 + kFPass - 1) / kFPass) * kFPass;
-        for (int jb = c0 + 2 * lane; jb < pend; jb += kFPass) {         // lane: samples jb, jb + 1, jb + 64, jb + 65 (16-byte lane stride)
-            const float4 ab = *reinterpret_cast<const float4*>(zw + jb), cd4 = *reinterpret_cast<const float4*>(zw + jb + 64);
-            float zv[4] = {ab.x, ab.z, cd4.x, cd4.z};
-            const float lv[4] = {ab.y, ab.w, cd4.y, cd4.w};
-            float wv[4];
-#pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const bool valid = jb + (r & 1) + 64 * (r >> 1) < c1;
-                const float w = valid ? ex2f(lv[r] - mref) : 0.f;
-                zv[r] = valid ? zv[r] : zlast;
-                wv[r] = w;
-                const float u = zv[r] - zr, wu = w * u;
-                m0 += w;
-                m1 = fmaf(w, w, m1);
-                m2 += wu;
-                m3 = fmaf(wu, u, m3);
-            }
-            *reinterpret_cast<float4*>(zw + jb) = make_float4(zv[0], wv[0], zv[1], wv[1]);
-            *reinterpret_cast<float4*>(zw + jb + 64) = make_float4(zv[2], wv[2], zv[3], wv[3]);
-        }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             m0 += __shfl_xor_sync(0xffffffffu, m0, o);
@@ -226,11 +227,11 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
             m3 += __shfl_xor_sync(0xffffffffu, m3, o);
         }
         if (lane == 0) {
-            S.c_mx[wid] = mx; S.c_zr[wid] = zr; S.c_mp2[wid] = mp2x;
+            S.c_ref[wid] = ref_unset ? -INFINITY : ref;
             S.c_mom[wid][0] = m0; S.c_mom[wid][1] = m1; S.c_mom[wid][2] = m2; S.c_mom[wid][3] = m3;
         }
     } else if (lane == 0) {
-        S.c_mx[wid] = -INFINITY; S.c_zr[wid] = 0.f; S.c_mp2[wid] = -INFINITY;
+        S.c_ref[wid] = -INFINITY;
         S.c_mom[wid][0] = 0.f; S.c_mom[wid][1] = 0.f; S.c_mom[wid][2] = 0.f; S.c_mom[wid][3] = 0.f;
     }
     __syncthreads();                                                    // (2) chunk statistics and the samples are complete
@@ -238,24 +239,19 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     // ---- every warp: the event's moments from the eight chunks (lane c takes chunk c), bandwidth, expansion geometry -------------
     // fp32 throughout: all sums are sums of positive terms (the second moment is taken about the weighted mean in a second
     // step), n_eff >= neff_min (64; 24 for many-1d pixels) on this path, and dh/h = 1e-6 moves log I by ~5e-9
-    const float cm = (lane < kFW) ? S.c_mx[lane] : -INFINITY;
-    float gmx = cm, gmp2 = (lane < kFW) ? S.c_mp2[lane] : -INFINITY;
+    const float cm = (lane < kFW) ? S.c_ref[lane] : -INFINITY;
+    float gref = cm;
 #pragma unroll
-    for (int o = 4; o > 0; o >>= 1) {
-        gmx = fmaxf(gmx, __shfl_xor_sync(0xffffffffu, gmx, o));
-        gmp2 = fmaxf(gmp2, __shfl_xor_sync(0xffffffffu, gmp2, o));
-    }
-    gmx = __shfl_sync(0xffffffffu, gmx, 0);
-    gmp2 = __shfl_sync(0xffffffffu, gmp2, 0);
+    for (int o = 4; o > 0; o >>= 1) gref = fmaxf(gref, __shfl_xor_sync(0xffffffffu, gref, o));
+    gref = __shfl_sync(0xffffffffu, gref, 0);
     mbar_wait(&S.mbar_q, 0);                                            // q_g has landed (also: no copy in flight at any exit below)
-    if (!(gmx > -INFINITY) || gmx != gmx) CHIM_FAST_HANDOVER();         // no weighted sample on this path: k_events decides
+    if (!(gref > -INFINITY)) CHIM_FAST_HANDOVER();                      // no weighted sample on this path: k_events decides
     const bool live = lane < kFW && cm > -INFINITY;
-    const float f = live ? ex2f(cm - gmx) : 0.f;                        // chunk-relative weights -> relative to the event's largest
-    const float dl = live ? S.c_zr[lane] - S.c_zr[0] : 0.f;             // chunk reference relative to the first chunk's
+    const float f = live ? ex2f(cm - gref) : 0.f;                       // chunk-relative weights -> relative to the largest chunk reference
     const float wc = live ? S.c_mom[lane][0] : 0.f, qc = live ? S.c_mom[lane][1] : 0.f;
     const float bc = live ? S.c_mom[lane][2] : 0.f, ac = live ? S.c_mom[lane][3] : 0.f;
     if (wid == 0 && lane < kFW) S.c_f[lane] = f;
-    float SW = f * wc, SQ = f * f * qc, SB = f * fmaf(dl, wc, bc);
+    float SW = f * wc, SQ = f * f * qc, SB = f * bc;
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1) {
         SW += __shfl_xor_sync(0xffffffffu, SW, o);
@@ -265,7 +261,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     SW = __shfl_sync(0xffffffffu, SW, 0);
     SQ = __shfl_sync(0xffffffffu, SQ, 0);
     SB = __shfl_sync(0xffffffffu, SB, 0);
-    const float ubar = SB / SW, de = dl - ubar;                         // weighted mean (relative to the first chunk's reference)
+    const float de = -SB / SW;                                          // minus the weighted mean (relative to z_mid)
     float SA = f * fmaf(de, fmaf(de, wc, 2.f * bc), ac);                // sum w (u + de)^2 >= 0 per chunk
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1) SA += __shfl_xor_sync(0xffffffffu, SA, o);
@@ -280,7 +276,25 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     }
     // handed over: no bandwidth; few effective samples (fp32 weights, moments and the plain form of Scott's rule are good for
     // n_eff >> 1 only); every supported secondary deep in the smoothing window (m2' < ~0.3 sqrt(delta): d ln w = delta/m2'^2 x 1e-6)
-    bool hand = !(h > 0.0) || !isfinite(h) || !(neff >= P.neff_min) || gmp2 * gmp2 < 0.1f * F.delta;
+    // the largest m2' of the event, bounded from below chunk by chunk: the chunk's largest m2d (packed at init) at the chunk's far
+    // end, where 1/(1+z) is smallest (within 0.5 % of the exact value; the unit is handed over whenever the exact criterion would)
+    float gmp2 = -INFINITY;
+    if (lane < kFW) {
+        const float2 ct = __ldg(P.ev.chunk_top + (size_t)ev * kFW + lane);   // {largest m2d, t of the last sample} of chunk `lane`
+        float un, a1;
+        unpack2(Cf.ua[kPolyN - 2], un, a1);
+#pragma unroll
+        for (int n = kPolyN - 3; n >= 0; --n) {
+            float an;
+            unpack2(Cf.ua[n], un, an);
+            a1 = fmaf(a1, ct.y, an);
+        }
+        gmp2 = fmaf(ct.x, a1, -F.mlow_hi);                               // (empty chunks: m2d = 0)
+    }
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) gmp2 = fmaxf(gmp2, __shfl_xor_sync(0xffffffffu, gmp2, o));
+    gmp2 = __shfl_sync(0xffffffffu, gmp2, 0);
+    bool hand = !(h > 0.0) || !isfinite(h) || !(neff >= P.neff_min) || gmp2 < 0.f || gmp2 * gmp2 < 0.1f * F.delta;
     // local-expansion geometry: y = z'/(sqrt(2) h), boxes of m grid spacings centred on grid points
     const double udz = __ldg(P.ev.uni_dz + ev), zfirst = __ldg(P.ev.zc + g0);
     const float scy = (float)(0.70710678118654752440 / h);
@@ -427,10 +441,10 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         double tot = 0.0;
 #pragma unroll
         for (int k = 0; k < kFW; ++k) tot += S.c_sum[k];                // fixed order: deterministic
-        // K(z) = 1/(N_s h sqrt(2 pi)) sum_j w_j exp(..); the weights were divided by 2^gmx, the prior and q_g scales factored out
+        // K(z) = 1/(N_s h sqrt(2 pi)) sum_j w_j exp(..); the weights were divided by 2^gref, the prior and q_g scales factored out
         const double I = tot / ((double)ns * h * 2.50662827463100050242);
         if (I > 0.0 && isfinite(I)) {
-            *out = log(I) + (double)gmx * 0.69314718055994530942 + __ldg(P.ln_shift + ev) + __ldg(P.ln_qscale + ev);
+            *out = log(I) + (double)gref * 0.69314718055994530942 + __ldg(P.ln_shift + ev) + __ldg(P.ln_qscale + ev);
         } else {   // nothing within the cut-off (or not a number): k_events evaluates the unit in log space
             const unsigned k_ = atomicAdd(P.work_count, 1u);
             P.worklist[k_] = (uint32_t)l * (uint32_t)P.ev.n_events + (uint32_t)ev;
