@@ -397,6 +397,65 @@ __device__ __forceinline__ void poly_sample(const LamF& F, const float gk2, cons
     poly_sample<kFit>(F, gk2, cpsi, C, A, Bq, M, tm_lo, tm_hi, zc, l2w, mp2);
 }
 
+// The same sample in two halves, for the sweeps that stream their records through registers (k_events_fast, k_inject).  The head
+// consumes the record (both halves) and leaves seven numbers; the tail needs no record.  A sweep runs the heads of two samples,
+// requests the records of the next two (one group of loads: ptxas puts every global load of a loop on one scoreboard, so
+// waiting for the oldest load waits for the newest -- the group must be the only one in flight and as old as possible at the
+// next head), then the two tails.
+struct PolyMid {
+    float zc, rb, u, mp1, mp2, tf;   // z - z_ref; r + beta2 ln m2d + log2(1/prior); ln(1+z); m1', m2'; fraction of the mass-table row
+    int row;                         // staged row of the mass table (variant folded in)
+};
+__device__ __forceinline__ void poly_head(const LamF& F, const PolyCoef& C, const float4 A, const float2 Bq, const MassLookup& M,
+                                          const float tm_lo, const float tm_hi, PolyMid& m) {
+    const f32x2 t2 = pack2(A.z, A.z);
+    f32x2 zr = C.zr[6], ua = C.ua[5];
+#pragma unroll
+    for (int n = 5; n >= 0; --n) zr = fma2(zr, t2, C.zr[n]);
+#pragma unroll
+    for (int n = 4; n >= 0; --n) ua = fma2(ua, t2, C.ua[n]);
+    float r, a;
+    unpack2(zr, m.zc, r);
+    unpack2(ua, m.u, a);
+    unpack2(fma2(pack2(A.x, A.y), pack2(a, a), pack2(-F.mlow_hi, -F.mlow_hi)), m.mp1, m.mp2);   // m' = m^d a - m_low
+    float tm = fmaf(A.w - m.u, F.tm_scale, F.mlow_tm);
+    tm = fminf(fmaxf(tm, tm_lo), tm_hi);
+    const float ti = (tm - 0.5f) + 12582912.f;
+    m.tf = tm - (ti - 12582912.f);
+    m.row = (__float_as_int(ti) - 0x4B400000) - M.lo + ((m.mp1 > F.mhigh_p) ? M.cap : 0);
+    m.rb = r + fmaf(F.beta2, Bq.x, Bq.y);
+}
+template <bool kTurn, bool kWinS>
+__device__ __forceinline__ float poly_tail(const LamF& F, const float gk2, const float cpsi, const MassLookup& M, const PolyMid& m,
+                                           const float4* __restrict__ win_s) {
+    const float4 c = M.s[m.row];
+    float l = fmaf(fmaf(fmaf(c.w, m.tf, c.z), m.tf, c.y), m.tf, c.x) + m.rb;
+    l = fmaf(-2.f, lg2f(m.mp1), l);          // m1' <= 0 implies m2' <= 0: discarded below
+    if (kTurn) l -= lg2f(1.0f + ex2f(fmaf(gk2, m.u, -cpsi)));
+    if (__any_sync(0xffffffffu, m.mp2 < F.delta)) {
+        const float4 wc = kWinS ? *win_s : make_float4(F.win_lo, F.win_hi, F.two_dl2e, F.d2l2e);
+        const float mc = fminf(fmaxf(m.mp2, wc.x), wc.y);
+        const float f2 = fmaf(wc.z, mc, -wc.w) * rcpf(mc * (mc - F.delta));
+        const float ls = (f2 > 64.f) ? f2 : lg2f(1.0f + ex2f(f2));
+        l -= (m.mp2 < F.delta) ? ls : 0.f;
+    }
+    return (m.mp2 > 0.f) ? l : -INFINITY;    // R15 support: m_low < m2
+}
+// The records of the next two blocks into R0 / R1, behind the heads that consumed the previous ones (`a0`, `a1`: a value from
+// each head; the predicate is a true dependency the assembler cannot remove -- always true for numbers).
+__device__ __forceinline__ void ldg_stream_pair_after(PRec& R0, PRec& R1, const float4* pa0, const float2* pb0, const float4* pa1,
+                                                      const float2* pb1, float a0, float a1) {
+    asm volatile(
+        "{\n .reg .pred p;\n setp.le.f32 p, %16, 0f7F800000;\n setp.le.and.f32 p, %17, 0f7F800000, p;\n"
+        " @p ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%12];\n"
+        " @p ld.global.nc.L1::no_allocate.v2.f32 {%4,%5}, [%13];\n"
+        " @p ld.global.nc.L1::no_allocate.v4.f32 {%6,%7,%8,%9}, [%14];\n"
+        " @p ld.global.nc.L1::no_allocate.v2.f32 {%10,%11}, [%15];\n}"
+        : "+f"(R0.A.x), "+f"(R0.A.y), "+f"(R0.A.z), "+f"(R0.A.w), "+f"(R0.B.x), "+f"(R0.B.y), "+f"(R1.A.x), "+f"(R1.A.y), "+f"(R1.A.z),
+          "+f"(R1.A.w), "+f"(R1.B.x), "+f"(R1.B.y)
+        : "l"(pa0), "l"(pb0), "l"(pa1), "l"(pb1), "f"(a0), "f"(a1));
+}
+
 // k_events_fast: eight warps, each on a contiguous chunk of the event's (d_L-sorted) samples; chunks are whole passes of 128
 constexpr int kFastWarps = 8;
 constexpr int kFastPass = 128;

@@ -168,11 +168,9 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         const float4* pa_t = pa + c0 + lane;
         const float2* pb_t = pb + c0 + lane;
         float2* zw_t = zw + c0 + lane;
-        float l2w_;
-#define CHIM_FAST_SAMPLE(REC, OFF, IN, SEARCH)                                                                    \
+#define CHIM_FAST_TAIL(MID, OFF, IN, SEARCH)                                                                      \
         {                                                                                                         \
-            float zc_, mp2_;                                                                                      \
-            poly_sample<true, true, true>(F, F.gk2, F.cpsi, Cf, (REC).A, (REC).B, M, tm_lo, tm_hi, zc_, l2w_, mp2_, &S.win); \
+            const float l2w_ = poly_tail<true, true>(F, F.gk2, F.cpsi, M, MID, &S.win);                           \
             const float lw_ = (IN) ? l2w_ : -INFINITY;                                                            \
             if ((SEARCH) && ref_unset) {   /* (warp-uniform) */                                                   \
                 float b_ = lw_;                                                                                   \
@@ -182,43 +180,51 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
                     ref_unset = false;                                                                            \
                 }                                                                                                 \
             }                                                                                                     \
-            const float w_ = ex2f(lw_ - ref), u_ = zc_ - zmid, wu_ = w_ * u_;                                     \
+            const float w_ = ex2f(lw_ - ref), u_ = (MID).zc - zmid, wu_ = w_ * u_;                                \
             m0 += w_;                                                                                             \
             m1 = fmaf(w_, w_, m1);                                                                                \
             m2 += wu_;                                                                                            \
             m3 = fmaf(wu_, u_, m3);                                                                               \
-            zw_t[OFF] = make_float2(zc_, w_);                                                                     \
+            zw_t[OFF] = make_float2((MID).zc, w_);                                                                \
         }
+        // Two samples per iteration: both heads (they consume the records), the records of the next two blocks as one group of
+        // loads -- a full tail phase and the next heads away from their use -- then both tails.  The record arrays carry a spare
+        // tail, so the loads are unconditional.
 #define CHIM_FAST_PAIR(SEARCH)                                                                                    \
         {                                                                                                         \
-            CHIM_FAST_SAMPLE(R0, 0, true, SEARCH)                                                                 \
-            R0.A = ldg_stream_a(pa_t + 64);                                                                       \
-            ldg_stream_b(R0.B, pb_t + 64, l2w_);                                                                  \
-            CHIM_FAST_SAMPLE(R1, 32, true, SEARCH)                                                                \
-            R1.A = ldg_stream_a(pa_t + 96);                                                                       \
-            ldg_stream_b(R1.B, pb_t + 96, l2w_);                                                                  \
+            PolyMid M0, M1;                                                                                       \
+            poly_head(F, Cf, R0.A, R0.B, M, tm_lo, tm_hi, M0);                                                    \
+            poly_head(F, Cf, R1.A, R1.B, M, tm_lo, tm_hi, M1);                                                    \
+            ldg_stream_pair_after(R0, R1, pa_t + 64, pb_t + 64, pa_t + 96, pb_t + 96, M0.rb, M1.rb);              \
+            CHIM_FAST_TAIL(M0, 0, true, SEARCH)                                                                   \
+            CHIM_FAST_TAIL(M1, 32, true, SEARCH)                                                                  \
             pa_t += 64;                                                                                           \
             pb_t += 64;                                                                                           \
             zw_t += 64;                                                                                           \
         }
-        // the records are streamed two blocks ahead (one doubled iteration ~ 160 instructions x 6 warps per scheduler: the L2
-        // latency); the record arrays carry a spare tail, so the loads are unconditional.  Half A may be requested as soon as the
-        // sample's polynomials are done, half B only behind its use at the very end of the sample (ldg_stream_b).  The first loop
-        // runs until the chunk's reference is set (normally one iteration), the second is the plain one.
+        // the first loop runs until the chunk's reference is set (normally one iteration), the second is the plain one
 #pragma unroll 1
         for (; nblk >= 2 && ref_unset; nblk -= 2) CHIM_FAST_PAIR(true)
 #pragma unroll 1
         for (; nblk >= 2; nblk -= 2) CHIM_FAST_PAIR(false)
-        if (nblk) {
-            CHIM_FAST_SAMPLE(R0, 0, true, true)
-            zw_t += 32;
-            R0 = R1;
+        // an odd block, then the ragged end of the event (records padded to whole warps with copies of the last sample:
+        // poly_tail votes); the lanes beyond the event store that sample's redshift with weight 0 -- S3 reads the pair of the
+        // last sample unmasked
+        {
+            PolyMid M0;
+            if (nblk) {
+                poly_head(F, Cf, R0.A, R0.B, M, tm_lo, tm_hi, M0);
+                CHIM_FAST_TAIL(M0, 0, true, true)
+                zw_t += 32;
+                R0 = R1;
+            }
+            if (ragged) {
+                poly_head(F, Cf, R0.A, R0.B, M, tm_lo, tm_hi, M0);
+                CHIM_FAST_TAIL(M0, 0, (int)(zw_t - zw) < c1, true)
+            }
         }
-        // the ragged end of the event (records padded to whole warps with copies of the last sample: poly_sample votes); the lanes
-        // beyond it store that sample's redshift with weight 0 -- S3 reads the pair of the last sample unmasked
-        if (ragged) CHIM_FAST_SAMPLE(R0, 0, (int)(zw_t - zw) < c1, true)
 #undef CHIM_FAST_PAIR
-#undef CHIM_FAST_SAMPLE
+#undef CHIM_FAST_TAIL
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             m0 += __shfl_xor_sync(0xffffffffu, m0, o);
