@@ -122,37 +122,45 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             k0 = lo ? __ffs(lo) - 1 : (hi ? 32 + __ffs(hi) - 1 : kInjChunkBlocks);
             k0 = max(0, min(k0, nblk - 1));
         }
-#define CHIM_INJ_SAMPLE(TURN, REC, JJ)                                                                                \
+#define CHIM_INJ_TAIL(TURN, MID, JJ)                                                                                  \
         {                                                                                                             \
-            float zc, mp2_;                                                                                           \
-            poly_sample<true, TURN>(F, F.gk2_inj, F.cpsi_inj, C, (REC).A, (REC).B, M, 1.0f, tm_hi, zc, l2w, mp2_);    \
-            const double s = (zc <= 0.f && (JJ) < n) ? ex2_to_double(l2w) : 0.0;                                      \
+            const float l2w = poly_tail<TURN, false>(F, F.gk2_inj, F.cpsi_inj, M, MID, nullptr);                      \
+            const double s = ((MID).zc <= 0.f && (JJ) < n) ? ex2_to_double(l2w) : 0.0;                                \
             acc[0] += s;                                                                                              \
             acc[1] = fma(s, s, acc[1]);                                                                               \
             if (kDbg && (JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale;                                   \
         }
-        // records two blocks ahead; half B of a record is requested behind its use at the end of the sample (ldg_stream_b)
+        // two blocks per iteration: both heads (they consume the records), the records of the next two blocks as one group of
+        // loads, then both tails (chim_internal.cuh: poly_head / poly_tail)
 #define CHIM_INJ_SWEEP(TURN)                                                                                          \
         {                                                                                                             \
             int j = tid + k0 * kInjThreads;                                                                           \
-            float l2w;                                                                                                \
-            PRec R0 = ldg_stream_prec(pa + j, pb + j), R1 = ldg_stream_prec(pa + j + kInjThreads, pb + j + kInjThreads); \
+            const float4* pa_t = pa + j;                                                                              \
+            const float2* pb_t = pb + j;                                                                              \
+            PRec R0 = ldg_stream_prec(pa_t, pb_t), R1 = ldg_stream_prec(pa_t + kInjThreads, pb_t + kInjThreads);      \
             _Pragma("unroll 1") for (; j + kInjThreads < n32; j += 2 * kInjThreads) {                                 \
-                CHIM_INJ_SAMPLE(TURN, R0, j)                                                                          \
-                R0.A = ldg_stream_a(pa + j + 2 * kInjThreads);                                                        \
-                ldg_stream_b(R0.B, pb + j + 2 * kInjThreads, l2w);                                                    \
-                CHIM_INJ_SAMPLE(TURN, R1, j + kInjThreads)                                                            \
-                R1.A = ldg_stream_a(pa + j + 3 * kInjThreads);                                                        \
-                ldg_stream_b(R1.B, pb + j + 3 * kInjThreads, l2w);                                                    \
+                PolyMid M0, M1;                                                                                       \
+                poly_head(F, C, R0.A, R0.B, M, 1.0f, tm_hi, M0);                                                      \
+                poly_head(F, C, R1.A, R1.B, M, 1.0f, tm_hi, M1);                                                      \
+                ldg_stream_pair_after(R0, R1, pa_t + 2 * kInjThreads, pb_t + 2 * kInjThreads, pa_t + 3 * kInjThreads, \
+                                      pb_t + 3 * kInjThreads, M0.rb, M1.rb);                                          \
+                CHIM_INJ_TAIL(TURN, M0, j)                                                                            \
+                CHIM_INJ_TAIL(TURN, M1, j + kInjThreads)                                                              \
+                pa_t += 2 * kInjThreads;                                                                              \
+                pb_t += 2 * kInjThreads;                                                                              \
             }                                                                                                         \
-            if (j < n32) CHIM_INJ_SAMPLE(TURN, R0, j)                                                                 \
+            if (j < n32) {                                                                                            \
+                PolyMid M0;                                                                                           \
+                poly_head(F, C, R0.A, R0.B, M, 1.0f, tm_hi, M0);                                                      \
+                CHIM_INJ_TAIL(TURN, M0, j)                                                                            \
+            }                                                                                                         \
         }
         if (kDbg)
             for (int j = tid; j < min(k0 * kInjThreads, n); j += kInjThreads) P.dbg_s[P.inj.perm[j0 + j]] = 0.0;
         if (turn_folded) CHIM_INJ_SWEEP(false)
         else CHIM_INJ_SWEEP(true)
 #undef CHIM_INJ_SWEEP
-#undef CHIM_INJ_SAMPLE
+#undef CHIM_INJ_TAIL
     } else if (L.flags == 0) {
         const float4* rows = reinterpret_cast<const float4*>(P.tab + (size_t)l * P.tab_rows);
         const int64_t j1w = j0 + ((j1 - j0 + 31) & ~(int64_t)31);    // whole warps stay in the loop (sample_eval votes)
