@@ -28,7 +28,8 @@ constexpr int kFW = kFastWarps;      // warps = sample chunks
 constexpr int kFPass = kFastPass;    // samples per warp pass (4 per lane)
 constexpr int kFLeP = 12;            // terms of the local expansion
 constexpr int kFMaxBox = 96;         // boxes per event
-constexpr int kFBoxPerWarp = kFMaxBox / kFW;
+constexpr int kFBoxRec = 16;          // floats per box in shared memory: 12 coefficients, the box centre, 3 unused (64-byte records)
+constexpr int kFGroup = 5;            // boxes whose coefficients one warp builds at a time
 constexpr float kFMaxW = 1.3f;       // largest box width in units of sqrt(2) h
 constexpr int kFMaxD = 256;          // largest half-width of the psi table (grid points; ~60 on the spectroscopic, ~240 on the 4096-point photometric grids)
 constexpr int kFQPad = 2 * kFMaxD;   // zeros on both sides of the staged q_g: the coefficient build reads g_b +- d unchecked
@@ -41,13 +42,12 @@ struct FastSmem {
     float c_mom[kFW][4];             // sum w, sum w^2, sum w u, sum w u^2 with w relative to c_ref, u = z - z_mid
     float c_f[kFW];                  // 2^(c_ref - largest c_ref): chunk-relative weights -> one scale for the event
     double c_sum[kFW];               // per warp: sum_j w_j A_j over its boxes, relative to the event's largest weight
-    int bnd[kFMaxBox + 1];           // first sample of every box (samples are sorted)
 };
 
 __host__ __device__ inline size_t fast_nz4(size_t nz) { return (nz + 3) / 4 * 4; }
 __host__ __device__ inline size_t fast_aux_bytes() {
     const size_t a = 2 * (size_t)kFMassStage * sizeof(MassRow);
-    const size_t b = 4 * (size_t)kFLeP * ((size_t)(kFMaxD + 1) + (size_t)kFMaxBox);
+    const size_t b = 4 * ((size_t)kFLeP * (size_t)(kFMaxD + 1) + (size_t)kFBoxRec * (size_t)kFMaxBox);
     return a > b ? a : b;
 }
 size_t events_fast_smem_bytes(int max_ns, int max_nz) {
@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     unsigned char* aux = reinterpret_cast<unsigned char*>(qs + 2 * (size_t)kFQPad + fast_nz4((size_t)P.ev.max_nz));
     MassRow* mass_s = reinterpret_cast<MassRow*>(aux);                  // S2: both variants of the event's slice of the mass table
     float* psi = reinterpret_cast<float*>(aux);                         // S3: psi table [(D+1) x 12] ...
-    float* Bc = psi + (size_t)kFLeP * (kFMaxD + 1);                     // ... and the expansion coefficients [warp][box][12]
+    float* Bc = psi + (size_t)kFLeP * (kFMaxD + 1);                     // ... and the box records [box][16]: 12 expansion coefficients, centre
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
 
     const int l = blockIdx.x % P.n_lambda;                              // lambda fastest: CTAs in flight share an event
@@ -314,24 +314,8 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
            !(fD <= (float)kFMaxD) || !(fabsf(fb_lo) * (float)m < 1e8f) || !(fabsf(fb_hi) * (float)m < 1e8f);
     if (hand) CHIM_FAST_HANDOVER();
     const int D = (int)fD, b_lo = (int)fb_lo, nbox = (int)(fb_hi - fb_lo) + 1;
-    // once per CTA, one thread per entry: the first sample of every box (binary search in the sorted samples; box b holds the
-    // samples with y in [c_b - w/2, c_b + w/2), c_b = yfirst + (b_lo + b) w) from the low threads, and from the high ones the
-    // psi table psi_n(d dy) = exp(-t^2) H_n(t)/n!, t = d dy, by the three-term recurrence
-    if (tid <= nbox) {
-        int lo = 0, hi = ns;
-        if (tid == 0) hi = 0;
-        else if (tid == nbox) lo = ns;
-        else {
-            const float zb = (yfirst + ((float)(b_lo + tid) - 0.5f) * wbox) / scy;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (zw[mid].x < zb) lo = mid + 1;
-                else hi = mid;
-            }
-        }
-        S.bnd[tid] = lo;
-    }
-    for (int d = kFT - 1 - tid; d <= D; d += kFT) {
+    // once per CTA, one thread per entry: the psi table psi_n(d dy) = exp(-t^2) H_n(t)/n!, t = d dy, by the three-term recurrence
+    for (int d = tid; d <= D; d += kFT) {
         const float t = (float)d * dy, t2 = 2.f * t;
         float p0v = ex2f(-t * t * 1.44269504088896341f), p1v = t2 * p0v;
         float* o = psi + (size_t)d * kFLeP;
@@ -345,22 +329,18 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
             p1v = p2v;
         }
     }
-    __syncthreads();                                                    // (3) psi table, box ranges (the staged mass rows are dead)
+    __syncthreads();                                                    // (3) psi table (the staged mass rows are dead)
 
-    // ---- S3 + S4, warp w on the boxes w, w + 8, ...: their coefficients, then one degree-11 polynomial per sample ------------------
-    double lsum = 0.0;
-    const int nbw = (wid < nbox) ? (nbox - wid + kFW - 1) / kFW : 0;    // boxes of this warp
-    if (nbw > 0) {
-        float* Bw = Bc + (size_t)wid * kFBoxPerWarp * kFLeP;
-        // coefficients B_bn = sum_{|d| <= D} q_{g_b+d} psi_n(d dy): lane = (half of the d range, box, quad of n), five boxes per
-        // round; psi_n(-t) = (-1)^n psi_n(t), so even n take (q_+ + q_-) psi_n and odd n (q_+ - q_-) psi_n -- the pairs (n, n+1)
-        // of a packed FMA
+    // ---- S3, coefficients: groups of five consecutive boxes, group g built by warp g mod 8 -----------------------------------------
+    // B_bn = sum_{|d| <= D} q_{g_b+d} psi_n(d dy): lane = (half of the d range, box of the group, quad of n); psi_n(-t) =
+    // (-1)^n psi_n(t), so even n take (q_+ + q_-) psi_n and odd n (q_+ - q_-) psi_n -- the pairs (n, n+1) of a packed FMA
+    {
         const int half = lane >= 15 ? 1 : 0, sub = lane - 15 * half, quad = sub % 3, bsub = sub / 3;
         const int Dh = D >> 1, d_lo = half ? Dh + 1 : 1, d_hi = half ? D : Dh;
-        for (int base = 0; base < nbw; base += 5) {
+        for (int base = kFGroup * wid; base < nbox; base += kFGroup * kFW) {
             const int bi = base + bsub;
-            const bool valid = lane < 30 && bi < nbw;
-            const int gc = (b_lo + wid + kFW * (valid ? bi : 0)) * m;   // grid index of the box centre
+            const bool valid = lane < 30 && bi < nbox;
+            const int gc = (b_lo + (valid ? bi : 0)) * m;               // grid index of the box centre
             const bool reach = valid && gc > -D - 1 && gc < nz + D;     // else no grid point within the box's cut-off: B = 0
             const float* qp = qs + kFQPad + (reach ? gc : 0) + d_lo;
             const float* qm = qs + kFQPad + (reach ? gc : 0) - d_lo;
@@ -404,42 +384,47 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
             acc.y += __shfl_down_sync(0xffffffffu, acc.y, 15);
             acc.z += __shfl_down_sync(0xffffffffu, acc.z, 15);
             acc.w += __shfl_down_sync(0xffffffffu, acc.w, 15);
-            if (valid && !half) reinterpret_cast<float4*>(Bw + (size_t)bi * kFLeP)[quad] = acc;
-        }
-        __syncwarp();
-        // evaluation box by box: the samples [bnd[b], bnd[b+1]) in passes of 128 (4 consecutive per lane, aligned to 4; lanes beyond
-        // the range masked), the box's 12 coefficients in registers, s = y - c_b
-        const float invC = 1.0f / (float)C;                             // chunk of a pair of samples: floor((jb + 1) / C), exact in fp32 (jb even, C a multiple of 128)
-        for (int k = 0; k < nbw; ++k) {
-            const int b = wid + kFW * k;
-            const int j_lo = S.bnd[b], j_hi = S.bnd[b + 1];
-            if (j_hi <= j_lo) continue;
-            const float cb = fmaf((float)((b_lo + b) * m), dy, yfirst);
-            const float4* bp = reinterpret_cast<const float4*>(Bw + (size_t)k * kFLeP);
-            const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
-            const int jsafe = (ns - 1) & ~1;                                // (lanes beyond the range read a valid pair; their weights are masked)
-            for (int jb = (j_lo & ~1) + 2 * lane; jb - 2 * lane < j_hi; jb += kFPass) {   // lane: samples jb, jb + 1, jb + 64, jb + 65
-                const float4 ab = *reinterpret_cast<const float4*>(zw + min(jb, jsafe)), cd4 = *reinterpret_cast<const float4*>(zw + min(jb + 64, jsafe));
-                const f32x2 s01 = pack2(fmaf(ab.x, scy, -cb), fmaf(ab.z, scy, -cb)), s23 = pack2(fmaf(cd4.x, scy, -cb), fmaf(cd4.z, scy, -cb));
-                f32x2 a01 = pack2(k2.w, k2.w), a23 = a01;
-#define CHIM_LE_STEP(cf) { const f32x2 q_ = pack2(cf, cf); a01 = fma2(a01, s01, q_); a23 = fma2(a23, s23, q_); }
-                CHIM_LE_STEP(k2.z) CHIM_LE_STEP(k2.y) CHIM_LE_STEP(k2.x)
-                CHIM_LE_STEP(k1.w) CHIM_LE_STEP(k1.z) CHIM_LE_STEP(k1.y) CHIM_LE_STEP(k1.x)
-                CHIM_LE_STEP(k0.w) CHIM_LE_STEP(k0.z) CHIM_LE_STEP(k0.y) CHIM_LE_STEP(k0.x)
-#undef CHIM_LE_STEP
-                float v[4];
-                unpack2(a01, v[0], v[1]);
-                unpack2(a23, v[2], v[3]);
-                const float wv[4] = {ab.y, ab.w, cd4.y, cd4.w};
-                const unsigned rel = (unsigned)(jb - j_lo), span = (unsigned)(j_hi - j_lo);   // sample jb + o is in the box iff rel + o < span (unsigned)
-                // the two pairs may lie in different chunks: the weights are relative to their chunk's largest
-                const float f01 = S.c_f[min(__float2int_rd((float)(jb + 1) * invC), kFW - 1)], f23 = S.c_f[min(__float2int_rd((float)(jb + 65) * invC), kFW - 1)];   // (clamped: masked lanes may point past the last chunk)
-                const float a0 = fmaf((rel < span) ? wv[0] : 0.f, v[0], ((rel + 1u < span) ? wv[1] : 0.f) * v[1]);
-                const float a1 = fmaf((rel + 64u < span) ? wv[2] : 0.f, v[2], ((rel + 65u < span) ? wv[3] : 0.f) * v[3]);
-                lsum += (double)fmaf(a0, f01, a1 * f23);
+            if (valid && !half) {
+                reinterpret_cast<float4*>(Bc + (size_t)bi * kFBoxRec)[quad] = acc;
+                if (quad == 0) Bc[(size_t)bi * kFBoxRec + kFLeP] = fmaf((float)gc, dy, yfirst);   // the box centre c_b
             }
         }
-        lsum = warp_sum(lsum);
+    }
+    __syncthreads();                                                    // (4) the box records are complete
+
+    // ---- S3 + S4, evaluation: warp w on its own chunk of the samples (the one it wrote in S2: one weight scale per warp) --------------
+    // per sample its box b = round((y - y_first)/w) - b_lo (any box whose centre is within ~w/2 serves; clamped to the boxes that
+    // exist), the box record from shared memory (neighbouring lanes mostly share it: broadcast), s = y - c_b and one degree-11
+    // polynomial; four samples per lane and pass (pairs jb, jb + 1 and jb + 64, jb + 65: 16-byte lane stride)
+    double lsum = 0.0;
+    if (c0 < ns) {
+        const float kb = 0.5f - (float)b_lo - yfirst * inv_w;
+        const int bmax = nbox - 1;
+        const float4* B4 = reinterpret_cast<const float4*>(Bc);
+        const int jsafe = (ns - 1) & ~1;                                // (slots beyond the chunk's last pair read that pair; their weights are masked)
+        const int pend = c0 + ((c1 - c0 + kFPass - 1) / kFPass) * kFPass;
+        for (int jb = c0 + 2 * lane; jb < pend; jb += kFPass) {
+            const float4 ab = *reinterpret_cast<const float4*>(zw + min(jb, jsafe)), cd4 = *reinterpret_cast<const float4*>(zw + min(jb + 64, jsafe));
+            const float zv[4] = {ab.x, ab.z, cd4.x, cd4.z};
+            const float wv[4] = {ab.y, ab.w, cd4.y, cd4.w};
+            float a = 0.f;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const float y = zv[r] * scy;
+                const int b = min(max(__float2int_rd(fmaf(y, inv_w, kb)), 0), bmax);
+                const float4* bp = B4 + b * (kFBoxRec / 4);
+                const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
+                const float sv = y - bp[3].x;
+                float v = k2.w;
+                v = fmaf(v, sv, k2.z); v = fmaf(v, sv, k2.y); v = fmaf(v, sv, k2.x);
+                v = fmaf(v, sv, k1.w); v = fmaf(v, sv, k1.z); v = fmaf(v, sv, k1.y); v = fmaf(v, sv, k1.x);
+                v = fmaf(v, sv, k0.w); v = fmaf(v, sv, k0.z); v = fmaf(v, sv, k0.y); v = fmaf(v, sv, k0.x);
+                const bool in = jb + (r & 1) + 64 * (r >> 1) < c1;
+                a = fmaf(in ? wv[r] : 0.f, v, a);
+            }
+            lsum += (double)a;
+        }
+        lsum = warp_sum(lsum) * (double)S.c_f[wid];
     }
     if (lane == 0) S.c_sum[wid] = lsum;
     __syncthreads();                                                    // (4)
