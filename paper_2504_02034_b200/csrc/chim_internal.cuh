@@ -456,10 +456,11 @@ __device__ __forceinline__ void ldg_stream_pair_after(PRec& R0, PRec& R1, const 
         : "l"(pa0), "l"(pb0), "l"(pa1), "l"(pb1), "f"(a0), "f"(a1));
 }
 
-// k_events_fast: eight warps, each on a contiguous chunk of the event's (d_L-sorted) samples; chunks are whole passes of 128
+// k_events_fast: eight warps, each on a contiguous chunk of the event's (d_L-sorted) samples; chunks are whole blocks of 32
+// samples, the evaluation takes them in passes of 128
 constexpr int kFastWarps = 8;
 constexpr int kFastPass = 128;
-__host__ __device__ inline int fast_chunk(int ns) { return ((ns + kFastWarps * kFastPass - 1) / (kFastWarps * kFastPass)) * kFastPass; }
+__host__ __device__ inline int fast_chunk(int ns) { return ((ns + kFastWarps * 32 - 1) / (kFastWarps * 32)) * 32; }   // whole blocks of 32
 
 // ---- TMA bulk copy + mbarrier  ---------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -68,23 +68,36 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
 
     const int l = blockIdx.x % P.n_lambda;                              // lambda fastest: CTAs in flight share an event
     const int ev = P.fast_events[blockIdx.x / P.n_lambda];
-    const int64_t s0 = P.ev.sample_off[ev], g0 = P.ev.grid_off[ev];
-    const int ns = (int)(P.ev.sample_off[ev + 1] - s0), nz = (int)(P.ev.grid_off[ev + 1] - g0);
-    double* out = P.logI + (size_t)l * P.ev.n_events + ev;
+    // Everything the unit needs from global memory is requested here in one batch, before the first branch that depends on any
+    // of it (three dependent round trips -- event, these, records / mass rows -- instead of six): offsets, the per-lambda
+    // constants, the 28-float record of k_polyfit (26 polynomial coefficients and the slice of the mass table to stage).
     const LamConst* Lg = P.Lc + l;
-    if (__ldg(&Lg->flags)) {   // invalid lambda: NaN
+    const float* pr = P.poly + ((size_t)l * P.ev.n_events + ev) * (4 * kPolyN);
+    float4 v[7];
+    {
+        const float4* q = reinterpret_cast<const float4*>(pr);
+#pragma unroll
+        for (int k = 0; k < 7; ++k) v[k] = __ldg(q + k);
+    }
+    LamF F;
+    load_lamf_hot(F, &Lg->F);
+    const uint32_t lflags = __ldg(&Lg->flags);
+    const double tkmax = __ldg(&Lg->tkmax_ev);
+    const int64_t s0 = __ldg(P.ev.sample_off + ev), s1 = __ldg(P.ev.sample_off + ev + 1);
+    const int64_t g0 = __ldg(P.ev.grid_off + ev), g1 = __ldg(P.ev.grid_off + ev + 1);
+    const int64_t p0 = __ldg(P.ev.poly_off + ev), q0off = __ldg(P.ev.q4_off + ev);
+    const double tk_h = __ldg(P.ev.tk_h + ev), tk_c = __ldg(P.ev.tk_c + ev);
+    const int ns = (int)(s1 - s0), nz = (int)(g1 - g0);
+    double* out = P.logI + (size_t)l * P.ev.n_events + ev;
+    if (lflags) {   // invalid lambda: NaN
         if (tid == 0) *out = NAN;
         return;
     }
-    const float* pr = P.poly + ((size_t)l * P.ev.n_events + ev) * (4 * kPolyN);
     // the event-local polynomials exist (k_polyfit) iff the whole d_L range of the event lies inside the table
     int mlo = 0, nr = 0;
-    {
-        const double tk_h = __ldg(P.ev.tk_h + ev), tk_c = __ldg(P.ev.tk_c + ev);
-        if (tk_h > 0.0 && tk_c + tk_h < __ldg(&Lg->tkmax_ev)) {
-            mlo = __float_as_int(__ldg(pr + 26));
-            nr = __float_as_int(__ldg(pr + 27));    // > 0: every mass-table row the event can address fits the stage
-        }
+    if (tk_h > 0.0 && tk_c + tk_h < tkmax) {
+        mlo = __float_as_int(v[6].z);
+        nr = __float_as_int(v[6].w);                // > 0: every mass-table row the event can address fits the stage
     }
 #define CHIM_FAST_HANDOVER()                                                    \
     do {                                                                        \
@@ -99,6 +112,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     const size_t nz4 = fast_nz4((size_t)nz);
     const MassRow* mtab = P.mtab + (size_t)l * 2 * (P.n_mass + 2);
     if (tid == 0) {
+        S.win = make_float4(F.win_lo, F.win_hi, F.two_dl2e, F.d2l2e);
         mbar_init(&S.mbar_mass, 1);
         mbar_init(&S.mbar_q, 1);
         const uint32_t mbytes = (uint32_t)nr * (uint32_t)sizeof(MassRow);
@@ -107,34 +121,27 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         bulk_g2s(mass_s + kFMassStage, mtab + (P.n_mass + 2) + mlo, mbytes, &S.mbar_mass);
         const uint32_t qbytes = (uint32_t)nz4 * 4u;
         mbar_expect_tx(&S.mbar_q, qbytes);
-        bulk_g2s(qs + kFQPad, P.ev.qn4 + P.ev.q4_off[ev], qbytes, &S.mbar_q);
+        bulk_g2s(qs + kFQPad, P.ev.qn4 + q0off, qbytes, &S.mbar_q);
     }
     for (int i = tid; i < kFQPad; i += kFT) {
         qs[i] = 0.f;
         qs[kFQPad + nz4 + i] = 0.f;
     }
-    // per-thread copies: the 26 polynomial coefficients (seven 128-bit loads) and the fp32 constants of S2 (four)
+    // per-thread copies of the 26 polynomial coefficients, paired for the packed FMAs
     PolyCoef Cf;
     {
-        const float4* q = reinterpret_cast<const float4*>(pr);
-        float4 v[7];
-#pragma unroll
-        for (int k = 0; k < 7; ++k) v[k] = __ldg(q + k);
         const float* f = reinterpret_cast<const float*>(v);
 #pragma unroll
         for (int n = 0; n < kPolyN; ++n) Cf.zr[n] = pack2(f[2 * n], f[2 * n + 1]);
 #pragma unroll
         for (int n = 0; n < kPolyN - 1; ++n) Cf.ua[n] = pack2(f[2 * kPolyN + 2 * n], f[2 * kPolyN + 2 * n + 1]);
     }
-    LamF F;
-    load_lamf_hot(F, &Lg->F);
-    if (tid == 0) S.win = make_float4(F.win_lo, F.win_hi, F.two_dl2e, F.d2l2e);
     // the warp's chunk [c0, c1) of the (d_L-sorted) samples; its first two blocks of records are requested here, ahead of the
     // barrier and of the wait for the mass rows
     const int C = fast_chunk(ns);
     const int c0 = wid * C, c1 = min(c0 + C, ns);
-    const float4* pa = P.ev.prec_a + P.ev.poly_off[ev];
-    const float2* pb = P.ev.prec_b + P.ev.poly_off[ev];
+    const float4* pa = P.ev.prec_a + p0;
+    const float2* pb = P.ev.prec_b + p0;
     PRec R0, R1;
     {
         const int jf = min(c0, ns - 1) + lane;                          // (warps beyond the event read its last block and drop it)
@@ -267,18 +274,18 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     SW = __shfl_sync(0xffffffffu, SW, 0);
     SQ = __shfl_sync(0xffffffffu, SQ, 0);
     SB = __shfl_sync(0xffffffffu, SB, 0);
-    const float de = -SB / SW;                                          // minus the weighted mean (relative to z_mid)
+    const float de = -__fdividef(SB, SW);                                          // minus the weighted mean (relative to z_mid)
     float SA = f * fmaf(de, fmaf(de, wc, 2.f * bc), ac);                // sum w (u + de)^2 >= 0 per chunk
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1) SA += __shfl_xor_sync(0xffffffffu, SA, o);
     SA = __shfl_sync(0xffffffffu, SA, 0);
-    const float s2 = SQ / (SW * SW), neff = 1.0f / s2;                  // sum w^^2, Kish n_eff
-    double h;
+    const float s2 = __fdividef(SQ, SW * SW), neff = __fdividef(1.0f, s2);   // sum w^^2, Kish n_eff
+    float h;   // (fast divisions and MUFU powers: dh/h = 1e-6 moves log I by ~5e-9)
     if (P.bw_rule == CHIM_BW_FIXED) {
-        h = __ldg(P.ev.fixed_bw + ev);
+        h = (float)__ldg(P.ev.fixed_bw + ev);
     } else {   // Scott on the weighted sample (R3, O7): sigma^2 = sum w^(z - zbar)^2 / (1 - sum w^^2), h = sigma n_eff^(-1/5)
-        const float var = SA / (SW * (1.0f - s2));
-        h = (var > 0.f) ? (double)(sqrtf(var) * exp2f(0.2f * log2f(s2))) : NAN;
+        const float var = __fdividef(SA, SW * (1.0f - s2));
+        h = (var > 0.f) ? sqrtf(var) * ex2f(0.2f * lg2f(s2)) : NAN;
     }
     // handed over: no bandwidth; few effective samples (fp32 weights, moments and the plain form of Scott's rule are good for
     // n_eff >> 1 only); every supported secondary deep in the smoothing window (m2' < ~0.3 sqrt(delta): d ln w = delta/m2'^2 x 1e-6)
@@ -300,16 +307,16 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1) gmp2 = fmaxf(gmp2, __shfl_xor_sync(0xffffffffu, gmp2, o));
     gmp2 = __shfl_sync(0xffffffffu, gmp2, 0);
-    bool hand = !(h > 0.0) || !isfinite(h) || !(neff >= P.neff_min) || gmp2 < 0.f || gmp2 * gmp2 < 0.1f * F.delta;
+    bool hand = !(h > 0.f) || !isfinite(h) || !(neff >= P.neff_min) || gmp2 < 0.f || gmp2 * gmp2 < 0.1f * F.delta;
     // local-expansion geometry: y = z'/(sqrt(2) h), boxes of m grid spacings centred on grid points
     const double udz = __ldg(P.ev.uni_dz + ev), zfirst = __ldg(P.ev.zc + g0);
-    const float scy = (float)(0.70710678118654752440 / h);
+    const float scy = 0.70710678118654752440f / h;
     const float dy = (float)(udz * (double)scy);
-    const int m = max(1, (int)lrintf(1.0f / dy));
-    const float wbox = (float)m * dy, Ty = (float)(P.cutoff * 0.70710678118654752440);
-    const float yfirst = (float)(zfirst * (double)scy), inv_w = 1.0f / wbox;
+    const int m = max(1, (int)lrintf(__fdividef(1.0f, dy)));
+    const float wbox = (float)m * dy, Ty = (float)P.cutoff * 0.70710678118654752440f;
+    const float yfirst = (float)(zfirst * (double)scy), inv_w = __fdividef(1.0f, wbox);
     const float fb_lo = floorf((zw[0].x * scy - yfirst) * inv_w + 0.5f), fb_hi = floorf((zw[ns - 1].x * scy - yfirst) * inv_w + 0.5f);
-    const float fD = ceilf((Ty + 0.5f * wbox) / dy) + 1.0f;
+    const float fD = ceilf(__fdividef(Ty + 0.5f * wbox, dy)) + 1.0f;
     hand = hand || !(wbox <= kFMaxW) || !(fb_hi - fb_lo < (float)kFMaxBox) || !(fabsf(fb_lo) < 1e6f) || !(fabsf(fb_hi) < 1e6f) ||
            !(fD <= (float)kFMaxD) || !(fabsf(fb_lo) * (float)m < 1e8f) || !(fabsf(fb_hi) * (float)m < 1e8f);
     if (hand) CHIM_FAST_HANDOVER();
@@ -433,7 +440,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
 #pragma unroll
         for (int k = 0; k < kFW; ++k) tot += S.c_sum[k];                // fixed order: deterministic
         // K(z) = 1/(N_s h sqrt(2 pi)) sum_j w_j exp(..); the weights were divided by 2^gref, the prior and q_g scales factored out
-        const double I = tot / ((double)ns * h * 2.50662827463100050242);
+        const double I = tot / ((double)ns * (double)h * 2.50662827463100050242);
         if (I > 0.0 && isfinite(I)) {
             *out = log(I) + (double)gref * 0.69314718055994530942 + __ldg(P.ln_shift + ev) + __ldg(P.ln_qscale + ev);
         } else {   // nothing within the cut-off (or not a number): k_events evaluates the unit in log space
