@@ -34,7 +34,7 @@ ORACLE_KERNEL = [0, 0]        # oracle kernel id and bin count of the timed orac
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
-NCU_TRAFFIC_BYTES = 53.27e6 + 1.68e6   # k_events_fast, O5-spectroscopic, 256-lambda launch: dram read + write (profiles/r02)
+NCU_TRAFFIC_BYTES = 53.30e6 + 1.25e6   # k_events_fast, O5-spectroscopic, 256-lambda launch: dram read + write (profiles/r02_ncu_full.md)
 
 
 def default_workload(args):
@@ -411,7 +411,7 @@ def run_ours(args):
                          # SURVEY 8(d) recipe on what the kernel executes (ncu instruction counts x live time), and the issue slots
                          "executed": kb["roofline_k_events_fast"],
                          "traffic": (NCU_TRAFFIC_BYTES if default_workload(args) else None),
-                         "traffic_source": ("profiles/r02_k_events_fast_k_inject_ncu_full.md" if default_workload(args) else None),
+                         "traffic_source": ("profiles/r02_ncu_full.md" if default_workload(args) else None),
                          "algorithmic_dram_bytes_per_launch": alg_bytes,
                          "measured_alu_peaks_gops": r.get("alu"),
                          "peak_source": f"148 SM x 128 fp32 FMA lanes/clk x {clk_max:.0f} MHz ({peak_src} sm_max_mhz); see DESIGN.md sec. 6"},
