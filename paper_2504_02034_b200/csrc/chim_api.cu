@@ -521,6 +521,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     std::vector<float> qn(NG);
     std::vector<double> ep0(NG + n_events), ep1(NG + n_events), ep2(NG + n_events);   // Epanechnikov prefix sums
     std::vector<double> lm_lo(n_events), lm_hi(n_events);
+    const int fw = fast_warps_for(max_ns), fmd = fast_max_d_for(max_ns, max_nz);
     std::vector<float2> chunk_top((size_t)n_events * kFastWarps, make_float2(0.f, 1.f));   // k_events_fast: per chunk {largest m2d, t of its last sample}
     std::vector<double> tk_c(n_events), tk_h(n_events);
     std::vector<uint32_t> tkq_c(n_events);
@@ -566,7 +567,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
                 const double t = ((double)f_bits(rec[2 * js].x) - (double)tkq_c[i]) / (half * fq);
                 prec_a[p0 + j] = make_float4((float)h_m1[o], (float)h_m2[o], (float)t, (float)std::log(h_m1[o]));
                 if (j < ns) {
-                    float2& ct = chunk_top[(size_t)i * kFastWarps + std::min<int64_t>(j / fast_chunk((int)ns), kFastWarps - 1)];
+                    float2& ct = chunk_top[(size_t)i * kFastWarps + std::min<int64_t>(j / fast_chunk((int)ns, fw), fw - 1)];
                     ct.x = std::max(ct.x, (float)h_m2[o]);
                     ct.y = (float)t;                                   // (samples in d_L order: the last one written is the chunk's last)
                 }
@@ -614,7 +615,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     std::vector<float> qn4((size_t)q4n + 4, 0.f);
     for (int i = 0; i < n_events; ++i) std::copy(qn.begin() + go[i], qn.begin() + go[i + 1], qn4.begin() + q4off[i]);
     std::vector<int32_t> fast_ev, slow_ev;
-    const bool fast_fits = events_fast_smem_bytes(max_ns, max_nz) <= kMaxSmemOptin;
+    const bool fast_fits = events_fast_smem_bytes(max_ns, max_nz, fw, fmd) <= kMaxSmemOptin;
     for (int i = 0; i < n_events; ++i) (fast_fits && tk_h[i] > 0.0 && udz[i] > 0.0 ? fast_ev : slow_ev).push_back(i);
     // replace the previous set
     cudaStreamSynchronize(ctx->stream);
@@ -625,7 +626,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     drop_work(ctx);
     ctx->have_events = false;
     EventSetDev E{};
-    E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz;
+    E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz; E.fast_warps = fw; E.fast_max_d = fmd;
     CK(upload(ctx->owned_ev, &E.sample_off, so)); CK(upload(ctx->owned_ev, &E.grid_off, go));
     CK(upload(ctx->owned_ev, &E.rec, rec));
     CK(upload(ctx->owned_ev, &E.k_lo, k_lo)); CK(upload(ctx->owned_ev, &E.k_hi, k_hi));

@@ -458,9 +458,13 @@ __device__ __forceinline__ void ldg_stream_pair_after(PRec& R0, PRec& R1, const 
 
 // k_events_fast: eight warps, each on a contiguous chunk of the event's (d_L-sorted) samples; chunks are whole blocks of 32
 // samples, the evaluation takes them in passes of 128
-constexpr int kFastWarps = 8;
+constexpr int kFastWarps = 8;            // (the largest; small sample sets run with four)
 constexpr int kFastPass = 128;
-__host__ __device__ inline int fast_chunk(int ns) { return ((ns + kFastWarps * 32 - 1) / (kFastWarps * 32)) * 32; }   // whole blocks of 32
+__host__ __device__ inline int fast_chunk(int ns, int warps) { return ((ns + warps * 32 - 1) / (warps * 32)) * 32; }   // whole blocks of 32
+// warps per CTA and half-width cap of the psi table for an event set: sets of short sample lists (many-1d pixels) run four
+// warps per CTA and more CTAs per SM (their phases between the barriers are latency-bound); fine grids get a wider table
+__host__ inline int fast_warps_for(int max_ns) { return max_ns <= 2560 ? 4 : 8; }
+__host__ inline int fast_max_d_for(int max_ns, int max_nz) { return max_nz > 2048 ? 384 : (max_ns <= 2560 ? 160 : 256); }
 
 // ---- TMA bulk copy + mbarrier  ---------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -530,6 +534,7 @@ struct EventSetDev {
     const double* lnm1_lo;      // [n_events] smallest / largest ln m1d of the event's samples
     const double* lnm1_hi;
     const float2* chunk_top;    // [n_events][kFastWarps] k_events_fast: {largest m2d, t of the last sample} of every warp's chunk
+    int32_t fast_warps, fast_max_d;   // warps per CTA of k_events_fast for this set (chunk_top is laid out for it), psi-table cap
     const int32_t* k_lo;        // [n_events] first / last row of the z(ln d_L) table the event's samples address
     const int32_t* k_hi;
     const double* fixed_bw;     // [n_events] or null
@@ -637,7 +642,7 @@ cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int
 int events_mass_stage_rows(int n_mass);   // rows of the mass table a k_events CTA stages per variant
 cudaError_t launch_events(const EventKernelParams& P, bool count_pairs, cudaStream_t st);
 cudaError_t launch_events_fast(const FastEventParams& P, int n_fast, cudaStream_t st);
-size_t events_fast_smem_bytes(int max_ns, int max_nz);
+size_t events_fast_smem_bytes(int max_ns, int max_nz, int warps, int max_d);
 cudaError_t launch_inject(const InjKernelParams& P, int n_blocks, cudaStream_t st);
 cudaError_t launch_combine(const CombineParams& P, cudaStream_t st);
 cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, int64_t n, const double* dL,

@@ -23,18 +23,18 @@ namespace chim {
 #ifndef CHIM_FAST_BLOCKS
 #define CHIM_FAST_BLOCKS 3
 #endif
-constexpr int kFT = 32 * kFastWarps;  // threads per CTA
-constexpr int kFW = kFastWarps;      // warps = sample chunks
+// (threads per CTA kFT = 32 kFW, warps = sample chunks kFW: template parameter of the kernel, 8 or 4)
 constexpr int kFPass = kFastPass;    // samples per warp pass (4 per lane)
 constexpr int kFLeP = 12;            // terms of the local expansion
 constexpr int kFMaxBox = 96;         // boxes per event
 constexpr int kFBoxRec = 16;          // floats per box in shared memory: 12 coefficients, the box centre, 3 unused (64-byte records)
 constexpr int kFGroup = 5;            // boxes whose coefficients one warp builds at a time
 constexpr float kFMaxW = 1.3f;       // largest box width in units of sqrt(2) h
-constexpr int kFMaxD = 256;          // largest half-width of the psi table (grid points; ~60 on the spectroscopic, ~240 on the 4096-point photometric grids)
-constexpr int kFQPad = 2 * kFMaxD;   // zeros on both sides of the staged q_g: the coefficient build reads g_b +- d unchecked
+// largest half-width of the psi table: EventSetDev::fast_max_d (grid points; ~60 on the spectroscopic, ~240 on the 4096-point
+// photometric grids); 2 max_d zeros on both sides of the staged q_g: the coefficient build reads g_b +- d unchecked
 constexpr int kFMassStage = 384;     // mass-table rows staged per variant (>= events_mass_stage_rows: k_polyfit sizes the slice)
 
+template <int kFW>
 struct FastSmem {
     unsigned long long mbar_mass, mbar_q;
     float4 win;                      // the window constants of S(m2) {win_lo, win_hi, two_dl2e, d2l2e} (read inside the vote only)
@@ -45,21 +45,25 @@ struct FastSmem {
 };
 
 __host__ __device__ inline size_t fast_nz4(size_t nz) { return (nz + 3) / 4 * 4; }
-__host__ __device__ inline size_t fast_aux_bytes() {
+__host__ __device__ inline size_t fast_aux_bytes(int max_d) {
     const size_t a = 2 * (size_t)kFMassStage * sizeof(MassRow);
-    const size_t b = 4 * ((size_t)kFLeP * (size_t)(kFMaxD + 1) + (size_t)kFBoxRec * (size_t)kFMaxBox);
+    const size_t b = 4 * ((size_t)kFLeP * (size_t)(max_d + 1) + (size_t)kFBoxRec * (size_t)kFMaxBox);
     return a > b ? a : b;
 }
-size_t events_fast_smem_bytes(int max_ns, int max_nz) {
-    return ((sizeof(FastSmem) + 127) / 128) * 128 + sizeof(float2) * (size_t)kFW * fast_chunk(max_ns) +
-           sizeof(float) * (2 * (size_t)kFQPad + fast_nz4((size_t)max_nz)) + fast_aux_bytes();
+size_t events_fast_smem_bytes(int max_ns, int max_nz, int warps, int max_d) {
+    const size_t head = warps == 8 ? sizeof(FastSmem<8>) : sizeof(FastSmem<4>);
+    return ((head + 127) / 128) * 128 + sizeof(float2) * (size_t)warps * fast_chunk(max_ns, warps) +
+           sizeof(float) * (4 * (size_t)max_d + fast_nz4((size_t)max_nz)) + fast_aux_bytes(max_d);
 }
 
-__global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEventParams P) {
+template <int kFW, int kFMaxD>
+__global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : 6) k_events_fast(FastEventParams P) {
+    constexpr int kFT = 32 * kFW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    FastSmem& S = *reinterpret_cast<FastSmem*>(smem_raw);
-    float2* zw = reinterpret_cast<float2*>(smem_raw + ((sizeof(FastSmem) + 127) / 128) * 128);   // (z_j - z0, log2 w_j -> w_j)
-    float* qs = reinterpret_cast<float*>(zw + (size_t)kFW * fast_chunk(P.ev.max_ns));            // [kFQPad | nz4 | kFQPad]
+    FastSmem<kFW>& S = *reinterpret_cast<FastSmem<kFW>*>(smem_raw);
+    constexpr int kFQPad = 2 * kFMaxD;                                  // (kFMaxD = EventSetDev::fast_max_d of the set)
+    float2* zw = reinterpret_cast<float2*>(smem_raw + ((sizeof(FastSmem<kFW>) + 127) / 128) * 128);   // (z_j - z0, log2 w_j -> w_j)
+    float* qs = reinterpret_cast<float*>(zw + (size_t)kFW * fast_chunk(P.ev.max_ns, kFW));       // [kFQPad | nz4 | kFQPad]
     unsigned char* aux = reinterpret_cast<unsigned char*>(qs + 2 * (size_t)kFQPad + fast_nz4((size_t)P.ev.max_nz));
     MassRow* mass_s = reinterpret_cast<MassRow*>(aux);                  // S2: both variants of the event's slice of the mass table
     float* psi = reinterpret_cast<float*>(aux);                         // S3: psi table [(D+1) x 12] ...
@@ -138,7 +142,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     }
     // the warp's chunk [c0, c1) of the (d_L-sorted) samples; its first two blocks of records are requested here, ahead of the
     // barrier and of the wait for the mass rows
-    const int C = fast_chunk(ns);
+    const int C = fast_chunk(ns, kFW);
     const int c0 = wid * C, c1 = min(c0 + C, ns);
     const float4* pa = P.ev.prec_a + p0;
     const float2* pb = P.ev.prec_b + p0;
@@ -255,7 +259,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     const float cm = (lane < kFW) ? S.c_ref[lane] : -INFINITY;
     float gref = cm;
 #pragma unroll
-    for (int o = 4; o > 0; o >>= 1) gref = fmaxf(gref, __shfl_xor_sync(0xffffffffu, gref, o));
+    for (int o = kFW / 2; o > 0; o >>= 1) gref = fmaxf(gref, __shfl_xor_sync(0xffffffffu, gref, o));
     gref = __shfl_sync(0xffffffffu, gref, 0);
     mbar_wait(&S.mbar_q, 0);                                            // q_g has landed (also: no copy in flight at any exit below)
     if (!(gref > -INFINITY)) CHIM_FAST_HANDOVER();                      // no weighted sample on this path: k_events decides
@@ -266,7 +270,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     if (wid == 0 && lane < kFW) S.c_f[lane] = f;
     float SW = f * wc, SQ = f * f * qc, SB = f * bc;
 #pragma unroll
-    for (int o = 4; o > 0; o >>= 1) {
+    for (int o = kFW / 2; o > 0; o >>= 1) {
         SW += __shfl_xor_sync(0xffffffffu, SW, o);
         SQ += __shfl_xor_sync(0xffffffffu, SQ, o);
         SB += __shfl_xor_sync(0xffffffffu, SB, o);
@@ -277,7 +281,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     const float de = -__fdividef(SB, SW);                                          // minus the weighted mean (relative to z_mid)
     float SA = f * fmaf(de, fmaf(de, wc, 2.f * bc), ac);                // sum w (u + de)^2 >= 0 per chunk
 #pragma unroll
-    for (int o = 4; o > 0; o >>= 1) SA += __shfl_xor_sync(0xffffffffu, SA, o);
+    for (int o = kFW / 2; o > 0; o >>= 1) SA += __shfl_xor_sync(0xffffffffu, SA, o);
     SA = __shfl_sync(0xffffffffu, SA, 0);
     const float s2 = __fdividef(SQ, SW * SW), neff = __fdividef(1.0f, s2);   // sum w^^2, Kish n_eff
     float h;   // (fast divisions and MUFU powers: dh/h = 1e-6 moves log I by ~5e-9)
@@ -293,7 +297,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
     // end, where 1/(1+z) is smallest (within 0.5 % of the exact value; the unit is handed over whenever the exact criterion would)
     float gmp2 = -INFINITY;
     if (lane < kFW) {
-        const float2 ct = __ldg(P.ev.chunk_top + (size_t)ev * kFW + lane);   // {largest m2d, t of the last sample} of chunk `lane`
+        const float2 ct = __ldg(P.ev.chunk_top + (size_t)ev * kFastWarps + lane);   // {largest m2d, t of the last sample} of chunk `lane`
         float un, a1;
         unpack2(Cf.ua[kPolyN - 2], un, a1);
 #pragma unroll
@@ -305,7 +309,7 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
         gmp2 = fmaf(ct.x, a1, -F.mlow_hi);                               // (empty chunks: m2d = 0)
     }
 #pragma unroll
-    for (int o = 4; o > 0; o >>= 1) gmp2 = fmaxf(gmp2, __shfl_xor_sync(0xffffffffu, gmp2, o));
+    for (int o = kFW / 2; o > 0; o >>= 1) gmp2 = fmaxf(gmp2, __shfl_xor_sync(0xffffffffu, gmp2, o));
     gmp2 = __shfl_sync(0xffffffffu, gmp2, 0);
     bool hand = !(h > 0.f) || !isfinite(h) || !(neff >= P.neff_min) || gmp2 < 0.f || gmp2 * gmp2 < 0.1f * F.delta;
     // local-expansion geometry: y = z'/(sqrt(2) h), boxes of m grid spacings centred on grid points
@@ -451,14 +455,25 @@ __global__ void __launch_bounds__(kFT, CHIM_FAST_BLOCKS) k_events_fast(FastEvent
 #undef CHIM_FAST_HANDOVER
 }
 
+template <int kFW, int kFMaxD>
+static cudaError_t launch_fast_t(const FastEventParams& P, long long nb, size_t smem, cudaStream_t st) {
+    cudaError_t e = cudaFuncSetAttribute(k_events_fast<kFW, kFMaxD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_events_fast<kFW, kFMaxD><<<(unsigned)nb, 32 * kFW, smem, st>>>(P);
+    return cudaGetLastError();
+}
+
+// the instantiations fast_warps_for() / fast_max_d_for() (chim_internal.cuh) can ask for
 cudaError_t launch_events_fast(const FastEventParams& P, int n_fast, cudaStream_t st) {
     const long long nb = (long long)P.n_lambda * n_fast;
     if (nb <= 0) return cudaSuccess;
-    const size_t smem = events_fast_smem_bytes(P.ev.max_ns, P.ev.max_nz);
-    cudaError_t e = cudaFuncSetAttribute(k_events_fast, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    k_events_fast<<<(unsigned)nb, kFT, smem, st>>>(P);
-    return cudaGetLastError();
+    const int w = P.ev.fast_warps, d = P.ev.fast_max_d;
+    const size_t smem = events_fast_smem_bytes(P.ev.max_ns, P.ev.max_nz, w, d);
+    if (w == 8 && d == 256) return launch_fast_t<8, 256>(P, nb, smem, st);
+    if (w == 8 && d == 384) return launch_fast_t<8, 384>(P, nb, smem, st);
+    if (w == 4 && d == 160) return launch_fast_t<4, 160>(P, nb, smem, st);
+    if (w == 4 && d == 384) return launch_fast_t<4, 384>(P, nb, smem, st);
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace chim
