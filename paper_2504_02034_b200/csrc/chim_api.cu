@@ -55,6 +55,7 @@ struct chim_ctx {
     // k_events_fast: the events it takes / leaves to k_events, and the per-chunk work list of the units it hands over
     const int32_t* fast_ev = nullptr; const int32_t* slow_ev = nullptr;
     int n_fast = 0, n_slow = 0;
+    int n_fast_c[2] = {0, 0}, max_ns_c[2] = {0, 0};   // the two classes of k_events_fast (4 / 8 warps): events, longest sample list
     uint32_t* worklist = nullptr; unsigned int* work_count = nullptr;
     // staging for the host-pointer entry point
     int host_nl = 0;
@@ -273,8 +274,13 @@ int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* 
         FP.logI = ctx->logI; FP.ln_shift = ctx->ev_ln_shift; FP.ln_qscale = ctx->ev_ln_qscale;
         FP.fast_events = ctx->fast_ev; FP.worklist = ctx->worklist; FP.work_count = ctx->work_count;
         CK(cudaMemsetAsync(ctx->work_count, 0, sizeof(unsigned int), st));
-        { Bracket b(ctx, 1); CK(launch_events_fast(FP, ctx->n_fast, st)); }
-        ctx->launches += 1;
+        for (int c = 0, first = 0; c < 2; first += ctx->n_fast_c[c], ++c) {
+            if (ctx->n_fast_c[c] == 0) continue;
+            FP.fast_events = ctx->fast_ev + first;
+            FP.warps = c == 0 ? 4 : 8; FP.max_d = fast_max_d_for(FP.warps, ctx->ev.max_nz); FP.max_ns = ctx->max_ns_c[c];
+            { Bracket b(ctx, 1); CK(launch_events_fast(FP, ctx->n_fast_c[c], st)); }
+            ctx->launches += 1;
+        }
         if (ctx->n_slow > 0) {
             EP.ev_list = ctx->slow_ev; EP.n_ev_list = ctx->n_slow;
             { Bracket b(ctx, 4); CK(launch_events(EP, false, st)); }
@@ -521,7 +527,6 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     std::vector<float> qn(NG);
     std::vector<double> ep0(NG + n_events), ep1(NG + n_events), ep2(NG + n_events);   // Epanechnikov prefix sums
     std::vector<double> lm_lo(n_events), lm_hi(n_events);
-    const int fw = fast_warps_for(max_ns), fmd = fast_max_d_for(max_ns, max_nz);
     std::vector<float2> chunk_top((size_t)n_events * kFastWarps, make_float2(0.f, 1.f));   // k_events_fast: per chunk {largest m2d, t of its last sample}
     std::vector<double> tk_c(n_events), tk_h(n_events);
     std::vector<uint32_t> tkq_c(n_events);
@@ -567,7 +572,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
                 const double t = ((double)f_bits(rec[2 * js].x) - (double)tkq_c[i]) / (half * fq);
                 prec_a[p0 + j] = make_float4((float)h_m1[o], (float)h_m2[o], (float)t, (float)std::log(h_m1[o]));
                 if (j < ns) {
-                    float2& ct = chunk_top[(size_t)i * kFastWarps + std::min<int64_t>(j / fast_chunk((int)ns, fw), fw - 1)];
+                    float2& ct = chunk_top[(size_t)i * kFastWarps + std::min<int64_t>(j / fast_chunk((int)ns, fast_warps_for((int)ns)), fast_warps_for((int)ns) - 1)];
                     ct.x = std::max(ct.x, (float)h_m2[o]);
                     ct.y = (float)t;                                   // (samples in d_L order: the last one written is the chunk's last)
                 }
@@ -614,9 +619,22 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     for (int i = 0; i < n_events; ++i) { q4off[i] = q4n; q4n += ((go[i + 1] - go[i] + 3) / 4) * 4; }
     std::vector<float> qn4((size_t)q4n + 4, 0.f);
     for (int i = 0; i < n_events; ++i) std::copy(qn.begin() + go[i], qn.begin() + go[i + 1], qn4.begin() + q4off[i]);
+    // k_events_fast takes the events with a narrow d_L range on an equally spaced grid, in two classes by the length of the
+    // sample list (chim_internal.cuh: fast_warps_for), the four-warp class first in the list
     std::vector<int32_t> fast_ev, slow_ev;
-    const bool fast_fits = events_fast_smem_bytes(max_ns, max_nz, fw, fmd) <= kMaxSmemOptin;
-    for (int i = 0; i < n_events; ++i) (fast_fits && tk_h[i] > 0.0 && udz[i] > 0.0 ? fast_ev : slow_ev).push_back(i);
+    int n_fast_c[2] = {0, 0}, max_ns_c[2] = {0, 0};
+    for (int c = 0; c < 2; ++c) {
+        const int w = c == 0 ? 4 : 8;
+        for (int i = 0; i < n_events; ++i)
+            if (fast_warps_for((int)(so[i + 1] - so[i])) == w) max_ns_c[c] = std::max(max_ns_c[c], (int)(so[i + 1] - so[i]));
+        const bool fits = events_fast_smem_bytes(max_ns_c[c], max_nz, w, fast_max_d_for(w, max_nz)) <= kMaxSmemOptin;
+        for (int i = 0; i < n_events; ++i) {
+            if (fast_warps_for((int)(so[i + 1] - so[i])) != w) continue;
+            if (fits && tk_h[i] > 0.0 && udz[i] > 0.0) { fast_ev.push_back(i); ++n_fast_c[c]; }
+            else slow_ev.push_back(i);
+        }
+    }
+    std::sort(slow_ev.begin(), slow_ev.end());
     // replace the previous set
     cudaStreamSynchronize(ctx->stream);
     free_pool(ctx->owned_grp);
@@ -626,7 +644,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     drop_work(ctx);
     ctx->have_events = false;
     EventSetDev E{};
-    E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz; E.fast_warps = fw; E.fast_max_d = fmd;
+    E.n_events = n_events; E.max_ns = max_ns; E.max_nz = max_nz;
     CK(upload(ctx->owned_ev, &E.sample_off, so)); CK(upload(ctx->owned_ev, &E.grid_off, go));
     CK(upload(ctx->owned_ev, &E.rec, rec));
     CK(upload(ctx->owned_ev, &E.k_lo, k_lo)); CK(upload(ctx->owned_ev, &E.k_hi, k_hi));
@@ -641,6 +659,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     CK(upload(ctx->owned_ev, &E.qn4, qn4)); CK(upload(ctx->owned_ev, &E.q4_off, q4off));
     CK(upload(ctx->owned_ev, &ctx->fast_ev, fast_ev)); CK(upload(ctx->owned_ev, &ctx->slow_ev, slow_ev));
     ctx->n_fast = (int)fast_ev.size(); ctx->n_slow = (int)slow_ev.size();
+    for (int c = 0; c < 2; ++c) { ctx->n_fast_c[c] = n_fast_c[c]; ctx->max_ns_c[c] = max_ns_c[c]; }
     CK(upload(ctx->owned_ev, &ctx->ev_ln_shift, shift));
     CK(upload(ctx->owned_ev, &ctx->ev_ln_qscale, qshift));
     ctx->ev = E;

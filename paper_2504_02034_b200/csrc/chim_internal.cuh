@@ -461,10 +461,12 @@ __device__ __forceinline__ void ldg_stream_pair_after(PRec& R0, PRec& R1, const 
 constexpr int kFastWarps = 8;            // (the largest; small sample sets run with four)
 constexpr int kFastPass = 128;
 __host__ __device__ inline int fast_chunk(int ns, int warps) { return ((ns + warps * 32 - 1) / (warps * 32)) * 32; }   // whole blocks of 32
-// warps per CTA and half-width cap of the psi table for an event set: sets of short sample lists (many-1d pixels) run four
-// warps per CTA and more CTAs per SM (their phases between the barriers are latency-bound); fine grids get a wider table
-__host__ inline int fast_warps_for(int max_ns) { return max_ns <= 2560 ? 4 : 8; }
-__host__ inline int fast_max_d_for(int max_ns, int max_nz) { return max_nz > 2048 ? 384 : (max_ns <= 2560 ? 160 : 256); }
+// Two classes of events, each with its own launch: short sample lists (many-1d pixels) run four warps per CTA and more CTAs per
+// SM -- their phases between the barriers are latency-bound -- long ones eight.  Half-width cap of the psi table per class:
+// fine grids get a wider table, short lists (wider kernels relative to the grid) a narrower stage.
+constexpr int kFastSmallNs = 1280;
+__host__ inline int fast_warps_for(int ns) { return ns <= kFastSmallNs ? 4 : 8; }
+__host__ inline int fast_max_d_for(int warps, int max_nz) { return max_nz > 2048 ? 384 : (warps == 4 ? 160 : 256); }
 
 // ---- TMA bulk copy + mbarrier  ---------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -534,7 +536,7 @@ struct EventSetDev {
     const double* lnm1_lo;      // [n_events] smallest / largest ln m1d of the event's samples
     const double* lnm1_hi;
     const float2* chunk_top;    // [n_events][kFastWarps] k_events_fast: {largest m2d, t of the last sample} of every warp's chunk
-    int32_t fast_warps, fast_max_d;   // warps per CTA of k_events_fast for this set (chunk_top is laid out for it), psi-table cap
+                                // (laid out for the warps of the event's class: fast_warps_for(N_s))
     const int32_t* k_lo;        // [n_events] first / last row of the z(ln d_L) table the event's samples address
     const int32_t* k_hi;
     const double* fixed_bw;     // [n_events] or null
@@ -590,7 +592,8 @@ struct FastEventParams {
     double cutoff;
     double* logI;            // [n_lambda][n_events]
     const double* ln_shift; const double* ln_qscale;
-    const int32_t* fast_events;   // the events this kernel takes (narrow d_L range, equally spaced grid)
+    const int32_t* fast_events;   // the events this launch takes (narrow d_L range, equally spaced grid; one class)
+    int32_t warps, max_d, max_ns; // the class: warps per CTA, psi-table cap, longest sample list (sizes the shared memory)
     uint32_t* worklist; unsigned int* work_count;
 };
 

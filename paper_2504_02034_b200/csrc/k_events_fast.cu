@@ -30,7 +30,7 @@ constexpr int kFMaxBox = 96;         // boxes per event
 constexpr int kFBoxRec = 16;          // floats per box in shared memory: 12 coefficients, the box centre, 3 unused (64-byte records)
 constexpr int kFGroup = 5;            // boxes whose coefficients one warp builds at a time
 constexpr float kFMaxW = 1.3f;       // largest box width in units of sqrt(2) h
-// largest half-width of the psi table: EventSetDev::fast_max_d (grid points; ~60 on the spectroscopic, ~240 on the 4096-point
+// largest half-width of the psi table: FastEventParams::max_d (grid points; ~60 on the spectroscopic, ~240 on the 4096-point
 // photometric grids); 2 max_d zeros on both sides of the staged q_g: the coefficient build reads g_b +- d unchecked
 constexpr int kFMassStage = 384;     // mass-table rows staged per variant (>= events_mass_stage_rows: k_polyfit sizes the slice)
 
@@ -61,9 +61,9 @@ __global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : 6) k_e
     constexpr int kFT = 32 * kFW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     FastSmem<kFW>& S = *reinterpret_cast<FastSmem<kFW>*>(smem_raw);
-    constexpr int kFQPad = 2 * kFMaxD;                                  // (kFMaxD = EventSetDev::fast_max_d of the set)
+    constexpr int kFQPad = 2 * kFMaxD;                                  // (kFMaxD = the cap of the launch's class)
     float2* zw = reinterpret_cast<float2*>(smem_raw + ((sizeof(FastSmem<kFW>) + 127) / 128) * 128);   // (z_j - z0, log2 w_j -> w_j)
-    float* qs = reinterpret_cast<float*>(zw + (size_t)kFW * fast_chunk(P.ev.max_ns, kFW));       // [kFQPad | nz4 | kFQPad]
+    float* qs = reinterpret_cast<float*>(zw + (size_t)kFW * fast_chunk(P.max_ns, kFW));          // [kFQPad | nz4 | kFQPad]
     unsigned char* aux = reinterpret_cast<unsigned char*>(qs + 2 * (size_t)kFQPad + fast_nz4((size_t)P.ev.max_nz));
     MassRow* mass_s = reinterpret_cast<MassRow*>(aux);                  // S2: both variants of the event's slice of the mass table
     float* psi = reinterpret_cast<float*>(aux);                         // S3: psi table [(D+1) x 12] ...
@@ -467,8 +467,8 @@ static cudaError_t launch_fast_t(const FastEventParams& P, long long nb, size_t 
 cudaError_t launch_events_fast(const FastEventParams& P, int n_fast, cudaStream_t st) {
     const long long nb = (long long)P.n_lambda * n_fast;
     if (nb <= 0) return cudaSuccess;
-    const int w = P.ev.fast_warps, d = P.ev.fast_max_d;
-    const size_t smem = events_fast_smem_bytes(P.ev.max_ns, P.ev.max_nz, w, d);
+    const int w = P.warps, d = P.max_d;
+    const size_t smem = events_fast_smem_bytes(P.max_ns, P.ev.max_nz, w, d);
     if (w == 8 && d == 256) return launch_fast_t<8, 256>(P, nb, smem, st);
     if (w == 8 && d == 384) return launch_fast_t<8, 384>(P, nb, smem, st);
     if (w == 4 && d == 160) return launch_fast_t<4, 160>(P, nb, smem, st);
