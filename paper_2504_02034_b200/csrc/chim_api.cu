@@ -52,6 +52,12 @@ struct chim_ctx {
     double* dc_tab = nullptr; double* logI = nullptr; double2* partial = nullptr; uint32_t* flags = nullptr;
     unsigned long long* stats = nullptr;
     float* poly_ev = nullptr; float* poly_inj = nullptr;   // local polynomials per (lambda, event) / (lambda, chunk)
+    // S1 of the next lambda chunk runs on a stream of its own while S2-S6 of the current one fill the SMs (k_tables / k_polyfit
+    // are latency-bound: few CTAs, many barriers): two sets of the S1 outputs, the pointers above name the set in use
+    struct S1Set { LamConst* Lc; Row* tab_ev; Row* tab_inj; MassRow* mtab; double* dc_tab; float* poly_ev; float* poly_inj; };
+    S1Set s1[2] = {};
+    cudaStream_t aux_stream = nullptr;
+    cudaEvent_t ev_begin = nullptr, ev_s1[2] = {nullptr, nullptr}, ev_rest[2] = {nullptr, nullptr};
     // k_events_fast: the events it takes / leaves to k_events, and the per-chunk work list of the units it hands over
     const int32_t* fast_ev = nullptr; const int32_t* slow_ev = nullptr;
     int n_fast = 0, n_slow = 0;
@@ -153,6 +159,7 @@ void drop_work(chim_ctx* ctx) {
     ctx->Lc = nullptr; ctx->tab_ev = nullptr; ctx->tab_inj = nullptr; ctx->mtab = nullptr; ctx->dc_tab = nullptr;
     ctx->logI = nullptr; ctx->partial = nullptr; ctx->flags = nullptr; ctx->stats = nullptr;
     ctx->poly_ev = nullptr; ctx->poly_inj = nullptr;
+    ctx->s1[0] = chim_ctx::S1Set{}; ctx->s1[1] = chim_ctx::S1Set{};
     ctx->worklist = nullptr; ctx->work_count = nullptr;
     free_pool(ctx->owned_host);
     ctx->host_nl = 0;
@@ -188,9 +195,27 @@ int ensure_work(chim_ctx* ctx, int nl) {
     CK(dev_alloc(ctx->owned_work, &ctx->poly_inj, (size_t)nl * std::max(ctx->inj_blocks, 1) * 4 * kPolyN));
     CK(dev_alloc(ctx->owned_work, &ctx->worklist, (size_t)nl * ctx->ev.n_events));
     CK(dev_alloc(ctx->owned_work, &ctx->work_count, 4));
+    ctx->s1[0] = chim_ctx::S1Set{ctx->Lc, ctx->tab_ev, ctx->tab_inj, ctx->mtab, ctx->dc_tab, ctx->poly_ev, ctx->poly_inj};
+    {   // the second set of the S1 outputs
+        chim_ctx::S1Set& B = ctx->s1[1];
+        CK(dev_alloc(ctx->owned_work, &B.Lc, nl));
+        CK(dev_alloc(ctx->owned_work, &B.tab_ev, (size_t)nl * ctx->ev_grid.rows()));
+        CK(dev_alloc(ctx->owned_work, &B.tab_inj, (size_t)nl * (ctx->have_inj ? ctx->inj_grid.rows() : 1)));
+        CK(dev_alloc(ctx->owned_work, &B.mtab, (size_t)nl * 2 * (ctx->cfg.n_mass_table + 2)));
+        B.dc_tab = nullptr;
+        if (need_dc) CK(dev_alloc(ctx->owned_work, &B.dc_tab, (size_t)nl * (ctx->cfg.n_table + 1 + kZPad)));
+        CK(dev_alloc(ctx->owned_work, &B.poly_ev, (size_t)nl * ctx->ev.n_events * 4 * kPolyN));
+        CK(dev_alloc(ctx->owned_work, &B.poly_inj, (size_t)nl * std::max(ctx->inj_blocks, 1) * 4 * kPolyN));
+    }
     ctx->work_nl = nl;
     ctx->work_has_dc = need_dc;
     return CHIM_OK;
+}
+
+void use_s1_set(chim_ctx* ctx, int k) {
+    const chim_ctx::S1Set& B = ctx->s1[k];
+    ctx->Lc = B.Lc; ctx->tab_ev = B.tab_ev; ctx->tab_inj = B.tab_inj; ctx->mtab = B.mtab; ctx->dc_tab = B.dc_tab;
+    ctx->poly_ev = B.poly_ev; ctx->poly_inj = B.poly_inj;
 }
 
 TableParams table_params(const chim_ctx* ctx) {
@@ -242,24 +267,35 @@ struct Bracket {
     ~Bracket() { if (on) cudaEventRecord(ctx->ev_pool[2 * slot + 1], ctx->stream); }
 };
 
-// one pass over a chunk of lambdas: S1 -> S2-S4 -> S5 -> S6
-int run_chunk(chim_ctx* ctx, int nl, const double* lam, double* out_ll, double* out_ev, double* out_xi, double* out_neff,
-              uint32_t* out_fl) {
-    cudaStream_t st = ctx->stream;
+// S1 of one chunk of lambdas into the set of buffers in use, on stream `st` (timed only when it is the context's stream)
+int run_s1(chim_ctx* ctx, int nl, const double* lam, cudaStream_t st) {
     TableParams TP = table_params(ctx);
+    const bool timed = st == ctx->stream;
+    const bool prof = ctx->profiling;
+    if (!timed) ctx->profiling = false;
+    int rc = [&]() -> int {
+        { Bracket b(ctx, 0); CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, st)); }
+        {   // local-polynomial fits (part of S1: per-lambda interpolants)
+            Bracket b(ctx, 0);
+            CK(launch_polyfit(ctx->Lc, ctx->tab_ev, ctx->ev_grid.rows(), nl, ctx->ev.n_events, ctx->ev.tk_c, ctx->ev.tk_h, ctx->ev.z0, 0.0,
+                              false, ctx->poly_mats, ctx->ev.lnm1_lo, ctx->ev.lnm1_hi, ctx->cfg.n_mass_table,
+                              events_mass_stage_rows(ctx->cfg.n_mass_table), ctx->ev_grid.dx, ctx->poly_ev, st));
+            if (ctx->have_inj)
+                CK(launch_polyfit(ctx->Lc, ctx->tab_inj, ctx->inj_grid.rows(), nl, ctx->inj_blocks, ctx->inj.tk_c, ctx->inj.tk_h, nullptr,
+                                  ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->inj_grid.dx, ctx->poly_inj, st));
+            ctx->launches += ctx->have_inj ? 2 : 1;
+        }
+        ctx->launches += 1;   // (k_tables)
+        return CHIM_OK;
+    }();
+    ctx->profiling = prof;
+    return rc;
+}
+
+// S2-S4 -> S5 -> S6 of one chunk on the context's stream, from the set of S1 outputs in use
+int run_rest(chim_ctx* ctx, int nl, double* out_ll, double* out_ev, double* out_xi, double* out_neff, uint32_t* out_fl) {
+    cudaStream_t st = ctx->stream;
     CK(cudaMemsetAsync(ctx->flags, 0, sizeof(uint32_t) * nl, st));
-    { Bracket b(ctx, 0); CK(launch_tables(lam, nl, TP, ctx->Lc, ctx->dc_tab, ctx->tab_ev, ctx->tab_inj, ctx->mtab, st)); }
-    {   // local-polynomial fits (part of S1: per-lambda interpolants)
-        Bracket b(ctx, 0);
-        CK(launch_polyfit(ctx->Lc, ctx->tab_ev, ctx->ev_grid.rows(), nl, ctx->ev.n_events, ctx->ev.tk_c, ctx->ev.tk_h, ctx->ev.z0, 0.0,
-                          false, ctx->poly_mats, ctx->ev.lnm1_lo, ctx->ev.lnm1_hi, ctx->cfg.n_mass_table,
-                          events_mass_stage_rows(ctx->cfg.n_mass_table), ctx->ev_grid.dx, ctx->poly_ev, st));
-        if (ctx->have_inj)
-            CK(launch_polyfit(ctx->Lc, ctx->tab_inj, ctx->inj_grid.rows(), nl, ctx->inj_blocks, ctx->inj.tk_c, ctx->inj.tk_h, nullptr,
-                              ctx->cfg.z_cat_max, true, ctx->poly_mats, nullptr, nullptr, 0, 0, ctx->inj_grid.dx, ctx->poly_inj, st));
-        ctx->launches += ctx->have_inj ? 2 : 1;
-    }
-    ctx->launches += 1;   // (k_tables)
     EventKernelParams EP = event_params(ctx, nl);
     const chim_config& cf = ctx->cfg;
     // the regular units go to k_events_fast: default configuration (Gaussian kernel, local-expansion form, weights on the samples,
@@ -433,6 +469,13 @@ int chim_create(const chim_config* cfg, chim_ctx** out) {
     }
     ce = upload_gauss_legendre();
     if (ce == cudaSuccess) ce = upload_poly_matrices(ctx);
+    if (ce == cudaSuccess) {   // the auxiliary stream of S1 (highest priority: its few CTAs go ahead of the queued S2-S5 ones) and its events
+        int pr_lo = 0, pr_hi = 0;
+        cudaDeviceGetStreamPriorityRange(&pr_lo, &pr_hi);
+        ce = cudaStreamCreateWithPriority(&ctx->aux_stream, cudaStreamNonBlocking, pr_hi);
+        cudaEvent_t* evs[5] = {&ctx->ev_begin, &ctx->ev_s1[0], &ctx->ev_s1[1], &ctx->ev_rest[0], &ctx->ev_rest[1]};
+        for (int i = 0; i < 5 && ce == cudaSuccess; ++i) ce = cudaEventCreateWithFlags(evs[i], cudaEventDisableTiming);
+    }
     if (ce != cudaSuccess) {
         chim_destroy(ctx);
         return fail(nullptr, ce == cudaErrorMemoryAllocation ? CHIM_ENOMEM : CHIM_ECUDA, std::string("chim_create: ") + cudaGetErrorString(ce));
@@ -445,6 +488,9 @@ void chim_destroy(chim_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->cfg.device);
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->aux_stream) { cudaStreamSynchronize(ctx->aux_stream); cudaStreamDestroy(ctx->aux_stream); }
+    for (cudaEvent_t e : {ctx->ev_begin, ctx->ev_s1[0], ctx->ev_s1[1], ctx->ev_rest[0], ctx->ev_rest[1]})
+        if (e) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     free_pool(ctx->owned_ev);
     free_pool(ctx->owned_inj);
@@ -901,14 +947,43 @@ int chim_loglike_batch(chim_ctx* ctx, int32_t n_lambda, const double* lambda, do
     ctx->launches = 0;
     ctx->ev_kind.clear();
     CK(cudaMemsetAsync(ctx->stats, 0, 4 * sizeof(unsigned long long), ctx->stream));
-    for (int c0 = 0; c0 < n_lambda; c0 += chunk) {
-        const int nl = std::min(chunk, n_lambda - c0);
-        rc = run_chunk(ctx, nl, lambda + (size_t)c0 * CHIM_N_LAMBDA_PARAMS, out_loglike + c0,
-                       out_event_logI ? out_event_logI + (size_t)c0 * ctx->ev.n_events : nullptr,
-                       out_logxi ? out_logxi + c0 : nullptr, out_neff ? out_neff + c0 : nullptr,
-                       out_flags ? out_flags + c0 : nullptr);
+    const int n_chunks = (n_lambda + chunk - 1) / chunk;
+    // several chunks: S1 of chunk c + 1 on the auxiliary stream while S2-S6 of chunk c run (with per-kernel timing on, everything
+    // stays on the context's stream, one kernel after the other, so that the times add up)
+    const bool overlap = n_chunks > 1 && !ctx->profiling && ctx->aux_stream != nullptr;
+    auto lam_of = [&](int c) { return lambda + (size_t)c * chunk * CHIM_N_LAMBDA_PARAMS; };
+    auto nl_of = [&](int c) { return std::min(chunk, n_lambda - c * chunk); };
+    if (overlap) {
+        CK(cudaEventRecord(ctx->ev_begin, ctx->stream));
+        CK(cudaStreamWaitEvent(ctx->aux_stream, ctx->ev_begin, 0));
+        use_s1_set(ctx, 0);
+        rc = run_s1(ctx, nl_of(0), lam_of(0), ctx->aux_stream);
         if (rc != CHIM_OK) return rc;
+        CK(cudaEventRecord(ctx->ev_s1[0], ctx->aux_stream));
     }
+    for (int c = 0; c < n_chunks; ++c) {
+        const int c0 = c * chunk, nl = nl_of(c), k = c & 1;
+        if (overlap) {
+            CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_s1[k], 0));
+            if (c + 1 < n_chunks) {
+                if (c >= 1) CK(cudaStreamWaitEvent(ctx->aux_stream, ctx->ev_rest[k ^ 1], 0));   // (chunk c - 1 has left that set)
+                use_s1_set(ctx, k ^ 1);
+                rc = run_s1(ctx, nl_of(c + 1), lam_of(c + 1), ctx->aux_stream);
+                if (rc != CHIM_OK) return rc;
+                CK(cudaEventRecord(ctx->ev_s1[k ^ 1], ctx->aux_stream));
+            }
+            use_s1_set(ctx, k);
+        } else {
+            use_s1_set(ctx, 0);
+            rc = run_s1(ctx, nl, lam_of(c), ctx->stream);
+            if (rc != CHIM_OK) return rc;
+        }
+        rc = run_rest(ctx, nl, out_loglike + c0, out_event_logI ? out_event_logI + (size_t)c0 * ctx->ev.n_events : nullptr,
+                      out_logxi ? out_logxi + c0 : nullptr, out_neff ? out_neff + c0 : nullptr, out_flags ? out_flags + c0 : nullptr);
+        if (rc != CHIM_OK) return rc;
+        if (overlap) CK(cudaEventRecord(ctx->ev_rest[k], ctx->stream));
+    }
+    use_s1_set(ctx, 0);
     ctx->last.kde_pairs_dense = 0;
     for (int i = 0; i < ctx->ev.n_events; ++i)
         ctx->last.kde_pairs_dense += (uint64_t)(ctx->h_sample_off[i + 1] - ctx->h_sample_off[i]) *
