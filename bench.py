@@ -34,12 +34,12 @@ ORACLE_KERNEL = [0, 0]        # oracle kernel id and bin count of the timed orac
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
-NCU_TRAFFIC_BYTES = 53.30e6 + 1.25e6   # k_events_fast, O5-spectroscopic, 256-lambda launch: dram read + write (profiles/r02_ncu_full.md)
+NCU_TRAFFIC_BYTES = 102.8e6 + 6.5e6   # k_events_fast, O5-spectroscopic, 1024-lambda launch: dram read + write (profiles/r02_ncu_full.md)
 
 
 def default_workload(args):
     return (args.config == "o5_spec" and args.catalog == 0 and not (args.n_events or args.n_det or args.n_lambda)
-            and args.pixels == 0 and args.bins == 0 and args.kde_kernel == "gauss" and args.lambda_chunk == 256)
+            and args.pixels == 0 and args.bins == 0 and args.kde_kernel == "gauss" and args.lambda_chunk == 1024)
 
 
 def load_peaks():
@@ -459,7 +459,7 @@ def main():
     ap.add_argument("--config", default="o5_spec")
     ap.add_argument("--catalog", type=int, default=0)
     ap.add_argument("--cutoff", type=float, default=6.0)
-    ap.add_argument("--lambda-chunk", type=int, default=256)
+    ap.add_argument("--lambda-chunk", type=int, default=1024)
     ap.add_argument("--n-events", type=int, default=0, help="override (debug only; invalidates the number)")
     ap.add_argument("--n-det", type=int, default=0, help="override (debug only)")
     ap.add_argument("--n-lambda", type=int, default=0, help="override (debug only)")

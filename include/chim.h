@@ -111,7 +111,7 @@ typedef struct chim_config {
 } chim_config;
 
 /* Fills *cfg with the defaults: device 0, HOST, NULL stream, ON_SAMPLES, SCOTT, kde_cutoff 6.0,
- * z_cat_max 1.5, z_table_max 10, n_table 2048, n_dl_table 0 (auto), n_win_table 512, lambda_chunk 256,
+ * z_cat_max 1.5, z_table_max 10, n_table 2048, n_dl_table 0 (auto), n_win_table 512, lambda_chunk 1024,
  * neff_factor 5, kde_method AUTO, n_mass_table 1024, count_pairs 0, kde_kernel GAUSS, n_bins 0. */
 void chim_default_config(chim_config *cfg);
 

@@ -403,7 +403,7 @@ void chim_default_config(chim_config* cfg) {
     cfg->n_table = 2048;
     cfg->n_dl_table = 0;
     cfg->n_win_table = 512;
-    cfg->lambda_chunk = 256;
+    cfg->lambda_chunk = 1024;
     cfg->neff_factor = 5.0;
     cfg->kde_method = CHIM_KDE_AUTO;
     cfg->n_mass_table = 1024;

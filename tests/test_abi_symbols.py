@@ -39,7 +39,7 @@ def test_default_config_and_no_device_failure():
     import paper_2504_02034_b200 as pkg
     cfg = pkg.chim_default_config()
     assert (cfg.kde_cutoff, cfg.z_cat_max, cfg.z_table_max) == (6.0, 1.5, 10.0)
-    assert (cfg.n_table, cfg.n_dl_table, cfg.n_win_table, cfg.lambda_chunk) == (2048, 0, 512, 256)
+    assert (cfg.n_table, cfg.n_dl_table, cfg.n_win_table, cfg.lambda_chunk) == (2048, 0, 512, 1024)
     assert cfg.placement == pkg.CHIM_ON_SAMPLES and cfg.bw_rule == pkg.CHIM_BW_SCOTT
     import torch
     if not torch.cuda.is_available():

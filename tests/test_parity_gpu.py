@@ -62,7 +62,7 @@ GOLD = os.path.join(os.path.dirname(__file__), "golden")
 
 
 def _run_full(P, w, lam=None, **kw):
-    """The workload at full size, launched as bench.py launches it (default config, lambda_chunk 256, no pair counting)."""
+    """The workload at full size, launched as bench.py launches it (default config, lambda_chunk 1024, no pair counting)."""
     import torch
     c = P.Context(z_cat_max=w.z_cat_max, **kw)
     c.init_workload(w)
