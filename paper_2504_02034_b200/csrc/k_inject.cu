@@ -122,13 +122,31 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             k0 = lo ? __ffs(lo) - 1 : (hi ? 32 + __ffs(hi) - 1 : kInjChunkBlocks);
             k0 = max(0, min(k0, nblk - 1));
         }
+        // kDbg: s_j as a double through the exponent field, every one written out.  Production: fp32 sums of s_j / 2^ref and its
+        // square per THREAD, ref the thread's own running reference -- raised (and the sums rescaled) whenever a weight exceeds
+        // it by more than 2^40, a rare thread-local branch; the thread's sums become doubles once, at the end.  Weights more than
+        // 2^126 below the reference are flushed: less than 2^-86 of the thread's largest.  8 instructions per injection less
+        // than the fp64 accumulation.
 #define CHIM_INJ_TAIL(TURN, MID, JJ)                                                                                  \
         {                                                                                                             \
             const float l2w = poly_tail<TURN, false>(F, F.gk2_inj, F.cpsi_inj, M, MID, nullptr);                      \
-            const double s = ((MID).zc <= 0.f && (JJ) < n) ? ex2_to_double(l2w) : 0.0;                                \
-            acc[0] += s;                                                                                              \
-            acc[1] = fma(s, s, acc[1]);                                                                               \
-            if (kDbg && (JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale;                                   \
+            if (kDbg) {                                                                                               \
+                const double s = ((MID).zc <= 0.f && (JJ) < n) ? ex2_to_double(l2w) : 0.0;                            \
+                acc[0] += s;                                                                                          \
+                acc[1] = fma(s, s, acc[1]);                                                                           \
+                if ((JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale;                                       \
+            } else {                                                                                                  \
+                const float lw = ((MID).zc <= 0.f && (JJ) < n) ? l2w : -INFINITY;                                     \
+                if (lw > ref + 40.f) {   /* (NaN never enters: it fails the comparison and poisons the sums below) */  \
+                    const float dn = ex2f(ref - lw);                                                                  \
+                    f0 *= dn;                                                                                         \
+                    f1 *= dn * dn;                                                                                    \
+                    ref = lw;                                                                                         \
+                }                                                                                                     \
+                const float s = ex2f(lw - ref);                                                                       \
+                f0 += s;                                                                                              \
+                f1 = fmaf(s, s, f1);                                                                                  \
+            }                                                                                                         \
         }
         // two blocks per iteration: both heads (they consume the records), the records of the next two blocks as one group of
         // loads, then both tails (chim_internal.cuh: poly_head / poly_tail)
@@ -157,8 +175,14 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
         }
         if (kDbg)
             for (int j = tid; j < min(k0 * kInjThreads, n); j += kInjThreads) P.dbg_s[P.inj.perm[j0 + j]] = 0.0;
+        float ref = -1e30f, f0 = 0.f, f1 = 0.f;
         if (turn_folded) CHIM_INJ_SWEEP(false)
         else CHIM_INJ_SWEEP(true)
+        if (!kDbg) {   // the thread's sums on the absolute scale: s = 2^ref x relative weight
+            const double sc = ex2_to_double(ref);                      // (ref never raised: f0 = f1 = 0, sc = 0)
+            acc[0] = (double)f0 * sc;
+            acc[1] = (double)f1 * sc * sc;
+        }
 #undef CHIM_INJ_SWEEP
 #undef CHIM_INJ_TAIL
     } else if (L.flags == 0) {
