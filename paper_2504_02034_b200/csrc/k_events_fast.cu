@@ -418,20 +418,45 @@ __global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : 6) k_e
             const float4 ab = *reinterpret_cast<const float4*>(zw + min(jb, jsafe)), cd4 = *reinterpret_cast<const float4*>(zw + min(jb + 64, jsafe));
             const float zv[4] = {ab.x, ab.z, cd4.x, cd4.z};
             const float wv[4] = {ab.y, ab.w, cd4.y, cd4.w};
+            float y[4], v[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) y[r] = zv[r] * scy;
+            // the samples are sorted: if the first and the last sample of the pass fall into the same box, all 128 do (dense
+            // boxes: most passes) -- then the box record is read once, broadcast, and two samples share a packed FMA
+            const int bf = min(max(__float2int_rd(fmaf(y[0], inv_w, kb)), 0), bmax), bl = min(max(__float2int_rd(fmaf(y[3], inv_w, kb)), 0), bmax);
+            const int b_first = __shfl_sync(0xffffffffu, bf, 0), b_last = __shfl_sync(0xffffffffu, bl, 31);
+            if (b_first == b_last) {
+                const float4* bp = B4 + b_first * (kFBoxRec / 4);
+                const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
+                const float cb = bp[3].x;
+                const f32x2 s01 = pack2(y[0] - cb, y[1] - cb), s23 = pack2(y[2] - cb, y[3] - cb);
+                f32x2 a01 = pack2(k2.w, k2.w), a23 = a01;
+#define CHIM_LE_STEP(cf) { const f32x2 q_ = pack2(cf, cf); a01 = fma2(a01, s01, q_); a23 = fma2(a23, s23, q_); }
+                CHIM_LE_STEP(k2.z) CHIM_LE_STEP(k2.y) CHIM_LE_STEP(k2.x)
+                CHIM_LE_STEP(k1.w) CHIM_LE_STEP(k1.z) CHIM_LE_STEP(k1.y) CHIM_LE_STEP(k1.x)
+                CHIM_LE_STEP(k0.w) CHIM_LE_STEP(k0.z) CHIM_LE_STEP(k0.y) CHIM_LE_STEP(k0.x)
+#undef CHIM_LE_STEP
+                unpack2(a01, v[0], v[1]);
+                unpack2(a23, v[2], v[3]);
+            } else {
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int b = (r == 0) ? bf : (r == 3) ? bl : min(max(__float2int_rd(fmaf(y[r], inv_w, kb)), 0), bmax);
+                    const float4* bp = B4 + b * (kFBoxRec / 4);
+                    const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
+                    const float sv = y[r] - bp[3].x;
+                    float t = k2.w;
+                    t = fmaf(t, sv, k2.z); t = fmaf(t, sv, k2.y); t = fmaf(t, sv, k2.x);
+                    t = fmaf(t, sv, k1.w); t = fmaf(t, sv, k1.z); t = fmaf(t, sv, k1.y); t = fmaf(t, sv, k1.x);
+                    t = fmaf(t, sv, k0.w); t = fmaf(t, sv, k0.z); t = fmaf(t, sv, k0.y); t = fmaf(t, sv, k0.x);
+                    v[r] = t;
+                }
+            }
             float a = 0.f;
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
-                const float y = zv[r] * scy;
-                const int b = min(max(__float2int_rd(fmaf(y, inv_w, kb)), 0), bmax);
-                const float4* bp = B4 + b * (kFBoxRec / 4);
-                const float4 k0 = bp[0], k1 = bp[1], k2 = bp[2];
-                const float sv = y - bp[3].x;
-                float v = k2.w;
-                v = fmaf(v, sv, k2.z); v = fmaf(v, sv, k2.y); v = fmaf(v, sv, k2.x);
-                v = fmaf(v, sv, k1.w); v = fmaf(v, sv, k1.z); v = fmaf(v, sv, k1.y); v = fmaf(v, sv, k1.x);
-                v = fmaf(v, sv, k0.w); v = fmaf(v, sv, k0.z); v = fmaf(v, sv, k0.y); v = fmaf(v, sv, k0.x);
                 const bool in = jb + (r & 1) + 64 * (r >> 1) < c1;
-                a = fmaf(in ? wv[r] : 0.f, v, a);
+                a = fmaf(in ? wv[r] : 0.f, v[r], a);
             }
             lsum += (double)a;
         }
