@@ -295,14 +295,15 @@ __device__ __forceinline__ void load_poly(PolyCoef& C, const float* __restrict__
     for (int n = 0; n < kPolyN - 1; ++n) C.ua[n] = q[kPolyN + n];
 }
 
-// One warp: lanes 0..6 read the table at the Chebyshev nodes of [tk_c - tk_h, tk_c + tk_h] (table coordinates; fp64 from
-// the rows' hi + lo terms), then lane n < 7 forms coefficient n of the four polynomials; out[4][7] floats.
+// One segment of eight lanes per fit (four fits per warp; all 32 lanes call it, `valid` says whether the segment's item exists):
+// lanes 0..6 of the segment read the table at the Chebyshev nodes of [tk_c - tk_h, tk_c + tk_h] (table coordinates; fp64 from the
+// rows' hi + lo terms), then lane n < 7 forms coefficient n of the four polynomials; out[4][7] floats.
 //   r = table r + log2(1 + 2^(gk2 u - cpsi)) - beta2 u   (turnover taken out, -beta ln(1+z) of m2^beta folded in)
 __device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restrict__ tab, int K, double tk_c, double tk_h,
-                                          double z_ref, bool turn_on, const double* __restrict__ pm, float* __restrict__ out) {
-    const int lane = threadIdx.x & 31;
+                                          double z_ref, bool turn_on, const double* __restrict__ pm, float* __restrict__ out, bool valid) {
+    const int lane = threadIdx.x & 7;
     double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
-    if (lane < kPolyN) {
+    if (valid && lane < kPolyN) {
         const double tk = tk_c + tk_h * __ldg(pm + lane);
         const int k = max(1, min((int)tk, K));
         const float t = (float)(tk - (double)k);
@@ -324,12 +325,12 @@ __device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restri
 #pragma unroll
     for (int k = 0; k < kPolyN; ++k) {
         const double a7 = __ldg(m7 + k), a6 = __ldg(m6 + k);
-        c0 = fma(a7, __shfl_sync(0xffffffffu, v0, k), c0);
-        c1 = fma(a6, __shfl_sync(0xffffffffu, v1, k), c1);
-        c2 = fma(a6, __shfl_sync(0xffffffffu, v2, k), c2);
-        c3 = fma(a7, __shfl_sync(0xffffffffu, v3, k), c3);
+        c0 = fma(a7, __shfl_sync(0xffffffffu, v0, k, 8), c0);
+        c1 = fma(a6, __shfl_sync(0xffffffffu, v1, k, 8), c1);
+        c2 = fma(a6, __shfl_sync(0xffffffffu, v2, k, 8), c2);
+        c3 = fma(a7, __shfl_sync(0xffffffffu, v3, k, 8), c3);
     }
-    if (lane < kPolyN) {        // out: float2 zr[7] = (z_n, r_n), float2 ua[7] = (u_n, a_n)
+    if (valid && lane < kPolyN) {        // out: float2 zr[7] = (z_n, r_n), float2 ua[7] = (u_n, a_n)
         out[2 * lane] = (float)c0;
         out[2 * lane + 1] = (float)c3;
         out[2 * kPolyN + 2 * lane] = (float)c1;

@@ -486,7 +486,7 @@ cudaError_t launch_tables(const double* lam, int n_lambda, const TableParams& P,
 }
 
 // Diagnostics: evaluate the event table at arbitrary d_L (single lambda).
-// Local-polynomial fits for k_events (per (event, lambda)) and k_inject (per (chunk, lambda)): one warp per item.
+// Local-polynomial fits for k_events (per (event, lambda)) and k_inject (per (chunk, lambda)): eight lanes per item.
 // out[(l * n_ranges + r) * 4 * kPolyN ..]; items whose range is too wide (tk_h = 0), beyond the table or whose lambda is
 // invalid are left untouched (the consumers test the same conditions and take the table path).
 __global__ void __launch_bounds__(256) k_polyfit(const LamConst* __restrict__ Lc, const Row* __restrict__ tab, int tab_rows,
@@ -495,33 +495,34 @@ __global__ void __launch_bounds__(256) k_polyfit(const LamConst* __restrict__ Lc
                                                  double z_ref_const, int is_inj, const double* __restrict__ pm,
                                                  const double* __restrict__ lnm1_lo, const double* __restrict__ lnm1_hi,
                                                  int n_mass, int mcap, double dx_tab, float* __restrict__ out) {
-    const long long item = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
-    if (item >= (long long)n_lambda * n_ranges) return;
-    const int l = (int)(item % n_lambda), r = (int)(item / n_lambda);
+    // four items per warp, one per segment of eight lanes (the fp64 node evaluations occupy seven lanes of a segment)
+    const long long item = ((long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * 4 + ((threadIdx.x & 31) >> 3);
+    const int sl = threadIdx.x & 7;
+    bool valid = item < (long long)n_lambda * n_ranges;
+    const int l = valid ? (int)(item % n_lambda) : 0, r = valid ? (int)(item / n_lambda) : 0;
     const LamConst& L = Lc[l];
     const double h = tk_h[r], c = tk_c[r];
-    if (L.flags || !(h > 0.0) || !(c + h < (is_inj ? L.tkmax_inj : L.tkmax_ev))) return;
+    valid = valid && !L.flags && (h > 0.0) && (c + h < (is_inj ? L.tkmax_inj : L.tkmax_ev));
     float* o = out + ((size_t)l * n_ranges + r) * (4 * kPolyN);
     // the Madau-Dickinson turnover log2(1 + ((1+z)/(1+z_p))^(gamma+kappa)) is kept out of the fitted polynomial r (its poles sit
     // ~0.5 from the real axis in ln(1+z)) -- except for injection chunks narrower than 0.2 in ln d_L, where degree 6 takes it
     // to < 1e-9 and k_inject saves two MUFU per injection (slot 26 of the record: 1 = folded)
     const bool fold = is_inj && h * dx_tab <= 0.1;
-    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, !fold && (is_inj || L.F.gk2 != 0.f), pm, o);
+    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, !fold && (is_inj || L.F.gk2 != 0.f), pm, o, valid);
     if (is_inj) {
         __syncwarp();
-        if ((threadIdx.x & 31) == 0) o[26] = __int_as_float(fold ? 1 : 0);
+        if (valid && sl == 0) o[26] = __int_as_float(fold ? 1 : 0);
     }
     if (lnm1_lo) {
         // k_events: the rows of the mass table the event can address, ln m1 = ln m1d - u, u = ln(1+z) between the ends of the
         // event's range (the fitted polynomial at t = -1, +1), so that the CTA can issue its TMA copy at once.  Slots 26, 27 of
         // the record (the unused degree-6 terms of u and a): first staged row, and the row count (negative: does not fit)
         __syncwarp();
-        const int lane = threadIdx.x & 31;
-        const float cu = (lane < kPolyN - 1) ? o[2 * kPolyN + 2 * lane] : 0.f;          // u_n
-        float up = cu, um = (lane & 1) ? -cu : cu;
+        const float cu = (valid && sl < kPolyN - 1) ? o[2 * kPolyN + 2 * sl] : 0.f;          // u_n
+        float up = cu, um = (sl & 1) ? -cu : cu;
 #pragma unroll
-        for (int k = 16; k > 0; k >>= 1) { up += __shfl_xor_sync(0xffffffffu, up, k); um += __shfl_xor_sync(0xffffffffu, um, k); }
-        if (lane == 0) {
+        for (int k = 4; k > 0; k >>= 1) { up += __shfl_xor_sync(0xffffffffu, up, k); um += __shfl_xor_sync(0xffffffffu, um, k); }
+        if (valid && sl == 0) {
             const double u_lo = fmin((double)um, (double)up) - 1e-4, u_hi = fmax((double)um, (double)up) + 1e-4;
             const int ma = max(1, min((int)fma(lnm1_lo[r] - u_hi - L.lm0, L.inv_dlm, 1.0), n_mass));
             const int mb = max(1, min((int)fma(lnm1_hi[r] - u_lo - L.lm0, L.inv_dlm, 1.0), n_mass));
@@ -539,7 +540,7 @@ cudaError_t launch_polyfit(const LamConst* Lc, const Row* tab, int tab_rows, int
                            const double* lnm1_lo, const double* lnm1_hi, int n_mass, int mcap, double dx_tab, float* out, cudaStream_t st) {
     const long long items = (long long)n_lambda * n_ranges;
     if (items <= 0) return cudaSuccess;
-    k_polyfit<<<(unsigned)((items + 7) / 8), 256, 0, st>>>(Lc, tab, tab_rows, n_lambda, n_ranges, tk_c, tk_h, z_ref, z_ref_const,
+    k_polyfit<<<(unsigned)((items + 31) / 32), 256, 0, st>>>(Lc, tab, tab_rows, n_lambda, n_ranges, tk_c, tk_h, z_ref, z_ref_const,
                                                             is_inj ? 1 : 0, pm, lnm1_lo, lnm1_hi, n_mass, mcap, dx_tab, out);
     return cudaGetLastError();
 }
