@@ -34,7 +34,7 @@ ORACLE_KERNEL = [0, 0]        # oracle kernel id and bin count of the timed orac
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
-NCU_TRAFFIC_BYTES = 102.8e6 + 6.5e6   # k_events_fast, O5-spectroscopic, 1024-lambda launch: dram read + write (profiles/r02_ncu_full.md)
+NCU_TRAFFIC_BYTES = 103.2e6 + 4.7e6   # k_events_fast, O5-spectroscopic, 1024-lambda launch: dram read + write (profiles/r02_ncu_full.md)
 
 
 def default_workload(args):
