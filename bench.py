@@ -34,6 +34,7 @@ ORACLE_KERNEL = [0, 0]        # oracle kernel id and bin count of the timed orac
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
+KDE_PHASE_SHARE = 0.354   # S3 + S4 share of k_events_fast's warp-state samples (ncu, SASS segments between the barriers; profiles/r02_ncu_full.md)
 NCU_TRAFFIC_BYTES = 103.2e6 + 4.7e6   # k_events_fast, O5-spectroscopic, 1024-lambda launch: dram read + write (profiles/r02_ncu_full.md)
 
 
@@ -419,6 +420,10 @@ def run_ours(args):
                          "algorithmic_ops_per_launch": pairs_cut / n_launch, "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
                          # SURVEY 8(d) recipe on what the kernel executes (ncu instruction counts x live time), and the issue slots
                          "executed": kb["roofline_k_events_fast"],
+                         # the KDE phase alone (S3 + S4): its share of the kernel's time from the committed ncu capture (warp-state samples
+                         # per SASS segment), applied to the live time
+                         "kde_phase": ({"share_of_kernel_time": KDE_PHASE_SHARE, "frac": achieved / KDE_PHASE_SHARE / peak_g,
+                                        "source": "profiles/r02_ncu_full.md"} if default_workload(args) else None),
                          "traffic": (NCU_TRAFFIC_BYTES if default_workload(args) else None),
                          "traffic_source": ("profiles/r02_ncu_full.md" if default_workload(args) else None),
                          "algorithmic_dram_bytes_per_launch": alg_bytes,
