@@ -61,7 +61,7 @@ struct chim_ctx {
     // k_events_fast: the events it takes / leaves to k_events, and the per-chunk work list of the units it hands over
     const int32_t* fast_ev = nullptr; const int32_t* slow_ev = nullptr;
     int n_fast = 0, n_slow = 0;
-    int n_fast_c[2] = {0, 0}, max_ns_c[2] = {0, 0};   // the two classes of k_events_fast (4 / 8 warps): events, longest sample list
+    int n_fast_c[kFastClasses] = {}, max_ns_c[kFastClasses] = {};   // the classes of k_events_fast (2 / 4 / 8 warps): events, longest sample list
     uint32_t* worklist = nullptr; unsigned int* work_count = nullptr;
     // staging for the host-pointer entry point
     int host_nl = 0;
@@ -310,10 +310,10 @@ int run_rest(chim_ctx* ctx, int nl, double* out_ll, double* out_ev, double* out_
         FP.logI = ctx->logI; FP.ln_shift = ctx->ev_ln_shift; FP.ln_qscale = ctx->ev_ln_qscale;
         FP.fast_events = ctx->fast_ev; FP.worklist = ctx->worklist; FP.work_count = ctx->work_count;
         CK(cudaMemsetAsync(ctx->work_count, 0, sizeof(unsigned int), st));
-        for (int c = 0, first = 0; c < 2; first += ctx->n_fast_c[c], ++c) {
+        for (int c = 0, first = 0; c < kFastClasses; first += ctx->n_fast_c[c], ++c) {
             if (ctx->n_fast_c[c] == 0) continue;
             FP.fast_events = ctx->fast_ev + first;
-            FP.warps = c == 0 ? 4 : 8; FP.max_d = fast_max_d_for(FP.warps, ctx->ev.max_nz); FP.max_ns = ctx->max_ns_c[c];
+            FP.warps = 2 << c; FP.max_d = fast_max_d_for(FP.warps, ctx->ev.max_nz); FP.max_ns = ctx->max_ns_c[c];
             { Bracket b(ctx, 1); CK(launch_events_fast(FP, ctx->n_fast_c[c], st)); }
             ctx->launches += 1;
         }
@@ -666,11 +666,11 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     std::vector<float> qn4((size_t)q4n + 4, 0.f);
     for (int i = 0; i < n_events; ++i) std::copy(qn.begin() + go[i], qn.begin() + go[i + 1], qn4.begin() + q4off[i]);
     // k_events_fast takes the events with a narrow d_L range on an equally spaced grid, in two classes by the length of the
-    // sample list (chim_internal.cuh: fast_warps_for), the four-warp class first in the list
+    // sample list (chim_internal.cuh: fast_warps_for), the classes one after the other in the list
     std::vector<int32_t> fast_ev, slow_ev;
-    int n_fast_c[2] = {0, 0}, max_ns_c[2] = {0, 0};
-    for (int c = 0; c < 2; ++c) {
-        const int w = c == 0 ? 4 : 8;
+    int n_fast_c[kFastClasses] = {}, max_ns_c[kFastClasses] = {};
+    for (int c = 0; c < kFastClasses; ++c) {
+        const int w = 2 << c;
         for (int i = 0; i < n_events; ++i)
             if (fast_warps_for((int)(so[i + 1] - so[i])) == w) max_ns_c[c] = std::max(max_ns_c[c], (int)(so[i + 1] - so[i]));
         const bool fits = events_fast_smem_bytes(max_ns_c[c], max_nz, w, fast_max_d_for(w, max_nz)) <= kMaxSmemOptin;
@@ -705,7 +705,7 @@ int chim_init_events(chim_ctx* ctx, int32_t n_events, const int64_t* sample_off,
     CK(upload(ctx->owned_ev, &E.qn4, qn4)); CK(upload(ctx->owned_ev, &E.q4_off, q4off));
     CK(upload(ctx->owned_ev, &ctx->fast_ev, fast_ev)); CK(upload(ctx->owned_ev, &ctx->slow_ev, slow_ev));
     ctx->n_fast = (int)fast_ev.size(); ctx->n_slow = (int)slow_ev.size();
-    for (int c = 0; c < 2; ++c) { ctx->n_fast_c[c] = n_fast_c[c]; ctx->max_ns_c[c] = max_ns_c[c]; }
+    for (int c = 0; c < kFastClasses; ++c) { ctx->n_fast_c[c] = n_fast_c[c]; ctx->max_ns_c[c] = max_ns_c[c]; }
     CK(upload(ctx->owned_ev, &ctx->ev_ln_shift, shift));
     CK(upload(ctx->owned_ev, &ctx->ev_ln_qscale, qshift));
     ctx->ev = E;

@@ -465,9 +465,10 @@ __host__ __device__ inline int fast_chunk(int ns, int warps) { return ((ns + war
 // Two classes of events, each with its own launch: short sample lists (many-1d pixels) run four warps per CTA and more CTAs per
 // SM -- their phases between the barriers are latency-bound -- long ones eight.  Half-width cap of the psi table per class:
 // fine grids get a wider table, short lists (wider kernels relative to the grid) a narrower stage.
-constexpr int kFastSmallNs = 1280;
-__host__ inline int fast_warps_for(int ns) { return ns <= kFastSmallNs ? 4 : 8; }
-__host__ inline int fast_max_d_for(int warps, int max_nz) { return max_nz > 2048 ? 384 : (warps == 4 ? 160 : 256); }
+constexpr int kFastSmallNs = 1280, kFastTinyNs = 384;
+constexpr int kFastClasses = 3;            // 2, 4, 8 warps
+__host__ inline int fast_warps_for(int ns) { return ns <= kFastTinyNs ? 2 : (ns <= kFastSmallNs ? 4 : 8); }
+__host__ inline int fast_max_d_for(int warps, int max_nz) { return max_nz > 2048 ? 384 : (warps < 8 ? 160 : 256); }
 
 // ---- TMA bulk copy + mbarrier  ---------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -51,13 +51,13 @@ __host__ __device__ inline size_t fast_aux_bytes(int max_d) {
     return a > b ? a : b;
 }
 size_t events_fast_smem_bytes(int max_ns, int max_nz, int warps, int max_d) {
-    const size_t head = warps == 8 ? sizeof(FastSmem<8>) : sizeof(FastSmem<4>);
+    const size_t head = warps == 8 ? sizeof(FastSmem<8>) : (warps == 4 ? sizeof(FastSmem<4>) : sizeof(FastSmem<2>));
     return ((head + 127) / 128) * 128 + sizeof(float2) * (size_t)warps * fast_chunk(max_ns, warps) +
            sizeof(float) * (4 * (size_t)max_d + fast_nz4((size_t)max_nz)) + fast_aux_bytes(max_d);
 }
 
 template <int kFW, int kFMaxD>
-__global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : 6) k_events_fast(FastEventParams P) {
+__global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : (kFW == 4 ? 6 : 12)) k_events_fast(FastEventParams P) {
     constexpr int kFT = 32 * kFW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     FastSmem<kFW>& S = *reinterpret_cast<FastSmem<kFW>*>(smem_raw);
@@ -498,6 +498,8 @@ cudaError_t launch_events_fast(const FastEventParams& P, int n_fast, cudaStream_
     if (w == 8 && d == 384) return launch_fast_t<8, 384>(P, nb, smem, st);
     if (w == 4 && d == 160) return launch_fast_t<4, 160>(P, nb, smem, st);
     if (w == 4 && d == 384) return launch_fast_t<4, 384>(P, nb, smem, st);
+    if (w == 2 && d == 160) return launch_fast_t<2, 160>(P, nb, smem, st);
+    if (w == 2 && d == 384) return launch_fast_t<2, 384>(P, nb, smem, st);
     return cudaErrorInvalidValue;
 }
 
