@@ -465,7 +465,13 @@ __host__ __device__ inline int fast_chunk(int ns, int warps) { return ((ns + war
 // Two classes of events, each with its own launch: short sample lists (many-1d pixels) run four warps per CTA and more CTAs per
 // SM -- their phases between the barriers are latency-bound -- long ones eight.  Half-width cap of the psi table per class:
 // fine grids get a wider table, short lists (wider kernels relative to the grid) a narrower stage.
-constexpr int kFastSmallNs = 1280, kFastTinyNs = 384;
+#ifndef CHIM_FAST_SMALL_NS
+#define CHIM_FAST_SMALL_NS 2048
+#endif
+#ifndef CHIM_FAST_TINY_NS
+#define CHIM_FAST_TINY_NS 896
+#endif
+constexpr int kFastSmallNs = CHIM_FAST_SMALL_NS, kFastTinyNs = CHIM_FAST_TINY_NS;
 constexpr int kFastClasses = 3;            // 2, 4, 8 warps
 __host__ inline int fast_warps_for(int ns) { return ns <= kFastTinyNs ? 2 : (ns <= kFastSmallNs ? 4 : 8); }
 __host__ inline int fast_max_d_for(int warps, int max_nz) { return max_nz > 2048 ? 384 : (warps < 8 ? 160 : 256); }
