@@ -967,3 +967,38 @@ def test_loglike_gradient_argument_checks_and_undefined_points(P):
     assert np.isnan(out["loglike"].cpu().numpy()[0]) and np.isnan(out["grad"].cpu().numpy()[0]).all()
     assert int(out["flags"].cpu().numpy()[0]) & P.CHIM_FLAG_LAMBDA_DOMAIN
     c.close()
+
+
+def test_hot_path_runs_the_fast_kernel_in_every_class_and_chunked_batches_agree(P):
+    """The product path of the BASELINE shapes is k_events_fast (one launch per class of sample-list length: two, four, eight warps
+    per CTA), not the general kernel: with per-kernel timing on, a set that mixes the three classes shows three fast launches per
+    lambda chunk and spends most of its S2-S4 time there.  And a batch cut into several lambda chunks -- S1 of the next chunk on the
+    library's auxiliary stream while S2-S6 of the current one run -- gives the results of the single-chunk run bit for bit."""
+    import torch
+    w = make_workload("o5_spec", n_events=9, n_lambda=24, n_det=20_000)
+    ns = np.array([5000, 3000, 2100, 2000, 1500, 900, 800, 300, 100])        # classes: 8, 8, 8 | 4, 4, 4 | 2, 2, 2 warps
+    so = np.concatenate(([0], np.cumsum(ns)))
+    sel = np.concatenate([np.arange(w.sample_off[i], w.sample_off[i] + ns[i]) for i in range(w.n_events)])
+    w.dL, w.m1d, w.m2d, w.ln_prior = w.dL[sel], w.m1d[sel], w.m2d[sel], w.ln_prior[sel]
+    w.sample_off = so
+    ref = O.loglike_workload(w)
+    outs = {}
+    for chunk in (1024, 5):
+        c = P.Context(z_cat_max=w.z_cat_max, lambda_chunk=chunk)
+        c.init_workload(w)
+        lam = torch.as_tensor(w.lam, device=c.device).contiguous()
+        out = c.loglike_batch(lam)
+        torch.cuda.synchronize()
+        outs[chunk] = {k: v.cpu().numpy() for k, v in out.items()}
+        if chunk == 1024:
+            c.set_profiling(True)
+            c.loglike_batch(lam)
+            kt = c.kernel_times()
+            c.set_profiling(False)
+            assert kt["events_launches"] == 3, kt                          # one k_events_fast launch per class
+            assert kt["events_ms"] > kt["events_general_ms"], kt
+        c.close()
+    rel, dtot, dxi = _compare(outs[1024], ref, w.n_events)
+    assert rel < REL_EVENT and dtot < ABS_TOTAL
+    for k in ("loglike", "event_logI", "logxi", "neff"):
+        assert np.array_equal(outs[1024][k], outs[5][k], equal_nan=True), k
