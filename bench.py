@@ -247,7 +247,7 @@ def measure(pkg, torch, dist, args, name, catalog, pixels, K, W, rank, world, lo
         sampler.start()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     keys = ("tables_ms", "events_ms", "events_general_ms", "inject_ms", "combine_ms", "events_launches", "events_general_launches",
-            "inject_launches")
+            "inject_launches", "events_handed_over")
     ktimes = {k: 0.0 for k in keys}
     barrier()
     t_wall0 = time.perf_counter()
@@ -330,6 +330,7 @@ def kernel_block(r, counts, workload_key, clk_hz):
     return {"ms_per_step": r["t_dev"] / K * 1e3, "value": units * K / r["t_dev"], "steps": K, "warmup": r["W"],
             "kernel_ms_per_step": {"tables_ms": kt["tables_ms"] / K, "events_fast_ms": ev_ms, "events_general_ms": kt["events_general_ms"] / K,
                                    "inject_ms": inj_ms, "combine_ms": kt["combine_ms"] / K},
+            "units_handed_over_per_step": kt["events_handed_over"] / K,   # (event, lambda) units k_events_fast left to k_events (last lambda chunk of a step)
             "nonfinite_lambda": r["nonfinite_lambda"], "flagged_lambda": r["flagged_lambda"],
             "roofline_k_events_fast": recipe_entry(counts, workload_key, "k_events_fast", n_sub, ev_ms, clk_hz),
             "roofline_k_inject": recipe_entry(counts, workload_key, "k_inject", n_inj, inj_ms, clk_hz),

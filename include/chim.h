@@ -255,7 +255,8 @@ typedef struct chim_kernel_times {
     double tables_ms, events_ms, inject_ms, combine_ms;
     uint32_t tables_launches, events_launches, inject_launches, combine_launches;
     double events_general_ms;
-    uint32_t events_general_launches, reserved;
+    uint32_t events_general_launches;
+    uint32_t events_handed_over; /* (event, lambda) units k_events_fast left to k_events in the LAST lambda chunk of the batch */
 } chim_kernel_times;
 int chim_set_profiling(chim_ctx *ctx, int32_t enable);
 int chim_get_kernel_times(chim_ctx *ctx, chim_kernel_times *out);

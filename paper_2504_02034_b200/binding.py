@@ -42,7 +42,7 @@ class ChimKernelTimes(C.Structure):
     _fields_ = [("tables_ms", C.c_double), ("events_ms", C.c_double), ("inject_ms", C.c_double),
                 ("combine_ms", C.c_double), ("tables_launches", C.c_uint32), ("events_launches", C.c_uint32),
                 ("inject_launches", C.c_uint32), ("combine_launches", C.c_uint32), ("events_general_ms", C.c_double),
-                ("events_general_launches", C.c_uint32), ("reserved", C.c_uint32)]
+                ("events_general_launches", C.c_uint32), ("events_handed_over", C.c_uint32)]
 
 
 class ChimAluPeaks(C.Structure):

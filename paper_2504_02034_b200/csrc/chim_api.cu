@@ -1092,6 +1092,11 @@ int chim_get_kernel_times(chim_ctx* ctx, chim_kernel_times* out) {
         *ms[ctx->ev_kind[i]] += t;
         *nl[ctx->ev_kind[i]] += 1;
     }
+    if (ctx->work_count) {
+        unsigned int n = 0;
+        CK(cudaMemcpy(&n, ctx->work_count, sizeof n, cudaMemcpyDeviceToHost));
+        out->events_handed_over = n;
+    }
     return CHIM_OK;
 }
 
