@@ -941,7 +941,8 @@ int chim_loglike_batch(chim_ctx* ctx, int32_t n_lambda, const double* lambda, do
         return fail(ctx, CHIM_EINVAL, "chim_loglike_batch: null lambda/out_loglike or n_lambda < 0");
     if (n_lambda == 0) return CHIM_OK;
     CK(cudaSetDevice(ctx->cfg.device));
-    const int chunk = std::min<int>(ctx->cfg.lambda_chunk, n_lambda);
+    // (a work-list entry holds lambda x n_events + event in 31 bits)
+    const int chunk = (int)std::min<long long>(std::min<int>(ctx->cfg.lambda_chunk, n_lambda), std::max<long long>(1, 0x7FFFFFFFLL / std::max(ctx->ev.n_events, 1)));
     int rc = ensure_work(ctx, chunk);
     if (rc != CHIM_OK) return rc;
     ctx->launches = 0;

@@ -459,7 +459,8 @@ __device__ __noinline__ double exact_log2_kde(const LamConst& L, const double* _
 // One (event, lambda) unit.  Block-uniform returns only.  again: the CTA has processed a unit before (work-list mode): the
 // one-shot mbarrier is invalidated and initialised anew.
 template <bool kStats>
-__device__ __forceinline__ void events_unit(const EventKernelParams& P, const int l, const int ev, unsigned char* smem_raw, const bool again) {
+__device__ __forceinline__ void events_unit(const EventKernelParams& P, const int l, const int ev, unsigned char* smem_raw, const bool again,
+                                            const bool force_careful) {
     EvSmem& S = *reinterpret_cast<EvSmem*>(smem_raw);
     float* zf = reinterpret_cast<float*>(smem_raw + ((sizeof(EvSmem) + 127) / 128) * 128);
     const size_t ns_pad = ev_ns_pad(P.ev.max_ns);
@@ -563,7 +564,7 @@ __device__ __forceinline__ void events_unit(const EventKernelParams& P, const in
     // samples are sorted in d_L: one of them lies beyond the table iff the last one does
     if (tid == 0 && __float_as_uint(__ldg(rec + 2 * (size_t)(ns - 1)).x) > L.F.tkmax_ev_q) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
     bool careful = true;
-    if (use_poly) {
+    if (use_poly && !force_careful) {   // (force_careful: k_events_fast found the unit in need of the careful sweep already)
         if (S.mass_fit) mx = s2_sweep_poly<true>(P.ev.prec_a + p0, P.ev.prec_b + p0, L.F, S.poly, M, ns, zf, wl, jd);
         else mx = s2_sweep_poly<false>(P.ev.prec_a + p0, P.ev.prec_b + p0, L.F, S.poly, M, ns, zf, wl, jd);
         block_argmax(mx, jd, S.kred);
@@ -1034,8 +1035,8 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         const unsigned n = *P.work_count;
         bool again = false;
         for (unsigned u = blockIdx.x; u < n; u += gridDim.x) {
-            const uint32_t unit = P.worklist[u];
-            events_unit<kStats>(P, (int)(unit / (uint32_t)P.ev.n_events), (int)(unit % (uint32_t)P.ev.n_events), smem_raw, again);
+            const uint32_t entry = P.worklist[u], unit = entry & 0x7FFFFFFFu;     // (bit 31: take the careful sweep at once)
+            events_unit<kStats>(P, (int)(unit / (uint32_t)P.ev.n_events), (int)(unit % (uint32_t)P.ev.n_events), smem_raw, again, (entry >> 31) != 0u);
             again = true;
             __syncthreads();
         }
@@ -1048,7 +1049,7 @@ __global__ void __launch_bounds__(kEvThreads, CHIM_EV_BLOCKS) k_events(EventKern
         ev = blockIdx.x / P.n_lambda;
         if (P.ev_list) ev = P.ev_list[ev];
     }
-    events_unit<kStats>(P, l, ev, smem_raw, false);
+    events_unit<kStats>(P, l, ev, smem_raw, false, false);
 }
 
 int events_mass_stage_rows(int n_mass) { return min(kMassStage, n_mass + 2); }

@@ -103,15 +103,16 @@ __global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : (kFW =
         mlo = __float_as_int(v[6].z);
         nr = __float_as_int(v[6].w);                // > 0: every mass-table row the event can address fits the stage
     }
-#define CHIM_FAST_HANDOVER()                                                    \
+    // (bit 31 of a work-list entry: the unit needs the careful sweep of k_events -- it then skips its own fast one)
+#define CHIM_FAST_HANDOVER(CAREFUL)                                             \
     do {                                                                        \
         if (tid == 0) {                                                         \
             const unsigned k_ = atomicAdd(P.work_count, 1u);                    \
-            P.worklist[k_] = (uint32_t)l * (uint32_t)P.ev.n_events + (uint32_t)ev; \
+            P.worklist[k_] = ((uint32_t)l * (uint32_t)P.ev.n_events + (uint32_t)ev) | ((CAREFUL) ? 0x80000000u : 0u); \
         }                                                                       \
         return;                                                                 \
     } while (0)
-    if (nr <= 0 || nr > kFMassStage) CHIM_FAST_HANDOVER();
+    if (nr <= 0 || nr > kFMassStage) CHIM_FAST_HANDOVER(false);
 
     const size_t nz4 = fast_nz4((size_t)nz);
     const MassRow* mtab = P.mtab + (size_t)l * 2 * (P.n_mass + 2);
@@ -262,7 +263,7 @@ __global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : (kFW =
     for (int o = kFW / 2; o > 0; o >>= 1) gref = fmaxf(gref, __shfl_xor_sync(0xffffffffu, gref, o));
     gref = __shfl_sync(0xffffffffu, gref, 0);
     mbar_wait(&S.mbar_q, 0);                                            // q_g has landed (also: no copy in flight at any exit below)
-    if (!(gref > -INFINITY)) CHIM_FAST_HANDOVER();                      // no weighted sample on this path: k_events decides
+    if (!(gref > -INFINITY)) CHIM_FAST_HANDOVER(true);                   // no weighted sample on this path: k_events decides
     const bool live = lane < kFW && cm > -INFINITY;
     const float f = live ? ex2f(cm - gref) : 0.f;                       // chunk-relative weights -> relative to the largest chunk reference
     const float wc = live ? S.c_mom[lane][0] : 0.f, qc = live ? S.c_mom[lane][1] : 0.f;
@@ -311,7 +312,8 @@ __global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : (kFW =
 #pragma unroll
     for (int o = kFW / 2; o > 0; o >>= 1) gmp2 = fmaxf(gmp2, __shfl_xor_sync(0xffffffffu, gmp2, o));
     gmp2 = __shfl_sync(0xffffffffu, gmp2, 0);
-    bool hand = !(h > 0.f) || !isfinite(h) || !(neff >= P.neff_min) || gmp2 < 0.f || gmp2 * gmp2 < 0.1f * F.delta;
+    const bool hand_careful = !(h > 0.f) || !isfinite(h) || !(neff >= P.neff_min) || gmp2 < 0.f || gmp2 * gmp2 < 0.1f * F.delta;
+    bool hand = hand_careful;
     // local-expansion geometry: y = z'/(sqrt(2) h), boxes of m grid spacings centred on grid points
     const double udz = __ldg(P.ev.uni_dz + ev), zfirst = __ldg(P.ev.zc + g0);
     const float scy = 0.70710678118654752440f / h;
@@ -323,7 +325,7 @@ __global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : (kFW =
     const float fD = ceilf(__fdividef(Ty + 0.5f * wbox, dy)) + 1.0f;
     hand = hand || !(wbox <= kFMaxW) || !(fb_hi - fb_lo < (float)kFMaxBox) || !(fabsf(fb_lo) < 1e6f) || !(fabsf(fb_hi) < 1e6f) ||
            !(fD <= (float)kFMaxD) || !(fabsf(fb_lo) * (float)m < 1e8f) || !(fabsf(fb_hi) * (float)m < 1e8f);
-    if (hand) CHIM_FAST_HANDOVER();
+    if (hand) CHIM_FAST_HANDOVER(hand_careful);
     const int D = (int)fD, b_lo = (int)fb_lo, nbox = (int)(fb_hi - fb_lo) + 1;
     // once per CTA, one thread per entry: the psi table psi_n(d dy) = exp(-t^2) H_n(t)/n!, t = d dy, by the three-term recurrence
     for (int d = tid; d <= D; d += kFT) {
