@@ -976,7 +976,7 @@ def test_hot_path_runs_the_fast_kernel_in_every_class_and_chunked_batches_agree(
     library's auxiliary stream while S2-S6 of the current one run -- gives the results of the single-chunk run bit for bit."""
     import torch
     w = make_workload("o5_spec", n_events=9, n_lambda=24, n_det=20_000)
-    ns = np.array([5000, 3000, 2100, 2000, 1500, 900, 800, 300, 100])        # classes: 8, 8, 8 | 4, 4, 4 | 2, 2, 2 warps
+    ns = np.array([5000, 2081, 2049, 2048, 2047, 897, 896, 895, 33])         # classes: 8, 8, 8 | 4, 4, 4 | 2, 2, 2 warps (at the class limits)
     so = np.concatenate(([0], np.cumsum(ns)))
     sel = np.concatenate([np.arange(w.sample_off[i], w.sample_off[i] + ns[i]) for i in range(w.n_events)])
     w.dL, w.m1d, w.m2d, w.ln_prior = w.dL[sel], w.m1d[sel], w.m2d[sel], w.ln_prior[sel]
