@@ -34,8 +34,8 @@ ORACLE_KERNEL = [0, 0]        # oracle kernel id and bin count of the timed orac
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
-KDE_PHASE_SHARE = 0.354   # S3 + S4 share of k_events_fast's warp-state samples (ncu, SASS segments between the barriers; profiles/r02_ncu_full.md)
-NCU_TRAFFIC_BYTES = 103.2e6 + 4.7e6   # k_events_fast, O5-spectroscopic, 1024-lambda launch: dram read + write (profiles/r02_ncu_full.md)
+KDE_PHASE_SHARE = 0.331   # S3 + S4 share of k_events_fast's warp-state samples (ncu, SASS segments between the barriers; profiles/r02_ncu_full.md)
+NCU_TRAFFIC_BYTES = 102.6e6 + 4.3e6   # k_events_fast, O5-spectroscopic, 1024-lambda launch: dram read + write (profiles/r02_ncu_full.md)
 
 
 def default_workload(args):
