@@ -258,7 +258,6 @@ def measure(pkg, torch, dist, args, name, catalog, pixels, K, W, rank, world, lo
         evs[i][1].record(stream)
     barrier()
     t_wall = time.perf_counter() - t_wall0
-    clocks = sampler.stop() if rank == 0 else None
     ll_timed = out["loglike"].cpu().numpy()
     # per-kernel times: the same K batches once more with the library's CUDA events around every launch -- in that mode the kernels
     # run one after the other on one stream (S1 of the next lambda chunk is not overlapped with S2-S6), so the times add up to
@@ -271,6 +270,7 @@ def measure(pkg, torch, dist, args, name, catalog, pixels, K, W, rank, world, lo
         for k in keys:
             ktimes[k] += kt[k]
     ctx.set_profiling(False)
+    clocks = sampler.stop() if rank == 0 else None   # (sampled over the timed steps and the per-kernel pass: the same load)
     assert np.allclose(ll_timed, out["loglike"].cpu().numpy(), rtol=0, atol=1e-9, equal_nan=True)   # same kernels, same inputs
     t_dev = float(np.sum([a.elapsed_time(b) for a, b in evs])) / 1e3
     ll_last = out["loglike"].cpu().numpy()
