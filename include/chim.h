@@ -187,6 +187,41 @@ int chim_build_pgal(chim_ctx *ctx, double omega_m, double z_max, int32_t n_los, 
                     const double *p_compl, const int64_t *grid_off, const double *z_grid, double *p_gal_out, double *f_R_out);
 
 /*
+ * chim_build_pcat for callers that must not allocate device memory: eq. 8 exactly as chim_build_pcat computes it,
+ * but nothing is cudaMalloc'ed, cudaFree'd or copied to the host.
+ *
+ * Why it exists: chim_build_pcat makes device copies of its inputs and needs one double of scratch per galaxy, all from
+ * cudaMalloc, and frees them with cudaFree before it returns.  That is fine at start-up.  It is not possible (a) inside a
+ * JAX / PyTorch process whose framework has already reserved nearly all of the GPU's memory for its own pool -- a cudaMalloc
+ * from a foreign library then fails although the framework has room -- and (b) it is unwelcome between likelihood batches,
+ * because cudaMalloc and cudaFree synchronise the whole device and so stall a batch still running on another stream.  Such a
+ * caller hands over DEVICE pointers for every input and the output (here always DEVICE, whatever cfg.mem says), and the per-
+ * galaxy scratch lives in a fixed array inside the library's device image.
+ *
+ * The limit: at most CHIM_PCAT_STATIC_MAX_GALAXIES galaxies in one call, over all lines of sight together (2 MiB of fp64; every
+ * GPU on which libchim.so is loaded holds that array until the process exits, used or not).  A larger n_gal_total is rejected
+ * with CHIM_EINVAL and a message naming both numbers; split the lines of sight over several calls, or use chim_build_pcat.
+ *
+ *   n_gal_total = gal_off[n_los], passed by value because the offsets are never read on the host.  The kernel checks every
+ *                 line of sight's range against it: a line of sight whose galaxy range is empty, negative or ends beyond
+ *                 n_gal_total gets NaN on its whole grid (nothing is written outside the array).
+ *   everything else as chim_build_pcat; w_gal may be NULL.  The VALUES are not validated (that would need a copy to the host):
+ *   sigma_gal <= 0, a negative redshift etc. come out as NaN / inf instead of CHIM_EINVAL.
+ *
+ * Enqueue-only on cfg.stream: no host synchronisation, the caller synchronises before reading p_cat_out.
+ * One array per GPU, shared by all contexts and calls: calls that may overlap on the GPU (other streams, other contexts, other
+ * host threads) race on it and corrupt each other's result; calls on one stream are ordered and safe.  The array keeps the
+ * previous call's contents; nothing in it needs to start at zero (each line of sight writes its coefficients before reading
+ * them), so it is never cleared.
+ * The first call on each device also looks the array's device address up (and may load the kernel image): make it once at
+ * start-up, before any stream capture and before the phase in which the process must leave the allocator alone.
+ */
+#define CHIM_PCAT_STATIC_MAX_GALAXIES 262144
+int chim_build_pcat_static(chim_ctx *ctx, double omega_m, int32_t n_los, int64_t n_gal_total, const int64_t *gal_off,
+                           const double *z_gal, const double *sigma_gal, const double *w_gal, const int64_t *grid_off,
+                           const double *z_grid, double *p_cat_out);
+
+/*
  * Detected injections for the selection term: n_det stored injections out of
  * n_inj_total drawn; ln_pdraw = ln of the draw density in (d_L, m1d, m2d) (R7).  Optional: without
  * injections log xi := 0 and loglike = sum_i log I_i.  n_det == 0 removes a previous set.

@@ -15,6 +15,7 @@ CHIM_KDE_AUTO, CHIM_KDE_DIRECT, CHIM_KDE_POWER, CHIM_KDE_NONE = 0, 1, 2, 3
 CHIM_KERNEL_GAUSS, CHIM_KERNEL_EPANECHNIKOV = 0, 1
 CHIM_FLAG_LAMBDA_DOMAIN, CHIM_FLAG_DL_NONMONOTONE, CHIM_FLAG_EVENT_ZERO, CHIM_FLAG_XI_ZERO = 1, 2, 4, 8
 CHIM_FLAG_NEFF_LOW, CHIM_FLAG_TABLE_RANGE, CHIM_FLAG_BW_DEGENERATE = 16, 32, 64
+CHIM_PCAT_STATIC_MAX_GALAXIES = 262144
 N_LAMBDA_PARAMS = 15
 
 
@@ -81,6 +82,7 @@ def lib():
     L.chim_set_event_groups.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
     L.chim_build_pcat.argtypes = [C.c_void_p, C.c_double, C.c_int32] + [C.c_void_p] * 7
     L.chim_build_pgal.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int32] + [C.c_void_p] * 11
+    L.chim_build_pcat_static.argtypes = [C.c_void_p, C.c_double, C.c_int32, C.c_int64] + [C.c_void_p] * 7
     L.chim_loglike_batch.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_loglike_batch_host.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 6
     L.chim_loglike_grad_batch.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -151,6 +153,12 @@ def chim_set_event_groups(ctx, n_groups, group_off, ln_factor):
 def chim_build_pcat(ctx, omega_m, n_los, gal_off, z_gal, sigma_gal, w_gal, grid_off, z_grid, p_cat_out):
     _check(ctx, lib().chim_build_pcat(ctx, omega_m, n_los, *[_addr(a) for a in (gal_off, z_gal, sigma_gal, w_gal, grid_off,
                                                                                z_grid, p_cat_out)]))
+
+
+def chim_build_pcat_static(ctx, omega_m, n_los, n_gal_total, gal_off, z_gal, sigma_gal, w_gal, grid_off, z_grid, p_cat_out):
+    """chim_build_pcat for callers that must not allocate device memory (include/chim.h): DEVICE pointers only, enqueue-only."""
+    _check(ctx, lib().chim_build_pcat_static(ctx, omega_m, n_los, n_gal_total, *[_addr(a) for a in (gal_off, z_gal, sigma_gal, w_gal,
+                                                                                                  grid_off, z_grid, p_cat_out)]))
 
 
 def chim_build_pgal(ctx, omega_m, z_max, n_los, gal_off, z_gal, sigma_gal, w_gal, compl_off, z_compl, p_compl, grid_off, z_grid,
@@ -260,6 +268,22 @@ class Context:
         chim_build_pcat(self.h, float(omega_m), len(go) - 1, go, _f64(z_gal), _f64(sigma_gal),
                         None if w_gal is None else _f64(w_gal), po, zg, out)
         return out
+
+    def build_pcat_static(self, omega_m, n_gal_total, gal_off, z_gal, sigma_gal, grid_off, z_grid, p_cat_out, w_gal=None):
+        """PAPER.md:62 eq. 8 for a caller that cannot let this library allocate on the GPU (the memory belongs to a framework's
+        pool, or a cudaMalloc / cudaFree would stall a running batch).  Every array is a CUDA tensor the caller owns -- int64
+        offsets, float64 values, p_cat_out included -- and n_gal_total = gal_off[-1] is passed by value (the offsets stay on the
+        device).  At most CHIM_PCAT_STATIC_MAX_GALAXIES galaxies per call: the per-galaxy scratch is a fixed array inside
+        libchim.so, shared by all calls on the GPU, so calls that may overlap there must not be issued.  Enqueues on the
+        context's stream and returns p_cat_out; nothing is validated beyond the sizes."""
+        t = self.torch
+        for a, dt in ((gal_off, t.int64), (grid_off, t.int64), (z_gal, t.float64), (sigma_gal, t.float64), (z_grid, t.float64),
+                      (p_cat_out, t.float64)) + (((w_gal, t.float64),) if w_gal is not None else ()):
+            assert a.is_cuda and a.dtype == dt and a.is_contiguous()
+        assert p_cat_out.numel() == z_grid.numel() and gal_off.numel() == grid_off.numel()
+        chim_build_pcat_static(self.h, float(omega_m), gal_off.numel() - 1, int(n_gal_total), gal_off, z_gal, sigma_gal, w_gal,
+                               grid_off, z_grid, p_cat_out)
+        return p_cat_out
 
     def build_pgal(self, omega_m, z_max, gal_off, z_gal, sigma_gal, compl_off, z_compl, p_compl, grid_off, z_grid, w_gal=None):
         """PAPER.md:58 eq. 7 with eq. 9-10 on the given grids (host arrays in); returns (p_gal, f_R per line of sight)."""

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libchim.so")
-SOURCES = ["chim_api.cu", "k_tables.cu", "k_events.cu", "k_events_fast.cu", "k_inject.cu", "k_grad.cu", "k_peaks.cu"]
+SOURCES = ["chim_api.cu", "k_tables.cu", "k_events.cu", "k_events_fast.cu", "k_inject.cu", "k_grad.cu", "k_peaks.cu", "k_pcat_static.cu"]
 HEADERS = ["chim_internal.cuh", os.path.join("..", "..", "include", "chim.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=true", "-Xptxas", "-v"]

@@ -828,6 +828,27 @@ int chim_build_pgal(chim_ctx* ctx, double omega_m, double z_max, int32_t n_los, 
                            grid_off, z_grid, p_gal_out, f_r_out);
 }
 
+// eq. 8 for callers that cannot allocate (include/chim.h; k_pcat_static.cu): device pointers only, enqueue-only, and on this
+// path no cudaMalloc / cudaFree / host copy -- the failure messages below are the only place that touches the host heap.
+int chim_build_pcat_static(chim_ctx* ctx, double omega_m, int32_t n_los, int64_t n_gal_total, const int64_t* gal_off,
+                           const double* z_gal, const double* sigma_gal, const double* w_gal, const int64_t* grid_off,
+                           const double* z_grid, double* p_cat_out) {
+    if (!ctx) return CHIM_EINVAL;
+    if (n_los < 1 || !gal_off || !z_gal || !sigma_gal || !grid_off || !z_grid || !p_cat_out || !(omega_m > 0.0) || !(omega_m <= 1.0))
+        return fail(ctx, CHIM_EINVAL, "chim_build_pcat_static: null pointer, n_los < 1 or omega_m outside (0, 1]");
+    if (n_gal_total < n_los)
+        return fail(ctx, CHIM_EINVAL, "chim_build_pcat_static: n_gal_total < n_los (every line of sight needs >= 1 galaxy)");
+    if (n_gal_total > (int64_t)pcat_static_max_galaxies())
+        return fail(ctx, CHIM_EINVAL, "chim_build_pcat_static: n_gal_total = " + std::to_string(n_gal_total) +
+                                          " exceeds CHIM_PCAT_STATIC_MAX_GALAXIES = " + std::to_string(pcat_static_max_galaxies()) +
+                                          " (the fixed scratch array); split the lines of sight over several calls or use chim_build_pcat");
+    CK(cudaSetDevice(ctx->cfg.device));
+    cudaError_t e = launch_pcat_static(omega_m, n_los, (long long)n_gal_total, gal_off, z_gal, sigma_gal, w_gal, grid_off, z_grid,
+                                       p_cat_out, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "chim_build_pcat_static");
+    return CHIM_OK;
+}
+
 int chim_init_injections(chim_ctx* ctx, int64_t n_det, int64_t n_inj_total, const double* dL, const double* m1d,
                          const double* m2d, const double* ln_pdraw) {
     if (!ctx) return CHIM_EINVAL;

@@ -663,6 +663,10 @@ cudaError_t launch_table_lookup(const LamConst* Lc, const Row* tab, DlGrid g, in
                                 double z_table_max, double* z_out, double* r_out, cudaStream_t st);
 cudaError_t launch_pcat(double Om, int n_los, const int64_t* gal_off, const double* zt, const double* st, const double* wg,
                         const int64_t* grid_off, const double* zg, double* coef, double* out, cudaStream_t st_);
+// (k_pcat_static.cu) k_pcat with its per-galaxy scratch in a file-scope __device__ array: no allocation anywhere
+cudaError_t launch_pcat_static(double Om, int n_los, long long n_gal, const int64_t* gal_off, const double* zt, const double* st,
+                               const double* wg, const int64_t* grid_off, const double* zg, double* out, cudaStream_t st_);
+int pcat_static_max_galaxies();
 cudaError_t launch_pgal(double Om, double zmax, int n_los, const int64_t* compl_off, const double* zc, const double* pc,
                         const int64_t* grid_off, const double* zg, double* out, double* fr_out, cudaStream_t st_);
 cudaError_t launch_grad_expand(const double* lam, int n_lambda, double rel, double* ext, cudaStream_t st);
