@@ -34,9 +34,6 @@ ORACLE_KERNEL = [0, 0]        # oracle kernel id and bin count of the timed orac
 FMA_LANES_PER_CLK_PER_SM = 128   # fp32 FMA lanes per SM per clock on sm_100, reached with packed FFMA2
 
 
-KDE_PHASE_SHARE = 0.331   # S3 + S4 share of k_events_fast's warp-state samples (ncu, SASS segments between the barriers; profiles/r02_ncu_full.md)
-NCU_TRAFFIC_BYTES = 102.6e6 + 4.3e6   # k_events_fast, O5-spectroscopic, 1024-lambda launch: dram read + write (profiles/r02_ncu_full.md)
-
 
 def default_workload(args):
     return (args.config == "o5_spec" and args.catalog == 0 and not (args.n_events or args.n_det or args.n_lambda)
@@ -178,22 +175,32 @@ def workload_config(w, args):
 
 
 def load_instruction_counts():
-    """Per-unit instruction counts of the two hot kernels from the committed ncu captures (profiles/r02_instruction_counts.csv;
-    the .md beside it names the commands): {(workload, kernel): row}.  Absent file -> {} and the recipe entries read null."""
+    """Per-unit instruction counts and per-launch DRAM bytes of the two hot kernels from the committed ncu captures
+    (profiles/r02_instruction_counts.csv; the .md beside it names the commands): {(workload, kernel): row}.  Absent file -> {} and
+    the recipe entries read null.  Every row names the sha256[:16] of the kernel's .cu file at capture; a row whose kernel source
+    has changed since is marked stale and its figures are not used for `roofline.frac`."""
     import csv
+    import hashlib
     p = os.path.join(ROOT, "profiles", "r02_instruction_counts.csv")
     out = {}
     if os.path.exists(p):
+        sha = {}
         with open(p) as f:
             for r in csv.DictReader(f):
+                k = r["kernel"]
+                if k not in sha:
+                    src = os.path.join(ROOT, "paper_2504_02034_b200", "csrc", k + ".cu")
+                    sha[k] = hashlib.sha256(open(src, "rb").read()).hexdigest()[:16] if os.path.exists(src) else None
+                r["stale"] = sha[k] != r.get("kernel_src_sha16")
                 out[(r["workload"], r["kernel"])] = r
     return out
 
 
 def recipe_entry(counts, workload, kernel, units_per_step, ms_per_step, clk_hz):
     """t_min = max(n_x / P_sfu, n_f / P_fp32) with the kernel's executed instruction counts (ncu), P_sfu = 148 x 16
-    lanes/clk, P_fp32 = 148 x 128 lanes/clk; fraction = t_min / t_measured (live).  Beside it the issue-slot fraction: warp
-    instructions / (148 SM x 4 schedulers x clock) / t_measured."""
+    lanes/clk, P_fp32 = 148 x 128 lanes/clk; fraction = t_min / t_measured (live).  `achieved` / `peak` are those of the pipe that
+    binds (the larger of the two times), so achieved / peak = frac.  Beside it the issue-slot fraction: warp instructions /
+    (148 SM x 4 schedulers x clock) / t_measured."""
     r = counts.get((workload, kernel))
     if r is None or ms_per_step <= 0:
         return None
@@ -202,10 +209,15 @@ def recipe_entry(counts, workload, kernel, units_per_step, ms_per_step, clk_hz):
     n_i = float(r["warp_inst_per_unit"]) * units_per_step
     p_sfu, p_fp32, p_issue = SM_COUNT * 16 * clk_hz, SM_COUNT * FMA_LANES_PER_CLK_PER_SM * clk_hz, SM_COUNT * 4 * clk_hz
     t = ms_per_step / 1e3
+    fp32_binds = n_f / p_fp32 >= n_x / p_sfu
     return {"t_min_ms": 1e3 * max(n_x / p_sfu, n_f / p_fp32), "frac": max(n_x / p_sfu, n_f / p_fp32) / t,
+            "binding_pipe": "fp32" if fp32_binds else "sfu",
+            "achieved_gops": (n_f if fp32_binds else n_x) / t / 1e9, "peak_gops": (p_fp32 if fp32_binds else p_sfu) / 1e9,
             "sfu_frac": n_x / p_sfu / t, "fp32_frac": n_f / p_fp32 / t, "issue_slot_frac": n_i / p_issue / t,
             "sfu_thread_inst_per_unit": float(r["sfu_thread_inst_per_unit"]), "fp32_lane_ops_per_unit": float(r["fp32_lane_ops_per_unit"]),
-            "warp_inst_per_unit": float(r["warp_inst_per_unit"]), "capture": r["capture"]}
+            "warp_inst_per_unit": float(r["warp_inst_per_unit"]),
+            "dram_bytes_per_launch": float(r["dram_bytes_per_launch"]) if r.get("dram_bytes_per_launch") else None,
+            "counts_stale": bool(r["stale"]), "capture": r["capture"]}
 
 
 def measure(pkg, torch, dist, args, name, catalog, pixels, K, W, rank, world, local, want_pairs, want_e2e):
@@ -398,6 +410,31 @@ def run_ours(args):
         # records are written by S1 in the same chunk and come back from L2, but count as the kernel's own input
         chunk = min(args.lambda_chunk, w.n_lambda)
         alg_bytes = 24 * ns_tot + 4 * nz_tot + chunk * int(w.n_events) * (112 + 2 * 200 * 16)
+        # SURVEY 8(d) on what k_events_fast executes: instruction counts of the committed ncu capture x the units of this run, over
+        # the live-measured kernel time; achieved / peak are those of the binding pipe.  The pair-based figure (the method's
+        # Gaussian pairs inside the cut-off per second) is an algorithmic-equivalent throughput, NOT a pipe utilisation: the
+        # local expansion executes ~0.2 FMA per pair, so it may exceed any pipe's peak.
+        ex = kb["roofline_k_events_fast"]
+        use_recipe = ex is not None and not ex["counts_stale"]
+        frac = ex["frac"] if use_recipe else achieved / peak_g
+        roofline = {"bound": "alu", "kernel": "k_events_fast (S2-S4: weights + KDE + integral)",
+                    "recipe": ("SURVEY 8(d): t_min = max(n_x / P_sfu, n_f / P_fp32) on executed counts, frac = t_min / t_measured"
+                               if use_recipe else
+                               "no current instruction counts for this workload: pair-based figure (1 fp32 FMA lane-op per in-cut-off Gaussian pair)"),
+                    "achieved": ex["achieved_gops"] if use_recipe else achieved,
+                    "peak": ex["peak_gops"] if use_recipe else peak_g,
+                    "unit": (f"G {ex['binding_pipe']} lane-ops/s (executed)" if use_recipe else "G pairs/s"),
+                    "frac": frac, "frac_at_sampled_clock": frac * clk_max / clk_run,
+                    "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
+                    "executed": ex,
+                    "pairs_equivalent": {"algorithmic_ops_per_launch": pairs_cut / n_launch, "g_pairs_per_s": achieved,
+                                         "pairs_frac": achieved / peak_g,
+                                         "note": "in-cut-off Gaussian pairs / kernel time / P_fp32: algorithmic-equivalent throughput, not a utilisation"},
+                    "traffic": ex["dram_bytes_per_launch"] if use_recipe else None,
+                    "traffic_source": ex["capture"] if use_recipe else None,
+                    "algorithmic_dram_bytes_per_launch": alg_bytes,
+                    "measured_alu_peaks_gops": r.get("alu"),
+                    "peak_source": f"148 SM x (128 fp32 | 16 MUFU) lanes/clk x {clk_max:.0f} MHz ({peak_src} sm_max_mhz); see DESIGN.md sec. 6"}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": t_dev_max / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -413,23 +450,7 @@ def run_ours(args):
             "gpu_launches": int(st["kernel_launches"]) * K,
             "clocks": clocks,
             "init_s": kb["init_s"],
-            "roofline": {"bound": "alu", "kernel": "k_events_fast (S2-S4: weights + KDE + integral)",
-                         # headline figure: the method's work -- Gaussian (sample, grid point) pairs inside the t*h cut-off, one fp32
-                         # FMA lane-op each in the cheapest exact formulation -- over the kernel's live-measured time
-                         "achieved": achieved, "peak": peak_g, "unit": "G pairs/s (1 fp32 FMA lane-op per Gaussian pair)",
-                         "frac": achieved / peak_g, "frac_at_sampled_clock": achieved / (peak_g * clk_run / clk_max),
-                         "algorithmic_ops_per_launch": pairs_cut / n_launch, "avg_launch_ms": ktimes["events_ms"] / n_launch, "launches": n_launch,
-                         # SURVEY 8(d) recipe on what the kernel executes (ncu instruction counts x live time), and the issue slots
-                         "executed": kb["roofline_k_events_fast"],
-                         # the KDE phase alone (S3 + S4): its share of the kernel's time from the committed ncu capture (warp-state samples
-                         # per SASS segment), applied to the live time
-                         "kde_phase": ({"share_of_kernel_time": KDE_PHASE_SHARE, "frac": achieved / KDE_PHASE_SHARE / peak_g,
-                                        "source": "profiles/r02_ncu_full.md"} if default_workload(args) else None),
-                         "traffic": (NCU_TRAFFIC_BYTES if default_workload(args) else None),
-                         "traffic_source": ("profiles/r02_ncu_full.md" if default_workload(args) else None),
-                         "algorithmic_dram_bytes_per_launch": alg_bytes,
-                         "measured_alu_peaks_gops": r.get("alu"),
-                         "peak_source": f"148 SM x 128 fp32 FMA lanes/clk x {clk_max:.0f} MHz ({peak_src} sm_max_mhz); see DESIGN.md sec. 6"},
+            "roofline": roofline,
             "roofline_k_inject": dict(kb["roofline_k_inject"] or {}, kernel="k_inject (S5)",
                                       evals_per_s=int(w.n_det) * w.n_lambda * K / max(ktimes["inject_ms"] / 1e3, 1e-12),
                                       ms_per_step=ktimes["inject_ms"] / K),
