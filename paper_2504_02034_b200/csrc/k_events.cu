@@ -488,7 +488,14 @@ __device__ __forceinline__ void events_unit(const EventKernelParams& P, const in
         for (int i = tid; i < nw; i += kEvThreads) dst[i] = src[i];
         if (tid == 0) {
             S.pass_counter = 0;
-            if (again) asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&S.mbar)) : "memory");
+            if (again) {
+                // work-list mode: the previous unit of this CTA wrote the staged regions (grid factors, psi coefficients, rows)
+                // with ordinary stores; the bulk copies below write the same shared memory through the async proxy.  The
+                // __syncthreads after the previous unit ordered those stores before this point for the generic proxy only:
+                // the cross-proxy fence makes them visible to (ordered before) the async-proxy writes that follow.
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(&S.mbar)) : "memory");
+            }
             mbar_init(&S.mbar, 1);
             // polynomial path: the stage bounds were computed by k_polyfit, so the TMA copy of the mass rows starts now and
             // runs beside the staging of the constants (the same test as use_poly below, on the global copy of the constants)
