@@ -122,6 +122,10 @@ int chim_create(const chim_config *cfg, chim_ctx **out);
 void chim_destroy(chim_ctx *ctx);
 const char *chim_last_error(const chim_ctx *ctx); /* never NULL; "" if no error yet; ctx == NULL: the last failed chim_create */
 int chim_version(void);
+/* Hash of the sources this library was compiled from (paper_2504_02034_b200/build.py: source_hash(); "unknown" for a build made
+ * by hand).  The Python binding refuses a library whose id differs from the sources beside it: a stale libchim.so must not be
+ * tested or benchmarked in place of the checked-out code. */
+const char *chim_build_id(void);
 
 /*
  * Events (PE samples, the fixed per-event redshift grid, p_gal on it).

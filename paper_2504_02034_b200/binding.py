@@ -69,6 +69,12 @@ def lib():
         raise ImportError(f"{p} not found: build it with `python -m paper_2504_02034_b200.build` "
                           "(nvcc, sm_100a). There is no CPU or PyTorch fallback.")
     L = C.CDLL(p)
+    L.chim_build_id.restype = C.c_char_p
+    from . import build as _build
+    have, want = L.chim_build_id().decode(), _build.source_hash()
+    if have != want:
+        raise ImportError(f"{p} was built from other sources (build id {have}, sources {want}): rebuild it with "
+                          "`python -m paper_2504_02034_b200.build`. A stale library is never used.")
     L.chim_default_config.argtypes = [C.POINTER(ChimConfig)]
     L.chim_default_config.restype = None
     L.chim_create.argtypes = [C.POINTER(ChimConfig), C.POINTER(C.c_void_p)]

@@ -414,6 +414,11 @@ void chim_default_config(chim_config* cfg) {
 
 int chim_version(void) { return CHIM_VERSION; }
 
+#ifndef CHIM_BUILD_ID
+#define CHIM_BUILD_ID "unknown"
+#endif
+const char* chim_build_id(void) { return CHIM_BUILD_ID; }
+
 const char* chim_last_error(const chim_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
 int chim_create(const chim_config* cfg, chim_ctx** out) {
