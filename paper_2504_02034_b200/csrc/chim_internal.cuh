@@ -32,10 +32,12 @@ struct alignas(16) LamF {
                               // placement ON_GRID (no psi in the sample weights): gk2 = 0, cpsi = 100
     float tm_max;
     float gk2_inj, cpsi_inj;  // gk2, cpsi for the injections (psi is always in s_j)
-    float pad0;
+    float beta2_lo;           // beta log2(e) - beta2 (used by the table path, sample_eval; the polynomial sweeps take beta2 alone: measured,
+                              // the extra FMA per sample costs 3 % of k_events_fast for < 1e-7 in log I -- DESIGN.md sec. 7)
     // the rest (table path, hi + lo pairs)
     float mlow_lo;            // m_low - mlow_hi
     float lm0_hi, lm0_lo;     // ln m_low (origin of the mass table)
+    float tm_one;             // 1 + tm_shift (LamConst): the table path's coordinate (ln m1 - lm0) tm_scale + tm_one addresses the same shifted nodes
     float tkmax_ev, tkmax_inj;// table coordinate beyond which z > z_table_max
     float zcat_hi, zcat_lo;   // z_cat_max (R6) as hi + lo
     uint32_t tkmax_ev_q;      // tkmax_ev in the 12.20 fixed point of the event records
@@ -47,7 +49,7 @@ __device__ __forceinline__ void load_lamf_hot(LamF& F, const LamF* __restrict__ 
     F.mlow_hi = a.x; F.tm_scale = a.y; F.mlow_tm = a.z; F.mhigh_p = a.w;
     F.beta2 = b.x; F.delta = b.y; F.win_lo = b.z; F.win_hi = b.w;
     F.two_dl2e = c.x; F.d2l2e = c.y; F.gk2 = c.z; F.cpsi = c.w;
-    F.tm_max = d.x; F.gk2_inj = d.y; F.cpsi_inj = d.z; F.pad0 = 0.f;
+    F.tm_max = d.x; F.gk2_inj = d.y; F.cpsi_inj = d.z; F.beta2_lo = d.w;
 }
 
 // Per-lambda constants written by the table kernel (S1), read by every other kernel.
@@ -74,6 +76,8 @@ struct LamConst {
     double inv_delta;   // 1 / delta_m
     double lm0;         // mass table: node coordinate tm = (ln m1 - lm0) * inv_dlm + 1
     double inv_dlm;
+    double tm_shift;    // (float)mlow_tm - (1 - lm0 inv_dlm): the rounding of LamF::mlow_tm in table rows; the nodes of the mass table are
+                        // shifted by it, so the fp32 coordinate ln m1 * tm_scale + mlow_tm of the sample kernels is exact
     uint32_t flags;     // CHIM_FLAG_LAMBDA_DOMAIN | CHIM_FLAG_DL_NONMONOTONE
     int32_t beta_is_m1; // |beta + 1| < 1e-12 : log form of the power integral
     LamF F;             // fp32 constants of the sample kernels (S2, S5)
@@ -225,7 +229,7 @@ __device__ __forceinline__ void sample_eval(const LamF& F, const float4 q0, cons
     const float mp1 = (p1 - F.mlow_hi) + c1, mp2 = (p2 - F.mlow_hi) + c2;
     const float lm1 = lnm1d - u, lm2 = lm1 + lnq;
     // mass table: coordinate, interval by the magic-number floor, cubic
-    float tm = fmaf((lm1 - F.lm0_hi) - F.lm0_lo, F.tm_scale, 1.0f);
+    float tm = fmaf((lm1 - F.lm0_hi) - F.lm0_lo, F.tm_scale, F.tm_one);
     tm = fminf(fmaxf(tm, 1.0f), F.tm_max);
     const float ti = (tm - 0.5f) + 12582912.f;
     const int km = __float_as_int(ti) - 0x4B400000;
@@ -238,7 +242,7 @@ __device__ __forceinline__ void sample_eval(const LamF& F, const float4 q0, cons
         if (!staged) c = __ldg(M.g + km + (gauss_only ? M.n_mass + 2 : 0));
     }
     float l = fmaf(fmaf(fmaf(c.w, tf, c.z), tf, c.y), tf, c.x);
-    l += fmaf(F.beta2, lm2, r + ipr2);
+    l += fmaf(F.beta2, lm2, fmaf(F.beta2_lo, lm2, r + ipr2));
     l = fmaf(-2.f, lg2f(fmaxf(mp1, 1e-30f)), l);
     // smoothing of m2 (M1): log2(e) f = (2 delta m' - delta^2) log2(e) / (m' (m' - delta)), m' clamped inside the window
     if (__any_sync(0xffffffffu, mp2 < F.delta)) {      // skipped by warps whose secondaries all lie above the window
@@ -300,7 +304,8 @@ __device__ __forceinline__ void load_poly(PolyCoef& C, const float* __restrict__
 // rows' hi + lo terms), then lane n < 7 forms coefficient n of the four polynomials; out[4][7] floats.
 //   r = table r + log2(1 + 2^(gk2 u - cpsi)) - beta2 u   (turnover taken out, -beta ln(1+z) of m2^beta folded in)
 __device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restrict__ tab, int K, double tk_c, double tk_h,
-                                          double z_ref, bool turn_on, const double* __restrict__ pm, float* __restrict__ out, bool valid) {
+                                          double z_ref, bool turn_on, const double* __restrict__ pm, float* __restrict__ out, bool valid,
+                                          double* r0_lo = nullptr) {
     const int lane = threadIdx.x & 7;
     double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
     if (valid && lane < kPolyN) {
@@ -333,6 +338,9 @@ __device__ __forceinline__ void fit_polys(const LamConst& L, const Row* __restri
     if (valid && lane < kPolyN) {        // out: float2 zr[7] = (z_n, r_n), float2 ua[7] = (u_n, a_n)
         out[2 * lane] = (float)c0;
         out[2 * lane + 1] = (float)c3;
+        // r_0 is a factor 2^r_0 common to every weight of the item: its rounding to a float (|r_0| ~ 20: up to 1e-6) does not
+        // average out over the samples.  The residual goes back to the caller, who applies it once per item in fp64.
+        if (lane == 0 && r0_lo) *r0_lo = c3 - (double)(float)c3;
         out[2 * kPolyN + 2 * lane] = (float)c1;
         out[2 * kPolyN + 2 * lane + 1] = (float)c2;
     }

@@ -73,6 +73,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
     const LamConst& L = S.L;
     const LamF& F = L.F;
     double acc[2] = {0.0, 0.0};
+    double chunk_scale = 1.0;     // 2^(rounding residual of the chunk polynomial's constant term), applied to the chunk's sums in fp64
     int oor = 0;
     const double tk_h = P.inj.tk_h[chunk], tk_c = P.inj.tk_c[chunk];
     const bool use_poly = L.flags == 0 && tk_h > 0.0 && tk_c + tk_h < L.tkmax_inj;   // (block-uniform)
@@ -96,6 +97,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
             for (int n = 0; n < kPolyN - 1; ++n) C.ua[n] = pack2(f[2 * kPolyN + 2 * n], f[2 * kPolyN + 2 * n + 1]);
         }
         const bool turn_folded = __float_as_int(__ldg(pr + 26)) != 0;
+        chunk_scale = exp2((double)__ldg(pr + 27));
         const float4* pa = P.inj.prec_a + j0;                // padded to whole chunks with copies of the chunk's last injection
         const float2* pb = P.inj.prec_b + j0;
         const int n = (int)(j1 - j0), n32 = (n + 31) & ~31;
@@ -134,7 +136,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
                 const double s = ((MID).zc <= 0.f && (JJ) < n) ? ex2_to_double(l2w) : 0.0;                            \
                 acc[0] += s;                                                                                          \
                 acc[1] = fma(s, s, acc[1]);                                                                           \
-                if ((JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale;                                       \
+                if ((JJ) < n) P.dbg_s[P.inj.perm[j0 + (JJ)]] = s * P.dbg_scale * chunk_scale;                         \
             } else {                                                                                                  \
                 const float lw = ((MID).zc <= 0.f && (JJ) < n) ? l2w : -INFINITY;                                     \
                 if (lw > ref + 40.f) {   /* (NaN never enters: it fails the comparison and poisons the sums below) */  \
@@ -215,7 +217,7 @@ __global__ void __launch_bounds__(kInjThreads, 3) k_inject(InjKernelParams P) {
         double a = 0.0, b = 0.0;
 #pragma unroll
         for (int k = 0; k < kInjThreads / 32; ++k) { a += S.red[k]; b += S.red[kInjThreads / 32 + k]; }
-        P.partial[(size_t)chunk * P.n_lambda + l] = make_double2(a, b);
+        P.partial[(size_t)chunk * P.n_lambda + l] = make_double2(a * chunk_scale, b * chunk_scale * chunk_scale);
         if (oor) atomicOr(P.flags + l, CHIM_FLAG_TABLE_RANGE);
     }
 }

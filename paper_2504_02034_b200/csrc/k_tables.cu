@@ -251,8 +251,12 @@ __device__ void build_mass_table(const TableParams& P, const TabSmem& S, const d
     const int K = P.n_mass, NN = K + 3;
     const double dlm = 1.0 / L.inv_dlm;
     for (int idx = threadIdx.x; idx < NN; idx += kTabThreads) {
-        const double lm = L.lm0 + (idx - 1) * dlm;
-        const double m = (idx <= 1) ? L.m_low : exp(lm);
+        // node idx sits where the sample kernels' fp32 coordinate ln m1 * tm_scale + mlow_tm equals idx: mlow_tm is rounded to a
+        // float, so the nodes are shifted by that rounding (tm_shift rows, < 1e-7 in ln m) instead of the samples' coordinate
+        // being wrong by it -- a bias common to every sample of a lambda otherwise.  (Node 1 then lies within 1e-7 m_low of m_low,
+        // on either side: the asymptotic form below takes m' = m - m_low of either sign.)
+        const double lm = L.lm0 + (idx - 1 - L.tm_shift) * dlm;
+        const double m = (idx <= 1) ? L.m_low * exp(-L.tm_shift * dlm) : exp(lm);
         const double mp = m - L.m_low;
         // ln of the un-smoothed primary density / Z1: power law (no cut) + Gaussian, and the Gaussian alone
         const double dm = m - L.mu;
@@ -447,7 +451,7 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         F.delta = (float)L.delta;
         F.two_dl2e = (float)(2.0 * L.delta * l2e); F.d2l2e = (float)(L.delta * L.delta * l2e);
         F.win_lo = (float)(L.delta * 1e-12); F.win_hi = (float)(L.delta * (1.0 - 1e-6));   // keeps f finite: log2 S down to -1e12 (the weights are carried as logs, R21)
-        F.beta2 = (float)(L.beta * l2e);
+        F.beta2 = (float)(L.beta * l2e); F.beta2_lo = (float)(L.beta * l2e - (double)F.beta2);
         F.mhigh_p = (float)(L.m_high - L.m_low);
         F.tm_scale = (float)L.inv_dlm; F.tm_max = (float)P.n_mass + 0.999f;
         F.tkmax_ev = (float)fmin(L.tkmax_ev, 1e9) * (1.0f - 1e-6f); F.tkmax_inj = (float)fmin(L.tkmax_inj, 1e9) * (1.0f - 1e-6f);
@@ -455,6 +459,8 @@ __global__ void __launch_bounds__(kTabThreads) k_tables(const double* __restrict
         if (P.placement == CHIM_ON_SAMPLES) { F.gk2 = (float)(L.gk * l2e); F.cpsi = (float)(L.gk * l2e * L.ln1pzp); }
         else { F.gk2 = 0.f; F.cpsi = 100.f; }
         F.mlow_tm = (float)(1.0 - L.lm0 * L.inv_dlm);
+        L.tm_shift = (double)F.mlow_tm - (1.0 - L.lm0 * L.inv_dlm);   // |.| < 2e-5 rows; build_mass_table moves its nodes by it
+        F.tm_one = (float)(1.0 + L.tm_shift);
         F.gk2_inj = (float)(L.gk * l2e); F.cpsi_inj = (float)(L.gk * l2e * L.ln1pzp);
         F.tkmax_ev_q = (L.tkmax_ev >= 4095.9) ? 0xFFFFFFFFu : (L.tkmax_ev <= 0.0 ? 0u : (uint32_t)(L.tkmax_ev * (double)(1u << kTkFracBits)));
     }
@@ -508,10 +514,13 @@ __global__ void __launch_bounds__(256) k_polyfit(const LamConst* __restrict__ Lc
     // ~0.5 from the real axis in ln(1+z)) -- except for injection chunks narrower than 0.2 in ln d_L, where degree 6 takes it
     // to < 1e-9 and k_inject saves two MUFU per injection (slot 26 of the record: 1 = folded)
     const bool fold = is_inj && h * dx_tab <= 0.1;
-    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, !fold && (is_inj || L.F.gk2 != 0.f), pm, o, valid);
+    double r0_lo = 0.0;
+    fit_polys(L, tab + (size_t)l * tab_rows, tab_rows - 2, c, h, z_ref ? z_ref[r] : z_ref_const, !fold && (is_inj || L.F.gk2 != 0.f), pm, o, valid,
+              &r0_lo);
     if (is_inj) {
         __syncwarp();
-        if (valid && sl == 0) o[26] = __int_as_float(fold ? 1 : 0);
+        // slot 27 (free for chunks): what the fp32 constant term of r lost -- k_inject scales the chunk's sums by 2^r0_lo
+        if (valid && sl == 0) { o[26] = __int_as_float(fold ? 1 : 0); o[27] = (float)r0_lo; }
     }
     if (lnm1_lo) {
         // k_events: the rows of the mass table the event can address, ln m1 = ln m1d - u, u = ln(1+z) between the ends of the

@@ -114,7 +114,7 @@ def _golden(name, w):
     return g
 
 
-def _compare_with_golden(P, w, r, g, n_events):
+def _compare_with_golden(P, w, r, g, n_events, soft_total=False):
     """Every unit and every total of the cached oracle run (tests/golden/make_reference.py) against the CUDA path: rows of the
     batch are read out of the full-size launch `r`; the box corners (not in the batch) get a launch of their own."""
     idx = g["lam_index"]
@@ -153,14 +153,17 @@ def _compare_with_golden(P, w, r, g, n_events):
     assert abs(err[ordinary].mean()) < 5e-7
     assert np.max(np.abs(got["logxi"][ok] - g["logxi"][ok])) < 1e-6
     assert np.max(np.abs(got["neff"][ok] / g["neff"][ok] - 1)) < 1e-5
-    # north_star states the absolute 1e-3 for 300-event batches; the total is a sum over events, so the 5000-event config is held
-    # to the same error per event (measured there: 2.0e-3 = 4e-7 per event, the common part of the fp32 weight errors)
+    # north_star: the total log L to an absolute 1e-3, whatever the number of events.  (soft_total: the caller checks it and
+    # reports an expected failure -- the 5000-event config, see test_full_size_other_configs_against_the_cached_oracle)
     dtot = np.abs(got["loglike"][ok] - g["loglike"][ok])
-    assert dtot.max() < ABS_TOTAL * max(1.0, n_events / 300.0), (dtot.max(), int(np.argmax(dtot)))
+    if not soft_total:
+        assert dtot.max() < ABS_TOTAL, (dtot.max(), int(np.argmax(dtot)))
+    # the part of the error common to all events of a lambda, against the selection term's: what N_events multiplies
+    common = (a - b)[ok].mean(axis=1) - (got["logxi"][ok] - g["logxi"][ok]) if np.isfinite(b[ok]).all() else np.zeros(1)
     assert np.array_equal(np.isnan(got["loglike"]), np.isnan(g["loglike"])) and np.array_equal(np.isneginf(got["loglike"]), np.isneginf(g["loglike"]))
     assert np.array_equal(fl, g["flags"].astype(np.uint32)), np.flatnonzero(fl != g["flags"])[:10]
     return dict(max_rel=float(rel.max()), max_abs=float(np.abs(err[ordinary]).max()), rms=float(np.sqrt(np.mean(err[ordinary] ** 2))),
-                mean=float(err[ordinary].mean()), max_total=float(dtot.max()),
+                mean=float(err[ordinary].mean()), max_total=float(dtot.max()), max_common=float(np.abs(common).max()),
                 n_units=int(a.size), n_nonfinite=int((~fin).sum()))
 
 
@@ -202,8 +205,17 @@ def test_full_size_other_configs_against_the_cached_oracle(P, name):
     # (full_pop: 5000 events against 10^6 injections -- N_eff < 5 N_events is the expected state there: NEFF_LOW, report only, R8)
     assert fin.sum() >= 0.75 * w.n_lambda and ((r["flags"][fin] & ~np.uint32(P.CHIM_FLAG_NEFF_LOW)) == 0).all()
     assert np.max(np.abs(r["loglike"][fin] - (r["event_logI"][fin].sum(axis=1) - w.n_events * r["logxi"][fin]))) < 1e-7
-    st = _compare_with_golden(P, w, r, _golden(name, w), w.n_events)
+    # full_pop (5000 events): every per-unit, log xi and N_eff bound above holds, but the TOTAL misses north_star's absolute 1e-3:
+    # measured 2.1e-3.  Sum_i log I_i and N_e log xi each carry an error common to all events of a lambda (here -1.1e-7 and
+    # +1.8e-7 per event: fp32 log-weights, the one-sided error of lg2.approx, rounded per-lambda constants -- DESIGN.md sec. 7),
+    # and 5000 events multiply the difference.  Reported as an expected failure, not hidden behind a scaled tolerance.
+    st = _compare_with_golden(P, w, r, _golden(name, w), w.n_events, soft_total=(name == "full_pop"))
     print(f"{name}: golden {st}")
+    if name == "full_pop":
+        assert st["max_total"] < 3e-3 and st["max_common"] < 6e-7          # (no worse than measured)
+        if st["max_total"] >= ABS_TOTAL:
+            pytest.xfail(f"full_pop: |d log L| = {st['max_total']:.2e} >= 1e-3 over {w.n_events} events "
+                         f"(common error per event {st['max_common']:.1e}); every other bound of the test holds")
 
 
 # ---------------------------------------------------------------- T2: intermediates, step by step
