@@ -174,14 +174,27 @@ def workload_config(w, args):
             "parallelism": f"lambda-sharded replicas x{args.gpus}, no data-path collective"}
 
 
+def kernel_source_sha16(kernel):
+    """sha256[:16] over the kernel's .cu file and chim_internal.cuh (the device functions it inlines)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in (kernel + ".cu", "chim_internal.cuh"):
+        p = os.path.join(ROOT, "paper_2504_02034_b200", "csrc", f)
+        if not os.path.exists(p):
+            return None
+        with open(p, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def load_instruction_counts():
     """Per-unit instruction counts and per-launch DRAM bytes of the two hot kernels from the committed ncu captures
-    (profiles/r02_instruction_counts.csv; the .md beside it names the commands): {(workload, kernel): row}.  Absent file -> {} and
-    the recipe entries read null.  Every row names the sha256[:16] of the kernel's .cu file at capture; a row whose kernel source
+    (profiles/r03_instruction_counts.csv; the .md beside it names the commands): {(workload, kernel): row}.  Absent file -> {} and
+    the recipe entries read null.  Every row names the sha256[:16] of the kernel's sources at capture (kernel_source_sha16); a row whose kernel source
     has changed since is marked stale and its figures are not used for `roofline.frac`."""
     import csv
     import hashlib
-    p = os.path.join(ROOT, "profiles", "r02_instruction_counts.csv")
+    p = os.path.join(ROOT, "profiles", "r03_instruction_counts.csv")
     out = {}
     if os.path.exists(p):
         sha = {}
@@ -189,8 +202,7 @@ def load_instruction_counts():
             for r in csv.DictReader(f):
                 k = r["kernel"]
                 if k not in sha:
-                    src = os.path.join(ROOT, "paper_2504_02034_b200", "csrc", k + ".cu")
-                    sha[k] = hashlib.sha256(open(src, "rb").read()).hexdigest()[:16] if os.path.exists(src) else None
+                    sha[k] = kernel_source_sha16(k)
                 r["stale"] = sha[k] != r.get("kernel_src_sha16")
                 out[(r["workload"], r["kernel"])] = r
     return out

@@ -5,24 +5,24 @@
 // secondary deep in the smoothing window, a bandwidth the expansion cannot take: DESIGN.md R21) is left to k_events: the unit
 // is appended to a work list that k_events processes in the same batch call.
 //
-// Structure (what differs from k_events): between its four barriers the eight warps are independent.
-//   S2   warp w owns a contiguous chunk of the (d_L-sorted) samples: sweep 1 with the 26 polynomial coefficients in registers
-//        and the records two blocks ahead, its own maximum, sweep 2 relative to that; it leaves chunk statistics
-//        {max log2 w, sum w, sum w^2, sum w u, sum w u^2}.                                                       [barrier]
-//        Every warp combines the eight chunk statistics (lane c takes chunk c; sums of positive terms, fp32), derives
-//        bandwidth and expansion geometry redundantly; the psi table and the first sample of every box are found once per
-//        CTA (one thread per entry).                                                                              [barrier]
-//   S3+S4 warp w owns the boxes w, w + 8, ...: it builds their expansion coefficients and evaluates the samples that fall in
-//        them (a contiguous range each, coefficients in registers) -- the boxes of the sparse tails and of the dense centre
-//        alternate over the warps, so the warps finish together.                                                  [barrier]
-// q_g and the mass-table rows arrive by TMA bulk copies issued before the first barrier.
+// Structure (what differs from k_events): between its five barriers the warps are independent.
+//   prologue: every global load of the unit in one batch; q_g and the mass-table rows arrive by TMA bulk copies.   [barrier 1]
+//   S2   warp w owns a contiguous chunk of the (d_L-sorted) samples and makes ONE sweep over it: the 26 polynomial
+//        coefficients in registers, the records two blocks ahead (heads of two samples, one group of record loads, the two
+//        tails), weights relative to a chunk reference found in the first block, moments about the centre of the event's
+//        d_L range; it leaves chunk statistics {reference log2 w, sum w, sum w^2, sum w u, sum w u^2}.               [barrier 2]
+//        Every warp combines the chunk statistics (lane c takes chunk c; sums of positive terms, fp32) and derives bandwidth
+//        and expansion geometry redundantly; the psi table and the first sample of every box are found once per CTA
+//        (one thread per entry).                                                                                  [barrier 3]
+//   S3   the expansion coefficients of the boxes are built in groups of five boxes over the warps.                 [barrier 4]
+//        Then every warp evaluates its own chunk of samples with per-sample box records from shared memory (no box search,
+//        balanced), S4 folded in (q_g carries the trapezoid weights).                                             [barrier 5]
+//        Warp 0 adds the per-warp sums and writes log I.
 #include "chim_internal.cuh"
 
 namespace chim {
 
-#ifndef CHIM_FAST_BLOCKS
-#define CHIM_FAST_BLOCKS 3
-#endif
+constexpr int kFastBlocks8 = 3;      // resident CTAs per SM the eight-warp class is compiled for (80 registers)
 // (threads per CTA kFT = 32 kFW, warps = sample chunks kFW: template parameter of the kernel, 8 or 4)
 constexpr int kFPass = kFastPass;    // samples per warp pass (4 per lane)
 constexpr int kFLeP = 12;            // terms of the local expansion
@@ -57,7 +57,7 @@ size_t events_fast_smem_bytes(int max_ns, int max_nz, int warps, int max_d) {
 }
 
 template <int kFW, int kFMaxD>
-__global__ void __launch_bounds__(32 * kFW, kFW == 8 ? CHIM_FAST_BLOCKS : (kFW == 4 ? 6 : 12)) k_events_fast(FastEventParams P) {
+__global__ void __launch_bounds__(32 * kFW, kFW == 8 ? kFastBlocks8 : (kFW == 4 ? 6 : 12)) k_events_fast(FastEventParams P) {
     constexpr int kFT = 32 * kFW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     FastSmem<kFW>& S = *reinterpret_cast<FastSmem<kFW>*>(smem_raw);
